@@ -1,0 +1,458 @@
+/*
+ * rubix_oracle.c -- fp64 CPU ORACLE for the RUBIX hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This file is the slow, plain, by-the-definition implementation that the CUDA path is
+ * compared against.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call it.  It shares no code, header, table or
+ * constant generator with paper_2412_08265_b200/csrc/ and never calls into it.
+ *
+ * What it computes (section 3 "RUBIX Codebase"): "orientate the galaxy in the
+ * field of view" -> "particles are assigned to the IFU spaxels" -> "Each star spectrum is
+ * calculated as a lookup from a simple stellar population (SSP) library" -> "Doppler
+ * shifted based on ... line-of-sight velocity" -> "resampling ... to match the wavelength
+ * grid of the observed telescope" -> "the stellar spectra in each spaxel are summed up" ->
+ * "point-spread function (PSF) and line-spread function (LSF) convolution"; and the
+ * gradients "through the entire pipeline" (PAPER.md L22 abstract).  The paper gives no
+ * formulas; the numerical readings are BASELINE.json:north_star and SURVEY.md section 8(c),
+ * listed in DESIGN.md ("Readings of the paper").  Each function cites its row.
+ *
+ * Arithmetic: fp64 from the same fp32 input arrays the GPU sees (promoted on load), EXCEPT
+ * the binning of step 1-2 which SURVEY.md 8(c)-2 defines in fp32 with a fixed operation
+ * order so that spaxel keys can be compared bit for bit.  Build with -ffp-contract=off and
+ * without -ffast-math (oracle/__init__.py does).
+ *
+ * Pins (tests/test_oracle_*.py, all run without a GPU): numpy.histogram2d and hand-checked
+ * edges (binning); numpy.argsort(kind='stable') (sort); node reproduction, the bilinear
+ * closed form and partition of unity (lookup); numpy.interp, the a+b*lambda closed form and
+ * the line-centroid shift lambda(1+v/c) (Doppler/resample); superposition, permutation
+ * invariance, flux conservation, brute-force Python loops (accumulate); delta response,
+ * scipy.ndimage.convolve1d, numpy.convolve, flux conservation (PSF/LSF); central finite
+ * differences, the dot-product test and the linear-template closed form (adjoint).
+ * No function here is "parity unpinned".
+ *
+ * No blocking, fusion or reordering beyond the definitions; the only parallelism is an
+ * OpenMP "parallel for" over independent outputs (spaxels / voxels / particles).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_C_KMS 299792.458     /* speed of light, km/s (SURVEY.md 8 notation) */
+#define ORC_VCAP_KMS 14989.623f  /* 0.05 c: |v_los| above this (or NaN) => particle dropped
+                                    (reading R5; physical stars never reach it) */
+
+/* ------------------------------------------------------------------------------------
+ * Steps 1-2: rotate, project, bin.  SURVEY.md 8(a) rows 1-2, 8(c) rows 1-2.
+ * fp32, round-to-nearest, every * and + separately rounded, in exactly this order:
+ *   xr = (R00*x + R01*y) + R02*z ; yr likewise ; vl = (R20*vx + R21*vy) + R22*vz
+ *   hx = (0.5f*N_x)*s ; u = (xr + hx) / s ; inside iff 0 <= u < N_x (same for y)
+ *   key = floor(u)*N_y + floor(v) if inside (and |vl| <= cap) else N_x*N_y
+ * Line of sight = +z' (receding positive).
+ * ------------------------------------------------------------------------------------ */
+void orc_rotate_bin(int64_t n, const float *pos, const float *vel, const float *R,
+                    int32_t n_x, int32_t n_y, float s, int32_t *key, float *vlos)
+{
+    const float hx = (0.5f * (float)n_x) * s;
+    const float hy = (0.5f * (float)n_y) * s;
+    for (int64_t i = 0; i < n; ++i) {
+        const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+        const float vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        const float xr = (R[0] * x + R[1] * y) + R[2] * z;
+        const float yr = (R[3] * x + R[4] * y) + R[5] * z;
+        const float vl = (R[6] * vx + R[7] * vy) + R[8] * vz;
+        const float u = (xr + hx) / s;
+        const float v = (yr + hy) / s;
+        const int inside = (u >= 0.0f) && (u < (float)n_x) && (v >= 0.0f) && (v < (float)n_y)
+                           && (fabsf(vl) <= ORC_VCAP_KMS);
+        key[i] = inside ? (int32_t)floorf(u) * n_y + (int32_t)floorf(v) : n_x * n_y;
+        vlos[i] = vl;
+    }
+}
+
+/* ------------------------------------------------------------------------------------
+ * Step 3: stable order by (key, original index) and segment offsets.
+ * SURVEY.md 8(a) row 3, 8(c) row 3.  seg_off has n_s+2 entries: segment s is
+ * perm[seg_off[s] .. seg_off[s+1]), s = n_s is the out-of-FoV segment.
+ * ------------------------------------------------------------------------------------ */
+void orc_sort(int64_t n, const int32_t *key, int32_t n_s, int32_t *perm, int32_t *seg_off)
+{
+    int64_t *cursor = (int64_t *)calloc((size_t)n_s + 2, sizeof(int64_t));
+    for (int64_t i = 0; i < n; ++i) cursor[key[i] + 1] += 1;
+    for (int32_t s = 0; s <= n_s; ++s) cursor[s + 1] += cursor[s];
+    for (int32_t s = 0; s <= n_s + 1; ++s) seg_off[s] = (int32_t)cursor[s];
+    for (int64_t i = 0; i < n; ++i) perm[cursor[key[i]]++] = (int32_t)i;  /* ascending i */
+    free(cursor);
+}
+
+/* ------------------------------------------------------------------------------------
+ * Step 4a: SSP cell and interpolation parameter on one axis.  SURVEY.md 8(c) row 4:
+ *   i = clamp(max{j : A[j] <= q}, 0, n-2),  t = clamp((q - A[i]) / (A[i+1] - A[i]), 0, 1)
+ * ------------------------------------------------------------------------------------ */
+static void axis_cell(const float *A, int32_t n, float qf, int32_t *cell, double *t)
+{
+    const double q = (double)qf;
+    int32_t i = -1;
+    for (int32_t j = 0; j < n; ++j)
+        if ((double)A[j] <= q) i = j;
+    if (i < 0) i = 0;
+    if (i > n - 2) i = n - 2;
+    double tt = (q - (double)A[i]) / ((double)A[i + 1] - (double)A[i]);
+    if (tt < 0.0) tt = 0.0;
+    if (tt > 1.0) tt = 1.0;
+    *cell = i;
+    *t = tt;
+}
+
+void orc_ssp_cells(int64_t n, const float *log_age, const float *log_z, int32_t n_age,
+                   int32_t n_z, const float *age_axis, const float *z_axis, int32_t *ia,
+                   int32_t *iz, double *ta, double *tz)
+{
+    for (int64_t p = 0; p < n; ++p) {
+        axis_cell(age_axis, n_age, log_age[p], &ia[p], &ta[p]);
+        axis_cell(z_axis, n_z, log_z[p], &iz[p], &tz[p]);
+    }
+}
+
+/* ------------------------------------------------------------------------------------
+ * Steps 4b-5: one particle's observed spectrum.  SURVEY.md 8(c) rows 4-5.
+ *   S(j)  = m * [ (1-ta)(1-tz) T[i][j'] + ta(1-tz) T[i+1][j'] + (1-ta)tz T[i][j'+1]
+ *                 + ta tz T[i+1][j'+1] ](j)          (linear in flux, array order [age][Z][lambda])
+ *   F[k]  = S evaluated by linear interpolation at rest wavelength lambda_k / (1 + beta),
+ *           beta = v_los / c, 0 outside the SSP wavelength coverage
+ *         = numpy.interp(lambda_obs/(1+beta), lambda_ssp, S, left=0, right=0)
+ * flux: [n_age][n_z][n_lambda].  If dS (length n_c) is non-NULL it receives the slope
+ * dS/dx at the sample (x in SSP-sample units), used by the analytic adjoint.
+ * ------------------------------------------------------------------------------------ */
+static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, double tz,
+                              double vlos, const float *flux, int32_t n_z, int32_t n_lambda,
+                              double l0_ssp, double dl_ssp, int32_t n_c, double l0_obs,
+                              double dl_obs, double *F, double *dS)
+{
+    const float *T00 = flux + ((int64_t)ia * n_z + iz) * n_lambda;
+    const float *T10 = flux + ((int64_t)(ia + 1) * n_z + iz) * n_lambda;
+    const float *T01 = flux + ((int64_t)ia * n_z + iz + 1) * n_lambda;
+    const float *T11 = flux + ((int64_t)(ia + 1) * n_z + iz + 1) * n_lambda;
+    const double w00 = (1.0 - ta) * (1.0 - tz), w10 = ta * (1.0 - tz);
+    const double w01 = (1.0 - ta) * tz, w11 = ta * tz;
+    const double beta = vlos / ORC_C_KMS;
+    const double lam_first = l0_ssp;
+    const double lam_last = l0_ssp + dl_ssp * (double)(n_lambda - 1);
+    for (int32_t k = 0; k < n_c; ++k) {
+        const double lam_obs = l0_obs + dl_obs * (double)k;
+        const double lam_rest = lam_obs / (1.0 + beta);
+        if (lam_rest < lam_first || lam_rest > lam_last) {
+            F[k] = 0.0;
+            if (dS) dS[k] = 0.0;
+            continue;
+        }
+        const double x = (lam_rest - l0_ssp) / dl_ssp;
+        int32_t j = (int32_t)floor(x);
+        if (j > n_lambda - 2) j = n_lambda - 2;
+        const double f = x - (double)j;
+        const double s0 = mass * (w00 * T00[j] + w10 * T10[j] + w01 * T01[j] + w11 * T11[j]);
+        const double s1 = mass * (w00 * T00[j + 1] + w10 * T10[j + 1] + w01 * T01[j + 1]
+                                  + w11 * T11[j + 1]);
+        F[k] = s0 + f * (s1 - s0);
+        if (dS) dS[k] = s1 - s0;
+    }
+}
+
+void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, int32_t n_age,
+                           int32_t n_z, int32_t n_lambda, const float *age_axis,
+                           const float *z_axis, float l0_ssp, float dl_ssp, const float *flux,
+                           int32_t n_c, float l0_obs, float dl_obs, double *F)
+{
+    int32_t ia, iz;
+    double ta, tz;
+    axis_cell(age_axis, n_age, log_age, &ia, &ta);
+    axis_cell(z_axis, n_z, log_z, &iz, &tz);
+    particle_spectrum((double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
+                      (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs, (double)dl_obs, F, 0);
+}
+
+/* Same, but with the interpolation parameters given in fp64 (finite differences perturb
+ * log age / log Z / v_los by steps far below fp32 resolution). */
+void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double vlos,
+                               int32_t n_age, int32_t n_z, int32_t n_lambda,
+                               const float *age_axis, const float *z_axis, float l0_ssp,
+                               float dl_ssp, const float *flux, int32_t n_c, float l0_obs,
+                               float dl_obs, int32_t ia, int32_t iz, double *F)
+{
+    /* cell (ia, iz) is held fixed by the caller: FD stays inside one bilinear patch */
+    const double a0 = age_axis[ia], a1 = age_axis[ia + 1];
+    const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
+    (void)n_age;
+    particle_spectrum(mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0), vlos,
+                      flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                      (double)dl_obs, F, 0);
+}
+
+/* ------------------------------------------------------------------------------------
+ * Step 6: cube[s][k] = sum over particles with key == s of F_p[k].  SURVEY.md 8(c) row 6.
+ * If n_sel > 0 only the listed spaxels are computed and cube is [n_sel][n_c]; otherwise
+ * cube is [n_s][n_c].  Particles are visited in the stable order of step 3.
+ * ------------------------------------------------------------------------------------ */
+void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *mass,
+                    const float *log_age, const float *log_z, const float *R, int32_t n_age,
+                    int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
+                    float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
+                    float spaxel, int32_t n_c, float l0_obs, float dl_obs, const int32_t *sel,
+                    int32_t n_sel, double *cube)
+{
+    const int32_t n_s = n_x * n_y;
+    int32_t *key = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *perm = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t *seg = (int32_t *)malloc(sizeof(int32_t) * ((size_t)n_s + 2));
+    float *vlos = (float *)malloc(sizeof(float) * (size_t)(n > 0 ? n : 1));
+    orc_rotate_bin(n, pos, vel, R, n_x, n_y, spaxel, key, vlos);
+    orc_sort(n, key, n_s, perm, seg);
+    const int32_t n_out = n_sel > 0 ? n_sel : n_s;
+#pragma omp parallel
+    {
+        double *F = (double *)malloc(sizeof(double) * (size_t)n_c);
+#pragma omp for schedule(dynamic, 1)
+        for (int32_t o = 0; o < n_out; ++o) {
+            const int32_t s = n_sel > 0 ? sel[o] : o;
+            double *row = cube + (int64_t)o * n_c;
+            for (int32_t k = 0; k < n_c; ++k) row[k] = 0.0;
+            for (int32_t q = seg[s]; q < seg[s + 1]; ++q) {
+                const int32_t p = perm[q];
+                int32_t ia, iz;
+                double ta, tz;
+                axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
+                axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
+                particle_spectrum((double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux, n_z,
+                                  n_lambda, (double)l0_ssp, (double)dl_ssp, n_c,
+                                  (double)l0_obs, (double)dl_obs, F, 0);
+                for (int32_t k = 0; k < n_c; ++k) row[k] += F[k];
+            }
+        }
+        free(F);
+    }
+    free(key); free(perm); free(seg); free(vlos);
+}
+
+/* ------------------------------------------------------------------------------------
+ * Steps 7-8: Gaussian taps and the PSF / LSF convolutions.  SURVEY.md 8(c) rows 7-8.
+ *   taps g[i] = exp(-i^2 / (2 sigma^2)), i = -(size-1)/2 .. (size-1)/2, point-sampled,
+ *   normalised to sum 1.  PSF = g (x) g over (x, y), the same for every channel; LSF = h
+ *   along the channel axis; 'same' output, zero padding.  size 0 = that stage is off.
+ * orc_convolve applies the LSF, then the direct (size x size)-tap 2-D PSF.
+ * ------------------------------------------------------------------------------------ */
+void orc_gauss_taps(int32_t size, double sigma, double *taps)
+{
+    const int32_t h = (size - 1) / 2;
+    double sum = 0.0;
+    for (int32_t i = -h; i <= h; ++i) {
+        taps[i + h] = exp(-((double)i * (double)i) / (2.0 * sigma * sigma));
+        sum += taps[i + h];
+    }
+    for (int32_t i = 0; i < size; ++i) taps[i] /= sum;
+}
+
+void orc_convolve(const double *in, int32_t n_x, int32_t n_y, int32_t n_c, int32_t psf_size,
+                  double psf_sigma, int32_t lsf_size, double lsf_sigma, double *out)
+{
+    const int64_t n_vox = (int64_t)n_x * n_y * n_c;
+    double *tmp = (double *)malloc(sizeof(double) * (size_t)(n_vox > 0 ? n_vox : 1));
+    /* LSF along the channel, per spaxel */
+    if (lsf_size > 0) {
+        const int32_t h = (lsf_size - 1) / 2;
+        double *taps = (double *)malloc(sizeof(double) * (size_t)lsf_size);
+        orc_gauss_taps(lsf_size, lsf_sigma, taps);
+#pragma omp parallel for schedule(static)
+        for (int64_t s = 0; s < (int64_t)n_x * n_y; ++s)
+            for (int32_t k = 0; k < n_c; ++k) {
+                double acc = 0.0;
+                for (int32_t d = -h; d <= h; ++d)
+                    if (k + d >= 0 && k + d < n_c) acc += taps[d + h] * in[s * n_c + k + d];
+                tmp[s * n_c + k] = acc;
+            }
+        free(taps);
+    } else {
+        memcpy(tmp, in, sizeof(double) * (size_t)n_vox);
+    }
+    /* PSF over (x, y), per channel: direct 2-D sum with the outer-product kernel */
+    if (psf_size > 0) {
+        const int32_t h = (psf_size - 1) / 2;
+        double *taps = (double *)malloc(sizeof(double) * (size_t)psf_size);
+        orc_gauss_taps(psf_size, psf_sigma, taps);
+#pragma omp parallel for schedule(static) collapse(2)
+        for (int32_t x = 0; x < n_x; ++x)
+            for (int32_t y = 0; y < n_y; ++y) {
+                double *o = out + ((int64_t)x * n_y + y) * n_c;
+                for (int32_t k = 0; k < n_c; ++k) o[k] = 0.0;
+                for (int32_t dx = -h; dx <= h; ++dx)
+                    for (int32_t dy = -h; dy <= h; ++dy) {
+                        const int32_t xx = x + dx, yy = y + dy;
+                        if (xx < 0 || xx >= n_x || yy < 0 || yy >= n_y) continue;
+                        const double w = taps[dx + h] * taps[dy + h];
+                        const double *r = tmp + ((int64_t)xx * n_y + yy) * n_c;
+                        for (int32_t k = 0; k < n_c; ++k) o[k] += w * r[k];
+                    }
+            }
+        free(taps);
+    } else {
+        memcpy(out, tmp, sizeof(double) * (size_t)n_vox);
+    }
+    free(tmp);
+}
+
+/* Brute force on sampled output voxels of a (possibly huge) fp32 input cube: the full
+ * size x size x lsf_size sum per voxel.  vox[i] = flat index ((x*n_y)+y)*n_c + k. */
+void orc_convolve_voxels_f32(const float *in, int32_t n_x, int32_t n_y, int32_t n_c,
+                             int32_t psf_size, double psf_sigma, int32_t lsf_size,
+                             double lsf_sigma, const int64_t *vox, int64_t n_vox, double *out)
+{
+    const int32_t hp = psf_size > 0 ? (psf_size - 1) / 2 : 0;
+    const int32_t hl = lsf_size > 0 ? (lsf_size - 1) / 2 : 0;
+    double *g = (double *)malloc(sizeof(double) * (size_t)(2 * hp + 1));
+    double *hh = (double *)malloc(sizeof(double) * (size_t)(2 * hl + 1));
+    if (psf_size > 0) orc_gauss_taps(psf_size, psf_sigma, g); else g[0] = 1.0;
+    if (lsf_size > 0) orc_gauss_taps(lsf_size, lsf_sigma, hh); else hh[0] = 1.0;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_vox; ++i) {
+        const int64_t v = vox[i];
+        const int32_t k = (int32_t)(v % n_c);
+        const int32_t y = (int32_t)((v / n_c) % n_y);
+        const int32_t x = (int32_t)(v / ((int64_t)n_c * n_y));
+        double acc = 0.0;
+        for (int32_t dx = -hp; dx <= hp; ++dx)
+            for (int32_t dy = -hp; dy <= hp; ++dy) {
+                const int32_t xx = x + dx, yy = y + dy;
+                if (xx < 0 || xx >= n_x || yy < 0 || yy >= n_y) continue;
+                for (int32_t dc = -hl; dc <= hl; ++dc) {
+                    const int32_t kk = k + dc;
+                    if (kk < 0 || kk >= n_c) continue;
+                    acc += g[dx + hp] * g[dy + hp] * hh[dc + hl]
+                           * (double)in[((int64_t)xx * n_y + yy) * n_c + kk];
+                }
+            }
+        out[i] = acc;
+    }
+    free(g); free(hh);
+}
+
+/* Transpose of orc_convolve (true scatter form, not assuming symmetry):
+ * in_grad = LSF^T PSF^T out_grad.  Used by the adjoint and by the dot-product pin. */
+void orc_convolve_transpose(const double *gout, int32_t n_x, int32_t n_y, int32_t n_c,
+                            int32_t psf_size, double psf_sigma, int32_t lsf_size,
+                            double lsf_sigma, double *gin)
+{
+    const int64_t n_vox = (int64_t)n_x * n_y * n_c;
+    double *tmp = (double *)calloc((size_t)(n_vox > 0 ? n_vox : 1), sizeof(double));
+    if (psf_size > 0) {
+        const int32_t h = (psf_size - 1) / 2;
+        double *taps = (double *)malloc(sizeof(double) * (size_t)psf_size);
+        orc_gauss_taps(psf_size, psf_sigma, taps);
+        for (int32_t x = 0; x < n_x; ++x)          /* scatter: serial, small cubes only */
+            for (int32_t y = 0; y < n_y; ++y)
+                for (int32_t dx = -h; dx <= h; ++dx)
+                    for (int32_t dy = -h; dy <= h; ++dy) {
+                        const int32_t xx = x + dx, yy = y + dy;
+                        if (xx < 0 || xx >= n_x || yy < 0 || yy >= n_y) continue;
+                        const double w = taps[dx + h] * taps[dy + h];
+                        const double *o = gout + ((int64_t)x * n_y + y) * n_c;
+                        double *t = tmp + ((int64_t)xx * n_y + yy) * n_c;
+                        for (int32_t k = 0; k < n_c; ++k) t[k] += w * o[k];
+                    }
+        free(taps);
+    } else {
+        memcpy(tmp, gout, sizeof(double) * (size_t)n_vox);
+    }
+    if (lsf_size > 0) {
+        const int32_t h = (lsf_size - 1) / 2;
+        double *taps = (double *)malloc(sizeof(double) * (size_t)lsf_size);
+        orc_gauss_taps(lsf_size, lsf_sigma, taps);
+        for (int64_t i = 0; i < n_vox; ++i) gin[i] = 0.0;
+        for (int64_t s = 0; s < (int64_t)n_x * n_y; ++s)
+            for (int32_t k = 0; k < n_c; ++k)
+                for (int32_t d = -h; d <= h; ++d)
+                    if (k + d >= 0 && k + d < n_c)
+                        gin[s * n_c + k + d] += taps[d + h] * tmp[s * n_c + k];
+        free(taps);
+    } else {
+        memcpy(gin, tmp, sizeof(double) * (size_t)n_vox);
+    }
+    free(tmp);
+}
+
+/* ------------------------------------------------------------------------------------
+ * Step 9: analytic adjoint.  SURVEY.md 8(a) row 9, 8(c) row 9.  Given G = dL/d(final cube):
+ *   G' = LSF^T PSF^T G ; for particle p in spaxel s, with x_k its rest position (in SSP
+ *   samples) at channel k, cell corners c with weights w_c(ta, tz):
+ *     D_c    = sum_k G'[s][k] * lerp(T_c; x_k)
+ *     E      = sum_k G'[s][k] * lambda_k * sum_c w_c * (T_c[j+1] - T_c[j]) / dl_ssp
+ *     dL/dm      = sum_c w_c D_c
+ *     dL/dlogA   = m * sum_c (dw_c/dta) D_c / (A[i+1] - A[i])    (0 if ta is clamped)
+ *     dL/dlogZ   likewise
+ *     dL/dv_los  = -m E / (c (1+beta)^2)
+ *   out-of-FoV particles get 0.  Output in ORIGINAL particle order, fp64.
+ * ------------------------------------------------------------------------------------ */
+void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mass,
+                 const float *log_age, const float *log_z, const float *R, int32_t n_age,
+                 int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
+                 float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
+                 float spaxel, int32_t n_c, float l0_obs, float dl_obs, int32_t psf_size,
+                 double psf_sigma, int32_t lsf_size, double lsf_sigma, const double *grad_cube,
+                 double *g_mass, double *g_log_age, double *g_log_z, double *g_vlos)
+{
+    const int32_t n_s = n_x * n_y;
+    const int64_t n_vox = (int64_t)n_s * n_c;
+    double *gp = (double *)malloc(sizeof(double) * (size_t)(n_vox > 0 ? n_vox : 1));
+    orc_convolve_transpose(grad_cube, n_x, n_y, n_c, psf_size, psf_sigma, lsf_size, lsf_sigma, gp);
+    int32_t *key = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    float *vlos = (float *)malloc(sizeof(float) * (size_t)(n > 0 ? n : 1));
+    orc_rotate_bin(n, pos, vel, R, n_x, n_y, spaxel, key, vlos);
+#pragma omp parallel
+    {
+        double *F = (double *)malloc(sizeof(double) * (size_t)n_c);
+        double *dS = (double *)malloc(sizeof(double) * (size_t)n_c);
+#pragma omp for schedule(static)
+        for (int64_t p = 0; p < n; ++p) {
+            g_mass[p] = g_log_age[p] = g_log_z[p] = g_vlos[p] = 0.0;
+            if (key[p] >= n_s) continue;
+            const double *g = gp + (int64_t)key[p] * n_c;
+            int32_t ia, iz;
+            double ta, tz;
+            axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
+            axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
+            /* D_c: dot of G' with the resampled corner template (unit mass, weight 1) */
+            double D[4];
+            for (int32_t c = 0; c < 4; ++c) {
+                const double cta = (c & 1) ? 1.0 : 0.0, ctz = (c & 2) ? 1.0 : 0.0;
+                particle_spectrum(1.0, ia, iz, cta, ctz, (double)vlos[p], flux, n_z, n_lambda,
+                                  (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                                  (double)dl_obs, F, 0);
+                double acc = 0.0;
+                for (int32_t k = 0; k < n_c; ++k) acc += g[k] * F[k];
+                D[c] = acc;  /* c = 0:(i,j) 1:(i+1,j) 2:(i,j+1) 3:(i+1,j+1) */
+            }
+            /* E: needs the slope of the blended unit-mass spectrum */
+            particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
+                              (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                              (double)dl_obs, F, dS);
+            double E = 0.0;
+            for (int32_t k = 0; k < n_c; ++k)
+                E += g[k] * ((double)l0_obs + (double)dl_obs * k) * dS[k] / (double)dl_ssp;
+            const double m = (double)mass[p];
+            const double beta = (double)vlos[p] / ORC_C_KMS;
+            g_mass[p] = (1 - ta) * (1 - tz) * D[0] + ta * (1 - tz) * D[1] + (1 - ta) * tz * D[2]
+                        + ta * tz * D[3];
+            const double dA = (double)age_axis[ia + 1] - (double)age_axis[ia];
+            const double dZ = (double)z_axis[iz + 1] - (double)z_axis[iz];
+            const int a_free = ((double)log_age[p] > (double)age_axis[0])
+                               && ((double)log_age[p] < (double)age_axis[n_age - 1]);
+            const int z_free = ((double)log_z[p] > (double)z_axis[0])
+                               && ((double)log_z[p] < (double)z_axis[n_z - 1]);
+            g_log_age[p] = a_free ? m * (-(1 - tz) * D[0] + (1 - tz) * D[1] - tz * D[2] + tz * D[3]) / dA
+                                  : 0.0;
+            g_log_z[p] = z_free ? m * (-(1 - ta) * D[0] - ta * D[1] + (1 - ta) * D[2] + ta * D[3]) / dZ
+                                : 0.0;
+            g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));
+        }
+        free(F); free(dS);
+    }
+    free(gp); free(key); free(vlos);
+}
