@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the RUBIX hot path on B200 (contract: task prompt section 4).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload medium]
+
+A "step" is one pass of the whole hot path (rotate, bin, sort, SSP
+lookup, Doppler resample, accumulate, PSF, LSF) over one synthetic galaxy.  Default workload:
+BASELINE.json configs[2] "medium (headline)": 1 M star particles, SSP 50x7x4300, detector
+300x300x3700, PSF 15x15 + LSF 9 taps.  metric = particle*channel samples per second.
+
+  value        device-resident inputs, CUDA events around K steps, max over ranks
+  e2e          the same metric through rubix_forward_host: pinned HOST buffers, H2D of the particle
+               arrays + SSP grid and D2H of the final cube inside the timed region
+  roofline     the dominant kernel (k_accumulate), its time from CUDA event pairs recorded by the
+               library on the launching stream inside the timed region
+  cpu_baseline the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
+N > 1 (torchrun): replicas only -- every rank builds its own galaxy (seed + rank); no collective
+on the data path; time = max over ranks.
+--impl reference times the oracle (this tier's reference arm) on rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particle_channel_samples_per_s"
+UNIT = "G particle*channel/s"
+# four corner templates x 4 B x (dl_obs / dl_ssp) SSP samples per channel
+GATHER_BYTES_PER_SAMPLE = lambda tel, ssp: 16.0 * float(tel.dlambda) / float(ssp.dlambda)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="medium", choices=["tiny", "small", "medium", "contention"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_config(w):
+    t, s = w.telescope, w.ssp
+    return {"workload": f"{w.name}: {w.particles.n} star particles (disc+bulge), SSP "
+                        f"{s.flux.shape[0]}x{s.flux.shape[1]}x{s.flux.shape[2]}, detector "
+                        f"{t.n_x}x{t.n_y}x{t.n_channels}, PSF {t.psf_size}x{t.psf_size} + LSF {t.lsf_size} taps"
+                        f" (BASELINE.json configs[{['tiny', 'small', 'medium', 'contention'].index(w.name)}])",
+            "n_particles": w.particles.n, "n_spaxels": t.n_spaxels, "n_channels": t.n_channels,
+            "euler_deg": [round(float(v), 4) for v in w.euler_deg],
+            "l2_policy": "cube (%.2f GB) and workspace exceed the 126 MB L2: no flush needed"
+                         % (t.n_spaxels * t.n_channels * 4 / 1e9),
+            "parallelism": "replicas only (one galaxy per GPU, no collective)"}
+
+
+# ------------------------------------------------------------------------------------- oracle arm
+def oracle_sample_time(w, n_sample, patch):
+    """Oracle (fp64, as it stands) on a bounded sample of the workload: the first ``n_sample``
+    particles through build, and PSF/LSF on a ``patch`` x ``patch`` spaxel sub-cube.  Returns the
+    extrapolated seconds per full cube and a description."""
+    import oracle
+    t = w.telescope
+    sub = w.particles.subset(slice(0, n_sample))
+    t0 = time.perf_counter()
+    cube = oracle.build_cube(sub, w.rotation, w.ssp, t)
+    t_build = time.perf_counter() - t0
+    t_conv, frac_conv = 0.0, 1.0
+    if t.psf_size > 0 or t.lsf_size > 0:
+        px = min(patch, t.n_x)
+        py = min(patch, t.n_y)
+        x0, y0 = (t.n_x - px) // 2, (t.n_y - py) // 2
+        piece = np.ascontiguousarray(cube[x0:x0 + px, y0:y0 + py])
+        t0 = time.perf_counter()
+        oracle.convolve(piece, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)
+        t_conv = time.perf_counter() - t0
+        frac_conv = (px * py) / float(t.n_x * t.n_y)
+    del cube
+    full = t_build * (w.particles.n / float(n_sample)) + t_conv / frac_conv
+    desc = (f"oracle build on the first {n_sample} of {w.particles.n} particles ({t_build:.2f} s) + oracle "
+            f"PSF/LSF on a central {min(patch, t.n_x)}x{min(patch, t.n_y)}-spaxel sub-cube ({t_conv:.2f} s), "
+            f"scaled to the full workload: {full:.1f} s per cube")
+    return full, t_build + t_conv, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2412_08265_b200 import synth
+    oracle.build()
+    w = synth.make_workload(args.workload)
+    n_sample = min(w.particles.n, 50_000)
+    for _ in range(max(args.warmup, 0) and 1):            # one warm-up is plenty for a CPU loop
+        oracle_sample_time(w, min(n_sample, 10_000), 16)
+    secs = []
+    desc = ""
+    for _ in range(args.steps):
+        full, _, desc = oracle_sample_time(w, n_sample, 32)
+        secs.append(full)
+    t_step = float(np.mean(secs))
+    value = w.particles.n * w.telescope.n_channels / t_step / 1e9
+    cores = oracle.n_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(w),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"} if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else \
+                {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def result(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2412_08265_b200 import binding as B
+    from paper_2412_08265_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.load()
+
+    # replicas: rank r gets its own galaxy (same recipe, seed + r)
+    base = synth.make_workload(args.workload)
+    w = base if rank == 0 else synth.make_workload(args.workload, seed=1000 + 10 * rank + 2)
+    t, n = w.telescope, w.particles.n
+    dw = B.DeviceWorkload(w, device=dev)
+    cube = torch.empty(dw.shape, dtype=torch.float32, device=dev)
+    final = torch.empty_like(cube)
+    has_conv = t.psf_size > 0 or t.lsf_size > 0
+    launches_per_step = [0]
+
+    def step():
+        B.rubix_build_cube(dw.particles, dw.ssp, dw.tel, dw.R, cube, dw.workspace)
+        launches_per_step[0] = B.rubix_last_launch_count()
+        if has_conv:
+            B.rubix_convolve_psf_lsf(dw.tel, cube, final, dw.workspace)
+            launches_per_step[0] += B.rubix_last_launch_count()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    B.rubix_stage_timing_enable(True)
+    B.rubix_stage_timing_read()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    elapsed_ms = e0.elapsed_time(e1)
+    stages = B.rubix_stage_timing_read()
+    B.rubix_stage_timing_enable(False)
+    if world > 1:
+        tt = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(tt.item())
+    ms_per_step = elapsed_ms / args.steps
+    samples_per_step = float(n) * t.n_channels
+    value = world * samples_per_step / (ms_per_step * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer entry point
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    p = w.particles
+    hp = [pin(x) for x in (p.pos, p.vel, p.mass, p.log_age, p.log_z)]
+    hflux = pin(w.ssp.flux)
+    hcube = torch.empty(dw.shape, dtype=torch.float32).pin_memory()
+    cp, cs, ct = B.c_particles(*hp), B.c_ssp(w.ssp, hflux), dw.tel
+    del cube, final
+    scratch = torch.empty(B.rubix_forward_host_scratch_bytes(n, cs, ct), dtype=torch.uint8, device=dev)
+    h2d = sum(x.numel() * 4 for x in hp) + hflux.numel() * 4
+    d2h = hcube.numel() * 4
+    for _ in range(2):
+        B.rubix_forward_host(cp, cs, ct, w.rotation, hcube, scratch)
+    barrier()
+    e0.record()
+    for _ in range(args.e2e_steps):
+        B.rubix_forward_host(cp, cs, ct, w.rotation, hcube, scratch)
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        tt = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_ms = float(tt.item())
+    e2e_ms /= args.e2e_steps
+    e2e_value = world * samples_per_step / (e2e_ms * 1e-3) / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_accumulate), measured on-chip peaks
+    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+    if os.path.exists(peaks_file):
+        hbm_peak, hbm_src = float(json.load(open(peaks_file))["hbm_gbs"]), "MEASURED_PEAKS.json"
+    onchip = B.rubix_measure_peaks(scratch)
+    acc_ms = stages["accumulate"]["ms"] / max(stages["accumulate"]["calls"], 1)
+    gather_b = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * samples_per_step
+    hbm_b = t.n_spaxels * t.n_channels * 4.0 + w.ssp.flux.size * 4.0 + 48.0 * n
+    achieved = gather_b / (acc_ms * 1e-3) / 1e9
+    roofline = {"kernel": "k_accumulate (steps 4-6)", "bound": "l2", "achieved": achieved,
+                "peak": onchip["l2_gbs"], "unit": "GB/s", "frac": achieved / onchip["l2_gbs"],
+                "traffic": None,
+                "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks "
+                               "(MEASURED_PEAKS.json has no L2 figure; SURVEY.md 8(d))",
+                "algorithmic_bytes_per_launch": gather_b, "kernel_ms": acc_ms,
+                "hbm_view": {"bound": "hbm", "achieved": hbm_b / (acc_ms * 1e-3) / 1e9, "peak": hbm_peak,
+                             "unit": "GB/s", "frac": hbm_b / (acc_ms * 1e-3) / 1e9 / hbm_peak,
+                             "peak_source": hbm_src, "algorithmic_bytes_per_launch": hbm_b},
+                "measured_peaks": onchip}
+    stage_ms = {k: (v["ms"] / max(v["calls"], 1) if v["calls"] else 0.0) for k, v in stages.items()}
+    if has_conv:
+        conv_b = 2.0 * t.n_spaxels * t.n_channels * 4.0
+        roofline["psf_lsf"] = {"bound": "hbm", "achieved": conv_b / (stage_ms["psf_lsf"] * 1e-3) / 1e9,
+                               "peak": hbm_peak, "unit": "GB/s",
+                               "frac": conv_b / (stage_ms["psf_lsf"] * 1e-3) / 1e9 / hbm_peak,
+                               "algorithmic_bytes_per_launch": conv_b, "kernel_ms": stage_ms["psf_lsf"]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(w), "clocks": sampler.result(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "api": "rubix_forward_host (pinned host buffers)"},
+            "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
+            "stage_ms": stage_ms, "roofline": roofline}
+
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        full, spent, desc = oracle_sample_time(base, min(n, 300_000), 64)
+        line["cpu_baseline"] = {"value": n * t.n_channels / full / 1e9, "unit": UNIT,
+                                "cores": oracle.n_threads(), "kind": "oracle", "sample": desc,
+                                "seconds_per_cube": full}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -1,0 +1,154 @@
+/*
+ * rubix.h -- C ABI of the B200-native hot path of RUBIX's IFU forward model
+ * (arXiv 2412.08265; section 3 "RUBIX Codebase", L40).
+ *
+ * The path, in the paper's order: "orientate the galaxy in the field of
+ * view" -> "particles are assigned to the IFU spaxels" -> "Each star spectrum is calculated as
+ * a lookup from a simple stellar population (SSP) library" -> "Doppler shifted based on ...
+ * line-of-sight velocity" -> "resampling ... to match the wavelength grid of the observed
+ * telescope" -> "the stellar spectra in each spaxel are summed up" -> "point-spread function
+ * (PSF) and line-spread function (LSF) convolution"; plus "gradient computations through the
+ * entire pipeline".  The paper gives no formulas: the numerical definition of
+ * every step is BASELINE.json:north_star as spelled out in SURVEY.md section 8(a)/(c) and
+ * restated in DESIGN.md ("The path" / "Readings").
+ *
+ * Conventions (all entry points)
+ *   - Plain C: pointers and sizes only.  Each pointer is marked HOST or DEVICE.
+ *   - The caller owns every buffer.  The library never allocates or frees device memory and
+ *     never synchronises: all work is enqueued on `stream` (a cudaStream_t passed as void*)
+ *     and is complete when the stream is.  Host arrays (R, the SSP axes, the structs) are
+ *     read before the call returns and may be freed right after it.
+ *   - Device arrays are dense, row-major, fp32 / int32 as stated, 16-byte aligned.
+ *   - Errors: every call validates its arguments on the host BEFORE any launch and returns a
+ *     rubix_status; nothing throws or aborts.  rubix_last_error() gives a thread-local message.
+ *   - There is no CPU fallback: without a CUDA device the compute calls return RUBIX_ERR_CUDA.
+ *
+ * Notation: N particles; N_x x N_y spaxels, N_s = N_x*N_y; N_c channels; SSP grid
+ * N_a x N_z x N_l; beta = v_los / c, c = 299792.458 km/s.
+ */
+#ifndef RUBIX_B200_H
+#define RUBIX_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    RUBIX_OK = 0,
+    RUBIX_ERR_NULL = 1,          /* a required pointer is NULL */
+    RUBIX_ERR_INVALID_ARG = 2,   /* bad size, even stencil, non-increasing axis, dlambda <= 0 ... */
+    RUBIX_ERR_UNSUPPORTED = 3,   /* valid but outside this build's limits (see each call) */
+    RUBIX_ERR_WORKSPACE = 4,     /* workspace NULL / misaligned / smaller than rubix_workspace_bytes */
+    RUBIX_ERR_CUDA = 5           /* a CUDA runtime call failed (message has the CUDA error string) */
+} rubix_status;
+
+/* Stellar particles ("star ... particle information"; BASELINE.json north_star:
+ * "position, velocity, mass, age, metallicity").  All DEVICE, fp32. */
+typedef struct {
+    int64_t n;              /* number of particles, >= 0 (0 is valid: all-zero cube)        */
+    const float *pos;       /* [n][3] kpc, galaxy-centred                                  */
+    const float *vel;       /* [n][3] km/s, systemic velocity removed                      */
+    const float *mass;      /* [n] Msun                                                    */
+    const float *log_age;   /* [n] log10(age / Gyr)                                        */
+    const float *log_z;     /* [n] log10(Z)                                                */
+} rubix_particles;
+
+/* SSP template library ("lookup from a simple stellar population (SSP) library").
+ * Limits: n_age <= 512, n_z <= 128, n_age*n_z*n_lambda < 2^31. */
+typedef struct {
+    int32_t n_age, n_z, n_lambda;   /* each >= 2                                            */
+    const float *log_age_axis;      /* HOST [n_age], strictly increasing                    */
+    const float *log_z_axis;        /* HOST [n_z],   strictly increasing                    */
+    float lambda0, dlambda;         /* uniform rest-frame grid, Angstrom, dlambda > 0       */
+    const float *flux;              /* DEVICE [n_age][n_z][n_lambda], per unit mass         */
+} rubix_ssp;
+
+/* Detector ("telescope-specific configurations", L44 Gaussian PSF and LSF). */
+typedef struct {
+    int32_t n_x, n_y;               /* spaxels; FoV centred on the origin                   */
+    float spaxel_size;              /* kpc, > 0                                             */
+    int32_t n_channels;             /* >= 1                                                 */
+    float lambda0, dlambda;         /* observed grid, Angstrom, dlambda > 0                 */
+    int32_t psf_size;               /* odd taps <= 63 along x and along y; 0 = PSF off      */
+    float psf_sigma;                /* spaxels, > 0 when psf_size > 0                       */
+    int32_t lsf_size;               /* odd taps <= 63 along the channel axis; 0 = LSF off   */
+    float lsf_sigma;                /* channels, > 0 when lsf_size > 0                      */
+} rubix_telescope;
+
+/* Bytes of DEVICE scratch that any of the three compute calls below may need for this problem
+ * size (the maximum over the three).  Returns 0 on invalid arguments (rubix_last_error says
+ * why).  The workspace must be 256-byte aligned. */
+size_t rubix_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel);
+
+/* Steps 1-6: rotate into the field of view, project and bin to a
+ * spaxel, sort by spaxel key, SSP bilinear lookup x mass, Doppler shift + linear resampling onto
+ * the observed grid, per-spaxel sum.
+ *   R     HOST  [9] row-major rotation; r' = R r, line of sight = +z' (receding positive).
+ *   cube  DEVICE [n_x][n_y][n_channels] fp32, channel-contiguous; EVERY voxel is written
+ *         exactly once (empty spaxels get 0); no atomics, bit-reproducible run to run.
+ * Binning is the fp32 fixed-order arithmetic of SURVEY.md 8(c)-2 (bit-exact vs the oracle);
+ * particles outside the FoV, with non-finite coordinates, or with |v_los| > 0.05 c are dropped.
+ * Returns RUBIX_ERR_UNSUPPORTED if dlambda_obs/dlambda_ssp >= 15 (resampler fixed-point range).
+ * Leaves the sort artefacts in `workspace` (see rubix_get_sort_artifacts). */
+rubix_status rubix_build_cube(const rubix_particles *particles, const rubix_ssp *ssp,
+                              const rubix_telescope *tel, const float *R, float *cube,
+                              void *workspace, size_t workspace_bytes, void *stream);
+
+/* Steps 7-8: Gaussian PSF over (x, y), the same for
+ * every channel, and Gaussian LSF along the channel axis.  Taps exp(-i^2 / 2 sigma^2) sampled at
+ * integer offsets and normalised to sum 1; 'same' output; zero padding.  A size of 0 switches
+ * that stage off (both 0: plain copy).
+ *   cube_in, cube_out  DEVICE [n_x][n_y][n_channels] fp32; must not overlap. */
+rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cube_in,
+                                    float *cube_out, void *workspace, size_t workspace_bytes,
+                                    void *stream);
+
+/* Step 9: gradients of a scalar loss L of the FINAL cube
+ * (after PSF/LSF, if tel switches them on) with respect to each particle's mass, log age,
+ * log Z and line-of-sight velocity.
+ *   grad_cube  DEVICE [n_x][n_y][n_channels] fp32 = dL/d(final cube) (any loss: the caller
+ *              forms it, e.g. 2 (cube - target) for BASELINE.json configs[4]).
+ *   g_*        DEVICE [n] fp32, ORIGINAL particle order; dropped particles get 0; clamped
+ *              ages / metallicities get 0 for that component.  g_vlos is per km/s.
+ * Runs its own particle pass; no atomics (one warp owns one particle). */
+rubix_status rubix_cube_adjoint(const rubix_particles *particles, const rubix_ssp *ssp,
+                                const rubix_telescope *tel, const float *R,
+                                const float *grad_cube, float *g_mass, float *g_log_age,
+                                float *g_log_z, float *g_vlos, void *workspace,
+                                size_t workspace_bytes, void *stream);
+
+/* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_cube_adjoint on
+ * this workspace address (compared bit for bit with the oracle):
+ *   key     [n]      spaxel key of each particle in original order (n_s = dropped)
+ *   perm    [n]      stable order by (key, original index)
+ *   seg_off [n_s+2]  segment s is perm[seg_off[s] .. seg_off[s+1]); s = n_s: dropped particles
+ * Valid once the stream of that call has completed. */
+rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key,
+                                      const int32_t **perm, const int32_t **seg_off);
+
+/* Whole path with HOST buffers: copies the particle arrays and the SSP grid host->device,
+ * runs rubix_build_cube and (if switched on) rubix_convolve_psf_lsf, and copies the final cube
+ * device->host, all on `stream`; returns after enqueueing (pinned host memory makes the copies
+ * asynchronous).  This is the end-to-end call bench.py times.
+ *   h_particles  the five arrays are HOST pointers here;  h_ssp->flux is a HOST pointer here
+ *   h_cube       HOST [n_x][n_y][n_channels] fp32
+ *   device_scratch  DEVICE, at least rubix_forward_host_scratch_bytes(...) bytes, 256-B aligned */
+size_t rubix_forward_host_scratch_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel);
+rubix_status rubix_forward_host(const rubix_particles *h_particles, const rubix_ssp *h_ssp,
+                                const rubix_telescope *tel, const float *R, float *h_cube,
+                                void *device_scratch, size_t scratch_bytes, void *stream);
+
+/* Number of kernel launches the last compute call on this thread enqueued (bench.py's
+ * gpu_launches claim is the sum over the timed region). */
+int32_t rubix_last_launch_count(void);
+
+/* Thread-local, NUL-terminated message of the last failing call on this thread ("" if none). */
+const char *rubix_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RUBIX_B200_H */

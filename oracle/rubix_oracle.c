@@ -31,7 +31,7 @@
  * No function here is "parity unpinned".
  *
  * No blocking, fusion or reordering beyond the definitions; the only parallelism is an
- * OpenMP "parallel for" over independent outputs (spaxels / voxels / particles).
+ * OpenMP "parallel for" over independent outputs (spaxel x channel block / voxels / particles).
  */
 #include <math.h>
 #include <stdint.h>
@@ -126,9 +126,9 @@ void orc_ssp_cells(int64_t n, const float *log_age, const float *log_z, int32_t 
  * ------------------------------------------------------------------------------------ */
 static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, double tz,
                               double vlos, const float *flux, int32_t n_z, int32_t n_lambda,
-                              double l0_ssp, double dl_ssp, int32_t n_c, double l0_obs,
-                              double dl_obs, double *F, double *dS)
-{
+                              double l0_ssp, double dl_ssp, int32_t k_begin, int32_t k_end,
+                              double l0_obs, double dl_obs, double *F, double *dS)
+{   /* fills F[k] (and dS[k]) for channels k_begin <= k < k_end */
     const float *T00 = flux + ((int64_t)ia * n_z + iz) * n_lambda;
     const float *T10 = flux + ((int64_t)(ia + 1) * n_z + iz) * n_lambda;
     const float *T01 = flux + ((int64_t)ia * n_z + iz + 1) * n_lambda;
@@ -138,7 +138,7 @@ static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, do
     const double beta = vlos / ORC_C_KMS;
     const double lam_first = l0_ssp;
     const double lam_last = l0_ssp + dl_ssp * (double)(n_lambda - 1);
-    for (int32_t k = 0; k < n_c; ++k) {
+    for (int32_t k = k_begin; k < k_end; ++k) {
         const double lam_obs = l0_obs + dl_obs * (double)k;
         const double lam_rest = lam_obs / (1.0 + beta);
         if (lam_rest < lam_first || lam_rest > lam_last) {
@@ -168,7 +168,7 @@ void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, i
     axis_cell(age_axis, n_age, log_age, &ia, &ta);
     axis_cell(z_axis, n_z, log_z, &iz, &tz);
     particle_spectrum((double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
-                      (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs, (double)dl_obs, F, 0);
+                      (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs, (double)dl_obs, F, 0);
 }
 
 /* Same, but with the interpolation parameters given in fp64 (finite differences perturb
@@ -184,7 +184,7 @@ void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double
     const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
     (void)n_age;
     particle_spectrum(mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0), vlos,
-                      flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                      flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
                       (double)dl_obs, F, 0);
 }
 
@@ -208,26 +208,33 @@ void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *
     orc_rotate_bin(n, pos, vel, R, n_x, n_y, spaxel, key, vlos);
     orc_sort(n, key, n_s, perm, seg);
     const int32_t n_out = n_sel > 0 ? n_sel : n_s;
+    /* Independent outputs: (spaxel, block of channels).  Splitting the channels only spreads
+     * one heavy spaxel over several threads; each voxel still sums its particles in the
+     * stable order of step 3. */
+    enum { N_BLK = 8 };
 #pragma omp parallel
     {
         double *F = (double *)malloc(sizeof(double) * (size_t)n_c);
-#pragma omp for schedule(dynamic, 1)
-        for (int32_t o = 0; o < n_out; ++o) {
-            const int32_t s = n_sel > 0 ? sel[o] : o;
-            double *row = cube + (int64_t)o * n_c;
-            for (int32_t k = 0; k < n_c; ++k) row[k] = 0.0;
-            for (int32_t q = seg[s]; q < seg[s + 1]; ++q) {
-                const int32_t p = perm[q];
-                int32_t ia, iz;
-                double ta, tz;
-                axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
-                axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
-                particle_spectrum((double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux, n_z,
-                                  n_lambda, (double)l0_ssp, (double)dl_ssp, n_c,
-                                  (double)l0_obs, (double)dl_obs, F, 0);
-                for (int32_t k = 0; k < n_c; ++k) row[k] += F[k];
+#pragma omp for schedule(dynamic, 1) collapse(2)
+        for (int32_t o = 0; o < n_out; ++o)
+            for (int32_t blk = 0; blk < N_BLK; ++blk) {
+                const int32_t s = n_sel > 0 ? sel[o] : o;
+                const int32_t kb = (int32_t)(((int64_t)n_c * blk) / N_BLK);
+                const int32_t ke = (int32_t)(((int64_t)n_c * (blk + 1)) / N_BLK);
+                double *row = cube + (int64_t)o * n_c;
+                for (int32_t k = kb; k < ke; ++k) row[k] = 0.0;
+                for (int32_t q = seg[s]; q < seg[s + 1]; ++q) {
+                    const int32_t p = perm[q];
+                    int32_t ia, iz;
+                    double ta, tz;
+                    axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
+                    axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
+                    particle_spectrum((double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux, n_z,
+                                      n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke,
+                                      (double)l0_obs, (double)dl_obs, F, 0);
+                    for (int32_t k = kb; k < ke; ++k) row[k] += F[k];
+                }
             }
-        }
         free(F);
     }
     free(key); free(perm); free(seg); free(vlos);
@@ -423,7 +430,7 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
             for (int32_t c = 0; c < 4; ++c) {
                 const double cta = (c & 1) ? 1.0 : 0.0, ctz = (c & 2) ? 1.0 : 0.0;
                 particle_spectrum(1.0, ia, iz, cta, ctz, (double)vlos[p], flux, n_z, n_lambda,
-                                  (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                                  (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
                                   (double)dl_obs, F, 0);
                 double acc = 0.0;
                 for (int32_t k = 0; k < n_c; ++k) acc += g[k] * F[k];
@@ -431,7 +438,7 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
             }
             /* E: needs the slope of the blended unit-mass spectrum */
             particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
-                              (double)l0_ssp, (double)dl_ssp, n_c, (double)l0_obs,
+                              (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
                               (double)dl_obs, F, dS);
             double E = 0.0;
             for (int32_t k = 0; k < n_c; ++k)

@@ -1,0 +1,286 @@
+"""Thin ctypes binding of ``librubix_b200.so`` (include/rubix.h): argument marshalling only.
+
+Same names as the C ABI.  PyTorch is used for device memory and streams and nothing else: every
+step of the path runs in the library's kernels.  There is no fallback of any kind -- a missing
+library raises at load time and a failing call raises ``RubixError`` with the library's message.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librubix_b200.so")
+
+RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ERR_WORKSPACE, \
+    RUBIX_ERR_CUDA = range(6)
+
+EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf",
+           "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
+           "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error",
+           # include/rubix_peaks.h (measurement helpers)
+           "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
+N_STAGES = 5
+STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
+
+
+class RubixError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"rubix status {status}: {message}")
+        self.status = status
+
+
+class CParticles(C.Structure):
+    _fields_ = [("n", C.c_int64), ("pos", C.c_void_p), ("vel", C.c_void_p), ("mass", C.c_void_p),
+                ("log_age", C.c_void_p), ("log_z", C.c_void_p)]
+
+
+class CSSP(C.Structure):
+    _fields_ = [("n_age", C.c_int32), ("n_z", C.c_int32), ("n_lambda", C.c_int32),
+                ("log_age_axis", C.c_void_p), ("log_z_axis", C.c_void_p),
+                ("lambda0", C.c_float), ("dlambda", C.c_float), ("flux", C.c_void_p)]
+
+
+class CTelescope(C.Structure):
+    _fields_ = [("n_x", C.c_int32), ("n_y", C.c_int32), ("spaxel_size", C.c_float),
+                ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
+                ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
+                ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float)]
+
+
+_lib = None
+
+
+def load():
+    """Loads the in-tree library (build it with ``python -m paper_2412_08265_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2412_08265_b200.build` "
+                               "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.rubix_workspace_bytes.restype = C.c_size_t
+        lib.rubix_workspace_bytes.argtypes = [C.c_int64, C.POINTER(CSSP), C.POINTER(CTelescope)]
+        lib.rubix_forward_host_scratch_bytes.restype = C.c_size_t
+        lib.rubix_forward_host_scratch_bytes.argtypes = [C.c_int64, C.POINTER(CSSP), C.POINTER(CTelescope)]
+        lib.rubix_build_cube.restype = C.c_int
+        lib.rubix_build_cube.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_convolve_psf_lsf.restype = C.c_int
+        lib.rubix_convolve_psf_lsf.argtypes = [C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_size_t, C.c_void_p]
+        lib.rubix_cube_adjoint.restype = C.c_int
+        lib.rubix_cube_adjoint.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_get_sort_artifacts.restype = C.c_int
+        lib.rubix_get_sort_artifacts.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                                 C.POINTER(C.c_void_p)]
+        lib.rubix_forward_host.restype = C.c_int
+        lib.rubix_forward_host.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_measure_peaks.restype = C.c_int32
+        lib.rubix_measure_peaks.argtypes = [C.POINTER(C.c_float), C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_stage_timing_enable.restype = None
+        lib.rubix_stage_timing_enable.argtypes = [C.c_int32]
+        lib.rubix_stage_timing_read.restype = C.c_int32
+        lib.rubix_stage_timing_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+        lib.rubix_last_launch_count.restype = C.c_int32
+        lib.rubix_last_error.restype = C.c_char_p
+        _lib = lib
+    return _lib
+
+
+def rubix_last_error() -> str:
+    return load().rubix_last_error().decode()
+
+
+def rubix_last_launch_count() -> int:
+    return int(load().rubix_last_launch_count())
+
+
+def _check(status):
+    if status != RUBIX_OK:
+        raise RubixError(status, rubix_last_error())
+
+
+def _ptr(t):
+    """Address of a torch tensor / numpy array / None."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def _host_f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+class _Keep:
+    """ctypes struct plus the host arrays it points to (kept alive for the call)."""
+
+    def __init__(self, struct, *refs):
+        self.struct, self.refs = struct, refs
+
+    def ref(self):
+        return C.byref(self.struct)
+
+
+def c_telescope(tel) -> _Keep:
+    return _Keep(CTelescope(int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
+                            float(tel.lambda0), float(tel.dlambda), int(tel.psf_size),
+                            float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma)))
+
+
+def c_ssp(ssp, flux) -> _Keep:
+    """``ssp``: object with log_age_axis, log_z_axis (host), lambda0, dlambda; ``flux``: the
+    [n_age, n_z, n_lambda] array the struct should point to (device tensor, or host array for
+    rubix_forward_host)."""
+    age, zed = _host_f32(ssp.log_age_axis), _host_f32(ssp.log_z_axis)
+    n_age, n_z, n_lambda = (int(v) for v in flux.shape)
+    return _Keep(CSSP(n_age, n_z, n_lambda, age.ctypes.data, zed.ctypes.data, float(ssp.lambda0),
+                      float(ssp.dlambda), _ptr(flux)), age, zed, flux)
+
+
+def c_particles(pos, vel, mass, log_age, log_z) -> _Keep:
+    return _Keep(CParticles(int(mass.shape[0]), _ptr(pos), _ptr(vel), _ptr(mass), _ptr(log_age),
+                            _ptr(log_z)), pos, vel, mass, log_age, log_z)
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    return C.c_void_p(int(stream))
+
+
+# ------------------------------------------------------------------------------ the C ABI
+def rubix_workspace_bytes(n, ssp: _Keep, tel: _Keep) -> int:
+    b = int(load().rubix_workspace_bytes(int(n), ssp.ref() if ssp is not None else None, tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_build_cube(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_build_cube(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
+                                   _ptr(workspace), int(workspace.numel() * workspace.element_size()),
+                                   _stream(stream)))
+
+
+def rubix_convolve_psf_lsf(tel: _Keep, cube_in, cube_out, workspace, stream=None):
+    nbytes = 0 if workspace is None else int(workspace.numel() * workspace.element_size())
+    _check(load().rubix_convolve_psf_lsf(tel.ref(), _ptr(cube_in), _ptr(cube_out), _ptr(workspace),
+                                         nbytes, _stream(stream)))
+
+
+def rubix_cube_adjoint(particles: _Keep, ssp: _Keep, tel: _Keep, R, grad_cube, g_mass, g_log_age,
+                       g_log_z, g_vlos, workspace, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_cube_adjoint(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data,
+                                     _ptr(grad_cube), _ptr(g_mass), _ptr(g_log_age), _ptr(g_log_z),
+                                     _ptr(g_vlos), _ptr(workspace),
+                                     int(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
+def rubix_get_sort_artifacts(workspace, n, n_s):
+    """(key[n], perm[n], seg_off[n_s+2]) as int32 torch tensors copied out of the workspace."""
+    import torch
+    k, p, s = C.c_void_p(), C.c_void_p(), C.c_void_p()
+    _check(load().rubix_get_sort_artifacts(_ptr(workspace), C.byref(k), C.byref(p), C.byref(s)))
+    base = workspace.data_ptr()
+    flat = workspace.view(torch.uint8)
+
+    def view(addr, count):
+        off = addr - base
+        return flat[off:off + 4 * count].view(torch.int32).clone()
+
+    return view(k.value, n), view(p.value, n), view(s.value, n_s + 2)
+
+
+def rubix_forward_host_scratch_bytes(n, ssp: _Keep, tel: _Keep) -> int:
+    b = int(load().rubix_forward_host_scratch_bytes(int(n), ssp.ref(), tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_forward_host(particles: _Keep, ssp: _Keep, tel: _Keep, R, h_cube, scratch, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_forward_host(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(h_cube),
+                                     _ptr(scratch), int(scratch.numel() * scratch.element_size()),
+                                     _stream(stream)))
+
+
+# ------------------------------------------------------------------------------ rubix_peaks.h
+def rubix_measure_peaks(scratch, stream=None) -> dict:
+    out = (C.c_float * 4)()
+    _check(load().rubix_measure_peaks(out, _ptr(scratch), int(scratch.numel() * scratch.element_size()),
+                                      _stream(stream)))
+    return {"l2_gbs": out[0], "smem_gbs": out[1], "fma_tflops": out[2], "hbm_copy_gbs": out[3]}
+
+
+def rubix_stage_timing_enable(on: bool):
+    load().rubix_stage_timing_enable(1 if on else 0)
+
+
+def rubix_stage_timing_read() -> dict:
+    ms = (C.c_float * N_STAGES)()
+    calls = (C.c_int32 * N_STAGES)()
+    _check(load().rubix_stage_timing_read(ms, calls))
+    return {name: {"ms": float(ms[i]), "calls": int(calls[i])} for i, name in enumerate(STAGES)}
+
+
+# ------------------------------------------------------------------------------ conveniences
+class DeviceWorkload:
+    """A synth.Workload uploaded to the GPU, with the marshalled structs and a workspace."""
+
+    def __init__(self, w, device="cuda:0", adjoint=False):
+        import torch
+        self.w = w
+        self.device = torch.device(device)
+        p = w.particles
+        up = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(self.device)
+        self.pos, self.vel, self.mass = up(p.pos), up(p.vel), up(p.mass)
+        self.log_age, self.log_z = up(p.log_age), up(p.log_z)
+        self.flux = up(w.ssp.flux)
+        self.particles = c_particles(self.pos, self.vel, self.mass, self.log_age, self.log_z)
+        self.ssp = c_ssp(w.ssp, self.flux)
+        self.tel = c_telescope(w.telescope)
+        self.R = _host_f32(w.rotation)
+        t = w.telescope
+        self.shape = (t.n_x, t.n_y, t.n_channels)
+        self.workspace = torch.empty(rubix_workspace_bytes(p.n, self.ssp, self.tel), dtype=torch.uint8,
+                                     device=self.device)
+
+    def build_cube(self, out=None):
+        import torch
+        cube = torch.empty(self.shape, dtype=torch.float32, device=self.device) if out is None else out
+        rubix_build_cube(self.particles, self.ssp, self.tel, self.R, cube, self.workspace)
+        return cube
+
+    def convolve(self, cube, out=None):
+        import torch
+        res = torch.empty(self.shape, dtype=torch.float32, device=self.device) if out is None else out
+        rubix_convolve_psf_lsf(self.tel, cube, res, self.workspace)
+        return res
+
+    def forward(self):
+        cube = self.build_cube()
+        t = self.w.telescope
+        return self.convolve(cube) if (t.psf_size > 0 or t.lsf_size > 0) else cube
+
+    def adjoint(self, grad_cube):
+        import torch
+        n = self.w.particles.n
+        g = [torch.empty(n, dtype=torch.float32, device=self.device) for _ in range(4)]
+        rubix_cube_adjoint(self.particles, self.ssp, self.tel, self.R, grad_cube, *g, self.workspace)
+        return g
+
+    def sort_artifacts(self):
+        t = self.w.telescope
+        return rubix_get_sort_artifacts(self.workspace, self.w.particles.n, t.n_x * t.n_y)

@@ -1,0 +1,336 @@
+// C ABI of include/rubix.h: argument validation, workspace carve-up, launches.  No CPU fallback.
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <mutex>
+#include <unordered_map>
+
+#include "common.cuh"
+
+namespace rubix {
+thread_local int g_launches = 0;
+}
+
+using namespace rubix;
+
+namespace {
+
+thread_local char t_err[512] = "";
+
+rubix_status fail(rubix_status st, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+rubix_status cuda_fail(cudaError_t e, const char *where)
+{
+    return fail(RUBIX_ERR_CUDA, "%s: %s", where, cudaGetErrorString(e));
+}
+
+struct Artifacts { const int32_t *key, *perm, *seg_off; };
+std::mutex g_mu;
+std::unordered_map<const void *, Artifacts> g_artifacts;
+
+rubix_status check_ssp(const rubix_ssp *s, bool flux_required)
+{
+    if (!s) return fail(RUBIX_ERR_NULL, "ssp is NULL");
+    if (!s->log_age_axis || !s->log_z_axis || (flux_required && !s->flux))
+        return fail(RUBIX_ERR_NULL, "ssp axis / flux pointer is NULL");
+    if (s->n_age < 2 || s->n_z < 2 || s->n_lambda < 2)
+        return fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
+    if (!(s->dlambda > 0.0f) || !isfinite(s->dlambda) || !isfinite(s->lambda0))
+        return fail(RUBIX_ERR_INVALID_ARG, "ssp dlambda must be > 0 and finite");
+    if (s->n_age > kMaxAge || s->n_z > kMaxZ)
+        return fail(RUBIX_ERR_UNSUPPORTED, "ssp axes limited to n_age <= %d, n_z <= %d", kMaxAge, kMaxZ);
+    if ((double)s->n_age * s->n_z * s->n_lambda >= 2147483648.0)
+        return fail(RUBIX_ERR_UNSUPPORTED, "ssp grid must have fewer than 2^31 samples");
+    for (int i = 1; i < s->n_age; ++i)
+        if (!(s->log_age_axis[i] > s->log_age_axis[i - 1]))
+            return fail(RUBIX_ERR_INVALID_ARG, "log_age_axis must be strictly increasing");
+    for (int i = 1; i < s->n_z; ++i)
+        if (!(s->log_z_axis[i] > s->log_z_axis[i - 1]))
+            return fail(RUBIX_ERR_INVALID_ARG, "log_z_axis must be strictly increasing");
+    return RUBIX_OK;
+}
+
+rubix_status check_tel(const rubix_telescope *t)
+{
+    if (!t) return fail(RUBIX_ERR_NULL, "telescope is NULL");
+    if (t->n_x < 1 || t->n_y < 1 || t->n_channels < 1)
+        return fail(RUBIX_ERR_INVALID_ARG, "detector needs n_x, n_y, n_channels >= 1");
+    if ((double)t->n_x * t->n_y >= 2147483647.0 / 2 || (double)t->n_x * t->n_y * t->n_channels >= 9.0e15)
+        return fail(RUBIX_ERR_UNSUPPORTED, "detector too large");
+    if (!(t->spaxel_size > 0.0f) || !isfinite(t->spaxel_size))
+        return fail(RUBIX_ERR_INVALID_ARG, "spaxel_size must be > 0");
+    if (!(t->dlambda > 0.0f) || !isfinite(t->dlambda) || !isfinite(t->lambda0))
+        return fail(RUBIX_ERR_INVALID_ARG, "telescope dlambda must be > 0 and finite");
+    const int sz[2] = {t->psf_size, t->lsf_size};
+    const float sg[2] = {t->psf_sigma, t->lsf_sigma};
+    for (int i = 0; i < 2; ++i) {
+        if (sz[i] < 0 || (sz[i] > 0 && sz[i] % 2 == 0))
+            return fail(RUBIX_ERR_INVALID_ARG, "stencil sizes must be 0 or odd");
+        if (sz[i] > kMaxTaps) return fail(RUBIX_ERR_UNSUPPORTED, "stencil sizes limited to %d taps", kMaxTaps);
+        if (sz[i] > 0 && (!(sg[i] > 0.0f) || !isfinite(sg[i])))
+            return fail(RUBIX_ERR_INVALID_ARG, "stencil sigma must be > 0");
+    }
+    return RUBIX_OK;
+}
+
+rubix_status check_particles(const rubix_particles *p)
+{
+    if (!p) return fail(RUBIX_ERR_NULL, "particles is NULL");
+    if (p->n < 0) return fail(RUBIX_ERR_INVALID_ARG, "n must be >= 0");
+    if (p->n >= 2147483647LL) return fail(RUBIX_ERR_UNSUPPORTED, "n limited to < 2^31 particles");
+    if (p->n > 0 && (!p->pos || !p->vel || !p->mass || !p->log_age || !p->log_z))
+        return fail(RUBIX_ERR_NULL, "a particle array is NULL");
+    return RUBIX_OK;
+}
+
+rubix_status check_resampler(const rubix_ssp *s, const rubix_telescope *t)
+{
+    const double b_max = (double)t->dlambda / (double)s->dlambda / (1.0 - kBetaCap);
+    if (b_max >= 15.0)
+        return fail(RUBIX_ERR_UNSUPPORTED, "dlambda_obs / dlambda_ssp = %.3f is outside the resampler range (< 14.25)",
+                    (double)t->dlambda / (double)s->dlambda);
+    return RUBIX_OK;
+}
+
+rubix_status check_ws(const void *ws, size_t have, size_t need)
+{
+    if (!ws) return fail(RUBIX_ERR_WORKSPACE, "workspace is NULL");
+    if (((uintptr_t)ws & 255u) != 0) return fail(RUBIX_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    if (have < need) return fail(RUBIX_ERR_WORKSPACE, "workspace has %zu bytes, needs %zu", have, need);
+    return RUBIX_OK;
+}
+
+void remember(const void *ws, const Layout &L)
+{
+    const char *b = (const char *)ws;
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_artifacts[ws] = Artifacts{(const int32_t *)(b + L.off_key),
+                                (const int32_t *)(b + L.off_permbuf[L.final_buf]),
+                                (const int32_t *)(b + L.off_seg)};
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *rubix_last_error(void) { return t_err; }
+int32_t rubix_last_launch_count(void) { return g_launches; }
+
+size_t rubix_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
+{
+    t_err[0] = 0;
+    if (n < 0 || n >= 2147483647LL) { fail(RUBIX_ERR_INVALID_ARG, "n out of range"); return 0; }
+    if (check_tel(tel) != RUBIX_OK) return 0;
+    if (ssp && (ssp->n_age < 2 || ssp->n_z < 2 || ssp->n_lambda < 2)) {
+        fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
+        return 0;
+    }
+    return make_layout(n, tel->n_x * tel->n_y, tel->n_channels).bytes_total;
+}
+
+rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                              const float *R, float *cube, void *workspace, size_t workspace_bytes,
+                              void *stream)
+{
+    t_err[0] = 0;
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !cube) return fail(RUBIX_ERR_NULL, "R or cube is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels);
+    if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    PassInputs in{p, ssp, tel, R};
+    cudaError_t e;
+    {
+        StageTimer t(0, st);
+        e = launch_particle_pass(in, L, (char *)workspace, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+    e = launch_accumulate(in, L, (char *)workspace, cube, st);
+    if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+    remember(workspace, L);
+    return RUBIX_OK;
+}
+
+rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cube_in, float *cube_out,
+                                    void *workspace, size_t workspace_bytes, void *stream)
+{
+    t_err[0] = 0;
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!cube_in || !cube_out) return fail(RUBIX_ERR_NULL, "cube_in or cube_out is NULL");
+    const size_t cube_bytes = (size_t)tel->n_x * tel->n_y * tel->n_channels * 4;
+    const char *a = (const char *)cube_in, *b = (const char *)cube_out;
+    if (a < b + cube_bytes && b < a + cube_bytes)
+        return fail(RUBIX_ERR_INVALID_ARG, "cube_in and cube_out overlap");
+    float *tmp = nullptr;
+    if (tel->psf_size > 0) {
+        if ((s = check_ws(workspace, workspace_bytes, align_up(cube_bytes, 256))) != RUBIX_OK) return s;
+        tmp = (float *)workspace;
+    }
+    cudaError_t e;
+    {
+        StageTimer t(3, (cudaStream_t)stream);
+        e = launch_convolve(tel, cube_in, cube_out, tmp, (cudaStream_t)stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "convolve");
+    return RUBIX_OK;
+}
+
+rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                                const float *R, const float *grad_cube, float *g_mass, float *g_log_age,
+                                float *g_log_z, float *g_vlos, void *workspace, size_t workspace_bytes,
+                                void *stream)
+{
+    t_err[0] = 0;
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !grad_cube) return fail(RUBIX_ERR_NULL, "R or grad_cube is NULL");
+    if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
+        return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels);
+    if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    PassInputs in{p, ssp, tel, R};
+    cudaError_t e;
+    {
+        StageTimer t(0, st);
+        e = launch_particle_pass(in, L, ws, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+    // G' = LSF^T PSF^T G: zero-padded symmetric stencils are self-adjoint
+    const float *gconv = grad_cube;
+    if (tel->psf_size > 0 || tel->lsf_size > 0) {
+        {
+            StageTimer t(3, st);
+            e = launch_convolve(tel, grad_cube, (float *)(ws + L.off_cube_a), (float *)(ws + L.off_cube_b), st);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
+        gconv = (const float *)(ws + L.off_cube_a);
+    }
+    {
+        StageTimer t(4, st);
+        e = launch_adjoint(in, L, ws, gconv, g_mass, g_log_age, g_log_z, g_vlos, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "adjoint");
+    remember(workspace, L);
+    return RUBIX_OK;
+}
+
+rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key, const int32_t **perm,
+                                      const int32_t **seg_off)
+{
+    t_err[0] = 0;
+    if (!workspace || !key || !perm || !seg_off) return fail(RUBIX_ERR_NULL, "NULL argument");
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_artifacts.find(workspace);
+    if (it == g_artifacts.end())
+        return fail(RUBIX_ERR_INVALID_ARG, "no rubix_build_cube / rubix_cube_adjoint call has used this workspace");
+    *key = it->second.key;
+    *perm = it->second.perm;
+    *seg_off = it->second.seg_off;
+    return RUBIX_OK;
+}
+
+// ---- end-to-end entry with host buffers ------------------------------------------------------
+namespace {
+struct HostLayout { size_t pos, vel, mass, age, z, flux, cube, cube2, ws, total; };
+HostLayout host_layout(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
+{
+    HostLayout H{};
+    size_t off = 0;
+    auto take = [&](size_t b) { size_t o = off; off = align_up(off + b, 256); return o; };
+    const size_t nn = (size_t)(n > 0 ? n : 1);
+    H.pos = take(nn * 12);
+    H.vel = take(nn * 12);
+    H.mass = take(nn * 4);
+    H.age = take(nn * 4);
+    H.z = take(nn * 4);
+    H.flux = take((size_t)ssp->n_age * ssp->n_z * ssp->n_lambda * 4);
+    const size_t cube = (size_t)tel->n_x * tel->n_y * tel->n_channels * 4;
+    H.cube = take(cube);
+    H.cube2 = take(cube);
+    H.ws = off;
+    H.total = off + make_layout(n, tel->n_x * tel->n_y, tel->n_channels).bytes_total;
+    return H;
+}
+}  // namespace
+
+size_t rubix_forward_host_scratch_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
+{
+    t_err[0] = 0;
+    if (n < 0 || n >= 2147483647LL || !ssp || check_tel(tel) != RUBIX_OK || ssp->n_age < 2 || ssp->n_z < 2 ||
+        ssp->n_lambda < 2) {
+        if (!t_err[0]) fail(RUBIX_ERR_INVALID_ARG, "bad arguments");
+        return 0;
+    }
+    return host_layout(n, ssp, tel).total;
+}
+
+rubix_status rubix_forward_host(const rubix_particles *hp, const rubix_ssp *hs, const rubix_telescope *tel,
+                                const float *R, float *h_cube, void *scratch, size_t scratch_bytes,
+                                void *stream)
+{
+    t_err[0] = 0;
+    rubix_status s;
+    if ((s = check_particles(hp)) != RUBIX_OK) return s;
+    if ((s = check_ssp(hs, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !h_cube) return fail(RUBIX_ERR_NULL, "R or h_cube is NULL");
+    const HostLayout H = host_layout(hp->n, hs, tel);
+    if ((s = check_ws(scratch, scratch_bytes, H.total)) != RUBIX_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *d = (char *)scratch;
+    const size_t n = (size_t)hp->n;
+    cudaError_t e = cudaSuccess;
+    auto up = [&](size_t off, const void *src, size_t bytes) {
+        if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(d + off, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    up(H.pos, hp->pos, n * 12);
+    up(H.vel, hp->vel, n * 12);
+    up(H.mass, hp->mass, n * 4);
+    up(H.age, hp->log_age, n * 4);
+    up(H.z, hp->log_z, n * 4);
+    up(H.flux, hs->flux, (size_t)hs->n_age * hs->n_z * hs->n_lambda * 4);
+    if (e != cudaSuccess) return cuda_fail(e, "host->device copy");
+    rubix_particles dp{hp->n, (const float *)(d + H.pos), (const float *)(d + H.vel), (const float *)(d + H.mass),
+                       (const float *)(d + H.age), (const float *)(d + H.z)};
+    rubix_ssp ds = *hs;
+    ds.flux = (const float *)(d + H.flux);
+    const size_t ws_bytes = scratch_bytes - H.ws;
+    s = rubix_build_cube(&dp, &ds, tel, R, (float *)(d + H.cube), d + H.ws, ws_bytes, stream);
+    if (s != RUBIX_OK) return s;
+    int launches = g_launches;
+    float *final_cube = (float *)(d + H.cube);
+    if (tel->psf_size > 0 || tel->lsf_size > 0) {
+        s = rubix_convolve_psf_lsf(tel, (const float *)(d + H.cube), (float *)(d + H.cube2), d + H.ws, ws_bytes, stream);
+        if (s != RUBIX_OK) return s;
+        launches += g_launches;
+        final_cube = (float *)(d + H.cube2);
+    }
+    g_launches = launches;
+    e = cudaMemcpyAsync(h_cube, final_cube, (size_t)tel->n_x * tel->n_y * tel->n_channels * 4,
+                        cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(e, "device->host copy");
+    return RUBIX_OK;
+}
+
+}  // extern "C"

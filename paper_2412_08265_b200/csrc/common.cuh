@@ -1,0 +1,113 @@
+// Shared declarations of the CUDA path (never included by oracle/).
+// Notation follows SURVEY.md section 8: N particles, N_s spaxels, N_c channels, SSP N_a x N_z x N_l.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/rubix.h"
+
+namespace rubix {
+
+// ---- fixed constants of the method ------------------------------------
+constexpr double kCkms = 299792.458;        // speed of light, km/s
+constexpr float kVcapKms = 14989.623f;      // 0.05 c: |v_los| beyond this drops the particle
+constexpr double kBetaCap = 0.05;
+
+// ---- implementation constants ------------------------------------------------------------------
+constexpr int kFxFrac = 28;                 // fractional bits of the rest-position fixed point
+constexpr int kChunk = 128;                 // particles per work unit of the accumulate kernel
+constexpr int kMaxAge = 512, kMaxZ = 128;   // SSP axes travel as kernel parameters
+constexpr int kMaxTaps = 63;
+constexpr int kAccThreads = 256;            // threads per CTA of the accumulate kernel
+constexpr int kTabMax = 4096;               // table entries addressable by the 12.20 local format
+constexpr int kSortWarps = 8;               // warps per CTA in the radix passes
+constexpr int kSortItems = 1024;            // keys per warp per radix pass
+constexpr int kSortMaxDigitBits = 9;
+
+// Sorted-order particle record consumed by the accumulate kernel (48 B, 16-B aligned).
+struct __align__(16) Rec {
+    float w[4];        // mass x bilinear weights of corners (i,j) (i+1,j) (i,j+1) (i+1,j+1)
+    int32_t cell;      // float offset of T[i][j][0] in the flux array
+    uint32_t b_fx;     // B = dl_obs / (dl_ssp (1+beta)) in 4.28 fixed point
+    int64_t a_fx;      // A = (l0_obs/(1+beta) - l0_ssp)/dl_ssp in 36.28 fixed point
+    int32_t k_lo, k_hi;  // channels whose rest position lies inside the SSP coverage
+    int32_t pad[2];
+};
+static_assert(sizeof(Rec) == 48, "Rec layout");
+
+// One work unit of the accumulate kernel: up to kChunk consecutive sorted particles of one spaxel.
+struct __align__(16) Unit {
+    int32_t start;     // first sorted index
+    int32_t count;     // 0 = empty spaxel (zero fill)
+    int32_t spaxel;
+    int32_t part_row;  // >= 0: write a partial row (multi-chunk spaxel); -1: write the cube row
+};
+
+struct AxisParams {               // SSP axes, passed by value
+    float age[kMaxAge];
+    float z[kMaxZ];
+    int32_t n_age, n_z;
+};
+
+struct Taps {
+    float w[kMaxTaps];
+    int32_t size;                 // 0 = stage off
+};
+
+// ---- workspace carve-up (host) ---------------------------------------------------------------
+struct Layout {
+    int64_t n;
+    int32_t n_s, n_c;
+    int32_t sort_passes, digit_bits, n_wchunks;
+    int64_t max_units, max_part_rows, max_multi;
+    size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
+        off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_units, off_rec,
+        off_partials, off_cube_a, off_cube_b;
+    size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
+    int final_buf;                // which of the ping-pong buffers holds the final sort
+};
+
+Layout make_layout(int64_t n, int32_t n_s, int32_t n_c);
+
+// ---- host launchers (each returns the CUDA status of its launches) ----------------------------
+struct PassInputs {
+    const rubix_particles *p;
+    const rubix_ssp *ssp;
+    const rubix_telescope *tel;
+    const float *R;
+};
+
+cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
+cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube,
+                              cudaStream_t st);
+cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp,
+                            cudaStream_t st);
+cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
+                           float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st);
+
+void make_taps(int size, float sigma, Taps *t);
+
+extern thread_local int g_launches;
+
+// Records a CUDA event pair around a stage when stage timing is on (include/rubix_peaks.h).
+class StageTimer {
+public:
+    StageTimer(int stage, cudaStream_t st);
+    ~StageTimer();
+private:
+    int stage_;
+    cudaStream_t st_;
+    cudaEvent_t a_;
+};
+
+#define RUBIX_LAUNCH_CHECK()                         \
+    do {                                             \
+        ++::rubix::g_launches;                       \
+        cudaError_t e_ = cudaGetLastError();         \
+        if (e_ != cudaSuccess) return e_;            \
+    } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace rubix

@@ -1,0 +1,453 @@
+// Particle pass: steps 1-3 of the hot path plus the per-particle records for steps 4-5.
+//   K1  k_rotate_bin        rotate, project, bin  (fp32, fixed order)
+//   K2  k_sort_*            stable LSD radix sort of (key, index)            (8(a) row 3)
+//       k_segment_offsets   seg_off[s] = lower_bound(sorted keys, s)  -- no atomics anywhere
+//       k_scan_units        work units (chunks of <= kChunk particles) per spaxel, partial rows
+//       k_build_units       unit descriptors
+//   K2c k_prepare_records   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
+#include "common.cuh"
+
+namespace rubix {
+
+// --------------------------------------------------------------------------------------------
+// K1.  Every * and + is a separately rounded fp32 op (no FMA contraction), in the order
+//   xr = (R00*x + R01*y) + R02*z ;  u = (xr + (0.5f*N_x)*s) / s ;  key = floor(u)*N_y + floor(v)
+// so the key equals the oracle's bit for bit.  NaN fails every comparison => dropped.
+// --------------------------------------------------------------------------------------------
+struct BinParams {
+    float R[9];
+    int32_t n_x, n_y;
+    float s;
+    int64_t n;
+};
+
+__global__ void __launch_bounds__(256)
+k_rotate_bin(const float *__restrict__ pos, const float *__restrict__ vel, BinParams P,
+             int32_t *__restrict__ key, float *__restrict__ vlos)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    const float vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+    const float xr = __fadd_rn(__fadd_rn(__fmul_rn(P.R[0], x), __fmul_rn(P.R[1], y)), __fmul_rn(P.R[2], z));
+    const float yr = __fadd_rn(__fadd_rn(__fmul_rn(P.R[3], x), __fmul_rn(P.R[4], y)), __fmul_rn(P.R[5], z));
+    const float vl = __fadd_rn(__fadd_rn(__fmul_rn(P.R[6], vx), __fmul_rn(P.R[7], vy)), __fmul_rn(P.R[8], vz));
+    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x), P.s);
+    const float hy = __fmul_rn(__fmul_rn(0.5f, (float)P.n_y), P.s);
+    const float u = __fdiv_rn(__fadd_rn(xr, hx), P.s);
+    const float v = __fdiv_rn(__fadd_rn(yr, hy), P.s);
+    const bool inside = (u >= 0.0f) && (u < (float)P.n_x) && (v >= 0.0f) && (v < (float)P.n_y) &&
+                        (fabsf(vl) <= kVcapKms);
+    key[i] = inside ? (int32_t)floorf(u) * P.n_y + (int32_t)floorf(v) : P.n_x * P.n_y;
+    vlos[i] = vl;
+}
+
+// --------------------------------------------------------------------------------------------
+// K2.  Stable LSD radix sort.  Each WARP owns kSortItems consecutive keys ("warp chunk") and is
+// one column of the classic counting-sort histogram matrix histT[digit][warp chunk]; ranks
+// inside a 32-key round come from __match_any_sync, so equal keys keep their index order.
+// --------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, int n_wchunks,
+            int32_t *__restrict__ histT)
+{
+    __shared__ int32_t cnt[kSortWarps][1 << kSortMaxDigitBits];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = blockIdx.x * kSortWarps + warp;
+    if (wc >= n_wchunks) return;
+    for (int d = lane; d <= mask; d += 32) cnt[warp][d] = 0;
+    __syncwarp();
+    const int64_t base = (int64_t)wc * kSortItems;
+    for (int r = 0; r < kSortItems; r += 32) {
+        const int64_t i = base + r + lane;
+        if (i < n) atomicAdd(&cnt[warp][(key_in[i] >> shift) & mask], 1);
+    }
+    __syncwarp();
+    for (int d = lane; d <= mask; d += 32) histT[(int64_t)d * n_wchunks + wc] = cnt[warp][d];
+}
+
+// one CTA per digit: exclusive scan of its row of histT, row total to digit_total
+__global__ void __launch_bounds__(256)
+k_sort_rowscan(int32_t *__restrict__ histT, int n_wchunks, int32_t *__restrict__ digit_total)
+{
+    __shared__ int32_t warp_sum[8];
+    __shared__ int32_t carry_s;
+    int32_t *row = histT + (int64_t)blockIdx.x * n_wchunks;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < n_wchunks; base += 256) {
+        const int i = base + threadIdx.x;
+        const int32_t v = i < n_wchunks ? row[i] : 0;
+        int32_t inc = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) warp_sum[warp] = inc;
+        __syncthreads();
+        int32_t wpre = 0;
+        for (int w = 0; w < warp; ++w) wpre += warp_sum[w];
+        const int32_t carry = carry_s;
+        if (i < n_wchunks) row[i] = carry + wpre + inc - v;
+        __syncthreads();
+        if (threadIdx.x == 255) carry_s = carry + wpre + inc;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) digit_total[blockIdx.x] = carry_s;
+}
+
+__global__ void __launch_bounds__(1 << kSortMaxDigitBits)
+k_sort_digitscan(const int32_t *__restrict__ digit_total, int n_digits, int32_t *__restrict__ digit_base)
+{
+    __shared__ int32_t s[1 << kSortMaxDigitBits];
+    const int t = threadIdx.x;
+    s[t] = t < n_digits ? digit_total[t] : 0;
+    __syncthreads();
+    for (int o = 1; o < (1 << kSortMaxDigitBits); o <<= 1) {
+        const int32_t v = t >= o ? s[t - o] : 0;
+        __syncthreads();
+        s[t] += v;
+        __syncthreads();
+    }
+    if (t < n_digits) digit_base[t] = s[t] - digit_total[t];
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_sort_scatter(const int32_t *__restrict__ key_in, const int32_t *__restrict__ perm_in, int64_t n,
+               int shift, int mask, int n_wchunks, const int32_t *__restrict__ histT,
+               const int32_t *__restrict__ digit_base, int32_t *__restrict__ key_out,
+               int32_t *__restrict__ perm_out)
+{
+    __shared__ int32_t cur[kSortWarps][1 << kSortMaxDigitBits];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = blockIdx.x * kSortWarps + warp;
+    if (wc >= n_wchunks) return;
+    for (int d = lane; d <= mask; d += 32)
+        cur[warp][d] = digit_base[d] + histT[(int64_t)d * n_wchunks + wc];
+    __syncwarp();
+    const int64_t base = (int64_t)wc * kSortItems;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int r = 0; r < kSortItems; r += 32) {
+        const int64_t i = base + r + lane;
+        const bool valid = i < n;
+        const int32_t k = valid ? key_in[i] : 0;
+        const int32_t v = valid ? (FIRST ? (int32_t)i : perm_in[i]) : 0;
+        const int d = valid ? ((k >> shift) & mask) : (0x10000 + lane);   // invalid lanes never match
+        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const int rank = __popc(peers & lt);
+        int32_t dst = 0;
+        if (valid) dst = cur[warp][d] + rank;
+        __syncwarp();
+        if (valid && rank == 0) cur[warp][d] += __popc(peers);
+        __syncwarp();
+        if (valid) {
+            key_out[dst] = k;
+            perm_out[dst] = v;
+        }
+    }
+}
+
+// seg_off[s] = first sorted position whose key is >= s   (s = 0 .. n_s+1)
+__global__ void __launch_bounds__(256)
+k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s,
+                  int32_t *__restrict__ seg_off)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s > n_s + 1) return;
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (key_sorted[mid] < s) lo = mid + 1; else hi = mid;
+    }
+    seg_off[s] = (int32_t)lo;
+}
+
+// Single CTA: three exclusive scans over the spaxels in one sweep.
+//   unit_off: max(1, chunks(s))     part_off: chunks(s) if > 1 else 0     multi index: chunks(s) > 1
+// totals = { n_units, n_part_rows, n_multi }
+__global__ void __launch_bounds__(1024)
+k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restrict__ unit_off,
+             int32_t *__restrict__ part_off, int32_t *__restrict__ multi_list,
+             int32_t *__restrict__ totals)
+{
+    __shared__ int32_t wsum[3][32];
+    __shared__ int32_t carry[3];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < 3) carry[threadIdx.x] = 0;
+    __syncthreads();
+    for (int base = 0; base < n_s; base += 1024) {
+        const int s = base + threadIdx.x;
+        int32_t v[3] = {0, 0, 0};
+        if (s < n_s) {
+            const int32_t cnt = seg_off[s + 1] - seg_off[s];
+            const int32_t chunks = (cnt + kChunk - 1) / kChunk;
+            v[0] = chunks > 1 ? chunks : 1;
+            v[1] = chunks > 1 ? chunks : 0;
+            v[2] = chunks > 1 ? 1 : 0;
+        }
+        int32_t inc[3];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            inc[q] = v[q];
+            for (int o = 1; o < 32; o <<= 1) {
+                const int32_t t = __shfl_up_sync(0xffffffffu, inc[q], o);
+                if (lane >= o) inc[q] += t;
+            }
+            if (lane == 31) wsum[q][warp] = inc[q];
+        }
+        __syncthreads();
+        int32_t ex[3];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            int32_t wpre = 0;
+            for (int w = 0; w < warp; ++w) wpre += wsum[q][w];
+            ex[q] = carry[q] + wpre + inc[q] - v[q];
+        }
+        if (s < n_s) {
+            unit_off[s] = ex[0];
+            part_off[s] = ex[1];
+            if (v[2]) multi_list[ex[2]] = s;
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) carry[q] = ex[q] + v[q];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        unit_off[n_s] = carry[0];
+        part_off[n_s] = carry[1];
+        totals[0] = carry[0];
+        totals[1] = carry[1];
+        totals[2] = carry[2];
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_build_units(const int32_t *__restrict__ seg_off, const int32_t *__restrict__ unit_off,
+              const int32_t *__restrict__ part_off, int32_t n_s, Unit *__restrict__ units)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= unit_off[n_s]) return;
+    int lo = 0, hi = n_s - 1;          // largest s with unit_off[s] <= u
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (unit_off[mid] <= u) lo = mid; else hi = mid - 1;
+    }
+    const int s = lo, c = u - unit_off[s];
+    const int32_t first = seg_off[s], cnt = seg_off[s + 1] - first;
+    Unit U;
+    U.spaxel = s;
+    U.start = first + c * kChunk;
+    U.count = cnt > 0 ? min(kChunk, cnt - c * kChunk) : 0;
+    U.part_row = cnt > kChunk ? part_off[s] + c : -1;
+    units[u] = U;
+}
+
+// --------------------------------------------------------------------------------------------
+// K2c.  Per in-FoV particle, in sorted order:
+//   cell i = clamp(max{j : A[j] <= q}, 0, n-2), t = clamp((q - A[i]) / (A[i+1] - A[i]), 0, 1)
+//   w = mass * {(1-ta)(1-tz), ta(1-tz), (1-ta)tz, ta tz}                       (fp64 -> fp32)
+//   rest position of channel k in SSP samples:  x_k = A + B k,
+//   A = (l0_obs/(1+beta) - l0_ssp)/dl_ssp,  B = dl_obs/((1+beta) dl_ssp),  beta = v_los/c  (fp64)
+//   stored as 28-bit-fraction fixed point so every kernel evaluates x_k with the same integers;
+//   [k_lo, k_hi] = channels with 0 <= x_k <= N_l - 1 (zero contribution outside the coverage).
+// --------------------------------------------------------------------------------------------
+struct PrepParams {
+    AxisParams ax;
+    int32_t n_lambda, n_c, n_s;
+    float l0_ssp, dl_ssp, l0_obs, dl_obs;
+};
+
+__device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *cell, double *t)
+{
+    int lo = 0, hi = n - 1;            // largest j with A[j] <= q, or 0
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (A[mid] <= q) lo = mid; else hi = mid - 1;
+    }
+    int i = min(lo, n - 2);
+    double tt = ((double)q - (double)A[i]) / ((double)A[i + 1] - (double)A[i]);
+    tt = fmin(fmax(tt, 0.0), 1.0);
+    *cell = i;
+    *t = tt;
+}
+
+__global__ void __launch_bounds__(256)
+k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
+                  const float *__restrict__ vlos, const float *__restrict__ mass,
+                  const float *__restrict__ log_age, const float *__restrict__ log_z,
+                  const __grid_constant__ PrepParams P, Rec *__restrict__ rec)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= seg_off[P.n_s]) return;            // dropped particles sort last and get no record
+    const int p = perm[i];
+    int ia, iz;
+    double ta, tz;
+    axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta);
+    axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz);
+    const double m = (double)mass[p];
+    Rec r;
+    r.w[0] = (float)(m * (1.0 - ta) * (1.0 - tz));
+    r.w[1] = (float)(m * ta * (1.0 - tz));
+    r.w[2] = (float)(m * (1.0 - ta) * tz);
+    r.w[3] = (float)(m * ta * tz);
+    r.cell = (ia * P.ax.n_z + iz) * P.n_lambda;
+    const double inv = 1.0 / (1.0 + (double)vlos[p] / kCkms);
+    const double scale = (double)(1 << kFxFrac);
+    const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
+    const double B = (double)P.dl_obs * inv / (double)P.dl_ssp;
+    const int64_t a_fx = __double2ll_rn(A * scale);
+    const uint32_t b_fx = (uint32_t)__double2ll_rn(B * scale);
+    r.a_fx = a_fx;
+    r.b_fx = b_fx;
+    const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
+    int64_t k_lo = a_fx >= 0 ? 0 : (-a_fx + (int64_t)b_fx - 1) / (int64_t)b_fx;
+    int64_t k_hi = a_fx > x_max ? -1 : (x_max - a_fx) / (int64_t)b_fx;
+    if (k_hi > P.n_c - 1) k_hi = P.n_c - 1;
+    if (k_lo > P.n_c) k_lo = P.n_c;
+    r.k_lo = (int32_t)k_lo;
+    r.k_hi = (int32_t)k_hi;
+    r.pad[0] = r.pad[1] = 0;
+    rec[i] = r;
+}
+
+// --------------------------------------------------------------------------------------------
+// host side
+// --------------------------------------------------------------------------------------------
+static int bits_for(int32_t max_value)
+{
+    int b = 1;
+    while ((1ll << b) <= (long long)max_value) ++b;
+    return b;
+}
+
+Layout make_layout(int64_t n, int32_t n_s, int32_t n_c)
+{
+    Layout L{};
+    L.n = n;
+    L.n_s = n_s;
+    L.n_c = n_c;
+    const int bits = bits_for(n_s);                      // keys are 0 .. n_s
+    L.sort_passes = (bits + kSortMaxDigitBits - 1) / kSortMaxDigitBits;
+    L.digit_bits = (bits + L.sort_passes - 1) / L.sort_passes;
+    L.n_wchunks = (int32_t)((n + kSortItems - 1) / kSortItems);
+    L.max_units = (int64_t)n_s + n / kChunk + 1;
+    L.max_part_rows = 2 * (n / kChunk) + 2;
+    L.max_multi = n / kChunk + 1;
+    L.final_buf = (L.sort_passes - 1) & 1;
+    const size_t nn = (size_t)(n > 0 ? n : 1);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    // two cube-sized buffers come first: rubix_convolve_psf_lsf (which does not know n) uses the
+    // first one as its temporary, so it never touches the sort artefacts behind them
+    const size_t cube = (size_t)n_s * (size_t)n_c * 4;
+    L.off_cube_a = take(cube);
+    L.off_cube_b = take(cube);
+    L.off_key = take(nn * 4);
+    L.off_vlos = take(nn * 4);
+    L.off_seg = take(((size_t)n_s + 2) * 4);
+    for (int b = 0; b < 2; ++b) {
+        L.off_keybuf[b] = take(nn * 4);
+        L.off_permbuf[b] = take(nn * 4);
+    }
+    L.off_hist = take((size_t)(1 << L.digit_bits) * (size_t)(L.n_wchunks > 0 ? L.n_wchunks : 1) * 4);
+    L.off_dtot = take((size_t)(1 << kSortMaxDigitBits) * 4);
+    L.off_dbase = take((size_t)(1 << kSortMaxDigitBits) * 4);
+    L.off_unitoff = take(((size_t)n_s + 1) * 4);
+    L.off_partoff = take(((size_t)n_s + 1) * 4);
+    L.off_multi = take((size_t)L.max_multi * 4);
+    L.off_totals = take(16);
+    L.off_units = take((size_t)L.max_units * sizeof(Unit));
+    L.off_rec = take(nn * sizeof(Rec));
+    L.off_partials = take((size_t)L.max_part_rows * (size_t)n_c * 4);
+    L.bytes_total = off;
+    return L;
+}
+
+cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st)
+{
+    const int64_t n = L.n;
+    const int32_t n_s = L.n_s;
+    int32_t *key = (int32_t *)(ws + L.off_key);
+    float *vlos = (float *)(ws + L.off_vlos);
+    int32_t *seg = (int32_t *)(ws + L.off_seg);
+    int32_t *kbuf[2] = {(int32_t *)(ws + L.off_keybuf[0]), (int32_t *)(ws + L.off_keybuf[1])};
+    int32_t *pbuf[2] = {(int32_t *)(ws + L.off_permbuf[0]), (int32_t *)(ws + L.off_permbuf[1])};
+    int32_t *histT = (int32_t *)(ws + L.off_hist);
+    int32_t *dtot = (int32_t *)(ws + L.off_dtot);
+    int32_t *dbase = (int32_t *)(ws + L.off_dbase);
+    int32_t *unit_off = (int32_t *)(ws + L.off_unitoff);
+    int32_t *part_off = (int32_t *)(ws + L.off_partoff);
+    int32_t *multi = (int32_t *)(ws + L.off_multi);
+    int32_t *totals = (int32_t *)(ws + L.off_totals);
+    Unit *units = (Unit *)(ws + L.off_units);
+    Rec *rec = (Rec *)(ws + L.off_rec);
+
+    if (n > 0) {
+        BinParams B;
+        for (int i = 0; i < 9; ++i) B.R[i] = in.R[i];
+        B.n_x = in.tel->n_x;
+        B.n_y = in.tel->n_y;
+        B.s = in.tel->spaxel_size;
+        B.n = n;
+        k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, key, vlos);
+        RUBIX_LAUNCH_CHECK();
+
+        const int mask = (1 << L.digit_bits) - 1;
+        const int n_digits = 1 << L.digit_bits;
+        const unsigned sort_grid = (unsigned)((L.n_wchunks + kSortWarps - 1) / kSortWarps);
+        const int32_t *kin = key;
+        const int32_t *pin = nullptr;
+        for (int pass = 0; pass < L.sort_passes; ++pass) {
+            const int shift = pass * L.digit_bits;
+            int32_t *kout = kbuf[pass & 1], *pout = pbuf[pass & 1];
+            k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, histT);
+            RUBIX_LAUNCH_CHECK();
+            k_sort_rowscan<<<n_digits, 256, 0, st>>>(histT, L.n_wchunks, dtot);
+            RUBIX_LAUNCH_CHECK();
+            k_sort_digitscan<<<1, 1 << kSortMaxDigitBits, 0, st>>>(dtot, n_digits, dbase);
+            RUBIX_LAUNCH_CHECK();
+            if (pass == 0)
+                k_sort_scatter<true><<<sort_grid, kSortWarps * 32, 0, st>>>(
+                    kin, pin, n, shift, mask, L.n_wchunks, histT, dbase, kout, pout);
+            else
+                k_sort_scatter<false><<<sort_grid, kSortWarps * 32, 0, st>>>(
+                    kin, pin, n, shift, mask, L.n_wchunks, histT, dbase, kout, pout);
+            RUBIX_LAUNCH_CHECK();
+            kin = kout;
+            pin = pout;
+        }
+    }
+    const int32_t *key_sorted = kbuf[L.final_buf];
+    const int32_t *perm = pbuf[L.final_buf];
+    k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, seg);
+    RUBIX_LAUNCH_CHECK();
+    k_scan_units<<<1, 1024, 0, st>>>(seg, n_s, unit_off, part_off, multi, totals);
+    RUBIX_LAUNCH_CHECK();
+    k_build_units<<<(unsigned)((L.max_units + 255) / 256), 256, 0, st>>>(seg, unit_off, part_off, n_s, units);
+    RUBIX_LAUNCH_CHECK();
+    if (n > 0) {
+        PrepParams P;
+        P.ax.n_age = in.ssp->n_age;
+        P.ax.n_z = in.ssp->n_z;
+        for (int i = 0; i < in.ssp->n_age; ++i) P.ax.age[i] = in.ssp->log_age_axis[i];
+        for (int i = 0; i < in.ssp->n_z; ++i) P.ax.z[i] = in.ssp->log_z_axis[i];
+        P.n_lambda = in.ssp->n_lambda;
+        P.n_c = in.tel->n_channels;
+        P.n_s = n_s;
+        P.l0_ssp = in.ssp->lambda0;
+        P.dl_ssp = in.ssp->dlambda;
+        P.l0_obs = in.tel->lambda0;
+        P.dl_obs = in.tel->dlambda;
+        k_prepare_records<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
+            perm, seg, vlos, in.p->mass, in.p->log_age, in.p->log_z, P, rec);
+        RUBIX_LAUNCH_CHECK();
+    }
+    return cudaSuccess;
+}
+
+}  // namespace rubix

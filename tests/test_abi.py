@@ -1,0 +1,150 @@
+"""The C-ABI library: it builds, loads without a GPU, exports every symbol include/rubix.h
+declares, and validates its arguments on the host before any launch.
+No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2412_08265_b200 import binding as B
+from paper_2412_08265_b200 import build as builder
+from paper_2412_08265_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+FAKE = 0x10000          # non-NULL, 256-byte aligned "device" address that is never dereferenced
+
+
+@pytest.fixture(scope="module")
+def lib():
+    builder.build()
+    return B.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    import glob
+    header = "".join(open(h).read() for h in sorted(glob.glob(os.path.join(ROOT, "include", "*.h"))))
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(rubix_[a-z_]+)\s*\(", header))
+    assert declared == set(B.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_struct_layouts_match_the_header():
+    assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 48 and C.sizeof(B.CTelescope) == 40
+
+
+def _structs(tel=None, ssp=None):
+    tel = tel or synth.make_telescope("medium")
+    ssp = ssp or synth.make_ssp(8, 4, 512, 3500.0, 9500.0, 1)
+    fake_flux = np.empty((ssp.flux.shape), np.float32)
+    return B.c_ssp(ssp, fake_flux), B.c_telescope(tel)
+
+
+def test_workspace_bytes(lib):
+    ssp, tel = _structs()
+    small = B.rubix_workspace_bytes(0, ssp, tel)
+    big = B.rubix_workspace_bytes(1_000_000, ssp, tel)
+    cube = 300 * 300 * 3700 * 4
+    assert small >= 2 * cube and big > small and big < small + 1_000_000 * 120 + (1 << 28)
+    with pytest.raises(B.RubixError):
+        B.rubix_workspace_bytes(-1, ssp, tel)
+    assert "n out of range" in B.rubix_last_error()
+
+
+def _call_build(lib, particles, ssp, tel, R=None, cube=FAKE, ws=FAKE, ws_bytes=1 << 40):
+    R = np.eye(3, dtype=np.float32).reshape(9) if R is None else R
+    return lib.rubix_build_cube(particles.ref() if particles else None, ssp.ref() if ssp else None,
+                                tel.ref() if tel else None, R.ctypes.data if R is not False else None,
+                                cube, ws, ws_bytes, None)
+
+
+def _fake_particles(n=10):
+    class T:  # minimal stand-in with data_ptr/shape
+        def __init__(self, shape): self.shape = shape
+        def data_ptr(self): return FAKE
+    return B.c_particles(T((n, 3)), T((n, 3)), T((n,)), T((n,)), T((n,)))
+
+
+def test_argument_validation_happens_before_any_launch(lib):
+    ssp, tel = _structs()
+    P = _fake_particles()
+    assert _call_build(lib, None, ssp, tel) == B.RUBIX_ERR_NULL
+    assert _call_build(lib, P, None, tel) == B.RUBIX_ERR_NULL
+    assert _call_build(lib, P, ssp, None) == B.RUBIX_ERR_NULL
+    assert _call_build(lib, P, ssp, tel, R=False) == B.RUBIX_ERR_NULL
+    assert _call_build(lib, P, ssp, tel, cube=None) == B.RUBIX_ERR_NULL
+    assert _call_build(lib, P, ssp, tel, ws=None) == B.RUBIX_ERR_WORKSPACE
+    assert _call_build(lib, P, ssp, tel, ws=FAKE + 8) == B.RUBIX_ERR_WORKSPACE          # misaligned
+    assert _call_build(lib, P, ssp, tel, ws_bytes=1024) == B.RUBIX_ERR_WORKSPACE
+    assert "needs" in B.rubix_last_error()
+    neg = _fake_particles()
+    neg.struct.n = -5
+    assert _call_build(lib, neg, ssp, tel) == B.RUBIX_ERR_INVALID_ARG
+    nullarr = _fake_particles()
+    nullarr.struct.mass = None
+    assert _call_build(lib, nullarr, ssp, tel) == B.RUBIX_ERR_NULL
+
+
+@pytest.mark.parametrize("field,value,status", [
+    ("psf_size", 14, B.RUBIX_ERR_INVALID_ARG), ("lsf_size", -1, B.RUBIX_ERR_INVALID_ARG),
+    ("psf_size", 65, B.RUBIX_ERR_UNSUPPORTED), ("psf_sigma", 0.0, B.RUBIX_ERR_INVALID_ARG),
+    ("dlambda", 0.0, B.RUBIX_ERR_INVALID_ARG), ("dlambda", float("nan"), B.RUBIX_ERR_INVALID_ARG),
+    ("spaxel_size", -1.0, B.RUBIX_ERR_INVALID_ARG), ("n_x", 0, B.RUBIX_ERR_INVALID_ARG),
+    ("n_channels", 0, B.RUBIX_ERR_INVALID_ARG), ("dlambda", 400.0, B.RUBIX_ERR_UNSUPPORTED)])
+def test_bad_telescope(lib, field, value, status):
+    ssp, tel = _structs()
+    setattr(tel.struct, field, value)
+    assert _call_build(lib, _fake_particles(), ssp, tel) == status
+    assert B.rubix_last_error() != ""
+
+
+def test_bad_ssp(lib):
+    P = _fake_particles()
+    base = synth.make_ssp(8, 4, 512, 3500.0, 9500.0, 1)
+    for mutate, status in [
+        (lambda s: s.log_age_axis.__setitem__(3, s.log_age_axis[2]), B.RUBIX_ERR_INVALID_ARG),
+        (lambda s: s.log_z_axis.__setitem__(slice(None), s.log_z_axis[::-1].copy()), B.RUBIX_ERR_INVALID_ARG),
+        (lambda s: setattr(s, "dlambda", np.float32(-1.0)), B.RUBIX_ERR_INVALID_ARG)]:
+        s = synth.SSPGrid(base.log_age_axis.copy(), base.log_z_axis.copy(), base.lambda0, base.dlambda, base.flux)
+        mutate(s)
+        ssp, tel = _structs(ssp=s)
+        assert _call_build(lib, P, ssp, tel) == status
+    ssp, tel = _structs()
+    ssp.struct.n_age = 1
+    assert _call_build(lib, P, ssp, tel) == B.RUBIX_ERR_INVALID_ARG
+    ssp, tel = _structs()
+    ssp.struct.n_age = 600
+    assert _call_build(lib, P, ssp, tel) == B.RUBIX_ERR_UNSUPPORTED
+    ssp, tel = _structs()
+    ssp.struct.flux = None
+    assert _call_build(lib, P, ssp, tel) == B.RUBIX_ERR_NULL
+
+
+def test_convolve_and_adjoint_validation(lib):
+    ssp, tel = _structs()
+    cube_bytes = 300 * 300 * 3700 * 4
+    f = lib.rubix_convolve_psf_lsf
+    assert f(tel.ref(), None, FAKE, FAKE, 1 << 40, None) == B.RUBIX_ERR_NULL
+    assert f(tel.ref(), FAKE, FAKE + 4096, FAKE, 1 << 40, None) == B.RUBIX_ERR_INVALID_ARG   # overlap
+    assert f(tel.ref(), FAKE, FAKE + 2 * cube_bytes, FAKE, 16, None) == B.RUBIX_ERR_WORKSPACE
+    g = lib.rubix_cube_adjoint
+    R = np.eye(3, dtype=np.float32).reshape(9)
+    P = _fake_particles()
+    assert g(P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, None, FAKE, FAKE, FAKE, FAKE, FAKE, 1 << 40, None) \
+        == B.RUBIX_ERR_NULL
+    assert g(P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, FAKE, FAKE, None, FAKE, FAKE, FAKE, 1 << 40, None) \
+        == B.RUBIX_ERR_NULL
+    assert g(P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, FAKE, FAKE, FAKE, FAKE, FAKE, FAKE, 64, None) \
+        == B.RUBIX_ERR_WORKSPACE
+    k = C.c_void_p()
+    assert lib.rubix_get_sort_artifacts(0x20000, C.byref(k), C.byref(k), C.byref(k)) == B.RUBIX_ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback_without_the_library(monkeypatch):
+    monkeypatch.setattr(B, "_lib", None)
+    monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/librubix_b200.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        B.load()
