@@ -2,6 +2,15 @@
 // ("Gaussian PSF and LSF").
 // 'same' output, zero padding, taps point-sampled and normalised to 1 (host, fp64 -> fp32).
 // The PSF kernel g (x) g factorises exactly, so two 1-D passes equal the size x size 2-D kernel.
+//
+// Fast path (psf_size <= 15, lsf_size <= 9, even n_channels): two "marching" kernels.  A thread
+// owns one channel pair of one line and walks along the stencil axis with a ring of 15 partial
+// sums in registers: every input is read exactly once (8-byte loads, 256 B contiguous per warp,
+// five steps prefetched), every output written exactly once, no shared memory.
+//   pass 1  along y, with the LSF fused in: the 9 channel taps come from the neighbouring lanes
+//           by warp shuffle (a warp covers 56 output channels plus 2 halo pairs on each side)
+//   pass 2  along x
+// Anything else (larger stencils, odd channel counts) takes the generic one-axis kernel.
 #include <math.h>
 
 #include "common.cuh"
@@ -21,55 +30,143 @@ void make_taps(int size, float sigma, Taps *t)
     for (int i = 0; i < size; ++i) t->w[i] = (float)(w[i] / sum);
 }
 
-// One 1-D stencil pass along an axis with element stride `stride` and extent `len`.
-// Voxels are enumerated channel-fastest, so a warp always touches contiguous addresses.
-template <int VEC>
+// ------------------------------------------------------------------------------------------
+// generic fallback: one 1-D stencil pass along an axis with element stride `stride`
+// ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_stencil_axis(const float *__restrict__ in, float *__restrict__ out, int64_t n_vec, int64_t stride,
+k_stencil_axis(const float *__restrict__ in, float *__restrict__ out, int64_t n_vox, int64_t stride,
                int32_t len, const __grid_constant__ Taps T)
 {
     const int h = (T.size - 1) / 2;
-    for (int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; v < n_vec;
-         v += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t e = v * VEC;                        // first element of this thread's vector
-        const int32_t pos = (int32_t)((e / stride) % len);  // coordinate along the stencil axis
-        float acc[VEC];
-#pragma unroll
-        for (int q = 0; q < VEC; ++q) acc[q] = 0.0f;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_vox;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t pos = (int32_t)((e / stride) % len);
+        float acc = 0.0f;
         for (int d = -h; d <= h; ++d) {
             const int32_t pp = pos + d;
             if (pp < 0 || pp >= len) continue;
-            const float w = T.w[d + h];
-            const float *src = in + e + (int64_t)d * stride;
-            if (VEC == 4) {
-                const float4 x = __ldg(reinterpret_cast<const float4 *>(src));
-                acc[0] = fmaf(w, x.x, acc[0]);
-                acc[1] = fmaf(w, x.y, acc[1]);
-                acc[2] = fmaf(w, x.z, acc[2]);
-                acc[3] = fmaf(w, x.w, acc[3]);
-            } else {
-                acc[0] = fmaf(w, __ldg(src), acc[0]);
-            }
+            acc = fmaf(T.w[d + h], __ldg(in + e + (int64_t)d * stride), acc);
         }
-        if (VEC == 4) *reinterpret_cast<float4 *>(out + e) = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        else out[e] = acc[0];
+        out[e] = acc;
     }
 }
 
-static cudaError_t stencil(const float *in, float *out, int64_t n_vox, int64_t stride, int32_t len,
-                           const Taps &T, bool vec4, cudaStream_t st)
+static cudaError_t stencil_generic(const float *in, float *out, int64_t n_vox, int64_t stride, int32_t len,
+                                   const Taps &T, cudaStream_t st)
 {
-    // vectorised only across the channel axis and only when the stencil axis is not the channel
-    if (vec4) {
-        const int64_t n_vec = n_vox / 4;
-        const unsigned grid = (unsigned)((n_vec + 255) / 256 < 148 * 64 ? (n_vec + 255) / 256 : 148 * 64);
-        k_stencil_axis<4><<<grid ? grid : 1, 256, 0, st>>>(in, out, n_vec, stride, len, T);
-    } else {
-        const unsigned grid = (unsigned)((n_vox + 255) / 256 < 148 * 64 ? (n_vox + 255) / 256 : 148 * 64);
-        k_stencil_axis<1><<<grid ? grid : 1, 256, 0, st>>>(in, out, n_vox, stride, len, T);
-    }
+    const int64_t blocks = (n_vox + 255) / 256;
+    const unsigned grid = (unsigned)(blocks < 148 * 64 ? blocks : 148 * 64);
+    k_stencil_axis<<<grid ? grid : 1, 256, 0, st>>>(in, out, n_vox, stride, len, T);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
+}
+
+// ------------------------------------------------------------------------------------------
+// marching kernels
+// ------------------------------------------------------------------------------------------
+struct MarchParams {
+    const float *in;
+    float *out;
+    int64_t line_stride, step_stride;   // elements
+    int32_t n_lines, n_steps, n_c, cblocks;
+    float g[15];                        // stencil along the marching axis, zero padded, centred
+    float h[9];                         // LSF taps along the channel, zero padded, centred
+};
+
+__device__ __forceinline__ float2 shfl_up2(float2 v, int d)
+{
+    return make_float2(__shfl_up_sync(0xffffffffu, v.x, d), __shfl_up_sync(0xffffffffu, v.y, d));
+}
+__device__ __forceinline__ float2 shfl_down2(float2 v, int d)
+{
+    return make_float2(__shfl_down_sync(0xffffffffu, v.x, d), __shfl_down_sync(0xffffffffu, v.y, d));
+}
+
+// 9-tap stencil along the channel for the pair (c, c+1) held by this lane; lanes hold
+// consecutive pairs, so offsets -4..+5 live in lanes -2..+2
+__device__ __forceinline__ float2 lsf_pair(float2 v, const float *h)
+{
+    const float2 m2 = shfl_up2(v, 2), m1 = shfl_up2(v, 1), p1 = shfl_down2(v, 1), p2 = shfl_down2(v, 2);
+    float2 o;
+    o.x = h[0] * m2.x;
+    o.x = fmaf(h[1], m2.y, o.x); o.x = fmaf(h[2], m1.x, o.x); o.x = fmaf(h[3], m1.y, o.x);
+    o.x = fmaf(h[4], v.x, o.x);  o.x = fmaf(h[5], v.y, o.x);  o.x = fmaf(h[6], p1.x, o.x);
+    o.x = fmaf(h[7], p1.y, o.x); o.x = fmaf(h[8], p2.x, o.x);
+    o.y = h[0] * m2.y;
+    o.y = fmaf(h[1], m1.x, o.y); o.y = fmaf(h[2], m1.y, o.y); o.y = fmaf(h[3], v.x, o.y);
+    o.y = fmaf(h[4], v.y, o.y);  o.y = fmaf(h[5], p1.x, o.y); o.y = fmaf(h[6], p1.y, o.y);
+    o.y = fmaf(h[7], p2.x, o.y); o.y = fmaf(h[8], p2.y, o.y);
+    return o;
+}
+
+template <bool LSF>
+__global__ void __launch_bounds__(256)
+k_march(const __grid_constant__ MarchParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * 256 + threadIdx.x) >> 5;
+    const int line = (int)(gw / P.cblocks), cblock = (int)(gw % P.cblocks);
+    if (line >= P.n_lines) return;
+    const int c = LSF ? cblock * 56 + 2 * (lane - 2) : cblock * 64 + 2 * lane;
+    const bool c_ok = c >= 0 && c + 1 < P.n_c;
+    const bool st_ok = c_ok && (!LSF || (lane >= 2 && lane < 30));
+    const size_t off = (size_t)line * P.line_stride + (size_t)(c_ok ? c : 0);
+    const float *src = P.in + off;
+    float *dst = P.out + off;
+    auto load = [&](int s) -> float2 {
+        if (c_ok && s < P.n_steps) return __ldcs(reinterpret_cast<const float2 *>(src + (size_t)s * P.step_stride));
+        return make_float2(0.0f, 0.0f);
+    };
+    float2 acc[15], pf[5];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) acc[i] = make_float2(0.0f, 0.0f);
+#pragma unroll
+    for (int i = 0; i < 5; ++i) pf[i] = load(i);
+    for (int s0 = 0; s0 < P.n_steps + 7; s0 += 15) {
+#pragma unroll
+        for (int u = 0; u < 15; ++u) {
+            const int s = s0 + u;
+            float2 v = pf[u % 5];
+            pf[u % 5] = load(s + 5);
+            if (LSF) v = lsf_pair(v, P.h);
+#pragma unroll
+            for (int d = -7; d <= 7; ++d) {
+                const int slot = (u - d + 15) % 15;           // output s - d
+                acc[slot].x = fmaf(P.g[d + 7], v.x, acc[slot].x);
+                acc[slot].y = fmaf(P.g[d + 7], v.y, acc[slot].y);
+            }
+            const int o = s - 7, so = (u + 8) % 15;           // output o is complete
+            if (st_ok && o >= 0 && o < P.n_steps)
+                __stcs(reinterpret_cast<float2 *>(dst + (size_t)o * P.step_stride), acc[so]);
+            acc[so] = make_float2(0.0f, 0.0f);
+        }
+    }
+}
+
+// LSF alone (PSF off): one pair per thread, same shuffle stencil
+__global__ void __launch_bounds__(256)
+k_lsf_rows(const __grid_constant__ MarchParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * 256 + threadIdx.x) >> 5;
+    const int64_t row = gw / P.cblocks;
+    const int cblock = (int)(gw % P.cblocks);
+    if (row >= P.n_lines) return;
+    const int c = cblock * 56 + 2 * (lane - 2);
+    const bool c_ok = c >= 0 && c + 1 < P.n_c;
+    const size_t off = (size_t)row * P.n_c + (size_t)(c_ok ? c : 0);
+    float2 v = make_float2(0.0f, 0.0f);
+    if (c_ok) v = __ldcs(reinterpret_cast<const float2 *>(P.in + off));
+    v = lsf_pair(v, P.h);
+    if (c_ok && lane >= 2 && lane < 30) __stcs(reinterpret_cast<float2 *>(P.out + off), v);
+}
+
+static void centre_taps(const Taps &t, int width, float *dst)
+{
+    for (int i = 0; i < width; ++i) dst[i] = 0.0f;
+    if (t.size <= 0) { dst[width / 2] = 1.0f; return; }
+    const int shift = (width - t.size) / 2;
+    for (int i = 0; i < t.size; ++i) dst[shift + i] = t.w[i];
 }
 
 cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp,
@@ -81,25 +178,63 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     Taps lsf, psf;
     make_taps(tel->lsf_size, tel->lsf_sigma, &lsf);
     make_taps(tel->psf_size, tel->psf_sigma, &psf);
-    const bool v4 = (n_c % 4 == 0) && (((uintptr_t)in & 15u) == 0) && (((uintptr_t)out & 15u) == 0) &&
-                    (((uintptr_t)tmp & 15u) == 0);
+    if (lsf.size <= 0 && psf.size <= 0)
+        return cudaMemcpyAsync(out, in, (size_t)n_vox * 4, cudaMemcpyDeviceToDevice, st);
+
+    const bool aligned = (n_c % 2 == 0) && (((uintptr_t)in & 7u) == 0) && (((uintptr_t)out & 7u) == 0) &&
+                         (tmp == nullptr || ((uintptr_t)tmp & 7u) == 0);
+    const bool fast = aligned && psf.size <= 15 && lsf.size <= 9;
     cudaError_t e;
-    if (lsf.size <= 0 && psf.size <= 0) {
-        e = cudaMemcpyAsync(out, in, (size_t)n_vox * 4, cudaMemcpyDeviceToDevice, st);
-        return e;
+    if (!fast) {
+        const float *src = in;
+        if (lsf.size > 0) {
+            if ((e = stencil_generic(src, out, n_vox, 1, n_c, lsf, st)) != cudaSuccess) return e;
+            src = out;
+        }
+        if (psf.size > 0) {
+            if ((e = stencil_generic(src, tmp, n_vox, n_c, n_y, psf, st)) != cudaSuccess) return e;
+            if ((e = stencil_generic(tmp, out, n_vox, (int64_t)n_c * n_y, n_x, psf, st)) != cudaSuccess) return e;
+        }
+        return cudaSuccess;
     }
-    const float *src = in;
+
+    MarchParams P;
+    P.n_c = n_c;
+    centre_taps(psf, 15, P.g);
+    centre_taps(lsf, 9, P.h);
+    if (psf.size <= 0) {                                   // LSF only
+        P.in = in; P.out = out;
+        P.n_lines = n_x * n_y; P.n_steps = 1; P.line_stride = n_c; P.step_stride = 0;
+        P.cblocks = (n_c + 55) / 56;
+        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
+        k_lsf_rows<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
+        RUBIX_LAUNCH_CHECK();
+        return cudaSuccess;
+    }
+    // pass 1: along y (lines = x), LSF fused when on
+    P.in = in; P.out = tmp;
+    P.n_lines = n_x; P.n_steps = n_y;
+    P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
     if (lsf.size > 0) {
-        e = stencil(src, out, n_vox, 1, n_c, lsf, false, st);          // along the channel
-        if (e != cudaSuccess) return e;
-        src = out;
+        P.cblocks = (n_c + 55) / 56;
+        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
+        k_march<true><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
+    } else {
+        P.cblocks = (n_c + 63) / 64;
+        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
+        k_march<false><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
     }
-    if (psf.size > 0) {
-        e = stencil(src, tmp, n_vox, n_c, n_y, psf, v4, st);           // along y
-        if (e != cudaSuccess) return e;
-        e = stencil(tmp, out, n_vox, (int64_t)n_c * n_y, n_x, psf, v4, st);   // along x
-        if (e != cudaSuccess) return e;
+    RUBIX_LAUNCH_CHECK();
+    // pass 2: along x (lines = y)
+    P.in = tmp; P.out = out;
+    P.n_lines = n_y; P.n_steps = n_x;
+    P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
+    P.cblocks = (n_c + 63) / 64;
+    {
+        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
+        k_march<false><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
     }
+    RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }
 

@@ -164,9 +164,11 @@ k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s
     seg_off[s] = (int32_t)lo;
 }
 
-// Single CTA: three exclusive scans over the spaxels in one sweep.
+// Single CTA: three exclusive scans over the spaxels in one sweep, kScanItems spaxels per thread.
 //   unit_off: max(1, chunks(s))     part_off: chunks(s) if > 1 else 0     multi index: chunks(s) > 1
 // totals = { n_units, n_part_rows, n_multi }
+constexpr int kScanItems = 8;
+
 __global__ void __launch_bounds__(1024)
 k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restrict__ unit_off,
              int32_t *__restrict__ part_off, int32_t *__restrict__ multi_list,
@@ -177,20 +179,28 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restri
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x < 3) carry[threadIdx.x] = 0;
     __syncthreads();
-    for (int base = 0; base < n_s; base += 1024) {
-        const int s = base + threadIdx.x;
-        int32_t v[3] = {0, 0, 0};
-        if (s < n_s) {
-            const int32_t cnt = seg_off[s + 1] - seg_off[s];
-            const int32_t chunks = (cnt + kChunk - 1) / kChunk;
-            v[0] = chunks > 1 ? chunks : 1;
-            v[1] = chunks > 1 ? chunks : 0;
-            v[2] = chunks > 1 ? 1 : 0;
+    for (int base = 0; base < n_s; base += 1024 * kScanItems) {
+        const int s0 = base + threadIdx.x * kScanItems;
+        int32_t chunks[kScanItems];
+        int32_t tot[3] = {0, 0, 0};
+        int32_t prev = s0 <= n_s ? seg_off[s0] : 0;
+#pragma unroll
+        for (int i = 0; i < kScanItems; ++i) {
+            const int s = s0 + i;
+            chunks[i] = -1;
+            if (s < n_s) {
+                const int32_t next = seg_off[s + 1];
+                chunks[i] = (next - prev + kChunk - 1) / kChunk;
+                prev = next;
+                tot[0] += chunks[i] > 1 ? chunks[i] : 1;
+                tot[1] += chunks[i] > 1 ? chunks[i] : 0;
+                tot[2] += chunks[i] > 1 ? 1 : 0;
+            }
         }
         int32_t inc[3];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
-            inc[q] = v[q];
+            inc[q] = tot[q];
             for (int o = 1; o < 32; o <<= 1) {
                 const int32_t t = __shfl_up_sync(0xffffffffu, inc[q], o);
                 if (lane >= o) inc[q] += t;
@@ -203,17 +213,25 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restri
         for (int q = 0; q < 3; ++q) {
             int32_t wpre = 0;
             for (int w = 0; w < warp; ++w) wpre += wsum[q][w];
-            ex[q] = carry[q] + wpre + inc[q] - v[q];
+            ex[q] = carry[q] + wpre + inc[q] - tot[q];
         }
-        if (s < n_s) {
-            unit_off[s] = ex[0];
-            part_off[s] = ex[1];
-            if (v[2]) multi_list[ex[2]] = s;
+        int32_t run[3] = {ex[0], ex[1], ex[2]};
+#pragma unroll
+        for (int i = 0; i < kScanItems; ++i) {
+            if (chunks[i] >= 0) {
+                const int s = s0 + i;
+                unit_off[s] = run[0];
+                part_off[s] = run[1];
+                if (chunks[i] > 1) multi_list[run[2]] = s;
+                run[0] += chunks[i] > 1 ? chunks[i] : 1;
+                run[1] += chunks[i] > 1 ? chunks[i] : 0;
+                run[2] += chunks[i] > 1 ? 1 : 0;
+            }
         }
         __syncthreads();
         if (threadIdx.x == 1023) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) carry[q] = ex[q] + v[q];
+            for (int q = 0; q < 3; ++q) carry[q] = run[q];
         }
         __syncthreads();
     }

@@ -5,12 +5,15 @@
 // CTA (256 threads) per unit; thread t owns channels k0 + t + 256 i (i < CPT) and keeps their sums
 // in registers, so a spaxel's spectrum is reduced without any atomic.  Per particle:
 //   blend    the four corner templates are read once over the particle's rest-wavelength window
-//            (16-byte loads, coalesced), blended with the mass-scaled bilinear weights and stored
-//            in shared memory as interval entries  (S_j - D_j, D_j),  D_j = S_{j+1} - S_j ;
+//            (8-byte loads, 256 B contiguous per warp instruction), blended with the mass-scaled
+//            bilinear weights and stored in shared memory as interval entries
+//            (S_j - D_j, D_j),  D_j = S_{j+1} - S_j   (S_{j+1} comes from the next lane by shuffle);
 //   resample channel k reads ONE 8-byte entry: value = (S_j - D_j) + f1 * D_j with f1 = 1 + frac(x_k),
 //            x_k from exact integer arithmetic (32-bit 12.20 local fixed point).
-// The table is double buffered: the blend of particle p+1 overlaps the resampling of particle p
-// with one __syncthreads per particle.
+// The table is double buffered and the loop is software pipelined: the template loads of particle
+// p+1 are issued, then particle p is resampled while they fly, then p+1 is blended (each further
+// pass of loads is issued before the previous pass is consumed); one __syncthreads per particle.
+// The unit's records are staged in shared memory once.
 // Single-chunk spaxels write their cube row directly (each voxel exactly once, coalesced);
 // spaxels with more particles write partial rows that k_reduce_partials sums in fixed order.
 #include "common.cuh"
@@ -27,14 +30,28 @@ struct AccumParams {
     int32_t n_lambda, n_z, n_c, n_tiles, wcap;
 };
 
-__device__ __forceinline__ float4 ld4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+constexpr int kWarpSpan = 126;                       // table entries produced per warp per pass
+constexpr int kPassSpan = kWarpSpan * (kAccThreads / 32);
 
-template <int CPT, bool VEC4>
-__global__ void __launch_bounds__(kAccThreads)
+__device__ __forceinline__ float2 ld2(const float *p) { return __ldg(reinterpret_cast<const float2 *>(p)); }
+
+struct Win {                 // one particle's window in one channel tile
+    const float *T;          // corner (i, j) template row
+    int64_t base;            // x(k0) - j0 in 36.28 fixed point
+    uint32_t b;              // step per channel, 4.28
+    int32_t ka, kb;          // channels of this tile inside the SSP coverage (ka > kb: none)
+    int32_t j0, nw;          // first SSP sample of the window (multiple of 4), entries needed
+    float w0, w1, w2, w3;
+};
+
+struct LoadSet { float2 c[4][2]; };                  // 4 corners x 2 pair blocks
+
+template <int CPT, bool VEC>
+__global__ void __launch_bounds__(kAccThreads, 3)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
-    extern __shared__ __align__(16) float2 tab[];           // [2][wcap] interval entries
-    const int tid = threadIdx.x;
+    extern __shared__ __align__(16) float2 tab[];           // [2][wcap] interval entries, then records
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x % P.n_tiles;
     const int u = blockIdx.x / P.n_tiles;
     if (u >= P.totals[0]) return;
@@ -48,106 +65,147 @@ k_accumulate(const __grid_constant__ AccumParams P)
 #pragma unroll
     for (int i = 0; i < CPT; ++i) acc[i] = 0.0f;
 
-    // per-particle state of the particle being resampled (cur) and being blended (nxt)
-    struct Win { int64_t base; uint32_t b; int32_t ka, kb; };
-    Win cur{0, 0, 1, 0}, nxt{0, 0, 1, 0};
-    const size_t row_a = (size_t)P.n_z * P.n_lambda;        // (i+1, j) - (i, j)
-    const size_t row_z = (size_t)P.n_lambda;                // (i, j+1) - (i, j)
+    if (U.count > 0) {
+        int4 *srec = reinterpret_cast<int4 *>(tab + 2 * (size_t)P.wcap);
+        {
+            const int4 *g = reinterpret_cast<const int4 *>(P.rec + U.start);
+            for (int i = tid; i < U.count * 3; i += kAccThreads) srec[i] = __ldg(g + i);
+        }
+        __syncthreads();
+        const size_t row_a = (size_t)P.n_z * P.n_lambda;    // (i+1, j) - (i, j)
+        const size_t row_z = (size_t)P.n_lambda;            // (i, j+1) - (i, j)
+        const int nlm1 = P.n_lambda - 1, nlm2 = P.n_lambda - 2;
 
-    auto blend = [&](int q, float2 *buf) -> Win {
-        const int4 *rp = reinterpret_cast<const int4 *>(P.rec + U.start + q);
-        const int4 ra = __ldg(rp), rb = __ldg(rp + 1), rc = __ldg(rp + 2);
-        const float w0 = __int_as_float(ra.x), w1 = __int_as_float(ra.y);
-        const float w2 = __int_as_float(ra.z), w3 = __int_as_float(ra.w);
-        const uint32_t b = (uint32_t)rb.y;
-        const int64_t a = (int64_t)(((uint64_t)(uint32_t)rb.w << 32) | (uint32_t)rb.z);
-        Win W;
-        W.b = b;
-        W.ka = max(k0, rc.x);
-        W.kb = min(k_end, rc.y);
-        W.base = 0;
-        if (W.ka > W.kb) return W;                          // nothing of this particle in the tile
-        const int64_t xa = a + (int64_t)b * W.ka, xb = a + (int64_t)b * W.kb;
-        const int j0 = (int)(xa >> kFxFrac) & ~3;
-        const int jb = (int)(xb >> kFxFrac);                // <= n_lambda - 1
-        W.base = a + (int64_t)b * k0 - ((int64_t)j0 << kFxFrac);
-        const float *T = P.flux + rb.x;
-        if (VEC4) {
-            const int nq = min((jb - j0 + 4) >> 2, P.wcap >> 2);
-            for (int qd = tid; qd < nq; qd += kAccThreads) {
-                const int j = j0 + 4 * qd;
-                const float *t = T + j;
-                const float4 c0 = ld4(t), c1 = ld4(t + row_a), c2 = ld4(t + row_z), c3 = ld4(t + row_a + row_z);
-                float s[5];
-                s[0] = fmaf(w3, c3.x, fmaf(w2, c2.x, fmaf(w1, c1.x, w0 * c0.x)));
-                s[1] = fmaf(w3, c3.y, fmaf(w2, c2.y, fmaf(w1, c1.y, w0 * c0.y)));
-                s[2] = fmaf(w3, c3.z, fmaf(w2, c2.z, fmaf(w1, c1.z, w0 * c0.z)));
-                s[3] = fmaf(w3, c3.w, fmaf(w2, c2.w, fmaf(w1, c1.w, w0 * c0.w)));
-                if (j + 4 < P.n_lambda) {
-                    s[4] = fmaf(w3, __ldg(t + row_a + row_z + 4),
-                                fmaf(w2, __ldg(t + row_z + 4), fmaf(w1, __ldg(t + row_a + 4), w0 * __ldg(t + 4))));
-                } else {
-                    s[4] = s[3];                            // interval N_l-1: flat, only f = 0 reaches it
-                }
-                float4 e0, e1;
-                e0.y = s[1] - s[0]; e0.x = s[0] - e0.y;
-                e0.w = s[2] - s[1]; e0.z = s[1] - e0.w;
-                e1.y = s[3] - s[2]; e1.x = s[2] - e1.y;
-                e1.w = s[4] - s[3]; e1.z = s[3] - e1.w;
-                float4 *dst = reinterpret_cast<float4 *>(buf + 4 * qd);
-                dst[0] = e0;
-                dst[1] = e1;
+        auto window = [&](int q) -> Win {
+            const int4 ra = srec[3 * q], rb = srec[3 * q + 1], rc = srec[3 * q + 2];
+            Win W;
+            W.w0 = __int_as_float(ra.x); W.w1 = __int_as_float(ra.y);
+            W.w2 = __int_as_float(ra.z); W.w3 = __int_as_float(ra.w);
+            W.b = (uint32_t)rb.y;
+            const int64_t a = (int64_t)(((uint64_t)(uint32_t)rb.w << 32) | (uint32_t)rb.z);
+            W.ka = max(k0, rc.x);
+            W.kb = min(k_end, rc.y);
+            W.T = P.flux + rb.x;
+            W.base = 0; W.j0 = 0; W.nw = 0;
+            if (W.ka <= W.kb) {
+                const int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * W.kb;
+                W.j0 = (int)(xa >> kFxFrac) & ~3;
+                W.nw = min((int)(xb >> kFxFrac) - W.j0 + 1, P.wcap);    // last entry <= n_lambda-1
+                W.base = a + (int64_t)W.b * k0 - ((int64_t)W.j0 << kFxFrac);
             }
-        } else {
-            const int nw = min(jb - j0 + 1, P.wcap);
-            for (int e = tid; e < nw; e += kAccThreads) {
-                const int j = j0 + e;
-                const int jn = min(j + 1, P.n_lambda - 1);
-                const float *t = T;
-                const float s0 = fmaf(w3, __ldg(t + row_a + row_z + j),
-                                      fmaf(w2, __ldg(t + row_z + j), fmaf(w1, __ldg(t + row_a + j), w0 * __ldg(t + j))));
-                const float s1 = fmaf(w3, __ldg(t + row_a + row_z + jn),
-                                      fmaf(w2, __ldg(t + row_z + jn), fmaf(w1, __ldg(t + row_a + jn), w0 * __ldg(t + jn))));
+            return W;
+        };
+
+        // ---- vector path: warp `warp`, pass starting at entry sb, lane handles entry pairs
+        //      sb + 2 lane (+0, +64); lane 31 of the second block only feeds lane 30's neighbour
+        auto issue = [&](LoadSet &L, const Win &W, int sb) {
+            const int j1 = min(W.j0 + sb + 2 * lane, nlm2), j2 = min(W.j0 + sb + 64 + 2 * lane, nlm2);
+            const float *t = W.T;
+            L.c[0][0] = ld2(t + j1);                 L.c[0][1] = ld2(t + j2);
+            L.c[1][0] = ld2(t + row_a + j1);         L.c[1][1] = ld2(t + row_a + j2);
+            L.c[2][0] = ld2(t + row_z + j1);         L.c[2][1] = ld2(t + row_z + j2);
+            L.c[3][0] = ld2(t + row_a + row_z + j1); L.c[3][1] = ld2(t + row_a + row_z + j2);
+        };
+        auto consume = [&](const LoadSet &L, const Win &W, int sb, float2 *buf) {
+            const int p1 = sb + 2 * lane, p2 = p1 + 64;
+            const float s10 = fmaf(W.w3, L.c[3][0].x, fmaf(W.w2, L.c[2][0].x, fmaf(W.w1, L.c[1][0].x, W.w0 * L.c[0][0].x)));
+            const float s11 = fmaf(W.w3, L.c[3][0].y, fmaf(W.w2, L.c[2][0].y, fmaf(W.w1, L.c[1][0].y, W.w0 * L.c[0][0].y)));
+            const float s20 = fmaf(W.w3, L.c[3][1].x, fmaf(W.w2, L.c[2][1].x, fmaf(W.w1, L.c[1][1].x, W.w0 * L.c[0][1].x)));
+            const float s21 = fmaf(W.w3, L.c[3][1].y, fmaf(W.w2, L.c[2][1].y, fmaf(W.w1, L.c[1][1].y, W.w0 * L.c[0][1].y)));
+            float nb1 = __shfl_sync(0xffffffffu, lane == 0 ? s20 : s10, (lane + 1) & 31);
+            float nb2 = __shfl_down_sync(0xffffffffu, s20, 1);
+            if (W.j0 + p1 + 2 > nlm1) nb1 = s11;            // interval N_l-1 is flat (only f = 0 reaches it)
+            if (W.j0 + p2 + 2 > nlm1) nb2 = s21;
+            float4 e1, e2;
+            e1.y = s11 - s10; e1.x = s10 - e1.y; e1.w = nb1 - s11; e1.z = s11 - e1.w;
+            e2.y = s21 - s20; e2.x = s20 - e2.y; e2.w = nb2 - s21; e2.z = s21 - e2.w;
+            if (p1 < W.nw) *reinterpret_cast<float4 *>(buf + p1) = e1;
+            if (lane < 31 && p2 < W.nw) *reinterpret_cast<float4 *>(buf + p2) = e2;
+        };
+        // ---- scalar path (row length odd or misaligned flux): plain per-entry blend
+        auto blend_scalar = [&](const Win &W, float2 *buf) {
+            for (int e = tid; e < W.nw; e += kAccThreads) {
+                const int j = W.j0 + e, jn = min(j + 1, nlm1);
+                const float *t = W.T;
+                const float s0 = fmaf(W.w3, __ldg(t + row_a + row_z + j),
+                                      fmaf(W.w2, __ldg(t + row_z + j), fmaf(W.w1, __ldg(t + row_a + j), W.w0 * __ldg(t + j))));
+                const float s1 = fmaf(W.w3, __ldg(t + row_a + row_z + jn),
+                                      fmaf(W.w2, __ldg(t + row_z + jn), fmaf(W.w1, __ldg(t + row_a + jn), W.w0 * __ldg(t + jn))));
                 const float d = s1 - s0;
                 buf[e] = make_float2(s0 - d, d);
             }
-        }
-        return W;
-    };
-
-    auto resample = [&](const Win &W, const float2 *buf) {
-        if (W.ka > W.kb) return;
-        const char *bytes = reinterpret_cast<const char *>(buf);
-        // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
-        const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
-        if (W.ka == k0 && W.kb == k_end) {                  // whole tile inside the SSP coverage
-#pragma unroll
-            for (int i = 0; i < CPT; ++i) {
-                const uint32_t x = x0 + (uint32_t)i * W.b;
-                const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & 0x7FF8u));
-                const float f1 = __uint_as_float(((x << 3) & 0x7FFFF8u) | 0x3F800000u);
-                acc[i] += fmaf(f1, e.y, e.x);
+        };
+        // all passes after the first one, software pipelined (A holds the pass being consumed)
+        auto blend_rest = [&](LoadSet &A, const Win &W, float2 *buf) {
+            LoadSet B;
+            int sb = warp * kWarpSpan;
+            while (true) {
+                int nb = sb + kPassSpan;
+                bool more = nb < W.nw;
+                if (more) issue(B, W, nb);
+                consume(A, W, sb, buf);
+                if (!more) break;
+                sb = nb; nb += kPassSpan; more = nb < W.nw;
+                if (more) issue(A, W, nb);
+                consume(B, W, sb, buf);
+                if (!more) break;
+                sb = nb;
             }
-        } else {
+        };
+
+        auto resample = [&](const Win &W, const float2 *buf) {
+            const char *bytes = reinterpret_cast<const char *>(buf);
+            // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
+            const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
+            if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
 #pragma unroll
-            for (int i = 0; i < CPT; ++i) {
-                const int k = k0 + tid + i * kAccThreads;
-                if (k >= W.ka && k <= W.kb) {
+                for (int i = 0; i < CPT; ++i) {
                     const uint32_t x = x0 + (uint32_t)i * W.b;
                     const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & 0x7FF8u));
                     const float f1 = __uint_as_float(((x << 3) & 0x7FFFF8u) | 0x3F800000u);
                     acc[i] += fmaf(f1, e.y, e.x);
                 }
+            } else {
+#pragma unroll
+                for (int i = 0; i < CPT; ++i) {
+                    const int k = k0 + tid + i * kAccThreads;
+                    if (k >= W.ka && k <= W.kb) {
+                        const uint32_t x = x0 + (uint32_t)i * W.b;
+                        const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & 0x7FF8u));
+                        const float f1 = __uint_as_float(((x << 3) & 0x7FFFF8u) | 0x3F800000u);
+                        acc[i] += fmaf(f1, e.y, e.x);
+                    }
+                }
+            }
+        };
+
+        // prologue: table of particle 0
+        Win cur = window(0);
+        if (cur.ka <= cur.kb) {
+            if (VEC) {
+                LoadSet A;
+                if (warp * kWarpSpan < cur.nw) { issue(A, cur, warp * kWarpSpan); blend_rest(A, cur, tab); }
+            } else {
+                blend_scalar(cur, tab);
             }
         }
-    };
-
-    if (U.count > 0) {
-        cur = blend(0, tab);
         __syncthreads();
         for (int q = 0; q < U.count; ++q) {
-            if (q + 1 < U.count) nxt = blend(q + 1, tab + (size_t)((q + 1) & 1) * P.wcap);
-            resample(cur, tab + (size_t)(q & 1) * P.wcap);
+            float2 *buf_next = tab + (size_t)((q + 1) & 1) * P.wcap;
+            Win nxt;
+            nxt.ka = 1; nxt.kb = 0;
+            LoadSet A;
+            bool blend_next = false;
+            if (q + 1 < U.count) {
+                nxt = window(q + 1);
+                blend_next = (nxt.ka <= nxt.kb) && (!VEC || warp * kWarpSpan < nxt.nw);
+                if (VEC && blend_next) issue(A, nxt, warp * kWarpSpan);     // loads fly during resample
+            }
+            if (cur.ka <= cur.kb) resample(cur, tab + (size_t)(q & 1) * P.wcap);
+            if (blend_next) {
+                if (VEC) blend_rest(A, nxt, buf_next);
+                else blend_scalar(nxt, buf_next);
+            }
             cur = nxt;
             __syncthreads();
         }
@@ -183,10 +241,10 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
 }
 
 template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, bool vec4, unsigned grid, size_t smem, cudaStream_t st)
+static cudaError_t launch_acc(const AccumParams &P, bool vec, unsigned grid, size_t smem, cudaStream_t st)
 {
     cudaError_t e;
-    if (vec4) {
+    if (vec) {
         e = cudaFuncSetAttribute(k_accumulate<CPT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         k_accumulate<CPT, true><<<grid, kAccThreads, smem, st>>>(P);
@@ -238,19 +296,19 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const int tc = cpt * kAccThreads;
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
-    const bool vec4 = (in.ssp->n_lambda % 4 == 0) && (((uintptr_t)in.ssp->flux & 15u) == 0);
-    const size_t smem = (size_t)2 * wcap * sizeof(float2);
+    const bool vec = (in.ssp->n_lambda % 2 == 0) && (((uintptr_t)in.ssp->flux & 7u) == 0);
+    const size_t smem = (size_t)2 * wcap * sizeof(float2) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
     {
-    StageTimer t(1, st);
-    switch (cpt) {
-        case 15: e = launch_acc<15>(P, vec4, grid, smem, st); break;
-        case 8: e = launch_acc<8>(P, vec4, grid, smem, st); break;
-        case 4: e = launch_acc<4>(P, vec4, grid, smem, st); break;
-        case 2: e = launch_acc<2>(P, vec4, grid, smem, st); break;
-        default: e = launch_acc<1>(P, vec4, grid, smem, st); break;
-    }
+        StageTimer t(1, st);
+        switch (cpt) {
+            case 15: e = launch_acc<15>(P, vec, grid, smem, st); break;
+            case 8: e = launch_acc<8>(P, vec, grid, smem, st); break;
+            case 4: e = launch_acc<4>(P, vec, grid, smem, st); break;
+            case 2: e = launch_acc<2>(P, vec, grid, smem, st); break;
+            default: e = launch_acc<1>(P, vec, grid, smem, st); break;
+        }
     }
     if (e != cudaSuccess) return e;
     StageTimer t2(2, st);
