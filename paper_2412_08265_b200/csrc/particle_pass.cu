@@ -329,7 +329,12 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     if (k_lo > P.n_c) k_lo = P.n_c;
     r.k_lo = (int32_t)k_lo;
     r.k_hi = (int32_t)k_hi;
-    r.pad[0] = r.pad[1] = 0;
+    r.j0 = 0;
+    r.nw = 0;
+    if (k_lo <= k_hi) {
+        r.j0 = (int32_t)((a_fx + (int64_t)b_fx * k_lo) >> kFxFrac) & ~3;
+        r.nw = (int32_t)((a_fx + (int64_t)b_fx * k_hi) >> kFxFrac) - r.j0 + 1;
+    }
     rec[i] = r;
 }
 
@@ -343,7 +348,7 @@ static int bits_for(int32_t max_value)
     return b;
 }
 
-Layout make_layout(int64_t n, int32_t n_s, int32_t n_c)
+Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, size_t flux_elems)
 {
     Layout L{};
     L.n = n;
@@ -382,6 +387,8 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c)
     L.off_units = take((size_t)L.max_units * sizeof(Unit));
     L.off_rec = take(nn * sizeof(Rec));
     L.off_partials = take((size_t)L.max_part_rows * (size_t)n_c * 4);
+    L.flux_elems = flux_elems;
+    L.off_flux = take((flux_elems + kFluxPad) * 4);
     L.bytes_total = off;
     return L;
 }

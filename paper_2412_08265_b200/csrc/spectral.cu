@@ -5,8 +5,9 @@
 // CTA (256 threads) per unit; thread t owns channels k0 + t + 256 i (i < CPT) and keeps their sums
 // in registers, so a spaxel's spectrum is reduced without any atomic.  Per particle:
 //   blend    the four corner templates are read once over the particle's rest-wavelength window
-//            (8-byte loads, 256 B contiguous per warp instruction), blended with the mass-scaled
-//            bilinear weights and stored in shared memory as interval entries
+//            (8-byte loads, 256 B contiguous per warp instruction, from a zero-padded workspace
+//            copy of the grid so no load needs clamping), blended with the mass-scaled bilinear
+//            weights (packed fp32x2 FMAs) and stored in shared memory as interval entries
 //            (S_j - D_j, D_j),  D_j = S_{j+1} - S_j   (S_{j+1} comes from the next lane by shuffle);
 //   resample channel k reads ONE 8-byte entry: value = (S_j - D_j) + f1 * D_j with f1 = 1 + frac(x_k),
 //            x_k from exact integer arithmetic (32-bit 12.20 local fixed point).
@@ -33,27 +34,64 @@ struct AccumParams {
 constexpr int kWarpSpan = 126;                       // table entries produced per warp per pass
 constexpr int kPassSpan = kWarpSpan * (kAccThreads / 32);
 
-__device__ __forceinline__ float2 ld2(const float *p) { return __ldg(reinterpret_cast<const float2 *>(p)); }
+// ---- packed fp32x2 arithmetic (sm_100+): one issue slot, two FMAs ------------------------------
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long v)
+{
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long fmul2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// (a & b) | c in one LOP3 (b, c stay in registers)
+__device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long ld2u(const float *p)
+{
+    unsigned long long v;
+    asm volatile("ld.global.nc.b64 %0, [%1];" : "=l"(v) : "l"(p));
+    return v;
+}
 
 struct Win {                 // one particle's window in one channel tile
-    const float *T;          // corner (i, j) template row
     int64_t base;            // x(k0) - j0 in 36.28 fixed point
     uint32_t b;              // step per channel, 4.28
     int32_t ka, kb;          // channels of this tile inside the SSP coverage (ka > kb: none)
-    int32_t j0, nw;          // first SSP sample of the window (multiple of 4), entries needed
+    int32_t first, nw;       // flux index of (corner (i,j), sample j0); entries needed
     float w0, w1, w2, w3;
 };
 
-struct LoadSet { float2 c[4][2]; };                  // 4 corners x 2 pair blocks
+struct LoadSet { unsigned long long c[4][2]; };      // 4 corners x 2 pair blocks, packed pairs
 
-template <int CPT, bool VEC>
+// SINGLE: the whole spectrum is one tile (n_tiles == 1): window (j0, nw) comes from the record.
+template <int CPT, bool VEC, bool SINGLE>
 __global__ void __launch_bounds__(kAccThreads, 3)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
     extern __shared__ __align__(16) float2 tab[];           // [2][wcap] interval entries, then records
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = blockIdx.x % P.n_tiles;
-    const int u = blockIdx.x / P.n_tiles;
+    const int tile = SINGLE ? 0 : blockIdx.x % P.n_tiles;
+    const int u = SINGLE ? blockIdx.x : blockIdx.x / P.n_tiles;
     if (u >= P.totals[0]) return;
     const Unit U = P.units[u];
     constexpr int TC = CPT * kAccThreads;
@@ -72,9 +110,9 @@ k_accumulate(const __grid_constant__ AccumParams P)
             for (int i = tid; i < U.count * 3; i += kAccThreads) srec[i] = __ldg(g + i);
         }
         __syncthreads();
-        const size_t row_a = (size_t)P.n_z * P.n_lambda;    // (i+1, j) - (i, j)
-        const size_t row_z = (size_t)P.n_lambda;            // (i, j+1) - (i, j)
-        const int nlm1 = P.n_lambda - 1, nlm2 = P.n_lambda - 2;
+        const int row_a = P.n_z * P.n_lambda;               // (i+1, j) - (i, j)
+        const int row_z = P.n_lambda;                       // (i, j+1) - (i, j)
+        const int nlm1 = P.n_lambda - 1;
 
         auto window = [&](int q) -> Win {
             const int4 ra = srec[3 * q], rb = srec[3 * q + 1], rc = srec[3 * q + 2];
@@ -83,59 +121,66 @@ k_accumulate(const __grid_constant__ AccumParams P)
             W.w2 = __int_as_float(ra.z); W.w3 = __int_as_float(ra.w);
             W.b = (uint32_t)rb.y;
             const int64_t a = (int64_t)(((uint64_t)(uint32_t)rb.w << 32) | (uint32_t)rb.z);
-            W.ka = max(k0, rc.x);
-            W.kb = min(k_end, rc.y);
-            W.T = P.flux + rb.x;
-            W.base = 0; W.j0 = 0; W.nw = 0;
-            if (W.ka <= W.kb) {
-                const int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * W.kb;
-                W.j0 = (int)(xa >> kFxFrac) & ~3;
-                W.nw = min((int)(xb >> kFxFrac) - W.j0 + 1, P.wcap);    // last entry <= n_lambda-1
-                W.base = a + (int64_t)W.b * k0 - ((int64_t)W.j0 << kFxFrac);
+            int j0;
+            if (SINGLE) {                                   // k0 = 0, k_end = n_c - 1 >= k_hi
+                W.ka = rc.x; W.kb = rc.y;
+                j0 = rc.z; W.nw = min(rc.w, P.wcap);
+            } else {
+                W.ka = max(k0, rc.x);
+                W.kb = min(k_end, rc.y);
+                j0 = 0; W.nw = 0;
+                if (W.ka <= W.kb) {
+                    const int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * W.kb;
+                    j0 = (int)(xa >> kFxFrac) & ~3;
+                    W.nw = min((int)(xb >> kFxFrac) - j0 + 1, P.wcap);  // last entry <= n_lambda-1
+                }
             }
+            W.first = rb.x + j0;
+            W.base = a + (int64_t)W.b * k0 - ((int64_t)j0 << kFxFrac);
             return W;
         };
 
-        // ---- vector path: warp `warp`, pass starting at entry sb, lane handles entry pairs
-        //      sb + 2 lane (+0, +64); lane 31 of the second block only feeds lane 30's neighbour
+        // ---- vector path: warp `warp`, pass starting at entry sb; the lane handles the entry pairs
+        //      sb + 2 lane and sb + 64 + 2 lane; lane 31 of the second block only feeds lane 30's
+        //      neighbour.  P.flux is the padded workspace copy, so reads past a window are harmless.
         auto issue = [&](LoadSet &L, const Win &W, int sb) {
-            const int j1 = min(W.j0 + sb + 2 * lane, nlm2), j2 = min(W.j0 + sb + 64 + 2 * lane, nlm2);
-            const float *t = W.T;
-            L.c[0][0] = ld2(t + j1);                 L.c[0][1] = ld2(t + j2);
-            L.c[1][0] = ld2(t + row_a + j1);         L.c[1][1] = ld2(t + row_a + j2);
-            L.c[2][0] = ld2(t + row_z + j1);         L.c[2][1] = ld2(t + row_z + j2);
-            L.c[3][0] = ld2(t + row_a + row_z + j1); L.c[3][1] = ld2(t + row_a + row_z + j2);
+            const int i0 = W.first + sb + 2 * lane;
+            const float *t0 = P.flux + i0, *t1 = P.flux + (i0 + row_a);
+            const float *t2 = P.flux + (i0 + row_z), *t3 = P.flux + (i0 + row_a + row_z);
+            L.c[0][0] = ld2u(t0); L.c[0][1] = ld2u(t0 + 64);
+            L.c[1][0] = ld2u(t1); L.c[1][1] = ld2u(t1 + 64);
+            L.c[2][0] = ld2u(t2); L.c[2][1] = ld2u(t2 + 64);
+            L.c[3][0] = ld2u(t3); L.c[3][1] = ld2u(t3 + 64);
         };
         auto consume = [&](const LoadSet &L, const Win &W, int sb, float2 *buf) {
             const int p1 = sb + 2 * lane, p2 = p1 + 64;
-            const float s10 = fmaf(W.w3, L.c[3][0].x, fmaf(W.w2, L.c[2][0].x, fmaf(W.w1, L.c[1][0].x, W.w0 * L.c[0][0].x)));
-            const float s11 = fmaf(W.w3, L.c[3][0].y, fmaf(W.w2, L.c[2][0].y, fmaf(W.w1, L.c[1][0].y, W.w0 * L.c[0][0].y)));
-            const float s20 = fmaf(W.w3, L.c[3][1].x, fmaf(W.w2, L.c[2][1].x, fmaf(W.w1, L.c[1][1].x, W.w0 * L.c[0][1].x)));
-            const float s21 = fmaf(W.w3, L.c[3][1].y, fmaf(W.w2, L.c[2][1].y, fmaf(W.w1, L.c[1][1].y, W.w0 * L.c[0][1].y)));
-            float nb1 = __shfl_sync(0xffffffffu, lane == 0 ? s20 : s10, (lane + 1) & 31);
-            float nb2 = __shfl_down_sync(0xffffffffu, s20, 1);
-            if (W.j0 + p1 + 2 > nlm1) nb1 = s11;            // interval N_l-1 is flat (only f = 0 reaches it)
-            if (W.j0 + p2 + 2 > nlm1) nb2 = s21;
+            const unsigned long long w0 = pack2(W.w0, W.w0), w1 = pack2(W.w1, W.w1);
+            const unsigned long long w2 = pack2(W.w2, W.w2), w3 = pack2(W.w3, W.w3);
+            const float2 s1 = unpack2(ffma2(w3, L.c[3][0], ffma2(w2, L.c[2][0], ffma2(w1, L.c[1][0], fmul2(w0, L.c[0][0])))));
+            const float2 s2 = unpack2(ffma2(w3, L.c[3][1], ffma2(w2, L.c[2][1], ffma2(w1, L.c[1][1], fmul2(w0, L.c[0][1])))));
+            // S_{j+2} of each pair from the next lane; the last interval (N_l-1) is only ever
+            // evaluated at f = 0, where (S - D) + D = S whatever D is, so no special case
+            const float nb1 = __shfl_sync(0xffffffffu, lane == 0 ? s2.x : s1.x, (lane + 1) & 31);
+            const float nb2 = __shfl_down_sync(0xffffffffu, s2.x, 1);
             float4 e1, e2;
-            e1.y = s11 - s10; e1.x = s10 - e1.y; e1.w = nb1 - s11; e1.z = s11 - e1.w;
-            e2.y = s21 - s20; e2.x = s20 - e2.y; e2.w = nb2 - s21; e2.z = s21 - e2.w;
+            e1.y = s1.y - s1.x; e1.x = s1.x - e1.y; e1.w = nb1 - s1.y; e1.z = s1.y - e1.w;
+            e2.y = s2.y - s2.x; e2.x = s2.x - e2.y; e2.w = nb2 - s2.y; e2.z = s2.y - e2.w;
             if (p1 < W.nw) *reinterpret_cast<float4 *>(buf + p1) = e1;
             if (lane < 31 && p2 < W.nw) *reinterpret_cast<float4 *>(buf + p2) = e2;
         };
         // ---- scalar path (row length odd or misaligned flux): plain per-entry blend
         auto blend_scalar = [&](const Win &W, float2 *buf) {
             for (int e = tid; e < W.nw; e += kAccThreads) {
-                const int j = W.j0 + e, jn = min(j + 1, nlm1);
-                const float *t = W.T;
-                const float s0 = fmaf(W.w3, __ldg(t + row_a + row_z + j),
-                                      fmaf(W.w2, __ldg(t + row_z + j), fmaf(W.w1, __ldg(t + row_a + j), W.w0 * __ldg(t + j))));
-                const float s1 = fmaf(W.w3, __ldg(t + row_a + row_z + jn),
-                                      fmaf(W.w2, __ldg(t + row_z + jn), fmaf(W.w1, __ldg(t + row_a + jn), W.w0 * __ldg(t + jn))));
+                const float *t = P.flux + W.first + e;
+                const float s0 = fmaf(W.w3, __ldg(t + row_a + row_z),
+                                      fmaf(W.w2, __ldg(t + row_z), fmaf(W.w1, __ldg(t + row_a), W.w0 * __ldg(t))));
+                const float s1 = fmaf(W.w3, __ldg(t + row_a + row_z + 1),
+                                      fmaf(W.w2, __ldg(t + row_z + 1), fmaf(W.w1, __ldg(t + row_a + 1), W.w0 * __ldg(t + 1))));
                 const float d = s1 - s0;
                 buf[e] = make_float2(s0 - d, d);
             }
         };
-        // all passes after the first one, software pipelined (A holds the pass being consumed)
+        // all passes, software pipelined (A holds the pass being consumed, loads already issued)
         auto blend_rest = [&](LoadSet &A, const Win &W, float2 *buf) {
             LoadSet B;
             int sb = warp * kWarpSpan;
@@ -153,28 +198,24 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
         };
 
+        const uint32_t m_addr = 0x7FF8u, m_frac = 0x7FFFF8u, one_bits = 0x3F800000u;
+        auto sample = [&](int i, uint32_t x, const char *bytes) {
+            const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & m_addr));
+            const float f1 = __uint_as_float(and_or(x << 3, m_frac, one_bits));   // 1 + frac(x_k)
+            acc[i] += fmaf(f1, e.y, e.x);                   // (S_j - D_j) + f1 D_j
+        };
         auto resample = [&](const Win &W, const float2 *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
             // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
             const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
 #pragma unroll
-                for (int i = 0; i < CPT; ++i) {
-                    const uint32_t x = x0 + (uint32_t)i * W.b;
-                    const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & 0x7FF8u));
-                    const float f1 = __uint_as_float(((x << 3) & 0x7FFFF8u) | 0x3F800000u);
-                    acc[i] += fmaf(f1, e.y, e.x);
-                }
+                for (int i = 0; i < CPT; ++i) sample(i, x0 + (uint32_t)i * W.b, bytes);
             } else {
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k >= W.ka && k <= W.kb) {
-                        const uint32_t x = x0 + (uint32_t)i * W.b;
-                        const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & 0x7FF8u));
-                        const float f1 = __uint_as_float(((x << 3) & 0x7FFFF8u) | 0x3F800000u);
-                        acc[i] += fmaf(f1, e.y, e.x);
-                    }
+                    if (k >= W.ka && k <= W.kb) sample(i, x0 + (uint32_t)i * W.b, bytes);
                 }
             }
         };
@@ -209,6 +250,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
             cur = nxt;
             __syncthreads();
         }
+        (void)nlm1;
     }
 #pragma unroll
     for (int i = 0; i < CPT; ++i) {
@@ -240,21 +282,22 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
+template <int CPT, bool VEC, bool SINGLE>
+static cudaError_t launch_acc3(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_accumulate<CPT, VEC, SINGLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_accumulate<CPT, VEC, SINGLE><<<grid, kAccThreads, smem, st>>>(P);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
 template <int CPT>
 static cudaError_t launch_acc(const AccumParams &P, bool vec, unsigned grid, size_t smem, cudaStream_t st)
 {
-    cudaError_t e;
-    if (vec) {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_accumulate<CPT, true><<<grid, kAccThreads, smem, st>>>(P);
-    } else {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_accumulate<CPT, false><<<grid, kAccThreads, smem, st>>>(P);
-    }
-    RUBIX_LAUNCH_CHECK();
-    return cudaSuccess;
+    const bool single = P.n_tiles == 1;
+    if (vec) return single ? launch_acc3<CPT, true, true>(P, grid, smem, st) : launch_acc3<CPT, true, false>(P, grid, smem, st);
+    return single ? launch_acc3<CPT, false, true>(P, grid, smem, st) : launch_acc3<CPT, false, false>(P, grid, smem, st);
 }
 
 // Largest CPT in {15, 8, 4, 2, 1} whose table fits the 12.20 format; returns window capacity.
@@ -283,8 +326,15 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     int wcap = 0;
     const int cpt = choose_cpt(L.n_c, b_max, &wcap);
     if (cpt == 0) return cudaErrorInvalidConfiguration;
+    // padded workspace copy of the SSP grid: reads past a window's end (next row or the zero
+    // pad) are harmless, so the blend needs no clamping
+    float *flux_pad = (float *)(ws + L.off_flux);
+    cudaError_t ce = cudaMemcpyAsync(flux_pad, in.ssp->flux, L.flux_elems * 4, cudaMemcpyDeviceToDevice, st);
+    if (ce != cudaSuccess) return ce;
+    ce = cudaMemsetAsync(flux_pad + L.flux_elems, 0, (size_t)kFluxPad * 4, st);
+    if (ce != cudaSuccess) return ce;
     AccumParams P;
-    P.flux = in.ssp->flux;
+    P.flux = flux_pad;
     P.rec = (const Rec *)(ws + L.off_rec);
     P.units = (const Unit *)(ws + L.off_units);
     P.totals = (const int32_t *)(ws + L.off_totals);
@@ -296,7 +346,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const int tc = cpt * kAccThreads;
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
-    const bool vec = (in.ssp->n_lambda % 2 == 0) && (((uintptr_t)in.ssp->flux & 7u) == 0);
+    const bool vec = (in.ssp->n_lambda % 2 == 0);
     const size_t smem = (size_t)2 * wcap * sizeof(float2) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
