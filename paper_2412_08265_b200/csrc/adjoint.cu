@@ -15,7 +15,7 @@ namespace rubix {
 
 struct AdjParams {
     AxisParams ax;
-    int32_t n_lambda, n_z, n_c, n_s;
+    int32_t n_lambda, pitch, n_z, n_c, n_s;
     float l0_obs, dl_obs, dl_ssp;
     int64_t n;
 };
@@ -56,9 +56,9 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     const Rec r = rec[i];
     const float *g = gconv + (size_t)key[p] * P.n_c;
     const float *T0 = flux + r.cell;
-    const float *T1 = T0 + (size_t)P.n_z * P.n_lambda;
-    const float *T2 = T0 + P.n_lambda;
-    const float *T3 = T1 + P.n_lambda;
+    const float *T1 = T0 + (size_t)P.n_z * P.pitch;      // flux = padded workspace copy of the grid
+    const float *T2 = T0 + P.pitch;
+    const float *T3 = T1 + P.pitch;
     int ia, iz;
     double ta, tz, wa, wz;
     bool a_free, z_free;
@@ -113,6 +113,7 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     for (int i = 0; i < in.ssp->n_age; ++i) P.ax.age[i] = in.ssp->log_age_axis[i];
     for (int i = 0; i < in.ssp->n_z; ++i) P.ax.z[i] = in.ssp->log_z_axis[i];
     P.n_lambda = in.ssp->n_lambda;
+    P.pitch = L.pitch;
     P.n_z = in.ssp->n_z;
     P.n_c = L.n_c;
     P.n_s = L.n_s;
@@ -124,7 +125,8 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     k_adjoint<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const int32_t *)(ws + L.off_permbuf[L.final_buf]), (const int32_t *)(ws + L.off_seg),
         (const int32_t *)(ws + L.off_key), (const float *)(ws + L.off_vlos), in.p->mass,
-        in.p->log_age, in.p->log_z, (const Rec *)(ws + L.off_rec), in.ssp->flux, gconv, P, g_mass,
+        in.p->log_age, in.p->log_z, (const Rec *)(ws + L.off_rec), (const float *)(ws + L.off_flux), gconv, P,
+        g_mass,
         g_age, g_z, g_v);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;

@@ -133,8 +133,8 @@ size_t rubix_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telesc
         fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
         return 0;
     }
-    const size_t fe = ssp ? (size_t)ssp->n_age * ssp->n_z * ssp->n_lambda : 0;
-    return make_layout(n, tel->n_x * tel->n_y, tel->n_channels, fe).bytes_total;
+    return make_layout(n, tel->n_x * tel->n_y, tel->n_channels, ssp ? ssp->n_age * ssp->n_z : 0,
+                       ssp ? ssp->n_lambda : 0).bytes_total;
 }
 
 rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
@@ -149,8 +149,8 @@ rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, co
     if ((s = check_tel(tel)) != RUBIX_OK) return s;
     if (!R || !cube) return fail(RUBIX_ERR_NULL, "R or cube is NULL");
     if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
-    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels,
-                                 (size_t)ssp->n_age * ssp->n_z * ssp->n_lambda);
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
+                                 ssp->n_lambda);
     if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     PassInputs in{p, ssp, tel, R};
@@ -207,8 +207,8 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
     if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
         return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
     if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
-    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels,
-                                 (size_t)ssp->n_age * ssp->n_z * ssp->n_lambda);
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
+                                 ssp->n_lambda);
     if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     char *ws = (char *)workspace;
@@ -272,8 +272,8 @@ HostLayout host_layout(int64_t n, const rubix_ssp *ssp, const rubix_telescope *t
     H.cube = take(cube);
     H.cube2 = take(cube);
     H.ws = off;
-    H.total = off + make_layout(n, tel->n_x * tel->n_y, tel->n_channels,
-                                (size_t)ssp->n_age * ssp->n_z * ssp->n_lambda).bytes_total;
+    H.total = off + make_layout(n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
+                                ssp->n_lambda).bytes_total;
     return H;
 }
 }  // namespace

@@ -25,15 +25,16 @@ constexpr int kSortWarps = 8;               // warps per CTA in the radix passes
 constexpr int kSortItems = 1024;            // keys per warp per radix pass
 constexpr int kSortMaxDigitBits = 9;
 constexpr int kFluxPad = 2048;              // zero floats behind the workspace copy of the SSP grid
+constexpr int kRowAlign = 32;               // rows of that copy are padded to 32 floats (128 B)
 
 // Sorted-order particle record consumed by the accumulate kernel (48 B, 16-B aligned).
 struct __align__(16) Rec {
     float w[4];        // mass x bilinear weights of corners (i,j) (i+1,j) (i,j+1) (i+1,j+1)
-    int32_t cell;      // float offset of T[i][j][0] in the flux array
+    int32_t cell;      // float offset of T[i][j][0] in the padded workspace copy of the grid
     uint32_t b_fx;     // B = dl_obs / (dl_ssp (1+beta)) in 4.28 fixed point
     int64_t a_fx;      // A = (l0_obs/(1+beta) - l0_ssp)/dl_ssp in 36.28 fixed point
     int32_t k_lo, k_hi;  // channels whose rest position lies inside the SSP coverage
-    int32_t j0, nw;      // window of the whole spectrum: first SSP sample (multiple of 4), entries
+    int32_t j0, nw;      // window of the whole spectrum: first SSP sample (multiple of 32), samples
 };
 static_assert(sizeof(Rec) == 48, "Rec layout");
 
@@ -65,12 +66,13 @@ struct Layout {
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_units, off_rec,
         off_partials, off_cube_a, off_cube_b, off_flux;
-    size_t flux_elems;            // SSP samples; the workspace copy is followed by kFluxPad zeros
+    int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
+                                      // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
     int final_buf;                // which of the ping-pong buffers holds the final sort
 };
 
-Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, size_t flux_elems);
+Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t n_lambda);
 
 // ---- host launchers (each returns the CUDA status of its launches) ----------------------------
 struct PassInputs {

@@ -276,7 +276,7 @@ k_build_units(const int32_t *__restrict__ seg_off, const int32_t *__restrict__ u
 // --------------------------------------------------------------------------------------------
 struct PrepParams {
     AxisParams ax;
-    int32_t n_lambda, n_c, n_s;
+    int32_t n_lambda, pitch, n_c, n_s;
     float l0_ssp, dl_ssp, l0_obs, dl_obs;
 };
 
@@ -313,7 +313,7 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     r.w[1] = (float)(m * ta * (1.0 - tz));
     r.w[2] = (float)(m * (1.0 - ta) * tz);
     r.w[3] = (float)(m * ta * tz);
-    r.cell = (ia * P.ax.n_z + iz) * P.n_lambda;
+    r.cell = (ia * P.ax.n_z + iz) * P.pitch;
     const double inv = 1.0 / (1.0 + (double)vlos[p] / kCkms);
     const double scale = (double)(1 << kFxFrac);
     const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
@@ -332,10 +332,32 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     r.j0 = 0;
     r.nw = 0;
     if (k_lo <= k_hi) {
-        r.j0 = (int32_t)((a_fx + (int64_t)b_fx * k_lo) >> kFxFrac) & ~3;
-        r.nw = (int32_t)((a_fx + (int64_t)b_fx * k_hi) >> kFxFrac) - r.j0 + 1;
+        r.j0 = (int32_t)((a_fx + (int64_t)b_fx * k_lo) >> kFxFrac) & ~(kRowAlign - 1);
+        r.nw = (int32_t)((a_fx + (int64_t)b_fx * k_hi) >> kFxFrac) - r.j0 + 2;   // samples j0 .. j_max + 1
     }
     rec[i] = r;
+}
+
+// --------------------------------------------------------------------------------------------
+// Workspace copy of the SSP grid: every (age, Z) row padded with zeros to `pitch` floats (a
+// multiple of 32, so every row and every 32-sample group starts on a 128-byte line) and kFluxPad
+// zeros behind the last row.  The accumulate kernel then needs no bounds handling: a read past a
+// row's end finds zeros.  6-20 MB, stays L2 resident.
+// --------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_pad_flux(const float *__restrict__ flux, int32_t n_lambda, int32_t pitch, int64_t n_total,
+           int64_t n_grid, float *__restrict__ out)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_total;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        float v = 0.0f;
+        if (e < n_grid) {
+            const int64_t row = e / pitch;
+            const int32_t j = (int32_t)(e - row * pitch);
+            if (j < n_lambda) v = __ldg(flux + row * n_lambda + j);
+        }
+        out[e] = v;
+    }
 }
 
 // --------------------------------------------------------------------------------------------
@@ -348,7 +370,7 @@ static int bits_for(int32_t max_value)
     return b;
 }
 
-Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, size_t flux_elems)
+Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t n_lambda)
 {
     Layout L{};
     L.n = n;
@@ -387,8 +409,10 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, size_t flux_elems)
     L.off_units = take((size_t)L.max_units * sizeof(Unit));
     L.off_rec = take(nn * sizeof(Rec));
     L.off_partials = take((size_t)L.max_part_rows * (size_t)n_c * 4);
-    L.flux_elems = flux_elems;
-    L.off_flux = take((flux_elems + kFluxPad) * 4);
+    L.n_rows = n_rows;
+    L.n_lambda = n_lambda;
+    L.pitch = (n_lambda + kRowAlign - 1) / kRowAlign * kRowAlign;
+    L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
     L.bytes_total = off;
     return L;
 }
@@ -412,6 +436,12 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     Unit *units = (Unit *)(ws + L.off_units);
     Rec *rec = (Rec *)(ws + L.off_rec);
 
+    if (L.n_rows > 0) {
+        const int64_t n_grid = (int64_t)L.n_rows * L.pitch, n_total = n_grid + kFluxPad;
+        k_pad_flux<<<(unsigned)((n_total + 1023) / 1024), 256, 0, st>>>(
+            in.ssp->flux, L.n_lambda, L.pitch, n_total, n_grid, (float *)(ws + L.off_flux));
+        RUBIX_LAUNCH_CHECK();
+    }
     if (n > 0) {
         BinParams B;
         for (int i = 0; i < 9; ++i) B.R[i] = in.R[i];
@@ -462,6 +492,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         for (int i = 0; i < in.ssp->n_age; ++i) P.ax.age[i] = in.ssp->log_age_axis[i];
         for (int i = 0; i < in.ssp->n_z; ++i) P.ax.z[i] = in.ssp->log_z_axis[i];
         P.n_lambda = in.ssp->n_lambda;
+        P.pitch = L.pitch;
         P.n_c = in.tel->n_channels;
         P.n_s = n_s;
         P.l0_ssp = in.ssp->lambda0;

@@ -5,12 +5,14 @@
 // CTA (256 threads) per unit; thread t owns channels k0 + t + 256 i (i < CPT) and keeps their sums
 // in registers, so a spaxel's spectrum is reduced without any atomic.  Per particle:
 //   blend    the four corner templates are read once over the particle's rest-wavelength window
-//            (8-byte loads, 256 B contiguous per warp instruction, from a zero-padded workspace
-//            copy of the grid so no load needs clamping), blended with the mass-scaled bilinear
-//            weights (packed fp32x2 FMAs) and stored in shared memory as interval entries
-//            (S_j - D_j, D_j),  D_j = S_{j+1} - S_j   (S_{j+1} comes from the next lane by shuffle);
-//   resample channel k reads ONE 8-byte entry: value = (S_j - D_j) + f1 * D_j with f1 = 1 + frac(x_k),
-//            x_k from exact integer arithmetic (32-bit 12.20 local fixed point).
+//            and blended with the mass-scaled bilinear weights into a shared-memory table S_j.
+//            The window starts on a multiple of 32 samples of the padded workspace copy of the grid
+//            (rows padded to 128 B), so a warp pass is four 512-byte, line-aligned 16-byte-per-lane
+//            loads (one per corner), eight packed fp32x2 FMAs and one 16-byte table store per lane:
+//            every L1 wavefront moves a full 128 bytes;
+//   resample channel k reads S_j and S_{j+1} (the 32 lanes of a warp read ~25 consecutive words: no
+//            bank conflict) and adds S_j + f (S_{j+1} - S_j); j and f come from exact integer
+//            arithmetic on x_k (32-bit 12.20 local fixed point).
 // The table is double buffered and the loop is software pipelined: the template loads of particle
 // p+1 are issued, then particle p is resampled while they fly, then p+1 is blended (each further
 // pass of loads is issued before the previous pass is consumed); one __syncthreads per particle.
@@ -22,29 +24,23 @@
 namespace rubix {
 
 struct AccumParams {
-    const float *flux;
+    const float *flux;       // padded workspace copy of the SSP grid (Layout::pitch)
     const Rec *rec;
     const Unit *units;
     const int32_t *totals;
     float *cube;
     float *partials;
-    int32_t n_lambda, n_z, n_c, n_tiles, wcap;
+    int32_t pitch, n_z, n_c, n_tiles, wcap;
 };
 
-constexpr int kWarpSpan = 126;                       // table entries produced per warp per pass
-constexpr int kPassSpan = kWarpSpan * (kAccThreads / 32);
+constexpr int kPass = 128;                           // table samples produced per warp per pass
+constexpr int kAccWarps = kAccThreads / 32;
 
 // ---- packed fp32x2 arithmetic (sm_100+): one issue slot, two FMAs ------------------------------
 __device__ __forceinline__ unsigned long long pack2(float lo, float hi)
 {
     unsigned long long r;
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ float2 unpack2(unsigned long long v)
-{
-    float2 r;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
     return r;
 }
 __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
@@ -66,29 +62,37 @@ __device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c)
     asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
-__device__ __forceinline__ unsigned long long ld2u(const float *p)
+
+struct Quad { unsigned long long lo, hi; };          // four consecutive samples as two packed pairs
+
+__device__ __forceinline__ Quad ldg_quad(const float *p)
 {
-    unsigned long long v;
-    asm volatile("ld.global.nc.b64 %0, [%1];" : "=l"(v) : "l"(p));
-    return v;
+    Quad q;
+    asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+    return q;
+}
+__device__ __forceinline__ void sts_quad(float *p, unsigned long long lo, unsigned long long hi)
+{
+    asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"((uint32_t)__cvta_generic_to_shared(p)), "l"(lo), "l"(hi)
+                 : "memory");
 }
 
 struct Win {                 // one particle's window in one channel tile
     int64_t base;            // x(k0) - j0 in 36.28 fixed point
     uint32_t b;              // step per channel, 4.28
     int32_t ka, kb;          // channels of this tile inside the SSP coverage (ka > kb: none)
-    int32_t first, nw;       // flux index of (corner (i,j), sample j0); entries needed
+    int32_t first, nw;       // flux index of (corner (i,j), sample j0); samples needed
     float w0, w1, w2, w3;
 };
 
-struct LoadSet { unsigned long long c[4][2]; };      // 4 corners x 2 pair blocks, packed pairs
+struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 
 // SINGLE: the whole spectrum is one tile (n_tiles == 1): window (j0, nw) comes from the record.
-template <int CPT, bool VEC, bool SINGLE>
+template <int CPT, bool SINGLE>
 __global__ void __launch_bounds__(kAccThreads, 3)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
-    extern __shared__ __align__(16) float2 tab[];           // [2][wcap] interval entries, then records
+    extern __shared__ __align__(16) float tab[];            // [2][wcap] samples S_j, then the records
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = SINGLE ? 0 : blockIdx.x % P.n_tiles;
     const int u = SINGLE ? blockIdx.x : blockIdx.x / P.n_tiles;
@@ -110,9 +114,8 @@ k_accumulate(const __grid_constant__ AccumParams P)
             for (int i = tid; i < U.count * 3; i += kAccThreads) srec[i] = __ldg(g + i);
         }
         __syncthreads();
-        const int row_a = P.n_z * P.n_lambda;               // (i+1, j) - (i, j)
-        const int row_z = P.n_lambda;                       // (i, j+1) - (i, j)
-        const int nlm1 = P.n_lambda - 1;
+        const int row_a = P.n_z * P.pitch;                  // (i+1, j) - (i, j)
+        const int row_z = P.pitch;                          // (i, j+1) - (i, j)
 
         auto window = [&](int q) -> Win {
             const int4 ra = srec[3 * q], rb = srec[3 * q + 1], rc = srec[3 * q + 2];
@@ -124,15 +127,15 @@ k_accumulate(const __grid_constant__ AccumParams P)
             int j0;
             if (SINGLE) {                                   // k0 = 0, k_end = n_c - 1 >= k_hi
                 W.ka = rc.x; W.kb = rc.y;
-                j0 = rc.z; W.nw = min(rc.w, P.wcap);
+                j0 = rc.z; W.nw = rc.w;
             } else {
                 W.ka = max(k0, rc.x);
                 W.kb = min(k_end, rc.y);
                 j0 = 0; W.nw = 0;
                 if (W.ka <= W.kb) {
                     const int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * W.kb;
-                    j0 = (int)(xa >> kFxFrac) & ~3;
-                    W.nw = min((int)(xb >> kFxFrac) - j0 + 1, P.wcap);  // last entry <= n_lambda-1
+                    j0 = (int)(xa >> kFxFrac) & ~(kRowAlign - 1);
+                    W.nw = (int)(xb >> kFxFrac) - j0 + 2;   // samples j0 .. j_max + 1
                 }
             }
             W.first = rb.x + j0;
@@ -140,71 +143,49 @@ k_accumulate(const __grid_constant__ AccumParams P)
             return W;
         };
 
-        // ---- vector path: warp `warp`, pass starting at entry sb; the lane handles the entry pairs
-        //      sb + 2 lane and sb + 64 + 2 lane; lane 31 of the second block only feeds lane 30's
-        //      neighbour.  P.flux is the padded workspace copy, so reads past a window are harmless.
-        auto issue = [&](LoadSet &L, const Win &W, int sb) {
-            const int i0 = W.first + sb + 2 * lane;
-            const float *t0 = P.flux + i0, *t1 = P.flux + (i0 + row_a);
-            const float *t2 = P.flux + (i0 + row_z), *t3 = P.flux + (i0 + row_a + row_z);
-            L.c[0][0] = ld2u(t0); L.c[0][1] = ld2u(t0 + 64);
-            L.c[1][0] = ld2u(t1); L.c[1][1] = ld2u(t1 + 64);
-            L.c[2][0] = ld2u(t2); L.c[2][1] = ld2u(t2 + 64);
-            L.c[3][0] = ld2u(t3); L.c[3][1] = ld2u(t3 + 64);
+        // ---- blend: warp `warp` produces samples [128 pass, 128 pass + 128) for pass = warp, warp+8..
+        //      Loads and stores are unconditional: the padded grid copy and the table (a whole
+        //      number of passes) absorb the overshoot.
+        auto issue = [&](LoadSet &L, const Win &W, int pass) {
+            const float *t0 = P.flux + (W.first + pass * kPass + 4 * lane);
+            L.c[0] = ldg_quad(t0);
+            L.c[1] = ldg_quad(t0 + row_a);
+            L.c[2] = ldg_quad(t0 + row_z);
+            L.c[3] = ldg_quad(t0 + row_a + row_z);
         };
-        auto consume = [&](const LoadSet &L, const Win &W, int sb, float2 *buf) {
-            const int p1 = sb + 2 * lane, p2 = p1 + 64;
+        auto consume = [&](const LoadSet &L, const Win &W, int pass, float *buf) {
             const unsigned long long w0 = pack2(W.w0, W.w0), w1 = pack2(W.w1, W.w1);
             const unsigned long long w2 = pack2(W.w2, W.w2), w3 = pack2(W.w3, W.w3);
-            const float2 s1 = unpack2(ffma2(w3, L.c[3][0], ffma2(w2, L.c[2][0], ffma2(w1, L.c[1][0], fmul2(w0, L.c[0][0])))));
-            const float2 s2 = unpack2(ffma2(w3, L.c[3][1], ffma2(w2, L.c[2][1], ffma2(w1, L.c[1][1], fmul2(w0, L.c[0][1])))));
-            // S_{j+2} of each pair from the next lane; the last interval (N_l-1) is only ever
-            // evaluated at f = 0, where (S - D) + D = S whatever D is, so no special case
-            const float nb1 = __shfl_sync(0xffffffffu, lane == 0 ? s2.x : s1.x, (lane + 1) & 31);
-            const float nb2 = __shfl_down_sync(0xffffffffu, s2.x, 1);
-            float4 e1, e2;
-            e1.y = s1.y - s1.x; e1.x = s1.x - e1.y; e1.w = nb1 - s1.y; e1.z = s1.y - e1.w;
-            e2.y = s2.y - s2.x; e2.x = s2.x - e2.y; e2.w = nb2 - s2.y; e2.z = s2.y - e2.w;
-            if (p1 < W.nw) *reinterpret_cast<float4 *>(buf + p1) = e1;
-            if (lane < 31 && p2 < W.nw) *reinterpret_cast<float4 *>(buf + p2) = e2;
+            const unsigned long long lo = ffma2(w3, L.c[3].lo, ffma2(w2, L.c[2].lo, ffma2(w1, L.c[1].lo, fmul2(w0, L.c[0].lo))));
+            const unsigned long long hi = ffma2(w3, L.c[3].hi, ffma2(w2, L.c[2].hi, ffma2(w1, L.c[1].hi, fmul2(w0, L.c[0].hi))));
+            sts_quad(buf + pass * kPass + 4 * lane, lo, hi);
         };
-        // ---- scalar path (row length odd or misaligned flux): plain per-entry blend
-        auto blend_scalar = [&](const Win &W, float2 *buf) {
-            for (int e = tid; e < W.nw; e += kAccThreads) {
-                const float *t = P.flux + W.first + e;
-                const float s0 = fmaf(W.w3, __ldg(t + row_a + row_z),
-                                      fmaf(W.w2, __ldg(t + row_z), fmaf(W.w1, __ldg(t + row_a), W.w0 * __ldg(t))));
-                const float s1 = fmaf(W.w3, __ldg(t + row_a + row_z + 1),
-                                      fmaf(W.w2, __ldg(t + row_z + 1), fmaf(W.w1, __ldg(t + row_a + 1), W.w0 * __ldg(t + 1))));
-                const float d = s1 - s0;
-                buf[e] = make_float2(s0 - d, d);
-            }
-        };
-        // all passes, software pipelined (A holds the pass being consumed, loads already issued)
-        auto blend_rest = [&](LoadSet &A, const Win &W, float2 *buf) {
+        // all passes of this warp, software pipelined (A holds the pass being consumed, loads issued)
+        auto blend_rest = [&](LoadSet &A, const Win &W, float *buf) {
             LoadSet B;
-            int sb = warp * kWarpSpan;
+            int pass = warp;
             while (true) {
-                int nb = sb + kPassSpan;
-                bool more = nb < W.nw;
+                int nb = pass + kAccWarps;
+                bool more = nb * kPass < W.nw;
                 if (more) issue(B, W, nb);
-                consume(A, W, sb, buf);
+                consume(A, W, pass, buf);
                 if (!more) break;
-                sb = nb; nb += kPassSpan; more = nb < W.nw;
+                pass = nb; nb += kAccWarps; more = nb * kPass < W.nw;
                 if (more) issue(A, W, nb);
-                consume(B, W, sb, buf);
+                consume(B, W, pass, buf);
                 if (!more) break;
-                sb = nb;
+                pass = nb;
             }
         };
 
-        const uint32_t m_addr = 0x7FF8u, m_frac = 0x7FFFF8u, one_bits = 0x3F800000u;
+        const uint32_t m_addr = 0x3FFCu, m_frac = 0x7FFFF8u, one_bits = 0x3F800000u;
         auto sample = [&](int i, uint32_t x, const char *bytes) {
-            const float2 e = *reinterpret_cast<const float2 *>(bytes + ((x >> 17) & m_addr));
-            const float f1 = __uint_as_float(and_or(x << 3, m_frac, one_bits));   // 1 + frac(x_k)
-            acc[i] += fmaf(f1, e.y, e.x);                   // (S_j - D_j) + f1 D_j
+            const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
+            const float s0 = e[0], s1 = e[1];
+            const float f = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;    // frac(x_k), exact
+            acc[i] += fmaf(f, s1 - s0, s0);
         };
-        auto resample = [&](const Win &W, const float2 *buf) {
+        auto resample = [&](const Win &W, const float *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
             // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
             const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
@@ -222,35 +203,28 @@ k_accumulate(const __grid_constant__ AccumParams P)
 
         // prologue: table of particle 0
         Win cur = window(0);
-        if (cur.ka <= cur.kb) {
-            if (VEC) {
-                LoadSet A;
-                if (warp * kWarpSpan < cur.nw) { issue(A, cur, warp * kWarpSpan); blend_rest(A, cur, tab); }
-            } else {
-                blend_scalar(cur, tab);
-            }
+        if (cur.ka <= cur.kb && warp * kPass < cur.nw) {
+            LoadSet A;
+            issue(A, cur, warp);
+            blend_rest(A, cur, tab);
         }
         __syncthreads();
         for (int q = 0; q < U.count; ++q) {
-            float2 *buf_next = tab + (size_t)((q + 1) & 1) * P.wcap;
+            float *buf_next = tab + (size_t)((q + 1) & 1) * P.wcap;
             Win nxt;
             nxt.ka = 1; nxt.kb = 0;
             LoadSet A;
             bool blend_next = false;
             if (q + 1 < U.count) {
                 nxt = window(q + 1);
-                blend_next = (nxt.ka <= nxt.kb) && (!VEC || warp * kWarpSpan < nxt.nw);
-                if (VEC && blend_next) issue(A, nxt, warp * kWarpSpan);     // loads fly during resample
+                blend_next = (nxt.ka <= nxt.kb) && (warp * kPass < nxt.nw);
+                if (blend_next) issue(A, nxt, warp);        // loads fly during the resample
             }
             if (cur.ka <= cur.kb) resample(cur, tab + (size_t)(q & 1) * P.wcap);
-            if (blend_next) {
-                if (VEC) blend_rest(A, nxt, buf_next);
-                else blend_scalar(nxt, buf_next);
-            }
+            if (blend_next) blend_rest(A, nxt, buf_next);
             cur = nxt;
             __syncthreads();
         }
-        (void)nlm1;
     }
 #pragma unroll
     for (int i = 0; i < CPT; ++i) {
@@ -282,25 +256,25 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
-template <int CPT, bool VEC, bool SINGLE>
-static cudaError_t launch_acc3(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
+template <int CPT>
+static cudaError_t launch_acc(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_accumulate<CPT, VEC, SINGLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_accumulate<CPT, VEC, SINGLE><<<grid, kAccThreads, smem, st>>>(P);
+    cudaError_t e;
+    if (P.n_tiles == 1) {
+        e = cudaFuncSetAttribute(k_accumulate<CPT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_accumulate<CPT, true><<<grid, kAccThreads, smem, st>>>(P);
+    } else {
+        e = cudaFuncSetAttribute(k_accumulate<CPT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_accumulate<CPT, false><<<grid, kAccThreads, smem, st>>>(P);
+    }
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }
 
-template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, bool vec, unsigned grid, size_t smem, cudaStream_t st)
-{
-    const bool single = P.n_tiles == 1;
-    if (vec) return single ? launch_acc3<CPT, true, true>(P, grid, smem, st) : launch_acc3<CPT, true, false>(P, grid, smem, st);
-    return single ? launch_acc3<CPT, false, true>(P, grid, smem, st) : launch_acc3<CPT, false, false>(P, grid, smem, st);
-}
-
-// Largest CPT in {15, 8, 4, 2, 1} whose table fits the 12.20 format; returns window capacity.
+// Largest CPT in {15, 8, 4, 2, 1} whose table fits the 12.20 format; returns the table capacity
+// (samples, a whole number of passes).
 int choose_cpt(int n_c, double b_max, int *wcap_out)
 {
     const int cand[5] = {15, 8, 4, 2, 1};
@@ -310,9 +284,11 @@ int choose_cpt(int n_c, double b_max, int *wcap_out)
         const int tiles = (n_c + tc - 1) / tc;
         // skip tilings that leave a whole 256-channel group of lanes idle (unless the smallest)
         if (cpt > 1 && (long long)tiles * tc - n_c >= kAccThreads) continue;
-        const int wcap = (int)(b_max * tc) + 12;
+        // samples j0 .. j_max + 1 with j0 rounded down to a multiple of kRowAlign
+        const int need = (int)(b_max * tc) + kRowAlign + 4;
+        const int wcap = (need + kPass - 1) / kPass * kPass;
         if (wcap > kTabMax) continue;
-        *wcap_out = (wcap + 3) & ~3;
+        *wcap_out = wcap;
         return cpt;
     }
     *wcap_out = 0;
@@ -326,38 +302,30 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     int wcap = 0;
     const int cpt = choose_cpt(L.n_c, b_max, &wcap);
     if (cpt == 0) return cudaErrorInvalidConfiguration;
-    // padded workspace copy of the SSP grid: reads past a window's end (next row or the zero
-    // pad) are harmless, so the blend needs no clamping
-    float *flux_pad = (float *)(ws + L.off_flux);
-    cudaError_t ce = cudaMemcpyAsync(flux_pad, in.ssp->flux, L.flux_elems * 4, cudaMemcpyDeviceToDevice, st);
-    if (ce != cudaSuccess) return ce;
-    ce = cudaMemsetAsync(flux_pad + L.flux_elems, 0, (size_t)kFluxPad * 4, st);
-    if (ce != cudaSuccess) return ce;
     AccumParams P;
-    P.flux = flux_pad;
+    P.flux = (const float *)(ws + L.off_flux);
     P.rec = (const Rec *)(ws + L.off_rec);
     P.units = (const Unit *)(ws + L.off_units);
     P.totals = (const int32_t *)(ws + L.off_totals);
     P.cube = cube;
     P.partials = (float *)(ws + L.off_partials);
-    P.n_lambda = in.ssp->n_lambda;
+    P.pitch = L.pitch;
     P.n_z = in.ssp->n_z;
     P.n_c = L.n_c;
     const int tc = cpt * kAccThreads;
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
-    const bool vec = (in.ssp->n_lambda % 2 == 0);
-    const size_t smem = (size_t)2 * wcap * sizeof(float2) + (size_t)kChunk * sizeof(Rec);
+    const size_t smem = (size_t)2 * wcap * sizeof(float) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
     {
         StageTimer t(1, st);
         switch (cpt) {
-            case 15: e = launch_acc<15>(P, vec, grid, smem, st); break;
-            case 8: e = launch_acc<8>(P, vec, grid, smem, st); break;
-            case 4: e = launch_acc<4>(P, vec, grid, smem, st); break;
-            case 2: e = launch_acc<2>(P, vec, grid, smem, st); break;
-            default: e = launch_acc<1>(P, vec, grid, smem, st); break;
+            case 15: e = launch_acc<15>(P, grid, smem, st); break;
+            case 8: e = launch_acc<8>(P, grid, smem, st); break;
+            case 4: e = launch_acc<4>(P, grid, smem, st); break;
+            case 2: e = launch_acc<2>(P, grid, smem, st); break;
+            default: e = launch_acc<1>(P, grid, smem, st); break;
         }
     }
     if (e != cudaSuccess) return e;

@@ -187,9 +187,9 @@ def test_contention(B):
     assert counts.max() > 0.03 * w.particles.n
     order = np.argsort(counts)
     rng = np.random.default_rng(15)
-    # heaviest spaxel is ~1e6 particles x 3700 channels = several 1e9 oracle samples: take the
+    # the heaviest spaxel (~1e6 particles x 3700 channels = a few 1e9 oracle samples, ~10 s), the
     # 5th..8th heaviest (still > 1e5 particles, thousands of chunks) plus lighter ones
-    sel = np.unique(np.concatenate([order[-8:-4], order[-400:-8:60],
+    sel = np.unique(np.concatenate([order[-1:], order[-8:-4], order[-400:-8:60],
                                     rng.choice(np.nonzero(counts > 0)[0], 30)])).astype(np.int32)
     ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t, sel=sel)
     got = cube.view(t.n_spaxels, -1)[torch.from_numpy(sel.astype(np.int64)).cuda()].cpu().numpy().astype(np.float64)
@@ -201,9 +201,9 @@ def test_contention(B):
     assert (np.abs(got.sum(-1) - ref.sum(-1))[pos] / ref.sum(-1)[pos]).max() <= FLUX_TOL
     empty = torch.from_numpy(counts == 0).cuda()
     assert not cube.view(t.n_spaxels, -1)[empty].any().item()
-    # heaviest spaxel: invariant instead of the oracle -- its flux equals the sum of its particles'
-    # masses times the mean template level within a loose physical bound, and it is the global max
-    assert int(cube.sum(-1).argmax().item()) == int(order[-1])
+    # the brightest spaxel is one of the four central ones (their counts differ by a few per cent, so
+    # which of them wins depends on the masses and ages it drew)
+    assert int(cube.sum(-1).argmax().item()) in set(int(v) for v in order[-4:])
 
 
 # ------------------------------------------------------------------ config 4: adjoint
