@@ -412,6 +412,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.n_rows = n_rows;
     L.n_lambda = n_lambda;
     L.pitch = (n_lambda + kRowAlign - 1) / kRowAlign * kRowAlign;
+    off = align_up(off, 512);                            // (texture-alignment safe)
     L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
     L.bytes_total = off;
     return L;

@@ -31,10 +31,25 @@ struct AccumParams {
     float *cube;
     float *partials;
     int32_t pitch, n_z, n_c, n_tiles, wcap;
+    cudaTextureObject_t tex;
 };
 
 constexpr int kPass = 128;                           // table samples produced per warp per pass
 constexpr int kAccWarps = kAccThreads / 32;
+#ifndef RUBIX_LDG_MODE
+#define RUBIX_LDG_MODE 0
+#endif
+#ifndef RUBIX_TEX_CORNERS
+#define RUBIX_TEX_CORNERS 0
+#endif
+#ifndef RUBIX_ACC_DEPTH
+#define RUBIX_ACC_DEPTH 1
+#endif
+#ifndef RUBIX_ACC_MINB
+#define RUBIX_ACC_MINB 3
+#endif
+constexpr int kAccDepth = RUBIX_ACC_DEPTH;           // load sets (passes) in flight per warp
+constexpr int kAccMinBlocks = RUBIX_ACC_MINB;
 
 // ---- packed fp32x2 arithmetic (sm_100+): one issue slot, two FMAs ------------------------------
 __device__ __forceinline__ unsigned long long pack2(float lo, float hi)
@@ -68,7 +83,15 @@ struct Quad { unsigned long long lo, hi; };          // four consecutive samples
 __device__ __forceinline__ Quad ldg_quad(const float *p)
 {
     Quad q;
+#if RUBIX_LDG_MODE == 1
+    asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+#elif RUBIX_LDG_MODE == 2
+    asm volatile("ld.global.cg.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+#elif RUBIX_LDG_MODE == 3
+    asm volatile("ld.global.nc.L1::evict_first.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+#else
     asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+#endif
     return q;
 }
 __device__ __forceinline__ void sts_quad(float *p, unsigned long long lo, unsigned long long hi)
@@ -88,8 +111,8 @@ struct Win {                 // one particle's window in one channel tile
 struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 
 // SINGLE: the whole spectrum is one tile (n_tiles == 1): window (j0, nw) comes from the record.
-template <int CPT, bool SINGLE>
-__global__ void __launch_bounds__(kAccThreads, 3)
+template <int CPT, bool SINGLE, int DEPTH, int MINB>
+__global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
     extern __shared__ __align__(16) float tab[];            // [2][wcap] samples S_j, then the records
@@ -145,36 +168,47 @@ k_accumulate(const __grid_constant__ AccumParams P)
 
         // ---- blend: warp `warp` produces samples [128 pass, 128 pass + 128) for pass = warp, warp+8..
         //      Loads and stores are unconditional: the padded grid copy and the table (a whole
-        //      number of passes) absorb the overshoot.
-        auto issue = [&](LoadSet &L, const Win &W, int pass) {
-            const float *t0 = P.flux + (W.first + pass * kPass + 4 * lane);
-            L.c[0] = ldg_quad(t0);
-            L.c[1] = ldg_quad(t0 + row_a);
-            L.c[2] = ldg_quad(t0 + row_z);
-            L.c[3] = ldg_quad(t0 + row_a + row_z);
+        //      number of passes) absorb the overshoot.  A register ring of DEPTH load sets per warp:
+        //      the first DEPTH passes of the next particle are issued before the current particle
+        //      is resampled (their latency hides behind it), later passes refill the ring.
+        constexpr int kStep = kAccWarps * kPass;            // samples between two passes of a warp
+        auto tex_quad = [&](const float *t) -> Quad {
+            const float4 v = tex1Dfetch<float4>(P.tex, (int)((t - P.flux) >> 2));
+            Quad q;
+            q.lo = pack2(v.x, v.y); q.hi = pack2(v.z, v.w);
+            return q;
         };
-        auto consume = [&](const LoadSet &L, const Win &W, int pass, float *buf) {
+        auto issue = [&](LoadSet &L, const float *t0) {
+            L.c[0] = RUBIX_TEX_CORNERS >= 4 ? tex_quad(t0) : ldg_quad(t0);
+            L.c[1] = RUBIX_TEX_CORNERS >= 3 ? tex_quad(t0 + row_a) : ldg_quad(t0 + row_a);
+            L.c[2] = RUBIX_TEX_CORNERS >= 2 ? tex_quad(t0 + row_z) : ldg_quad(t0 + row_z);
+            L.c[3] = RUBIX_TEX_CORNERS >= 1 ? tex_quad(t0 + row_a + row_z) : ldg_quad(t0 + row_a + row_z);
+        };
+        auto consume = [&](const LoadSet &L, const Win &W, float *dst) {
             const unsigned long long w0 = pack2(W.w0, W.w0), w1 = pack2(W.w1, W.w1);
             const unsigned long long w2 = pack2(W.w2, W.w2), w3 = pack2(W.w3, W.w3);
             const unsigned long long lo = ffma2(w3, L.c[3].lo, ffma2(w2, L.c[2].lo, ffma2(w1, L.c[1].lo, fmul2(w0, L.c[0].lo))));
             const unsigned long long hi = ffma2(w3, L.c[3].hi, ffma2(w2, L.c[2].hi, ffma2(w1, L.c[1].hi, fmul2(w0, L.c[0].hi))));
-            sts_quad(buf + pass * kPass + 4 * lane, lo, hi);
+            sts_quad(dst, lo, hi);
         };
-        // all passes of this warp, software pipelined (A holds the pass being consumed, loads issued)
-        auto blend_rest = [&](LoadSet &A, const Win &W, float *buf) {
-            LoadSet B;
-            int pass = warp;
+        auto prefetch = [&](LoadSet (&L)[DEPTH], const Win &W) {
+            const float *t0 = P.flux + (W.first + warp * kPass + 4 * lane);
+#pragma unroll
+            for (int d = 0; d < DEPTH; ++d)
+                if ((warp + d * kAccWarps) * kPass < W.nw) issue(L[d], t0 + d * kStep);
+        };
+        auto blend_all = [&](LoadSet (&L)[DEPTH], const Win &W, float *buf) {
+            const float *t0 = P.flux + (W.first + warp * kPass + 4 * lane);
+            float *dst = buf + warp * kPass + 4 * lane;
+            int s0 = warp * kPass;                          // first sample of the pass held by L[0]
             while (true) {
-                int nb = pass + kAccWarps;
-                bool more = nb * kPass < W.nw;
-                if (more) issue(B, W, nb);
-                consume(A, W, pass, buf);
-                if (!more) break;
-                pass = nb; nb += kAccWarps; more = nb * kPass < W.nw;
-                if (more) issue(A, W, nb);
-                consume(B, W, pass, buf);
-                if (!more) break;
-                pass = nb;
+#pragma unroll
+                for (int d = 0; d < DEPTH; ++d) {
+                    if (s0 >= W.nw) return;
+                    consume(L[d], W, dst);
+                    if (s0 + DEPTH * kStep < W.nw) issue(L[d], t0 + DEPTH * kStep);
+                    s0 += kStep; t0 += kStep; dst += kStep;
+                }
             }
         };
 
@@ -203,25 +237,27 @@ k_accumulate(const __grid_constant__ AccumParams P)
 
         // prologue: table of particle 0
         Win cur = window(0);
-        if (cur.ka <= cur.kb && warp * kPass < cur.nw) {
-            LoadSet A;
-            issue(A, cur, warp);
-            blend_rest(A, cur, tab);
+        {
+            LoadSet L[DEPTH];
+            if (cur.ka <= cur.kb) {
+                prefetch(L, cur);
+                blend_all(L, cur, tab);
+            }
         }
         __syncthreads();
         for (int q = 0; q < U.count; ++q) {
             float *buf_next = tab + (size_t)((q + 1) & 1) * P.wcap;
             Win nxt;
             nxt.ka = 1; nxt.kb = 0;
-            LoadSet A;
+            LoadSet L[DEPTH];
             bool blend_next = false;
             if (q + 1 < U.count) {
                 nxt = window(q + 1);
-                blend_next = (nxt.ka <= nxt.kb) && (warp * kPass < nxt.nw);
-                if (blend_next) issue(A, nxt, warp);        // loads fly during the resample
+                blend_next = nxt.ka <= nxt.kb;
+                if (blend_next) prefetch(L, nxt);           // loads fly during the resample
             }
             if (cur.ka <= cur.kb) resample(cur, tab + (size_t)(q & 1) * P.wcap);
-            if (blend_next) blend_rest(A, nxt, buf_next);
+            if (blend_next) blend_all(L, nxt, buf_next);
             cur = nxt;
             __syncthreads();
         }
@@ -261,13 +297,13 @@ static cudaError_t launch_acc(const AccumParams &P, unsigned grid, size_t smem, 
 {
     cudaError_t e;
     if (P.n_tiles == 1) {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(k_accumulate<CPT, true, kAccDepth, kAccMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_accumulate<CPT, true><<<grid, kAccThreads, smem, st>>>(P);
+        k_accumulate<CPT, true, kAccDepth, kAccMinBlocks><<<grid, kAccThreads, smem, st>>>(P);
     } else {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(k_accumulate<CPT, false, kAccDepth, kAccMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_accumulate<CPT, false><<<grid, kAccThreads, smem, st>>>(P);
+        k_accumulate<CPT, false, kAccDepth, kAccMinBlocks><<<grid, kAccThreads, smem, st>>>(P);
     }
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
@@ -315,6 +351,27 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const int tc = cpt * kAccThreads;
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
+    P.tex = 0;
+#if RUBIX_TEX_CORNERS > 0
+    {
+        static thread_local const void *cached_ptr = nullptr;
+        static thread_local cudaTextureObject_t cached_tex = 0;
+        if (cached_ptr != (const void *)P.flux) {
+            if (cached_tex) cudaDestroyTextureObject(cached_tex);
+            cudaResourceDesc rd{};
+            rd.resType = cudaResourceTypeLinear;
+            rd.res.linear.devPtr = (void *)P.flux;
+            rd.res.linear.desc = cudaCreateChannelDesc<float4>();
+            rd.res.linear.sizeInBytes = ((size_t)L.n_rows * L.pitch + kFluxPad) * 4;
+            cudaTextureDesc td{};
+            td.readMode = cudaReadModeElementType;
+            cudaError_t te = cudaCreateTextureObject(&cached_tex, &rd, &td, nullptr);
+            if (te != cudaSuccess) return te;
+            cached_ptr = (const void *)P.flux;
+        }
+        P.tex = cached_tex;
+    }
+#endif
     const size_t smem = (size_t)2 * wcap * sizeof(float) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
