@@ -175,7 +175,7 @@ def run_ours(args):
     import torch.distributed as dist
 
     from paper_2412_08265_b200 import binding as B
-    from paper_2412_08265_b200 import synth
+    from paper_2412_08265_b200 import replicas, synth
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -190,7 +190,8 @@ def run_ours(args):
 
     # replicas: rank r gets its own galaxy (same recipe, seed + r)
     base = synth.make_workload(args.workload)
-    w = base if rank == 0 else synth.make_workload(args.workload, seed=1000 + 10 * rank + 2)
+    widx = ["tiny", "small", "medium", "contention"].index(args.workload)
+    w = base if rank == 0 else synth.make_workload(args.workload, seed=replicas.replica_seed(widx, rank))
     t, n = w.telescope, w.particles.n
     dw = B.DeviceWorkload(w, device=dev)
     cube = torch.empty(dw.shape, dtype=torch.float32, device=dev)
@@ -230,13 +231,10 @@ def run_ours(args):
     elapsed_ms = e0.elapsed_time(e1)
     stages = B.rubix_stage_timing_read()
     B.rubix_stage_timing_enable(False)
-    if world > 1:
-        tt = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tt.item())
+    elapsed_ms = replicas.max_over_ranks(elapsed_ms, dev)
     ms_per_step = elapsed_ms / args.steps
     samples_per_step = float(n) * t.n_channels
-    value = world * samples_per_step / (ms_per_step * 1e-3) / 1e9
+    value = replicas.whole_job_value(samples_per_step, world, elapsed_ms, args.steps) / 1e9
 
     # ---- end to end through the host-buffer entry point
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -258,12 +256,9 @@ def run_ours(args):
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        tt = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
+    e2e_ms = replicas.max_over_ranks(e2e_ms, dev)
+    e2e_value = replicas.whole_job_value(samples_per_step, world, e2e_ms, args.e2e_steps) / 1e9
     e2e_ms /= args.e2e_steps
-    e2e_value = world * samples_per_step / (e2e_ms * 1e-3) / 1e9
 
     if rank != 0:
         if world > 1:

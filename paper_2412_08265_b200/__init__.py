@@ -7,4 +7,4 @@
 Nothing here falls back to the CPU: importing ``binding`` without the built library, or calling
 it without a CUDA device, raises.
 """
-__all__ = ["synth", "binding", "build"]
+__all__ = ["synth", "binding", "build", "replicas"]
