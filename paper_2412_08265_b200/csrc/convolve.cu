@@ -70,7 +70,7 @@ struct MarchParams {
     int64_t line_stride, step_stride;   // elements
     int32_t n_lines, n_steps, n_c, cblocks;
     float g[15];                        // stencil along the marching axis, zero padded, centred
-    float h[9];                         // LSF taps along the channel, zero padded, centred
+    float h[9];                         // LSF taps along the channel, zero padded, centred, symmetric
 };
 
 __device__ __forceinline__ float2 shfl_up2(float2 v, int d)
@@ -82,20 +82,18 @@ __device__ __forceinline__ float2 shfl_down2(float2 v, int d)
     return make_float2(__shfl_down_sync(0xffffffffu, v.x, d), __shfl_down_sync(0xffffffffu, v.y, d));
 }
 
-// 9-tap stencil along the channel for the pair (c, c+1) held by this lane; lanes hold
-// consecutive pairs, so offsets -4..+5 live in lanes -2..+2
-__device__ __forceinline__ float2 lsf_pair(float2 v, const float *h)
+// 9-tap symmetric stencil (h[4 - j] = h[4 + j]) along the channel for the pair (c, c+1) held by
+// this lane; lanes hold consecutive pairs, so offsets -4..+5 live in lanes -2..+2.  Even offsets
+// use the lanes' aligned pairs, odd offsets the straddling ones; packed fp32x2 arithmetic.
+// hp[j] = (h[4 + j], h[4 + j]).
+__device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned long long *hp)
 {
     const float2 m2 = shfl_up2(v, 2), m1 = shfl_up2(v, 1), p1 = shfl_down2(v, 1), p2 = shfl_down2(v, 2);
-    float2 o;
-    o.x = h[0] * m2.x;
-    o.x = fmaf(h[1], m2.y, o.x); o.x = fmaf(h[2], m1.x, o.x); o.x = fmaf(h[3], m1.y, o.x);
-    o.x = fmaf(h[4], v.x, o.x);  o.x = fmaf(h[5], v.y, o.x);  o.x = fmaf(h[6], p1.x, o.x);
-    o.x = fmaf(h[7], p1.y, o.x); o.x = fmaf(h[8], p2.x, o.x);
-    o.y = h[0] * m2.y;
-    o.y = fmaf(h[1], m1.x, o.y); o.y = fmaf(h[2], m1.y, o.y); o.y = fmaf(h[3], v.x, o.y);
-    o.y = fmaf(h[4], v.y, o.y);  o.y = fmaf(h[5], p1.x, o.y); o.y = fmaf(h[6], p1.y, o.y);
-    o.y = fmaf(h[7], p2.x, o.y); o.y = fmaf(h[8], p2.y, o.y);
+    unsigned long long o = fmul2(hp[0], pack2(v.x, v.y));
+    o = ffma2(hp[2], pack2(m1.x + p1.x, m1.y + p1.y), o);
+    o = ffma2(hp[4], pack2(m2.x + p2.x, m2.y + p2.y), o);
+    o = ffma2(hp[1], pack2(m1.y + v.y, v.x + p1.x), o);        // offsets -1, +1
+    o = ffma2(hp[3], pack2(m2.y + p1.y, m1.x + p2.x), o);      // offsets -3, +3
     return o;
 }
 
@@ -117,28 +115,28 @@ k_march(const __grid_constant__ MarchParams P)
         if (c_ok && s < P.n_steps) return __ldcs(reinterpret_cast<const float2 *>(src + (size_t)s * P.step_stride));
         return make_float2(0.0f, 0.0f);
     };
-    float2 acc[15], pf[5];
+    unsigned long long acc[15], g2[15], hp[5];
+    float2 pf[5];
 #pragma unroll
-    for (int i = 0; i < 15; ++i) acc[i] = make_float2(0.0f, 0.0f);
+    for (int i = 0; i < 15; ++i) { acc[i] = 0ull; g2[i] = pack2(P.g[i], P.g[i]); }
 #pragma unroll
-    for (int i = 0; i < 5; ++i) pf[i] = load(i);
+    for (int i = 0; i < 5; ++i) { hp[i] = pack2(P.h[4 + i], P.h[4 + i]); pf[i] = load(i); }
     for (int s0 = 0; s0 < P.n_steps + 7; s0 += 15) {
 #pragma unroll
         for (int u = 0; u < 15; ++u) {
             const int s = s0 + u;
-            float2 v = pf[u % 5];
+            const float2 raw = pf[u % 5];
             pf[u % 5] = load(s + 5);
-            if (LSF) v = lsf_pair(v, P.h);
+            const unsigned long long v = LSF ? lsf_pair(raw, hp) : pack2(raw.x, raw.y);
 #pragma unroll
             for (int d = -7; d <= 7; ++d) {
                 const int slot = (u - d + 15) % 15;           // output s - d
-                acc[slot].x = fmaf(P.g[d + 7], v.x, acc[slot].x);
-                acc[slot].y = fmaf(P.g[d + 7], v.y, acc[slot].y);
+                acc[slot] = ffma2(g2[d + 7], v, acc[slot]);
             }
             const int o = s - 7, so = (u + 8) % 15;           // output o is complete
             if (st_ok && o >= 0 && o < P.n_steps)
-                __stcs(reinterpret_cast<float2 *>(dst + (size_t)o * P.step_stride), acc[so]);
-            acc[so] = make_float2(0.0f, 0.0f);
+                __stcs(reinterpret_cast<float2 *>(dst + (size_t)o * P.step_stride), unpack2(acc[so]));
+            acc[so] = 0ull;
         }
     }
 }
@@ -157,8 +155,11 @@ k_lsf_rows(const __grid_constant__ MarchParams P)
     const size_t off = (size_t)row * P.n_c + (size_t)(c_ok ? c : 0);
     float2 v = make_float2(0.0f, 0.0f);
     if (c_ok) v = __ldcs(reinterpret_cast<const float2 *>(P.in + off));
-    v = lsf_pair(v, P.h);
-    if (c_ok && lane >= 2 && lane < 30) __stcs(reinterpret_cast<float2 *>(P.out + off), v);
+    unsigned long long hp[5];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) hp[i] = pack2(P.h[4 + i], P.h[4 + i]);
+    const unsigned long long o = lsf_pair(v, hp);
+    if (c_ok && lane >= 2 && lane < 30) __stcs(reinterpret_cast<float2 *>(P.out + off), unpack2(o));
 }
 
 static void centre_taps(const Taps &t, int width, float *dst)

@@ -2,7 +2,8 @@
 //   K1  k_rotate_bin        rotate, project, bin  (fp32, fixed order)
 //   K2  k_sort_*            stable LSD radix sort of (key, index)            (8(a) row 3)
 //       k_segment_offsets   seg_off[s] = lower_bound(sorted keys, s)  -- no atomics anywhere
-//       k_scan_units        work units (chunks of <= kChunk particles) per spaxel, partial rows
+//       k_unit_tile_totals, k_scan_units   work units (chunks of <= kChunk particles) per spaxel,
+//                           partial rows: tiled three-way exclusive scan
 //       k_build_units       unit descriptors
 //   K2c k_prepare_records   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
 #include "common.cuh"
@@ -164,83 +165,117 @@ k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s
     seg_off[s] = (int32_t)lo;
 }
 
-// Single CTA: three exclusive scans over the spaxels in one sweep, kScanItems spaxels per thread.
+// Three exclusive scans over the spaxels, two small kernels, kScanTile spaxels per CTA:
 //   unit_off: max(1, chunks(s))     part_off: chunks(s) if > 1 else 0     multi index: chunks(s) > 1
-// totals = { n_units, n_part_rows, n_multi }
-constexpr int kScanItems = 8;
+// k_unit_tile_totals writes the three sums of every tile; k_scan_units adds the sums of the tiles
+// before its own (a few hundred values at most) and scans its tile.  totals = { n_units,
+// n_part_rows, n_multi }.
+constexpr int kScanItems = 4;
+constexpr int kScanThreads = 256;
+constexpr int kScanTile = kScanItems * kScanThreads;
 
-__global__ void __launch_bounds__(1024)
-k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restrict__ unit_off,
-             int32_t *__restrict__ part_off, int32_t *__restrict__ multi_list,
-             int32_t *__restrict__ totals)
+__device__ __forceinline__ void unit_counts(const int32_t *__restrict__ seg_off, int32_t n_s, int s0,
+                                            int32_t (&chunks)[kScanItems], int32_t (&tot)[3])
 {
-    __shared__ int32_t wsum[3][32];
-    __shared__ int32_t carry[3];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x < 3) carry[threadIdx.x] = 0;
-    __syncthreads();
-    for (int base = 0; base < n_s; base += 1024 * kScanItems) {
-        const int s0 = base + threadIdx.x * kScanItems;
-        int32_t chunks[kScanItems];
-        int32_t tot[3] = {0, 0, 0};
-        int32_t prev = s0 <= n_s ? seg_off[s0] : 0;
+    tot[0] = tot[1] = tot[2] = 0;
+    int32_t prev = s0 <= n_s ? seg_off[s0] : 0;
 #pragma unroll
-        for (int i = 0; i < kScanItems; ++i) {
-            const int s = s0 + i;
-            chunks[i] = -1;
-            if (s < n_s) {
-                const int32_t next = seg_off[s + 1];
-                chunks[i] = (next - prev + kChunk - 1) / kChunk;
-                prev = next;
-                tot[0] += chunks[i] > 1 ? chunks[i] : 1;
-                tot[1] += chunks[i] > 1 ? chunks[i] : 0;
-                tot[2] += chunks[i] > 1 ? 1 : 0;
-            }
+    for (int i = 0; i < kScanItems; ++i) {
+        const int s = s0 + i;
+        chunks[i] = -1;
+        if (s < n_s) {
+            const int32_t next = seg_off[s + 1];
+            chunks[i] = (next - prev + kChunk - 1) / kChunk;
+            prev = next;
+            tot[0] += chunks[i] > 1 ? chunks[i] : 1;
+            tot[1] += chunks[i] > 1 ? chunks[i] : 0;
+            tot[2] += chunks[i] > 1 ? 1 : 0;
         }
-        int32_t inc[3];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            inc[q] = tot[q];
-            for (int o = 1; o < 32; o <<= 1) {
-                const int32_t t = __shfl_up_sync(0xffffffffu, inc[q], o);
-                if (lane >= o) inc[q] += t;
-            }
-            if (lane == 31) wsum[q][warp] = inc[q];
-        }
-        __syncthreads();
-        int32_t ex[3];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            int32_t wpre = 0;
-            for (int w = 0; w < warp; ++w) wpre += wsum[q][w];
-            ex[q] = carry[q] + wpre + inc[q] - tot[q];
-        }
-        int32_t run[3] = {ex[0], ex[1], ex[2]};
-#pragma unroll
-        for (int i = 0; i < kScanItems; ++i) {
-            if (chunks[i] >= 0) {
-                const int s = s0 + i;
-                unit_off[s] = run[0];
-                part_off[s] = run[1];
-                if (chunks[i] > 1) multi_list[run[2]] = s;
-                run[0] += chunks[i] > 1 ? chunks[i] : 1;
-                run[1] += chunks[i] > 1 ? chunks[i] : 0;
-                run[2] += chunks[i] > 1 ? 1 : 0;
-            }
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) {
-#pragma unroll
-            for (int q = 0; q < 3; ++q) carry[q] = run[q];
-        }
-        __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        unit_off[n_s] = carry[0];
-        part_off[n_s] = carry[1];
-        totals[0] = carry[0];
-        totals[1] = carry[1];
-        totals[2] = carry[2];
+}
+
+// block-wide sums of v[0..2]; every thread gets the results
+__device__ __forceinline__ void block_sum3(int32_t (&v)[3], int32_t (*sm)[kScanThreads / 32])
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+        if (lane == 0) sm[q][warp] = v[q];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        v[q] = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) v[q] += sm[q][w];
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_unit_tile_totals(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restrict__ tile_tot)
+{
+    __shared__ int32_t sm[3][kScanThreads / 32];
+    int32_t chunks[kScanItems], tot[3];
+    unit_counts(seg_off, n_s, blockIdx.x * kScanTile + threadIdx.x * kScanItems, chunks, tot);
+    block_sum3(tot, sm);
+    if (threadIdx.x < 3) tile_tot[3 * blockIdx.x + threadIdx.x] = tot[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__restrict__ tile_tot,
+             int32_t *__restrict__ unit_off, int32_t *__restrict__ part_off,
+             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals)
+{
+    __shared__ int32_t sm[3][kScanThreads / 32];
+    __shared__ int32_t wsum[3][kScanThreads / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // sums of the tiles before this one (and, in the last CTA, of all tiles)
+    int32_t before[3] = {0, 0, 0};
+    for (int t = threadIdx.x; t < (int)blockIdx.x; t += kScanThreads) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) before[q] += tile_tot[3 * t + q];
+    }
+    block_sum3(before, sm);
+    const int s0 = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+    int32_t chunks[kScanItems], tot[3], inc[3];
+    unit_counts(seg_off, n_s, s0, chunks, tot);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        inc[q] = tot[q];
+        for (int o = 1; o < 32; o <<= 1) {
+            const int32_t t = __shfl_up_sync(0xffffffffu, inc[q], o);
+            if (lane >= o) inc[q] += t;
+        }
+        if (lane == 31) wsum[q][warp] = inc[q];
+    }
+    __syncthreads();
+    int32_t run[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        int32_t wpre = 0;
+        for (int w = 0; w < warp; ++w) wpre += wsum[q][w];
+        run[q] = before[q] + wpre + inc[q] - tot[q];
+    }
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (chunks[i] >= 0) {
+            const int s = s0 + i;
+            unit_off[s] = run[0];
+            part_off[s] = run[1];
+            if (chunks[i] > 1) multi_list[run[2]] = s;
+            run[0] += chunks[i] > 1 ? chunks[i] : 1;
+            run[1] += chunks[i] > 1 ? chunks[i] : 0;
+            run[2] += chunks[i] > 1 ? 1 : 0;
+        }
+    }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == kScanThreads - 1) {   // holds the grand totals
+        unit_off[n_s] = run[0];
+        part_off[n_s] = run[1];
+        totals[0] = run[0];
+        totals[1] = run[1];
+        totals[2] = run[2];
     }
 }
 
@@ -406,6 +441,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_partoff = take(((size_t)n_s + 1) * 4);
     L.off_multi = take((size_t)L.max_multi * 4);
     L.off_totals = take(16);
+    L.off_tiletot = take(((size_t)n_s / kScanTile + 1) * 3 * 4);
     L.off_units = take((size_t)L.max_units * sizeof(Unit));
     L.off_rec = take(nn * sizeof(Rec));
     L.off_partials = take((size_t)L.max_part_rows * (size_t)n_c * 4);
@@ -482,8 +518,14 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     const int32_t *perm = pbuf[L.final_buf];
     k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, seg);
     RUBIX_LAUNCH_CHECK();
-    k_scan_units<<<1, 1024, 0, st>>>(seg, n_s, unit_off, part_off, multi, totals);
-    RUBIX_LAUNCH_CHECK();
+    {
+        int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
+        const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
+        k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot);
+        RUBIX_LAUNCH_CHECK();
+        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot, unit_off, part_off, multi, totals);
+        RUBIX_LAUNCH_CHECK();
+    }
     k_build_units<<<(unsigned)((L.max_units + 255) / 256), 256, 0, st>>>(seg, unit_off, part_off, n_s, units);
     RUBIX_LAUNCH_CHECK();
     if (n > 0) {

@@ -51,25 +51,6 @@ constexpr int kAccWarps = kAccThreads / 32;
 constexpr int kAccDepth = RUBIX_ACC_DEPTH;           // load sets (passes) in flight per warp
 constexpr int kAccMinBlocks = RUBIX_ACC_MINB;
 
-// ---- packed fp32x2 arithmetic (sm_100+): one issue slot, two FMAs ------------------------------
-__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
-{
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
-{
-    unsigned long long d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ unsigned long long fmul2(unsigned long long a, unsigned long long b)
-{
-    unsigned long long d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
 // (a & b) | c in one LOP3 (b, c stay in registers)
 __device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c)
 {
