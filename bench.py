@@ -36,6 +36,9 @@ METRIC = "particle_channel_samples_per_s"
 UNIT = "G particle*channel/s"
 # four corner templates x 4 B x (dl_obs / dl_ssp) SSP samples per channel
 GATHER_BYTES_PER_SAMPLE = lambda tel, ssp: 16.0 * float(tel.dlambda) / float(ssp.dlambda)
+# DRAM bytes of one k_accumulate launch on the medium workload, from the committed ncu --set full
+# capture (profiles/r01_full_medium.md): 0.053 GB read + 1.347 GB written
+NCU_DRAM_BYTES_K_ACCUMULATE = 1.400e9
 
 
 def parse():
@@ -47,6 +50,7 @@ def parse():
     ap.add_argument("--workload", default="medium", choices=["tiny", "small", "medium", "contention"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-adjoint", action="store_true")
     return ap.parse_args()
 
 
@@ -169,6 +173,38 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def time_adjoint(B, synth, dev, reps=10):
+    """rubix_cube_adjoint on BASELINE.json configs[4]: the config-1 galaxy with
+    config-2 PSF/LSF, upstream gradient 2 (cube - target); reported beside the headline step."""
+    import torch
+    w = synth.make_workload("adjoint")
+    other = synth.make_workload("adjoint")
+    other.particles = synth.make_particles_for("adjoint", seed=synth.ADJOINT_TARGET_SEED)
+    dw, dt = B.DeviceWorkload(w, device=dev), B.DeviceWorkload(other, device=dev)
+    grad = (2.0 * (dw.forward() - dt.forward())).contiguous()
+    for _ in range(3):
+        dw.adjoint(grad)
+    torch.cuda.synchronize()
+    B.rubix_stage_timing_enable(True)
+    B.rubix_stage_timing_read()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        dw.adjoint(grad)
+    e1.record()
+    torch.cuda.synchronize()
+    st = B.rubix_stage_timing_read()
+    B.rubix_stage_timing_enable(False)
+    t, n = w.telescope, w.particles.n
+    k_ms = st["adjoint"]["ms"] / max(st["adjoint"]["calls"], 1)
+    gather_b = 32.0 * n * t.n_channels                    # 4 corners x (T[j], T[j+1]) x 4 B per sample
+    return {"workload": "adjoint: BASELINE.json configs[4] (100k particles, 25x25x3700, PSF 15x15 + LSF 9)",
+            "ms_per_call": e0.elapsed_time(e1) / reps, "k_adjoint_ms": k_ms,
+            "value": n * t.n_channels / (e0.elapsed_time(e1) / reps * 1e-3) / 1e9, "unit": UNIT,
+            "note": "k_adjoint reads 8 template samples per (particle, channel) through L1 (32 B algorithmic)",
+            "l1_gather_gbs": gather_b / (k_ms * 1e-3) / 1e9}
+
+
 # ------------------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
@@ -275,9 +311,20 @@ def run_ours(args):
     gather_b = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * samples_per_step
     hbm_b = t.n_spaxels * t.n_channels * 4.0 + w.ssp.flux.size * 4.0 + 48.0 * n
     achieved = gather_b / (acc_ms * 1e-3) / 1e9
+    # L1 data-pipe view (the unit ncu shows saturated, profiles/r01_full_medium.md): bytes the SM's
+    # load/store pipe must carry per particle = 4 corner windows (LDG) + table store (STS) + two
+    # table reads per channel (LDS); peak = 148 SMs x 128 B/clk x max SM clock (nominal)
+    win = float(t.n_channels) * float(t.dlambda) / float(w.ssp.dlambda)
+    l1_b = (16.0 * win + 4.0 * win + 8.0 * t.n_channels) * n
+    l1_peak = 148 * 128 * 1.965
     roofline = {"kernel": "k_accumulate (steps 4-6)", "bound": "l2", "achieved": achieved,
                 "peak": onchip["l2_gbs"], "unit": "GB/s", "frac": achieved / onchip["l2_gbs"],
-                "traffic": None,
+                "traffic": NCU_DRAM_BYTES_K_ACCUMULATE if args.workload == "medium" else None,
+                "traffic_source": "profiles/r01_full_medium.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
+                "l1_view": {"bound": "l1 data pipe", "achieved": l1_b / (acc_ms * 1e-3) / 1e9, "peak": l1_peak,
+                            "unit": "GB/s", "frac": l1_b / (acc_ms * 1e-3) / 1e9 / l1_peak,
+                            "peak_source": "nominal 148 SMs x 128 B/clk x 1.965 GHz",
+                            "algorithmic_bytes_per_launch": l1_b},
                 "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks "
                                "(MEASURED_PEAKS.json has no L2 figure; SURVEY.md 8(d))",
                 "algorithmic_bytes_per_launch": gather_b, "kernel_ms": acc_ms,
@@ -293,6 +340,11 @@ def run_ours(args):
                                "frac": conv_b / (stage_ms["psf_lsf"] * 1e-3) / 1e9 / hbm_peak,
                                "algorithmic_bytes_per_launch": conv_b, "kernel_ms": stage_ms["psf_lsf"]}
 
+    adjoint_info = None
+    if not args.no_adjoint:
+        del scratch
+        adjoint_info = time_adjoint(B, synth, dev)
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -301,6 +353,8 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "api": "rubix_forward_host (pinned host buffers)"},
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
             "stage_ms": stage_ms, "roofline": roofline}
+    if adjoint_info is not None:
+        line["adjoint"] = adjoint_info
 
     if not args.no_cpu_baseline:
         import oracle

@@ -97,8 +97,16 @@ __device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned 
     return o;
 }
 
+#ifndef RUBIX_MARCH_PF
+#define RUBIX_MARCH_PF 5
+#endif
+#ifndef RUBIX_MARCH_MINB
+#define RUBIX_MARCH_MINB 4
+#endif
+constexpr int kMarchPf = RUBIX_MARCH_PF;          // steps prefetched per thread (divides 15)
+
 template <bool LSF>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, RUBIX_MARCH_MINB)
 k_march(const __grid_constant__ MarchParams P)
 {
     const int lane = threadIdx.x & 31;
@@ -116,17 +124,19 @@ k_march(const __grid_constant__ MarchParams P)
         return make_float2(0.0f, 0.0f);
     };
     unsigned long long acc[15], g2[15], hp[5];
-    float2 pf[5];
+    float2 pf[kMarchPf];
 #pragma unroll
     for (int i = 0; i < 15; ++i) { acc[i] = 0ull; g2[i] = pack2(P.g[i], P.g[i]); }
 #pragma unroll
-    for (int i = 0; i < 5; ++i) { hp[i] = pack2(P.h[4 + i], P.h[4 + i]); pf[i] = load(i); }
+    for (int i = 0; i < 5; ++i) hp[i] = pack2(P.h[4 + i], P.h[4 + i]);
+#pragma unroll
+    for (int i = 0; i < kMarchPf; ++i) pf[i] = load(i);
     for (int s0 = 0; s0 < P.n_steps + 7; s0 += 15) {
 #pragma unroll
         for (int u = 0; u < 15; ++u) {
             const int s = s0 + u;
-            const float2 raw = pf[u % 5];
-            pf[u % 5] = load(s + 5);
+            const float2 raw = pf[u % kMarchPf];
+            pf[u % kMarchPf] = load(s + kMarchPf);
             const unsigned long long v = LSF ? lsf_pair(raw, hp) : pack2(raw.x, raw.y);
 #pragma unroll
             for (int d = -7; d <= 7; ++d) {
