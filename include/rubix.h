@@ -76,7 +76,21 @@ typedef struct {
     float psf_sigma;                /* spaxels, > 0 when psf_size > 0                       */
     int32_t lsf_size;               /* odd taps <= 63 along the channel axis; 0 = LSF off   */
     float lsf_sigma;                /* channels, > 0 when lsf_size > 0                      */
+    int32_t resample;               /* RUBIX_RESAMPLE_POINT (0) or RUBIX_RESAMPLE_FLUX (1)  */
 } rubix_telescope;
+
+/* Resampling rule of step 5 ("Additional resampling is performed to match the
+ * wavelength grid of the observed telescope"; the paper does not say which rule):
+ *   RUBIX_RESAMPLE_POINT  F[k] = S~(lambda_k / (1+beta)): the piecewise-linear interpolant of the
+ *                         blended SSP samples, point-sampled at the channel centre (SURVEY.md
+ *                         8(c) row 5, numpy.interp with left = right = 0);
+ *   RUBIX_RESAMPLE_FLUX   F[k] = (1/dlambda_obs) * integral of S~(lambda / (1+beta)) over the bin
+ *                         [lambda_k - dlambda_obs/2, lambda_k + dlambda_obs/2], S~ = 0 outside the
+ *                         SSP coverage (sum_k F[k] dlambda_obs telescopes to the
+ *                         total flux exactly).  Forward only: rubix_cube_adjoint returns
+ *                         RUBIX_ERR_UNSUPPORTED for it. */
+#define RUBIX_RESAMPLE_POINT 0
+#define RUBIX_RESAMPLE_FLUX 1
 
 /* Bytes of DEVICE scratch that any of the three compute calls below may need for this problem
  * size (the maximum over the three).  Returns 0 on invalid arguments (rubix_last_error says

@@ -107,12 +107,14 @@ def ssp_cells(log_age, log_z, age_axis, z_axis):
 
 
 def particle_spectrum(mass, log_age, log_z, vlos, ssp, tel):
+    """One particle's spectrum on the observed grid; ``tel.resample`` picks the rule of step 5
+    (0 point-sampled, 1 flux-conserving bin average)."""
     flux = _f32(ssp.flux)
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    _load().orc_particle_spectrum(
-        C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
+    _load().orc_particle_spectrum_mode(
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
         C.c_float(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
@@ -152,8 +154,8 @@ def build_cube(particles, R, ssp, tel, sel=None):
         sel_arr = np.ascontiguousarray(sel, dtype=np.int32)
         n_sel = sel_arr.size
         cube = np.empty((n_sel, n_c), np.float64)
-    _load().orc_build_cube(
-        C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
+    _load().orc_build_cube_mode(
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
         C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis),
         C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_x), C.c_int32(tel.n_y), C.c_float(float(tel.spaxel_size)),

@@ -27,7 +27,9 @@
  * the line-centroid shift lambda(1+v/c) (Doppler/resample); superposition, permutation
  * invariance, flux conservation, brute-force Python loops (accumulate); delta response,
  * scipy.ndimage.convolve1d, numpy.convolve, flux conservation (PSF/LSF); central finite
- * differences, the dot-product test and the linear-template closed form (adjoint).
+ * differences, the dot-product test and the linear-template closed form (adjoint);
+ * the prefix-integral formulation, constant / linear templates, the (1,6,1)/8 identity and
+ * exact total-flux telescoping (flux-conserving resampling, tests/test_oracle_fluxcons.py).
  * No function here is "parity unpinned".
  *
  * No blocking, fusion or reordering beyond the definitions; the only parallelism is an
@@ -158,6 +160,84 @@ static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, do
     }
 }
 
+/* ------------------------------------------------------------------------------------
+ * Step 5, flux-conserving variant ("Additional resampling is
+ * performed to match the wavelength grid of the observed telescope"; reading R13).
+ * Channel k is the bin [lambda_k - dl_obs/2, lambda_k + dl_obs/2]; its value is the bin AVERAGE
+ * of the Doppler-shifted spectrum,
+ *   F[k] = (1/dl_obs) * integral over the bin of S~(lambda / (1 + beta)) d lambda,
+ * where S~ is the piecewise-linear interpolant of the blended samples S(j) on the SSP
+ * coverage and 0 outside it.  In SSP-sample units x = (lambda/(1+beta) - l0_ssp)/dl_ssp the
+ * bin is [x_lo, x_hi] with x_hi - x_lo = B = dl_obs / ((1+beta) dl_ssp) and
+ *   F[k] = (1/B) * integral_{x_lo}^{x_hi} S~(x) dx.
+ * The integral is taken exactly, one knot interval at a time (a trapezoid is exact for a
+ * linear piece).  No 1/(1+beta) flux-density factor, as in the point-sampled variant.
+ * ------------------------------------------------------------------------------------ */
+static void particle_spectrum_flux(double mass, int32_t ia, int32_t iz, double ta, double tz,
+                                   double vlos, const float *flux, int32_t n_z, int32_t n_lambda,
+                                   double l0_ssp, double dl_ssp, int32_t k_begin, int32_t k_end,
+                                   double l0_obs, double dl_obs, double *F)
+{
+    const float *T00 = flux + ((int64_t)ia * n_z + iz) * n_lambda;
+    const float *T10 = flux + ((int64_t)(ia + 1) * n_z + iz) * n_lambda;
+    const float *T01 = flux + ((int64_t)ia * n_z + iz + 1) * n_lambda;
+    const float *T11 = flux + ((int64_t)(ia + 1) * n_z + iz + 1) * n_lambda;
+    const double w00 = (1.0 - ta) * (1.0 - tz), w10 = ta * (1.0 - tz);
+    const double w01 = (1.0 - ta) * tz, w11 = ta * tz;
+    const double beta = vlos / ORC_C_KMS;
+    const double x_last = (double)(n_lambda - 1);
+    const double B = dl_obs / ((1.0 + beta) * dl_ssp);
+    for (int32_t k = k_begin; k < k_end; ++k) {
+        const double lam_c = l0_obs + dl_obs * (double)k;
+        double x_lo = ((lam_c - 0.5 * dl_obs) / (1.0 + beta) - l0_ssp) / dl_ssp;
+        double x_hi = ((lam_c + 0.5 * dl_obs) / (1.0 + beta) - l0_ssp) / dl_ssp;
+        if (x_lo < 0.0) x_lo = 0.0;
+        if (x_hi > x_last) x_hi = x_last;
+        double total = 0.0, pos = x_lo;
+        while (pos < x_hi) {
+            int32_t j = (int32_t)floor(pos);
+            if (j > n_lambda - 2) j = n_lambda - 2;
+            double next = (double)(j + 1);
+            if (next > x_hi) next = x_hi;
+            const double s0 = mass * (w00 * T00[j] + w10 * T10[j] + w01 * T01[j] + w11 * T11[j]);
+            const double s1 = mass * (w00 * T00[j + 1] + w10 * T10[j + 1] + w01 * T01[j + 1]
+                                      + w11 * T11[j + 1]);
+            const double va = s0 + (pos - (double)j) * (s1 - s0);
+            const double vb = s0 + (next - (double)j) * (s1 - s0);
+            total += 0.5 * (next - pos) * (va + vb);
+            pos = next;
+        }
+        F[k] = total / B;
+    }
+}
+
+/* mode 0: point-sampled linear interpolation; mode 1: bin average */
+static void particle_spectrum_mode(int32_t mode, double mass, int32_t ia, int32_t iz, double ta,
+                                   double tz, double vlos, const float *flux, int32_t n_z,
+                                   int32_t n_lambda, double l0_ssp, double dl_ssp, int32_t k_begin,
+                                   int32_t k_end, double l0_obs, double dl_obs, double *F)
+{
+    if (mode == 1)
+        particle_spectrum_flux(mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp, dl_ssp,
+                               k_begin, k_end, l0_obs, dl_obs, F);
+    else
+        particle_spectrum(mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp, dl_ssp, k_begin,
+                          k_end, l0_obs, dl_obs, F, 0);
+}
+
+void orc_particle_spectrum_mode(int32_t mode, float mass, float log_age, float log_z, float vlos,
+                                int32_t n_age, int32_t n_z, int32_t n_lambda, const float *age_axis,
+                                const float *z_axis, float l0_ssp, float dl_ssp, const float *flux,
+                                int32_t n_c, float l0_obs, float dl_obs, double *F)
+{
+    int32_t ia, iz;
+    double ta, tz;
+    axis_cell(age_axis, n_age, log_age, &ia, &ta);
+    axis_cell(z_axis, n_z, log_z, &iz, &tz);
+    particle_spectrum_mode(mode, (double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
+                           (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs, (double)dl_obs, F);
+}
+
 void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, int32_t n_age,
                            int32_t n_z, int32_t n_lambda, const float *age_axis,
                            const float *z_axis, float l0_ssp, float dl_ssp, const float *flux,
@@ -193,12 +273,12 @@ void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double
  * If n_sel > 0 only the listed spaxels are computed and cube is [n_sel][n_c]; otherwise
  * cube is [n_s][n_c].  Particles are visited in the stable order of step 3.
  * ------------------------------------------------------------------------------------ */
-void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *mass,
-                    const float *log_age, const float *log_z, const float *R, int32_t n_age,
-                    int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
-                    float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
-                    float spaxel, int32_t n_c, float l0_obs, float dl_obs, const int32_t *sel,
-                    int32_t n_sel, double *cube)
+void orc_build_cube_mode(int32_t mode, int64_t n, const float *pos, const float *vel, const float *mass,
+                         const float *log_age, const float *log_z, const float *R, int32_t n_age,
+                         int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
+                         float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
+                         float spaxel, int32_t n_c, float l0_obs, float dl_obs, const int32_t *sel,
+                         int32_t n_sel, double *cube)
 {
     const int32_t n_s = n_x * n_y;
     int32_t *key = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
@@ -229,15 +309,26 @@ void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *
                     double ta, tz;
                     axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
                     axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
-                    particle_spectrum((double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux, n_z,
-                                      n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke,
-                                      (double)l0_obs, (double)dl_obs, F, 0);
+                    particle_spectrum_mode(mode, (double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux,
+                                           n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke,
+                                           (double)l0_obs, (double)dl_obs, F);
                     for (int32_t k = kb; k < ke; ++k) row[k] += F[k];
                 }
             }
         free(F);
     }
     free(key); free(perm); free(seg); free(vlos);
+}
+
+void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *mass,
+                    const float *log_age, const float *log_z, const float *R, int32_t n_age,
+                    int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
+                    float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
+                    float spaxel, int32_t n_c, float l0_obs, float dl_obs, const int32_t *sel,
+                    int32_t n_sel, double *cube)
+{
+    orc_build_cube_mode(0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
+                        l0_ssp, dl_ssp, flux, n_x, n_y, spaxel, n_c, l0_obs, dl_obs, sel, n_sel, cube);
 }
 
 /* ------------------------------------------------------------------------------------

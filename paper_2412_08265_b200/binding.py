@@ -47,7 +47,7 @@ class CTelescope(C.Structure):
     _fields_ = [("n_x", C.c_int32), ("n_y", C.c_int32), ("spaxel_size", C.c_float),
                 ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
-                ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float)]
+                ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32)]
 
 
 _lib = None
@@ -132,7 +132,8 @@ class _Keep:
 def c_telescope(tel) -> _Keep:
     return _Keep(CTelescope(int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
                             float(tel.lambda0), float(tel.dlambda), int(tel.psf_size),
-                            float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma)))
+                            float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma),
+                            int(getattr(tel, "resample", 0))))
 
 
 def c_ssp(ssp, flux) -> _Keep:

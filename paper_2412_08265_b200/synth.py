@@ -179,6 +179,7 @@ class Telescope:
     psf_sigma: np.float32 = np.float32(0.0)   # spaxels
     lsf_size: int = 0         # odd taps; 0 = off
     lsf_sigma: np.float32 = np.float32(0.0)   # channels
+    resample: int = 0         # 0 = point-sampled linear interpolation, 1 = flux-conserving bin average
 
     @property
     def n_spaxels(self) -> int:
