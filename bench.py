@@ -340,6 +340,38 @@ def run_ours(args):
                                "frac": conv_b / (stage_ms["psf_lsf"] * 1e-3) / 1e9 / hbm_peak,
                                "algorithmic_bytes_per_launch": conv_b, "kernel_ms": stage_ms["psf_lsf"]}
 
+    # ---- SURVEY.md 8(f)-1 variant: the same step with flux-conserving resampling (RUBIX_RESAMPLE_FLUX)
+    import dataclasses
+    wf = dataclasses.replace(w, telescope=dataclasses.replace(t, resample=1))
+    dwf = B.DeviceWorkload(wf, device=dev)
+    cube_f = torch.empty(dw.shape, dtype=torch.float32, device=dev)
+    final_f = torch.empty_like(cube_f)
+
+    def step_flux():
+        B.rubix_build_cube(dwf.particles, dwf.ssp, dwf.tel, dwf.R, cube_f, dwf.workspace)
+        if has_conv:
+            B.rubix_convolve_psf_lsf(dwf.tel, cube_f, final_f, dwf.workspace)
+
+    for _ in range(3):
+        step_flux()
+    barrier()
+    B.rubix_stage_timing_enable(True)
+    B.rubix_stage_timing_read()
+    e0.record()
+    for _ in range(10):
+        step_flux()
+    e1.record()
+    barrier()
+    st_f = B.rubix_stage_timing_read()
+    B.rubix_stage_timing_enable(False)
+    flux_ms = e0.elapsed_time(e1) / 10
+    flux_acc_ms = st_f["accumulate"]["ms"] / max(st_f["accumulate"]["calls"], 1)
+    flux_variant = {"what": "same workload with RUBIX_RESAMPLE_FLUX (flux-conserving bin average, SURVEY.md 8(f)-1)",
+                    "ms_per_step": flux_ms, "k_accumulate_ms": flux_acc_ms,
+                    "value": samples_per_step / (flux_ms * 1e-3) / 1e9, "unit": UNIT,
+                    "l2_frac": gather_b / (flux_acc_ms * 1e-3) / 1e9 / onchip["l2_gbs"]}
+    del dwf, cube_f, final_f
+
     adjoint_info = None
     if not args.no_adjoint:
         del scratch
@@ -353,6 +385,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "api": "rubix_forward_host (pinned host buffers)"},
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
             "stage_ms": stage_ms, "roofline": roofline}
+    line["flux_variant"] = flux_variant
     if adjoint_info is not None:
         line["adjoint"] = adjoint_info
 

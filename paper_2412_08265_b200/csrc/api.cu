@@ -69,6 +69,8 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_INVALID_ARG, "spaxel_size must be > 0");
     if (!(t->dlambda > 0.0f) || !isfinite(t->dlambda) || !isfinite(t->lambda0))
         return fail(RUBIX_ERR_INVALID_ARG, "telescope dlambda must be > 0 and finite");
+    if (t->resample != RUBIX_RESAMPLE_POINT && t->resample != RUBIX_RESAMPLE_FLUX)
+        return fail(RUBIX_ERR_INVALID_ARG, "resample must be RUBIX_RESAMPLE_POINT (0) or RUBIX_RESAMPLE_FLUX (1)");
     const int sz[2] = {t->psf_size, t->lsf_size};
     const float sg[2] = {t->psf_sigma, t->lsf_sigma};
     for (int i = 0; i < 2; ++i) {
@@ -206,6 +208,8 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
     if (!R || !grad_cube) return fail(RUBIX_ERR_NULL, "R or grad_cube is NULL");
     if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
         return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
+    if (tel->resample != RUBIX_RESAMPLE_POINT)
+        return fail(RUBIX_ERR_UNSUPPORTED, "rubix_cube_adjoint supports RUBIX_RESAMPLE_POINT only");
     if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
     const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
                                  ssp->n_lambda);

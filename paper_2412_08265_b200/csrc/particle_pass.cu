@@ -311,7 +311,7 @@ k_build_units(const int32_t *__restrict__ seg_off, const int32_t *__restrict__ u
 // --------------------------------------------------------------------------------------------
 struct PrepParams {
     AxisParams ax;
-    int32_t n_lambda, pitch, n_c, n_s;
+    int32_t n_lambda, pitch, n_c, n_s, mode;
     float l0_ssp, dl_ssp, l0_obs, dl_obs;
 };
 
@@ -353,22 +353,42 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     const double scale = (double)(1 << kFxFrac);
     const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
     const double B = (double)P.dl_obs * inv / (double)P.dl_ssp;
-    const int64_t a_fx = __double2ll_rn(A * scale);
+    int64_t a_fx = __double2ll_rn(A * scale);
     const uint32_t b_fx = (uint32_t)__double2ll_rn(B * scale);
+    const int64_t b = (int64_t)b_fx;
+    const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
+    int64_t k_lo, k_hi, x_first, x_last;
+    if (P.mode == RUBIX_RESAMPLE_FLUX) {
+        // x_k = a_fx + b k is the LOWER EDGE of bin k (upper edge = lower edge of bin k + 1);
+        // [k_lo, k_hi] = bins that overlap the coverage [0, N_l - 1]
+        a_fx -= (int64_t)(b_fx >> 1);
+        const int64_t t = 1 - a_fx;                        // need a_fx + b (k + 1) >= 1
+        k_lo = t <= 0 ? 0 : (t + b - 1) / b - 1;
+        if (k_lo < 0) k_lo = 0;
+        k_hi = x_max - 1 - a_fx < 0 ? -1 : (x_max - 1 - a_fx) / b;
+        if (k_hi > P.n_c - 1) k_hi = P.n_c - 1;
+        if (k_lo > P.n_c) k_lo = P.n_c;
+        x_first = a_fx + b * k_lo;
+        x_last = a_fx + b * (k_hi + 1);
+        if (x_first < 0) x_first = 0;
+        if (x_last > x_max) x_last = x_max;
+    } else {
+        k_lo = a_fx >= 0 ? 0 : (-a_fx + b - 1) / b;
+        k_hi = a_fx > x_max ? -1 : (x_max - a_fx) / b;
+        if (k_hi > P.n_c - 1) k_hi = P.n_c - 1;
+        if (k_lo > P.n_c) k_lo = P.n_c;
+        x_first = a_fx + b * k_lo;
+        x_last = a_fx + b * k_hi;
+    }
     r.a_fx = a_fx;
     r.b_fx = b_fx;
-    const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
-    int64_t k_lo = a_fx >= 0 ? 0 : (-a_fx + (int64_t)b_fx - 1) / (int64_t)b_fx;
-    int64_t k_hi = a_fx > x_max ? -1 : (x_max - a_fx) / (int64_t)b_fx;
-    if (k_hi > P.n_c - 1) k_hi = P.n_c - 1;
-    if (k_lo > P.n_c) k_lo = P.n_c;
     r.k_lo = (int32_t)k_lo;
     r.k_hi = (int32_t)k_hi;
     r.j0 = 0;
     r.nw = 0;
     if (k_lo <= k_hi) {
-        r.j0 = (int32_t)((a_fx + (int64_t)b_fx * k_lo) >> kFxFrac) & ~(kRowAlign - 1);
-        r.nw = (int32_t)((a_fx + (int64_t)b_fx * k_hi) >> kFxFrac) - r.j0 + 2;   // samples j0 .. j_max + 1
+        r.j0 = (int32_t)(x_first >> kFxFrac) & ~(kRowAlign - 1);
+        r.nw = (int32_t)(x_last >> kFxFrac) - r.j0 + 2;   // samples j0 .. j_max + 1
     }
     rec[i] = r;
 }
@@ -538,6 +558,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.pitch = L.pitch;
         P.n_c = in.tel->n_channels;
         P.n_s = n_s;
+        P.mode = in.tel->resample;
         P.l0_ssp = in.ssp->lambda0;
         P.dl_ssp = in.ssp->dlambda;
         P.l0_obs = in.tel->lambda0;

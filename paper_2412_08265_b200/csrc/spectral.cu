@@ -30,7 +30,7 @@ struct AccumParams {
     const int32_t *totals;
     float *cube;
     float *partials;
-    int32_t pitch, n_z, n_c, n_tiles, wcap;
+    int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
     cudaTextureObject_t tex;
 };
 
@@ -86,13 +86,17 @@ struct Win {                 // one particle's window in one channel tile
     uint32_t b;              // step per channel, 4.28
     int32_t ka, kb;          // channels of this tile inside the SSP coverage (ka > kb: none)
     int32_t first, nw;       // flux index of (corner (i,j), sample j0); samples needed
+    int32_t j0;              // first table sample (multiple of 32)
     float w0, w1, w2, w3;
 };
 
 struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 
 // SINGLE: the whole spectrum is one tile (n_tiles == 1): window (j0, nw) comes from the record.
-template <int CPT, bool SINGLE, int DEPTH, int MINB>
+// FLUX: flux-conserving resampling (RUBIX_RESAMPLE_FLUX): x_k is the lower edge of bin k and the
+// channel value is the exact integral of the table's piecewise-linear interpolant over
+// [x_k, x_{k+1}] (clipped to the SSP coverage), divided by the bin width B.
+template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX>
 __global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
@@ -137,12 +141,17 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 W.kb = min(k_end, rc.y);
                 j0 = 0; W.nw = 0;
                 if (W.ka <= W.kb) {
-                    const int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * W.kb;
+                    int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * (W.kb + (FLUX ? 1 : 0));
+                    if (FLUX) {                             // bins are clipped to the coverage
+                        xa = max(xa, (int64_t)0);
+                        xb = min(xb, (int64_t)(P.n_lambda - 1) << kFxFrac);
+                    }
                     j0 = (int)(xa >> kFxFrac) & ~(kRowAlign - 1);
                     W.nw = (int)(xb >> kFxFrac) - j0 + 2;   // samples j0 .. j_max + 1
                 }
             }
             W.first = rb.x + j0;
+            W.j0 = j0;
             W.base = a + (int64_t)W.b * k0 - ((int64_t)j0 << kFxFrac);
             return W;
         };
@@ -200,8 +209,53 @@ k_accumulate(const __grid_constant__ AccumParams P)
             const float f = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;    // frac(x_k), exact
             acc[i] += fmaf(f, s1 - s0, s0);
         };
+        // exact integral of the table's interpolant over local positions [xl, xh] (12.20), times inv_b
+        auto flux_sample = [&](int i, uint32_t xl, uint32_t xh, float inv_b, const float *tabp) {
+            const uint32_t jl = xl >> 20, jh = xh >> 20;
+            const float fl = (float)(xl & 0xFFFFFu) * (1.0f / 1048576.0f);
+            const float fh = (float)(xh & 0xFFFFFu) * (1.0f / 1048576.0f);
+            const float a0 = tabp[jl], a1 = tabp[jl + 1];
+            float tot;
+            if (jl == jh) {
+                tot = (fh - fl) * fmaf(0.5f * (fl + fh), a1 - a0, a0);
+            } else {
+                const float c0 = tabp[jh], c1 = tabp[jh + 1];
+                tot = 0.5f * (1.0f - fl) * (fmaf(fl, a1 - a0, a0) + a1);
+                tot = fmaf(0.5f * fh, c0 + fmaf(fh, c1 - c0, c0), tot);
+                for (uint32_t j = jl + 1; j < jh; ++j) tot = fmaf(0.5f, tabp[j] + tabp[j + 1], tot);
+            }
+            acc[i] = fmaf(tot, inv_b, acc[i]);
+        };
         auto resample = [&](const Win &W, const float *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
+            if (FLUX) {
+                const float inv_b = (float)(1 << kFxFrac) / (float)W.b;
+                // coverage in local coordinates; W.base = x(k0) - (j0 << 28)
+                const int64_t j0s = (int64_t)W.j0 << kFxFrac;
+                const int64_t cov_lo = -j0s, cov_hi = ((int64_t)(P.n_lambda - 1) << kFxFrac) - j0s;
+                const int64_t e0 = W.base + (int64_t)W.b * tid;          // lower edge of channel k0 + tid
+                const bool interior = W.ka == k0 && W.kb == k_end && W.base >= cov_lo &&
+                                      W.base + (int64_t)W.b * (k_end - k0 + 1) <= cov_hi;
+                if (interior) {
+                    // both edges are truncated by the same function of k, so neighbouring bins share
+                    // their edge exactly (stride 256 b / 256 = b keeps the truncation exact)
+                    const uint32_t xl0 = (uint32_t)(e0 >> 8), xh0 = (uint32_t)((e0 + (int64_t)W.b) >> 8);
+#pragma unroll
+                    for (int i = 0; i < CPT; ++i)
+                        flux_sample(i, xl0 + (uint32_t)i * W.b, xh0 + (uint32_t)i * W.b, inv_b, buf);
+                } else {
+#pragma unroll
+                    for (int i = 0; i < CPT; ++i) {
+                        const int k = k0 + tid + i * kAccThreads;
+                        if (k >= W.ka && k <= W.kb) {
+                            const int64_t lo = e0 + (int64_t)W.b * (i * kAccThreads);
+                            const int64_t cl = max(lo, cov_lo), ch = min(lo + (int64_t)W.b, cov_hi);
+                            if (ch > cl) flux_sample(i, (uint32_t)(cl >> 8), (uint32_t)(ch >> 8), inv_b, buf);
+                        }
+                    }
+                }
+                return;
+            }
             // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
             const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
@@ -273,26 +327,28 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
-template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
+template <int CPT, bool SINGLE, bool FLUX>
+static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    cudaError_t e;
-    if (P.n_tiles == 1) {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, true, kAccDepth, kAccMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_accumulate<CPT, true, kAccDepth, kAccMinBlocks><<<grid, kAccThreads, smem, st>>>(P);
-    } else {
-        e = cudaFuncSetAttribute(k_accumulate<CPT, false, kAccDepth, kAccMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_accumulate<CPT, false, kAccDepth, kAccMinBlocks><<<grid, kAccThreads, smem, st>>>(P);
-    }
+    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, kAccMinBlocks, FLUX>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kAccThreads, smem, st>>>(P);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }
 
+template <int CPT>
+static cudaError_t launch_acc(const AccumParams &P, bool flux, unsigned grid, size_t smem, cudaStream_t st)
+{
+    if (P.n_tiles == 1)
+        return flux ? launch_acc2<CPT, true, true>(P, grid, smem, st) : launch_acc2<CPT, true, false>(P, grid, smem, st);
+    return flux ? launch_acc2<CPT, false, true>(P, grid, smem, st) : launch_acc2<CPT, false, false>(P, grid, smem, st);
+}
+
 // Largest CPT in {15, 8, 4, 2, 1} whose table fits the 12.20 format; returns the table capacity
 // (samples, a whole number of passes).
-int choose_cpt(int n_c, double b_max, int *wcap_out)
+int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 {
     const int cand[5] = {15, 8, 4, 2, 1};
     for (int c = 0; c < 5; ++c) {
@@ -302,7 +358,7 @@ int choose_cpt(int n_c, double b_max, int *wcap_out)
         // skip tilings that leave a whole 256-channel group of lanes idle (unless the smallest)
         if (cpt > 1 && (long long)tiles * tc - n_c >= kAccThreads) continue;
         // samples j0 .. j_max + 1 with j0 rounded down to a multiple of kRowAlign
-        const int need = (int)(b_max * tc) + kRowAlign + 4;
+        const int need = (int)(b_max * (tc + (flux ? 1 : 0))) + kRowAlign + 4;
         const int wcap = (need + kPass - 1) / kPass * kPass;
         if (wcap > kTabMax) continue;
         *wcap_out = wcap;
@@ -317,7 +373,8 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
     const double b_max = b0 / (1.0 - kBetaCap);
     int wcap = 0;
-    const int cpt = choose_cpt(L.n_c, b_max, &wcap);
+    const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
+    const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap);
     if (cpt == 0) return cudaErrorInvalidConfiguration;
     AccumParams P;
     P.flux = (const float *)(ws + L.off_flux);
@@ -332,6 +389,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const int tc = cpt * kAccThreads;
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
+    P.n_lambda = in.ssp->n_lambda;
     P.tex = 0;
 #if RUBIX_TEX_CORNERS > 0
     {
@@ -359,11 +417,11 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     {
         StageTimer t(1, st);
         switch (cpt) {
-            case 15: e = launch_acc<15>(P, grid, smem, st); break;
-            case 8: e = launch_acc<8>(P, grid, smem, st); break;
-            case 4: e = launch_acc<4>(P, grid, smem, st); break;
-            case 2: e = launch_acc<2>(P, grid, smem, st); break;
-            default: e = launch_acc<1>(P, grid, smem, st); break;
+            case 15: e = launch_acc<15>(P, flux, grid, smem, st); break;
+            case 8: e = launch_acc<8>(P, flux, grid, smem, st); break;
+            case 4: e = launch_acc<4>(P, flux, grid, smem, st); break;
+            case 2: e = launch_acc<2>(P, flux, grid, smem, st); break;
+            default: e = launch_acc<1>(P, flux, grid, smem, st); break;
         }
     }
     if (e != cudaSuccess) return e;
