@@ -240,9 +240,31 @@ k_accumulate(const __grid_constant__ AccumParams P)
                     // both edges are truncated by the same function of k, so neighbouring bins share
                     // their edge exactly (stride 256 b / 256 = b keeps the truncation exact)
                     const uint32_t xl0 = (uint32_t)(e0 >> 8), xh0 = (uint32_t)((e0 + (int64_t)W.b) >> 8);
+                    if (W.b <= (1u << kFxFrac)) {
+                        // bins no wider than one SSP sample touch at most two knot intervals: branch-free
+                        // I(u) = integral of the interpolant from knot jl to jl + u (u < 2) through
+                        // the three samples a0, a1, a2;  F = (I(fl + width) - I(fl)) / B
+                        const float width = (float)(xh0 - xl0) * (1.0f / 1048576.0f);
 #pragma unroll
-                    for (int i = 0; i < CPT; ++i)
-                        flux_sample(i, xl0 + (uint32_t)i * W.b, xh0 + (uint32_t)i * W.b, inv_b, buf);
+                        for (int i = 0; i < CPT; ++i) {
+                            const uint32_t x = xl0 + (uint32_t)i * W.b;
+                            const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
+                            const float a0 = e[0], a1 = e[1], a2r = e[2];
+                            const float fl = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;
+                            const float u = fl + width;
+                            const float u1 = fminf(u, 1.0f), u2 = fmaxf(u - 1.0f, 0.0f);
+                            const float a2 = u > 1.0f ? a2r : a1;     // e[2] may lie beyond the table
+                            const float d1 = a1 - a0, d2 = a2 - a1;
+                            const float il = fl * fmaf(0.5f * fl, d1, a0);
+                            float iu = u1 * fmaf(0.5f * u1, d1, a0);
+                            iu = fmaf(u2, fmaf(0.5f * u2, d2, a1), iu);
+                            acc[i] = fmaf(iu - il, inv_b, acc[i]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < CPT; ++i)
+                            flux_sample(i, xl0 + (uint32_t)i * W.b, xh0 + (uint32_t)i * W.b, inv_b, buf);
+                    }
                 } else {
 #pragma unroll
                     for (int i = 0; i < CPT; ++i) {
