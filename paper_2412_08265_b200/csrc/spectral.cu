@@ -337,15 +337,26 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
                   const int32_t *__restrict__ part_off, const int32_t *__restrict__ multi_list,
                   const int32_t *__restrict__ totals, int32_t n_c, float *__restrict__ cube)
 {
-    if ((int)blockIdx.x >= totals[2]) return;
-    const int s = multi_list[blockIdx.x];
+    for (int m = blockIdx.x; m < totals[2]; m += gridDim.x) {
+    const int s = multi_list[m];
     const int cnt = seg_off[s + 1] - seg_off[s];
     const int chunks = (cnt + kChunk - 1) / kChunk;
     const float *rows = partials + (size_t)part_off[s] * n_c;
+    // one thread per channel; eight chunk rows in flight per thread (the sum order stays c = 0, 1, ...)
     for (int k = blockIdx.y * 256 + threadIdx.x; k < n_c; k += gridDim.y * 256) {
+        const float *col = rows + k;
         double a = 0.0;
-        for (int c = 0; c < chunks; ++c) a += (double)__ldcs(rows + (size_t)c * n_c + k);
+        int c = 0;
+        for (; c + 8 <= chunks; c += 8) {
+            float v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = __ldcs(col + (size_t)(c + u) * n_c);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) a += (double)v[u];
+        }
+        for (; c < chunks; ++c) a += (double)__ldcs(col + (size_t)c * n_c);
         __stcs(cube + (size_t)s * n_c + k, (float)a);
+    }
     }
 }
 
@@ -448,8 +459,9 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     }
     if (e != cudaSuccess) return e;
     StageTimer t2(2, st);
-    const unsigned gy = (unsigned)((L.n_c + 1023) / 1024);
-    k_reduce_partials<<<dim3((unsigned)L.max_multi, gy), 256, 0, st>>>(
+    const unsigned gy = (unsigned)((L.n_c + 255) / 256);
+    const unsigned gx = (unsigned)(L.max_multi < 1184 ? L.max_multi : 1184);   // grid-stride over the multi-chunk spaxels
+    k_reduce_partials<<<dim3(gx, gy), 256, 0, st>>>(
         P.partials, (const int32_t *)(ws + L.off_seg), (const int32_t *)(ws + L.off_partoff),
         (const int32_t *)(ws + L.off_multi), P.totals, L.n_c, cube);
     RUBIX_LAUNCH_CHECK();
