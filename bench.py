@@ -315,17 +315,18 @@ def run_ours(args):
     achieved = gather_b / (acc_ms * 1e-3) / 1e9
     # L1 data-pipe view (the unit ncu shows saturated, profiles/r01_full_medium.md): bytes the SM's
     # load/store pipe must carry per particle = 4 corner windows (LDG) + table store (STS) + two
-    # table reads per channel (LDS); peak = 148 SMs x 128 B/clk x max SM clock (nominal)
+    # table reads per channel (LDS); peak = the shared-memory read bandwidth measured in this run
     win = float(t.n_channels) * float(t.dlambda) / float(w.ssp.dlambda)
     l1_b = (16.0 * win + 4.0 * win + 8.0 * t.n_channels) * n
-    l1_peak = 148 * 128 * 1.965
+    l1_peak = onchip["smem_gbs"]
     roofline = {"kernel": "k_accumulate (steps 4-6)", "bound": "l2", "achieved": achieved,
                 "peak": onchip["l2_gbs"], "unit": "GB/s", "frac": achieved / onchip["l2_gbs"],
                 "traffic": NCU_DRAM_BYTES_K_ACCUMULATE if args.workload == "medium" else None,
                 "traffic_source": "profiles/r01_full_medium.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
                 "l1_view": {"bound": "l1 data pipe", "achieved": l1_b / (acc_ms * 1e-3) / 1e9, "peak": l1_peak,
                             "unit": "GB/s", "frac": l1_b / (acc_ms * 1e-3) / 1e9 / l1_peak,
-                            "peak_source": "nominal 148 SMs x 128 B/clk x 1.965 GHz",
+                            "peak_source": "shared-memory / L1 data-pipe read bandwidth measured in this run by rubix_measure_peaks "
+                                           "(nominal 148 SMs x 128 B/clk x 1.965 GHz = 37.2 TB/s)",
                             "algorithmic_bytes_per_launch": l1_b},
                 "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks "
                                "(MEASURED_PEAKS.json has no L2 figure; SURVEY.md 8(d))",

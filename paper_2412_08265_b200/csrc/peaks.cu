@@ -71,7 +71,10 @@ __global__ void __launch_bounds__(256) k_peak_smem(int iters, float *sink)
     for (int it = 0; it < iters; ++it) {
 #pragma unroll 16
         for (int r = 0; r < 64; ++r) {
-            const float4 v = s[(idx + r * 256) & 1023];
+            float4 v;                                     // volatile: the compiler must not merge the loads
+            asm volatile("ld.volatile.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                         : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                         : "r"((uint32_t)__cvta_generic_to_shared(&s[(idx + r * 256) & 1023])));
             acc += v.x + v.y + v.z + v.w;
         }
         idx = (idx + 1) & 1023;
