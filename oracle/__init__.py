@@ -128,8 +128,8 @@ def particle_spectrum_f64(mass, log_age, log_z, vlos, ia, iz, ssp, tel):
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    _load().orc_particle_spectrum_f64(
-        C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
+    _load().orc_particle_spectrum_f64_mode(
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
         C.c_double(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
@@ -223,8 +223,8 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     grad_cube = np.ascontiguousarray(grad_cube, dtype=np.float64)
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
-    _load().orc_adjoint(
-        C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
+    _load().orc_adjoint_mode(
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
         C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis), C.c_float(float(ssp.lambda0)),
         C.c_float(float(ssp.dlambda)), _pf(flux), C.c_int32(tel.n_x), C.c_int32(tel.n_y),
         C.c_float(float(tel.spaxel_size)), C.c_int32(tel.n_channels),

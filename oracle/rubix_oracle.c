@@ -253,19 +253,29 @@ void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, i
 
 /* Same, but with the interpolation parameters given in fp64 (finite differences perturb
  * log age / log Z / v_los by steps far below fp32 resolution). */
+void orc_particle_spectrum_f64_mode(int32_t mode, double mass, double log_age, double log_z,
+                                    double vlos, int32_t n_age, int32_t n_z, int32_t n_lambda,
+                                    const float *age_axis, const float *z_axis, float l0_ssp,
+                                    float dl_ssp, const float *flux, int32_t n_c, float l0_obs,
+                                    float dl_obs, int32_t ia, int32_t iz, double *F)
+{
+    /* cell (ia, iz) is held fixed by the caller: FD stays inside one bilinear patch */
+    const double a0 = age_axis[ia], a1 = age_axis[ia + 1];
+    const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
+    (void)n_age;
+    particle_spectrum_mode(mode, mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0),
+                           vlos, flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c,
+                           (double)l0_obs, (double)dl_obs, F);
+}
+
 void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double vlos,
                                int32_t n_age, int32_t n_z, int32_t n_lambda,
                                const float *age_axis, const float *z_axis, float l0_ssp,
                                float dl_ssp, const float *flux, int32_t n_c, float l0_obs,
                                float dl_obs, int32_t ia, int32_t iz, double *F)
 {
-    /* cell (ia, iz) is held fixed by the caller: FD stays inside one bilinear patch */
-    const double a0 = age_axis[ia], a1 = age_axis[ia + 1];
-    const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
-    (void)n_age;
-    particle_spectrum(mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0), vlos,
-                      flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
-                      (double)dl_obs, F, 0);
+    orc_particle_spectrum_f64_mode(0, mass, log_age, log_z, vlos, n_age, n_z, n_lambda, age_axis,
+                                   z_axis, l0_ssp, dl_ssp, flux, n_c, l0_obs, dl_obs, ia, iz, F);
 }
 
 /* ------------------------------------------------------------------------------------
@@ -488,7 +498,7 @@ void orc_convolve_transpose(const double *gout, int32_t n_x, int32_t n_y, int32_
  *     dL/dv_los  = -m E / (c (1+beta)^2)
  *   out-of-FoV particles get 0.  Output in ORIGINAL particle order, fp64.
  * ------------------------------------------------------------------------------------ */
-void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mass,
+void orc_adjoint_mode(int32_t mode, int64_t n, const float *pos, const float *vel, const float *mass,
                  const float *log_age, const float *log_z, const float *R, int32_t n_age,
                  int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
                  float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
@@ -505,8 +515,8 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
     orc_rotate_bin(n, pos, vel, R, n_x, n_y, spaxel, key, vlos);
 #pragma omp parallel
     {
-        double *F = (double *)malloc(sizeof(double) * (size_t)n_c);
-        double *dS = (double *)malloc(sizeof(double) * (size_t)n_c);
+        double *F = (double *)malloc(sizeof(double) * (size_t)(n_c + 1));
+        double *dS = (double *)malloc(sizeof(double) * (size_t)(n_c + 1));
 #pragma omp for schedule(static)
         for (int64_t p = 0; p < n; ++p) {
             g_mass[p] = g_log_age[p] = g_log_z[p] = g_vlos[p] = 0.0;
@@ -520,20 +530,37 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
             double D[4];
             for (int32_t c = 0; c < 4; ++c) {
                 const double cta = (c & 1) ? 1.0 : 0.0, ctz = (c & 2) ? 1.0 : 0.0;
-                particle_spectrum(1.0, ia, iz, cta, ctz, (double)vlos[p], flux, n_z, n_lambda,
-                                  (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
-                                  (double)dl_obs, F, 0);
+                particle_spectrum_mode(mode, 1.0, ia, iz, cta, ctz, (double)vlos[p], flux, n_z, n_lambda,
+                                       (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
+                                       (double)dl_obs, F);
                 double acc = 0.0;
                 for (int32_t k = 0; k < n_c; ++k) acc += g[k] * F[k];
                 D[c] = acc;  /* c = 0:(i,j) 1:(i+1,j) 2:(i,j+1) 3:(i+1,j+1) */
             }
-            /* E: needs the slope of the blended unit-mass spectrum */
-            particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
-                              (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
-                              (double)dl_obs, F, dS);
             double E = 0.0;
-            for (int32_t k = 0; k < n_c; ++k)
-                E += g[k] * ((double)l0_obs + (double)dl_obs * k) * dS[k] / (double)dl_ssp;
+            if (mode == 1) {
+                /* Flux-conserving rule.  F[k] = (C(x_hi) - C(x_lo)) / B with C' = S~, the bin edges
+                 * x(lambda_e) = (lambda_e/(1+beta) - l0_ssp)/dl_ssp and B = dl_obs/((1+beta) dl_ssp):
+                 *   dF[k]/dbeta = F[k]/(1+beta) - (lambda_hi S~(x_hi) - lambda_lo S~(x_lo)) / (dl_obs (1+beta)),
+                 * an edge clipped to the coverage does not move (S~ = 0 outside the coverage gives
+                 * exactly that).  E = sum_k g[k] (lambda_hi S~(x_hi) - lambda_lo S~(x_lo)) for the blended
+                 * unit-mass spectrum, point-evaluated at the n_c + 1 bin edges. */
+                particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
+                                  (double)l0_ssp, (double)dl_ssp, 0, n_c + 1,
+                                  (double)l0_obs - 0.5 * (double)dl_obs, (double)dl_obs, F, 0);
+                for (int32_t k = 0; k < n_c; ++k) {
+                    const double lam_lo = (double)l0_obs + (double)dl_obs * ((double)k - 0.5);
+                    const double lam_hi = lam_lo + (double)dl_obs;
+                    E += g[k] * (lam_hi * F[k + 1] - lam_lo * F[k]);
+                }
+            } else {
+                /* E: needs the slope of the blended unit-mass spectrum */
+                particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
+                                  (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
+                                  (double)dl_obs, F, dS);
+                for (int32_t k = 0; k < n_c; ++k)
+                    E += g[k] * ((double)l0_obs + (double)dl_obs * k) * dS[k] / (double)dl_ssp;
+            }
             const double m = (double)mass[p];
             const double beta = (double)vlos[p] / ORC_C_KMS;
             g_mass[p] = (1 - ta) * (1 - tz) * D[0] + ta * (1 - tz) * D[1] + (1 - ta) * tz * D[2]
@@ -548,9 +575,25 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
                                   : 0.0;
             g_log_z[p] = z_free ? m * (-(1 - ta) * D[0] - ta * D[1] + (1 - ta) * D[2] + ta * D[3]) / dZ
                                 : 0.0;
-            g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));
+            if (mode == 1)
+                g_vlos[p] = m * (g_mass[p] - E / (double)dl_obs) / (ORC_C_KMS * (1.0 + beta));
+            else
+                g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));
         }
         free(F); free(dS);
     }
     free(gp); free(key); free(vlos);
+}
+
+void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mass,
+                 const float *log_age, const float *log_z, const float *R, int32_t n_age,
+                 int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
+                 float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
+                 float spaxel, int32_t n_c, float l0_obs, float dl_obs, int32_t psf_size,
+                 double psf_sigma, int32_t lsf_size, double lsf_sigma, const double *grad_cube,
+                 double *g_mass, double *g_log_age, double *g_log_z, double *g_vlos)
+{
+    orc_adjoint_mode(0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
+                     l0_ssp, dl_ssp, flux, n_x, n_y, spaxel, n_c, l0_obs, dl_obs, psf_size, psf_sigma,
+                     lsf_size, lsf_sigma, grad_cube, g_mass, g_log_age, g_log_z, g_vlos);
 }

@@ -128,3 +128,66 @@ def test_cube_is_the_sum_of_particle_spectra_and_mode_0_is_untouched():
     assert np.abs(c0 - cube).max() > 1e-4 * c0.max()      # the two rules do differ on this workload
     # a smooth spectrum sampled finely: bin average and point sample agree to second order
     assert np.abs(c0 - cube).max() < 0.2 * c0.max()
+
+
+# ----------------------------------------------------------------------------- adjoint of the flux rule
+def _fd_setup(n=500):
+    w = synth.make_workload("tiny", n=n)
+    tel_ = dataclasses.replace(w.telescope.with_psf_lsf(), resample=1)
+    other = synth.make_particles_for("tiny", n=n, seed=synth.ADJOINT_TARGET_SEED)
+    cube = oracle.forward(w.particles, w.rotation, w.ssp, tel_)
+    target = oracle.forward(other, w.rotation, w.ssp, tel_)
+    return w, tel_, cube, target
+
+
+def test_flux_adjoint_matches_central_finite_differences():
+    """BASELINE.json north_star: 'adjoint gradients match central finite differences' -- for the
+    flux-conserving rule.  F is C^1 in v_los here (an integral of a continuous function), so no knot
+    clearance is needed; L is quadratic in mass, log age and log Z inside a cell (FD exact)."""
+    w, tel_, cube, target = _fd_setup()
+    resid = cube - target
+    g = oracle.adjoint(w.particles, w.rotation, w.ssp, tel_, 2.0 * resid)
+    p, ssp = w.particles, w.ssp
+    key, _ = oracle.rotate_bin(p.pos, p.vel, w.rotation, tel_.n_x, tel_.n_y, tel_.spaxel_size)
+    ok = key < tel_.n_spaxels
+    for q, ax in ((p.log_age, ssp.log_age_axis), (p.log_z, ssp.log_z_axis)):
+        ok &= (q > ax[0] + 1e-3) & (q < ax[-1] - 1e-3) & (np.abs(q[:, None] - ax[None, :]).min(1) > 1e-3)
+    idx = np.random.default_rng(synth.ADJOINT_FD_SEED).choice(np.nonzero(ok)[0], 40, replace=False)
+    fd = oracle.fd_gradients(w.particles, w.rotation, ssp, tel_, resid, idx, h_v=1e-2)
+    for q, rtol in ((0, 1e-7), (1, 1e-6), (2, 1e-6), (3, 1e-4)):
+        scale = np.maximum(np.abs(fd[q]), 1e-3 * np.median(np.abs(fd[q])))
+        assert (np.abs(g[q][idx] - fd[q]) <= rtol * scale).all(), q
+    # and it is not the point-sampled gradient
+    g0 = oracle.adjoint(w.particles, w.rotation, w.ssp, dataclasses.replace(tel_, resample=0), 2.0 * resid)
+    assert np.abs(g0[3][idx] - g[3][idx]).max() > 1e-3 * np.abs(g[3][idx]).max()
+
+
+def test_flux_adjoint_closed_forms():
+    """Constant template: F does not depend on v (interior bins) => d/dv = 0, d/dm = sum of G.
+    Linear template a + b lambda: the bin average is the value at the bin centre, so the gradients
+    equal the point-sampled closed forms  d/dv = -m b sum_k G_k lambda_k / (c (1+beta)^2)."""
+    n_l = 400
+    lam = 3000.0 + 2.5 * np.arange(n_l)
+    t = synth.Telescope(4, 4, np.float32(1.0), 120, np.float32(3100.0), np.float32(6.0), resample=1)
+    w = synth.make_workload("tiny", n=40)
+    p = w.particles
+    p.pos[:] = np.random.default_rng(0).uniform(-1.9, 1.9, p.pos.shape)
+    p.log_age[:] = np.random.default_rng(1).uniform(-0.9, 0.9, p.n)
+    p.log_z[:] = np.random.default_rng(2).uniform(-3.9, -2.1, p.n)
+    R = np.eye(3, dtype=np.float32)
+    G = np.random.default_rng(3).normal(size=(4, 4, 120))
+    key, vlos = oracle.rotate_bin(p.pos, p.vel, R, 4, 4, 1.0)
+    rows = G.reshape(16, -1)[key]
+    beta = vlos.astype(np.float64) / C_KMS
+    axes = (np.array([-1, 0, 1], np.float32), np.array([-4, -3, -2], np.float32))
+    const = synth.SSPGrid(*axes, np.float32(3000.0), np.float32(2.5), np.full((3, 3, n_l), 1.5, np.float32))
+    g_m, g_a, g_z, g_v = oracle.adjoint(p, R, const, t, G)
+    assert np.allclose(g_m, 1.5 * rows.sum(1), rtol=1e-12)
+    assert np.abs(g_v).max() <= 1e-12 * np.abs(g_m * p.mass).max()
+    a, b = 2.0, 2.0 ** -12
+    lin = synth.SSPGrid(*axes, np.float32(3000.0), np.float32(2.5),
+                        np.ascontiguousarray(np.broadcast_to(a + b * lam, (3, 3, n_l)), np.float32))
+    g_m, g_a, g_z, g_v = oracle.adjoint(p, R, lin, t, G)
+    lam_k = t.wavelengths()
+    assert np.allclose(g_v, -(p.mass * b / (C_KMS * (1 + beta) ** 2)) * (rows * lam_k).sum(1), rtol=1e-9)
+    assert np.allclose(g_m, (rows * (a + b * lam_k[None, :] / (1 + beta[:, None]))).sum(1), rtol=1e-10)
