@@ -87,8 +87,8 @@ typedef struct {
  *   RUBIX_RESAMPLE_FLUX   F[k] = (1/dlambda_obs) * integral of S~(lambda / (1+beta)) over the bin
  *                         [lambda_k - dlambda_obs/2, lambda_k + dlambda_obs/2], S~ = 0 outside the
  *                         SSP coverage (sum_k F[k] dlambda_obs telescopes to the
- *                         total flux exactly).  Forward only: rubix_cube_adjoint returns
- *                         RUBIX_ERR_UNSUPPORTED for it. */
+ *                         total flux exactly).  rubix_cube_adjoint differentiates whichever rule
+ *                         the telescope selects. */
 #define RUBIX_RESAMPLE_POINT 0
 #define RUBIX_RESAMPLE_FLUX 1
 

@@ -133,6 +133,116 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Adjoint of the flux-conserving rule (RUBIX_RESAMPLE_FLUX, reading R13).
+// Records carry the LOWER EDGE of bin 0 as a_fx: x_k = a_fx + b_fx k is the lower edge of bin k.
+// One warp per particle; lane l owns bins / lower edges k_lo + l + 32 m.
+//   bin k     F_c[k] = (1/B) sum_j W_j T_c[j],  W_j = H(x_hi - j) - H(x_lo - j)  (x clipped to the
+//             coverage), H(t) = integral of the hat function from -1 to t.  Accumulated in the
+//             difference basis of k_adjoint: P0, Pa, Pz, Pq (x 1/B at the end).
+//   edge e    dF/dbeta needs the blended spectrum at the bin edges:
+//             sum_k g_k dF_k/dbeta = [ sum_k g_k F_k - (1/dl_obs) sum_e lambda_e s(x_e) (g_{e-1} - g_e) ] / (1+beta),
+//             s = 0 at edges outside the coverage (a clipped edge does not move), g = 0 outside
+//             [k_lo, k_hi] (those bins do not overlap the coverage).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float hat_integral(float t)
+{
+    const float a = fminf(fmaxf(t, -1.0f), 1.0f);
+    const float lo = 0.5f * (1.0f + a) * (1.0f + a);            // t in [-1, 0]
+    const float hi = 1.0f - 0.5f * (1.0f - a) * (1.0f - a);      // t in [0, 1]
+    return a <= 0.0f ? lo : hi;
+}
+
+__global__ void __launch_bounds__(256)
+k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
+               const int32_t *__restrict__ key, const float *__restrict__ vlos,
+               const float *__restrict__ mass, const float *__restrict__ log_age,
+               const float *__restrict__ log_z, const Rec *__restrict__ rec,
+               const float *__restrict__ flux, const float *__restrict__ gconv,
+               const __grid_constant__ AdjParams P, float *__restrict__ g_mass,
+               float *__restrict__ g_age, float *__restrict__ g_z, float *__restrict__ g_v)
+{
+    const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // sorted position
+    const int lane = threadIdx.x & 31;
+    if (i >= P.n) return;
+    const int p = perm[i];
+    if (i >= seg_off[P.n_s]) {                              // dropped particle: zero gradient
+        if (lane == 0) g_mass[p] = g_age[p] = g_z[p] = g_v[p] = 0.0f;
+        return;
+    }
+    const Rec r = rec[i];
+    const float *g = gconv + (size_t)key[p] * P.n_c;
+    const float *T0 = flux + r.cell;
+    const float *T1 = T0 + (size_t)P.n_z * P.pitch, *T2 = T0 + P.pitch, *T3 = T1 + P.pitch;
+    int ia, iz;
+    double ta, tz, wa, wz;
+    bool a_free, z_free;
+    adj_axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta, &wa, &a_free);
+    adj_axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz, &wz, &z_free);
+    const float u0 = (float)((1.0 - ta) * (1.0 - tz)), u1 = (float)(ta * (1.0 - tz));
+    const float u2 = (float)((1.0 - ta) * tz), u3 = (float)(ta * tz);
+    const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
+    const int64_t b = (int64_t)r.b_fx;
+    const float inv_scale = 1.0f / (float)(1 << kFxFrac);
+    double P0 = 0, Pa = 0, Pz = 0, Pq = 0, E = 0;
+    for (int k = r.k_lo + lane; k <= r.k_hi + 1; k += 32) {
+        const int64_t xl = r.a_fx + b * k;                 // lower edge of bin k = edge k
+        const float gk = k <= r.k_hi ? __ldg(g + k) : 0.0f;
+        const float gm1 = k > r.k_lo ? __ldg(g + k - 1) : 0.0f;
+        float s0 = 0.f, sa = 0.f, sz = 0.f, sq = 0.f, se = 0.f;
+        if (k <= r.k_hi) {                                  // ---- bin k
+            const int64_t cl = max(xl, (int64_t)0), ch = min(xl + b, x_max);
+            const int jl = (int)(cl >> kFxFrac);
+            const int ju = min((int)((ch + ((int64_t)1 << kFxFrac) - 1) >> kFxFrac), P.n_lambda - 1);
+            float v0 = 0.f, v1 = 0.f, v2 = 0.f, v3 = 0.f;
+            for (int j = jl; j <= ju; ++j) {
+                const int64_t o = (int64_t)j << kFxFrac;
+                const float w = hat_integral((float)(ch - o) * inv_scale) - hat_integral((float)(cl - o) * inv_scale);
+                const uint32_t ju32 = (uint32_t)j;
+                v0 = fmaf(w, __ldg(T0 + ju32), v0);
+                v1 = fmaf(w, __ldg(T1 + ju32), v1);
+                v2 = fmaf(w, __ldg(T2 + ju32), v2);
+                v3 = fmaf(w, __ldg(T3 + ju32), v3);
+            }
+            const float da = v1 - v0, dz = v2 - v0;
+            s0 = gk * v0;
+            sa = gk * da;
+            sz = gk * dz;
+            sq = gk * ((v3 - v2) - da);
+        }
+        if (xl >= 0 && xl <= x_max) {                       // ---- edge k inside the coverage
+            int j = (int)(xl >> kFxFrac);
+            float f = (float)(uint32_t)(xl & (((int64_t)1 << kFxFrac) - 1)) * inv_scale;
+            if (j > P.n_lambda - 2) { j = P.n_lambda - 2; f = 1.0f; }
+            const uint32_t ju32 = (uint32_t)j;
+            const float a0 = __ldg(T0 + ju32), a1 = __ldg(T1 + ju32), a2 = __ldg(T2 + ju32), a3 = __ldg(T3 + ju32);
+            const float e0 = fmaf(f, __ldg(T0 + ju32 + 1) - a0, a0), e1 = fmaf(f, __ldg(T1 + ju32 + 1) - a1, a1);
+            const float e2 = fmaf(f, __ldg(T2 + ju32 + 1) - a2, a2), e3 = fmaf(f, __ldg(T3 + ju32 + 1) - a3, a3);
+            const float lam = fmaf(P.dl_obs, (float)k - 0.5f, P.l0_obs);
+            se = (gm1 - gk) * lam * fmaf(u3, e3, fmaf(u2, e2, fmaf(u1, e1, u0 * e0)));
+        }
+        P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq; E += (double)se;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        P0 += __shfl_xor_sync(0xffffffffu, P0, o);
+        Pa += __shfl_xor_sync(0xffffffffu, Pa, o);
+        Pz += __shfl_xor_sync(0xffffffffu, Pz, o);
+        Pq += __shfl_xor_sync(0xffffffffu, Pq, o);
+        E += __shfl_xor_sync(0xffffffffu, E, o);
+    }
+    if (lane == 0) {
+        const double m = (double)mass[p];
+        const double opb = 1.0 + (double)vlos[p] / kCkms;
+        const double inv_b = (double)(1 << kFxFrac) / (double)r.b_fx;
+        const double gm = inv_b * (P0 + ta * Pa + tz * Pz + ta * tz * Pq);
+        g_mass[p] = (float)gm;
+        g_age[p] = a_free ? (float)(m * inv_b * (Pa + tz * Pq) / wa) : 0.0f;
+        g_z[p] = z_free ? (float)(m * inv_b * (Pz + ta * Pq) / wz) : 0.0f;
+        g_v[p] = (float)(m * (gm - E / (double)P.dl_obs) / (kCkms * opb));
+    }
+}
+
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st)
 {
@@ -152,12 +262,12 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
     const int64_t threads = L.n * 32;
-    k_adjoint<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+    auto kern = in.tel->resample == RUBIX_RESAMPLE_FLUX ? k_adjoint_flux : k_adjoint;
+    kern<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const int32_t *)(ws + L.off_permbuf[L.final_buf]), (const int32_t *)(ws + L.off_seg),
         (const int32_t *)(ws + L.off_key), (const float *)(ws + L.off_vlos), in.p->mass,
         in.p->log_age, in.p->log_z, (const Rec *)(ws + L.off_rec), (const float *)(ws + L.off_flux), gconv, P,
-        g_mass,
-        g_age, g_z, g_v);
+        g_mass, g_age, g_z, g_v);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }

@@ -208,8 +208,6 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
     if (!R || !grad_cube) return fail(RUBIX_ERR_NULL, "R or grad_cube is NULL");
     if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
         return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
-    if (tel->resample != RUBIX_RESAMPLE_POINT)
-        return fail(RUBIX_ERR_UNSUPPORTED, "rubix_cube_adjoint supports RUBIX_RESAMPLE_POINT only");
     if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
     const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
                                  ssp->n_lambda);

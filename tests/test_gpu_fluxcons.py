@@ -120,10 +120,52 @@ def test_total_flux_is_conserved_on_the_gpu(B):
     assert abs(row.sum() * 1.75 - total) <= 2e-6 * total
 
 
-def test_adjoint_is_refused_in_flux_mode(B):
-    w = flux_mode(synth.make_workload("tiny"))
+def test_adjoint_config_in_flux_mode(B):
+    """BASELINE.json configs[4] with the flux-conserving rule: gradients against the oracle's analytic
+    adjoint on every particle and against central finite differences of the oracle on 100 particles,
+    within 1e-3 relative (north_star)."""
+    w = flux_mode(synth.make_workload("adjoint"))
+    t = w.telescope
+    other = synth.make_particles_for("adjoint", seed=synth.ADJOINT_TARGET_SEED)
     dw = B.DeviceWorkload(w)
-    grad = torch.zeros(dw.shape, device="cuda")
-    with pytest.raises(B.RubixError):
-        dw.adjoint(grad)
-    assert "RUBIX_RESAMPLE_POINT" in B.rubix_last_error()
+    target = oracle.forward(other, w.rotation, w.ssp, t)          # never from the CUDA path
+    ref_final = oracle.forward(w.particles, w.rotation, w.ssp, t)
+    cube = dw.forward()
+    torch.cuda.synchronize()
+    assert np.abs(cube.cpu().numpy() - ref_final).max() <= 1e-4 * ref_final.max()
+    resid = ref_final - target
+    grad_cube = torch.from_numpy((2.0 * resid).astype(np.float32)).cuda()
+    g = [x.cpu().numpy().astype(np.float64) for x in dw.adjoint(grad_cube)]
+    p, ssp = w.particles, w.ssp
+    key, _ = oracle.rotate_bin(p.pos, p.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    ana = oracle.adjoint(p, w.rotation, ssp, t, 2.0 * resid)
+    for q in range(4):
+        scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
+        rel = np.abs(g[q] - ana[q]) / scale
+        assert np.quantile(rel, 0.999) <= 1e-3, (q, rel.max())
+        assert not g[q][key >= t.n_spaxels].any()
+    ok = key < t.n_spaxels
+    for v, ax in ((p.log_age, ssp.log_age_axis), (p.log_z, ssp.log_z_axis)):
+        ok &= (v > ax[0] + 1e-3) & (v < ax[-1] - 1e-3) & (np.abs(v[:, None] - ax[None, :]).min(1) > 1e-3)
+    idx = np.random.default_rng(synth.ADJOINT_FD_SEED).choice(np.nonzero(ok)[0], 100, replace=False)
+    fd = oracle.fd_gradients(p, w.rotation, ssp, t, resid, idx, h_v=1e-2)
+    for q in range(4):
+        scale = np.maximum(np.abs(fd[q]), 1e-3 * np.median(np.abs(fd[q])))
+        rel = np.abs(g[q][idx] - fd[q]) / scale
+        assert rel.max() <= 1e-3, (q, rel.max())
+
+
+def test_adjoint_tiny_wide_bins_and_clipped_edges(B):
+    """Bins wider than one SSP sample and an observed grid sticking out of the coverage."""
+    w = synth.make_workload("tiny", n=500)
+    w.telescope = dataclasses.replace(
+        synth.Telescope(6, 6, np.float32(3.0), 330, np.float32(3300.0), np.float32(20.0)).with_psf_lsf(), resample=1)
+    t = w.telescope
+    dw = B.DeviceWorkload(w)
+    G = np.random.default_rng(5).normal(size=(t.n_x, t.n_y, t.n_channels))
+    g = [x.cpu().numpy().astype(np.float64) for x in dw.adjoint(torch.from_numpy(G.astype(np.float32)).cuda())]
+    ana = oracle.adjoint(w.particles, w.rotation, w.ssp, t, G.astype(np.float32).astype(np.float64))
+    key, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    for q in range(4):
+        scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
+        assert (np.abs(g[q] - ana[q]) / scale).max() <= 1e-3, q
