@@ -185,11 +185,41 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
     const int64_t b = (int64_t)r.b_fx;
     const float inv_scale = 1.0f / (float)(1 << kFxFrac);
     double P0 = 0, Pa = 0, Pz = 0, Pq = 0, E = 0;
+    const bool narrow = r.b_fx <= (1u << kFxFrac);
+    const float width = (float)r.b_fx * inv_scale;
     for (int k = r.k_lo + lane; k <= r.k_hi + 1; k += 32) {
         const int64_t xl = r.a_fx + b * k;                 // lower edge of bin k = edge k
         const float gk = k <= r.k_hi ? __ldg(g + k) : 0.0f;
         const float gm1 = k > r.k_lo ? __ldg(g + k - 1) : 0.0f;
         float s0 = 0.f, sa = 0.f, sz = 0.f, sq = 0.f, se = 0.f;
+        if (narrow && k <= r.k_hi && xl >= 0 && xl + b <= x_max) {
+            // interior bin no wider than one SSP sample: it touches knots j, j+1, j+2 only, and its
+            // lower edge is sampled from the same loads.  w_0..2 = coefficients of the three samples in
+            // I(f + B) - I(f), I(u) = integral of the interpolant from knot j to j + u (u < 2)
+            const uint32_t j = (uint32_t)(xl >> kFxFrac);
+            const float f = __uint_as_float((((uint32_t)xl >> 5) & 0x7FFFFFu) | 0x3F800000u) - 1.0f;
+            const float u = f + width;
+            const float uu1 = fminf(u, 1.0f), uu2 = fmaxf(u - 1.0f, 0.0f);
+            const float q1 = 0.5f * (uu1 * uu1 - f * f);
+            const float w0 = (uu1 - f) - q1, w2 = 0.5f * uu2 * uu2, w1 = q1 + uu2 - w2;
+            const float a0 = __ldg(T0 + j), a1 = __ldg(T1 + j), a2 = __ldg(T2 + j), a3 = __ldg(T3 + j);
+            const float b0 = __ldg(T0 + j + 1), b1 = __ldg(T1 + j + 1), b2 = __ldg(T2 + j + 1), b3 = __ldg(T3 + j + 1);
+            const float v0 = fmaf(w2, __ldg(T0 + j + 2), fmaf(w1, b0, w0 * a0));
+            const float v1 = fmaf(w2, __ldg(T1 + j + 2), fmaf(w1, b1, w0 * a1));
+            const float v2 = fmaf(w2, __ldg(T2 + j + 2), fmaf(w1, b2, w0 * a2));
+            const float v3 = fmaf(w2, __ldg(T3 + j + 2), fmaf(w1, b3, w0 * a3));
+            const float da = v1 - v0, dz = v2 - v0;
+            s0 = gk * v0;
+            sa = gk * da;
+            sz = gk * dz;
+            sq = gk * ((v3 - v2) - da);
+            const float e0 = fmaf(f, b0 - a0, a0), e1 = fmaf(f, b1 - a1, a1);
+            const float e2 = fmaf(f, b2 - a2, a2), e3 = fmaf(f, b3 - a3, a3);
+            const float lam = fmaf(P.dl_obs, (float)k - 0.5f, P.l0_obs);
+            se = (gm1 - gk) * lam * fmaf(u3, e3, fmaf(u2, e2, fmaf(u1, e1, u0 * e0)));
+            P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq; E += (double)se;
+            continue;
+        }
         if (k <= r.k_hi) {                                  // ---- bin k
             const int64_t cl = max(xl, (int64_t)0), ch = min(xl + b, x_max);
             const int jl = (int)(cl >> kFxFrac);
