@@ -357,14 +357,14 @@ def run_ours(args):
 
     for _ in range(3):
         step_flux()
-    barrier()
+    torch.cuda.synchronize()                              # rank 0 only from here on: no collective
     B.rubix_stage_timing_enable(True)
     B.rubix_stage_timing_read()
     e0.record()
     for _ in range(10):
         step_flux()
     e1.record()
-    barrier()
+    torch.cuda.synchronize()                              # rank 0 only from here on: no collective
     st_f = B.rubix_stage_timing_read()
     B.rubix_stage_timing_enable(False)
     flux_ms = e0.elapsed_time(e1) / 10
