@@ -77,6 +77,10 @@ typedef struct {
     int32_t lsf_size;               /* odd taps <= 63 along the channel axis; 0 = LSF off   */
     float lsf_sigma;                /* channels, > 0 when lsf_size > 0                      */
     int32_t resample;               /* RUBIX_RESAMPLE_POINT (0) or RUBIX_RESAMPLE_FLUX (1)  */
+    float redshift;                 /* cosmological redshift z of the galaxy, 0 <= z <= 20:  */
+                                    /* lambda_rest = lambda_obs / ((1 + z)(1 + beta))        */
+    float flux_scale;               /* > 0: every spectrum is multiplied by it (distance     */
+                                    /* dimming / unit conversion chosen by the caller); 1 = off */
 } rubix_telescope;
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the

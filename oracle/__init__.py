@@ -114,7 +114,8 @@ def particle_spectrum(mass, log_age, log_z, vlos, ssp, tel):
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
     _load().orc_particle_spectrum_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
         C.c_float(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
@@ -129,7 +130,8 @@ def particle_spectrum_f64(mass, log_age, log_z, vlos, ia, iz, ssp, tel):
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
     _load().orc_particle_spectrum_f64_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
         C.c_double(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
@@ -155,7 +157,8 @@ def build_cube(particles, R, ssp, tel, sel=None):
         n_sel = sel_arr.size
         cube = np.empty((n_sel, n_c), np.float64)
     _load().orc_build_cube_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
         C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis),
         C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
         C.c_int32(tel.n_x), C.c_int32(tel.n_y), C.c_float(float(tel.spaxel_size)),
@@ -224,7 +227,8 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
     _load().orc_adjoint_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
+        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
         C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis), C.c_float(float(ssp.lambda0)),
         C.c_float(float(ssp.dlambda)), _pf(flux), C.c_int32(tel.n_x), C.c_int32(tel.n_y),
         C.c_float(float(tel.spaxel_size)), C.c_int32(tel.n_channels),
@@ -240,7 +244,8 @@ def knot_clearance(vlos, ssp, tel):
     finite-difference sample keeps away from those (non-differentiable points)."""
     beta = np.asarray(vlos, np.float64)[:, None] / C_KMS
     lam = np.float64(tel.lambda0) + np.float64(tel.dlambda) * np.arange(tel.n_channels)
-    x = (lam[None, :] / (1.0 + beta) - np.float64(ssp.lambda0)) / np.float64(ssp.dlambda)
+    x = (lam[None, :] / ((1.0 + beta) * (1.0 + float(getattr(tel, "redshift", 0.0)))) - np.float64(ssp.lambda0)) \
+        / np.float64(ssp.dlambda)
     return np.abs(x - np.round(x)).min(axis=1)
 
 

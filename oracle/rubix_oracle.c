@@ -225,7 +225,12 @@ static void particle_spectrum_mode(int32_t mode, double mass, int32_t ia, int32_
                           k_end, l0_obs, dl_obs, F, 0);
 }
 
-void orc_particle_spectrum_mode(int32_t mode, float mass, float log_age, float log_z, float vlos,
+/* Cosmological redshift and flux scaling (reading R14; "Doppler shifted based
+ * on the galaxy distance and line-of-sight velocity"): lambda_rest = lambda_obs / ((1+z)(1+beta)), which
+ * is the z = 0 computation on the observed grid divided by (1+z) (bin edges included: the bin average is
+ * unchanged by that rescaling); every spectrum is multiplied by flux_scale (passed on as a factor of the
+ * mass, in which the spectrum is linear). */
+void orc_particle_spectrum_mode(int32_t mode, double zc, double scale, float mass, float log_age, float log_z, float vlos,
                                 int32_t n_age, int32_t n_z, int32_t n_lambda, const float *age_axis,
                                 const float *z_axis, float l0_ssp, float dl_ssp, const float *flux,
                                 int32_t n_c, float l0_obs, float dl_obs, double *F)
@@ -234,8 +239,9 @@ void orc_particle_spectrum_mode(int32_t mode, float mass, float log_age, float l
     double ta, tz;
     axis_cell(age_axis, n_age, log_age, &ia, &ta);
     axis_cell(z_axis, n_z, log_z, &iz, &tz);
-    particle_spectrum_mode(mode, (double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
-                           (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs, (double)dl_obs, F);
+    particle_spectrum_mode(mode, scale * (double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
+                           (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs / (1.0 + zc),
+                           (double)dl_obs / (1.0 + zc), F);
 }
 
 void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, int32_t n_age,
@@ -253,7 +259,7 @@ void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, i
 
 /* Same, but with the interpolation parameters given in fp64 (finite differences perturb
  * log age / log Z / v_los by steps far below fp32 resolution). */
-void orc_particle_spectrum_f64_mode(int32_t mode, double mass, double log_age, double log_z,
+void orc_particle_spectrum_f64_mode(int32_t mode, double zc, double scale, double mass, double log_age, double log_z,
                                     double vlos, int32_t n_age, int32_t n_z, int32_t n_lambda,
                                     const float *age_axis, const float *z_axis, float l0_ssp,
                                     float dl_ssp, const float *flux, int32_t n_c, float l0_obs,
@@ -263,9 +269,9 @@ void orc_particle_spectrum_f64_mode(int32_t mode, double mass, double log_age, d
     const double a0 = age_axis[ia], a1 = age_axis[ia + 1];
     const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
     (void)n_age;
-    particle_spectrum_mode(mode, mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0),
+    particle_spectrum_mode(mode, scale * mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0),
                            vlos, flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c,
-                           (double)l0_obs, (double)dl_obs, F);
+                           (double)l0_obs / (1.0 + zc), (double)dl_obs / (1.0 + zc), F);
 }
 
 void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double vlos,
@@ -274,7 +280,7 @@ void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double
                                float dl_ssp, const float *flux, int32_t n_c, float l0_obs,
                                float dl_obs, int32_t ia, int32_t iz, double *F)
 {
-    orc_particle_spectrum_f64_mode(0, mass, log_age, log_z, vlos, n_age, n_z, n_lambda, age_axis,
+    orc_particle_spectrum_f64_mode(0, 0.0, 1.0, mass, log_age, log_z, vlos, n_age, n_z, n_lambda, age_axis,
                                    z_axis, l0_ssp, dl_ssp, flux, n_c, l0_obs, dl_obs, ia, iz, F);
 }
 
@@ -283,7 +289,7 @@ void orc_particle_spectrum_f64(double mass, double log_age, double log_z, double
  * If n_sel > 0 only the listed spaxels are computed and cube is [n_sel][n_c]; otherwise
  * cube is [n_s][n_c].  Particles are visited in the stable order of step 3.
  * ------------------------------------------------------------------------------------ */
-void orc_build_cube_mode(int32_t mode, int64_t n, const float *pos, const float *vel, const float *mass,
+void orc_build_cube_mode(int32_t mode, double zc, double scale, int64_t n, const float *pos, const float *vel, const float *mass,
                          const float *log_age, const float *log_z, const float *R, int32_t n_age,
                          int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
                          float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
@@ -319,9 +325,9 @@ void orc_build_cube_mode(int32_t mode, int64_t n, const float *pos, const float 
                     double ta, tz;
                     axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
                     axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
-                    particle_spectrum_mode(mode, (double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux,
+                    particle_spectrum_mode(mode, scale * (double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux,
                                            n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke,
-                                           (double)l0_obs, (double)dl_obs, F);
+                                           (double)l0_obs / (1.0 + zc), (double)dl_obs / (1.0 + zc), F);
                     for (int32_t k = kb; k < ke; ++k) row[k] += F[k];
                 }
             }
@@ -337,7 +343,7 @@ void orc_build_cube(int64_t n, const float *pos, const float *vel, const float *
                     float spaxel, int32_t n_c, float l0_obs, float dl_obs, const int32_t *sel,
                     int32_t n_sel, double *cube)
 {
-    orc_build_cube_mode(0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
+    orc_build_cube_mode(0, 0.0, 1.0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
                         l0_ssp, dl_ssp, flux, n_x, n_y, spaxel, n_c, l0_obs, dl_obs, sel, n_sel, cube);
 }
 
@@ -498,15 +504,17 @@ void orc_convolve_transpose(const double *gout, int32_t n_x, int32_t n_y, int32_
  *     dL/dv_los  = -m E / (c (1+beta)^2)
  *   out-of-FoV particles get 0.  Output in ORIGINAL particle order, fp64.
  * ------------------------------------------------------------------------------------ */
-void orc_adjoint_mode(int32_t mode, int64_t n, const float *pos, const float *vel, const float *mass,
+void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const float *pos, const float *vel, const float *mass,
                  const float *log_age, const float *log_z, const float *R, int32_t n_age,
                  int32_t n_z, int32_t n_lambda, const float *age_axis, const float *z_axis,
                  float l0_ssp, float dl_ssp, const float *flux, int32_t n_x, int32_t n_y,
-                 float spaxel, int32_t n_c, float l0_obs, float dl_obs, int32_t psf_size,
+                 float spaxel, int32_t n_c, float l0_obs_f, float dl_obs_f, int32_t psf_size,
                  double psf_sigma, int32_t lsf_size, double lsf_sigma, const double *grad_cube,
                  double *g_mass, double *g_log_age, double *g_log_z, double *g_vlos)
 {
     const int32_t n_s = n_x * n_y;
+    /* observed grid divided by (1 + z): see orc_particle_spectrum_mode */
+    const double l0_obs = (double)l0_obs_f / (1.0 + zc), dl_obs = (double)dl_obs_f / (1.0 + zc);
     const int64_t n_vox = (int64_t)n_s * n_c;
     double *gp = (double *)malloc(sizeof(double) * (size_t)(n_vox > 0 ? n_vox : 1));
     orc_convolve_transpose(grad_cube, n_x, n_y, n_c, psf_size, psf_sigma, lsf_size, lsf_sigma, gp);
@@ -561,8 +569,9 @@ void orc_adjoint_mode(int32_t mode, int64_t n, const float *pos, const float *ve
                 for (int32_t k = 0; k < n_c; ++k)
                     E += g[k] * ((double)l0_obs + (double)dl_obs * k) * dS[k] / (double)dl_ssp;
             }
-            const double m = (double)mass[p];
+            const double m = scale * (double)mass[p];
             const double beta = (double)vlos[p] / ORC_C_KMS;
+            /* unit-mass, unit-scale sum_k g_k F_k; scaled after g_vlos below has used it */
             g_mass[p] = (1 - ta) * (1 - tz) * D[0] + ta * (1 - tz) * D[1] + (1 - ta) * tz * D[2]
                         + ta * tz * D[3];
             const double dA = (double)age_axis[ia + 1] - (double)age_axis[ia];
@@ -579,6 +588,7 @@ void orc_adjoint_mode(int32_t mode, int64_t n, const float *pos, const float *ve
                 g_vlos[p] = m * (g_mass[p] - E / (double)dl_obs) / (ORC_C_KMS * (1.0 + beta));
             else
                 g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));
+            g_mass[p] *= scale;
         }
         free(F); free(dS);
     }
@@ -593,7 +603,7 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
                  double psf_sigma, int32_t lsf_size, double lsf_sigma, const double *grad_cube,
                  double *g_mass, double *g_log_age, double *g_log_z, double *g_vlos)
 {
-    orc_adjoint_mode(0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
+    orc_adjoint_mode(0, 0.0, 1.0, n, pos, vel, mass, log_age, log_z, R, n_age, n_z, n_lambda, age_axis, z_axis,
                      l0_ssp, dl_ssp, flux, n_x, n_y, spaxel, n_c, l0_obs, dl_obs, psf_size, psf_sigma,
                      lsf_size, lsf_sigma, grad_cube, g_mass, g_log_age, g_log_z, g_vlos);
 }

@@ -47,7 +47,8 @@ class CTelescope(C.Structure):
     _fields_ = [("n_x", C.c_int32), ("n_y", C.c_int32), ("spaxel_size", C.c_float),
                 ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
-                ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32)]
+                ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
+                ("redshift", C.c_float), ("flux_scale", C.c_float)]
 
 
 _lib = None
@@ -133,7 +134,8 @@ def c_telescope(tel) -> _Keep:
     return _Keep(CTelescope(int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
                             float(tel.lambda0), float(tel.dlambda), int(tel.psf_size),
                             float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma),
-                            int(getattr(tel, "resample", 0))))
+                            int(getattr(tel, "resample", 0)), float(getattr(tel, "redshift", 0.0)),
+                            float(getattr(tel, "flux_scale", 1.0))))
 
 
 def c_ssp(ssp, flux) -> _Keep:

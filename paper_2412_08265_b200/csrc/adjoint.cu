@@ -16,7 +16,8 @@ namespace rubix {
 struct AdjParams {
     AxisParams ax;
     int32_t n_lambda, pitch, n_z, n_c, n_s;
-    float l0_obs, dl_obs, dl_ssp;
+    float l0_obs, dl_obs, dl_ssp;     // observed grid already divided by (1 + z)
+    float flux_scale;
     int64_t n;
 };
 
@@ -124,9 +125,9 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
         E += __shfl_xor_sync(0xffffffffu, E, o);
     }
     if (lane == 0) {
-        const double m = (double)mass[p];
+        const double m = (double)mass[p] * (double)P.flux_scale;
         const double opb = 1.0 + (double)vlos[p] / kCkms;
-        g_mass[p] = (float)(P0 + ta * Pa + tz * Pz + ta * tz * Pq);
+        g_mass[p] = (float)((double)P.flux_scale * (P0 + ta * Pa + tz * Pz + ta * tz * Pq));
         g_age[p] = a_free ? (float)(m * (Pa + tz * Pq) / wa) : 0.0f;
         g_z[p] = z_free ? (float)(m * (Pz + ta * Pq) / wz) : 0.0f;
         g_v[p] = (float)(-m * E / ((double)P.dl_ssp * kCkms * opb * opb));
@@ -262,11 +263,11 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
         E += __shfl_xor_sync(0xffffffffu, E, o);
     }
     if (lane == 0) {
-        const double m = (double)mass[p];
+        const double m = (double)mass[p] * (double)P.flux_scale;
         const double opb = 1.0 + (double)vlos[p] / kCkms;
         const double inv_b = (double)(1 << kFxFrac) / (double)r.b_fx;
         const double gm = inv_b * (P0 + ta * Pa + tz * Pz + ta * tz * Pq);
-        g_mass[p] = (float)gm;
+        g_mass[p] = (float)((double)P.flux_scale * gm);
         g_age[p] = a_free ? (float)(m * inv_b * (Pa + tz * Pq) / wa) : 0.0f;
         g_z[p] = z_free ? (float)(m * inv_b * (Pz + ta * Pq) / wz) : 0.0f;
         g_v[p] = (float)(m * (gm - E / (double)P.dl_obs) / (kCkms * opb));
@@ -287,8 +288,9 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.n_z = in.ssp->n_z;
     P.n_c = L.n_c;
     P.n_s = L.n_s;
-    P.l0_obs = in.tel->lambda0;
-    P.dl_obs = in.tel->dlambda;
+    P.l0_obs = (float)((double)in.tel->lambda0 / (1.0 + (double)in.tel->redshift));
+    P.dl_obs = (float)((double)in.tel->dlambda / (1.0 + (double)in.tel->redshift));
+    P.flux_scale = in.tel->flux_scale;
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
     const int64_t threads = L.n * 32;

@@ -71,6 +71,10 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_INVALID_ARG, "telescope dlambda must be > 0 and finite");
     if (t->resample != RUBIX_RESAMPLE_POINT && t->resample != RUBIX_RESAMPLE_FLUX)
         return fail(RUBIX_ERR_INVALID_ARG, "resample must be RUBIX_RESAMPLE_POINT (0) or RUBIX_RESAMPLE_FLUX (1)");
+    if (!(t->redshift >= 0.0f) || !(t->redshift <= 20.0f))
+        return fail(RUBIX_ERR_INVALID_ARG, "redshift must be in [0, 20]");
+    if (!(t->flux_scale > 0.0f) || !isfinite(t->flux_scale))
+        return fail(RUBIX_ERR_INVALID_ARG, "flux_scale must be > 0 and finite (1 = no scaling)");
     const int sz[2] = {t->psf_size, t->lsf_size};
     const float sg[2] = {t->psf_sigma, t->lsf_sigma};
     for (int i = 0; i < 2; ++i) {

@@ -313,6 +313,7 @@ struct PrepParams {
     AxisParams ax;
     int32_t n_lambda, pitch, n_c, n_s, mode;
     float l0_ssp, dl_ssp, l0_obs, dl_obs;
+    float redshift, flux_scale;         // DESIGN.md reading R14
 };
 
 __device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *cell, double *t)
@@ -342,14 +343,14 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     double ta, tz;
     axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta);
     axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz);
-    const double m = (double)mass[p];
+    const double m = (double)mass[p] * (double)P.flux_scale;
     Rec r;
     r.w[0] = (float)(m * (1.0 - ta) * (1.0 - tz));
     r.w[1] = (float)(m * ta * (1.0 - tz));
     r.w[2] = (float)(m * (1.0 - ta) * tz);
     r.w[3] = (float)(m * ta * tz);
     r.cell = (ia * P.ax.n_z + iz) * P.pitch;
-    const double inv = 1.0 / (1.0 + (double)vlos[p] / kCkms);
+    const double inv = 1.0 / ((1.0 + (double)vlos[p] / kCkms) * (1.0 + (double)P.redshift));
     const double scale = (double)(1 << kFxFrac);
     const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
     const double B = (double)P.dl_obs * inv / (double)P.dl_ssp;
@@ -559,6 +560,8 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.n_c = in.tel->n_channels;
         P.n_s = n_s;
         P.mode = in.tel->resample;
+        P.redshift = in.tel->redshift;
+        P.flux_scale = in.tel->flux_scale;
         P.l0_ssp = in.ssp->lambda0;
         P.dl_ssp = in.ssp->dlambda;
         P.l0_obs = in.tel->lambda0;

@@ -180,6 +180,8 @@ class Telescope:
     lsf_size: int = 0         # odd taps; 0 = off
     lsf_sigma: np.float32 = np.float32(0.0)   # channels
     resample: int = 0         # 0 = point-sampled linear interpolation, 1 = flux-conserving bin average
+    redshift: np.float32 = np.float32(0.0)     # cosmological redshift of the galaxy
+    flux_scale: np.float32 = np.float32(1.0)   # multiplies every spectrum (distance dimming / units)
 
     @property
     def n_spaxels(self) -> int:
