@@ -138,6 +138,25 @@ rubix_status rubix_cube_adjoint(const rubix_particles *particles, const rubix_ss
                                 float *g_log_z, float *g_vlos, void *workspace,
                                 size_t workspace_bytes, void *stream);
 
+/* Fused forward + loss + adjoint for gradient-based fitting ("gradient computations
+ * through the entire pipeline"; BASELINE.json configs[4]): steps 1-8, then
+ *     L = sum over voxels of (final cube - target)^2       (fp64 sum in a fixed order: bit-reproducible)
+ * and step 9 with the upstream gradient 2 (final cube - target), sharing ONE particle pass (rotate, bin,
+ * sort, records) between the forward and the adjoint.  Equivalent to rubix_build_cube +
+ * rubix_convolve_psf_lsf + (caller forms the residual) + rubix_cube_adjoint.
+ *   target    DEVICE [n_x][n_y][n_channels] fp32
+ *   loss      DEVICE, one double
+ *   cube_out  DEVICE [n_x][n_y][n_channels] fp32 or NULL: receives the final cube when non-NULL
+ *   g_*       as rubix_cube_adjoint
+ * Needs rubix_loss_and_grad_workspace_bytes(...) bytes of workspace (one more cube-sized buffer than
+ * rubix_workspace_bytes, plus the loss partials); returns 0 on invalid arguments. */
+size_t rubix_loss_and_grad_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel);
+rubix_status rubix_loss_and_grad(const rubix_particles *particles, const rubix_ssp *ssp,
+                                 const rubix_telescope *tel, const float *R, const float *target,
+                                 double *loss, float *cube_out, float *g_mass, float *g_log_age,
+                                 float *g_log_z, float *g_vlos, void *workspace, size_t workspace_bytes,
+                                 void *stream);
+
 /* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_cube_adjoint on
  * this workspace address (compared bit for bit with the oracle):
  *   key     [n]      spaxel key of each particle in original order (n_s = dropped)

@@ -20,6 +20,7 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error",
+           "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
 N_STAGES = 5
@@ -76,6 +77,13 @@ def load():
         lib.rubix_cube_adjoint.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_loss_and_grad_workspace_bytes.restype = C.c_size_t
+        lib.rubix_loss_and_grad_workspace_bytes.argtypes = [C.c_int64, C.POINTER(CSSP), C.POINTER(CTelescope)]
+        lib.rubix_loss_and_grad.restype = C.c_int
+        lib.rubix_loss_and_grad.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
+                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
+                                            C.c_void_p]
         lib.rubix_get_sort_artifacts.restype = C.c_int
         lib.rubix_get_sort_artifacts.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                                  C.POINTER(C.c_void_p)]
@@ -190,6 +198,23 @@ def rubix_cube_adjoint(particles: _Keep, ssp: _Keep, tel: _Keep, R, grad_cube, g
                                      int(workspace.numel() * workspace.element_size()), _stream(stream)))
 
 
+def rubix_loss_and_grad_workspace_bytes(n, ssp: _Keep, tel: _Keep) -> int:
+    b = int(load().rubix_loss_and_grad_workspace_bytes(int(n), ssp.ref(), tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_loss_and_grad(particles: _Keep, ssp: _Keep, tel: _Keep, R, target, loss, cube_out, g_mass,
+                        g_log_age, g_log_z, g_vlos, workspace, stream=None):
+    """``loss``: one-element float64 device tensor; ``cube_out``: device tensor or None."""
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_loss_and_grad(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(target),
+                                      _ptr(loss), _ptr(cube_out), _ptr(g_mass), _ptr(g_log_age),
+                                      _ptr(g_log_z), _ptr(g_vlos), _ptr(workspace),
+                                      int(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
 def rubix_get_sort_artifacts(workspace, n, n_s):
     """(key[n], perm[n], seg_off[n_s+2]) as int32 torch tensors copied out of the workspace."""
     import torch
@@ -283,6 +308,19 @@ class DeviceWorkload:
         g = [torch.empty(n, dtype=torch.float32, device=self.device) for _ in range(4)]
         rubix_cube_adjoint(self.particles, self.ssp, self.tel, self.R, grad_cube, *g, self.workspace)
         return g
+
+    def loss_and_grad(self, target, want_cube=False):
+        """(loss [1] float64, (g_mass, g_log_age, g_log_z, g_vlos), final cube or None) in one fused call."""
+        import torch
+        n = self.w.particles.n
+        need = rubix_loss_and_grad_workspace_bytes(n, self.ssp, self.tel)
+        if self.workspace.numel() < need:
+            self.workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
+        loss = torch.zeros(1, dtype=torch.float64, device=self.device)
+        cube = torch.empty(self.shape, dtype=torch.float32, device=self.device) if want_cube else None
+        g = [torch.empty(n, dtype=torch.float32, device=self.device) for _ in range(4)]
+        rubix_loss_and_grad(self.particles, self.ssp, self.tel, self.R, target, loss, cube, *g, self.workspace)
+        return loss, g, cube
 
     def sort_artifacts(self):
         t = self.w.telescope

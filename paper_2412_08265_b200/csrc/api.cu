@@ -244,6 +244,84 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
     return RUBIX_OK;
 }
 
+size_t rubix_loss_and_grad_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
+{
+    const size_t base = rubix_workspace_bytes(n, ssp, tel);
+    if (base == 0) return 0;
+    const size_t cube_bytes = (size_t)tel->n_x * tel->n_y * tel->n_channels * 4;
+    return base + align_up(cube_bytes, 256) + loss_scratch_bytes();
+}
+
+rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                                 const float *R, const float *target, double *loss, float *cube_out,
+                                 float *g_mass, float *g_log_age, float *g_log_z, float *g_vlos,
+                                 void *workspace, size_t workspace_bytes, void *stream)
+{
+    t_err[0] = 0;
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !target || !loss) return fail(RUBIX_ERR_NULL, "R, target or loss is NULL");
+    if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
+        return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
+                                 ssp->n_lambda);
+    const int64_t n_vox = (int64_t)tel->n_x * tel->n_y * tel->n_channels;
+    const size_t cube_al = align_up((size_t)n_vox * 4, 256);
+    if ((s = check_ws(workspace, workspace_bytes, L.bytes_total + cube_al + loss_scratch_bytes())) != RUBIX_OK)
+        return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    float *buf_a = (float *)(ws + L.off_cube_a), *buf_b = (float *)(ws + L.off_cube_b);
+    float *buf_c = (float *)(ws + L.bytes_total);
+    double *partial = (double *)(ws + L.bytes_total + cube_al);
+    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
+    PassInputs in{p, ssp, tel, R};
+    cudaError_t e;
+    {
+        StageTimer t(0, st);
+        e = launch_particle_pass(in, L, ws, st);           // ONE particle pass serves forward and adjoint
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+    // forward: raw cube, then PSF/LSF
+    float *raw = conv ? buf_a : (cube_out ? cube_out : buf_a);
+    e = launch_accumulate(in, L, ws, raw, st);
+    if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+    const float *final_cube = raw;
+    if (conv) {
+        float *fin = cube_out ? cube_out : buf_c;
+        {
+            StageTimer t(3, st);
+            e = launch_convolve(tel, raw, fin, buf_b, st);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "convolve");
+        final_cube = fin;
+    }
+    // loss and upstream gradient 2 (cube - target); the raw cube is no longer needed when conv is on
+    float *grad = conv ? buf_a : buf_b;
+    e = launch_residual_loss(final_cube, target, n_vox, grad, partial, loss, st);
+    if (e != cudaSuccess) return cuda_fail(e, "loss");
+    const float *gconv = grad;
+    if (conv) {                                            // G' = LSF^T PSF^T G (self-adjoint stencils)
+        {
+            StageTimer t(3, st);
+            e = launch_convolve(tel, grad, buf_c, buf_b, st);   // buf_c is free: the final cube has been consumed
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
+        gconv = buf_c;
+    }
+    {
+        StageTimer t(4, st);
+        e = launch_adjoint(in, L, ws, gconv, g_mass, g_log_age, g_log_z, g_vlos, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "adjoint");
+    remember(workspace, L);
+    return RUBIX_OK;
+}
+
 rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key, const int32_t **perm,
                                       const int32_t **seg_off)
 {

@@ -1,0 +1,73 @@
+// Quadratic cube loss for the fused forward + adjoint entry point (BASELINE.json
+// configs[4]: L = sum (cube - target)^2).  One pass over the final cube and the target:
+//   grad[v] = 2 (cube[v] - target[v])                          (the upstream gradient of step 9)
+//   L       = sum_v (cube[v] - target[v])^2                    in fp64, FIXED order: per-thread
+//             grid-stride partial -> warp shuffle tree -> block tree -> one partial per CTA, then a
+//             single CTA adds the partials in index order, so the value is bit-reproducible.
+#include "common.cuh"
+
+namespace rubix {
+
+constexpr int kLossBlocks = 1184;          // 8 CTAs per SM
+constexpr int kLossThreads = 256;
+
+__device__ __forceinline__ double block_sum(double v, double *sm)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < kLossThreads / 32; ++w) t += sm[w];
+    return t;                               // valid in thread 0
+}
+
+__global__ void __launch_bounds__(kLossThreads)
+k_residual_loss(const float *__restrict__ cube, const float *__restrict__ target, int64_t n_vox,
+                float *__restrict__ grad, double *__restrict__ partial)
+{
+    __shared__ double sm[kLossThreads / 32];
+    double acc = 0.0;
+    const int64_t n4 = n_vox >> 2;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        const float4 c = __ldcs(reinterpret_cast<const float4 *>(cube) + i);
+        const float4 t = __ldcs(reinterpret_cast<const float4 *>(target) + i);
+        const float4 r = make_float4(c.x - t.x, c.y - t.y, c.z - t.z, c.w - t.w);
+        __stcs(reinterpret_cast<float4 *>(grad) + i, make_float4(2.0f * r.x, 2.0f * r.y, 2.0f * r.z, 2.0f * r.w));
+        acc += (double)r.x * r.x + (double)r.y * r.y + (double)r.z * r.z + (double)r.w * r.w;
+    }
+    for (int64_t i = (n4 << 2) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_vox; i += stride) {
+        const float r = cube[i] - target[i];
+        grad[i] = 2.0f * r;
+        acc += (double)r * r;
+    }
+    const double tot = block_sum(acc, sm);
+    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(kLossThreads)
+k_loss_final(const double *__restrict__ partial, int n, double *__restrict__ loss)
+{
+    __shared__ double sm[kLossThreads / 32];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += kLossThreads) acc += partial[i];
+    const double tot = block_sum(acc, sm);
+    if (threadIdx.x == 0) *loss = tot;
+}
+
+size_t loss_scratch_bytes() { return align_up((size_t)kLossBlocks * sizeof(double), 256); }
+
+cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
+                                 double *partial, double *loss, cudaStream_t st)
+{
+    k_residual_loss<<<kLossBlocks, kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial);
+    RUBIX_LAUNCH_CHECK();
+    k_loss_final<<<1, kLossThreads, 0, st>>>(partial, kLossBlocks, loss);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
+}  // namespace rubix

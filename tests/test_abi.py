@@ -143,6 +143,21 @@ def test_convolve_and_adjoint_validation(lib):
     assert lib.rubix_get_sort_artifacts(0x20000, C.byref(k), C.byref(k), C.byref(k)) == B.RUBIX_ERR_INVALID_ARG
 
 
+def test_loss_and_grad_validation(lib):
+    ssp, tel = _structs()
+    P = _fake_particles()
+    R = np.eye(3, dtype=np.float32).reshape(9)
+    f = lib.rubix_loss_and_grad
+    args = lambda target=FAKE, loss=FAKE, ws_bytes=1 << 40: (P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, target, loss,
+                                                             None, FAKE, FAKE, FAKE, FAKE, FAKE, ws_bytes, None)
+    assert f(*args(target=None)) == B.RUBIX_ERR_NULL
+    assert f(*args(loss=None)) == B.RUBIX_ERR_NULL
+    plain = B.rubix_workspace_bytes(10, ssp, tel)
+    fused = B.rubix_loss_and_grad_workspace_bytes(10, ssp, tel)
+    assert fused >= plain + 300 * 300 * 3700 * 4
+    assert f(*args(ws_bytes=plain)) == B.RUBIX_ERR_WORKSPACE            # one cube-sized buffer short
+
+
 def test_no_cpu_fallback_without_the_library(monkeypatch):
     monkeypatch.setattr(B, "_lib", None)
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/librubix_b200.so")
