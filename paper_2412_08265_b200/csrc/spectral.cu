@@ -187,17 +187,19 @@ k_accumulate(const __grid_constant__ AccumParams P)
             for (int d = 0; d < DEPTH; ++d)
                 if ((warp + d * kAccWarps) * kPass < W.nw) issue(L[d], t0 + d * kStep);
         };
+        // every pass sits at a compile-time offset from one per-particle pointer (immediate load / store
+        // offsets, no loop-carried address arithmetic); a warp has at most kTabMax / kStep passes
+        constexpr int kMaxPass = kTabMax / kStep;
         auto blend_all = [&](LoadSet (&L)[DEPTH], const Win &W, float *buf) {
             const float *t0 = P.flux + (W.first + warp * kPass + 4 * lane);
             float *dst = buf + warp * kPass + 4 * lane;
-            int s0 = warp * kPass;                          // first sample of the pass held by L[0]
-            while (true) {
+            const int left = W.nw - warp * kPass;           // samples from this warp's first pass to the end
 #pragma unroll
-                for (int d = 0; d < DEPTH; ++d) {
-                    if (s0 >= W.nw) return;
-                    consume(L[d], W, dst);
-                    if (s0 + DEPTH * kStep < W.nw) issue(L[d], t0 + DEPTH * kStep);
-                    s0 += kStep; t0 += kStep; dst += kStep;
+            for (int ps = 0; ps < kMaxPass; ++ps) {
+                if (ps * kStep < left) {
+                    consume(L[ps % DEPTH], W, dst + ps * kStep);
+                    if (ps + DEPTH < kMaxPass && (ps + DEPTH) * kStep < left)
+                        issue(L[ps % DEPTH], t0 + (ps + DEPTH) * kStep);
                 }
             }
         };
