@@ -18,6 +18,9 @@
  *     never synchronises: all work is enqueued on `stream` (a cudaStream_t passed as void*)
  *     and is complete when the stream is.  Host arrays (R, the SSP axes, the structs) are
  *     read before the call returns and may be freed right after it.
+ *     Consequently a sequence of calls can be captured in a CUDA graph (stage timing of
+ *     rubix_peaks.h off) and replayed; the kernels read their sizes from the workspace, not
+ *     from the host, after the call has returned.
  *   - Device arrays are dense, row-major, fp32 / int32 as stated, 16-byte aligned.
  *   - Errors: every call validates its arguments on the host BEFORE any launch and returns a
  *     rubix_status; nothing throws or aborts.  rubix_last_error() gives a thread-local message.
