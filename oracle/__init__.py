@@ -54,6 +54,14 @@ def n_threads() -> int:
     return int(env) if env else (os.cpu_count() or 1)
 
 
+def _mode(tel, ssp):
+    """bit 0: resampling rule (0 point-sampled, 1 flux-conserving); bit 1: log-sampled SSP grid."""
+    resample, log_grid = int(getattr(tel, "resample", 0)), int(getattr(ssp, "log_lambda", 0))
+    if resample == 1 and log_grid:
+        raise NotImplementedError("flux-conserving resampling is defined for linearly sampled SSP grids only")
+    return resample | (log_grid << 1)
+
+
 def _f32(a):
     return np.ascontiguousarray(a, dtype=np.float32)
 
@@ -114,7 +122,7 @@ def particle_spectrum(mass, log_age, log_z, vlos, ssp, tel):
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
     _load().orc_particle_spectrum_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
         C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
         C.c_float(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
@@ -130,7 +138,7 @@ def particle_spectrum_f64(mass, log_age, log_z, vlos, ia, iz, ssp, tel):
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
     _load().orc_particle_spectrum_f64_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
         C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
         C.c_double(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
         _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
@@ -157,7 +165,7 @@ def build_cube(particles, R, ssp, tel, sel=None):
         n_sel = sel_arr.size
         cube = np.empty((n_sel, n_c), np.float64)
     _load().orc_build_cube_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
         C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
         C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis),
         C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
@@ -227,7 +235,7 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
     _load().orc_adjoint_mode(
-        C.c_int32(int(getattr(tel, "resample", 0))), C.c_double(float(getattr(tel, "redshift", 0.0))),
+        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
         C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
         C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis), C.c_float(float(ssp.lambda0)),
         C.c_float(float(ssp.dlambda)), _pf(flux), C.c_int32(tel.n_x), C.c_int32(tel.n_y),

@@ -129,8 +129,11 @@ void orc_ssp_cells(int64_t n, const float *log_age, const float *log_z, int32_t 
 static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, double tz,
                               double vlos, const float *flux, int32_t n_z, int32_t n_lambda,
                               double l0_ssp, double dl_ssp, int32_t k_begin, int32_t k_end,
-                              double l0_obs, double dl_obs, double *F, double *dS)
-{   /* fills F[k] (and dS[k]) for channels k_begin <= k < k_end */
+                              double l0_obs, double dl_obs, double *F, double *dS, int32_t log_grid)
+{   /* fills F[k] (and dS[k]) for channels k_begin <= k < k_end.
+     * log_grid = 1 (reading R15): the SSP grid is log-sampled, lambda_j = l0_ssp * 10^(j dl_ssp)
+     * (dl_ssp in dex), the sampling coordinate is x = log10(lambda_rest / l0_ssp) / dl_ssp and the
+     * interpolant is linear in x between knots: numpy.interp(log10 lambda_rest, log10 lambda_ssp, S). */
     const float *T00 = flux + ((int64_t)ia * n_z + iz) * n_lambda;
     const float *T10 = flux + ((int64_t)(ia + 1) * n_z + iz) * n_lambda;
     const float *T01 = flux + ((int64_t)ia * n_z + iz + 1) * n_lambda;
@@ -139,7 +142,8 @@ static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, do
     const double w01 = (1.0 - ta) * tz, w11 = ta * tz;
     const double beta = vlos / ORC_C_KMS;
     const double lam_first = l0_ssp;
-    const double lam_last = l0_ssp + dl_ssp * (double)(n_lambda - 1);
+    const double lam_last = log_grid ? l0_ssp * pow(10.0, dl_ssp * (double)(n_lambda - 1))
+                                     : l0_ssp + dl_ssp * (double)(n_lambda - 1);
     for (int32_t k = k_begin; k < k_end; ++k) {
         const double lam_obs = l0_obs + dl_obs * (double)k;
         const double lam_rest = lam_obs / (1.0 + beta);
@@ -148,7 +152,8 @@ static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, do
             if (dS) dS[k] = 0.0;
             continue;
         }
-        const double x = (lam_rest - l0_ssp) / dl_ssp;
+        double x = log_grid ? log10(lam_rest / l0_ssp) / dl_ssp : (lam_rest - l0_ssp) / dl_ssp;
+        if (x < 0.0) x = 0.0;                              /* rounding at the first knot */
         int32_t j = (int32_t)floor(x);
         if (j > n_lambda - 2) j = n_lambda - 2;
         const double f = x - (double)j;
@@ -211,18 +216,19 @@ static void particle_spectrum_flux(double mass, int32_t ia, int32_t iz, double t
     }
 }
 
-/* mode 0: point-sampled linear interpolation; mode 1: bin average */
+/* mode bit 0: 0 = point-sampled linear interpolation, 1 = bin average (R13);
+ * mode bit 1: SSP grid log-sampled (R15; point-sampled rule only) */
 static void particle_spectrum_mode(int32_t mode, double mass, int32_t ia, int32_t iz, double ta,
                                    double tz, double vlos, const float *flux, int32_t n_z,
                                    int32_t n_lambda, double l0_ssp, double dl_ssp, int32_t k_begin,
                                    int32_t k_end, double l0_obs, double dl_obs, double *F)
 {
-    if (mode == 1)
+    if ((mode & 1) == 1)
         particle_spectrum_flux(mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp, dl_ssp,
                                k_begin, k_end, l0_obs, dl_obs, F);
     else
         particle_spectrum(mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp, dl_ssp, k_begin,
-                          k_end, l0_obs, dl_obs, F, 0);
+                          k_end, l0_obs, dl_obs, F, 0, (mode >> 1) & 1);
 }
 
 /* Cosmological redshift and flux scaling (reading R14; "Doppler shifted based
@@ -254,7 +260,7 @@ void orc_particle_spectrum(float mass, float log_age, float log_z, float vlos, i
     axis_cell(age_axis, n_age, log_age, &ia, &ta);
     axis_cell(z_axis, n_z, log_z, &iz, &tz);
     particle_spectrum((double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
-                      (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs, (double)dl_obs, F, 0);
+                      (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs, (double)dl_obs, F, 0, 0);
 }
 
 /* Same, but with the interpolation parameters given in fp64 (finite differences perturb
@@ -546,7 +552,7 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                 D[c] = acc;  /* c = 0:(i,j) 1:(i+1,j) 2:(i,j+1) 3:(i+1,j+1) */
             }
             double E = 0.0;
-            if (mode == 1) {
+            if ((mode & 1) == 1) {
                 /* Flux-conserving rule.  F[k] = (C(x_hi) - C(x_lo)) / B with C' = S~, the bin edges
                  * x(lambda_e) = (lambda_e/(1+beta) - l0_ssp)/dl_ssp and B = dl_obs/((1+beta) dl_ssp):
                  *   dF[k]/dbeta = F[k]/(1+beta) - (lambda_hi S~(x_hi) - lambda_lo S~(x_lo)) / (dl_obs (1+beta)),
@@ -555,7 +561,7 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                  * unit-mass spectrum, point-evaluated at the n_c + 1 bin edges. */
                 particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
                                   (double)l0_ssp, (double)dl_ssp, 0, n_c + 1,
-                                  (double)l0_obs - 0.5 * (double)dl_obs, (double)dl_obs, F, 0);
+                                  (double)l0_obs - 0.5 * (double)dl_obs, (double)dl_obs, F, 0, 0);
                 for (int32_t k = 0; k < n_c; ++k) {
                     const double lam_lo = (double)l0_obs + (double)dl_obs * ((double)k - 0.5);
                     const double lam_hi = lam_lo + (double)dl_obs;
@@ -565,9 +571,15 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                 /* E: needs the slope of the blended unit-mass spectrum */
                 particle_spectrum(1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z, n_lambda,
                                   (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
-                                  (double)dl_obs, F, dS);
-                for (int32_t k = 0; k < n_c; ++k)
-                    E += g[k] * ((double)l0_obs + (double)dl_obs * k) * dS[k] / (double)dl_ssp;
+                                  (double)dl_obs, F, dS, (mode >> 1) & 1);
+                /* dF/dbeta = dS/dx * dx/dbeta;  linear grid: dx/dbeta = -lambda_k / ((1+beta)^2 dl_ssp);
+                 * log grid: x = log10(lambda_k / ((1+beta) l0_ssp)) / dl_ssp, dx/dbeta = -1 / ((1+beta) dl_ssp ln 10),
+                 * written as the same expression with lambda_k replaced by (1+beta) / ln 10 */
+                for (int32_t k = 0; k < n_c; ++k) {
+                    const double lam_eff = ((mode >> 1) & 1) ? (1.0 + (double)vlos[p] / ORC_C_KMS) / log(10.0)
+                                                             : (double)l0_obs + (double)dl_obs * k;
+                    E += g[k] * lam_eff * dS[k] / (double)dl_ssp;
+                }
             }
             const double m = scale * (double)mass[p];
             const double beta = (double)vlos[p] / ORC_C_KMS;
@@ -584,7 +596,7 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                                   : 0.0;
             g_log_z[p] = z_free ? m * (-(1 - ta) * D[0] - ta * D[1] + (1 - ta) * D[2] + ta * D[3]) / dZ
                                 : 0.0;
-            if (mode == 1)
+            if ((mode & 1) == 1)
                 g_vlos[p] = m * (g_mass[p] - E / (double)dl_obs) / (ORC_C_KMS * (1.0 + beta));
             else
                 g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));

@@ -119,15 +119,19 @@ class SSPGrid:
     log_age_axis: np.ndarray  # [n_age] fp32, strictly increasing, log10(age/Gyr)
     log_z_axis: np.ndarray    # [n_z]   fp32, strictly increasing, log10(Z)
     lambda0: np.float32       # first rest wavelength, Angstrom
-    dlambda: np.float32       # uniform rest step, Angstrom
+    dlambda: np.float32       # uniform rest step: Angstrom, or dex (log10) when log_lambda = 1
     flux: np.ndarray          # [n_age, n_z, n_lambda] fp32, per unit mass, > 0
+    log_lambda: int = 0       # 1: log-sampled grid, lambda_j = lambda0 * 10^(j dlambda)
 
     @property
     def shape(self):
         return self.flux.shape
 
     def wavelengths(self) -> np.ndarray:
-        return np.float64(self.lambda0) + np.float64(self.dlambda) * np.arange(self.flux.shape[2])
+        j = np.arange(self.flux.shape[2])
+        if self.log_lambda:
+            return np.float64(self.lambda0) * 10.0 ** (np.float64(self.dlambda) * j)
+        return np.float64(self.lambda0) + np.float64(self.dlambda) * j
 
 
 def _jittered_axis(rng, lo, hi, n):
@@ -139,7 +143,7 @@ def _jittered_axis(rng, lo, hi, n):
 
 
 def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
-             seed: int, n_lines: int = 10) -> SSPGrid:
+             seed: int, n_lines: int = 10, log_lambda: bool = False) -> SSPGrid:
     """Smooth positive continuum times ``n_lines`` Gaussian absorption lines whose depths vary
     with age and Z (BASELINE.json configs[0]; recipe SURVEY.md §8(d))."""
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -147,6 +151,9 @@ def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
     z_ax = _jittered_axis(rng, -4.0, math.log10(0.03), n_z)
     dlam = (lam_hi - lam_lo) / (n_lambda - 1)
     lam = lam_lo + dlam * np.arange(n_lambda)
+    dlog = math.log10(lam_hi / lam_lo) / (n_lambda - 1)
+    if log_lambda:                                         # same recipe on a log-sampled grid (MaStar "SLOG")
+        lam = lam_lo * 10.0 ** (dlog * np.arange(n_lambda))
     u = ((age_ax - age_ax[0]) / (age_ax[-1] - age_ax[0]))[:, None, None]
     w = ((z_ax - z_ax[0]) / (z_ax[-1] - z_ax[0]))[None, :, None]
     ell = (lam / 5500.0)[None, None, :]
@@ -160,8 +167,8 @@ def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
         d = depth0[l] * (0.3 + 0.7 * (mix[l] * u + (1.0 - mix[l]) * w))
         flux = flux * (1.0 - d * np.exp(-0.5 * ((lam[None, None, :] - centre[l]) / width[l]) ** 2))
     return SSPGrid(age_ax.astype(np.float32), z_ax.astype(np.float32),
-                   np.float32(lam_lo), np.float32(dlam),
-                   np.ascontiguousarray(flux, dtype=np.float32))
+                   np.float32(lam_lo), np.float32(dlog if log_lambda else dlam),
+                   np.ascontiguousarray(flux, dtype=np.float32), 1 if log_lambda else 0)
 
 
 # --------------------------------------------------------------------------------------
