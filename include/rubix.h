@@ -67,6 +67,11 @@ typedef struct {
     const float *log_z_axis;        /* HOST [n_z],   strictly increasing                    */
     float lambda0, dlambda;         /* uniform rest-frame grid, Angstrom, dlambda > 0       */
     const float *flux;              /* DEVICE [n_age][n_z][n_lambda], per unit mass         */
+    int32_t log_lambda;             /* 0: lambda_j = lambda0 + j dlambda (Angstrom);          */
+                                    /* 1: log-sampled grid (e.g. MaStar "SLOG"): */
+                                    /*    lambda_j = lambda0 * 10^(j dlambda), dlambda in dex; */
+                                    /*    the interpolant is then linear in log lambda between */
+                                    /*    knots; RUBIX_RESAMPLE_POINT only                     */
 } rubix_ssp;
 
 /* Detector ("telescope-specific configurations", L44 Gaussian PSF and LSF). */

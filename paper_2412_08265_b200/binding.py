@@ -41,7 +41,8 @@ class CParticles(C.Structure):
 class CSSP(C.Structure):
     _fields_ = [("n_age", C.c_int32), ("n_z", C.c_int32), ("n_lambda", C.c_int32),
                 ("log_age_axis", C.c_void_p), ("log_z_axis", C.c_void_p),
-                ("lambda0", C.c_float), ("dlambda", C.c_float), ("flux", C.c_void_p)]
+                ("lambda0", C.c_float), ("dlambda", C.c_float), ("flux", C.c_void_p),
+                ("log_lambda", C.c_int32)]
 
 
 class CTelescope(C.Structure):
@@ -153,7 +154,7 @@ def c_ssp(ssp, flux) -> _Keep:
     age, zed = _host_f32(ssp.log_age_axis), _host_f32(ssp.log_z_axis)
     n_age, n_z, n_lambda = (int(v) for v in flux.shape)
     return _Keep(CSSP(n_age, n_z, n_lambda, age.ctypes.data, zed.ctypes.data, float(ssp.lambda0),
-                      float(ssp.dlambda), _ptr(flux)), age, zed, flux)
+                      float(ssp.dlambda), _ptr(flux), int(getattr(ssp, "log_lambda", 0))), age, zed, flux)
 
 
 def c_particles(pos, vel, mass, log_age, log_z) -> _Keep:

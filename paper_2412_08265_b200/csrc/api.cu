@@ -45,6 +45,10 @@ rubix_status check_ssp(const rubix_ssp *s, bool flux_required)
         return fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
     if (!(s->dlambda > 0.0f) || !isfinite(s->dlambda) || !isfinite(s->lambda0))
         return fail(RUBIX_ERR_INVALID_ARG, "ssp dlambda must be > 0 and finite");
+    if (s->log_lambda != 0 && s->log_lambda != 1)
+        return fail(RUBIX_ERR_INVALID_ARG, "ssp log_lambda must be 0 or 1");
+    if (s->log_lambda == 1 && !(s->lambda0 > 0.0f))
+        return fail(RUBIX_ERR_INVALID_ARG, "a log-sampled ssp grid needs lambda0 > 0");
     if (s->n_age > kMaxAge || s->n_z > kMaxZ)
         return fail(RUBIX_ERR_UNSUPPORTED, "ssp axes limited to n_age <= %d, n_z <= %d", kMaxAge, kMaxZ);
     if ((double)s->n_age * s->n_z * s->n_lambda >= 2147483648.0)
@@ -99,6 +103,18 @@ rubix_status check_particles(const rubix_particles *p)
 
 rubix_status check_resampler(const rubix_ssp *s, const rubix_telescope *t)
 {
+    if (s->log_lambda) {
+        if (t->resample != RUBIX_RESAMPLE_POINT)
+            return fail(RUBIX_ERR_UNSUPPORTED, "log-sampled ssp grids support RUBIX_RESAMPLE_POINT only");
+        // steepest d x / d k is at the first channel: dlambda_obs / (lambda_obs ln10 dlog)
+        const double lam_min = (double)t->lambda0 < (double)t->lambda0 + (double)t->dlambda * (t->n_channels - 1)
+                                   ? (double)t->lambda0 : (double)t->lambda0 + (double)t->dlambda * (t->n_channels - 1);
+        if (!(lam_min > 0.0)) return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths must be > 0 for a log-sampled ssp grid");
+        const double b0 = (double)t->dlambda / (lam_min * 2.302585092994046 * (double)s->dlambda);
+        if (b0 >= 14.25)
+            return fail(RUBIX_ERR_UNSUPPORTED, "d x / d channel = %.3f is outside the resampler range (< 14.25)", b0);
+        return RUBIX_OK;
+    }
     const double b_max = (double)t->dlambda / (double)s->dlambda / (1.0 - kBetaCap);
     if (b_max >= 15.0)
         return fail(RUBIX_ERR_UNSUPPORTED, "dlambda_obs / dlambda_ssp = %.3f is outside the resampler range (< 14.25)",

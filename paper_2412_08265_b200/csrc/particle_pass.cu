@@ -314,6 +314,8 @@ struct PrepParams {
     int32_t n_lambda, pitch, n_c, n_s, mode;
     float l0_ssp, dl_ssp, l0_obs, dl_obs;
     float redshift, flux_scale;         // DESIGN.md reading R14
+    int32_t log_grid;                   // reading R15: x_k = xtab[k] - log10(1+beta)/dlog
+    const int64_t *xtab;
 };
 
 __device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *cell, double *t)
@@ -359,7 +361,19 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     const int64_t b = (int64_t)b_fx;
     const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
     int64_t k_lo, k_hi, x_first, x_last;
-    if (P.mode == RUBIX_RESAMPLE_FLUX) {
+    if (P.log_grid) {
+        // x_k = xtab[k] + a_fx with a_fx = -log10(1 + beta) / dlog: the Doppler shift is a constant offset
+        // on a log-sampled grid; xtab is increasing, so the covered channels are found by bisection
+        a_fx = -__double2ll_rn(log10(1.0 + (double)vlos[p] / kCkms) / (double)P.dl_ssp * scale);
+        int lo = 0, hi = P.n_c;                            // first k with xtab[k] + a_fx >= 0
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (P.xtab[mid] + a_fx >= 0) hi = mid; else lo = mid + 1; }
+        k_lo = lo;
+        lo = -1; hi = P.n_c - 1;                           // last k with xtab[k] + a_fx <= x_max
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (P.xtab[mid] + a_fx <= x_max) lo = mid; else hi = mid - 1; }
+        k_hi = lo;
+        x_first = k_lo <= k_hi ? P.xtab[k_lo] + a_fx : 0;
+        x_last = k_lo <= k_hi ? P.xtab[k_hi] + a_fx : 0;
+    } else if (P.mode == RUBIX_RESAMPLE_FLUX) {
         // x_k = a_fx + b k is the LOWER EDGE of bin k (upper edge = lower edge of bin k + 1);
         // [k_lo, k_hi] = bins that overlap the coverage [0, N_l - 1]
         a_fx -= (int64_t)(b_fx >> 1);
@@ -392,6 +406,18 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
         r.nw = (int32_t)(x_last >> kFxFrac) - r.j0 + 2;   // samples j0 .. j_max + 1
     }
     rec[i] = r;
+}
+
+// --------------------------------------------------------------------------------------------
+// Log-sampled SSP grid (reading R15): rest position of channel k at beta = 0, in SSP samples,
+//   X0[k] = log10(lambda_k / ((1 + z) lambda0_ssp)) / dlog          (fp64 -> 36.28 fixed point)
+// --------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_log_positions(int32_t n_c, double l0_obs, double dl_obs, double l0_ssp, double dlog, int64_t *__restrict__ xtab)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > n_c) return;
+    xtab[k] = __double2ll_rn(log10((l0_obs + dl_obs * (double)k) / l0_ssp) / dlog * (double)(1 << kFxFrac));
 }
 
 // --------------------------------------------------------------------------------------------
@@ -471,6 +497,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.pitch = (n_lambda + kRowAlign - 1) / kRowAlign * kRowAlign;
     off = align_up(off, 512);                            // (texture-alignment safe)
     L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
+    L.off_xtab = take(((size_t)n_c + 1) * 8);           // X0[k] of a log-sampled SSP grid (reading R15)
     L.bytes_total = off;
     return L;
 }
@@ -560,6 +587,15 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.n_c = in.tel->n_channels;
         P.n_s = n_s;
         P.mode = in.tel->resample;
+        P.log_grid = in.ssp->log_lambda;
+        P.xtab = (const int64_t *)(ws + L.off_xtab);
+        if (P.log_grid) {
+            const double zp1 = 1.0 + (double)in.tel->redshift;
+            k_log_positions<<<(unsigned)((L.n_c + 256) / 256), 256, 0, st>>>(
+                L.n_c, (double)in.tel->lambda0 / zp1, (double)in.tel->dlambda / zp1, (double)in.ssp->lambda0,
+                (double)in.ssp->dlambda, (int64_t *)(ws + L.off_xtab));
+            RUBIX_LAUNCH_CHECK();
+        }
         P.redshift = in.tel->redshift;
         P.flux_scale = in.tel->flux_scale;
         P.l0_ssp = in.ssp->lambda0;

@@ -31,6 +31,7 @@ struct AccumParams {
     float *cube;
     float *partials;
     int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
+    const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
     cudaTextureObject_t tex;
 };
 
@@ -96,7 +97,9 @@ struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 // FLUX: flux-conserving resampling (RUBIX_RESAMPLE_FLUX): x_k is the lower edge of bin k and the
 // channel value is the exact integral of the table's piecewise-linear interpolant over
 // [x_k, x_{k+1}] (clipped to the SSP coverage), divided by the bin width B.
-template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX>
+// LOGX: log-sampled SSP grid (reading R15): x_k = xtab[k] + a (a = the particle's Doppler offset); the
+// thread keeps the positions of its CPT channels relative to the tile start in registers (12.20).
+template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX>
 __global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
@@ -112,8 +115,18 @@ k_accumulate(const __grid_constant__ AccumParams P)
     float *out = U.part_row >= 0 ? P.partials + (size_t)U.part_row * P.n_c
                                  : P.cube + (size_t)U.spaxel * P.n_c;
     float acc[CPT];
+    uint32_t xl[LOGX ? CPT : 1];
+    int64_t x_tile0 = 0;                                    // LOGX: xtab[k0]
 #pragma unroll
     for (int i = 0; i < CPT; ++i) acc[i] = 0.0f;
+    if (LOGX) {
+        x_tile0 = P.xtab[k0];
+#pragma unroll
+        for (int i = 0; i < CPT; ++i) {
+            const int k = k0 + tid + i * kAccThreads;
+            xl[i] = (uint32_t)((P.xtab[min(k, P.n_c)] - x_tile0) >> 8);
+        }
+    }
 
     if (U.count > 0) {
         int4 *srec = reinterpret_cast<int4 *>(tab + 2 * (size_t)P.wcap);
@@ -142,6 +155,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 j0 = 0; W.nw = 0;
                 if (W.ka <= W.kb) {
                     int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * (W.kb + (FLUX ? 1 : 0));
+                    if (LOGX) { xa = a + P.xtab[W.ka]; xb = a + P.xtab[W.kb]; }
                     if (FLUX) {                             // bins are clipped to the coverage
                         xa = max(xa, (int64_t)0);
                         xb = min(xb, (int64_t)(P.n_lambda - 1) << kFxFrac);
@@ -152,7 +166,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
             W.first = rb.x + j0;
             W.j0 = j0;
-            W.base = a + (int64_t)W.b * k0 - ((int64_t)j0 << kFxFrac);
+            W.base = a + (LOGX ? x_tile0 : (int64_t)W.b * k0) - ((int64_t)j0 << kFxFrac);
             return W;
         };
 
@@ -281,15 +295,16 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 return;
             }
             // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
-            const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
+            // LOGX: x = (tile-relative position of the channel) + (particle base), both truncated to 2^-20
+            const uint32_t x0 = LOGX ? (uint32_t)(W.base >> 8) : (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
 #pragma unroll
-                for (int i = 0; i < CPT; ++i) sample(i, x0 + (uint32_t)i * W.b, bytes);
+                for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + xl[i] : x0 + (uint32_t)i * W.b, bytes);
             } else {
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k >= W.ka && k <= W.kb) sample(i, x0 + (uint32_t)i * W.b, bytes);
+                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + xl[i] : x0 + (uint32_t)i * W.b, bytes);
                 }
             }
         };
@@ -362,10 +377,10 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
-template <int CPT, bool SINGLE, bool FLUX>
+template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false>
 static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, kAccMinBlocks, FLUX>;
+    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, LOGX ? 2 : kAccMinBlocks, FLUX, LOGX>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kAccThreads, smem, st>>>(P);
@@ -374,8 +389,11 @@ static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem,
 }
 
 template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, bool flux, unsigned grid, size_t smem, cudaStream_t st)
+static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsigned grid, size_t smem, cudaStream_t st)
 {
+    if (logx)
+        return P.n_tiles == 1 ? launch_acc2<CPT, true, false, true>(P, grid, smem, st)
+                              : launch_acc2<CPT, false, false, true>(P, grid, smem, st);
     if (P.n_tiles == 1)
         return flux ? launch_acc2<CPT, true, true>(P, grid, smem, st) : launch_acc2<CPT, true, false>(P, grid, smem, st);
     return flux ? launch_acc2<CPT, false, true>(P, grid, smem, st) : launch_acc2<CPT, false, false>(P, grid, smem, st);
@@ -405,8 +423,12 @@ int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, cudaStream_t st)
 {
+    const bool logx = in.ssp->log_lambda != 0;
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
-    const double b_max = b0 / (1.0 - kBetaCap);
+    // log-sampled grid: d x / d k = dlambda_obs / (lambda_k ln10 dlog), steepest at the first channel; a Doppler
+    // shift moves the window but does not stretch it
+    const double b_max = logx ? (double)in.tel->dlambda / ((double)in.tel->lambda0 * 2.302585092994046 * (double)in.ssp->dlambda)
+                              : b0 / (1.0 - kBetaCap);
     int wcap = 0;
     const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
     const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap);
@@ -425,6 +447,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
     P.n_lambda = in.ssp->n_lambda;
+    P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.tex = 0;
 #if RUBIX_TEX_CORNERS > 0
     {
@@ -452,11 +475,11 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     {
         StageTimer t(1, st);
         switch (cpt) {
-            case 15: e = launch_acc<15>(P, flux, grid, smem, st); break;
-            case 8: e = launch_acc<8>(P, flux, grid, smem, st); break;
-            case 4: e = launch_acc<4>(P, flux, grid, smem, st); break;
-            case 2: e = launch_acc<2>(P, flux, grid, smem, st); break;
-            default: e = launch_acc<1>(P, flux, grid, smem, st); break;
+            case 15: e = launch_acc<15>(P, flux, logx, grid, smem, st); break;
+            case 8: e = launch_acc<8>(P, flux, logx, grid, smem, st); break;
+            case 4: e = launch_acc<4>(P, flux, logx, grid, smem, st); break;
+            case 2: e = launch_acc<2>(P, flux, logx, grid, smem, st); break;
+            default: e = launch_acc<1>(P, flux, logx, grid, smem, st); break;
         }
     }
     if (e != cudaSuccess) return e;
