@@ -19,6 +19,7 @@ struct AdjParams {
     float l0_obs, dl_obs, dl_ssp;     // observed grid already divided by (1 + z)
     float flux_scale;
     const int64_t *xtab;              // log-sampled SSP grid (R15): x_k = xtab[k] + a_fx
+    double l0_over_dl;                // lambda0_obs / dlambda_obs (the (1+z) factors cancel)
     int64_t n;
 };
 
@@ -185,14 +186,24 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
     bool a_free, z_free;
     adj_axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta, &wa, &a_free);
     adj_axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz, &wz, &z_free);
-    const float u0 = (float)((1.0 - ta) * (1.0 - tz)), u1 = (float)(ta * (1.0 - tz));
-    const float u2 = (float)((1.0 - ta) * tz), u3 = (float)(ta * tz);
     const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
     const int64_t b = (int64_t)r.b_fx;
     const float inv_scale = 1.0f / (float)(1 << kFxFrac);
     double P0 = 0, Pa = 0, Pz = 0, Pq = 0, E = 0;
     const bool narrow = r.b_fx <= (1u << kFxFrac);
     const float width = (float)r.b_fx * inv_scale;
+    // lambda_e s(x_e) (g_{e-1} - g_e) / dl_obs for one edge, in fp64: lambda_e / dl_obs ~ 3000 multiplies the blended
+    // spectrum at the edge, and the sum over edges cancels to a derivative, so fp32 rounding of s(x_e) would show.
+    // `xrel` = x_e minus its knot (or x_e itself: only the low 28 bits are used, except for f = 1 at the last knot).
+    const double du0 = (1.0 - ta) * (1.0 - tz), du1 = ta * (1.0 - tz), du2 = (1.0 - ta) * tz, du3 = ta * tz;
+    auto edge_term = [&](int64_t xrel, int k, float dg, float a0, float a1, float a2, float a3, float b0, float b1,
+                         float b2, float b3) -> double {
+        const double fd = xrel == ((int64_t)1 << kFxFrac) ? 1.0
+                                                         : (double)(xrel & (((int64_t)1 << kFxFrac) - 1)) * (1.0 / (double)(1 << kFxFrac));
+        const double sa_ = du0 * a0 + du1 * a1 + du2 * a2 + du3 * a3;
+        const double sb_ = du0 * b0 + du1 * b1 + du2 * b2 + du3 * b3;
+        return (double)dg * (P.l0_over_dl + ((double)k - 0.5)) * (sa_ + fd * (sb_ - sa_));
+    };
     for (int k = r.k_lo + lane; k <= r.k_hi + 1; k += 32) {
         const int64_t xl = r.a_fx + b * k;                 // lower edge of bin k = edge k
         const float gk = k <= r.k_hi ? __ldg(g + k) : 0.0f;
@@ -219,11 +230,8 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
             sa = gk * da;
             sz = gk * dz;
             sq = gk * ((v3 - v2) - da);
-            const float e0 = fmaf(f, b0 - a0, a0), e1 = fmaf(f, b1 - a1, a1);
-            const float e2 = fmaf(f, b2 - a2, a2), e3 = fmaf(f, b3 - a3, a3);
-            const float lam = fmaf(P.dl_obs, (float)k - 0.5f, P.l0_obs);
-            se = (gm1 - gk) * lam * fmaf(u3, e3, fmaf(u2, e2, fmaf(u1, e1, u0 * e0)));
-            P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq; E += (double)se;
+            E += edge_term(xl & (((int64_t)1 << kFxFrac) - 1), k, gm1 - gk, a0, a1, a2, a3, b0, b1, b2, b3);
+            P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq;
             continue;
         }
         if (k <= r.k_hi) {                                  // ---- bin k
@@ -247,15 +255,12 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
             sq = gk * ((v3 - v2) - da);
         }
         if (xl >= 0 && xl <= x_max) {                       // ---- edge k inside the coverage
-            int j = (int)(xl >> kFxFrac);
-            float f = (float)(uint32_t)(xl & (((int64_t)1 << kFxFrac) - 1)) * inv_scale;
-            if (j > P.n_lambda - 2) { j = P.n_lambda - 2; f = 1.0f; }
+            const int j = min((int)(xl >> kFxFrac), P.n_lambda - 2);   // last knot: interval N_l - 2 with f = 1
             const uint32_t ju32 = (uint32_t)j;
-            const float a0 = __ldg(T0 + ju32), a1 = __ldg(T1 + ju32), a2 = __ldg(T2 + ju32), a3 = __ldg(T3 + ju32);
-            const float e0 = fmaf(f, __ldg(T0 + ju32 + 1) - a0, a0), e1 = fmaf(f, __ldg(T1 + ju32 + 1) - a1, a1);
-            const float e2 = fmaf(f, __ldg(T2 + ju32 + 1) - a2, a2), e3 = fmaf(f, __ldg(T3 + ju32 + 1) - a3, a3);
-            const float lam = fmaf(P.dl_obs, (float)k - 0.5f, P.l0_obs);
-            se = (gm1 - gk) * lam * fmaf(u3, e3, fmaf(u2, e2, fmaf(u1, e1, u0 * e0)));
+            const int64_t xe = (int64_t)j << kFxFrac;      // edge_term re-derives the fraction from xl - (j << 28)
+            E += edge_term(xl - xe, k, gm1 - gk, __ldg(T0 + ju32), __ldg(T1 + ju32), __ldg(T2 + ju32),
+                           __ldg(T3 + ju32), __ldg(T0 + ju32 + 1), __ldg(T1 + ju32 + 1), __ldg(T2 + ju32 + 1),
+                           __ldg(T3 + ju32 + 1));
         }
         P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq; E += (double)se;
     }
@@ -275,7 +280,7 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
         g_mass[p] = (float)((double)P.flux_scale * gm);
         g_age[p] = a_free ? (float)(m * inv_b * (Pa + tz * Pq) / wa) : 0.0f;
         g_z[p] = z_free ? (float)(m * inv_b * (Pz + ta * Pq) / wz) : 0.0f;
-        g_v[p] = (float)(m * (gm - E / (double)P.dl_obs) / (kCkms * opb));
+        g_v[p] = (float)(m * (gm - E) / (kCkms * opb));       // E carries the 1 / dl_obs already
     }
 }
 
@@ -296,6 +301,7 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.l0_obs = (float)((double)in.tel->lambda0 / (1.0 + (double)in.tel->redshift));
     P.dl_obs = (float)((double)in.tel->dlambda / (1.0 + (double)in.tel->redshift));
     P.flux_scale = in.tel->flux_scale;
+    P.l0_over_dl = (double)in.tel->lambda0 / (double)in.tel->dlambda;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
