@@ -62,6 +62,26 @@ def _mode(tel, ssp):
     return resample | (log_grid << 1)
 
 
+class _lambda_obs:
+    """Installs tel.lambda_obs (explicit observed wavelengths, reading R16) in the C oracle for one call."""
+
+    def __init__(self, tel):
+        arr = getattr(tel, "lambda_obs", None)
+        self.arr = None if arr is None else np.ascontiguousarray(arr, dtype=np.float32)
+        self.zp1 = 1.0 + float(getattr(tel, "redshift", 0.0))
+        if self.arr is not None and int(getattr(tel, "resample", 0)) != 0:
+            raise NotImplementedError("explicit observed wavelengths support the point-sampled rule only")
+
+    def __enter__(self):
+        if self.arr is not None:
+            assert self.arr.size == 0 or np.all(np.diff(self.arr) > 0)
+            _load().orc_set_lambda_obs(_pf(self.arr), C.c_double(self.zp1))
+
+    def __exit__(self, *exc):
+        if self.arr is not None:
+            _load().orc_set_lambda_obs(None, C.c_double(1.0))
+
+
 def _f32(a):
     return np.ascontiguousarray(a, dtype=np.float32)
 
@@ -121,13 +141,14 @@ def particle_spectrum(mass, log_age, log_z, vlos, ssp, tel):
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    _load().orc_particle_spectrum_mode(
-        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
-        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
-        C.c_float(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
-        _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
-        C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
-        _pd(out))
+    with _lambda_obs(tel):
+        _load().orc_particle_spectrum_mode(
+            C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
+            C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
+            C.c_float(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
+            _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
+            C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
+            _pd(out))
     return out
 
 
@@ -137,13 +158,14 @@ def particle_spectrum_f64(mass, log_age, log_z, vlos, ia, iz, ssp, tel):
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    _load().orc_particle_spectrum_f64_mode(
-        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
-        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
-        C.c_double(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
-        _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
-        C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
-        C.c_int32(int(ia)), C.c_int32(int(iz)), _pd(out))
+    with _lambda_obs(tel):
+        _load().orc_particle_spectrum_f64_mode(
+            C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
+            C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
+            C.c_double(float(vlos)), C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis),
+            _pf(z_axis), C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
+            C.c_int32(tel.n_channels), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
+            C.c_int32(int(ia)), C.c_int32(int(iz)), _pd(out))
     return out
 
 
@@ -164,14 +186,15 @@ def build_cube(particles, R, ssp, tel, sel=None):
         sel_arr = np.ascontiguousarray(sel, dtype=np.int32)
         n_sel = sel_arr.size
         cube = np.empty((n_sel, n_c), np.float64)
-    _load().orc_build_cube_mode(
-        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
-        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
-        C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis),
-        C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
-        C.c_int32(tel.n_x), C.c_int32(tel.n_y), C.c_float(float(tel.spaxel_size)),
-        C.c_int32(n_c), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
-        _pi(sel_arr), C.c_int32(n_sel), _pd(cube))
+    with _lambda_obs(tel):
+        _load().orc_build_cube_mode(
+            C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
+            C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
+            C.c_int32(na), C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis),
+            C.c_float(float(ssp.lambda0)), C.c_float(float(ssp.dlambda)), _pf(flux),
+            C.c_int32(tel.n_x), C.c_int32(tel.n_y), C.c_float(float(tel.spaxel_size)),
+            C.c_int32(n_c), C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)),
+            _pi(sel_arr), C.c_int32(n_sel), _pd(cube))
     return cube
 
 
@@ -234,15 +257,16 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     grad_cube = np.ascontiguousarray(grad_cube, dtype=np.float64)
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
-    _load().orc_adjoint_mode(
-        C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
-        C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
-        C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis), C.c_float(float(ssp.lambda0)),
-        C.c_float(float(ssp.dlambda)), _pf(flux), C.c_int32(tel.n_x), C.c_int32(tel.n_y),
-        C.c_float(float(tel.spaxel_size)), C.c_int32(tel.n_channels),
-        C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)), C.c_int32(tel.psf_size),
-        C.c_double(float(tel.psf_sigma)), C.c_int32(tel.lsf_size),
-        C.c_double(float(tel.lsf_sigma)), _pd(grad_cube), *(_pd(o) for o in out))
+    with _lambda_obs(tel):
+        _load().orc_adjoint_mode(
+            C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
+            C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
+            C.c_int32(nz), C.c_int32(nl), _pf(age_axis), _pf(z_axis), C.c_float(float(ssp.lambda0)),
+            C.c_float(float(ssp.dlambda)), _pf(flux), C.c_int32(tel.n_x), C.c_int32(tel.n_y),
+            C.c_float(float(tel.spaxel_size)), C.c_int32(tel.n_channels),
+            C.c_float(float(tel.lambda0)), C.c_float(float(tel.dlambda)), C.c_int32(tel.psf_size),
+            C.c_double(float(tel.psf_sigma)), C.c_int32(tel.lsf_size),
+            C.c_double(float(tel.lsf_sigma)), _pd(grad_cube), *(_pd(o) for o in out))
     return tuple(out)
 
 
@@ -251,7 +275,7 @@ def knot_clearance(vlos, ssp, tel):
     particle.  The spectrum has a kink in v_los wherever some x_k crosses an SSP knot; the
     finite-difference sample keeps away from those (non-differentiable points)."""
     beta = np.asarray(vlos, np.float64)[:, None] / C_KMS
-    lam = np.float64(tel.lambda0) + np.float64(tel.dlambda) * np.arange(tel.n_channels)
+    lam = tel.wavelengths()
     x = (lam[None, :] / ((1.0 + beta) * (1.0 + float(getattr(tel, "redshift", 0.0)))) - np.float64(ssp.lambda0)) \
         / np.float64(ssp.dlambda)
     return np.abs(x - np.round(x)).min(axis=1)

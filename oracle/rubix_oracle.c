@@ -41,6 +41,22 @@
 #include <string.h>
 
 #define ORC_C_KMS 299792.458     /* speed of light, km/s (SURVEY.md 8 notation) */
+/* Observed wavelengths (reading R16): lambda_k = l0_obs + k dl_obs, or, while an explicit array is
+ * installed with orc_set_lambda_obs, lambda_k = lambda_obs[k] / (1 + z) (arbitrary, increasing telescope grid;
+ * point-sampled rule only).  The array is installed by the Python wrapper around one call and removed
+ * afterwards; the OpenMP threads only read it. */
+static const float *g_lambda_obs = 0;
+static double g_lambda_div = 1.0;
+void orc_set_lambda_obs(const float *lambda_obs, double one_plus_z)
+{
+    g_lambda_obs = lambda_obs;
+    g_lambda_div = one_plus_z;
+}
+static double observed_lambda(int32_t k, double l0_obs, double dl_obs)
+{
+    return g_lambda_obs ? (double)g_lambda_obs[k] / g_lambda_div : l0_obs + dl_obs * (double)k;
+}
+
 #define ORC_VCAP_KMS 14989.623f  /* 0.05 c: |v_los| above this (or NaN) => particle dropped
                                     (reading R5; physical stars never reach it) */
 
@@ -145,7 +161,7 @@ static void particle_spectrum(double mass, int32_t ia, int32_t iz, double ta, do
     const double lam_last = log_grid ? l0_ssp * pow(10.0, dl_ssp * (double)(n_lambda - 1))
                                      : l0_ssp + dl_ssp * (double)(n_lambda - 1);
     for (int32_t k = k_begin; k < k_end; ++k) {
-        const double lam_obs = l0_obs + dl_obs * (double)k;
+        const double lam_obs = observed_lambda(k, l0_obs, dl_obs);
         const double lam_rest = lam_obs / (1.0 + beta);
         if (lam_rest < lam_first || lam_rest > lam_last) {
             F[k] = 0.0;
@@ -577,7 +593,7 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                  * written as the same expression with lambda_k replaced by (1+beta) / ln 10 */
                 for (int32_t k = 0; k < n_c; ++k) {
                     const double lam_eff = ((mode >> 1) & 1) ? (1.0 + (double)vlos[p] / ORC_C_KMS) / log(10.0)
-                                                             : (double)l0_obs + (double)dl_obs * k;
+                                                             : observed_lambda(k, (double)l0_obs, (double)dl_obs);
                     E += g[k] * lam_eff * dS[k] / (double)dl_ssp;
                 }
             }

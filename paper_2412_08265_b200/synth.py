@@ -189,12 +189,15 @@ class Telescope:
     resample: int = 0         # 0 = point-sampled linear interpolation, 1 = flux-conserving bin average
     redshift: np.float32 = np.float32(0.0)     # cosmological redshift of the galaxy
     flux_scale: np.float32 = np.float32(1.0)   # multiplies every spectrum (distance dimming / units)
+    lambda_obs: np.ndarray | None = None       # explicit, increasing channel wavelengths [n_channels] fp32 (else uniform)
 
     @property
     def n_spaxels(self) -> int:
         return self.n_x * self.n_y
 
     def wavelengths(self) -> np.ndarray:
+        if self.lambda_obs is not None:
+            return np.asarray(self.lambda_obs, np.float32).astype(np.float64)
         return np.float64(self.lambda0) + np.float64(self.dlambda) * np.arange(self.n_channels)
 
     def with_psf_lsf(self, fwhm_spaxels=3.0, psf_size=15, lsf_sigma=2.0, lsf_size=9) -> "Telescope":
