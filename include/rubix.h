@@ -89,6 +89,10 @@ typedef struct {
                                     /* lambda_rest = lambda_obs / ((1 + z)(1 + beta))        */
     float flux_scale;               /* > 0: every spectrum is multiplied by it (distance     */
                                     /* dimming / unit conversion chosen by the caller); 1 = off */
+    const float *lambda_obs;        /* HOST [n_channels] or NULL.  Non-NULL: explicit channel   */
+                                    /* wavelengths (Angstrom, > 0, strictly increasing) replace  */
+                                    /* lambda0 + k dlambda; RUBIX_RESAMPLE_POINT only.  Read (and */
+                                    /* copied to the workspace) before the call returns.         */
 } rubix_telescope;
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the

@@ -50,7 +50,7 @@ class CTelescope(C.Structure):
                 ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
                 ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
-                ("redshift", C.c_float), ("flux_scale", C.c_float)]
+                ("redshift", C.c_float), ("flux_scale", C.c_float), ("lambda_obs", C.c_void_p)]
 
 
 _lib = None
@@ -140,11 +140,14 @@ class _Keep:
 
 
 def c_telescope(tel) -> _Keep:
+    lam = getattr(tel, "lambda_obs", None)
+    lam = None if lam is None else np.ascontiguousarray(lam, dtype=np.float32)
     return _Keep(CTelescope(int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
                             float(tel.lambda0), float(tel.dlambda), int(tel.psf_size),
                             float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma),
                             int(getattr(tel, "resample", 0)), float(getattr(tel, "redshift", 0.0)),
-                            float(getattr(tel, "flux_scale", 1.0))))
+                            float(getattr(tel, "flux_scale", 1.0)),
+                            None if lam is None else lam.ctypes.data), lam)
 
 
 def c_ssp(ssp, flux) -> _Keep:

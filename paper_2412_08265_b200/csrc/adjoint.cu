@@ -18,7 +18,8 @@ struct AdjParams {
     int32_t n_lambda, pitch, n_z, n_c, n_s;
     float l0_obs, dl_obs, dl_ssp;     // observed grid already divided by (1 + z)
     float flux_scale;
-    const int64_t *xtab;              // log-sampled SSP grid (R15): x_k = xtab[k] + a_fx
+    const int64_t *xtab;              // table mode (R15 / R16): x_k = xtab[k] c + a_fx, c = b_fx / 2^30
+    int32_t log_grid;
     double l0_over_dl;                // lambda0_obs / dlambda_obs (the (1+z) factors cancel)
     int64_t n;
 };
@@ -83,14 +84,22 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     const int64_t step = (int64_t)r.b_fx << 5;
     int64_t x = r.a_fx + (int64_t)r.b_fx * (r.k_lo + lane);
     const int64_t *xt = P.xtab + r.k_lo + lane;          // LOGX: x_k = xtab[k] + a_fx, and dx/dbeta is the same
-    const float lam_log = (1.0f + vlos[p] / (float)kCkms) * 0.4342944819f;   // for every channel: lambda_k -> (1+beta)/ln10
+    const float lam_log = (1.0f + vlos[p] / (float)kCkms) * 0.4342944819f;
+    const double c_tab = (double)r.b_fx * (1.0 / (double)(1u << 30));
     const float lam_step = 32.0f * P.dl_obs;
     float lam = fmaf(P.dl_obs, (float)(r.k_lo + lane), P.l0_obs);
     const float *T1 = T0 + (size_t)P.n_z * P.pitch, *T2 = T0 + P.pitch, *T3 = T1 + P.pitch;
     const float *gp = g + r.k_lo + lane;
     float s0, sa, sz, sq, se;
     auto channel = [&]() {
-        if (LOGX) { x = r.a_fx + __ldg(xt); lam = lam_log; xt += 32; }
+        if (LOGX) {                                         // table mode
+            const int64_t y = __ldg(xt);
+            x = r.a_fx + __double2ll_rn((double)y * c_tab);
+            // d x_k / d beta = -lambda_k / ((1+z)(1+beta)^2 dl_ssp) on a linear SSP grid (lambda_k/(1+z) = Y dl_ssp);
+            // on a log-sampled one it is the same for every channel: lambda_k -> (1+beta) / ln 10
+            lam = P.log_grid ? lam_log : (float)((double)y * (1.0 / (double)(1 << kFxFrac))) * P.dl_ssp;
+            xt += 32;
+        }
         int j = (int)(x >> kFxFrac);
         float f = __uint_as_float((((uint32_t)x >> 5) & 0x7FFFFFu) | 0x3F800000u) - 1.0f;
         if (j > jmax) { j = jmax; f = 1.0f; }
@@ -303,11 +312,12 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.flux_scale = in.tel->flux_scale;
     P.l0_over_dl = (double)in.tel->lambda0 / (double)in.tel->dlambda;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
+    P.log_grid = in.ssp->log_lambda;
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
     const int64_t threads = L.n * 32;
     auto kern = in.tel->resample == RUBIX_RESAMPLE_FLUX ? k_adjoint_flux
-                                                        : (in.ssp->log_lambda ? k_adjoint<true> : k_adjoint<false>);
+                                                        : (table_mode(in.ssp, in.tel) ? k_adjoint<true> : k_adjoint<false>);
     kern<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const int32_t *)(ws + L.off_permbuf[L.final_buf]), (const int32_t *)(ws + L.off_seg),
         (const int32_t *)(ws + L.off_key), (const float *)(ws + L.off_vlos), in.p->mass,

@@ -79,6 +79,13 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_INVALID_ARG, "redshift must be in [0, 20]");
     if (!(t->flux_scale > 0.0f) || !isfinite(t->flux_scale))
         return fail(RUBIX_ERR_INVALID_ARG, "flux_scale must be > 0 and finite (1 = no scaling)");
+    if (t->lambda_obs) {
+        if (t->resample != RUBIX_RESAMPLE_POINT)
+            return fail(RUBIX_ERR_UNSUPPORTED, "explicit channel wavelengths support RUBIX_RESAMPLE_POINT only");
+        for (int k = 0; k < t->n_channels; ++k)
+            if (!(t->lambda_obs[k] > 0.0f) || !isfinite(t->lambda_obs[k]) || (k > 0 && !(t->lambda_obs[k] > t->lambda_obs[k - 1])))
+                return fail(RUBIX_ERR_INVALID_ARG, "lambda_obs must be positive, finite and strictly increasing");
+    }
     const int sz[2] = {t->psf_size, t->lsf_size};
     const float sg[2] = {t->psf_sigma, t->lsf_sigma};
     for (int i = 0; i < 2; ++i) {
@@ -103,15 +110,14 @@ rubix_status check_particles(const rubix_particles *p)
 
 rubix_status check_resampler(const rubix_ssp *s, const rubix_telescope *t)
 {
-    if (s->log_lambda) {
+    if (table_mode(s, t)) {
         if (t->resample != RUBIX_RESAMPLE_POINT)
-            return fail(RUBIX_ERR_UNSUPPORTED, "log-sampled ssp grids support RUBIX_RESAMPLE_POINT only");
-        // steepest d x / d k is at the first channel: dlambda_obs / (lambda_obs ln10 dlog)
-        const double lam_min = (double)t->lambda0 < (double)t->lambda0 + (double)t->dlambda * (t->n_channels - 1)
-                                   ? (double)t->lambda0 : (double)t->lambda0 + (double)t->dlambda * (t->n_channels - 1);
-        if (!(lam_min > 0.0)) return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths must be > 0 for a log-sampled ssp grid");
-        const double b0 = (double)t->dlambda / (lam_min * 2.302585092994046 * (double)s->dlambda);
-        if (b0 >= 14.25)
+            return fail(RUBIX_ERR_UNSUPPORTED,
+                        "log-sampled ssp grids and explicit channel wavelengths support RUBIX_RESAMPLE_POINT only");
+        if (!t->lambda_obs && !((double)t->lambda0 > 0.0))
+            return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths must be > 0 for a log-sampled ssp grid");
+        const double b0 = table_step_max(s, t);
+        if (!(b0 < 14.25))
             return fail(RUBIX_ERR_UNSUPPORTED, "d x / d channel = %.3f is outside the resampler range (< 14.25)", b0);
         return RUBIX_OK;
     }

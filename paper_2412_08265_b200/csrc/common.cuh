@@ -65,7 +65,7 @@ struct Layout {
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,
-        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab;
+        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs;
     int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
                                       // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
@@ -93,6 +93,12 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
 size_t loss_scratch_bytes();
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
                                  double *partial, double *loss, cudaStream_t st);
+
+// Table mode (readings R15 / R16): the rest position of channel k is x_k = Y[k] c + a with a per-launch
+// table Y and per-particle (c, a); used for log-sampled SSP grids and for explicit channel wavelengths.
+inline bool table_mode(const rubix_ssp *s, const rubix_telescope *t) { return s->log_lambda != 0 || t->lambda_obs != nullptr; }
+// largest d x / d channel over the detector, including the largest Doppler stretch (host, fp64)
+double table_step_max(const rubix_ssp *s, const rubix_telescope *t);
 
 void make_taps(int size, float sigma, Taps *t);
 

@@ -314,7 +314,7 @@ struct PrepParams {
     int32_t n_lambda, pitch, n_c, n_s, mode;
     float l0_ssp, dl_ssp, l0_obs, dl_obs;
     float redshift, flux_scale;         // DESIGN.md reading R14
-    int32_t log_grid;                   // reading R15: x_k = xtab[k] - log10(1+beta)/dlog
+    int32_t log_grid, table;            // table mode (R15 / R16): x_k = xtab[k] c + a
     const int64_t *xtab;
 };
 
@@ -361,18 +361,24 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     const int64_t b = (int64_t)b_fx;
     const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
     int64_t k_lo, k_hi, x_first, x_last;
-    if (P.log_grid) {
-        // x_k = xtab[k] + a_fx with a_fx = -log10(1 + beta) / dlog: the Doppler shift is a constant offset
-        // on a log-sampled grid; xtab is increasing, so the covered channels are found by bisection
-        a_fx = -__double2ll_rn(log10(1.0 + (double)vlos[p] / kCkms) / (double)P.dl_ssp * scale);
-        int lo = 0, hi = P.n_c;                            // first k with xtab[k] + a_fx >= 0
-        while (lo < hi) { const int mid = (lo + hi) >> 1; if (P.xtab[mid] + a_fx >= 0) hi = mid; else lo = mid + 1; }
+    uint32_t c_fx = 0;
+    if (P.table) {
+        // x_k = llrint(Y[k] c) + a_fx, c quantised to 2.30 fixed point so that every kernel uses the same value;
+        // Y is increasing, so the covered channels are found by bisection
+        const double opb = 1.0 + (double)vlos[p] / kCkms;
+        c_fx = P.log_grid ? (1u << 30) : (uint32_t)__double2ll_rn((double)(1u << 30) / opb);
+        const double c = (double)c_fx * (1.0 / (double)(1u << 30));
+        a_fx = P.log_grid ? -__double2ll_rn(log10(opb) / (double)P.dl_ssp * scale)
+                          : -__double2ll_rn((double)P.l0_ssp / (double)P.dl_ssp * scale);
+        auto xk = [&](int k) { return __double2ll_rn((double)P.xtab[k] * c) + a_fx; };
+        int lo = 0, hi = P.n_c;                            // first k with x_k >= 0
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (xk(mid) >= 0) hi = mid; else lo = mid + 1; }
         k_lo = lo;
-        lo = -1; hi = P.n_c - 1;                           // last k with xtab[k] + a_fx <= x_max
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (P.xtab[mid] + a_fx <= x_max) lo = mid; else hi = mid - 1; }
+        lo = -1; hi = P.n_c - 1;                           // last k with x_k <= x_max
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (xk(mid) <= x_max) lo = mid; else hi = mid - 1; }
         k_hi = lo;
-        x_first = k_lo <= k_hi ? P.xtab[k_lo] + a_fx : 0;
-        x_last = k_lo <= k_hi ? P.xtab[k_hi] + a_fx : 0;
+        x_first = k_lo <= k_hi ? xk((int)k_lo) : 0;
+        x_last = k_lo <= k_hi ? xk((int)k_hi) : 0;
     } else if (P.mode == RUBIX_RESAMPLE_FLUX) {
         // x_k = a_fx + b k is the LOWER EDGE of bin k (upper edge = lower edge of bin k + 1);
         // [k_lo, k_hi] = bins that overlap the coverage [0, N_l - 1]
@@ -396,7 +402,7 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
         x_last = a_fx + b * k_hi;
     }
     r.a_fx = a_fx;
-    r.b_fx = b_fx;
+    r.b_fx = P.table ? c_fx : b_fx;            // table mode: the Doppler factor c (2.30) takes B's slot
     r.k_lo = (int32_t)k_lo;
     r.k_hi = (int32_t)k_hi;
     r.j0 = 0;
@@ -409,15 +415,37 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
 }
 
 // --------------------------------------------------------------------------------------------
-// Log-sampled SSP grid (reading R15): rest position of channel k at beta = 0, in SSP samples,
-//   X0[k] = log10(lambda_k / ((1 + z) lambda0_ssp)) / dlog          (fp64 -> 36.28 fixed point)
+// Table mode (readings R15 / R16): x_k = Y[k] c + a with (c, a) per particle and
+//   log-sampled SSP grid:   Y[k] = log10(lambda_k / ((1+z) lambda0_ssp)) / dlog,   c = 1,  a = -log10(1+beta)/dlog
+//   linear SSP grid:        Y[k] = lambda_k / ((1+z) dlambda_ssp),                 c = 1/(1+beta),  a = -lambda0_ssp/dlambda_ssp
+// lambda_k = lam[k] (explicit channel wavelengths) or l0_obs + k dl_obs.  fp64 -> 36.28 fixed point.
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_log_positions(int32_t n_c, double l0_obs, double dl_obs, double l0_ssp, double dlog, int64_t *__restrict__ xtab)
+k_positions(int32_t n_c, const float *__restrict__ lam, double l0_obs, double dl_obs, double zp1, int32_t log_grid,
+            double l0_ssp, double dl_ssp, int64_t *__restrict__ ytab)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > n_c) return;
-    xtab[k] = __double2ll_rn(log10((l0_obs + dl_obs * (double)k) / l0_ssp) / dlog * (double)(1 << kFxFrac));
+    const double l = (lam ? (double)lam[min(k, n_c - 1)] : l0_obs + dl_obs * (double)k) / zp1;
+    const double y = log_grid ? log10(l / l0_ssp) / dl_ssp : l / dl_ssp;
+    ytab[k] = __double2ll_rn(y * (double)(1 << kFxFrac));
+}
+
+double table_step_max(const rubix_ssp *s, const rubix_telescope *t)
+{
+    const double zp1 = 1.0 + (double)t->redshift;
+    auto y = [&](int k) {
+        const double l = (t->lambda_obs ? (double)t->lambda_obs[k] : (double)t->lambda0 + (double)t->dlambda * k) / zp1;
+        return s->log_lambda ? log10(l / (double)s->lambda0) / (double)s->dlambda : l / (double)s->dlambda;
+    };
+    double m = 0.0;
+    if (t->n_channels < 2) return 0.0;
+    if (!t->lambda_obs) {                                  // uniform grid: steepest at one of the two ends
+        m = fmax(y(1) - y(0), y(t->n_channels - 1) - y(t->n_channels - 2));
+    } else {
+        for (int k = 1; k < t->n_channels; ++k) m = fmax(m, y(k) - y(k - 1));
+    }
+    return s->log_lambda ? m : m / (1.0 - kBetaCap);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -497,7 +525,8 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.pitch = (n_lambda + kRowAlign - 1) / kRowAlign * kRowAlign;
     off = align_up(off, 512);                            // (texture-alignment safe)
     L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
-    L.off_xtab = take(((size_t)n_c + 1) * 8);           // X0[k] of a log-sampled SSP grid (reading R15)
+    L.off_xtab = take(((size_t)n_c + 1) * 8);           // Y[k] of the table mode (readings R15 / R16)
+    L.off_lamobs = take(((size_t)n_c + 1) * 4);         // device copy of rubix_telescope.lambda_obs
     L.bytes_total = off;
     return L;
 }
@@ -588,12 +617,19 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.n_s = n_s;
         P.mode = in.tel->resample;
         P.log_grid = in.ssp->log_lambda;
+        P.table = table_mode(in.ssp, in.tel) ? 1 : 0;
         P.xtab = (const int64_t *)(ws + L.off_xtab);
-        if (P.log_grid) {
-            const double zp1 = 1.0 + (double)in.tel->redshift;
-            k_log_positions<<<(unsigned)((L.n_c + 256) / 256), 256, 0, st>>>(
-                L.n_c, (double)in.tel->lambda0 / zp1, (double)in.tel->dlambda / zp1, (double)in.ssp->lambda0,
-                (double)in.ssp->dlambda, (int64_t *)(ws + L.off_xtab));
+        if (P.table) {
+            const float *lam_dev = nullptr;
+            if (in.tel->lambda_obs) {                      // host array -> workspace (read before this call returns)
+                lam_dev = (const float *)(ws + L.off_lamobs);
+                cudaError_t ec = cudaMemcpyAsync(ws + L.off_lamobs, in.tel->lambda_obs, (size_t)L.n_c * 4,
+                                                 cudaMemcpyHostToDevice, st);
+                if (ec != cudaSuccess) return ec;
+            }
+            k_positions<<<(unsigned)((L.n_c + 256) / 256), 256, 0, st>>>(
+                L.n_c, lam_dev, (double)in.tel->lambda0, (double)in.tel->dlambda, 1.0 + (double)in.tel->redshift,
+                P.log_grid, (double)in.ssp->lambda0, (double)in.ssp->dlambda, (int64_t *)(ws + L.off_xtab));
             RUBIX_LAUNCH_CHECK();
         }
         P.redshift = in.tel->redshift;

@@ -97,8 +97,9 @@ struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 // FLUX: flux-conserving resampling (RUBIX_RESAMPLE_FLUX): x_k is the lower edge of bin k and the
 // channel value is the exact integral of the table's piecewise-linear interpolant over
 // [x_k, x_{k+1}] (clipped to the SSP coverage), divided by the bin width B.
-// LOGX: log-sampled SSP grid (reading R15): x_k = xtab[k] + a (a = the particle's Doppler offset); the
-// thread keeps the positions of its CPT channels relative to the tile start in registers (12.20).
+// LOGX: table mode (readings R15 / R16: log-sampled SSP grid, explicit channel wavelengths):
+// x_k = Y[k] c + a with the per-launch table Y = xtab and the particle's (c, a); c (2.30 fixed point) travels in
+// the record's b slot.  The thread keeps Y of its CPT channels relative to the tile start in registers (12.20).
 template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX>
 __global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
@@ -155,7 +156,11 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 j0 = 0; W.nw = 0;
                 if (W.ka <= W.kb) {
                     int64_t xa = a + (int64_t)W.b * W.ka, xb = a + (int64_t)W.b * (W.kb + (FLUX ? 1 : 0));
-                    if (LOGX) { xa = a + P.xtab[W.ka]; xb = a + P.xtab[W.kb]; }
+                    if (LOGX) {
+                        const double c = (double)W.b * (1.0 / (double)(1u << 30));
+                        xa = a + __double2ll_rn((double)P.xtab[W.ka] * c);
+                        xb = a + __double2ll_rn((double)P.xtab[W.kb] * c);
+                    }
                     if (FLUX) {                             // bins are clipped to the coverage
                         xa = max(xa, (int64_t)0);
                         xb = min(xb, (int64_t)(P.n_lambda - 1) << kFxFrac);
@@ -166,7 +171,8 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
             W.first = rb.x + j0;
             W.j0 = j0;
-            W.base = a + (LOGX ? x_tile0 : (int64_t)W.b * k0) - ((int64_t)j0 << kFxFrac);
+            W.base = a + (LOGX ? __double2ll_rn((double)x_tile0 * ((double)W.b * (1.0 / (double)(1u << 30))))
+                               : (int64_t)W.b * k0) - ((int64_t)j0 << kFxFrac);
             return W;
         };
 
@@ -295,16 +301,16 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 return;
             }
             // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
-            // LOGX: x = (tile-relative position of the channel) + (particle base), both truncated to 2^-20
+            // LOGX: x = (tile-relative table value of the channel) x c + (particle base), truncated to 2^-20
             const uint32_t x0 = LOGX ? (uint32_t)(W.base >> 8) : (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
 #pragma unroll
-                for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + xl[i] : x0 + (uint32_t)i * W.b, bytes);
+                for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * W.b, bytes);
             } else {
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + xl[i] : x0 + (uint32_t)i * W.b, bytes);
+                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * W.b, bytes);
                 }
             }
         };
@@ -423,12 +429,10 @@ int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, cudaStream_t st)
 {
-    const bool logx = in.ssp->log_lambda != 0;
+    const bool logx = table_mode(in.ssp, in.tel);
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
-    // log-sampled grid: d x / d k = dlambda_obs / (lambda_k ln10 dlog), steepest at the first channel; a Doppler
-    // shift moves the window but does not stretch it
-    const double b_max = logx ? (double)in.tel->dlambda / ((double)in.tel->lambda0 * 2.302585092994046 * (double)in.ssp->dlambda)
-                              : b0 / (1.0 - kBetaCap);
+    // table mode: the steepest d x / d k of the detector, largest Doppler stretch included
+    const double b_max = logx ? table_step_max(in.ssp, in.tel) : b0 / (1.0 - kBetaCap);
     int wcap = 0;
     const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
     const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap);
