@@ -29,7 +29,10 @@
  * scipy.ndimage.convolve1d, numpy.convolve, flux conservation (PSF/LSF); central finite
  * differences, the dot-product test and the linear-template closed form (adjoint);
  * the prefix-integral formulation, constant / linear templates, the (1,6,1)/8 identity and
- * exact total-flux telescoping (flux-conserving resampling, tests/test_oracle_fluxcons.py).
+ * exact total-flux telescoping (flux-conserving resampling, tests/test_oracle_fluxcons.py);
+ * numpy.interp at the doubly shifted wavelength, in log lambda, and at listed channel wavelengths
+ * (redshift, log-sampled grids, explicit observed grids: tests/test_oracle_redshift.py,
+ * test_oracle_loggrid.py, test_oracle_obsgrid.py), each with finite-difference and closed-form adjoint pins.
  * No function here is "parity unpinned".
  *
  * No blocking, fusion or reordering beyond the definitions; the only parallelism is an

@@ -42,6 +42,11 @@ def random_case(seed):
                           np.float32(l0 * (1 + z)), np.float32(dl * (1 + z)), psf, np.float32(rng.uniform(0.6, 3.0)),
                           lsf, np.float32(rng.uniform(0.6, 3.0)), resample, np.float32(z),
                           np.float32(rng.choice([1.0, 3.0e-3, 40.0])))
+    if resample == 0 and rng.integers(0, 3) == 0 and n_c >= 1:      # explicit, irregular channel wavelengths (R16)
+        steps = rng.uniform(0.4, 1.6, n_c)
+        lam = (float(tel.lambda0) + float(tel.dlambda) * (np.cumsum(steps) - steps[0])).astype(np.float32)
+        if np.all(np.diff(lam) > 0):
+            tel = dataclasses.replace(tel, lambda_obs=lam)
     n = int(rng.choice([0, 1, 7, 300, 2500]))
     w = synth.make_workload("tiny", n=max(n, 1), seed=int(rng.integers(1, 10 ** 6)))
     if n == 0:
@@ -52,12 +57,12 @@ def random_case(seed):
     return w
 
 
-@pytest.mark.parametrize("seed", range(40))
+@pytest.mark.parametrize("seed", range(60))
 def test_random_configuration(B, seed):
     w = random_case(1234 + seed)
     t = w.telescope
     what = f"seed {seed}: n={w.particles.n} {t.n_x}x{t.n_y}x{t.n_channels} psf={t.psf_size} lsf={t.lsf_size} " \
-           f"resample={t.resample} log={w.ssp.log_lambda} z={float(t.redshift)}"
+           f"resample={t.resample} log={w.ssp.log_lambda} z={float(t.redshift)} listed={t.lambda_obs is not None}"
     dw = B.DeviceWorkload(w)
     cube = dw.build_cube(out=torch.full(dw.shape, float("nan"), device="cuda"))
     final = dw.convolve(cube)
