@@ -19,7 +19,7 @@ constexpr int kFxFrac = 28;                 // fractional bits of the rest-posit
 constexpr int kChunk = 128;                 // particles per work unit of the accumulate kernel
 constexpr int kMaxAge = 512, kMaxZ = 128;   // SSP axes travel as kernel parameters
 constexpr int kMaxTaps = 63;
-constexpr int kAccThreads = 256;            // threads per CTA of the accumulate kernel
+constexpr int kAccThreads = 128;            // threads per CTA of the accumulate kernel (the 12.20 stride trick needs 128)
 constexpr int kTabMax = 4096;               // table entries addressable by the 12.20 local format
 constexpr int kSortWarps = 8;               // warps per CTA in the radix passes
 constexpr int kSortItems = 1024;            // keys per warp per radix pass

@@ -357,7 +357,9 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
     const double B = (double)P.dl_obs * inv / (double)P.dl_ssp;
     int64_t a_fx = __double2ll_rn(A * scale);
-    const uint32_t b_fx = (uint32_t)__double2ll_rn(B * scale);
+    // B is rounded to an EVEN number of 2^-28 units: the accumulate kernel strides by kAccThreads = 128 channels,
+    // i.e. by b / 2 in its 2^-20 local format, and that must stay exact
+    const uint32_t b_fx = (uint32_t)(2 * __double2ll_rn(B * scale * 0.5));
     const int64_t b = (int64_t)b_fx;
     const int64_t x_max = (int64_t)(P.n_lambda - 1) << kFxFrac;
     int64_t k_lo, k_hi, x_first, x_last;

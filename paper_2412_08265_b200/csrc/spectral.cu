@@ -2,8 +2,11 @@
 // ("The key part is the spectra calculation").
 //
 // Work unit = up to kChunk consecutive sorted particles of ONE spaxel x one channel tile.  One
-// CTA (256 threads) per unit; thread t owns channels k0 + t + 256 i (i < CPT) and keeps their sums
-// in registers, so a spaxel's spectrum is reduced without any atomic.  Per particle:
+// CTA (128 threads, five resident per SM) per unit; thread t owns channels k0 + t + 128 i (i < CPT, CPT = 29
+// for 3700 channels) and keeps their sums in registers, so a spaxel's spectrum is reduced without any atomic.
+// Small CTAs de-synchronise the load-heavy blend phases and the shared-memory-heavy resample phases of the
+// CTAs sharing an SM, which keeps the L1 data pipe busier (r01: 3.51 -> 3.28 ms against 256-thread CTAs).
+// Per particle:
 //   blend    the four corner templates are read once over the particle's rest-wavelength window
 //            and blended with the mass-scaled bilinear weights into a shared-memory table S_j.
 //            The window starts on a multiple of 32 samples of the padded workspace copy of the grid
@@ -47,7 +50,7 @@ constexpr int kAccWarps = kAccThreads / 32;
 #define RUBIX_ACC_DEPTH 1
 #endif
 #ifndef RUBIX_ACC_MINB
-#define RUBIX_ACC_MINB 3
+#define RUBIX_ACC_MINB 5
 #endif
 constexpr int kAccDepth = RUBIX_ACC_DEPTH;           // load sets (passes) in flight per warp
 constexpr int kAccMinBlocks = RUBIX_ACC_MINB;
@@ -260,7 +263,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                                       W.base + (int64_t)W.b * (k_end - k0 + 1) <= cov_hi;
                 if (interior) {
                     // both edges are truncated by the same function of k, so neighbouring bins share
-                    // their edge exactly (stride 256 b / 256 = b keeps the truncation exact)
+                    // their edge exactly (stride 128 b / 256 = b / 2 with even b keeps the truncation exact)
                     const uint32_t xl0 = (uint32_t)(e0 >> 8), xh0 = (uint32_t)((e0 + (int64_t)W.b) >> 8);
                     if (W.b <= (1u << kFxFrac)) {
                         // bins no wider than one SSP sample touch at most two knot intervals: branch-free
@@ -269,7 +272,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                         const float width = (float)(xh0 - xl0) * (1.0f / 1048576.0f);
 #pragma unroll
                         for (int i = 0; i < CPT; ++i) {
-                            const uint32_t x = xl0 + (uint32_t)i * W.b;
+                            const uint32_t x = xl0 + (uint32_t)i * (W.b >> 1);
                             const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
                             const float a0 = e[0], a1 = e[1], a2r = e[2];
                             const float fl = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;
@@ -285,7 +288,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                     } else {
 #pragma unroll
                         for (int i = 0; i < CPT; ++i)
-                            flux_sample(i, xl0 + (uint32_t)i * W.b, xh0 + (uint32_t)i * W.b, inv_b, buf);
+                            flux_sample(i, xl0 + (uint32_t)i * (W.b >> 1), xh0 + (uint32_t)i * (W.b >> 1), inv_b, buf);
                     }
                 } else {
 #pragma unroll
@@ -300,17 +303,17 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 }
                 return;
             }
-            // 12.20 local fixed point: exact truncation of the 36.28 value (stride 256 b / 256 = b)
+            // 12.20 local fixed point: exact truncation of the 36.28 value (channel stride 128 b / 256 = b / 2, b is even)
             // LOGX: x = (tile-relative table value of the channel) x c + (particle base), truncated to 2^-20
             const uint32_t x0 = LOGX ? (uint32_t)(W.base >> 8) : (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
 #pragma unroll
-                for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * W.b, bytes);
+                for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * (W.b >> 1), bytes);
             } else {
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * W.b, bytes);
+                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * (W.b >> 1), bytes);
                 }
             }
         };
@@ -386,7 +389,7 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
 template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false>
 static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, LOGX ? 2 : kAccMinBlocks, FLUX, LOGX>;
+    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, LOGX ? 3 : kAccMinBlocks, FLUX, LOGX>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kAccThreads, smem, st>>>(P);
@@ -409,8 +412,8 @@ static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsign
 // (samples, a whole number of passes).
 int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 {
-    const int cand[5] = {15, 8, 4, 2, 1};
-    for (int c = 0; c < 5; ++c) {
+    const int cand[6] = {29, 15, 8, 4, 2, 1};
+    for (int c = 0; c < 6; ++c) {
         const int cpt = cand[c];
         const int tc = cpt * kAccThreads;
         const int tiles = (n_c + tc - 1) / tc;
@@ -479,6 +482,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     {
         StageTimer t(1, st);
         switch (cpt) {
+            case 29: e = launch_acc<29>(P, flux, logx, grid, smem, st); break;
             case 15: e = launch_acc<15>(P, flux, logx, grid, smem, st); break;
             case 8: e = launch_acc<8>(P, flux, logx, grid, smem, st); break;
             case 4: e = launch_acc<4>(P, flux, logx, grid, smem, st); break;
