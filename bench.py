@@ -388,6 +388,28 @@ def run_ours(args):
                     "l2_frac": gather_b / (flux_acc_ms * 1e-3) / 1e9 / onchip["l2_gbs"]}
     del dwf, cube_f, final_f
 
+    # ---- SURVEY.md 8(f)-1 variant: log-sampled SSP grid of the same size (reading R15, table mode)
+    table_variant = None
+    if args.workload in ("small", "medium", "contention"):
+        na, nz, nl = w.ssp.flux.shape
+        wl = dataclasses.replace(w, ssp=synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, log_lambda=True))
+        dwl = B.DeviceWorkload(wl, device=dev)
+        cube_l = torch.empty(dw.shape, dtype=torch.float32, device=dev)
+        for _ in range(3):
+            dwl.build_cube(out=cube_l)
+        torch.cuda.synchronize()
+        B.rubix_stage_timing_enable(True)
+        B.rubix_stage_timing_read()
+        for _ in range(10):
+            dwl.build_cube(out=cube_l)
+        torch.cuda.synchronize()
+        st_l = B.rubix_stage_timing_read()
+        B.rubix_stage_timing_enable(False)
+        table_variant = {"what": "rubix_build_cube on a log-sampled SSP grid of the same size (table mode, reading R15)",
+                         "k_accumulate_ms": st_l["accumulate"]["ms"] / max(st_l["accumulate"]["calls"], 1),
+                         "particle_pass_ms": st_l["particle_pass"]["ms"] / max(st_l["particle_pass"]["calls"], 1)}
+        del dwl, cube_l
+
     adjoint_info = None
     if not args.no_adjoint:
         del scratch
@@ -402,6 +424,8 @@ def run_ours(args):
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
             "stage_ms": stage_ms, "roofline": roofline}
     line["flux_variant"] = flux_variant
+    if table_variant is not None:
+        line["log_grid_variant"] = table_variant
     if adjoint_info is not None:
         line["adjoint"] = adjoint_info
 
