@@ -333,3 +333,26 @@ def fd_gradients(particles, R, ssp, tel, residual, idx, h_mass=1e-3, h_log=1e-4,
                 dl.append(delta_loss(spec - base, sx, sy))
             out[q, n_i] = (dl[0] - dl[1]) / (2.0 * h)
     return out[0], out[1], out[2], out[3]
+
+
+# ----------------------------------------------------------------------------- noise stage (reading R17)
+def philox4x32_10(counter, key):
+    c = (C.c_uint32 * 4)(*[int(v) for v in counter])
+    k = (C.c_uint32 * 2)(*[int(v) for v in key])
+    out = (C.c_uint32 * 4)()
+    _load().orc_philox4x32_10(c, k, out)
+    return [int(v) for v in out]
+
+
+def noise_normals(n, seed):
+    z = np.empty(int(n), np.float64)
+    _load().orc_noise_normals(C.c_int64(int(n)), C.c_uint64(int(seed)), _pd(z))
+    return z
+
+
+def add_noise(cube, sigma_read, gain, seed):
+    cube = np.ascontiguousarray(cube, dtype=np.float64)
+    out = np.empty_like(cube)
+    _load().orc_add_noise(_pd(cube), C.c_int64(cube.size), C.c_double(float(sigma_read)), C.c_double(float(gain)),
+                          C.c_uint64(int(seed)), _pd(out))
+    return out

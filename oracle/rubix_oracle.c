@@ -638,3 +638,64 @@ void orc_adjoint(int64_t n, const float *pos, const float *vel, const float *mas
                      l0_ssp, dl_ssp, flux, n_x, n_y, spaxel, n_c, l0_obs, dl_obs, psf_size, psf_sigma,
                      lsf_size, lsf_sigma, grad_cube, g_mass, g_log_age, g_log_z, g_vlos);
 }
+
+/* ------------------------------------------------------------------------------------
+ * Noise stage ("add realistic noise"; reading R17 -- the paper
+ * names no model).  cube_noisy[v] = cube[v] + sigma_v n_v,
+ *   sigma_v = sqrt(sigma_read^2 + gain * max(cube[v], 0))      (read noise + shot noise, flux units)
+ *   n_v ~ N(0, 1), independent, from a COUNTER-BASED generator so that both implementations draw the
+ *   same numbers: Philox4x32-10 (Salmon et al. 2011) with key = (seed low, seed high) and counter
+ *   (q low, q high, 0, 0), q = v / 4, gives four 32-bit words r0..r3 for voxels 4q .. 4q+3;
+ *   u_i = ((r_i >> 9) + 0.5) 2^-23 in (0, 1)  (exact in fp32);  Box-Muller:
+ *   n_{4q} = R0 cos(2 pi u1), n_{4q+1} = R0 sin(2 pi u1), R0 = sqrt(-2 ln u0); voxels 4q+2, 4q+3 from (u2, u3).
+ * ------------------------------------------------------------------------------------ */
+static uint32_t mulhilo32(uint32_t a, uint32_t b, uint32_t *hi)
+{
+    const uint64_t p = (uint64_t)a * (uint64_t)b;
+    *hi = (uint32_t)(p >> 32);
+    return (uint32_t)p;
+}
+
+void orc_philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+    uint32_t k0 = key_in[0], k1 = key_in[1];
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0, hi1;
+        const uint32_t lo0 = mulhilo32(0xD2511F53u, c0, &hi0);
+        const uint32_t lo1 = mulhilo32(0xCD9E8D57u, c2, &hi1);
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;                              /* Weyl sequence of the key schedule */
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void orc_noise_normals(int64_t n, uint64_t seed, double *normals)
+{   /* the standard normal deviates n_v alone (pinned on their own) */
+    const double two_pi = 6.283185307179586476925286766559;
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    for (int64_t q = 0; 4 * q < n; ++q) {
+        const uint32_t ctr[4] = {(uint32_t)(uint64_t)q, (uint32_t)((uint64_t)q >> 32), 0u, 0u};
+        uint32_t r[4];
+        orc_philox4x32_10(ctr, key, r);
+        double u[4], z[4];
+        for (int i = 0; i < 4; ++i) u[i] = ((double)(r[i] >> 9) + 0.5) * (1.0 / 8388608.0);
+        const double R0 = sqrt(-2.0 * log(u[0])), R1 = sqrt(-2.0 * log(u[2]));
+        z[0] = R0 * cos(two_pi * u[1]); z[1] = R0 * sin(two_pi * u[1]);
+        z[2] = R1 * cos(two_pi * u[3]); z[3] = R1 * sin(two_pi * u[3]);
+        for (int i = 0; i < 4 && 4 * q + i < n; ++i) normals[4 * q + i] = z[i];
+    }
+}
+
+void orc_add_noise(const double *cube, int64_t n, double sigma_read, double gain, uint64_t seed, double *out)
+{
+    double *z = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    orc_noise_normals(n, seed, z);
+    for (int64_t v = 0; v < n; ++v) {
+        const double f = cube[v] > 0.0 ? cube[v] : 0.0;
+        out[v] = cube[v] + sqrt(sigma_read * sigma_read + gain * f) * z[v];
+    }
+    free(z);
+}
