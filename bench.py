@@ -410,6 +410,26 @@ def run_ours(args):
                          "particle_pass_ms": st_l["particle_pass"]["ms"] / max(st_l["particle_pass"]["calls"], 1)}
         del dwl, cube_l
 
+    # ---- noise stage (reading R17): elementwise, read + write of the cube
+    noise_info = None
+    if has_conv:
+        nz_in = torch.empty(dw.shape, dtype=torch.float32, device=dev).uniform_(0.0, 10.0)
+        nz_out = torch.empty_like(nz_in)
+        for _ in range(3):
+            B.rubix_add_noise(nz_in, nz_out, 1.0, 0.1, 12345)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(10):
+            B.rubix_add_noise(nz_in, nz_out, 1.0, 0.1, 12345)
+        e1.record()
+        torch.cuda.synchronize()
+        nz_ms = e0.elapsed_time(e1) / 10
+        nz_b = 8.0 * nz_in.numel()
+        noise_info = {"what": "rubix_add_noise on a cube of the workload's size (Philox4x32-10 + Box-Muller, read + write)",
+                      "ms": nz_ms, "bound": "hbm", "achieved": nz_b / (nz_ms * 1e-3) / 1e9, "peak": hbm_peak,
+                      "unit": "GB/s", "frac": nz_b / (nz_ms * 1e-3) / 1e9 / hbm_peak}
+        del nz_in, nz_out
+
     adjoint_info = None
     if not args.no_adjoint:
         del scratch
@@ -426,6 +446,8 @@ def run_ours(args):
     line["flux_variant"] = flux_variant
     if table_variant is not None:
         line["log_grid_variant"] = table_variant
+    if noise_info is not None:
+        line["noise_stage"] = noise_info
     if adjoint_info is not None:
         line["adjoint"] = adjoint_info
 

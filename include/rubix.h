@@ -169,6 +169,16 @@ rubix_status rubix_loss_and_grad(const rubix_particles *particles, const rubix_s
                                  float *g_log_z, float *g_vlos, void *workspace, size_t workspace_bytes,
                                  void *stream);
 
+/* Noise stage ("add realistic noise"; the paper names no model -- DESIGN.md reading R17):
+ *     cube_out[v] = cube_in[v] + sqrt(sigma_read^2 + gain * max(cube_in[v], 0)) * n_v ,   n_v ~ N(0, 1)
+ * (read noise plus shot noise, in the cube's flux units).  The deviates come from the counter-based
+ * Philox4x32-10 generator keyed by `seed` with counter v / 4 and a Box-Muller map, so they depend only on
+ * (seed, v): reproducible, independent of the launch configuration.
+ *   cube_in, cube_out  DEVICE [n_voxels] fp32; cube_in == cube_out (in place) is allowed, partial overlap is not.
+ * The noise is not differentiated: rubix_cube_adjoint / rubix_loss_and_grad act on the noise-free cube. */
+rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_voxels, float sigma_read, float gain,
+                             uint64_t seed, void *stream);
+
 /* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_cube_adjoint on
  * this workspace address (compared bit for bit with the oracle):
  *   key     [n]      spaxel key of each particle in original order (n_s = dropped)

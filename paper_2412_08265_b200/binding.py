@@ -20,7 +20,7 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error",
-           "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad",
+           "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
 N_STAGES = 5
@@ -85,6 +85,8 @@ def load():
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                             C.c_void_p]
+        lib.rubix_add_noise.restype = C.c_int
+        lib.rubix_add_noise.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float, C.c_uint64, C.c_void_p]
         lib.rubix_get_sort_artifacts.restype = C.c_int
         lib.rubix_get_sort_artifacts.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                                  C.POINTER(C.c_void_p)]
@@ -217,6 +219,11 @@ def rubix_loss_and_grad(particles: _Keep, ssp: _Keep, tel: _Keep, R, target, los
                                       _ptr(loss), _ptr(cube_out), _ptr(g_mass), _ptr(g_log_age),
                                       _ptr(g_log_z), _ptr(g_vlos), _ptr(workspace),
                                       int(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
+def rubix_add_noise(cube_in, cube_out, sigma_read, gain, seed, stream=None):
+    _check(load().rubix_add_noise(_ptr(cube_in), _ptr(cube_out), int(cube_in.numel()), float(sigma_read), float(gain),
+                                  int(seed) & 0xFFFFFFFFFFFFFFFF, _stream(stream)))
 
 
 def rubix_get_sort_artifacts(workspace, n, n_s):

@@ -344,6 +344,25 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
     return RUBIX_OK;
 }
 
+rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_voxels, float sigma_read, float gain,
+                             uint64_t seed, void *stream)
+{
+    t_err[0] = 0;
+    g_launches = 0;
+    if (n_voxels < 0) return fail(RUBIX_ERR_INVALID_ARG, "n_voxels must be >= 0");
+    if (n_voxels > 0 && (!cube_in || !cube_out)) return fail(RUBIX_ERR_NULL, "cube_in or cube_out is NULL");
+    if (!(sigma_read >= 0.0f) || !isfinite(sigma_read) || !(gain >= 0.0f) || !isfinite(gain))
+        return fail(RUBIX_ERR_INVALID_ARG, "sigma_read and gain must be >= 0 and finite");
+    if (cube_in != cube_out) {
+        const char *a = (const char *)cube_in, *b = (const char *)cube_out;
+        if (a < b + (size_t)n_voxels * 4 && b < a + (size_t)n_voxels * 4)
+            return fail(RUBIX_ERR_INVALID_ARG, "cube_in and cube_out overlap (in place needs cube_in == cube_out)");
+    }
+    cudaError_t e = launch_add_noise(cube_in, cube_out, n_voxels, sigma_read, gain, seed, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "noise");
+    return RUBIX_OK;
+}
+
 rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key, const int32_t **perm,
                                       const int32_t **seg_off)
 {

@@ -90,6 +90,8 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st);
 
+cudaError_t launch_add_noise(const float *in, float *out, int64_t n, float sigma_read, float gain, uint64_t seed,
+                             cudaStream_t st);
 size_t loss_scratch_bytes();
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
                                  double *partial, double *loss, cudaStream_t st);

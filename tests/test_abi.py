@@ -158,6 +158,15 @@ def test_loss_and_grad_validation(lib):
     assert f(*args(ws_bytes=plain)) == B.RUBIX_ERR_WORKSPACE            # one cube-sized buffer short
 
 
+def test_add_noise_validation(lib):
+    f = lib.rubix_add_noise
+    assert f(None, FAKE, 16, 1.0, 0.0, 1, None) == B.RUBIX_ERR_NULL
+    assert f(FAKE, FAKE, -1, 1.0, 0.0, 1, None) == B.RUBIX_ERR_INVALID_ARG
+    assert f(FAKE, FAKE, 16, -1.0, 0.0, 1, None) == B.RUBIX_ERR_INVALID_ARG
+    assert f(FAKE, FAKE + 16, 16, 1.0, 0.0, 1, None) == B.RUBIX_ERR_INVALID_ARG      # partial overlap
+    assert f(None, None, 0, 1.0, 0.0, 1, None) == B.RUBIX_OK                          # nothing to do
+
+
 def test_no_cpu_fallback_without_the_library(monkeypatch):
     monkeypatch.setattr(B, "_lib", None)
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/librubix_b200.so")
