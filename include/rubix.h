@@ -20,7 +20,8 @@
  *     read before the call returns and may be freed right after it.
  *     Consequently a sequence of calls can be captured in a CUDA graph (stage timing of
  *     rubix_peaks.h off) and replayed; the kernels read their sizes from the workspace, not
- *     from the host, after the call has returned.
+ *     from the host, after the call has returned.  (Exception: with rubix_telescope.lambda_obs the call
+ *     copies that host array to the workspace; capture it only from pinned memory that stays alive.)
  *   - Device arrays are dense, row-major, fp32 / int32 as stated, 16-byte aligned.
  *   - Errors: every call validates its arguments on the host BEFORE any launch and returns a
  *     rubix_status; nothing throws or aborts.  rubix_last_error() gives a thread-local message.

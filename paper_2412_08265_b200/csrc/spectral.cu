@@ -123,16 +123,16 @@ k_accumulate(const __grid_constant__ AccumParams P)
     int64_t x_tile0 = 0;                                    // LOGX: xtab[k0]
 #pragma unroll
     for (int i = 0; i < CPT; ++i) acc[i] = 0.0f;
-    if (LOGX) {
-        x_tile0 = P.xtab[k0];
-#pragma unroll
-        for (int i = 0; i < CPT; ++i) {
-            const int k = k0 + tid + i * kAccThreads;
-            xl[i] = (uint32_t)((P.xtab[min(k, P.n_c)] - x_tile0) >> 8);
-        }
-    }
 
     if (U.count > 0) {
+        if (LOGX) {                                         // the table exists only when there are particles
+            x_tile0 = P.xtab[k0];
+#pragma unroll
+            for (int i = 0; i < CPT; ++i) {
+                const int k = k0 + tid + i * kAccThreads;
+                xl[i] = (uint32_t)((P.xtab[min(k, P.n_c)] - x_tile0) >> 8);
+            }
+        }
         int4 *srec = reinterpret_cast<int4 *>(tab + 2 * (size_t)P.wcap);
         {
             const int4 *g = reinterpret_cast<const int4 *>(P.rec + U.start);
