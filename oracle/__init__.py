@@ -199,42 +199,71 @@ def build_cube(particles, R, ssp, tel, sel=None):
 
 
 # ----------------------------------------------------------------------------- steps 7-8
+def psf_sigma_k(tel):
+    """Per-channel PSF width of reading R18, or None when the PSF is the same for every channel:
+    sigma_k = psf_sigma * (lambda_k / psf_lambda_ref) ** psf_alpha, lambda_k the observed wavelengths."""
+    alpha = float(getattr(tel, "psf_alpha", 0.0))
+    if alpha == 0.0 or tel.psf_size <= 0:
+        return None
+    return np.float64(tel.psf_sigma) * (tel.wavelengths() / np.float64(tel.psf_lambda_ref)) ** alpha
+
+
+class _psf_sigma:
+    """Installs a per-channel PSF width array in the C oracle for one call."""
+
+    def __init__(self, sigma_k):
+        self.arr = None if sigma_k is None else np.ascontiguousarray(sigma_k, dtype=np.float64)
+
+    def __enter__(self):
+        if self.arr is not None:
+            _load().orc_set_psf_sigma(_pd(self.arr))
+
+    def __exit__(self, *exc):
+        if self.arr is not None:
+            _load().orc_set_psf_sigma(None)
+
+
 def gauss_taps(size, sigma):
     taps = np.empty(size, np.float64)
     _load().orc_gauss_taps(C.c_int32(size), C.c_double(float(sigma)), _pd(taps))
     return taps
 
 
-def convolve(cube, psf_size, psf_sigma, lsf_size, lsf_sigma):
+def convolve(cube, psf_size, psf_sigma, lsf_size, lsf_sigma, sigma_k=None):
+    """LSF along the channel, then the PSF over (x, y); ``sigma_k``: per-channel PSF widths (reading R18)."""
     cube = np.ascontiguousarray(cube, dtype=np.float64)
     n_x, n_y, n_c = cube.shape
     out = np.empty_like(cube)
-    _load().orc_convolve(_pd(cube), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c),
-                         C.c_int32(psf_size), C.c_double(float(psf_sigma)), C.c_int32(lsf_size),
-                         C.c_double(float(lsf_sigma)), _pd(out))
+    assert sigma_k is None or len(sigma_k) == n_c
+    with _psf_sigma(sigma_k):
+        _load().orc_convolve(_pd(cube), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c),
+                             C.c_int32(psf_size), C.c_double(float(psf_sigma)), C.c_int32(lsf_size),
+                             C.c_double(float(lsf_sigma)), _pd(out))
     return out
 
 
-def convolve_transpose(gout, psf_size, psf_sigma, lsf_size, lsf_sigma):
+def convolve_transpose(gout, psf_size, psf_sigma, lsf_size, lsf_sigma, sigma_k=None):
     gout = np.ascontiguousarray(gout, dtype=np.float64)
     n_x, n_y, n_c = gout.shape
     gin = np.empty_like(gout)
-    _load().orc_convolve_transpose(_pd(gout), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c),
-                                   C.c_int32(psf_size), C.c_double(float(psf_sigma)),
-                                   C.c_int32(lsf_size), C.c_double(float(lsf_sigma)), _pd(gin))
+    with _psf_sigma(sigma_k):
+        _load().orc_convolve_transpose(_pd(gout), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c),
+                                       C.c_int32(psf_size), C.c_double(float(psf_sigma)),
+                                       C.c_int32(lsf_size), C.c_double(float(lsf_sigma)), _pd(gin))
     return gin
 
 
-def convolve_voxels_f32(cube_f32, vox, psf_size, psf_sigma, lsf_size, lsf_sigma):
+def convolve_voxels_f32(cube_f32, vox, psf_size, psf_sigma, lsf_size, lsf_sigma, sigma_k=None):
     """Brute-force value of sampled output voxels (flat indices) of an fp32 input cube."""
     assert cube_f32.dtype == np.float32 and cube_f32.flags.c_contiguous
     n_x, n_y, n_c = cube_f32.shape
     vox = np.ascontiguousarray(vox, dtype=np.int64)
     out = np.empty(vox.size, np.float64)
-    _load().orc_convolve_voxels_f32(
-        _pf(cube_f32), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c), C.c_int32(psf_size),
-        C.c_double(float(psf_sigma)), C.c_int32(lsf_size), C.c_double(float(lsf_sigma)),
-        _p(vox, C.c_int64), C.c_int64(vox.size), _pd(out))
+    with _psf_sigma(sigma_k):
+        _load().orc_convolve_voxels_f32(
+            _pf(cube_f32), C.c_int32(n_x), C.c_int32(n_y), C.c_int32(n_c), C.c_int32(psf_size),
+            C.c_double(float(psf_sigma)), C.c_int32(lsf_size), C.c_double(float(lsf_sigma)),
+            _p(vox, C.c_int64), C.c_int64(vox.size), _pd(out))
     return out
 
 
@@ -242,7 +271,7 @@ def forward(particles, R, ssp, tel):
     """Whole path: build + PSF/LSF (whatever ``tel`` switches on).  fp64 [n_x, n_y, n_c]."""
     cube = build_cube(particles, R, ssp, tel)
     if tel.psf_size > 0 or tel.lsf_size > 0:
-        cube = convolve(cube, tel.psf_size, tel.psf_sigma, tel.lsf_size, tel.lsf_sigma)
+        cube = convolve(cube, tel.psf_size, tel.psf_sigma, tel.lsf_size, tel.lsf_sigma, psf_sigma_k(tel))
     return cube
 
 
@@ -257,7 +286,7 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     grad_cube = np.ascontiguousarray(grad_cube, dtype=np.float64)
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
-    with _lambda_obs(tel):
+    with _lambda_obs(tel), _psf_sigma(psf_sigma_k(tel)):
         _load().orc_adjoint_mode(
             C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
             C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
@@ -296,8 +325,14 @@ def fd_gradients(particles, R, ssp, tel, residual, idx, h_mass=1e-3, h_log=1e-4,
     key, vlos = rotate_bin(particles.pos, particles.vel, R, tel.n_x, tel.n_y, tel.spaxel_size)
     ia, iz, _, _ = ssp_cells(particles.log_age, particles.log_z, ssp.log_age_axis, ssp.log_z_axis)
     n_c = tel.n_channels
-    g = gauss_taps(tel.psf_size, tel.psf_sigma) if tel.psf_size > 0 else np.ones(1)
-    hp = (g.size - 1) // 2
+    # PSF taps per channel, [n_c, psf_size] (all rows equal unless the PSF depends on wavelength, reading R18)
+    if tel.psf_size > 0:
+        sk = psf_sigma_k(tel)
+        gk = np.stack([gauss_taps(tel.psf_size, tel.psf_sigma if sk is None else sk[k]) for k in range(n_c)]) \
+            if sk is not None else np.broadcast_to(gauss_taps(tel.psf_size, tel.psf_sigma), (n_c, tel.psf_size))
+    else:
+        gk = np.ones((n_c, 1))
+    hp = (gk.shape[1] - 1) // 2
 
     def lsf(row):
         if tel.lsf_size <= 0:
@@ -306,14 +341,14 @@ def fd_gradients(particles, R, ssp, tel, residual, idx, h_mass=1e-3, h_log=1e-4,
 
     def delta_loss(delta, sx, sy):
         row = lsf(delta)
-        rr = float(row @ row)
         acc = 0.0
         for dx in range(-hp, hp + 1):
             for dy in range(-hp, hp + 1):
                 x, y = sx + dx, sy + dy
                 if 0 <= x < tel.n_x and 0 <= y < tel.n_y:
-                    w = g[dx + hp] * g[dy + hp]
-                    acc += 2.0 * w * float(residual[x, y] @ row) + w * w * rr
+                    w = gk[:, dx + hp] * gk[:, dy + hp]            # per channel
+                    wr = w * row
+                    acc += 2.0 * float(residual[x, y] @ wr) + float(wr @ wr)
         return acc
 
     out = np.zeros((4, len(idx)), np.float64)

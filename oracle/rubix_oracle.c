@@ -390,6 +390,19 @@ void orc_gauss_taps(int32_t size, double sigma, double *taps)
     for (int32_t i = 0; i < size; ++i) taps[i] /= sum;
 }
 
+/* Wavelength-dependent PSF (reading R18): while an array is installed with orc_set_psf_sigma, channel k
+ * uses taps of width psf_sigma_k[k] (the wrapper computes sigma_k = psf_sigma (lambda_k / lambda_ref)^alpha);
+ * otherwise every channel uses psf_sigma.  Table [n_c][psf_size] of normalised taps. */
+static const double *g_psf_sigma_k = 0;
+void orc_set_psf_sigma(const double *sigma_k) { g_psf_sigma_k = sigma_k; }
+static double *psf_taps_table(int32_t psf_size, double psf_sigma, int32_t n_c)
+{
+    double *t = (double *)malloc(sizeof(double) * (size_t)psf_size * (size_t)(n_c > 0 ? n_c : 1));
+    for (int32_t k = 0; k < n_c; ++k)
+        orc_gauss_taps(psf_size, g_psf_sigma_k ? g_psf_sigma_k[k] : psf_sigma, t + (size_t)k * psf_size);
+    return t;
+}
+
 void orc_convolve(const double *in, int32_t n_x, int32_t n_y, int32_t n_c, int32_t psf_size,
                   double psf_sigma, int32_t lsf_size, double lsf_sigma, double *out)
 {
@@ -415,8 +428,7 @@ void orc_convolve(const double *in, int32_t n_x, int32_t n_y, int32_t n_c, int32
     /* PSF over (x, y), per channel: direct 2-D sum with the outer-product kernel */
     if (psf_size > 0) {
         const int32_t h = (psf_size - 1) / 2;
-        double *taps = (double *)malloc(sizeof(double) * (size_t)psf_size);
-        orc_gauss_taps(psf_size, psf_sigma, taps);
+        double *taps = psf_taps_table(psf_size, psf_sigma, n_c);     /* [n_c][psf_size] */
 #pragma omp parallel for schedule(static) collapse(2)
         for (int32_t x = 0; x < n_x; ++x)
             for (int32_t y = 0; y < n_y; ++y) {
@@ -426,9 +438,9 @@ void orc_convolve(const double *in, int32_t n_x, int32_t n_y, int32_t n_c, int32
                     for (int32_t dy = -h; dy <= h; ++dy) {
                         const int32_t xx = x + dx, yy = y + dy;
                         if (xx < 0 || xx >= n_x || yy < 0 || yy >= n_y) continue;
-                        const double w = taps[dx + h] * taps[dy + h];
                         const double *r = tmp + ((int64_t)xx * n_y + yy) * n_c;
-                        for (int32_t k = 0; k < n_c; ++k) o[k] += w * r[k];
+                        for (int32_t k = 0; k < n_c; ++k)
+                            o[k] += taps[(size_t)k * psf_size + dx + h] * taps[(size_t)k * psf_size + dy + h] * r[k];
                     }
             }
         free(taps);
@@ -446,9 +458,11 @@ void orc_convolve_voxels_f32(const float *in, int32_t n_x, int32_t n_y, int32_t 
 {
     const int32_t hp = psf_size > 0 ? (psf_size - 1) / 2 : 0;
     const int32_t hl = lsf_size > 0 ? (lsf_size - 1) / 2 : 0;
-    double *g = (double *)malloc(sizeof(double) * (size_t)(2 * hp + 1));
+    const int32_t np = 2 * hp + 1;
+    double *g = 0;                                         /* [n_c][np] */
     double *hh = (double *)malloc(sizeof(double) * (size_t)(2 * hl + 1));
-    if (psf_size > 0) orc_gauss_taps(psf_size, psf_sigma, g); else g[0] = 1.0;
+    if (psf_size > 0) g = psf_taps_table(psf_size, psf_sigma, n_c);
+    else { g = (double *)malloc(sizeof(double) * (size_t)n_c); for (int32_t k = 0; k < n_c; ++k) g[k] = 1.0; }
     if (lsf_size > 0) orc_gauss_taps(lsf_size, lsf_sigma, hh); else hh[0] = 1.0;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < n_vox; ++i) {
@@ -464,7 +478,8 @@ void orc_convolve_voxels_f32(const float *in, int32_t n_x, int32_t n_y, int32_t 
                 for (int32_t dc = -hl; dc <= hl; ++dc) {
                     const int32_t kk = k + dc;
                     if (kk < 0 || kk >= n_c) continue;
-                    acc += g[dx + hp] * g[dy + hp] * hh[dc + hl]
+                    /* LSF first, then the PSF of the OUTPUT channel k (the PSF acts per channel after the LSF) */
+                    acc += g[(size_t)k * np + dx + hp] * g[(size_t)k * np + dy + hp] * hh[dc + hl]
                            * (double)in[((int64_t)xx * n_y + yy) * n_c + kk];
                 }
             }
@@ -483,18 +498,17 @@ void orc_convolve_transpose(const double *gout, int32_t n_x, int32_t n_y, int32_
     double *tmp = (double *)calloc((size_t)(n_vox > 0 ? n_vox : 1), sizeof(double));
     if (psf_size > 0) {
         const int32_t h = (psf_size - 1) / 2;
-        double *taps = (double *)malloc(sizeof(double) * (size_t)psf_size);
-        orc_gauss_taps(psf_size, psf_sigma, taps);
+        double *taps = psf_taps_table(psf_size, psf_sigma, n_c);
         for (int32_t x = 0; x < n_x; ++x)          /* scatter: serial, small cubes only */
             for (int32_t y = 0; y < n_y; ++y)
                 for (int32_t dx = -h; dx <= h; ++dx)
                     for (int32_t dy = -h; dy <= h; ++dy) {
                         const int32_t xx = x + dx, yy = y + dy;
                         if (xx < 0 || xx >= n_x || yy < 0 || yy >= n_y) continue;
-                        const double w = taps[dx + h] * taps[dy + h];
                         const double *o = gout + ((int64_t)x * n_y + y) * n_c;
                         double *t = tmp + ((int64_t)xx * n_y + yy) * n_c;
-                        for (int32_t k = 0; k < n_c; ++k) t[k] += w * o[k];
+                        for (int32_t k = 0; k < n_c; ++k)
+                            t[k] += taps[(size_t)k * psf_size + dx + h] * taps[(size_t)k * psf_size + dy + h] * o[k];
                     }
         free(taps);
     } else {

@@ -190,6 +190,8 @@ class Telescope:
     redshift: np.float32 = np.float32(0.0)     # cosmological redshift of the galaxy
     flux_scale: np.float32 = np.float32(1.0)   # multiplies every spectrum (distance dimming / units)
     lambda_obs: np.ndarray | None = None       # explicit, increasing channel wavelengths [n_channels] fp32 (else uniform)
+    psf_alpha: np.float32 = np.float32(0.0)    # PSF width ~ (lambda / psf_lambda_ref)^psf_alpha; 0 = the same for every channel
+    psf_lambda_ref: np.float32 = np.float32(1.0)
 
     @property
     def n_spaxels(self) -> int:
