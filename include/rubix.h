@@ -94,6 +94,11 @@ typedef struct {
                                     /* wavelengths (Angstrom, > 0, strictly increasing) replace  */
                                     /* lambda0 + k dlambda; RUBIX_RESAMPLE_POINT only.  Read (and */
                                     /* copied to the workspace) before the call returns.         */
+    float psf_alpha;                /* wavelength-dependent PSF: channel k uses the width         */
+    float psf_lambda_ref;           /* psf_sigma (lambda_k / psf_lambda_ref)^psf_alpha (e.g. -0.2 */
+                                    /* for seeing); 0 = the same PSF for every channel.  Needs    */
+                                    /* psf_size <= 15, lsf_size <= 9 and an even n_channels.      */
+                                    /* The PSF then acts AFTER the LSF (they no longer commute).  */
 } rubix_telescope;
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the

@@ -50,7 +50,8 @@ class CTelescope(C.Structure):
                 ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
                 ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
-                ("redshift", C.c_float), ("flux_scale", C.c_float), ("lambda_obs", C.c_void_p)]
+                ("redshift", C.c_float), ("flux_scale", C.c_float), ("lambda_obs", C.c_void_p),
+                ("psf_alpha", C.c_float), ("psf_lambda_ref", C.c_float)]
 
 
 _lib = None
@@ -149,7 +150,8 @@ def c_telescope(tel) -> _Keep:
                             float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma),
                             int(getattr(tel, "resample", 0)), float(getattr(tel, "redshift", 0.0)),
                             float(getattr(tel, "flux_scale", 1.0)),
-                            None if lam is None else lam.ctypes.data), lam)
+                            None if lam is None else lam.ctypes.data, float(getattr(tel, "psf_alpha", 0.0)),
+                            float(getattr(tel, "psf_lambda_ref", 1.0))), lam)
 
 
 def c_ssp(ssp, flux) -> _Keep:

@@ -79,6 +79,15 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_INVALID_ARG, "redshift must be in [0, 20]");
     if (!(t->flux_scale > 0.0f) || !isfinite(t->flux_scale))
         return fail(RUBIX_ERR_INVALID_ARG, "flux_scale must be > 0 and finite (1 = no scaling)");
+    if (t->psf_alpha != 0.0f && t->psf_size > 0) {
+        if (!isfinite(t->psf_alpha) || fabsf(t->psf_alpha) > 4.0f || !(t->psf_lambda_ref > 0.0f) || !isfinite(t->psf_lambda_ref))
+            return fail(RUBIX_ERR_INVALID_ARG, "psf_alpha must be finite with |psf_alpha| <= 4 and psf_lambda_ref > 0");
+        if (t->psf_size > 15 || t->lsf_size > 9 || (t->n_channels % 2) != 0)
+            return fail(RUBIX_ERR_UNSUPPORTED,
+                        "a wavelength-dependent PSF needs psf_size <= 15, lsf_size <= 9 and an even n_channels");
+        if (!t->lambda_obs && !((double)t->lambda0 > 0.0 && (double)t->lambda0 + (double)t->dlambda * (t->n_channels - 1) > 0.0))
+            return fail(RUBIX_ERR_INVALID_ARG, "a wavelength-dependent PSF needs positive channel wavelengths");
+    }
     if (t->lambda_obs) {
         if (t->resample != RUBIX_RESAMPLE_POINT)
             return fail(RUBIX_ERR_UNSUPPORTED, "explicit channel wavelengths support RUBIX_RESAMPLE_POINT only");
@@ -206,15 +215,18 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
     const char *a = (const char *)cube_in, *b = (const char *)cube_out;
     if (a < b + cube_bytes && b < a + cube_bytes)
         return fail(RUBIX_ERR_INVALID_ARG, "cube_in and cube_out overlap");
-    float *tmp = nullptr;
+    float *tmp = nullptr, *taps = nullptr;
     if (tel->psf_size > 0) {
-        if ((s = check_ws(workspace, workspace_bytes, align_up(cube_bytes, 256))) != RUBIX_OK) return s;
+        const bool var = tel->psf_alpha != 0.0f;
+        const size_t need = align_up(cube_bytes, 256) + (var ? psf_taps_bytes(tel->n_channels) : 0);
+        if ((s = check_ws(workspace, workspace_bytes, need)) != RUBIX_OK) return s;
         tmp = (float *)workspace;
+        if (var) taps = (float *)((char *)workspace + align_up(cube_bytes, 256));   // start of the second cube buffer
     }
     cudaError_t e;
     {
         StageTimer t(3, (cudaStream_t)stream);
-        e = launch_convolve(tel, cube_in, cube_out, tmp, (cudaStream_t)stream);
+        e = launch_convolve(tel, cube_in, cube_out, tmp, taps, false, (cudaStream_t)stream);
     }
     if (e != cudaSuccess) return cuda_fail(e, "convolve");
     return RUBIX_OK;
@@ -252,7 +264,8 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
     if (tel->psf_size > 0 || tel->lsf_size > 0) {
         {
             StageTimer t(3, st);
-            e = launch_convolve(tel, grad_cube, (float *)(ws + L.off_cube_a), (float *)(ws + L.off_cube_b), st);
+            e = launch_convolve(tel, grad_cube, (float *)(ws + L.off_cube_a), (float *)(ws + L.off_cube_b),
+                                (float *)(ws + L.off_psftaps), true, st);
         }
         if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
         gconv = (const float *)(ws + L.off_cube_a);
@@ -317,7 +330,7 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
         float *fin = cube_out ? cube_out : buf_c;
         {
             StageTimer t(3, st);
-            e = launch_convolve(tel, raw, fin, buf_b, st);
+            e = launch_convolve(tel, raw, fin, buf_b, (float *)(ws + L.off_psftaps), false, st);
         }
         if (e != cudaSuccess) return cuda_fail(e, "convolve");
         final_cube = fin;
@@ -330,7 +343,7 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
     if (conv) {                                            // G' = LSF^T PSF^T G (self-adjoint stencils)
         {
             StageTimer t(3, st);
-            e = launch_convolve(tel, grad, buf_c, buf_b, st);   // buf_c is free: the final cube has been consumed
+            e = launch_convolve(tel, grad, buf_c, buf_b, (float *)(ws + L.off_psftaps), true, st);   // buf_c is free
         }
         if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
         gconv = buf_c;

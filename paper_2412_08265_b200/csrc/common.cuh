@@ -9,6 +9,8 @@
 
 namespace rubix {
 
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
 // ---- fixed constants of the method ------------------------------------
 constexpr double kCkms = 299792.458;        // speed of light, km/s
 constexpr float kVcapKms = 14989.623f;      // 0.05 c: |v_los| beyond this drops the particle
@@ -65,7 +67,7 @@ struct Layout {
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,
-        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs;
+        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps;
     int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
                                       // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
@@ -85,8 +87,11 @@ struct PassInputs {
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube,
                               cudaStream_t st);
-cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp,
-                            cudaStream_t st);
+// taps_dev: device scratch of psf_taps_bytes(n_channels) for a wavelength-dependent PSF (reading R18), else unused.
+// transpose: apply LSF^T PSF^T (PSF first, then LSF) instead of PSF LSF; only differs when the PSF depends on lambda.
+cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
+                            bool transpose, cudaStream_t st);
+inline size_t psf_taps_bytes(int32_t n_c) { return align_up((size_t)15 * ((size_t)n_c + 2) * 4, 256); }
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st);
 
@@ -156,6 +161,5 @@ __device__ __forceinline__ float2 unpack2(unsigned long long v)
     return r;
 }
 
-static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace rubix

@@ -13,6 +13,8 @@
 // Anything else (larger stencils, odd channel counts) takes the generic one-axis kernel.
 #include <math.h>
 
+#include <vector>
+
 #include "common.cuh"
 
 namespace rubix {
@@ -71,6 +73,8 @@ struct MarchParams {
     int32_t n_lines, n_steps, n_c, cblocks;
     float g[15];                        // stencil along the marching axis, zero padded, centred
     float h[9];                         // LSF taps along the channel, zero padded, centred, symmetric
+    const float *taps;                  // VAR: per-channel PSF taps, tap-major [15][tstride] (reading R18)
+    int32_t tstride;
 };
 
 __device__ __forceinline__ float2 shfl_up2(float2 v, int d)
@@ -105,8 +109,10 @@ __device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned 
 #endif
 constexpr int kMarchPf = RUBIX_MARCH_PF;          // steps prefetched per thread (divides 15)
 
-template <bool LSF>
-__global__ void __launch_bounds__(256, RUBIX_MARCH_MINB)
+// VAR: the stencil along the marching axis differs per channel (wavelength-dependent PSF, reading R18): the
+// thread loads the 15 taps of its two channels once; they then live in registers (two resident CTAs per SM).
+template <bool LSF, bool VAR = false>
+__global__ void __launch_bounds__(256, VAR ? 2 : RUBIX_MARCH_MINB)
 k_march(const __grid_constant__ MarchParams P)
 {
     const int lane = threadIdx.x & 31;
@@ -126,7 +132,15 @@ k_march(const __grid_constant__ MarchParams P)
     unsigned long long acc[15], g2[15], hp[5];
     float2 pf[kMarchPf];
 #pragma unroll
-    for (int i = 0; i < 15; ++i) { acc[i] = 0ull; g2[i] = pack2(P.g[i], P.g[i]); }
+    for (int i = 0; i < 15; ++i) {
+        acc[i] = 0ull;
+        if (VAR) {
+            const float2 t = c_ok ? *reinterpret_cast<const float2 *>(P.taps + (size_t)i * P.tstride + c) : make_float2(0.f, 0.f);
+            g2[i] = pack2(t.x, t.y);
+        } else {
+            g2[i] = pack2(P.g[i], P.g[i]);
+        }
+    }
 #pragma unroll
     for (int i = 0; i < 5; ++i) hp[i] = pack2(P.h[4 + i], P.h[4 + i]);
 #pragma unroll
@@ -180,8 +194,33 @@ static void centre_taps(const Taps &t, int width, float *dst)
     for (int i = 0; i < t.size; ++i) dst[shift + i] = t.w[i];
 }
 
-cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp,
-                            cudaStream_t st)
+// per-channel PSF taps (reading R18), tap-major [15][tstride], computed on the host in fp64 like make_taps
+static void var_psf_taps(const rubix_telescope *tel, int tstride, float *dst)
+{
+    const int h = (tel->psf_size - 1) / 2, shift = (15 - tel->psf_size) / 2;
+    for (int i = 0; i < 15 * tstride; ++i) dst[i] = 0.0f;
+    const double zp1 = 1.0;                                // observed wavelengths: the telescope's own grid
+    for (int k = 0; k < tel->n_channels; ++k) {
+        const double lam = (tel->lambda_obs ? (double)tel->lambda_obs[k] : (double)tel->lambda0 + (double)tel->dlambda * k) / zp1;
+        const double sigma = (double)tel->psf_sigma * pow(lam / (double)tel->psf_lambda_ref, (double)tel->psf_alpha);
+        double w[15], sum = 0.0;
+        for (int i = -h; i <= h; ++i) { w[i + h] = exp(-((double)i * i) / (2.0 * sigma * sigma)); sum += w[i + h]; }
+        for (int i = 0; i < tel->psf_size; ++i) dst[(size_t)(shift + i) * tstride + k] = (float)(w[i] / sum);
+    }
+}
+
+template <bool LSF, bool VAR>
+static cudaError_t march(MarchParams &P, cudaStream_t st)
+{
+    P.cblocks = LSF ? (P.n_c + 55) / 56 : (P.n_c + 63) / 64;
+    const int64_t warps = (int64_t)P.n_lines * P.cblocks;
+    k_march<LSF, VAR><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
+cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
+                            bool transpose, cudaStream_t st)
 {
     const int32_t n_x = tel->n_x, n_y = tel->n_y, n_c = tel->n_channels;
     const int64_t n_vox = (int64_t)n_x * n_y * n_c;
@@ -192,11 +231,13 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     if (lsf.size <= 0 && psf.size <= 0)
         return cudaMemcpyAsync(out, in, (size_t)n_vox * 4, cudaMemcpyDeviceToDevice, st);
 
+    const bool var = psf.size > 0 && tel->psf_alpha != 0.0f;
     const bool aligned = (n_c % 2 == 0) && (((uintptr_t)in & 7u) == 0) && (((uintptr_t)out & 7u) == 0) &&
                          (tmp == nullptr || ((uintptr_t)tmp & 7u) == 0);
     const bool fast = aligned && psf.size <= 15 && lsf.size <= 9;
     cudaError_t e;
     if (!fast) {
+        if (var) return cudaErrorNotSupported;             // api.cu refuses this combination beforehand
         const float *src = in;
         if (lsf.size > 0) {
             if ((e = stencil_generic(src, out, n_vox, 1, n_c, lsf, st)) != cudaSuccess) return e;
@@ -211,42 +252,59 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
 
     MarchParams P;
     P.n_c = n_c;
+    P.taps = nullptr;
+    P.tstride = 0;
     centre_taps(psf, 15, P.g);
     centre_taps(lsf, 9, P.h);
-    if (psf.size <= 0) {                                   // LSF only
-        P.in = in; P.out = out;
+    auto lsf_rows = [&](const float *src, float *dst) -> cudaError_t {
+        P.in = src; P.out = dst;
         P.n_lines = n_x * n_y; P.n_steps = 1; P.line_stride = n_c; P.step_stride = 0;
         P.cblocks = (n_c + 55) / 56;
         const int64_t warps = (int64_t)P.n_lines * P.cblocks;
         k_lsf_rows<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
         RUBIX_LAUNCH_CHECK();
         return cudaSuccess;
+    };
+    auto along_y = [&](const float *src, float *dst) {     // lines = x
+        P.in = src; P.out = dst;
+        P.n_lines = n_x; P.n_steps = n_y;
+        P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
+    };
+    auto along_x = [&](const float *src, float *dst) {     // lines = y
+        P.in = src; P.out = dst;
+        P.n_lines = n_y; P.n_steps = n_x;
+        P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
+    };
+    if (psf.size <= 0) return lsf_rows(in, out);           // LSF only
+
+    if (var) {
+        // wavelength-dependent PSF: per-channel taps go to the device once per call
+        P.tstride = n_c + 2;
+        P.taps = taps_dev;
+        static thread_local std::vector<float> host_taps;
+        host_taps.resize((size_t)15 * P.tstride);
+        var_psf_taps(tel, P.tstride, host_taps.data());
+        e = cudaMemcpyAsync(taps_dev, host_taps.data(), host_taps.size() * 4, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return e;
+        if (transpose && lsf.size > 0) {                   // LSF^T PSF^T: PSF first (y, x), then the LSF
+            along_y(in, out);
+            if ((e = march<false, true>(P, st)) != cudaSuccess) return e;
+            along_x(out, tmp);
+            if ((e = march<false, true>(P, st)) != cudaSuccess) return e;
+            return lsf_rows(tmp, out);
+        }
+        along_y(in, tmp);                                  // PSF LSF: LSF fused into the pass along y
+        e = lsf.size > 0 ? march<true, true>(P, st) : march<false, true>(P, st);
+        if (e != cudaSuccess) return e;
+        along_x(tmp, out);
+        return march<false, true>(P, st);
     }
-    // pass 1: along y (lines = x), LSF fused when on
-    P.in = in; P.out = tmp;
-    P.n_lines = n_x; P.n_steps = n_y;
-    P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
-    if (lsf.size > 0) {
-        P.cblocks = (n_c + 55) / 56;
-        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
-        k_march<true><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
-    } else {
-        P.cblocks = (n_c + 63) / 64;
-        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
-        k_march<false><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
-    }
-    RUBIX_LAUNCH_CHECK();
-    // pass 2: along x (lines = y)
-    P.in = tmp; P.out = out;
-    P.n_lines = n_y; P.n_steps = n_x;
-    P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
-    P.cblocks = (n_c + 63) / 64;
-    {
-        const int64_t warps = (int64_t)P.n_lines * P.cblocks;
-        k_march<false><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
-    }
-    RUBIX_LAUNCH_CHECK();
-    return cudaSuccess;
+    // pass 1: along y (lines = x), LSF fused when on; pass 2: along x (lines = y)
+    along_y(in, tmp);
+    e = lsf.size > 0 ? march<true, false>(P, st) : march<false, false>(P, st);
+    if (e != cudaSuccess) return e;
+    along_x(tmp, out);
+    return march<false, false>(P, st);
 }
 
 }  // namespace rubix

@@ -529,6 +529,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
     L.off_xtab = take(((size_t)n_c + 1) * 8);           // Y[k] of the table mode (readings R15 / R16)
     L.off_lamobs = take(((size_t)n_c + 1) * 4);         // device copy of rubix_telescope.lambda_obs
+    L.off_psftaps = take(psf_taps_bytes(n_c));          // per-channel PSF taps (reading R18)
     L.bytes_total = off;
     return L;
 }
