@@ -47,6 +47,9 @@ def random_case(seed):
         lam = (float(tel.lambda0) + float(tel.dlambda) * (np.cumsum(steps) - steps[0])).astype(np.float32)
         if np.all(np.diff(lam) > 0):
             tel = dataclasses.replace(tel, lambda_obs=lam)
+    if 0 < psf <= 15 and lsf <= 9 and n_c % 2 == 0 and rng.integers(0, 3) == 0:     # wavelength-dependent PSF (R18)
+        tel = dataclasses.replace(tel, psf_alpha=np.float32(rng.choice([-0.2, -1.0, 0.8])),
+                                  psf_lambda_ref=np.float32(rng.uniform(4000.0, 9000.0)))
     n = int(rng.choice([0, 1, 7, 300, 2500]))
     w = synth.make_workload("tiny", n=max(n, 1), seed=int(rng.integers(1, 10 ** 6)))
     if n == 0:
@@ -57,12 +60,12 @@ def random_case(seed):
     return w
 
 
-@pytest.mark.parametrize("seed", range(60))
+@pytest.mark.parametrize("seed", range(80))
 def test_random_configuration(B, seed):
     w = random_case(1234 + seed)
     t = w.telescope
     what = f"seed {seed}: n={w.particles.n} {t.n_x}x{t.n_y}x{t.n_channels} psf={t.psf_size} lsf={t.lsf_size} " \
-           f"resample={t.resample} log={w.ssp.log_lambda} z={float(t.redshift)} listed={t.lambda_obs is not None}"
+           f"resample={t.resample} log={w.ssp.log_lambda} z={float(t.redshift)} listed={t.lambda_obs is not None} alpha={float(t.psf_alpha)}"
     dw = B.DeviceWorkload(w)
     cube = dw.build_cube(out=torch.full(dw.shape, float("nan"), device="cuda"))
     final = dw.convolve(cube)
@@ -81,7 +84,7 @@ def test_random_configuration(B, seed):
     if pos.any():
         assert (np.abs(got.sum(-1) - fr)[pos] / fr[pos]).max() <= 1e-5, what
     assert not got[fr == 0].any(), what
-    ref_final = oracle.convolve(ref, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)
+    ref_final = oracle.convolve(ref, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma, oracle.psf_sigma_k(t))
     assert np.abs(final.cpu().numpy() - ref_final).max() <= 1e-4 * max(ref_final.max(), 1e-300), what
     if w.particles.n == 0:
         return
