@@ -206,6 +206,19 @@ rubix_status rubix_forward_host(const rubix_particles *h_particles, const rubix_
                                 const rubix_telescope *tel, const float *R, float *h_cube,
                                 void *device_scratch, size_t scratch_bytes, void *stream);
 
+/* Pipelined variant of rubix_forward_host for back-to-back cubes (mock-catalogue generation): the device->host copy
+ * of call i runs on an internal copy stream while call i + 1 computes on `stream`; two device buffers take the final
+ * cube in turn (scratch: rubix_forward_host_pipelined_scratch_bytes, one cube more).  Everything else is as
+ * rubix_forward_host, EXCEPT completion: h_cube of a call is complete once rubix_forward_host_drain(stream) has been
+ * called after it and `stream` has completed (or the device has been synchronised).  Host buffers must be pinned
+ * for the copies to overlap.  One pipeline per process (calls are serialised by a mutex). */
+size_t rubix_forward_host_pipelined_scratch_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel);
+rubix_status rubix_forward_host_pipelined(const rubix_particles *h_particles, const rubix_ssp *h_ssp,
+                                          const rubix_telescope *tel, const float *R, float *h_cube,
+                                          void *device_scratch, size_t scratch_bytes, void *stream);
+/* Makes `stream` wait for every device->host copy the pipelined calls have enqueued so far. */
+rubix_status rubix_forward_host_drain(void *stream);
+
 /* Number of kernel launches the last compute call on this thread enqueued (bench.py's
  * gpu_launches claim is the sum over the timed region). */
 int32_t rubix_last_launch_count(void);

@@ -20,6 +20,7 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error",
+           "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
@@ -94,6 +95,12 @@ def load():
         lib.rubix_forward_host.restype = C.c_int
         lib.rubix_forward_host.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_forward_host_pipelined_scratch_bytes.restype = C.c_size_t
+        lib.rubix_forward_host_pipelined_scratch_bytes.argtypes = [C.c_int64, C.POINTER(CSSP), C.POINTER(CTelescope)]
+        lib.rubix_forward_host_pipelined.restype = C.c_int
+        lib.rubix_forward_host_pipelined.argtypes = lib.rubix_forward_host.argtypes
+        lib.rubix_forward_host_drain.restype = C.c_int
+        lib.rubix_forward_host_drain.argtypes = [C.c_void_p]
         lib.rubix_measure_peaks.restype = C.c_int32
         lib.rubix_measure_peaks.argtypes = [C.POINTER(C.c_float), C.c_void_p, C.c_size_t, C.c_void_p]
         lib.rubix_stage_timing_enable.restype = None
@@ -255,6 +262,24 @@ def rubix_forward_host(particles: _Keep, ssp: _Keep, tel: _Keep, R, h_cube, scra
     _check(load().rubix_forward_host(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(h_cube),
                                      _ptr(scratch), int(scratch.numel() * scratch.element_size()),
                                      _stream(stream)))
+
+
+def rubix_forward_host_pipelined_scratch_bytes(n, ssp: _Keep, tel: _Keep) -> int:
+    b = int(load().rubix_forward_host_pipelined_scratch_bytes(int(n), ssp.ref(), tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_forward_host_pipelined(particles: _Keep, ssp: _Keep, tel: _Keep, R, h_cube, scratch, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_forward_host_pipelined(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(h_cube),
+                                               _ptr(scratch), int(scratch.numel() * scratch.element_size()),
+                                               _stream(stream)))
+
+
+def rubix_forward_host_drain(stream=None):
+    _check(load().rubix_forward_host_drain(_stream(stream)))
 
 
 # ------------------------------------------------------------------------------ rubix_peaks.h

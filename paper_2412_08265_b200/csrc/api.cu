@@ -427,9 +427,32 @@ size_t rubix_forward_host_scratch_bytes(int64_t n, const rubix_ssp *ssp, const r
     return host_layout(n, ssp, tel).total;
 }
 
-rubix_status rubix_forward_host(const rubix_particles *hp, const rubix_ssp *hs, const rubix_telescope *tel,
-                                const float *R, float *h_cube, void *scratch, size_t scratch_bytes,
-                                void *stream)
+namespace {
+// State of the pipelined end-to-end entry: the device->host copy of call i runs on an internal copy stream while
+// call i + 1 computes on the caller's stream; two device buffers take the final cube in turn.
+struct Pipe {
+    cudaStream_t copy = nullptr;
+    cudaEvent_t ready[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+    bool used[2] = {false, false};
+    int next = 0;
+};
+Pipe g_pipe;
+std::mutex g_pipe_mu;
+
+cudaError_t pipe_init()
+{
+    if (g_pipe.copy) return cudaSuccess;
+    cudaError_t e = cudaStreamCreateWithFlags(&g_pipe.copy, cudaStreamNonBlocking);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&g_pipe.ready[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_pipe.copied[i], cudaEventDisableTiming);
+    }
+    return e;
+}
+
+rubix_status forward_host_impl(const rubix_particles *hp, const rubix_ssp *hs, const rubix_telescope *tel,
+                               const float *R, float *h_cube, void *scratch, size_t scratch_bytes, void *stream,
+                               bool pipelined)
 {
     t_err[0] = 0;
     rubix_status s;
@@ -438,7 +461,9 @@ rubix_status rubix_forward_host(const rubix_particles *hp, const rubix_ssp *hs, 
     if ((s = check_tel(tel)) != RUBIX_OK) return s;
     if (!R || !h_cube) return fail(RUBIX_ERR_NULL, "R or h_cube is NULL");
     const HostLayout H = host_layout(hp->n, hs, tel);
-    if ((s = check_ws(scratch, scratch_bytes, H.total)) != RUBIX_OK) return s;
+    const size_t cube_bytes = (size_t)tel->n_x * tel->n_y * tel->n_channels * 4;
+    const size_t extra = pipelined ? align_up(cube_bytes, 256) : 0;      // the second final-cube buffer, at the end
+    if ((s = check_ws(scratch, scratch_bytes, H.total + extra)) != RUBIX_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     char *d = (char *)scratch;
     const size_t n = (size_t)hp->n;
@@ -457,21 +482,77 @@ rubix_status rubix_forward_host(const rubix_particles *hp, const rubix_ssp *hs, 
                        (const float *)(d + H.age), (const float *)(d + H.z)};
     rubix_ssp ds = *hs;
     ds.flux = (const float *)(d + H.flux);
-    const size_t ws_bytes = scratch_bytes - H.ws;
-    s = rubix_build_cube(&dp, &ds, tel, R, (float *)(d + H.cube), d + H.ws, ws_bytes, stream);
+    const size_t ws_bytes = H.total - H.ws;
+    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
+    // the buffer that takes the final cube of this call
+    int slot = 0;
+    float *final_cube = (float *)(d + (conv ? H.cube2 : H.cube));
+    std::unique_lock<std::mutex> lk(g_pipe_mu, std::defer_lock);
+    if (pipelined) {
+        lk.lock();
+        if ((e = pipe_init()) != cudaSuccess) return cuda_fail(e, "pipeline set-up");
+        slot = g_pipe.next;
+        g_pipe.next ^= 1;
+        if (slot == 1) final_cube = (float *)(d + H.total);
+        // the copy of the call before last read this buffer: it must have finished before we overwrite it
+        if (g_pipe.used[slot] && (e = cudaStreamWaitEvent(st, g_pipe.copied[slot], 0)) != cudaSuccess)
+            return cuda_fail(e, "pipeline wait");
+    }
+    float *raw = conv ? (float *)(d + H.cube) : final_cube;
+    s = rubix_build_cube(&dp, &ds, tel, R, raw, d + H.ws, ws_bytes, stream);
     if (s != RUBIX_OK) return s;
     int launches = g_launches;
-    float *final_cube = (float *)(d + H.cube);
-    if (tel->psf_size > 0 || tel->lsf_size > 0) {
-        s = rubix_convolve_psf_lsf(tel, (const float *)(d + H.cube), (float *)(d + H.cube2), d + H.ws, ws_bytes, stream);
+    if (conv) {
+        s = rubix_convolve_psf_lsf(tel, raw, final_cube, d + H.ws, ws_bytes, stream);
         if (s != RUBIX_OK) return s;
         launches += g_launches;
-        final_cube = (float *)(d + H.cube2);
     }
     g_launches = launches;
-    e = cudaMemcpyAsync(h_cube, final_cube, (size_t)tel->n_x * tel->n_y * tel->n_channels * 4,
-                        cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return cuda_fail(e, "device->host copy");
+    if (!pipelined) {
+        e = cudaMemcpyAsync(h_cube, final_cube, cube_bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(e, "device->host copy");
+        return RUBIX_OK;
+    }
+    if ((e = cudaEventRecord(g_pipe.ready[slot], st)) != cudaSuccess) return cuda_fail(e, "pipeline record");
+    if ((e = cudaStreamWaitEvent(g_pipe.copy, g_pipe.ready[slot], 0)) != cudaSuccess) return cuda_fail(e, "pipeline wait");
+    if ((e = cudaMemcpyAsync(h_cube, final_cube, cube_bytes, cudaMemcpyDeviceToHost, g_pipe.copy)) != cudaSuccess)
+        return cuda_fail(e, "device->host copy");
+    if ((e = cudaEventRecord(g_pipe.copied[slot], g_pipe.copy)) != cudaSuccess) return cuda_fail(e, "pipeline record");
+    g_pipe.used[slot] = true;
+    return RUBIX_OK;
+}
+}  // namespace
+
+rubix_status rubix_forward_host(const rubix_particles *hp, const rubix_ssp *hs, const rubix_telescope *tel,
+                                const float *R, float *h_cube, void *scratch, size_t scratch_bytes,
+                                void *stream)
+{
+    return forward_host_impl(hp, hs, tel, R, h_cube, scratch, scratch_bytes, stream, false);
+}
+
+size_t rubix_forward_host_pipelined_scratch_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
+{
+    const size_t base = rubix_forward_host_scratch_bytes(n, ssp, tel);
+    if (base == 0) return 0;
+    return base + align_up((size_t)tel->n_x * tel->n_y * tel->n_channels * 4, 256);
+}
+
+rubix_status rubix_forward_host_pipelined(const rubix_particles *hp, const rubix_ssp *hs, const rubix_telescope *tel,
+                                          const float *R, float *h_cube, void *scratch, size_t scratch_bytes,
+                                          void *stream)
+{
+    return forward_host_impl(hp, hs, tel, R, h_cube, scratch, scratch_bytes, stream, true);
+}
+
+rubix_status rubix_forward_host_drain(void *stream)
+{
+    t_err[0] = 0;
+    std::lock_guard<std::mutex> lk(g_pipe_mu);
+    for (int i = 0; i < 2; ++i)
+        if (g_pipe.used[i]) {
+            cudaError_t e = cudaStreamWaitEvent((cudaStream_t)stream, g_pipe.copied[i], 0);
+            if (e != cudaSuccess) return cuda_fail(e, "pipeline drain");
+        }
     return RUBIX_OK;
 }
 

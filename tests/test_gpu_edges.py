@@ -180,3 +180,33 @@ def test_calls_can_be_captured_in_a_cuda_graph(B):
         g.replay()
         torch.cuda.synchronize()
         assert torch.equal(final, ref)
+
+
+def test_pipelined_forward_host_matches_the_plain_call(B):
+    """Back-to-back cubes with the device->host copies on the internal copy stream: every cube equals the plain
+    end-to-end call's, also when host buffers alternate and when PSF/LSF is off (the raw buffer alternates)."""
+    for conv in (True, False):
+        w = synth.make_workload("tiny")
+        if conv:
+            w.telescope = w.telescope.with_psf_lsf()
+        p = w.particles
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hflux = pin(w.ssp.flux)
+        cs, ct = B.c_ssp(w.ssp, hflux), B.c_telescope(w.telescope)
+        shape = (w.telescope.n_x, w.telescope.n_y, w.telescope.n_channels)
+        scratch = torch.empty(B.rubix_forward_host_pipelined_scratch_bytes(p.n, cs, ct), dtype=torch.uint8, device="cuda")
+        outs, refs = [], []
+        for i in range(5):                                   # five galaxies differing by their masses
+            hp = [pin(x) for x in (p.pos, p.vel, p.mass * np.float32(1.0 + i), p.log_age, p.log_z)]
+            cp = B.c_particles(*hp)
+            ref = torch.empty(shape).pin_memory()
+            B.rubix_forward_host(cp, cs, ct, w.rotation, ref, scratch)
+            torch.cuda.synchronize()
+            refs.append(ref.clone())
+            outs.append((torch.empty(shape).pin_memory(), cp, hp))
+        for out, cp, _ in outs:
+            B.rubix_forward_host_pipelined(cp, cs, ct, w.rotation, out, scratch)
+        B.rubix_forward_host_drain()
+        torch.cuda.current_stream().synchronize()            # the caller's stream alone: drain made it wait for the copies
+        for (out, _, _), ref in zip(outs, refs):
+            assert torch.equal(out, ref)
