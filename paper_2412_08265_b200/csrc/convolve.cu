@@ -6,7 +6,8 @@
 // Fast path (psf_size <= 15, lsf_size <= 9, even n_channels): two "marching" kernels.  A thread
 // owns one channel pair of one line and walks along the stencil axis with a ring of 15 partial
 // sums in registers: every input is read exactly once (8-byte loads, 256 B contiguous per warp,
-// five steps prefetched), every output written exactly once, no shared memory.
+// five steps prefetched -- fifteen in the pass that fuses the LSF --), every output written exactly once, no shared
+// memory.
 //   pass 1  along y, with the LSF fused in: the 9 channel taps come from the neighbouring lanes
 //           by warp shuffle (a warp covers 56 output channels plus 2 halo pairs on each side)
 //   pass 2  along x
@@ -101,20 +102,28 @@ __device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned 
     return o;
 }
 
-#ifndef RUBIX_MARCH_PF
-#define RUBIX_MARCH_PF 5
+// steps prefetched per thread (divides 15) and resident CTAs per SM, for the pass with the fused LSF (1) and
+// for the plain passes (0)
+#ifndef RUBIX_MARCH_PF1
+#define RUBIX_MARCH_PF1 15
 #endif
-#ifndef RUBIX_MARCH_MINB
-#define RUBIX_MARCH_MINB 4
+#ifndef RUBIX_MARCH_MINB1
+#define RUBIX_MARCH_MINB1 3
 #endif
-constexpr int kMarchPf = RUBIX_MARCH_PF;          // steps prefetched per thread (divides 15)
+#ifndef RUBIX_MARCH_PF0
+#define RUBIX_MARCH_PF0 5
+#endif
+#ifndef RUBIX_MARCH_MINB0
+#define RUBIX_MARCH_MINB0 4
+#endif
 
 // VAR: the stencil along the marching axis differs per channel (wavelength-dependent PSF, reading R18): the
 // thread loads the 15 taps of its two channels once; they then live in registers (two resident CTAs per SM).
 template <bool LSF, bool VAR = false>
-__global__ void __launch_bounds__(256, VAR ? 2 : RUBIX_MARCH_MINB)
+__global__ void __launch_bounds__(256, VAR ? 2 : (LSF ? RUBIX_MARCH_MINB1 : RUBIX_MARCH_MINB0))
 k_march(const __grid_constant__ MarchParams P)
 {
+    constexpr int kMarchPf = LSF ? RUBIX_MARCH_PF1 : RUBIX_MARCH_PF0;
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * 256 + threadIdx.x) >> 5;
     const int line = (int)(gw / P.cblocks), cblock = (int)(gw % P.cblocks);
