@@ -78,7 +78,10 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     // so that the bilinear combinations below never subtract two large sums (the D_c of the header
     // are P0, P0 + Pa, P0 + Pz, P0 + Pa + Pz + Pq).  fp32 partial sums over kAdjBlock channels are
     // flushed into fp64 running sums.
-    constexpr int kAdjBlock = 4;
+#ifndef RUBIX_ADJ_BLOCK
+#define RUBIX_ADJ_BLOCK 4
+#endif
+    constexpr int kAdjBlock = RUBIX_ADJ_BLOCK;
     double P0 = 0, Pa = 0, Pz = 0, Pq = 0, E = 0;
     const int jmax = P.n_lambda - 2;
     const int64_t step = (int64_t)r.b_fx << 5;
