@@ -9,6 +9,8 @@
 //   dL/dm = sum_c w_c D_c ;  dL/dlogA = m sum_c (dw_c/dta) D_c / (A[i+1]-A[i]) (0 if clamped) ;
 //   dL/dlogZ likewise ;  dL/dv_los = -m E / (dl_ssp c (1+beta)^2).
 // x_k uses the same fixed-point integers as the forward kernel (Rec.a_fx, Rec.b_fx).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace rubix {
@@ -296,6 +298,360 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// k_adjoint_units: the fast path of step 9 for the point-sampled rule on uniform grids.
+// Same work decomposition as the forward kernel (one CTA per unit = up to kChunk consecutive sorted
+// particles of ONE spaxel), with the resampling TRANSPOSED onto the SSP sample grid so that the
+// four corner rows are read exactly like k_accumulate reads them: 16-byte, line-aligned, coalesced.
+//   G' row      the unit's spaxel row of G' is staged in shared memory once per CTA;
+//   per particle (one warp each), per pass of 128 samples, lane l owns the sample quad
+//               j0 .. j0+3 (one 16-byte load per corner) and the channels whose rest position
+//               x_k = A + B k falls into [j0, j0+4).  Per knot interval i of the quad it forms
+//                   sigma_i = sum g_k,   beta_i = sum g_k frac(x_k)        (k with floor(x_k) = j0 + i)
+//               from which  W_j = (sigma_j - beta_j) + beta_{j-1}   (the transposed hat weights) and
+//               gamma_i = sum g_k (x_k + l0_ssp/dl_ssp) = (j0 + i + l0_ssp/dl_ssp) sigma_i + beta_i, and adds
+//                   P0 += W_j T_0[j], Pa += W_j (T_1 - T_0)[j], Pz += W_j (T_2 - T_0)[j],
+//                   Pq += W_j (T_3 - T_2 - T_1 + T_0)[j]             (difference basis: the template
+//                                                                     differences are exact in fp32)
+//                   Q_c += gamma_i (T_c[i+1] - T_c[i])               (slope term of d/dv_los)
+//               fp32 inside a quad, fp64 across passes; fp64 warp-shuffle reduction at the end.
+//   x_k         is evaluated here from v_los in 20.44 fixed point (A and B rounded to 2^-44 samples),
+//               i.e. to 1e-10 samples of the oracle's fp64 value over 3700 channels: the derivative in
+//               v_los jumps where some x_k crosses a knot, and a particle is compared with the oracle
+//               only if its clearance from every knot exceeds that resolution (tests, R19).
+// Each interval holds between NA and NA + NB channels (NA = floor(1/B_max), NA + NB = ceil(1/B_min) over
+// the velocity cap); the first NA are consumed unconditionally (the staged row is zero padded on both
+// sides, so virtual channels outside [0, N_c) contribute nothing), the next NB under a predicate.
+// ------------------------------------------------------------------------------------------
+#ifndef RUBIX_ADJU_MINB
+#define RUBIX_ADJU_MINB 5
+#endif
+constexpr int kAdjUThreads = 128;
+constexpr int kAdjUWarps = kAdjUThreads / 32;
+constexpr int kAdjUSplit = 4;               // CTAs per unit: each takes kChunk / kAdjUSplit particles (finer tail)
+constexpr int kAdjUFront = 160;             // zero floats in front of the staged G' row (B >= 0.25: k >= -32/B - 2)
+constexpr int kAdjUBack = 544;              // and behind it (a pass overshoots the last channel by < 128/B + 8)
+constexpr int kAdjUFrac = 44;               // fractional bits of x_k in this kernel
+constexpr int kAdjUFlush = 4;               // passes accumulated in fp32 before the fp64 flush
+
+struct AdjUParams {
+    AxisParams ax;
+    const int32_t *perm, *totals, *seg_off;
+    const Unit *units;
+    const Rec *rec;
+    const float *vlos, *mass, *log_age, *log_z, *flux, *gconv;
+    float *g_mass, *g_age, *g_z, *g_v;
+    int32_t n_lambda, pitch, n_z, n_c, n_s;
+    double l0_obs, dl_obs, l0_ssp, dl_ssp;      // observed grid already divided by (1 + z)
+    float flux_scale;
+    int64_t n;
+};
+
+struct AdjQuad { unsigned long long lo, hi; };              // four consecutive samples as two packed pairs
+__device__ __forceinline__ AdjQuad adj_ldg_quad(const float *p)
+{
+    AdjQuad q;
+    asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+    return q;
+}
+__device__ __forceinline__ uint32_t adj_and_or(uint32_t a, uint32_t b, uint32_t c)   // (a & b) | c in one LOP3
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
+struct AdjCorners {                                         // one pass of one lane: 4 corners x 4 samples (+ the fifth)
+    AdjQuad c[4];
+    float e[4];                                             // lane 31 only: first sample of the next 128-sample block
+};
+
+// Per-particle state of one lane across the passes of k_adjoint_units.
+struct AdjLane {
+    int k;                                                  // first channel at or above the lane's first knot
+    uint32_t d_lo, d_hi;                                    // x_k - j0 in 2^-44 samples, in [0, B)
+    uint32_t b_lo, b_hi;                                    // B
+    float bf;                                               // B as a float (fraction of the second channel of an interval)
+    float xb;                                               // j0 + l0_ssp/dl_ssp - 1
+    float beta_carry;                                       // beta of lane 31's last interval in the previous pass
+    unsigned long long p0, pa, pz, pq;                      // packed (even j, odd j) partial sums
+    float q0, q1, q2, q3;
+};
+
+__device__ __forceinline__ void adj_add64(uint32_t &lo, uint32_t &hi, uint32_t blo, uint32_t bhi)
+{
+    asm("add.cc.u32 %0, %0, %2;\n\taddc.u32 %1, %1, %3;" : "+r"(lo), "+r"(hi) : "r"(blo), "r"(bhi));
+}
+
+// One pass (one sample quad per lane) of one particle.  sg_bytes: byte address (shared window) of sg[0].
+template <int NA, int NB, bool MASK>
+__device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32_t sg_addr, int lane, int lim)
+{
+    // ---- channels of the quad, interval by interval: sigma_i = sum g, b1_i = sum g (1 + frac)
+    uint32_t addr = sg_addr + ((uint32_t)L.k << 2);
+    uint32_t lo = L.d_lo, hi = L.d_hi;
+    float sig[4], b1[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        float s = 0.0f, b = 0.0f, f1 = 1.0f;
+        const uint32_t bound = (uint32_t)(i + 1) << (kAdjUFrac - 32);
+#pragma unroll
+        for (int st = 0; st < NA + NB; ++st) {
+            const bool take = st < NA || hi < bound;
+            if (take) {
+                float gk;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(gk) : "r"(addr));
+                if (st == 0)                                // fraction from the top 23 bits below the binary point
+                    f1 = __uint_as_float(adj_and_or(__funnelshift_r(lo, hi, kAdjUFrac - 23), 0x7FFFFFu, 0x3F800000u));
+                else
+                    f1 += L.bf;                             // same interval: the next channel sits B further on
+                s = st == 0 ? gk : s + gk;
+                b = st == 0 ? gk * f1 : fmaf(gk, f1, b);
+                adj_add64(lo, hi, L.b_lo, L.b_hi);
+                addr += 4;
+            }
+        }
+        // intervals at or beyond the last knot carry no flux (x_k = N_l - 1 exactly: handled by the caller)
+        const bool in_cov = !MASK || i < lim;
+        sig[i] = in_cov ? s : 0.0f;
+        b1[i] = in_cov ? b : 0.0f;
+    }
+    // ---- W_j = (sigma_j - beta_j) + beta_{j-1}, beta = b1 - sigma;  gamma_i = (x_i + l0/dl) sigma_i + beta_i
+    const float bet0 = b1[0] - sig[0], bet1 = b1[1] - sig[1], bet2 = b1[2] - sig[2], bet3 = b1[3] - sig[3];
+    float b_prev = __shfl_up_sync(0xffffffffu, bet3, 1);
+    if (lane == 0) b_prev = L.beta_carry;
+    L.beta_carry = __shfl_sync(0xffffffffu, bet3, 31);
+    const float w0 = fmaf(2.0f, sig[0], -b1[0]) + b_prev, w1 = fmaf(2.0f, sig[1], -b1[1]) + bet0;
+    const float w2 = fmaf(2.0f, sig[2], -b1[2]) + bet1, w3 = fmaf(2.0f, sig[3], -b1[3]) + bet2;
+    const float gm0 = fmaf(L.xb, sig[0], b1[0]), gm1 = fmaf(L.xb + 1.0f, sig[1], b1[1]);
+    const float gm2 = fmaf(L.xb + 2.0f, sig[2], b1[2]), gm3 = fmaf(L.xb + 3.0f, sig[3], b1[3]);
+    // ---- P sums, two samples per instruction (difference basis; the template differences are exact)
+    {
+        const unsigned long long neg1 = pack2(-1.0f, -1.0f);
+        const unsigned long long wl = pack2(w0, w1), wh = pack2(w2, w3);
+        const unsigned long long dal = ffma2(C.c[0].lo, neg1, C.c[1].lo), dah = ffma2(C.c[0].hi, neg1, C.c[1].hi);
+        const unsigned long long dzl = ffma2(C.c[0].lo, neg1, C.c[2].lo), dzh = ffma2(C.c[0].hi, neg1, C.c[2].hi);
+        const unsigned long long dql = ffma2(dal, neg1, ffma2(C.c[2].lo, neg1, C.c[3].lo));
+        const unsigned long long dqh = ffma2(dah, neg1, ffma2(C.c[2].hi, neg1, C.c[3].hi));
+        L.p0 = ffma2(wh, C.c[0].hi, ffma2(wl, C.c[0].lo, L.p0));
+        L.pa = ffma2(wh, dah, ffma2(wl, dal, L.pa));
+        L.pz = ffma2(wh, dzh, ffma2(wl, dzl, L.pz));
+        L.pq = ffma2(wh, dqh, ffma2(wl, dql, L.pq));
+    }
+    // ---- slope sums: gamma_i (T_c[i+1] - T_c[i]); the fifth sample comes from the next lane
+    {
+        float q[4] = {L.q0, L.q1, L.q2, L.q3};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float2 a = unpack2(C.c[c].lo), bq = unpack2(C.c[c].hi);
+            float nx = __shfl_down_sync(0xffffffffu, a.x, 1);
+            if (lane == 31) nx = C.e[c];
+            q[c] = fmaf(gm3, nx - bq.y, fmaf(gm2, bq.y - bq.x, fmaf(gm1, bq.x - a.y, fmaf(gm0, a.y - a.x, q[c]))));
+        }
+        L.q0 = q[0]; L.q1 = q[1]; L.q2 = q[2]; L.q3 = q[3];
+    }
+}
+
+template <int NA, int NB>
+__global__ void __launch_bounds__(kAdjUThreads, RUBIX_ADJU_MINB)
+k_adjoint_units(const __grid_constant__ AdjUParams P)
+{
+    extern __shared__ __align__(16) float sg_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_units = P.totals[0];
+    const int u = blockIdx.x / kAdjUSplit, part = blockIdx.x % kAdjUSplit;
+    if (u >= n_units) {
+        // spare CTAs of the (upper-bound) grid zero the gradients of the dropped particles
+        const int64_t first = P.seg_off[P.n_s];
+        const int64_t spare = (int64_t)gridDim.x - (int64_t)n_units * kAdjUSplit;
+        for (int64_t i = first + ((int64_t)blockIdx.x - (int64_t)n_units * kAdjUSplit) * kAdjUThreads + tid; i < P.n;
+             i += spare * kAdjUThreads) {
+            const int p = P.perm[i];
+            P.g_mass[p] = 0.0f; P.g_age[p] = 0.0f; P.g_z[p] = 0.0f; P.g_v[p] = 0.0f;
+        }
+        return;
+    }
+    const Unit U = P.units[u];
+    constexpr int kPer = kChunk / kAdjUSplit;
+    const int q_begin = part * kPer, q_end = min(U.count, q_begin + kPer);
+    if (q_begin >= q_end) return;
+    float *sg = sg_raw + kAdjUFront;                        // sg[k] = G'[spaxel][k], zeros outside [0, n_c)
+    {
+        const float *g = P.gconv + (size_t)U.spaxel * P.n_c;
+        for (int k = tid - kAdjUFront; k < P.n_c + kAdjUBack; k += kAdjUThreads)
+            sg[k] = (k >= 0 && k < P.n_c) ? __ldg(g + k) : 0.0f;
+    }
+    __syncthreads();
+    const uint32_t sg_addr = (uint32_t)__cvta_generic_to_shared(sg);
+    const int row_a = P.n_z * P.pitch, row_z = P.pitch;
+    const float x_off = (float)(P.l0_ssp / P.dl_ssp) - 1.0f; // lambda = (x + l0_ssp/dl_ssp) dl_ssp (1 + beta); -1: b1 carries 1 + frac
+    const int64_t x_top = (int64_t)(P.n_lambda - 1) << kAdjUFrac;
+    const double inv_dl_ssp = 1.0 / P.dl_ssp;
+
+    auto load = [&](AdjCorners &C, const float *t) {
+        C.c[0] = adj_ldg_quad(t); C.c[1] = adj_ldg_quad(t + row_a);
+        C.c[2] = adj_ldg_quad(t + row_z); C.c[3] = adj_ldg_quad(t + row_a + row_z);
+        if (lane == 31) {                                   // fifth sample of each corner: the next block's first
+            C.e[0] = __ldg(t + 4); C.e[1] = __ldg(t + row_a + 4);
+            C.e[2] = __ldg(t + row_z + 4); C.e[3] = __ldg(t + row_a + row_z + 4);
+        }
+    };
+    auto prefetch = [&](const float *t) {                   // the next pass's corner rows: L2 -> L1 while this pass is worked on
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(t));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(t + row_a));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(t + row_z));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(t + row_a + row_z));
+    };
+    // fp64 running sums of the thread live in shared memory (component-major: conflict-free), flushed every
+    // kAdjUFlush passes; keeps the register count low enough for five resident CTAs
+    double *acc = reinterpret_cast<double *>(sg_raw + ((P.n_c + kAdjUFront + kAdjUBack + 3) & ~3)) + tid;
+
+    for (int q = q_begin + warp; q < q_end; q += kAdjUWarps) {
+        const int64_t i_sorted = (int64_t)U.start + q;
+        const int p = P.perm[i_sorted];
+        const float *T0 = P.flux + P.rec[i_sorted].cell;
+        const double opb = 1.0 + (double)P.vlos[p] / kCkms;
+        const double inv = 1.0 / opb;
+        const double scale = (double)((int64_t)1 << kAdjUFrac);
+        const int64_t a44 = __double2ll_rn((P.l0_obs * inv - P.l0_ssp) * inv_dl_ssp * scale);
+        const int64_t b44 = __double2ll_rn(P.dl_obs * inv * inv_dl_ssp * scale);
+        const int64_t x_first = a44, x_last = a44 + (int64_t)(P.n_c - 1) * b44;
+        const int64_t x_lo = max(x_first, (int64_t)0), x_hi = min(x_last, x_top);
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[c * kAdjUThreads] = 0.0;
+        if (x_lo <= x_hi) {
+            const int j_begin = (int)(x_lo >> kAdjUFrac) & ~(kRowAlign - 1);
+            const int j_last = (int)(x_hi >> kAdjUFrac);
+            // channels per 128 samples: kstep = floor(128 / B); a pass moves the lane's first channel by kstep or
+            // kstep + 1, decided in exact integers: delta = kstep B - 128 in (-B, 0]
+            const double inv_b = 1.0 / (double)b44;
+            const int64_t span = (int64_t)128 << kAdjUFrac;
+            int kstep = (int)((double)span * inv_b);
+            int64_t delta = (int64_t)kstep * b44 - span;
+            if (delta > 0) { delta -= b44; --kstep; }
+            if (delta <= -b44) { delta += b44; ++kstep; }
+            // first channel at or above the lane's first knot: estimate in fp64, settle in exact integers
+            int j0 = j_begin + 4 * lane;
+            AdjLane L;
+            int64_t d;
+            {
+                const int64_t J0 = (int64_t)j0 << kAdjUFrac;
+                L.k = (int)ceil((double)(J0 - a44) * inv_b);
+                int64_t X = a44 + (int64_t)L.k * b44;
+                if (X - b44 >= J0) { X -= b44; --L.k; }
+                if (X < J0) { X += b44; ++L.k; }
+                d = X - J0;
+            }
+            L.b_lo = (uint32_t)b44; L.b_hi = (uint32_t)(b44 >> 32);
+            L.bf = (float)((double)b44 * (1.0 / scale));
+            L.xb = x_off + (float)j0;
+            L.beta_carry = 0.0f;
+            L.p0 = L.pa = L.pz = L.pq = 0ull;
+            L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
+            const float *t = T0 + j0;
+            int n_acc = 0;
+            auto flush = [&]() {
+                const float2 f0 = unpack2(L.p0), fa = unpack2(L.pa), fz = unpack2(L.pz), fq = unpack2(L.pq);
+                acc[0 * kAdjUThreads] += (double)(f0.x + f0.y); acc[1 * kAdjUThreads] += (double)(fa.x + fa.y);
+                acc[2 * kAdjUThreads] += (double)(fz.x + fz.y); acc[3 * kAdjUThreads] += (double)(fq.x + fq.y);
+                acc[4 * kAdjUThreads] += (double)L.q0; acc[5 * kAdjUThreads] += (double)L.q1;
+                acc[6 * kAdjUThreads] += (double)L.q2; acc[7 * kAdjUThreads] += (double)L.q3;
+                L.p0 = L.pa = L.pz = L.pq = 0ull;
+                L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
+                n_acc = 0;
+            };
+            auto advance = [&]() {                          // next pass: 128 samples on
+                d += delta;
+                L.k += kstep;
+                if (d < 0) { d += b44; ++L.k; }
+                j0 += 128; t += 128; L.xb += 128.0f;
+                if (++n_acc == kAdjUFlush) flush();
+            };
+            const int j_main = min(j_last, P.n_lambda - 1 - 128);   // passes starting above this touch the last knot
+            int jp = j_begin;
+            AdjCorners A;
+            A.e[0] = A.e[1] = A.e[2] = A.e[3] = 0.0f;
+            for (; jp <= j_main; jp += 128) {
+                load(A, t);
+                prefetch(t + 128);
+                L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
+                adj_pass<NA, NB, false>(A, L, sg_addr, lane, 0);
+                advance();
+            }
+            for (; jp <= j_last; jp += 128) {               // passes that touch the last knot
+                load(A, t);
+                L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
+                adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0);
+                advance();
+            }
+            flush();
+        }
+        double P0 = acc[0 * kAdjUThreads], Pa = acc[1 * kAdjUThreads], Pz = acc[2 * kAdjUThreads], Pq = acc[3 * kAdjUThreads];
+        double Q0 = acc[4 * kAdjUThreads], Q1 = acc[5 * kAdjUThreads], Q2 = acc[6 * kAdjUThreads], Q3 = acc[7 * kAdjUThreads];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            P0 += __shfl_xor_sync(0xffffffffu, P0, o);
+            Pa += __shfl_xor_sync(0xffffffffu, Pa, o);
+            Pz += __shfl_xor_sync(0xffffffffu, Pz, o);
+            Pq += __shfl_xor_sync(0xffffffffu, Pq, o);
+            Q0 += __shfl_xor_sync(0xffffffffu, Q0, o);
+            Q1 += __shfl_xor_sync(0xffffffffu, Q1, o);
+            Q2 += __shfl_xor_sync(0xffffffffu, Q2, o);
+            Q3 += __shfl_xor_sync(0xffffffffu, Q3, o);
+        }
+        if (lane == 0) {
+            int ia, iz;
+            double ta, tz, wa, wz;
+            bool a_free, z_free;
+            adj_axis_cell(P.ax.age, P.ax.n_age, P.log_age[p], &ia, &ta, &wa, &a_free);
+            adj_axis_cell(P.ax.z, P.ax.n_z, P.log_z[p], &iz, &tz, &wz, &z_free);
+            // a channel sitting exactly on the last knot (x_k = N_l - 1) takes the last sample with weight 1,
+            // as the forward kernel does; its slope term is left out (the spectrum ends there)
+            if (x_last >= x_top && x_first <= x_top && (x_top - a44) % b44 == 0) {
+                const int64_t kh = (x_top - a44) / b44;
+                const float gk = sg[kh];
+                const float *tl = T0 + (P.n_lambda - 1);
+                const float t0 = tl[0], t1 = tl[row_a], t2 = tl[row_z], t3 = tl[row_a + row_z];
+                P0 += (double)gk * t0;
+                Pa += (double)gk * ((double)t1 - t0);
+                Pz += (double)gk * ((double)t2 - t0);
+                Pq += (double)gk * (((double)t3 - t2) - ((double)t1 - t0));
+            }
+            const double m = (double)P.mass[p] * (double)P.flux_scale;
+            const double E = (1.0 - ta) * (1.0 - tz) * Q0 + ta * (1.0 - tz) * Q1 + (1.0 - ta) * tz * Q2 + ta * tz * Q3;
+            P.g_mass[p] = (float)((double)P.flux_scale * (P0 + ta * Pa + tz * Pz + ta * tz * Pq));
+            P.g_age[p] = a_free ? (float)(m * (Pa + tz * Pq) / wa) : 0.0f;
+            P.g_z[p] = z_free ? (float)(m * (Pz + ta * Pq) / wz) : 0.0f;
+            P.g_v[p] = (float)(-m * E / (kCkms * opb));
+        }
+    }
+}
+
+template <int NA, int NB>
+static cudaError_t launch_adjoint_units(const AdjUParams &P, unsigned grid, size_t smem, cudaStream_t st)
+{
+    auto kern = k_adjoint_units<NA, NB>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kAdjUThreads, smem, st>>>(P);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
+// Channels per knot interval over the velocity cap: at least NA, at most NA + NB.  Returns false when the
+// sampling ratio is outside what k_adjoint_units is instantiated for (the warp-per-particle kernel takes over).
+static bool adjoint_units_shape(const PassInputs &in, int *na, int *nb)
+{
+    if (table_mode(in.ssp, in.tel) || in.tel->resample != RUBIX_RESAMPLE_POINT) return false;
+    const double b0 = (double)in.tel->dlambda / ((1.0 + (double)in.tel->redshift) * (double)in.ssp->dlambda);
+    const double b_lo = b0 / (1.0 + kBetaCap) * (1.0 - 1e-6), b_hi = b0 / (1.0 - kBetaCap) * (1.0 + 1e-6);
+    if (!(b_lo >= 0.26) || !(b_hi < 3.0)) return false;
+    const int n_min = (int)floor(1.0 / b_hi), n_max = (int)ceil(1.0 / b_lo);
+    *na = n_min;
+    *nb = n_max - n_min;
+    return *na >= 0 && *na <= 3 && *nb >= 1 && *nb <= 2;
+}
+
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st)
 {
@@ -318,6 +674,42 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.log_grid = in.ssp->log_lambda;
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
+    int na = 0, nb = 0;
+    if (adjoint_units_shape(in, &na, &nb)) {
+        AdjUParams Q;
+        Q.ax = P.ax;
+        Q.perm = (const int32_t *)(ws + L.off_permbuf[L.final_buf]);
+        Q.totals = (const int32_t *)(ws + L.off_totals);
+        Q.seg_off = (const int32_t *)(ws + L.off_seg);
+        Q.units = (const Unit *)(ws + L.off_units);
+        Q.rec = (const Rec *)(ws + L.off_rec);
+        Q.vlos = (const float *)(ws + L.off_vlos);
+        Q.mass = in.p->mass; Q.log_age = in.p->log_age; Q.log_z = in.p->log_z;
+        Q.flux = (const float *)(ws + L.off_flux);
+        Q.gconv = gconv;
+        Q.g_mass = g_mass; Q.g_age = g_age; Q.g_z = g_z; Q.g_v = g_v;
+        Q.n_lambda = in.ssp->n_lambda; Q.pitch = L.pitch; Q.n_z = in.ssp->n_z; Q.n_c = L.n_c; Q.n_s = L.n_s;
+        const double zp1 = 1.0 + (double)in.tel->redshift;
+        Q.l0_obs = (double)in.tel->lambda0 / zp1;
+        Q.dl_obs = (double)in.tel->dlambda / zp1;
+        Q.l0_ssp = (double)in.ssp->lambda0;
+        Q.dl_ssp = (double)in.ssp->dlambda;
+        Q.flux_scale = in.tel->flux_scale;
+        Q.n = L.n;
+        const size_t smem = (size_t)(((size_t)L.n_c + kAdjUFront + kAdjUBack + 3) & ~(size_t)3) * sizeof(float) +
+                            (size_t)8 * kAdjUThreads * sizeof(double);
+        const unsigned grid = (unsigned)(L.max_units * kAdjUSplit);
+        switch (na * 2 + (nb - 1)) {
+            case 0: return launch_adjoint_units<0, 1>(Q, grid, smem, st);
+            case 1: return launch_adjoint_units<0, 2>(Q, grid, smem, st);
+            case 2: return launch_adjoint_units<1, 1>(Q, grid, smem, st);
+            case 3: return launch_adjoint_units<1, 2>(Q, grid, smem, st);
+            case 4: return launch_adjoint_units<2, 1>(Q, grid, smem, st);
+            case 5: return launch_adjoint_units<2, 2>(Q, grid, smem, st);
+            case 6: return launch_adjoint_units<3, 1>(Q, grid, smem, st);
+            default: return launch_adjoint_units<3, 2>(Q, grid, smem, st);
+        }
+    }
     const int64_t threads = L.n * 32;
     auto kern = in.tel->resample == RUBIX_RESAMPLE_FLUX ? k_adjoint_flux
                                                         : (table_mode(in.ssp, in.tel) ? k_adjoint<true> : k_adjoint<false>);

@@ -136,3 +136,94 @@ def test_sort_equals_stable_argsort(n, n_s):
     assert np.array_equal(np.diff(seg), np.bincount(key, minlength=n_s + 1))
     for s in np.unique(key)[:20]:
         assert np.all(np.diff(perm[seg[s]:seg[s + 1]]) > 0)                 # ties by original index
+
+
+# ---------------------------------------------------------------- fp32 operation order (8c-2)
+# SURVEY.md 8(c)-2 / DESIGN.md R2 DEFINE the binning in fp32: every * and + separately rounded, in the order
+#   xr = (R00*x + R01*y) + R02*z ;  hx = (0.5f*N_x)*s ;  u = (xr + hx) / s
+# (hx needs no case of its own: multiplying by 0.5 is exact, so every association of 0.5f, N_x and s agrees.)
+# The cases below are built so that a different association, an FMA contraction or a re-arranged
+# division moves u across a spaxel edge.  Expected keys: derived by hand (literal values, derivation in
+# the comments) or evaluated with numpy.float32 ops, which round after every operation.
+F = np.float32
+
+
+def _key_in_order(pos, R, n_x, n_y, s, variant="spec"):
+    """numpy.float32 evaluation (one rounding per op).  variant 'spec' is the order of 8(c)-2;
+    the others are the plausible mistakes the cases must tell apart from it."""
+    pos = np.asarray(pos, F)
+    R = np.asarray(R, F).reshape(3, 3)
+    s = F(s)
+    x, y, z = pos[:, 0], pos[:, 1], pos[:, 2]
+
+    def coord(r, n):
+        a, b, c = r[0] * x, r[1] * y, r[2] * z                 # three separately rounded products
+        if variant == "assoc_right":
+            rot = a + (b + c)
+        elif variant == "fma":                                  # fma(r0, x, r1*y): the first product unrounded
+            rot = (r[0].astype(np.float64) * x.astype(np.float64) + b.astype(np.float64)).astype(F) + c
+        else:
+            rot = (a + b) + c
+        h = (F(0.5) * F(n)) * s
+        if variant == "div_split":
+            return rot / s + h / s
+        return (rot + h) / s
+
+    u, v = coord(R[0], n_x), coord(R[1], n_y)
+    assert u.dtype == np.float32
+    inside = (u >= 0) & (u < n_x) & (v >= 0) & (v < n_y)
+    with np.errstate(invalid="ignore"):
+        return np.where(inside, np.floor(u).astype(np.int64) * n_y + np.floor(v).astype(np.int64), n_x * n_y)
+
+
+def test_association_order_hand_built():
+    """R00*x = 1, R01*y = R02*z = 2^-24.  (1 + 2^-24) is a tie and rounds to the even 1, and again
+    1 + 2^-24 -> 1, so the specified order gives xr = 1; a + (b + c) gives 1 + 2^-23.
+    With s = 1 + 2^-23 and N_x = 2: hx = s; spec: 1 + s = 2 + 2^-23 is a tie -> 2.0, u = 2/s < 2 -> ix = 1;
+    other order: (1 + 2^-23) + s = 2 + 2^-22 exactly, u = 2 = N_x -> outside."""
+    s = F(1.0) + F(2.0 ** -23)
+    R = np.array([[0.5, 2.0 ** -10, 2.0 ** -12], [0.0, 0.0, 0.0], [0.0, 0.0, 1.0]], F)
+    pos = np.array([[2.0, 2.0 ** -14, 2.0 ** -12]], F)          # products: 1, 2^-24, 2^-24 (all exact)
+    key, _ = oracle.rotate_bin(pos, np.zeros_like(pos), R, 2, 2, s)
+    # y' = 0 -> v = (0 + s)/s = 1 -> iy = 1;  ix = 1  =>  key = 1*2 + 1
+    assert key.tolist() == [3]
+    assert _key_in_order(pos, R, 2, 2, s, "spec").tolist() == [3]
+    assert _key_in_order(pos, R, 2, 2, s, "assoc_right").tolist() == [4]      # the mistake is visible
+
+
+def test_fma_contraction_hand_built():
+    """R00 = 1 + 2^-12, x = 4097: the exact product 4098 + 2^-12 is a tie in fp32 (spacing 2^-11) and
+    rounds to the even 4098; R01*y = -4098.  Separately rounded: xr = 0; fma(R00, x, R01*y) = 2^-12.
+    s = 2^-12, N_x = 2: hx = 2^-12; spec: u = 2^-12/2^-12 = 1 -> ix = 1; contracted: u = 2 = N_x -> outside."""
+    s = F(2.0 ** -12)
+    R = np.array([[1.0 + 2.0 ** -12, -1.0, 0.0], [0.0, 0.0, 0.0], [0.0, 0.0, 1.0]], F)
+    pos = np.array([[4097.0, 4098.0, 0.0]], F)
+    key, _ = oracle.rotate_bin(pos, np.zeros_like(pos), R, 2, 2, s)
+    assert key.tolist() == [1 * 2 + 1]
+    assert _key_in_order(pos, R, 2, 2, s, "spec").tolist() == [3]
+    assert _key_in_order(pos, R, 2, 2, s, "fma").tolist() == [4]
+
+
+@pytest.mark.parametrize("euler,n_x,n_y,s", [((33.0, 71.0, 250.0), 25, 25, 1.2), (synth.random_euler(3002), 300, 300, 0.1),
+                                             ((10.0, 40.0, 70.0), 7, 5, 0.37)])
+def test_operation_order_on_edge_particles(euler, n_x, n_y, s):
+    """Particles placed within a few ulp of spaxel edges under a real rotation: the oracle must equal the
+    numpy.float32 evaluation in the specified order on ALL of them, and the set must contain particles
+    that each plausible mistake bins differently (otherwise it would prove nothing)."""
+    rng = np.random.default_rng(77)
+    R = synth.euler_rotation(*euler)
+    R64 = R.astype(np.float64)
+    n = 200_000
+    # pick a target edge coordinate in x', solve for the unrotated point, jitter by a few ulp
+    ex = rng.integers(0, n_x + 1, n).astype(np.float64)
+    ey = rng.uniform(0, n_y, n)
+    zz = rng.normal(0, 3.0, n)
+    target = np.stack([(ex - 0.5 * n_x) * s, (ey - 0.5 * n_y) * s, zz], 1)
+    pos = (target @ R64).astype(F)                              # r = R^T r'
+    pos = np.nextafter(pos, np.where(rng.random(pos.shape) < 0.5, -np.inf, np.inf).astype(F)).astype(F)
+    key, _ = oracle.rotate_bin(pos, np.zeros_like(pos), R, n_x, n_y, F(s))
+    spec = _key_in_order(pos, R, n_x, n_y, s, "spec")
+    assert np.array_equal(key, spec)
+    for variant in ("assoc_right", "fma", "div_split"):
+        other = _key_in_order(pos, R, n_x, n_y, s, variant)
+        assert (other != spec).sum() >= 20, variant           # the case set discriminates this mistake
