@@ -335,11 +335,11 @@ constexpr int kAdjUFrac = 44;               // fractional bits of x_k in this ke
 constexpr int kAdjUFlush = 4;               // passes accumulated in fp32 before the fp64 flush
 
 struct AdjUParams {
-    AxisParams ax;
     const int32_t *perm, *totals, *seg_off;
     const Unit *units;
     const Rec *rec;
-    const float *vlos, *mass, *log_age, *log_z, *flux, *gconv;
+    const AdjAux *aux;
+    const float *vlos, *mass, *flux, *gconv;
     float *g_mass, *g_age, *g_z, *g_v;
     int32_t n_lambda, pitch, n_z, n_c, n_s;
     double l0_obs, dl_obs, l0_ssp, dl_ssp;      // observed grid already divided by (1 + z)
@@ -478,8 +478,22 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
     float *sg = sg_raw + kAdjUFront;                        // sg[k] = G'[spaxel][k], zeros outside [0, n_c)
     {
         const float *g = P.gconv + (size_t)U.spaxel * P.n_c;
-        for (int k = tid - kAdjUFront; k < P.n_c + kAdjUBack; k += kAdjUThreads)
-            sg[k] = (k >= 0 && k < P.n_c) ? __ldg(g + k) : 0.0f;
+        for (int k = tid - kAdjUFront; k < 0; k += kAdjUThreads) sg[k] = 0.0f;
+        for (int k = P.n_c + tid; k < P.n_c + kAdjUBack; k += kAdjUThreads) sg[k] = 0.0f;
+        if ((P.n_c & 3) == 0 && ((uintptr_t)P.gconv & 15u) == 0) {      // kAdjUFront is a multiple of 4: 16-byte stores
+            const float4 *g4 = reinterpret_cast<const float4 *>(g);
+            float4 *s4 = reinterpret_cast<float4 *>(sg);
+            const int n4 = P.n_c >> 2;
+            int k = tid;
+            for (; k + 3 * kAdjUThreads < n4; k += 4 * kAdjUThreads) {  // four loads in flight per thread
+                const float4 v0 = __ldg(g4 + k), v1 = __ldg(g4 + k + kAdjUThreads);
+                const float4 v2 = __ldg(g4 + k + 2 * kAdjUThreads), v3 = __ldg(g4 + k + 3 * kAdjUThreads);
+                s4[k] = v0; s4[k + kAdjUThreads] = v1; s4[k + 2 * kAdjUThreads] = v2; s4[k + 3 * kAdjUThreads] = v3;
+            }
+            for (; k < n4; k += kAdjUThreads) s4[k] = __ldg(g4 + k);
+        } else {
+            for (int k = tid; k < P.n_c; k += kAdjUThreads) sg[k] = __ldg(g + k);
+        }
     }
     __syncthreads();
     const uint32_t sg_addr = (uint32_t)__cvta_generic_to_shared(sg);
@@ -586,25 +600,26 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
             }
             flush();
         }
-        double P0 = acc[0 * kAdjUThreads], Pa = acc[1 * kAdjUThreads], Pz = acc[2 * kAdjUThreads], Pq = acc[3 * kAdjUThreads];
-        double Q0 = acc[4 * kAdjUThreads], Q1 = acc[5 * kAdjUThreads], Q2 = acc[6 * kAdjUThreads], Q3 = acc[7 * kAdjUThreads];
+        // sum the 32 lanes' running sums: lane l adds component (l & 7) of lanes 8 (l >> 3) .. + 7 from shared
+        // memory, two shuffle rounds combine the four groups; fixed order, so the result is reproducible
+        __syncwarp();
+        double part = 0.0;
+        {
+            const double *col = acc - lane + (lane & 7) * kAdjUThreads + 8 * (lane >> 3);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            P0 += __shfl_xor_sync(0xffffffffu, P0, o);
-            Pa += __shfl_xor_sync(0xffffffffu, Pa, o);
-            Pz += __shfl_xor_sync(0xffffffffu, Pz, o);
-            Pq += __shfl_xor_sync(0xffffffffu, Pq, o);
-            Q0 += __shfl_xor_sync(0xffffffffu, Q0, o);
-            Q1 += __shfl_xor_sync(0xffffffffu, Q1, o);
-            Q2 += __shfl_xor_sync(0xffffffffu, Q2, o);
-            Q3 += __shfl_xor_sync(0xffffffffu, Q3, o);
+            for (int r = 0; r < 8; ++r) part += col[r];
         }
+        part += __shfl_xor_sync(0xffffffffu, part, 8);
+        part += __shfl_xor_sync(0xffffffffu, part, 16);
+        const double P0 = __shfl_sync(0xffffffffu, part, 0), Pa = __shfl_sync(0xffffffffu, part, 1);
+        const double Pz = __shfl_sync(0xffffffffu, part, 2), Pq = __shfl_sync(0xffffffffu, part, 3);
+        const double Q0 = __shfl_sync(0xffffffffu, part, 4), Q1 = __shfl_sync(0xffffffffu, part, 5);
+        const double Q2 = __shfl_sync(0xffffffffu, part, 6), Q3 = __shfl_sync(0xffffffffu, part, 7);
+        __syncwarp();
         if (lane == 0) {
-            int ia, iz;
-            double ta, tz, wa, wz;
-            bool a_free, z_free;
-            adj_axis_cell(P.ax.age, P.ax.n_age, P.log_age[p], &ia, &ta, &wa, &a_free);
-            adj_axis_cell(P.ax.z, P.ax.n_z, P.log_z[p], &iz, &tz, &wz, &z_free);
+            const AdjAux ax = P.aux[i_sorted];
+            const double ta = (double)ax.ta, tz = (double)ax.tz;
+            double p0 = P0, pa = Pa, pz = Pz, pq = Pq;
             // a channel sitting exactly on the last knot (x_k = N_l - 1) takes the last sample with weight 1,
             // as the forward kernel does; its slope term is left out (the spectrum ends there)
             if (x_last >= x_top && x_first <= x_top && (x_top - a44) % b44 == 0) {
@@ -612,17 +627,17 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 const float gk = sg[kh];
                 const float *tl = T0 + (P.n_lambda - 1);
                 const float t0 = tl[0], t1 = tl[row_a], t2 = tl[row_z], t3 = tl[row_a + row_z];
-                P0 += (double)gk * t0;
-                Pa += (double)gk * ((double)t1 - t0);
-                Pz += (double)gk * ((double)t2 - t0);
-                Pq += (double)gk * (((double)t3 - t2) - ((double)t1 - t0));
+                p0 += (double)gk * t0;
+                pa += (double)gk * ((double)t1 - t0);
+                pz += (double)gk * ((double)t2 - t0);
+                pq += (double)gk * (((double)t3 - t2) - ((double)t1 - t0));
             }
             const double m = (double)P.mass[p] * (double)P.flux_scale;
             const double E = (1.0 - ta) * (1.0 - tz) * Q0 + ta * (1.0 - tz) * Q1 + (1.0 - ta) * tz * Q2 + ta * tz * Q3;
-            P.g_mass[p] = (float)((double)P.flux_scale * (P0 + ta * Pa + tz * Pz + ta * tz * Pq));
-            P.g_age[p] = a_free ? (float)(m * (Pa + tz * Pq) / wa) : 0.0f;
-            P.g_z[p] = z_free ? (float)(m * (Pz + ta * Pq) / wz) : 0.0f;
-            P.g_v[p] = (float)(-m * E / (kCkms * opb));
+            P.g_mass[p] = (float)((double)P.flux_scale * (p0 + ta * pa + tz * pz + ta * tz * pq));
+            P.g_age[p] = (float)(m * (pa + tz * pq) * (double)ax.inv_wa);
+            P.g_z[p] = (float)(m * (pz + ta * pq) * (double)ax.inv_wz);
+            P.g_v[p] = (float)(-m * E * inv / kCkms);
         }
     }
 }
@@ -677,14 +692,14 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     int na = 0, nb = 0;
     if (adjoint_units_shape(in, &na, &nb)) {
         AdjUParams Q;
-        Q.ax = P.ax;
         Q.perm = (const int32_t *)(ws + L.off_permbuf[L.final_buf]);
         Q.totals = (const int32_t *)(ws + L.off_totals);
         Q.seg_off = (const int32_t *)(ws + L.off_seg);
         Q.units = (const Unit *)(ws + L.off_units);
         Q.rec = (const Rec *)(ws + L.off_rec);
+        Q.aux = (const AdjAux *)(ws + L.off_aux);
         Q.vlos = (const float *)(ws + L.off_vlos);
-        Q.mass = in.p->mass; Q.log_age = in.p->log_age; Q.log_z = in.p->log_z;
+        Q.mass = in.p->mass;
         Q.flux = (const float *)(ws + L.off_flux);
         Q.gconv = gconv;
         Q.g_mass = g_mass; Q.g_age = g_age; Q.g_z = g_z; Q.g_v = g_v;

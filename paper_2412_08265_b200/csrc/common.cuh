@@ -40,6 +40,12 @@ struct __align__(16) Rec {
 };
 static_assert(sizeof(Rec) == 48, "Rec layout");
 
+// Per in-FoV particle, sorted order: what the adjoint kernel needs of the SSP cell (written by k_prepare_records).
+struct __align__(16) AdjAux {
+    float ta, tz;          // position inside the (log age, log Z) cell, in [0, 1]
+    float inv_wa, inv_wz;  // 1 / cell width along each axis, 0 where the particle is clamped to the grid edge
+};
+
 // One work unit of the accumulate kernel: up to kChunk consecutive sorted particles of one spaxel.
 struct __align__(16) Unit {
     int32_t start;     // first sorted index
@@ -67,7 +73,7 @@ struct Layout {
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,
-        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps;
+        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps, off_aux;
     int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
                                       // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch

@@ -336,7 +336,7 @@ __global__ void __launch_bounds__(256)
 k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
                   const float *__restrict__ vlos, const float *__restrict__ mass,
                   const float *__restrict__ log_age, const float *__restrict__ log_z,
-                  const __grid_constant__ PrepParams P, Rec *__restrict__ rec)
+                  const __grid_constant__ PrepParams P, Rec *__restrict__ rec, AdjAux *__restrict__ aux)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= seg_off[P.n_s]) return;            // dropped particles sort last and get no record
@@ -346,6 +346,17 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta);
     axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz);
     const double m = (double)mass[p] * (double)P.flux_scale;
+    {
+        const float qa = log_age[p], qz = log_z[p];
+        AdjAux x;
+        x.ta = (float)ta;
+        x.tz = (float)tz;
+        x.inv_wa = (qa > P.ax.age[0] && qa < P.ax.age[P.ax.n_age - 1])
+                       ? (float)(1.0 / ((double)P.ax.age[ia + 1] - (double)P.ax.age[ia])) : 0.0f;
+        x.inv_wz = (qz > P.ax.z[0] && qz < P.ax.z[P.ax.n_z - 1])
+                       ? (float)(1.0 / ((double)P.ax.z[iz + 1] - (double)P.ax.z[iz])) : 0.0f;
+        aux[i] = x;
+    }
     Rec r;
     r.w[0] = (float)(m * (1.0 - ta) * (1.0 - tz));
     r.w[1] = (float)(m * ta * (1.0 - tz));
@@ -521,6 +532,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_tiletot = take(((size_t)n_s / kScanTile + 1) * 3 * 4);
     L.off_units = take((size_t)L.max_units * sizeof(Unit));
     L.off_rec = take(nn * sizeof(Rec));
+    L.off_aux = take(nn * sizeof(AdjAux));
     L.off_partials = take((size_t)L.max_part_rows * (size_t)n_c * 4);
     L.n_rows = n_rows;
     L.n_lambda = n_lambda;
@@ -642,7 +654,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.l0_obs = in.tel->lambda0;
         P.dl_obs = in.tel->dlambda;
         k_prepare_records<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
-            perm, seg, vlos, in.p->mass, in.p->log_age, in.p->log_z, P, rec);
+            perm, seg, vlos, in.p->mass, in.p->log_age, in.p->log_z, P, rec, (AdjAux *)(ws + L.off_aux));
         RUBIX_LAUNCH_CHECK();
     }
     return cudaSuccess;
