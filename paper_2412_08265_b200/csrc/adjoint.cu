@@ -90,7 +90,9 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     int64_t x = r.a_fx + (int64_t)r.b_fx * (r.k_lo + lane);
     const int64_t *xt = P.xtab + r.k_lo + lane;          // LOGX: x_k = xtab[k] + a_fx, and dx/dbeta is the same
     const float lam_log = (1.0f + vlos[p] / (float)kCkms) * 0.4342944819f;
-    const double c_tab = (double)r.b_fx * (1.0 / (double)(1u << 30));
+    // table mode: the Doppler factor in full fp64 (the record's 2.30 value is 5e-6 samples off at x ~ 6000, enough to
+    // put a channel on the other side of a knot, where d/dv_los jumps); the channel range stays the record's
+    const double c_tab = P.log_grid ? 1.0 : 1.0 / (1.0 + (double)vlos[p] / kCkms);
     const float lam_step = 32.0f * P.dl_obs;
     float lam = fmaf(P.dl_obs, (float)(r.k_lo + lane), P.l0_obs);
     const float *T1 = T0 + (size_t)P.n_z * P.pitch, *T2 = T0 + P.pitch, *T3 = T1 + P.pitch;
@@ -99,7 +101,7 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
     auto channel = [&]() {
         if (LOGX) {                                         // table mode
             const int64_t y = __ldg(xt);
-            x = r.a_fx + __double2ll_rn((double)y * c_tab);
+            x = max((int64_t)(r.a_fx + __double2ll_rn((double)y * c_tab)), (int64_t)0);
             // d x_k / d beta = -lambda_k / ((1+z)(1+beta)^2 dl_ssp) on a linear SSP grid (lambda_k/(1+z) = Y dl_ssp);
             // on a log-sampled one it is the same for every channel: lambda_k -> (1+beta) / ln 10
             lam = P.log_grid ? lam_log : (float)((double)y * (1.0 / (double)(1 << kFxFrac))) * P.dl_ssp;
@@ -114,12 +116,14 @@ k_adjoint(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
         const float a1 = __ldg(T1 + ju), b1 = __ldg(T1 + ju + 1) - a1;
         const float a2 = __ldg(T2 + ju), b2 = __ldg(T2 + ju + 1) - a2;
         const float a3 = __ldg(T3 + ju), b3 = __ldg(T3 + ju + 1) - a3;
-        const float v0 = fmaf(f, b0, a0), v1 = fmaf(f, b1, a1), v2 = fmaf(f, b2, a2), v3 = fmaf(f, b3, a3);
-        const float da = v1 - v0, dz = v2 - v0;
+        // difference basis on the samples (their differences are exact in fp32), then the interpolation
+        const float v0 = fmaf(f, b0, a0);
+        const float da = fmaf(f, b1 - b0, a1 - a0), dz = fmaf(f, b2 - b0, a2 - a0);
+        const float dq = fmaf(f, (b3 - b2) - (b1 - b0), (a3 - a2) - (a1 - a0));
         s0 = fmaf(gk, v0, s0);
         sa = fmaf(gk, da, sa);
         sz = fmaf(gk, dz, sz);
-        sq = fmaf(gk, (v3 - v2) - da, sq);
+        sq = fmaf(gk, dq, sq);
         se = fmaf(gk * lam, fmaf(u3, b3, fmaf(u2, b2, fmaf(u1, b1, u0 * b0))), se);
         x += step; lam += lam_step; gp += 32;
     };
@@ -235,15 +239,16 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
             const float w0 = (uu1 - f) - q1, w2 = 0.5f * uu2 * uu2, w1 = q1 + uu2 - w2;
             const float a0 = __ldg(T0 + j), a1 = __ldg(T1 + j), a2 = __ldg(T2 + j), a3 = __ldg(T3 + j);
             const float b0 = __ldg(T0 + j + 1), b1 = __ldg(T1 + j + 1), b2 = __ldg(T2 + j + 1), b3 = __ldg(T3 + j + 1);
-            const float v0 = fmaf(w2, __ldg(T0 + j + 2), fmaf(w1, b0, w0 * a0));
-            const float v1 = fmaf(w2, __ldg(T1 + j + 2), fmaf(w1, b1, w0 * a1));
-            const float v2 = fmaf(w2, __ldg(T2 + j + 2), fmaf(w1, b2, w0 * a2));
-            const float v3 = fmaf(w2, __ldg(T3 + j + 2), fmaf(w1, b3, w0 * a3));
-            const float da = v1 - v0, dz = v2 - v0;
+            const float c0 = __ldg(T0 + j + 2), c1 = __ldg(T1 + j + 2), c2 = __ldg(T2 + j + 2), c3 = __ldg(T3 + j + 2);
+            // difference basis on the SAMPLES (exact in fp32), then the bin weights: no subtraction of rounded averages
+            const float v0 = fmaf(w2, c0, fmaf(w1, b0, w0 * a0));
+            const float da = fmaf(w2, c1 - c0, fmaf(w1, b1 - b0, w0 * (a1 - a0)));
+            const float dz = fmaf(w2, c2 - c0, fmaf(w1, b2 - b0, w0 * (a2 - a0)));
+            const float dq = fmaf(w2, (c3 - c2) - (c1 - c0), fmaf(w1, (b3 - b2) - (b1 - b0), w0 * ((a3 - a2) - (a1 - a0))));
             s0 = gk * v0;
             sa = gk * da;
             sz = gk * dz;
-            sq = gk * ((v3 - v2) - da);
+            sq = gk * dq;
             E += edge_term(xl & (((int64_t)1 << kFxFrac) - 1), k, gm1 - gk, a0, a1, a2, a3, b0, b1, b2, b3);
             P0 += (double)s0; Pa += (double)sa; Pz += (double)sz; Pq += (double)sq;
             continue;
@@ -252,21 +257,21 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
             const int64_t cl = max(xl, (int64_t)0), ch = min(xl + b, x_max);
             const int jl = (int)(cl >> kFxFrac);
             const int ju = min((int)((ch + ((int64_t)1 << kFxFrac) - 1) >> kFxFrac), P.n_lambda - 1);
-            float v0 = 0.f, v1 = 0.f, v2 = 0.f, v3 = 0.f;
+            float v0 = 0.f, da = 0.f, dz = 0.f, dq = 0.f;
             for (int j = jl; j <= ju; ++j) {
                 const int64_t o = (int64_t)j << kFxFrac;
                 const float w = hat_integral((float)(ch - o) * inv_scale) - hat_integral((float)(cl - o) * inv_scale);
                 const uint32_t ju32 = (uint32_t)j;
-                v0 = fmaf(w, __ldg(T0 + ju32), v0);
-                v1 = fmaf(w, __ldg(T1 + ju32), v1);
-                v2 = fmaf(w, __ldg(T2 + ju32), v2);
-                v3 = fmaf(w, __ldg(T3 + ju32), v3);
+                const float t0 = __ldg(T0 + ju32), t1 = __ldg(T1 + ju32), t2 = __ldg(T2 + ju32), t3 = __ldg(T3 + ju32);
+                v0 = fmaf(w, t0, v0);
+                da = fmaf(w, t1 - t0, da);
+                dz = fmaf(w, t2 - t0, dz);
+                dq = fmaf(w, (t3 - t2) - (t1 - t0), dq);
             }
-            const float da = v1 - v0, dz = v2 - v0;
             s0 = gk * v0;
             sa = gk * da;
             sz = gk * dz;
-            sq = gk * ((v3 - v2) - da);
+            sq = gk * dq;
         }
         if (xl >= 0 && xl <= x_max) {                       // ---- edge k inside the coverage
             const int j = min((int)(xl >> kFxFrac), P.n_lambda - 2);   // last knot: interval N_l - 2 with f = 1
@@ -452,7 +457,85 @@ __device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32
     }
 }
 
-template <int NA, int NB>
+// Flux-conserving rule (reading R13), same pass structure.  The lattice points are the n_c + 1 bin EDGES
+// x_e = A + B e (A = lower edge of bin 0); with D_e = g_{e-1} - g_e (g = 0 outside the detector) summation by parts gives
+//   B W_j = sum_e D_e H(x_e - j),  H = integral of the hat function  (edges beyond the coverage sit ON its end: H = 1/2 at
+//           the last knot, 1 below it; edges below the coverage add -g/2 to W_0: the caller's fix-up)
+//         = C_{j-1} + A_j + tail_j,   A_i = M0/2 + M1 - M2/2,  C_i = M2/2,  tail_j = g of the last edge below j + 1
+//   V_j   = sum_e D_e (x_e + l0/dl) hat(x_e - j) = VA_j + VC_{j-1},  VA_i = xi (M0 - M1) + M1 - M2,  VC_i = xi M1 + M2
+// from the moments M_n = sum over the edges of interval i of D_e frac(x_e)^n, xi = j0 + i + l0_ssp/dl_ssp.  The P sums
+// use W as in the point rule; the edge term of d/dv_los is sum_j V_j T_c[j] (no template differences needed).
+struct AdjLaneFlux {
+    float c_carry, vc_carry;                                // C and VC of lane 31's last interval in the previous pass
+    unsigned long long q0, q1, q2, q3;                      // packed (even j, odd j) sums of V_j T_c[j]
+};
+
+template <int NA, int NB, bool MASK>
+__device__ __forceinline__ void adj_pass_flux(const AdjCorners &C, AdjLane &L, AdjLaneFlux &F, uint32_t sg_addr, int lane, int lim)
+{
+    uint32_t addr = sg_addr + ((uint32_t)L.k << 2);
+    uint32_t lo = L.d_lo, hi = L.d_hi;
+    float g_prev;
+    asm volatile("ld.shared.f32 %0, [%1+-4];" : "=f"(g_prev) : "r"(addr));
+    float wa[4], wc[4], va[4], vc[4];                       // A_i + tail_i, C_i, VA_i, VC_i
+    float xi = L.xb;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        float m0 = 0.0f, m1 = 0.0f, m2 = 0.0f, f = 0.0f;
+        const float tail_prev = g_prev;
+        const uint32_t bound = (uint32_t)(i + 1) << (kAdjUFrac - 32);
+#pragma unroll
+        for (int st = 0; st < NA + NB; ++st) {
+            const bool take = st < NA || hi < bound;
+            if (take) {
+                float ge;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ge) : "r"(addr));
+                if (st == 0)
+                    f = __uint_as_float(adj_and_or(__funnelshift_r(lo, hi, kAdjUFrac - 23), 0x7FFFFFu, 0x3F800000u)) - 1.0f;
+                else
+                    f += L.bf;
+                const float dg = g_prev - ge;
+                const float t = dg * f;
+                m0 += dg;
+                m1 += t;
+                m2 = fmaf(t, f, m2);
+                g_prev = ge;
+                adj_add64(lo, hi, L.b_lo, L.b_hi);
+                addr += 4;
+            }
+        }
+        float a_i = fmaf(0.5f, m0 - m2, m1) + g_prev, c_i = 0.5f * m2;
+        float va_i = fmaf(xi, m0 - m1, m1 - m2), vc_i = fmaf(xi, m1, m2);
+        if (MASK && i >= lim) {                             // at or beyond the last knot
+            a_i = i == lim ? 0.5f * tail_prev : 0.0f;
+            c_i = 0.0f; va_i = 0.0f; vc_i = 0.0f;
+        }
+        wa[i] = a_i; wc[i] = c_i; va[i] = va_i; vc[i] = vc_i;
+        xi += 1.0f;
+    }
+    float c_prev = __shfl_up_sync(0xffffffffu, wc[3], 1), vc_prev = __shfl_up_sync(0xffffffffu, vc[3], 1);
+    if (lane == 0) { c_prev = F.c_carry; vc_prev = F.vc_carry; }
+    F.c_carry = __shfl_sync(0xffffffffu, wc[3], 31);
+    F.vc_carry = __shfl_sync(0xffffffffu, vc[3], 31);
+    const float w0 = wa[0] + c_prev, w1 = wa[1] + wc[0], w2 = wa[2] + wc[1], w3 = wa[3] + wc[2];
+    const float v0 = va[0] + vc_prev, v1 = va[1] + vc[0], v2 = va[2] + vc[1], v3 = va[3] + vc[2];
+    const unsigned long long neg1 = pack2(-1.0f, -1.0f);
+    const unsigned long long wl = pack2(w0, w1), wh = pack2(w2, w3), vl = pack2(v0, v1), vh = pack2(v2, v3);
+    const unsigned long long dal = ffma2(C.c[0].lo, neg1, C.c[1].lo), dah = ffma2(C.c[0].hi, neg1, C.c[1].hi);
+    const unsigned long long dzl = ffma2(C.c[0].lo, neg1, C.c[2].lo), dzh = ffma2(C.c[0].hi, neg1, C.c[2].hi);
+    const unsigned long long dql = ffma2(dal, neg1, ffma2(C.c[2].lo, neg1, C.c[3].lo));
+    const unsigned long long dqh = ffma2(dah, neg1, ffma2(C.c[2].hi, neg1, C.c[3].hi));
+    L.p0 = ffma2(wh, C.c[0].hi, ffma2(wl, C.c[0].lo, L.p0));
+    L.pa = ffma2(wh, dah, ffma2(wl, dal, L.pa));
+    L.pz = ffma2(wh, dzh, ffma2(wl, dzl, L.pz));
+    L.pq = ffma2(wh, dqh, ffma2(wl, dql, L.pq));
+    F.q0 = ffma2(vh, C.c[0].hi, ffma2(vl, C.c[0].lo, F.q0));
+    F.q1 = ffma2(vh, C.c[1].hi, ffma2(vl, C.c[1].lo, F.q1));
+    F.q2 = ffma2(vh, C.c[2].hi, ffma2(vl, C.c[2].lo, F.q2));
+    F.q3 = ffma2(vh, C.c[3].hi, ffma2(vl, C.c[3].lo, F.q3));
+}
+
+template <int NA, int NB, bool FLUX>
 __global__ void __launch_bounds__(kAdjUThreads, RUBIX_ADJU_MINB)
 k_adjoint_units(const __grid_constant__ AdjUParams P)
 {
@@ -498,14 +581,15 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
     __syncthreads();
     const uint32_t sg_addr = (uint32_t)__cvta_generic_to_shared(sg);
     const int row_a = P.n_z * P.pitch, row_z = P.pitch;
-    const float x_off = (float)(P.l0_ssp / P.dl_ssp) - 1.0f; // lambda = (x + l0_ssp/dl_ssp) dl_ssp (1 + beta); -1: b1 carries 1 + frac
+    // lambda = (x + l0_ssp/dl_ssp) dl_ssp (1 + beta); point rule: -1 because b1 carries 1 + frac
+    const float x_off = (float)(P.l0_ssp / P.dl_ssp) - (FLUX ? 0.0f : 1.0f);
     const int64_t x_top = (int64_t)(P.n_lambda - 1) << kAdjUFrac;
     const double inv_dl_ssp = 1.0 / P.dl_ssp;
 
     auto load = [&](AdjCorners &C, const float *t) {
         C.c[0] = adj_ldg_quad(t); C.c[1] = adj_ldg_quad(t + row_a);
         C.c[2] = adj_ldg_quad(t + row_z); C.c[3] = adj_ldg_quad(t + row_a + row_z);
-        if (lane == 31) {                                   // fifth sample of each corner: the next block's first
+        if (!FLUX && lane == 31) {                          // fifth sample of each corner: the next block's first
             C.e[0] = __ldg(t + 4); C.e[1] = __ldg(t + row_a + 4);
             C.e[2] = __ldg(t + row_z + 4); C.e[3] = __ldg(t + row_a + row_z + 4);
         }
@@ -527,15 +611,17 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
         const double opb = 1.0 + (double)P.vlos[p] / kCkms;
         const double inv = 1.0 / opb;
         const double scale = (double)((int64_t)1 << kAdjUFrac);
-        const int64_t a44 = __double2ll_rn((P.l0_obs * inv - P.l0_ssp) * inv_dl_ssp * scale);
+        // lattice: channel centres x_k (point rule, n_c points) or bin edges x_e (flux rule, n_c + 1 points)
+        const int64_t a44 = __double2ll_rn(((P.l0_obs - (FLUX ? 0.5 * P.dl_obs : 0.0)) * inv - P.l0_ssp) * inv_dl_ssp * scale);
         const int64_t b44 = __double2ll_rn(P.dl_obs * inv * inv_dl_ssp * scale);
-        const int64_t x_first = a44, x_last = a44 + (int64_t)(P.n_c - 1) * b44;
+        const int64_t x_first = a44, x_last = a44 + (int64_t)(FLUX ? P.n_c : P.n_c - 1) * b44;
         const int64_t x_lo = max(x_first, (int64_t)0), x_hi = min(x_last, x_top);
 #pragma unroll
         for (int c = 0; c < 8; ++c) acc[c * kAdjUThreads] = 0.0;
         if (x_lo <= x_hi) {
             const int j_begin = (int)(x_lo >> kAdjUFrac) & ~(kRowAlign - 1);
-            const int j_last = (int)(x_hi >> kAdjUFrac);
+            // the sample above the last lattice point still receives weight (beta / C of its interval)
+            const int j_last = min((int)(x_hi >> kAdjUFrac) + 1, P.n_lambda - 1);
             // channels per 128 samples: kstep = floor(128 / B); a pass moves the lane's first channel by kstep or
             // kstep + 1, decided in exact integers: delta = kstep B - 128 in (-B, 0]
             const double inv_b = 1.0 / (double)b44;
@@ -562,16 +648,26 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
             L.beta_carry = 0.0f;
             L.p0 = L.pa = L.pz = L.pq = 0ull;
             L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
+            AdjLaneFlux F;
+            F.c_carry = F.vc_carry = 0.0f;
+            F.q0 = F.q1 = F.q2 = F.q3 = 0ull;
             const float *t = T0 + j0;
             int n_acc = 0;
             auto flush = [&]() {
                 const float2 f0 = unpack2(L.p0), fa = unpack2(L.pa), fz = unpack2(L.pz), fq = unpack2(L.pq);
                 acc[0 * kAdjUThreads] += (double)(f0.x + f0.y); acc[1 * kAdjUThreads] += (double)(fa.x + fa.y);
                 acc[2 * kAdjUThreads] += (double)(fz.x + fz.y); acc[3 * kAdjUThreads] += (double)(fq.x + fq.y);
-                acc[4 * kAdjUThreads] += (double)L.q0; acc[5 * kAdjUThreads] += (double)L.q1;
-                acc[6 * kAdjUThreads] += (double)L.q2; acc[7 * kAdjUThreads] += (double)L.q3;
+                if (FLUX) {
+                    const float2 g0 = unpack2(F.q0), g1 = unpack2(F.q1), g2 = unpack2(F.q2), g3 = unpack2(F.q3);
+                    acc[4 * kAdjUThreads] += (double)(g0.x + g0.y); acc[5 * kAdjUThreads] += (double)(g1.x + g1.y);
+                    acc[6 * kAdjUThreads] += (double)(g2.x + g2.y); acc[7 * kAdjUThreads] += (double)(g3.x + g3.y);
+                    F.q0 = F.q1 = F.q2 = F.q3 = 0ull;
+                } else {
+                    acc[4 * kAdjUThreads] += (double)L.q0; acc[5 * kAdjUThreads] += (double)L.q1;
+                    acc[6 * kAdjUThreads] += (double)L.q2; acc[7 * kAdjUThreads] += (double)L.q3;
+                    L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
+                }
                 L.p0 = L.pa = L.pz = L.pq = 0ull;
-                L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
                 n_acc = 0;
             };
             auto advance = [&]() {                          // next pass: 128 samples on
@@ -589,13 +685,15 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 load(A, t);
                 prefetch(t + 128);
                 L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
-                adj_pass<NA, NB, false>(A, L, sg_addr, lane, 0);
+                if (FLUX) adj_pass_flux<NA, NB, false>(A, L, F, sg_addr, lane, 0);
+                else adj_pass<NA, NB, false>(A, L, sg_addr, lane, 0);
                 advance();
             }
             for (; jp <= j_last; jp += 128) {               // passes that touch the last knot
                 load(A, t);
                 L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
-                adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0);
+                if (FLUX) adj_pass_flux<NA, NB, true>(A, L, F, sg_addr, lane, P.n_lambda - 1 - j0);
+                else adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0);
                 advance();
             }
             flush();
@@ -619,33 +717,57 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
         if (lane == 0) {
             const AdjAux ax = P.aux[i_sorted];
             const double ta = (double)ax.ta, tz = (double)ax.tz;
-            double p0 = P0, pa = Pa, pz = Pz, pq = Pq;
-            // a channel sitting exactly on the last knot (x_k = N_l - 1) takes the last sample with weight 1,
-            // as the forward kernel does; its slope term is left out (the spectrum ends there)
-            if (x_last >= x_top && x_first <= x_top && (x_top - a44) % b44 == 0) {
-                const int64_t kh = (x_top - a44) / b44;
-                const float gk = sg[kh];
-                const float *tl = T0 + (P.n_lambda - 1);
-                const float t0 = tl[0], t1 = tl[row_a], t2 = tl[row_z], t3 = tl[row_a + row_z];
-                p0 += (double)gk * t0;
-                pa += (double)gk * ((double)t1 - t0);
-                pz += (double)gk * ((double)t2 - t0);
-                pq += (double)gk * (((double)t3 - t2) - ((double)t1 - t0));
+            double p0 = P0, pa = Pa, pz = Pz, pq = Pq, q0 = Q0, q1 = Q1, q2 = Q2, q3 = Q3;
+            const float *tl = T0 + (P.n_lambda - 1);
+            const bool on_top = x_last >= x_top && x_first <= x_top && (x_top - a44) % b44 == 0;
+            auto add_w = [&](double w, const float *tp) {  // weight w on one sample of the four corners
+                const float t0 = tp[0], t1 = tp[row_a], t2 = tp[row_z], t3 = tp[row_a + row_z];
+                p0 += w * t0;
+                pa += w * ((double)t1 - t0);
+                pz += w * ((double)t2 - t0);
+                pq += w * (((double)t3 - t2) - ((double)t1 - t0));
+            };
+            if (!FLUX) {
+                // a channel sitting exactly on the last knot (x_k = N_l - 1) takes the last sample with weight 1,
+                // as the forward kernel does; its slope term is left out (the spectrum ends there)
+                if (on_top) add_w((double)sg[(x_top - a44) / b44], tl);
+            } else {
+                // edges below the coverage sit on its first knot: -g_{e0-1} H(0) on W_0 (e0 = first edge at or above 0)
+                if (x_first < 0 && x_last >= 0) {
+                    const int64_t e0 = (-a44 + b44 - 1) / b44;
+                    add_w(-0.5 * (double)sg[e0 - 1], T0);
+                }
+                // an edge exactly on the last knot is inside the coverage: its term (x + l0/dl) D_e T_c[N_l - 1] of V
+                if (on_top) {
+                    const int64_t eh = (x_top - a44) / b44;
+                    const double v = ((double)(P.n_lambda - 1) + P.l0_ssp * inv_dl_ssp) * ((double)sg[eh - 1] - (double)sg[eh]);
+                    q0 += v * tl[0]; q1 += v * tl[row_a]; q2 += v * tl[row_z]; q3 += v * tl[row_a + row_z];
+                }
             }
             const double m = (double)P.mass[p] * (double)P.flux_scale;
-            const double E = (1.0 - ta) * (1.0 - tz) * Q0 + ta * (1.0 - tz) * Q1 + (1.0 - ta) * tz * Q2 + ta * tz * Q3;
-            P.g_mass[p] = (float)((double)P.flux_scale * (p0 + ta * pa + tz * pz + ta * tz * pq));
-            P.g_age[p] = (float)(m * (pa + tz * pq) * (double)ax.inv_wa);
-            P.g_z[p] = (float)(m * (pz + ta * pq) * (double)ax.inv_wz);
-            P.g_v[p] = (float)(-m * E * inv / kCkms);
+            const double E = (1.0 - ta) * (1.0 - tz) * q0 + ta * (1.0 - tz) * q1 + (1.0 - ta) * tz * q2 + ta * tz * q3;
+            const double gm = p0 + ta * pa + tz * pz + ta * tz * pq;
+            if (!FLUX) {
+                P.g_mass[p] = (float)((double)P.flux_scale * gm);
+                P.g_age[p] = (float)(m * (pa + tz * pq) * (double)ax.inv_wa);
+                P.g_z[p] = (float)(m * (pz + ta * pq) * (double)ax.inv_wz);
+                P.g_v[p] = (float)(-m * E * inv / kCkms);
+            } else {
+                // W and V carry a factor B: F_k = (1/B) integral;  d/dbeta sum g F = [sum g F - (1/B) sum V S] / (1 + beta)
+                const double inv_bw = scale / (double)b44;
+                P.g_mass[p] = (float)((double)P.flux_scale * inv_bw * gm);
+                P.g_age[p] = (float)(m * inv_bw * (pa + tz * pq) * (double)ax.inv_wa);
+                P.g_z[p] = (float)(m * inv_bw * (pz + ta * pq) * (double)ax.inv_wz);
+                P.g_v[p] = (float)(m * inv_bw * (gm - E) * inv / kCkms);
+            }
         }
     }
 }
 
 template <int NA, int NB>
-static cudaError_t launch_adjoint_units(const AdjUParams &P, unsigned grid, size_t smem, cudaStream_t st)
+static cudaError_t launch_adjoint_units(const AdjUParams &P, bool flux, unsigned grid, size_t smem, cudaStream_t st)
 {
-    auto kern = k_adjoint_units<NA, NB>;
+    auto kern = flux ? k_adjoint_units<NA, NB, true> : k_adjoint_units<NA, NB, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kAdjUThreads, smem, st>>>(P);
@@ -657,7 +779,7 @@ static cudaError_t launch_adjoint_units(const AdjUParams &P, unsigned grid, size
 // sampling ratio is outside what k_adjoint_units is instantiated for (the warp-per-particle kernel takes over).
 static bool adjoint_units_shape(const PassInputs &in, int *na, int *nb)
 {
-    if (table_mode(in.ssp, in.tel) || in.tel->resample != RUBIX_RESAMPLE_POINT) return false;
+    if (table_mode(in.ssp, in.tel)) return false;
     const double b0 = (double)in.tel->dlambda / ((1.0 + (double)in.tel->redshift) * (double)in.ssp->dlambda);
     const double b_lo = b0 / (1.0 + kBetaCap) * (1.0 - 1e-6), b_hi = b0 / (1.0 - kBetaCap) * (1.0 + 1e-6);
     if (!(b_lo >= 0.26) || !(b_hi < 3.0)) return false;
@@ -714,15 +836,16 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
         const size_t smem = (size_t)(((size_t)L.n_c + kAdjUFront + kAdjUBack + 3) & ~(size_t)3) * sizeof(float) +
                             (size_t)8 * kAdjUThreads * sizeof(double);
         const unsigned grid = (unsigned)(L.max_units * kAdjUSplit);
+        const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
         switch (na * 2 + (nb - 1)) {
-            case 0: return launch_adjoint_units<0, 1>(Q, grid, smem, st);
-            case 1: return launch_adjoint_units<0, 2>(Q, grid, smem, st);
-            case 2: return launch_adjoint_units<1, 1>(Q, grid, smem, st);
-            case 3: return launch_adjoint_units<1, 2>(Q, grid, smem, st);
-            case 4: return launch_adjoint_units<2, 1>(Q, grid, smem, st);
-            case 5: return launch_adjoint_units<2, 2>(Q, grid, smem, st);
-            case 6: return launch_adjoint_units<3, 1>(Q, grid, smem, st);
-            default: return launch_adjoint_units<3, 2>(Q, grid, smem, st);
+            case 0: return launch_adjoint_units<0, 1>(Q, flux, grid, smem, st);
+            case 1: return launch_adjoint_units<0, 2>(Q, flux, grid, smem, st);
+            case 2: return launch_adjoint_units<1, 1>(Q, flux, grid, smem, st);
+            case 3: return launch_adjoint_units<1, 2>(Q, flux, grid, smem, st);
+            case 4: return launch_adjoint_units<2, 1>(Q, flux, grid, smem, st);
+            case 5: return launch_adjoint_units<2, 2>(Q, flux, grid, smem, st);
+            case 6: return launch_adjoint_units<3, 1>(Q, flux, grid, smem, st);
+            default: return launch_adjoint_units<3, 2>(Q, flux, grid, smem, st);
         }
     }
     const int64_t threads = L.n * 32;
