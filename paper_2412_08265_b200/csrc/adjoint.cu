@@ -334,8 +334,9 @@ k_adjoint_flux(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg
 constexpr int kAdjUThreads = 128;
 constexpr int kAdjUWarps = kAdjUThreads / 32;
 constexpr int kAdjUSplit = 4;               // CTAs per unit: each takes kChunk / kAdjUSplit particles (finer tail)
-constexpr int kAdjUFront = 160;             // zero floats in front of the staged G' row (B >= 0.25: k >= -32/B - 2)
-constexpr int kAdjUBack = 544;              // and behind it (a pass overshoots the last channel by < 128/B + 8)
+// The staged G' row is zero padded: `front` floats before it (a pass starts up to 32 samples below the first
+// lattice point: k >= -32/B - 2) and `back` behind it (a pass overshoots the last one by < 128/B + 8 points); both are
+// multiples of 4, chosen by the host from the smallest B the velocity cap allows.
 constexpr int kAdjUFrac = 44;               // fractional bits of x_k in this kernel
 constexpr int kAdjUFlush = 4;               // passes accumulated in fp32 before the fp64 flush
 
@@ -347,6 +348,8 @@ struct AdjUParams {
     const float *vlos, *mass, *flux, *gconv;
     float *g_mass, *g_age, *g_z, *g_v;
     int32_t n_lambda, pitch, n_z, n_c, n_s;
+    int32_t front, back;                        // zero padding of the staged G' row, floats
+    int32_t na, nb;                             // lattice points per knot interval: at least na, at most na + nb
     double l0_obs, dl_obs, l0_ssp, dl_ssp;      // observed grid already divided by (1 + z)
     float flux_scale;
     int64_t n;
@@ -379,6 +382,7 @@ struct AdjLane {
     float bf;                                               // B as a float (fraction of the second channel of an interval)
     float xb;                                               // j0 + l0_ssp/dl_ssp - 1
     float beta_carry;                                       // beta of lane 31's last interval in the previous pass
+    int na, nb;                                             // runtime step counts of the generic instance (NA < 0)
     unsigned long long p0, pa, pz, pq;                      // packed (even j, odd j) partial sums
     float q0, q1, q2, q3;
 };
@@ -401,8 +405,9 @@ __device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32
         float s = 0.0f, b = 0.0f, f1 = 1.0f;
         const uint32_t bound = (uint32_t)(i + 1) << (kAdjUFrac - 32);
 #pragma unroll
-        for (int st = 0; st < NA + NB; ++st) {
-            const bool take = st < NA || hi < bound;
+        for (int st = 0; st < (NA < 0 ? L.na + L.nb : NA + NB); ++st) {
+            const bool take = st < (NA < 0 ? L.na : NA) || hi < bound;
+            if (NA < 0 && !take) break;
             if (take) {
                 float gk;
                 asm volatile("ld.shared.f32 %0, [%1];" : "=f"(gk) : "r"(addr));
@@ -410,8 +415,8 @@ __device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32
                     f1 = __uint_as_float(adj_and_or(__funnelshift_r(lo, hi, kAdjUFrac - 23), 0x7FFFFFu, 0x3F800000u));
                 else
                     f1 += L.bf;                             // same interval: the next channel sits B further on
-                s = st == 0 ? gk : s + gk;
-                b = st == 0 ? gk * f1 : fmaf(gk, f1, b);
+                s += gk;
+                b = fmaf(gk, f1, b);
                 adj_add64(lo, hi, L.b_lo, L.b_hi);
                 addr += 4;
             }
@@ -462,31 +467,33 @@ __device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32
 //   B W_j = sum_e D_e H(x_e - j),  H = integral of the hat function  (edges beyond the coverage sit ON its end: H = 1/2 at
 //           the last knot, 1 below it; edges below the coverage add -g/2 to W_0: the caller's fix-up)
 //         = C_{j-1} + A_j + tail_j,   A_i = M0/2 + M1 - M2/2,  C_i = M2/2,  tail_j = g of the last edge below j + 1
-//   V_j   = sum_e D_e (x_e + l0/dl) hat(x_e - j) = VA_j + VC_{j-1},  VA_i = xi (M0 - M1) + M1 - M2,  VC_i = xi M1 + M2
-// from the moments M_n = sum over the edges of interval i of D_e frac(x_e)^n, xi = j0 + i + l0_ssp/dl_ssp.  The P sums
-// use W as in the point rule; the edge term of d/dv_los is sum_j V_j T_c[j] (no template differences needed).
-struct AdjLaneFlux {
-    float c_carry, vc_carry;                                // C and VC of lane 31's last interval in the previous pass
-    unsigned long long q0, q1, q2, q3;                      // packed (even j, odd j) sums of V_j T_c[j]
-};
-
+// from the moments M_n = sum over the edges of interval i of D_e frac(x_e)^n.  The P sums use W as in the point rule.
+// d/dv_los: inside the coverage dF_k/dbeta = -(1 / (B (1 + beta))) integral over bin k of (x + l0/dl) s'(x) dx, and s' is
+// the constant S_{i+1} - S_i on knot interval i, so
+//   sum_k g_k dF_k/dbeta = -(1 / (B (1 + beta))) sum_i Gamma_i (S_{i+1} - S_i),
+//   Gamma_i = integral over [i, i+1) of g(x) (x + l0/dl) dx      (g(x) = g_k on bin k)
+//           = g_start (xi + 1/2) - [xi (M0 - M1) + (M0 - M2) / 2],   xi = i + l0_ssp/dl_ssp,
+// i.e. the point rule's slope sums with Gamma in place of gamma: exact template differences, no cancellation
+// (the equivalent edge form sum_e D_e lambda_e s(x_e) cancels to this derivative and loses 3 digits in fp32).
+// Bins cut by an end of the coverage add a boundary term each (the caller's fix-up).
 template <int NA, int NB, bool MASK>
-__device__ __forceinline__ void adj_pass_flux(const AdjCorners &C, AdjLane &L, AdjLaneFlux &F, uint32_t sg_addr, int lane, int lim)
+__device__ __forceinline__ void adj_pass_flux(const AdjCorners &C, AdjLane &L, float &c_carry, uint32_t sg_addr, int lane, int lim)
 {
     uint32_t addr = sg_addr + ((uint32_t)L.k << 2);
     uint32_t lo = L.d_lo, hi = L.d_hi;
     float g_prev;
     asm volatile("ld.shared.f32 %0, [%1+-4];" : "=f"(g_prev) : "r"(addr));
-    float wa[4], wc[4], va[4], vc[4];                       // A_i + tail_i, C_i, VA_i, VC_i
+    float wa[4], wc[4], gam[4];                             // A_i + tail_i, C_i, Gamma_i
     float xi = L.xb;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         float m0 = 0.0f, m1 = 0.0f, m2 = 0.0f, f = 0.0f;
-        const float tail_prev = g_prev;
+        const float g_start = g_prev;
         const uint32_t bound = (uint32_t)(i + 1) << (kAdjUFrac - 32);
 #pragma unroll
-        for (int st = 0; st < NA + NB; ++st) {
-            const bool take = st < NA || hi < bound;
+        for (int st = 0; st < (NA < 0 ? L.na + L.nb : NA + NB); ++st) {
+            const bool take = st < (NA < 0 ? L.na : NA) || hi < bound;
+            if (NA < 0 && !take) break;
             if (take) {
                 float ge;
                 asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ge) : "r"(addr));
@@ -505,22 +512,20 @@ __device__ __forceinline__ void adj_pass_flux(const AdjCorners &C, AdjLane &L, A
             }
         }
         float a_i = fmaf(0.5f, m0 - m2, m1) + g_prev, c_i = 0.5f * m2;
-        float va_i = fmaf(xi, m0 - m1, m1 - m2), vc_i = fmaf(xi, m1, m2);
+        float gam_i = fmaf(g_start, xi + 0.5f, -fmaf(xi, m0 - m1, 0.5f * (m0 - m2)));
         if (MASK && i >= lim) {                             // at or beyond the last knot
-            a_i = i == lim ? 0.5f * tail_prev : 0.0f;
-            c_i = 0.0f; va_i = 0.0f; vc_i = 0.0f;
+            a_i = i == lim ? 0.5f * g_start : 0.0f;
+            c_i = 0.0f; gam_i = 0.0f;
         }
-        wa[i] = a_i; wc[i] = c_i; va[i] = va_i; vc[i] = vc_i;
+        wa[i] = a_i; wc[i] = c_i; gam[i] = gam_i;
         xi += 1.0f;
     }
-    float c_prev = __shfl_up_sync(0xffffffffu, wc[3], 1), vc_prev = __shfl_up_sync(0xffffffffu, vc[3], 1);
-    if (lane == 0) { c_prev = F.c_carry; vc_prev = F.vc_carry; }
-    F.c_carry = __shfl_sync(0xffffffffu, wc[3], 31);
-    F.vc_carry = __shfl_sync(0xffffffffu, vc[3], 31);
+    float c_prev = __shfl_up_sync(0xffffffffu, wc[3], 1);
+    if (lane == 0) c_prev = c_carry;
+    c_carry = __shfl_sync(0xffffffffu, wc[3], 31);
     const float w0 = wa[0] + c_prev, w1 = wa[1] + wc[0], w2 = wa[2] + wc[1], w3 = wa[3] + wc[2];
-    const float v0 = va[0] + vc_prev, v1 = va[1] + vc[0], v2 = va[2] + vc[1], v3 = va[3] + vc[2];
     const unsigned long long neg1 = pack2(-1.0f, -1.0f);
-    const unsigned long long wl = pack2(w0, w1), wh = pack2(w2, w3), vl = pack2(v0, v1), vh = pack2(v2, v3);
+    const unsigned long long wl = pack2(w0, w1), wh = pack2(w2, w3);
     const unsigned long long dal = ffma2(C.c[0].lo, neg1, C.c[1].lo), dah = ffma2(C.c[0].hi, neg1, C.c[1].hi);
     const unsigned long long dzl = ffma2(C.c[0].lo, neg1, C.c[2].lo), dzh = ffma2(C.c[0].hi, neg1, C.c[2].hi);
     const unsigned long long dql = ffma2(dal, neg1, ffma2(C.c[2].lo, neg1, C.c[3].lo));
@@ -529,10 +534,16 @@ __device__ __forceinline__ void adj_pass_flux(const AdjCorners &C, AdjLane &L, A
     L.pa = ffma2(wh, dah, ffma2(wl, dal, L.pa));
     L.pz = ffma2(wh, dzh, ffma2(wl, dzl, L.pz));
     L.pq = ffma2(wh, dqh, ffma2(wl, dql, L.pq));
-    F.q0 = ffma2(vh, C.c[0].hi, ffma2(vl, C.c[0].lo, F.q0));
-    F.q1 = ffma2(vh, C.c[1].hi, ffma2(vl, C.c[1].lo, F.q1));
-    F.q2 = ffma2(vh, C.c[2].hi, ffma2(vl, C.c[2].lo, F.q2));
-    F.q3 = ffma2(vh, C.c[3].hi, ffma2(vl, C.c[3].lo, F.q3));
+    // slope sums: Gamma_i (T_c[i+1] - T_c[i]); the fifth sample comes from the next lane
+    float q[4] = {L.q0, L.q1, L.q2, L.q3};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float2 a = unpack2(C.c[c].lo), bq = unpack2(C.c[c].hi);
+        float nx = __shfl_down_sync(0xffffffffu, a.x, 1);
+        if (lane == 31) nx = C.e[c];
+        q[c] = fmaf(gam[3], nx - bq.y, fmaf(gam[2], bq.y - bq.x, fmaf(gam[1], bq.x - a.y, fmaf(gam[0], a.y - a.x, q[c]))));
+    }
+    L.q0 = q[0]; L.q1 = q[1]; L.q2 = q[2]; L.q3 = q[3];
 }
 
 template <int NA, int NB, bool FLUX>
@@ -558,12 +569,12 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
     constexpr int kPer = kChunk / kAdjUSplit;
     const int q_begin = part * kPer, q_end = min(U.count, q_begin + kPer);
     if (q_begin >= q_end) return;
-    float *sg = sg_raw + kAdjUFront;                        // sg[k] = G'[spaxel][k], zeros outside [0, n_c)
+    float *sg = sg_raw + P.front;                           // sg[k] = G'[spaxel][k], zeros outside [0, n_c)
     {
         const float *g = P.gconv + (size_t)U.spaxel * P.n_c;
-        for (int k = tid - kAdjUFront; k < 0; k += kAdjUThreads) sg[k] = 0.0f;
-        for (int k = P.n_c + tid; k < P.n_c + kAdjUBack; k += kAdjUThreads) sg[k] = 0.0f;
-        if ((P.n_c & 3) == 0 && ((uintptr_t)P.gconv & 15u) == 0) {      // kAdjUFront is a multiple of 4: 16-byte stores
+        for (int k = tid - P.front; k < 0; k += kAdjUThreads) sg[k] = 0.0f;
+        for (int k = P.n_c + tid; k < P.n_c + P.back; k += kAdjUThreads) sg[k] = 0.0f;
+        if ((P.n_c & 3) == 0 && ((uintptr_t)P.gconv & 15u) == 0) {      // front is a multiple of 4: 16-byte stores
             const float4 *g4 = reinterpret_cast<const float4 *>(g);
             float4 *s4 = reinterpret_cast<float4 *>(sg);
             const int n4 = P.n_c >> 2;
@@ -589,7 +600,7 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
     auto load = [&](AdjCorners &C, const float *t) {
         C.c[0] = adj_ldg_quad(t); C.c[1] = adj_ldg_quad(t + row_a);
         C.c[2] = adj_ldg_quad(t + row_z); C.c[3] = adj_ldg_quad(t + row_a + row_z);
-        if (!FLUX && lane == 31) {                          // fifth sample of each corner: the next block's first
+        if (lane == 31) {                                   // fifth sample of each corner: the next block's first
             C.e[0] = __ldg(t + 4); C.e[1] = __ldg(t + row_a + 4);
             C.e[2] = __ldg(t + row_z + 4); C.e[3] = __ldg(t + row_a + row_z + 4);
         }
@@ -602,7 +613,7 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
     };
     // fp64 running sums of the thread live in shared memory (component-major: conflict-free), flushed every
     // kAdjUFlush passes; keeps the register count low enough for five resident CTAs
-    double *acc = reinterpret_cast<double *>(sg_raw + ((P.n_c + kAdjUFront + kAdjUBack + 3) & ~3)) + tid;
+    double *acc = reinterpret_cast<double *>(sg_raw + ((P.n_c + P.front + P.back + 3) & ~3)) + tid;
 
     for (int q = q_begin + warp; q < q_end; q += kAdjUWarps) {
         const int64_t i_sorted = (int64_t)U.start + q;
@@ -646,27 +657,19 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
             L.bf = (float)((double)b44 * (1.0 / scale));
             L.xb = x_off + (float)j0;
             L.beta_carry = 0.0f;
+            L.na = P.na; L.nb = P.nb;
             L.p0 = L.pa = L.pz = L.pq = 0ull;
             L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
-            AdjLaneFlux F;
-            F.c_carry = F.vc_carry = 0.0f;
-            F.q0 = F.q1 = F.q2 = F.q3 = 0ull;
+            float c_carry = 0.0f;                           // flux rule: C of lane 31's last interval in the previous pass
             const float *t = T0 + j0;
             int n_acc = 0;
             auto flush = [&]() {
                 const float2 f0 = unpack2(L.p0), fa = unpack2(L.pa), fz = unpack2(L.pz), fq = unpack2(L.pq);
                 acc[0 * kAdjUThreads] += (double)(f0.x + f0.y); acc[1 * kAdjUThreads] += (double)(fa.x + fa.y);
                 acc[2 * kAdjUThreads] += (double)(fz.x + fz.y); acc[3 * kAdjUThreads] += (double)(fq.x + fq.y);
-                if (FLUX) {
-                    const float2 g0 = unpack2(F.q0), g1 = unpack2(F.q1), g2 = unpack2(F.q2), g3 = unpack2(F.q3);
-                    acc[4 * kAdjUThreads] += (double)(g0.x + g0.y); acc[5 * kAdjUThreads] += (double)(g1.x + g1.y);
-                    acc[6 * kAdjUThreads] += (double)(g2.x + g2.y); acc[7 * kAdjUThreads] += (double)(g3.x + g3.y);
-                    F.q0 = F.q1 = F.q2 = F.q3 = 0ull;
-                } else {
-                    acc[4 * kAdjUThreads] += (double)L.q0; acc[5 * kAdjUThreads] += (double)L.q1;
-                    acc[6 * kAdjUThreads] += (double)L.q2; acc[7 * kAdjUThreads] += (double)L.q3;
-                    L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
-                }
+                acc[4 * kAdjUThreads] += (double)L.q0; acc[5 * kAdjUThreads] += (double)L.q1;
+                acc[6 * kAdjUThreads] += (double)L.q2; acc[7 * kAdjUThreads] += (double)L.q3;
+                L.q0 = L.q1 = L.q2 = L.q3 = 0.f;
                 L.p0 = L.pa = L.pz = L.pq = 0ull;
                 n_acc = 0;
             };
@@ -685,14 +688,14 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 load(A, t);
                 prefetch(t + 128);
                 L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
-                if (FLUX) adj_pass_flux<NA, NB, false>(A, L, F, sg_addr, lane, 0);
+                if (FLUX) adj_pass_flux<NA, NB, false>(A, L, c_carry, sg_addr, lane, 0);
                 else adj_pass<NA, NB, false>(A, L, sg_addr, lane, 0);
                 advance();
             }
             for (; jp <= j_last; jp += 128) {               // passes that touch the last knot
                 load(A, t);
                 L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
-                if (FLUX) adj_pass_flux<NA, NB, true>(A, L, F, sg_addr, lane, P.n_lambda - 1 - j0);
+                if (FLUX) adj_pass_flux<NA, NB, true>(A, L, c_carry, sg_addr, lane, P.n_lambda - 1 - j0);
                 else adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0);
                 advance();
             }
@@ -732,15 +735,20 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 // as the forward kernel does; its slope term is left out (the spectrum ends there)
                 if (on_top) add_w((double)sg[(x_top - a44) / b44], tl);
             } else {
-                // edges below the coverage sit on its first knot: -g_{e0-1} H(0) on W_0 (e0 = first edge at or above 0)
+                const double off = P.l0_ssp * inv_dl_ssp;
+                // bins cut by the first knot: the edges below it sit ON it, -g H(0) on W_0; and the cut bin's boundary term
+                // -(0 + l0/dl) s(0) g of d/dv_los (a clipped edge does not move).  e0 = first edge at or above 0
                 if (x_first < 0 && x_last >= 0) {
                     const int64_t e0 = (-a44 + b44 - 1) / b44;
-                    add_w(-0.5 * (double)sg[e0 - 1], T0);
+                    const double gl = (double)sg[e0 - 1];
+                    add_w(-0.5 * gl, T0);
+                    const double v = gl * off;
+                    q0 += v * T0[0]; q1 += v * T0[row_a]; q2 += v * T0[row_z]; q3 += v * T0[row_a + row_z];
                 }
-                // an edge exactly on the last knot is inside the coverage: its term (x + l0/dl) D_e T_c[N_l - 1] of V
-                if (on_top) {
-                    const int64_t eh = (x_top - a44) / b44;
-                    const double v = ((double)(P.n_lambda - 1) + P.l0_ssp * inv_dl_ssp) * ((double)sg[eh - 1] - (double)sg[eh]);
+                // the bin cut by the last knot: boundary term +(N_l - 1 + l0/dl) s(N_l - 1) g
+                if (x_first <= x_top && x_last > x_top) {
+                    const int64_t kt = (x_top - a44) / b44;
+                    const double v = -(double)sg[kt] * ((double)(P.n_lambda - 1) + off);
                     q0 += v * tl[0]; q1 += v * tl[row_a]; q2 += v * tl[row_z]; q3 += v * tl[row_a + row_z];
                 }
             }
@@ -753,12 +761,12 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 P.g_z[p] = (float)(m * (pz + ta * pq) * (double)ax.inv_wz);
                 P.g_v[p] = (float)(-m * E * inv / kCkms);
             } else {
-                // W and V carry a factor B: F_k = (1/B) integral;  d/dbeta sum g F = [sum g F - (1/B) sum V S] / (1 + beta)
+                // W carries a factor B (F_k = (1/B) integral);  d/dbeta sum g F = -(1 / (B (1 + beta))) sum_i Gamma_i dS_i + boundary
                 const double inv_bw = scale / (double)b44;
                 P.g_mass[p] = (float)((double)P.flux_scale * inv_bw * gm);
                 P.g_age[p] = (float)(m * inv_bw * (pa + tz * pq) * (double)ax.inv_wa);
                 P.g_z[p] = (float)(m * inv_bw * (pz + ta * pq) * (double)ax.inv_wz);
-                P.g_v[p] = (float)(m * inv_bw * (gm - E) * inv / kCkms);
+                P.g_v[p] = (float)(-m * inv_bw * E * inv / kCkms);
             }
         }
     }
@@ -775,18 +783,25 @@ static cudaError_t launch_adjoint_units(const AdjUParams &P, bool flux, unsigned
     return cudaSuccess;
 }
 
-// Channels per knot interval over the velocity cap: at least NA, at most NA + NB.  Returns false when the
-// sampling ratio is outside what k_adjoint_units is instantiated for (the warp-per-particle kernel takes over).
-static bool adjoint_units_shape(const PassInputs &in, int *na, int *nb)
+// Lattice points per knot interval over the velocity cap: at least na, at most na + nb; zero padding of the staged row.
+// Returns false when k_adjoint_units cannot take the problem (table mode, or the staged row would not fit in shared
+// memory): the warp-per-particle kernels take over.
+static bool adjoint_units_shape(const PassInputs &in, const Layout &L, AdjUParams *Q, size_t *smem)
 {
     if (table_mode(in.ssp, in.tel)) return false;
     const double b0 = (double)in.tel->dlambda / ((1.0 + (double)in.tel->redshift) * (double)in.ssp->dlambda);
     const double b_lo = b0 / (1.0 + kBetaCap) * (1.0 - 1e-6), b_hi = b0 / (1.0 - kBetaCap) * (1.0 + 1e-6);
-    if (!(b_lo >= 0.26) || !(b_hi < 3.0)) return false;
-    const int n_min = (int)floor(1.0 / b_hi), n_max = (int)ceil(1.0 / b_lo);
-    *na = n_min;
-    *nb = n_max - n_min;
-    return *na >= 0 && *na <= 3 && *nb >= 1 && *nb <= 2;
+    if (!(b_lo > 0.0) || !(b_hi < 15.0)) return false;
+    const double front = ceil(32.0 / b_lo) + 16.0, back = ceil(128.0 / b_lo) + 16.0;
+    const double bytes = ((double)L.n_c + front + back + 8.0) * 4.0 + 8.0 * kAdjUThreads * sizeof(double);
+    if (bytes > 200.0 * 1024.0) return false;
+    Q->front = ((int32_t)front + 3) & ~3;
+    Q->back = ((int32_t)back + 3) & ~3;
+    Q->na = (int32_t)floor(1.0 / b_hi);
+    Q->nb = (int32_t)ceil(1.0 / b_lo) - Q->na;
+    *smem = (size_t)(((size_t)L.n_c + Q->front + Q->back + 3) & ~(size_t)3) * sizeof(float) +
+            (size_t)8 * kAdjUThreads * sizeof(double);
+    return true;
 }
 
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
@@ -811,9 +826,9 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
     P.log_grid = in.ssp->log_lambda;
     P.dl_ssp = in.ssp->dlambda;
     P.n = L.n;
-    int na = 0, nb = 0;
-    if (adjoint_units_shape(in, &na, &nb)) {
-        AdjUParams Q;
+    AdjUParams Q;
+    size_t smem = 0;
+    if (adjoint_units_shape(in, L, &Q, &smem)) {
         Q.perm = (const int32_t *)(ws + L.off_permbuf[L.final_buf]);
         Q.totals = (const int32_t *)(ws + L.off_totals);
         Q.seg_off = (const int32_t *)(ws + L.off_seg);
@@ -833,20 +848,21 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
         Q.dl_ssp = (double)in.ssp->dlambda;
         Q.flux_scale = in.tel->flux_scale;
         Q.n = L.n;
-        const size_t smem = (size_t)(((size_t)L.n_c + kAdjUFront + kAdjUBack + 3) & ~(size_t)3) * sizeof(float) +
-                            (size_t)8 * kAdjUThreads * sizeof(double);
         const unsigned grid = (unsigned)(L.max_units * kAdjUSplit);
         const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
-        switch (na * 2 + (nb - 1)) {
-            case 0: return launch_adjoint_units<0, 1>(Q, flux, grid, smem, st);
-            case 1: return launch_adjoint_units<0, 2>(Q, flux, grid, smem, st);
-            case 2: return launch_adjoint_units<1, 1>(Q, flux, grid, smem, st);
-            case 3: return launch_adjoint_units<1, 2>(Q, flux, grid, smem, st);
-            case 4: return launch_adjoint_units<2, 1>(Q, flux, grid, smem, st);
-            case 5: return launch_adjoint_units<2, 2>(Q, flux, grid, smem, st);
-            case 6: return launch_adjoint_units<3, 1>(Q, flux, grid, smem, st);
-            default: return launch_adjoint_units<3, 2>(Q, flux, grid, smem, st);
+        if (Q.na <= 3 && Q.nb <= 2) {
+            switch (Q.na * 2 + (Q.nb - 1)) {
+                case 0: return launch_adjoint_units<0, 1>(Q, flux, grid, smem, st);
+                case 1: return launch_adjoint_units<0, 2>(Q, flux, grid, smem, st);
+                case 2: return launch_adjoint_units<1, 1>(Q, flux, grid, smem, st);
+                case 3: return launch_adjoint_units<1, 2>(Q, flux, grid, smem, st);
+                case 4: return launch_adjoint_units<2, 1>(Q, flux, grid, smem, st);
+                case 5: return launch_adjoint_units<2, 2>(Q, flux, grid, smem, st);
+                case 6: return launch_adjoint_units<3, 1>(Q, flux, grid, smem, st);
+                default: return launch_adjoint_units<3, 2>(Q, flux, grid, smem, st);
+            }
         }
+        return launch_adjoint_units<-1, 0>(Q, flux, grid, smem, st);       // step counts at run time
     }
     const int64_t threads = L.n * 32;
     auto kern = in.tel->resample == RUBIX_RESAMPLE_FLUX ? k_adjoint_flux

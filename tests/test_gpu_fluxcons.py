@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 import oracle
+from gradcheck import assert_gradients
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -137,13 +138,9 @@ def test_adjoint_config_in_flux_mode(B):
     grad_cube = torch.from_numpy((2.0 * resid).astype(np.float32)).cuda()
     g = [x.cpu().numpy().astype(np.float64) for x in dw.adjoint(grad_cube)]
     p, ssp = w.particles, w.ssp
-    key, _ = oracle.rotate_bin(p.pos, p.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    key, vlos = oracle.rotate_bin(p.pos, p.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
     ana = oracle.adjoint(p, w.rotation, ssp, t, 2.0 * resid)
-    for q in range(4):
-        scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
-        rel = np.abs(g[q] - ana[q]) / scale
-        assert np.quantile(rel, 0.999) <= 1e-3, (q, rel.max())
-        assert not g[q][key >= t.n_spaxels].any()
+    print("flux rule, max relative gradient errors:", assert_gradients(g, ana, key, vlos, ssp, t, "flux rule"))
     ok = key < t.n_spaxels
     for v, ax in ((p.log_age, ssp.log_age_axis), (p.log_z, ssp.log_z_axis)):
         ok &= (v > ax[0] + 1e-3) & (v < ax[-1] - 1e-3) & (np.abs(v[:, None] - ax[None, :]).min(1) > 1e-3)

@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 import oracle
+from gradcheck import assert_gradients
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -91,18 +92,11 @@ def test_random_configuration(B, seed):
     G = np.random.default_rng(seed).normal(size=dw.shape).astype(np.float32)
     g = [x.cpu().numpy().astype(np.float64) for x in dw.adjoint(torch.from_numpy(G).cuda())]
     ana = oracle.adjoint(w.particles, w.rotation, w.ssp, t, G.astype(np.float64))
-    inside = okey < t.n_spaxels
-    for q in range(4):
-        assert np.isfinite(g[q]).all(), (what, q)
-        assert not g[q][~inside].any(), (what, q)
-        if inside.any() and np.abs(ana[q][inside]).max() > 0:
-            med = np.median(np.abs(ana[q][inside]))
-            # The upstream gradient here is WHITE NOISE, the worst case for d/dv_los: it is then a sum of
-            # N_c terms of size (lambda / dlambda) S g that cancels to O(sqrt(N_c)).  Its absolute accuracy is
-            # set by that sum (the oracle's own analytic and finite-difference values differ by ~5e-4 of the
-            # median gradient on such inputs), not by each particle's own, possibly tiny, value: the floor is
-            # the median gradient there.  (configs[4], with a physical residual, is held to the 1e-3 floor.)
-            floor = 1.0 if q == 3 else 1e-3
-            scale = np.maximum(np.abs(ana[q]), floor * max(med, 1e-3 * np.abs(ana[q]).max()))
-            rel = np.abs(g[q] - ana[q]) / scale
-            assert np.quantile(rel, 0.99) <= 2e-3, (what, q, float(rel.max()))
+    # Maximum over all particles (readings R12 / R19).  The upstream gradient here is WHITE NOISE, which no fp32
+    # pipeline can follow down to the R12 floor: rounding G' = LSF^T PSF^T G to fp32 alone moves a gradient by up to
+    # 6e-6 of the median gradient, the fp32 convolution by up to 2e-5 (measured by feeding the oracle's adjoint the
+    # GPU's G'), because the sum over channels cancels to O(sqrt(N_c)) while the rounding does not.  The floor of the
+    # comparison is therefore 3e-2 of the median here; configs[4] and the per-feature tests, with a physical residual,
+    # are held to the 1e-3 floor.
+    _, vlos = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    assert_gradients(g, ana, okey, vlos, w.ssp, t, what, floor=3e-2)

@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
+from gradcheck import assert_gradients
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -21,35 +22,49 @@ def B():
     return binding
 
 
-def check(B, w, seed_other, want_cube):
+def check(B, w, seed_other):
+    """The fused call stage by stage (reading R19): the final cube against the oracle's (1e-4 of its maximum),
+    the loss against the oracle's loss, and the gradients -- maximum over ALL particles, 1e-3 -- against the oracle's
+    adjoint of the upstream gradient the call itself formed, 2 (cube_out - target).  (How the cube's own voxel error
+    moves a gradient is linear, Adj(2 delta), and a property of the loss, not of the kernels: a particle whose gradient
+    nearly cancels can see 1e-2 of its value from a 1e-6 voxel error; that composition is bounded below as well.)"""
     t = w.telescope
     other = synth.make_particles_for("tiny" if w.name == "tiny" else "adjoint", n=w.particles.n, seed=seed_other)
     target = oracle.forward(other, w.rotation, w.ssp, t)               # never from the CUDA path
     ref_final = oracle.forward(w.particles, w.rotation, w.ssp, t)
     target32 = target.astype(np.float32)
     dw = B.DeviceWorkload(w)
-    loss, g, cube = dw.loss_and_grad(torch.from_numpy(target32).cuda(), want_cube=want_cube)
+    loss, g, cube = dw.loss_and_grad(torch.from_numpy(target32).cuda(), want_cube=True)
     torch.cuda.synchronize()
     resid = ref_final - target32.astype(np.float64)
     L_ref = float((resid ** 2).sum())
     assert abs(float(loss.item()) - L_ref) <= 2e-4 * L_ref
-    if want_cube:
-        assert np.abs(cube.cpu().numpy() - ref_final).max() <= 1e-4 * ref_final.max()
+    got_cube = cube.cpu().numpy().astype(np.float64)
+    assert np.abs(got_cube - ref_final).max() <= 1e-4 * ref_final.max()
+    key, vlos = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    gg = [x.cpu().numpy() for x in g]
+    # gradients of the upstream gradient the call formed: maximum over all particles
+    up = (2.0 * (cube.cpu().numpy() - target32)).astype(np.float64)    # fp32 subtraction, as the kernel does it
+    ana_own = oracle.adjoint(w.particles, w.rotation, w.ssp, t, up)
+    stats = assert_gradients(gg, ana_own, key, vlos, w.ssp, t, "fused call")
+    print("fused call, max relative gradient errors:", stats)
+    # composition: against the oracle's own residual the difference is Adj(2 delta), delta = the cube's voxel error
     ana = oracle.adjoint(w.particles, w.rotation, w.ssp, t, 2.0 * resid)
-    key, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    lin = oracle.adjoint(w.particles, w.rotation, w.ssp, t, 2.0 * (got_cube - ref_final))
     for q in range(4):
-        got = g[q].cpu().numpy().astype(np.float64)
         scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
-        rel = np.abs(got - ana[q]) / scale
-        # the upstream gradient is built from the GPU's own fp32 cube here, so allow its 1e-4 voxel error
-        assert np.quantile(rel, 0.995) <= 3e-3, (q, np.quantile(rel, 0.995))
-        assert not got[key >= t.n_spaxels].any()
+        assert (np.abs(gg[q] - ana[q] - lin[q]) / np.where(scale > 0, scale, 1.0)).max() <= 1e-3
+    # without cube_out the call runs the same kernels: loss and gradients bit for bit
+    loss2, g2, none = dw.loss_and_grad(torch.from_numpy(target32).cuda(), want_cube=False)
+    assert none is None and float(loss2.item()) == float(loss.item())  # fixed-order fp64 sum: bit-reproducible
+    for a, b2 in zip(g, g2):
+        assert torch.equal(a, b2)
     # and the fused call equals the three separate calls bit for bit (same kernels, same order)
     final = dw.forward()
     grad = 2.0 * (final - torch.from_numpy(target32).cuda())
     g_sep = dw.adjoint(grad)
-    for a, b in zip(g, g_sep):
-        assert torch.equal(a, b)
+    for a, b2 in zip(g, g_sep):
+        assert torch.equal(a, b2)
     return float(loss.item())
 
 
@@ -57,15 +72,12 @@ def check(B, w, seed_other, want_cube):
 def test_config4_fused(B, mode):
     w = synth.make_workload("adjoint", n=30000)
     w.telescope = dataclasses.replace(w.telescope, resample=mode)
-    l1 = check(B, w, synth.ADJOINT_TARGET_SEED, want_cube=True)
-    l2 = check(B, w, synth.ADJOINT_TARGET_SEED, want_cube=False)
-    assert l1 == l2                                                    # fixed-order fp64 sum: bit-reproducible
+    check(B, w, synth.ADJOINT_TARGET_SEED)
 
 
 def test_without_psf_lsf(B):
     w = synth.make_workload("tiny")
-    check(B, w, synth.ADJOINT_TARGET_SEED, want_cube=True)
-    check(B, w, synth.ADJOINT_TARGET_SEED, want_cube=False)
+    check(B, w, synth.ADJOINT_TARGET_SEED)
 
 
 def test_workspace_check(B):

@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 import oracle
+from gradcheck import assert_gradients
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -135,6 +136,8 @@ def medium():
 
 
 def test_medium_full_size(B, medium):
+    """The headline workload, WHOLE cube against the oracle: the build cube (steps 1-6) and the final cube (steps 7-8),
+    every voxel; about 20 s of oracle time and 10 GB of host memory."""
     w = medium
     t = w.telescope
     dw = B.DeviceWorkload(w)
@@ -142,35 +145,56 @@ def test_medium_full_size(B, medium):
     torch.cuda.synchronize()
     okey, oseg = check_sort(dw, w)
     counts = np.diff(oseg)[:-1]
-    # every empty spaxel is exactly zero
-    empty = torch.from_numpy(counts == 0).cuda()
-    assert not cube.view(t.n_spaxels, -1)[empty].any().item()
-    # sampled spaxels the oracle computes one by one: the heaviest, a ring of busy ones, random ones
-    rng = np.random.default_rng(14)
-    order = np.argsort(counts)
-    sel = np.unique(np.concatenate([order[-12:], order[-3000:-12:250], rng.choice(np.nonzero(counts > 0)[0], 60),
-                                    rng.choice(np.nonzero(counts == 0)[0], 4)])).astype(np.int32)
-    ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t, sel=sel)
-    got = cube.view(t.n_spaxels, -1)[torch.from_numpy(sel.astype(np.int64)).cuda()].cpu().numpy()
-    # the global max of the cube is in the heaviest spaxels, which are part of the sample
-    assert counts[sel].max() == counts.max()
-    check_cube(got, ref, "medium sampled spaxels")
-    # total flux per spaxel over the WHOLE cube against a property: positive where occupied
-    sums = cube.double().sum(-1).view(-1).cpu().numpy()
-    assert (sums[counts > 0] > 0).all()
+    ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t)
+    got = cube.cpu().numpy()
+    # every empty spaxel is exactly zero (check_cube asserts it), every voxel within 1e-4 of the cube's maximum,
+    # every spaxel's flux within 1e-5
+    assert int((ref.reshape(t.n_spaxels, -1).sum(-1) > 0).sum()) == int((counts > 0).sum())
+    check_cube(got, ref, "medium whole build cube")
+    del got
 
-    # final cube (PSF + LSF) on a patch around the brightest spaxel
     final = dw.convolve(cube)
     torch.cuda.synchronize()
-    bx, by = divmod(int(order[-1]), t.n_y)
-    bx, by = int(np.clip(bx, 12, t.n_x - 13)), int(np.clip(by, 12, t.n_y - 13))
-    xs, ys = np.arange(bx - 10, bx + 11), np.arange(by - 10, by + 11)
-    patch_sel = (xs[:, None] * t.n_y + ys[None, :]).reshape(-1).astype(np.int32)
-    patch = oracle.build_cube(w.particles, w.rotation, w.ssp, t, sel=patch_sel).reshape(21, 21, -1)
-    conv = oracle.convolve(patch, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)[7:14, 7:14]
-    gotp = final[bx - 3:bx + 4, by - 3:by + 4].cpu().numpy().astype(np.float64)
-    assert np.abs(gotp - conv).max() <= VOXEL_TOL * conv.max()
-    assert np.allclose(gotp.sum(-1), conv.sum(-1), rtol=FLUX_TOL)
+    ref_final = oracle.convolve(ref, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)
+    del ref
+    gotf = final.cpu().numpy()
+    scale = ref_final.max()
+    err = 0.0
+    for x0 in range(0, t.n_x, 50):                         # in slabs: keeps the fp64 temporaries small
+        d = gotf[x0:x0 + 50].astype(np.float64) - ref_final[x0:x0 + 50]
+        err = max(err, float(np.abs(d).max()))
+        fs, fr = gotf[x0:x0 + 50].astype(np.float64).sum(-1), ref_final[x0:x0 + 50].sum(-1)
+        assert np.allclose(fs, fr, rtol=FLUX_TOL, atol=FLUX_TOL * float(ref_final.sum(-1).max()))
+    assert err <= VOXEL_TOL * scale, f"medium whole final cube: max err {err:.3e} vs {VOXEL_TOL * scale:.3e}"
+
+
+def test_forward_host_entries_against_the_oracle(B, small, small_oracle_cube):
+    """rubix_forward_host and rubix_forward_host_pipelined (the calls bench.py's e2e leg times), HOST buffers in and
+    out, compared with the oracle directly: config 1 as is (no PSF/LSF) and with config 2's PSF/LSF."""
+    p = small.particles
+    for tel, ref in ((small.telescope, small_oracle_cube),
+                     (small.telescope.with_psf_lsf(), None)):
+        if ref is None:
+            ref = oracle.convolve(small_oracle_cube, tel.psf_size, tel.psf_sigma, tel.lsf_size, tel.lsf_sigma)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hp = [pin(x) for x in (p.pos, p.vel, p.mass, p.log_age, p.log_z)]
+        hflux = pin(small.ssp.flux)
+        cp, cs, ct = B.c_particles(*hp), B.c_ssp(small.ssp, hflux), B.c_telescope(tel)
+        shape = (tel.n_x, tel.n_y, tel.n_channels)
+        scratch = torch.empty(B.rubix_forward_host_pipelined_scratch_bytes(p.n, cs, ct), dtype=torch.uint8, device="cuda")
+        h1 = torch.full(shape, float("nan"), dtype=torch.float32).pin_memory()
+        B.rubix_forward_host(cp, cs, ct, small.rotation, h1, scratch)
+        torch.cuda.synchronize()
+        h2 = [torch.full(shape, float("nan"), dtype=torch.float32).pin_memory() for _ in range(3)]
+        for h in h2:                                       # three back-to-back cubes through the pipeline
+            B.rubix_forward_host_pipelined(cp, cs, ct, small.rotation, h, scratch)
+        B.rubix_forward_host_drain()
+        torch.cuda.synchronize()
+        for h in [h1] + h2:
+            got = h.numpy().astype(np.float64)
+            assert np.isfinite(got).all()
+            assert np.abs(got - ref).max() <= VOXEL_TOL * ref.max()
+            assert np.allclose(got.sum(-1), ref.sum(-1), rtol=FLUX_TOL, atol=FLUX_TOL * ref.sum(-1).max())
 
 
 # ------------------------------------------------------------------ config 3: contention
@@ -235,10 +259,7 @@ def test_adjoint_config(B):
         scale = np.maximum(np.abs(fd[q]), 1e-3 * np.median(np.abs(fd[q])))
         rel = np.abs(g[q][idx] - fd[q]) / scale
         assert rel.max() <= 1e-3, (q, rel.max())
-    # all particles against the oracle's analytic adjoint
+    # ALL particles against the oracle's analytic adjoint: maximum, not a percentile (readings R12 / R19)
     ana = oracle.adjoint(p, w.rotation, ssp, t, 2.0 * resid)
-    for q in range(4):
-        scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
-        rel = np.abs(g[q] - ana[q]) / scale
-        assert np.quantile(rel, 0.999) <= 1e-3, (q, rel.max())
-        assert not g[q][key >= t.n_spaxels].any()
+    stats = assert_gradients(g, ana, key, vlos, ssp, t, "configs[4]")
+    print("configs[4] max relative gradient errors (excluded):", stats)

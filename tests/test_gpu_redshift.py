@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
+from gradcheck import assert_gradients, upstream_gradient
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -64,15 +65,11 @@ def test_adjoint_with_redshift_and_scale(B, mode):
     w.telescope = shifted(w.telescope, 0.08, 2.5e-2, mode)
     t = w.telescope
     dw = B.DeviceWorkload(w)
-    G = np.random.default_rng(9).normal(size=(t.n_x, t.n_y, t.n_channels)).astype(np.float32)
+    G = upstream_gradient(w)                               # 2 (cube - target) of two galaxies, as in configs[4]
     g = [x.cpu().numpy().astype(np.float64) for x in dw.adjoint(torch.from_numpy(G).cuda())]
     ana = oracle.adjoint(w.particles, w.rotation, w.ssp, t, G.astype(np.float64))
-    key, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
-    for q in range(4):
-        scale = np.maximum(np.abs(ana[q]), 1e-3 * np.median(np.abs(ana[q][key < t.n_spaxels])))
-        rel = np.abs(g[q] - ana[q]) / scale
-        assert np.quantile(rel, 0.999) <= 1e-3, (mode, q, rel.max())
-        assert not g[q][key >= t.n_spaxels].any()
+    key, vlos = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
+    assert_gradients(g, ana, key, vlos, w.ssp, t, "test_gpu_redshift.py")
 
 
 def test_bad_redshift_and_scale_are_rejected(B):
