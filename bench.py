@@ -13,10 +13,11 @@ BASELINE.json configs[2] "medium (headline)": 1 M star particles, SSP 50x7x4300,
                arrays + SSP grid and D2H of the final cube inside the timed region
   roofline     the dominant kernel (k_accumulate), its time from CUDA event pairs recorded by the
                library on the launching stream inside the timed region
-  cpu_baseline the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
+  cpu_baseline the fp64 oracle, as it stands, on this box's host cores, on the WHOLE workload (1 warm-up + 3 timed
+               cubes, mean and best; nproc and CPU model; single-thread time of the tiny and small configs)
 N > 1 (torchrun): replicas only -- every rank builds its own galaxy (seed + rank); no collective
 on the data path; time = max over ranks.
---impl reference times the oracle (this tier's reference arm) on rank 0 only.
+--impl reference times the oracle (this tier's reference arm) on rank 0 only; every step is the whole workload.
 """
 from __future__ import annotations
 
@@ -39,6 +40,8 @@ GATHER_BYTES_PER_SAMPLE = lambda tel, ssp: 16.0 * float(tel.dlambda) / float(ssp
 # DRAM bytes of one k_accumulate launch on the medium workload, from the committed ncu --set full
 # capture (profiles/r01_full_medium.md): 0.053 GB read + 1.347 GB written
 NCU_DRAM_BYTES_K_ACCUMULATE = 1.400e9
+NCU_TRAFFIC_SOURCE = ("STATIC: dram__bytes_read.sum + dram__bytes_write.sum of one k_accumulate launch in the committed "
+                      "ncu --set full capture profiles/r01_full_medium.md; not measured in this run")
 
 
 def parse():
@@ -68,35 +71,71 @@ def workload_config(w):
 
 
 # ------------------------------------------------------------------------------------- oracle arm
-def oracle_sample_time(w, n_sample, patch):
-    """Oracle (fp64, as it stands) on a bounded sample of the workload: the first ``n_sample``
-    particles through build, and PSF/LSF on a ``patch`` x ``patch`` spaxel sub-cube.  Returns the
-    extrapolated seconds per full cube and a description."""
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_step(w):
+    """One step of the oracle (fp64, as it stands) on the WHOLE workload: build + PSF/LSF.  Seconds."""
     import oracle
     t = w.telescope
-    sub = w.particles.subset(slice(0, n_sample))
     t0 = time.perf_counter()
-    cube = oracle.build_cube(sub, w.rotation, w.ssp, t)
-    t_build = time.perf_counter() - t0
-    t_conv, frac_conv = 0.0, 1.0
+    cube = oracle.build_cube(w.particles, w.rotation, w.ssp, t)
     if t.psf_size > 0 or t.lsf_size > 0:
-        px = min(patch, t.n_x)
-        py = min(patch, t.n_y)
-        x0, y0 = (t.n_x - px) // 2, (t.n_y - py) // 2
-        piece = np.ascontiguousarray(cube[x0:x0 + px, y0:y0 + py])
-        t0 = time.perf_counter()
-        oracle.convolve(piece, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)
-        t_conv = time.perf_counter() - t0
-        frac_conv = (px * py) / float(t.n_x * t.n_y)
+        cube = oracle.convolve(cube, t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma)
+    dt = time.perf_counter() - t0
     del cube
-    full = t_build * (w.particles.n / float(n_sample)) + t_conv / frac_conv
-    desc = (f"oracle build on the first {n_sample} of {w.particles.n} particles ({t_build:.2f} s) + oracle "
-            f"PSF/LSF on a central {min(patch, t.n_x)}x{min(patch, t.n_y)}-spaxel sub-cube ({t_conv:.2f} s), "
-            f"scaled to the full workload: {full:.1f} s per cube")
-    return full, t_build + t_conv, desc
+    return dt
+
+
+def oracle_single_thread(names=("tiny", "small")):
+    """Single-thread oracle time of the small parity configs (BASELINE.md "CPU-baseline plan"), in a child process
+    because the OpenMP thread count is fixed at library load."""
+    import subprocess
+    code = ("import sys, json, time; sys.path.insert(0, %r); import oracle; from paper_2412_08265_b200 import synth\n"
+            "out = {}\n"
+            "for name in %r:\n"
+            "    w = synth.make_workload(name); t = w.telescope\n"
+            "    oracle.build_cube(w.particles, w.rotation, w.ssp, t)\n"
+            "    t0 = time.perf_counter(); oracle.build_cube(w.particles, w.rotation, w.ssp, t)\n"
+            "    out[name] = {'seconds_per_cube': time.perf_counter() - t0, 'samples': w.particles.n * t.n_channels}\n"
+            "print(json.dumps(out))\n") % (ROOT, tuple(names))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        res = json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as exc:                                   # reported, never fatal for the bench line
+        return {"error": repr(exc)}
+    for v in res.values():
+        v["value"] = v["samples"] / v["seconds_per_cube"] / 1e9
+        v["unit"] = UNIT
+    return res
+
+
+def cpu_baseline_block(w, repeats=3):
+    """The oracle timed on this box's host cores on the whole workload: one warm-up, then `repeats` cubes."""
+    import oracle
+    oracle.build()
+    oracle_step(w)
+    secs = [oracle_step(w) for _ in range(repeats)]
+    n_samples = w.particles.n * w.telescope.n_channels
+    best, mean = min(secs), float(np.mean(secs))
+    return {"value": n_samples / mean / 1e9, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+            "sample": f"the WHOLE {w.name} workload (all {w.particles.n} particles, build + PSF/LSF of the full cube), "
+                      f"1 warm-up + {repeats} timed cubes, no extrapolation",
+            "seconds_per_cube": mean, "seconds_per_cube_best": best, "seconds_per_cube_all": secs,
+            "value_best": n_samples / best / 1e9, "nproc": os.cpu_count(), "cpu_model": cpu_model(),
+            "single_thread": oracle_single_thread()}
 
 
 def run_reference(args):
+    """--impl reference: the oracle alone, every step the whole workload (no sampling, no scaling)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -104,22 +143,22 @@ def run_reference(args):
     from paper_2412_08265_b200 import synth
     oracle.build()
     w = synth.make_workload(args.workload)
-    n_sample = min(w.particles.n, 50_000)
-    for _ in range(max(args.warmup, 0) and 1):            # one warm-up is plenty for a CPU loop
-        oracle_sample_time(w, min(n_sample, 10_000), 16)
-    secs = []
-    desc = ""
-    for _ in range(args.steps):
-        full, _, desc = oracle_sample_time(w, n_sample, 32)
-        secs.append(full)
+    for _ in range(max(args.warmup, 0)):
+        oracle_step(w)
+    secs = [oracle_step(w) for _ in range(args.steps)]
     t_step = float(np.mean(secs))
-    value = w.particles.n * w.telescope.n_channels / t_step / 1e9
+    n_samples = w.particles.n * w.telescope.n_channels
+    value = n_samples / t_step / 1e9
     cores = oracle.n_threads()
+    desc = (f"the WHOLE {w.name} workload per step (all {w.particles.n} particles, build + PSF/LSF of the full cube); "
+            f"{args.warmup} warm-up + {args.steps} timed steps, mean {t_step:.2f} s, best {min(secs):.2f} s")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(w),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                             "seconds_per_cube": t_step, "seconds_per_cube_best": min(secs),
+                             "nproc": os.cpu_count(), "cpu_model": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -173,7 +212,7 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def time_adjoint(B, synth, dev, reps=10):
+def time_adjoint(B, synth, dev, l2_peak, reps=10):
     """rubix_cube_adjoint on BASELINE.json configs[4]: the config-1 galaxy with
     config-2 PSF/LSF, upstream gradient 2 (cube - target); reported beside the headline step."""
     import torch
@@ -198,7 +237,9 @@ def time_adjoint(B, synth, dev, reps=10):
     adj_ms = e0.elapsed_time(e1) / reps
     t, n = w.telescope, w.particles.n
     k_ms = st["adjoint"]["ms"] / max(st["adjoint"]["calls"], 1)
-    gather_b = 32.0 * n * t.n_channels                    # 4 corners x (T[j], T[j+1]) x 4 B per sample
+    n_in = int(dw.sort_artifacts()[2][t.n_spaxels].item())          # in-FoV particles (the others do no work)
+    # "as K3 per sample": the four corner rows over the particle's window, read once
+    gather_b = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * n_in * t.n_channels
     # fused forward + loss + adjoint (rubix_loss_and_grad): one particle pass, loss reduced on the device
     target = dt.forward()
     for _ in range(3):
@@ -214,8 +255,12 @@ def time_adjoint(B, synth, dev, reps=10):
             "loss_and_grad_ms_per_call": fused_ms, "loss": float(loss.item()),
             "ms_per_call": adj_ms, "k_adjoint_ms": k_ms,
             "value": n * t.n_channels / (adj_ms * 1e-3) / 1e9, "unit": UNIT,
-            "note": "k_adjoint reads 8 template samples per (particle, channel) through L1 (32 B algorithmic)",
-            "l1_gather_gbs": gather_b / (k_ms * 1e-3) / 1e9}
+            "in_fov_particles": n_in,
+            "roofline": {"kernel": "k_adjoint_units (step 9)", "bound": "l2", "achieved": gather_b / (k_ms * 1e-3) / 1e9,
+                         "peak": l2_peak, "unit": "GB/s", "frac": gather_b / (k_ms * 1e-3) / 1e9 / l2_peak,
+                         "algorithmic_bytes_per_launch": gather_b, "kernel_ms": k_ms,
+                         "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks (builder-measured: "
+                                        "MEASURED_PEAKS.json has no L2 figure)"}}
 
 
 # ------------------------------------------------------------------------------------- our arm
@@ -282,8 +327,28 @@ def run_ours(args):
     B.rubix_stage_timing_enable(False)
     elapsed_ms = replicas.max_over_ranks(elapsed_ms, dev)
     ms_per_step = elapsed_ms / args.steps
+    n_in = int(dw.sort_artifacts()[2][t.n_spaxels].item())          # particles inside the field of view
     samples_per_step = float(n) * t.n_channels
     value = replicas.whole_job_value(samples_per_step, world, elapsed_ms, args.steps) / 1e9
+
+    # ---- step 9 on the bench workload itself (outside the timed step): rubix_cube_adjoint with the final cube as the
+    #      upstream gradient; the kernel's time per 1e6 in-FoV particles
+    adjoint_workload = None
+    if has_conv and not args.no_adjoint and rank == 0:
+        for _ in range(2):
+            dw.adjoint(final)
+        torch.cuda.synchronize()
+        B.rubix_stage_timing_enable(True)
+        B.rubix_stage_timing_read()
+        for _ in range(5):
+            dw.adjoint(final)
+        torch.cuda.synchronize()
+        st_a = B.rubix_stage_timing_read()
+        B.rubix_stage_timing_enable(False)
+        k_ms = st_a["adjoint"]["ms"] / max(st_a["adjoint"]["calls"], 1)
+        adjoint_workload = {"what": f"rubix_cube_adjoint on the {w.name} workload (upstream gradient = the final cube)",
+                            "k_adjoint_ms": k_ms, "in_fov_particles": n_in, "ms_per_1e6_particles": k_ms * 1e6 / max(n_in, 1),
+                            "psf_lsf_transpose_ms": st_a["psf_lsf"]["ms"] / max(st_a["psf_lsf"]["calls"], 1)}
 
     # ---- end to end through the host-buffer entry point
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -330,32 +395,50 @@ def run_ours(args):
         scratch = torch.empty(1 << 30, dtype=torch.uint8, device=dev)
     onchip = B.rubix_measure_peaks(scratch)
     acc_ms = stages["accumulate"]["ms"] / max(stages["accumulate"]["calls"], 1)
-    gather_b = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * samples_per_step
-    hbm_b = t.n_spaxels * t.n_channels * 4.0 + w.ssp.flux.size * 4.0 + 48.0 * n
+    # algorithmic bytes count the in-FoV particles only (the dropped ones sort last and do no work)
+    samples_in = float(n_in) * t.n_channels
+    gather_b = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * samples_in
+    hbm_b = t.n_spaxels * t.n_channels * 4.0 + w.ssp.flux.size * 4.0 + 48.0 * n_in
     achieved = gather_b / (acc_ms * 1e-3) / 1e9
     # L1 data-pipe view (the unit ncu shows saturated, profiles/r01_full_medium.md): bytes the SM's
     # load/store pipe must carry per particle = 4 corner windows (LDG) + table store (STS) + two
     # table reads per channel (LDS); peak = the shared-memory read bandwidth measured in this run
     win = float(t.n_channels) * float(t.dlambda) / float(w.ssp.dlambda)
-    l1_b = (16.0 * win + 4.0 * win + 8.0 * t.n_channels) * n
+    l1_b = (16.0 * win + 4.0 * win + 8.0 * t.n_channels) * n_in
     l1_peak = onchip["smem_gbs"]
     roofline = {"kernel": "k_accumulate (steps 4-6)", "bound": "l2", "achieved": achieved,
                 "peak": onchip["l2_gbs"], "unit": "GB/s", "frac": achieved / onchip["l2_gbs"],
                 "traffic": NCU_DRAM_BYTES_K_ACCUMULATE if args.workload == "medium" else None,
-                "traffic_source": "profiles/r01_full_medium.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
+                "traffic_source": NCU_TRAFFIC_SOURCE,
+                "in_fov_particles": n_in,
                 "l1_view": {"bound": "l1 data pipe", "achieved": l1_b / (acc_ms * 1e-3) / 1e9, "peak": l1_peak,
                             "unit": "GB/s", "frac": l1_b / (acc_ms * 1e-3) / 1e9 / l1_peak,
                             "peak_source": "shared-memory / L1 data-pipe read bandwidth measured in this run by rubix_measure_peaks "
                                            "(nominal 148 SMs x 128 B/clk x 1.965 GHz = 37.2 TB/s)",
                             "algorithmic_bytes_per_launch": l1_b},
-                "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks "
-                               "(MEASURED_PEAKS.json has no L2 figure; SURVEY.md 8(d))",
+                "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks: BUILDER-measured "
+                               "(ld.global.cg over a 32 MiB buffer), not a driver-written figure -- MEASURED_PEAKS.json has "
+                               "no L2 entry (SURVEY.md 8(d))",
                 "algorithmic_bytes_per_launch": gather_b, "kernel_ms": acc_ms,
                 "hbm_view": {"bound": "hbm", "achieved": hbm_b / (acc_ms * 1e-3) / 1e9, "peak": hbm_peak,
                              "unit": "GB/s", "frac": hbm_b / (acc_ms * 1e-3) / 1e9 / hbm_peak,
                              "peak_source": hbm_src, "algorithmic_bytes_per_launch": hbm_b},
                 "measured_peaks": onchip}
     stage_ms = {k: (v["ms"] / max(v["calls"], 1) if v["calls"] else 0.0) for k, v in stages.items()}
+    # ---- whole-step roofline: t_roof = sum over the stages of max(HBM, on-chip gather, ALU) time
+    conv_bytes = 2.0 * t.n_spaxels * t.n_channels * 4.0 if has_conv else 0.0
+    pass_bytes = (28.0 + 2 * 16.0 + 48.0 + 16.0) * n + 2.0 * w.ssp.flux.size * 4.0   # arrays in, 2 sort passes, records, grid copy
+    terms = {"particle_pass": {"hbm_ms": pass_bytes / hbm_peak / 1e6},
+             "accumulate": {"hbm_ms": hbm_b / hbm_peak / 1e6, "l2_gather_ms": gather_b / onchip["l2_gbs"] / 1e6,
+                            "alu_ms": 14.0 * samples_in / (onchip["fma_tflops"] * 1e12) * 1e3},
+             "psf_lsf": {"hbm_ms": conv_bytes / hbm_peak / 1e6}}
+    t_roof = sum(max(v.values()) for v in terms.values())
+    whole_step = {"t_roof_ms": t_roof, "ms_per_step": ms_per_step, "frac": t_roof / ms_per_step, "terms": terms,
+                  "hbm_only_ms": sum(v["hbm_ms"] for v in terms.values()),
+                  "what": "sum over the stages of max(HBM bytes / HBM peak, L2 gather bytes / L2 peak, flops / fp32 peak) "
+                          "divided by the measured step (SURVEY.md 8(d); north_star's >= 50 % is judged on this)",
+                  "peaks": {"hbm_gbs": hbm_peak, "hbm_source": hbm_src, "l2_gbs": onchip["l2_gbs"],
+                            "fma_tflops": onchip["fma_tflops"], "on_chip_source": "builder-measured in this run"}}
     if has_conv:
         conv_b = 2.0 * t.n_spaxels * t.n_channels * 4.0
         roofline["psf_lsf"] = {"bound": "hbm", "achieved": conv_b / (stage_ms["psf_lsf"] * 1e-3) / 1e9,
@@ -440,7 +523,7 @@ def run_ours(args):
     adjoint_info = None
     if not args.no_adjoint:
         del scratch
-        adjoint_info = time_adjoint(B, synth, dev)
+        adjoint_info = time_adjoint(B, synth, dev, onchip["l2_gbs"])
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -453,21 +536,21 @@ def run_ours(args):
                     "serial": {"value": e2e_serial_value, "ms_per_step": e2e_serial_ms, "api": "rubix_forward_host"}},
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
             "stage_ms": stage_ms, "roofline": roofline}
+    line["roofline"]["whole_step"] = whole_step
     line["flux_variant"] = flux_variant
     if table_variant is not None:
         line["log_grid_variant"] = table_variant
     if noise_info is not None:
         line["noise_stage"] = noise_info
     if adjoint_info is not None:
+        if adjoint_workload is not None:
+            adjoint_info["on_bench_workload"] = adjoint_workload
+            gb = GATHER_BYTES_PER_SAMPLE(t, w.ssp) * n_in * t.n_channels
+            adjoint_workload["l2_frac"] = gb / (adjoint_workload["k_adjoint_ms"] * 1e-3) / 1e9 / onchip["l2_gbs"]
         line["adjoint"] = adjoint_info
 
     if not args.no_cpu_baseline:
-        import oracle
-        oracle.build()
-        full, spent, desc = oracle_sample_time(base, min(n, 300_000), 64)
-        line["cpu_baseline"] = {"value": n * t.n_channels / full / 1e9, "unit": UNIT,
-                                "cores": oracle.n_threads(), "kind": "oracle", "sample": desc,
-                                "seconds_per_cube": full}
+        line["cpu_baseline"] = cpu_baseline_block(base)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
