@@ -421,7 +421,11 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     r.j0 = 0;
     r.nw = 0;
     if (k_lo <= k_hi) {
-        r.j0 = (int32_t)(x_first >> kFxFrac) & ~(kRowAlign - 1);
+        // table mode: k_accumulate<LOGX> adds separately truncated terms and may land up to 2 units of 2^-20 below
+        // x_first; the window starts one group earlier when x_first is that close above a multiple of kRowAlign
+        // (at j0 = 0 the kernel clamps at the knot instead)
+        const int64_t x_j0 = P.table ? (x_first > 1024 ? x_first - 1024 : 0) : x_first;
+        r.j0 = (int32_t)(x_j0 >> kFxFrac) & ~(kRowAlign - 1);
         r.nw = (int32_t)(x_last >> kFxFrac) - r.j0 + 2;   // samples j0 .. j_max + 1
     }
     rec[i] = r;

@@ -168,7 +168,9 @@ k_accumulate(const __grid_constant__ AccumParams P)
                         xa = max(xa, (int64_t)0);
                         xb = min(xb, (int64_t)(P.n_lambda - 1) << kFxFrac);
                     }
-                    j0 = (int)(xa >> kFxFrac) & ~(kRowAlign - 1);
+                    // LOGX: the resampler's x may sit up to 2 units of 2^-20 below the exact value, so the window
+                    // starts one group earlier when x_ka is that close above a multiple of kRowAlign
+                    j0 = (int)(max(xa - (LOGX ? 1024 : 0), (int64_t)0) >> kFxFrac) & ~(kRowAlign - 1);
                     W.nw = (int)(xb >> kFxFrac) - j0 + 2;   // samples j0 .. j_max + 1
                 }
             }
@@ -306,14 +308,21 @@ k_accumulate(const __grid_constant__ AccumParams P)
             // 12.20 local fixed point: exact truncation of the 36.28 value (channel stride 128 b / 256 = b / 2, b is even)
             // LOGX: x = (tile-relative table value of the channel) x c + (particle base), truncated to 2^-20
             const uint32_t x0 = LOGX ? (uint32_t)(W.base >> 8) : (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
-            if (W.ka == k0 && W.kb == k_end) {              // whole tile inside the SSP coverage
+            // LOGX: the sum of separately truncated terms can sit 1-2 units of 2^-20 BELOW the exact x_k that
+            // k_prepare_records used for k_lo.  Where the window starts at knot 0 (j0 = 0) a channel just above
+            // the knot would wrap below zero: such windows take the guarded branch, which clamps at the knot.
+            if (W.ka == k0 && W.kb == k_end && !(LOGX && W.j0 == 0)) {   // whole tile inside the SSP coverage
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * (W.b >> 1), bytes);
             } else {
 #pragma unroll
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k >= W.ka && k <= W.kb) sample(i, LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * (W.b >> 1), bytes);
+                    if (k >= W.ka && k <= W.kb) {
+                        uint32_t x = LOGX ? x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30) : x0 + (uint32_t)i * (W.b >> 1);
+                        if (LOGX) x = x >= 0xFFF00000u ? 0u : x;   // entry 4095 is never addressed: a wrap below 0
+                        sample(i, x, bytes);
+                    }
                 }
             }
         };
@@ -408,7 +417,7 @@ static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsign
     return flux ? launch_acc2<CPT, false, true>(P, grid, smem, st) : launch_acc2<CPT, false, false>(P, grid, smem, st);
 }
 
-// Largest CPT in {15, 8, 4, 2, 1} whose table fits the 12.20 format; returns the table capacity
+// Largest CPT in {29, 15, 8, 4, 2, 1} whose table fits the 12.20 format; returns the table capacity
 // (samples, a whole number of passes).
 int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 {

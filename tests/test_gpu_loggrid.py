@@ -79,6 +79,63 @@ def test_coverage_edges_redshift_and_fast_particles(B):
     run_and_check(B, w, "fast particles")
 
 
+def _knot_sweep_workload(ssp, tel, k_star, j_star, half=220):
+    """One particle per spaxel, identity rotation, v_los = v_z swept in steps of ~1e-7 SSP samples (or one fp32 ulp of
+    v_los, if that is coarser) around the velocity that puts channel k_star's rest position exactly on SSP knot j_star
+    (log-sampled grid: x_k = log10(lambda_k / lambda0) / d - log10(1 + beta) / d)."""
+    lam_k = float(tel.wavelengths()[k_star])
+    d, l0 = float(ssp.dlambda), float(ssp.lambda0)
+    beta = lam_k / (l0 * 10.0 ** (j_star * d)) - 1.0
+    v0 = np.float32(beta * synth.C_KMS)
+    dv = max(1e-7 * d * np.log(10.0) * synth.C_KMS, float(np.spacing(np.abs(v0))))      # 1e-7 samples per step
+    v = (np.float64(v0) + dv * np.arange(-half, half + 1)).astype(np.float32)
+    n = v.size
+    assert n <= tel.n_x * tel.n_y
+    ix, iy = np.divmod(np.arange(n), tel.n_y)
+    pos = np.zeros((n, 3), np.float32)
+    pos[:, 0] = (ix + 0.5 - 0.5 * tel.n_x) * float(tel.spaxel_size)
+    pos[:, 1] = (iy + 0.5 - 0.5 * tel.n_y) * float(tel.spaxel_size)
+    vel = np.zeros((n, 3), np.float32)
+    vel[:, 2] = v
+    rng = np.random.default_rng(77)
+    p = synth.Particles(pos, vel, rng.uniform(0.5e5, 2e5, n).astype(np.float32),
+                        rng.uniform(ssp.log_age_axis[0], ssp.log_age_axis[-1], n).astype(np.float32),
+                        rng.uniform(ssp.log_z_axis[0], ssp.log_z_axis[-1], n).astype(np.float32))
+    return synth.Workload("knot-sweep", p, ssp, tel, np.eye(3, dtype=np.float32), (0.0, 0.0, 0.0))
+
+
+@pytest.mark.parametrize("case", ["first covered channel on knot 0 (detector starts blueward of the grid)",
+                                  "channel 0 on a knot that is a multiple of 32",
+                                  "first channel of a later tile on a multiple of 32"])
+def test_channel_within_a_fixed_point_unit_of_the_window_start(B, case):
+    """ADVICE r01 (spectral.cu, table mode): the resampler adds separately truncated 2^-20 terms and may sit 1-2 units
+    BELOW the exact x_k; with x_k within ~2e-6 samples above the first sample of the staged window that wrapped below
+    zero and read a table entry outside the window.  Deterministic sweep: 441 particles whose x_k differ by ~1e-7
+    samples, centred on the velocity that puts the critical channel exactly on the knot."""
+    ssp = log_ssp("tiny")
+    d = float(ssp.dlambda)
+    if case.startswith("first covered"):
+        tel = synth.Telescope(21, 21, np.float32(1.0), 700, np.float32(3000.0), np.float32(10.0))
+        k_star = int(np.searchsorted(tel.wavelengths(), 3500.0 * 1.0005))     # first channel redward of knot 0
+        w = _knot_sweep_workload(ssp, tel, k_star, 0)
+    elif case.startswith("channel 0"):
+        lam0 = np.float32(3500.0 * 10.0 ** (160.02 * d))
+        tel = synth.Telescope(21, 21, np.float32(1.0), 256, lam0, np.float32(18.0))
+        w = _knot_sweep_workload(ssp, tel, 0, 160)
+    else:
+        k_star = 1024                                                          # tiles of 8 x 128 channels
+        lam0 = np.float32(3500.0 * 10.0 ** (224.02 * d) - 0.9 * k_star)        # puts x_1024 just above knot 224 = 7 x 32
+        tel = synth.Telescope(21, 21, np.float32(1.0), 5000, lam0, np.float32(0.9))
+        w = _knot_sweep_workload(ssp, tel, k_star, 224)
+    assert np.abs(w.particles.vel[:, 2]).max() < 0.05 * synth.C_KMS
+    got, ref = run_and_check(B, w, case)
+    # every particle is alone in its spaxel: the bound holds per particle spectrum, not only against the cube maximum
+    n = w.particles.n
+    g2 = got.reshape(-1, got.shape[-1])[:n]
+    r2 = ref.reshape(-1, ref.shape[-1])[:n]
+    assert (np.abs(g2 - r2).max(1) <= 1e-4 * r2.max(1)).all(), case
+
+
 def test_adjoint(B):
     w = synth.make_workload("adjoint", n=20000)
     w.ssp = log_ssp("small")
