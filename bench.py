@@ -293,12 +293,14 @@ def run_ours(args):
     has_conv = t.psf_size > 0 or t.lsf_size > 0
     launches_per_step = [0]
 
-    def step():
-        B.rubix_build_cube(dw.particles, dw.ssp, dw.tel, dw.R, cube, dw.workspace)
+    def step():                                               # steps 1-8 in one device call
+        B.rubix_forward(dw.particles, dw.ssp, dw.tel, dw.R, final, dw.workspace)
         launches_per_step[0] = B.rubix_last_launch_count()
+
+    def step_two_calls():                                     # the same path as two plain calls (dense raw cube)
+        B.rubix_build_cube(dw.particles, dw.ssp, dw.tel, dw.R, cube, dw.workspace)
         if has_conv:
             B.rubix_convolve_psf_lsf(dw.tel, cube, final, dw.workspace)
-            launches_per_step[0] += B.rubix_last_launch_count()
 
     def barrier():
         torch.cuda.synchronize()
@@ -330,6 +332,18 @@ def run_ours(args):
     n_in = int(dw.sort_artifacts()[2][t.n_spaxels].item())          # particles inside the field of view
     samples_per_step = float(n) * t.n_channels
     value = replicas.whole_job_value(samples_per_step, world, elapsed_ms, args.steps) / 1e9
+
+    # ---- the same step as rubix_build_cube + rubix_convolve_psf_lsf (no occupancy masks), for comparison
+    for _ in range(2):
+        step_two_calls()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        step_two_calls()
+    e1.record()
+    torch.cuda.synchronize()
+    two_call_ms = e0.elapsed_time(e1) / 5
+    step()                                                    # `final` holds the fused call's cube again
 
     # ---- step 9 on the bench workload itself (outside the timed step): rubix_cube_adjoint with the final cube as the
     #      upstream gradient; the kernel's time per 1e6 in-FoV particles
@@ -535,7 +549,10 @@ def run_ours(args):
                            "overlaps the H2D and compute of cube i + 1)",
                     "serial": {"value": e2e_serial_value, "ms_per_step": e2e_serial_ms, "api": "rubix_forward_host"}},
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
-            "stage_ms": stage_ms, "roofline": roofline}
+            "stage_ms": stage_ms, "roofline": roofline,
+            "api": "rubix_forward (steps 1-8 in one device call; occupancy-masked PSF/LSF passes)",
+            "two_calls": {"ms_per_step": two_call_ms,
+                          "api": "rubix_build_cube + rubix_convolve_psf_lsf (dense raw cube, no masks; 5 steps)"}}
     line["roofline"]["whole_step"] = whole_step
     line["flux_variant"] = flux_variant
     if table_variant is not None:

@@ -20,8 +20,11 @@
  *     read before the call returns and may be freed right after it.
  *     Consequently a sequence of calls can be captured in a CUDA graph (stage timing of
  *     rubix_peaks.h off) and replayed; the kernels read their sizes from the workspace, not
- *     from the host, after the call has returned.  (Exception: with rubix_telescope.lambda_obs the call
- *     copies that host array to the workspace; capture it only from pinned memory that stays alive.)
+ *     from the host, after the call has returned.  NOT capturable: calls with rubix_telescope.lambda_obs
+ *     (the host array is copied to the workspace) and calls that apply a wavelength-dependent PSF
+ *     (psf_alpha != 0 with psf_size > 0: the per-channel taps are computed on the host and copied from
+ *     pageable memory); the rubix_forward_host* entries (host buffers).
+ *   - Every compute call is bracketed by an NVTX range carrying its name (visible in Nsight timelines).
  *   - Device arrays are dense, row-major, fp32 / int32 as stated, 16-byte aligned.
  *   - Errors: every call validates its arguments on the host BEFORE any launch and returns a
  *     rubix_status; nothing throws or aborts.  rubix_last_error() gives a thread-local message.
@@ -63,6 +66,8 @@ typedef struct {
 /* SSP template library ("lookup from a simple stellar population (SSP) library").
  * Limits: n_age <= 512, n_z <= 128, n_age*n_z*n_lambda < 2^31. */
 typedef struct {
+    uint32_t struct_size;           /* = sizeof(rubix_ssp) of the header the CALLER was built against; a mismatch */
+                                    /* is refused with RUBIX_ERR_INVALID_ARG (the struct grows with the library)    */
     int32_t n_age, n_z, n_lambda;   /* each >= 2                                            */
     const float *log_age_axis;      /* HOST [n_age], strictly increasing                    */
     const float *log_z_axis;        /* HOST [n_z],   strictly increasing                    */
@@ -77,6 +82,7 @@ typedef struct {
 
 /* Detector ("telescope-specific configurations", L44 Gaussian PSF and LSF). */
 typedef struct {
+    uint32_t struct_size;           /* = sizeof(rubix_telescope), checked like rubix_ssp.struct_size */
     int32_t n_x, n_y;               /* spaxels; FoV centred on the origin                   */
     float spaxel_size;              /* kpc, > 0                                             */
     int32_t n_channels;             /* >= 1                                                 */
@@ -100,6 +106,11 @@ typedef struct {
                                     /* psf_size <= 15, lsf_size <= 9 and an even n_channels.      */
                                     /* The PSF then acts AFTER the LSF (they no longer commute).  */
 } rubix_telescope;
+
+/* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
+ * rubix_abi_version() returns the value the LIBRARY was built with. */
+#define RUBIX_ABI_VERSION 3
+uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
  * wavelength grid of the observed telescope"; the paper does not say which rule):
@@ -141,6 +152,18 @@ rubix_status rubix_build_cube(const rubix_particles *particles, const rubix_ssp 
 rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cube_in,
                                     float *cube_out, void *workspace, size_t workspace_bytes,
                                     void *stream);
+
+/* Steps 1-8 in one call on DEVICE buffers (the whole forward model: rubix_build_cube followed by
+ * rubix_convolve_psf_lsf, same arithmetic, same results bit for bit).  The raw cube of step 6 lives in the workspace; with
+ * PSF/LSF on (psf_size <= 15, lsf_size <= 9, even n_channels) the sort's segment table tells the stencil passes which
+ * spaxels hold particles: rows of empty spaxels are neither written by step 6 nor read by step 7, and all-zero rows of
+ * the temporary between the two PSF passes are neither written nor read (the PSF/LSF floor is one read
+ * and one write of the cube).  Other stencil shapes run the two plain stages.
+ *   cube  DEVICE [n_x][n_y][n_channels] fp32: the FINAL cube (raw cube when PSF and LSF are off); every voxel written
+ *         exactly once; must not overlap the workspace.
+ * Arguments, limits, errors and sort artefacts as rubix_build_cube.  This is the device-resident call bench.py times. */
+rubix_status rubix_forward(const rubix_particles *particles, const rubix_ssp *ssp, const rubix_telescope *tel,
+                           const float *R, float *cube, void *workspace, size_t workspace_bytes, void *stream);
 
 /* Step 9: gradients of a scalar loss L of the FINAL cube
  * (after PSF/LSF, if tel switches them on) with respect to each particle's mass, log age,
@@ -185,8 +208,8 @@ rubix_status rubix_loss_and_grad(const rubix_particles *particles, const rubix_s
 rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_voxels, float sigma_read, float gain,
                              uint64_t seed, void *stream);
 
-/* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_cube_adjoint on
- * this workspace address (compared bit for bit with the oracle):
+/* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_forward / rubix_cube_adjoint /
+ * rubix_loss_and_grad on this workspace address (the library remembers the 256 most recently used addresses) (compared bit for bit with the oracle):
  *   key     [n]      spaxel key of each particle in original order (n_s = dropped)
  *   perm    [n]      stable order by (key, original index)
  *   seg_off [n_s+2]  segment s is perm[seg_off[s] .. seg_off[s+1]); s = n_s: dropped particles
@@ -195,7 +218,7 @@ rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key
                                       const int32_t **perm, const int32_t **seg_off);
 
 /* Whole path with HOST buffers: copies the particle arrays and the SSP grid host->device,
- * runs rubix_build_cube and (if switched on) rubix_convolve_psf_lsf, and copies the final cube
+ * runs rubix_forward (steps 1-8), and copies the final cube
  * device->host, all on `stream`; returns after enqueueing (pinned host memory makes the copies
  * asynchronous).  This is the end-to-end call bench.py times.
  *   h_particles  the five arrays are HOST pointers here;  h_ssp->flux is a HOST pointer here

@@ -17,13 +17,14 @@ LIB_PATH = os.path.join(_HERE, "librubix_b200.so")
 RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ERR_WORKSPACE, \
     RUBIX_ERR_CUDA = range(6)
 
-EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf",
+EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf", "rubix_forward",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
-           "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error",
+           "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
+ABI_VERSION = 3          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -40,14 +41,14 @@ class CParticles(C.Structure):
 
 
 class CSSP(C.Structure):
-    _fields_ = [("n_age", C.c_int32), ("n_z", C.c_int32), ("n_lambda", C.c_int32),
+    _fields_ = [("struct_size", C.c_uint32), ("n_age", C.c_int32), ("n_z", C.c_int32), ("n_lambda", C.c_int32),
                 ("log_age_axis", C.c_void_p), ("log_z_axis", C.c_void_p),
                 ("lambda0", C.c_float), ("dlambda", C.c_float), ("flux", C.c_void_p),
                 ("log_lambda", C.c_int32)]
 
 
 class CTelescope(C.Structure):
-    _fields_ = [("n_x", C.c_int32), ("n_y", C.c_int32), ("spaxel_size", C.c_float),
+    _fields_ = [("struct_size", C.c_uint32), ("n_x", C.c_int32), ("n_y", C.c_int32), ("spaxel_size", C.c_float),
                 ("n_channels", C.c_int32), ("lambda0", C.c_float), ("dlambda", C.c_float),
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
                 ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
@@ -73,6 +74,8 @@ def load():
         lib.rubix_build_cube.restype = C.c_int
         lib.rubix_build_cube.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope),
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.rubix_forward.restype = C.c_int
+        lib.rubix_forward.argtypes = lib.rubix_build_cube.argtypes
         lib.rubix_convolve_psf_lsf.restype = C.c_int
         lib.rubix_convolve_psf_lsf.argtypes = [C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p,
                                                C.c_size_t, C.c_void_p]
@@ -108,6 +111,10 @@ def load():
         lib.rubix_stage_timing_read.restype = C.c_int32
         lib.rubix_stage_timing_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_int32)]
         lib.rubix_last_launch_count.restype = C.c_int32
+        lib.rubix_abi_version.restype = C.c_uint32
+        if int(lib.rubix_abi_version()) != ABI_VERSION:
+            raise RuntimeError(f"{LIB_PATH} has ABI version {int(lib.rubix_abi_version())}, this binding expects "
+                               f"{ABI_VERSION}: rebuild with `python -m paper_2412_08265_b200.build --force`")
         lib.rubix_last_error.restype = C.c_char_p
         _lib = lib
     return _lib
@@ -152,7 +159,7 @@ class _Keep:
 def c_telescope(tel) -> _Keep:
     lam = getattr(tel, "lambda_obs", None)
     lam = None if lam is None else np.ascontiguousarray(lam, dtype=np.float32)
-    return _Keep(CTelescope(int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
+    return _Keep(CTelescope(C.sizeof(CTelescope), int(tel.n_x), int(tel.n_y), float(tel.spaxel_size), int(tel.n_channels),
                             float(tel.lambda0), float(tel.dlambda), int(tel.psf_size),
                             float(tel.psf_sigma), int(tel.lsf_size), float(tel.lsf_sigma),
                             int(getattr(tel, "resample", 0)), float(getattr(tel, "redshift", 0.0)),
@@ -167,7 +174,7 @@ def c_ssp(ssp, flux) -> _Keep:
     rubix_forward_host)."""
     age, zed = _host_f32(ssp.log_age_axis), _host_f32(ssp.log_z_axis)
     n_age, n_z, n_lambda = (int(v) for v in flux.shape)
-    return _Keep(CSSP(n_age, n_z, n_lambda, age.ctypes.data, zed.ctypes.data, float(ssp.lambda0),
+    return _Keep(CSSP(C.sizeof(CSSP), n_age, n_z, n_lambda, age.ctypes.data, zed.ctypes.data, float(ssp.lambda0),
                       float(ssp.dlambda), _ptr(flux), int(getattr(ssp, "log_lambda", 0))), age, zed, flux)
 
 
@@ -196,6 +203,13 @@ def rubix_build_cube(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspac
     _check(load().rubix_build_cube(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
                                    _ptr(workspace), int(workspace.numel() * workspace.element_size()),
                                    _stream(stream)))
+
+
+def rubix_forward(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_forward(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
+                                _ptr(workspace), int(workspace.numel() * workspace.element_size()),
+                                _stream(stream)))
 
 
 def rubix_convolve_psf_lsf(tel: _Keep, cube_in, cube_out, workspace, stream=None):
@@ -335,7 +349,14 @@ class DeviceWorkload:
         rubix_convolve_psf_lsf(self.tel, cube, res, self.workspace)
         return res
 
-    def forward(self):
+    def forward(self, out=None):
+        """Steps 1-8 through the fused device call rubix_forward."""
+        import torch
+        cube = torch.empty(self.shape, dtype=torch.float32, device=self.device) if out is None else out
+        rubix_forward(self.particles, self.ssp, self.tel, self.R, cube, self.workspace)
+        return cube
+
+    def forward_two_calls(self):
         cube = self.build_cube()
         t = self.w.telescope
         return self.convolve(cube) if (t.psf_size > 0 or t.lsf_size > 0) else cube

@@ -6,6 +6,8 @@
 #include <mutex>
 #include <unordered_map>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "common.cuh"
 
 namespace rubix {
@@ -32,13 +34,25 @@ rubix_status cuda_fail(cudaError_t e, const char *where)
     return fail(RUBIX_ERR_CUDA, "%s: %s", where, cudaGetErrorString(e));
 }
 
-struct Artifacts { const int32_t *key, *perm, *seg_off; };
+// sort artefacts of the most recently used workspace addresses (bounded: the oldest entry is dropped)
+struct Artifacts { const int32_t *key, *perm, *seg_off; uint64_t stamp; };
+constexpr size_t kMaxArtifacts = 256;
 std::mutex g_mu;
 std::unordered_map<const void *, Artifacts> g_artifacts;
+uint64_t g_stamp = 0;
+
+// NVTX range around one ABI call (ranges around the compute calls)
+struct Range {
+    explicit Range(const char *name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+};
 
 rubix_status check_ssp(const rubix_ssp *s, bool flux_required)
 {
     if (!s) return fail(RUBIX_ERR_NULL, "ssp is NULL");
+    if (s->struct_size != sizeof(rubix_ssp))
+        return fail(RUBIX_ERR_INVALID_ARG, "rubix_ssp.struct_size is %u, this library expects %zu (ABI version %d): the "
+                    "caller was built against another rubix.h", s->struct_size, sizeof(rubix_ssp), RUBIX_ABI_VERSION);
     if (!s->log_age_axis || !s->log_z_axis || (flux_required && !s->flux))
         return fail(RUBIX_ERR_NULL, "ssp axis / flux pointer is NULL");
     if (s->n_age < 2 || s->n_z < 2 || s->n_lambda < 2)
@@ -65,6 +79,10 @@ rubix_status check_ssp(const rubix_ssp *s, bool flux_required)
 rubix_status check_tel(const rubix_telescope *t)
 {
     if (!t) return fail(RUBIX_ERR_NULL, "telescope is NULL");
+    if (t->struct_size != sizeof(rubix_telescope))
+        return fail(RUBIX_ERR_INVALID_ARG, "rubix_telescope.struct_size is %u, this library expects %zu (ABI version %d): "
+                    "the caller was built against another rubix.h", t->struct_size, sizeof(rubix_telescope),
+                    RUBIX_ABI_VERSION);
     if (t->n_x < 1 || t->n_y < 1 || t->n_channels < 1)
         return fail(RUBIX_ERR_INVALID_ARG, "detector needs n_x, n_y, n_channels >= 1");
     if ((double)t->n_x * t->n_y >= 2147483647.0 / 2 || (double)t->n_x * t->n_y * t->n_channels >= 9.0e15)
@@ -149,9 +167,15 @@ void remember(const void *ws, const Layout &L)
 {
     const char *b = (const char *)ws;
     std::lock_guard<std::mutex> lk(g_mu);
+    if (g_artifacts.size() >= kMaxArtifacts && g_artifacts.find(ws) == g_artifacts.end()) {
+        auto oldest = g_artifacts.begin();
+        for (auto it = g_artifacts.begin(); it != g_artifacts.end(); ++it)
+            if (it->second.stamp < oldest->second.stamp) oldest = it;
+        g_artifacts.erase(oldest);
+    }
     g_artifacts[ws] = Artifacts{(const int32_t *)(b + L.off_key),
                                 (const int32_t *)(b + L.off_permbuf[L.final_buf]),
-                                (const int32_t *)(b + L.off_seg)};
+                                (const int32_t *)(b + L.off_seg), ++g_stamp};
 }
 
 }  // namespace
@@ -159,6 +183,7 @@ void remember(const void *ws, const Layout &L)
 extern "C" {
 
 const char *rubix_last_error(void) { return t_err; }
+uint32_t rubix_abi_version(void) { return RUBIX_ABI_VERSION; }
 int32_t rubix_last_launch_count(void) { return g_launches; }
 
 size_t rubix_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
@@ -166,6 +191,10 @@ size_t rubix_workspace_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telesc
     t_err[0] = 0;
     if (n < 0 || n >= 2147483647LL) { fail(RUBIX_ERR_INVALID_ARG, "n out of range"); return 0; }
     if (check_tel(tel) != RUBIX_OK) return 0;
+    if (ssp && ssp->struct_size != sizeof(rubix_ssp)) {
+        fail(RUBIX_ERR_INVALID_ARG, "rubix_ssp.struct_size is %u, this library expects %zu", ssp->struct_size, sizeof(rubix_ssp));
+        return 0;
+    }
     if (ssp && (ssp->n_age < 2 || ssp->n_z < 2 || ssp->n_lambda < 2)) {
         fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
         return 0;
@@ -179,6 +208,7 @@ rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, co
                               void *stream)
 {
     t_err[0] = 0;
+    Range nvtx_range("rubix_build_cube");
     g_launches = 0;
     rubix_status s;
     if ((s = check_particles(p)) != RUBIX_OK) return s;
@@ -197,8 +227,63 @@ rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, co
         e = launch_particle_pass(in, L, (char *)workspace, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "particle pass");
-    e = launch_accumulate(in, L, (char *)workspace, cube, st);
+    e = launch_accumulate(in, L, (char *)workspace, cube, false, st);
     if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+    remember(workspace, L);
+    return RUBIX_OK;
+}
+
+// Steps 1-8 on device buffers.  With the marching PSF/LSF kernels the raw cube lives in the workspace and only the
+// rows of occupied spaxels are written and read (launch_convolve's masks); otherwise the two plain stages run.
+static rubix_status forward_device(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                                   const float *R, float *cube_out, const Layout &L, char *ws, cudaStream_t st)
+{
+    PassInputs in{p, ssp, tel, R};
+    cudaError_t e;
+    {
+        StageTimer t(0, st);
+        e = launch_particle_pass(in, L, ws, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
+    if (!conv) {
+        e = launch_accumulate(in, L, ws, cube_out, false, st);
+        if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+        return RUBIX_OK;
+    }
+    float *raw = (float *)(ws + L.off_cube_a), *tmp = (float *)(ws + L.off_cube_b);
+    const bool sparse = convolve_fast_path(tel, raw, cube_out, tmp);
+    e = launch_accumulate(in, L, ws, raw, sparse, st);
+    if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+    {
+        StageTimer t(3, st);
+        e = launch_convolve(tel, raw, cube_out, tmp, (float *)(ws + L.off_psftaps), false,
+                            sparse ? (const uint8_t *)(ws + L.off_occ[0]) : nullptr,
+                            sparse ? (uint8_t *)(ws + L.off_occ[1]) : nullptr, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "convolve");
+    return RUBIX_OK;
+}
+
+rubix_status rubix_forward(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                           const float *R, float *cube, void *workspace, size_t workspace_bytes, void *stream)
+{
+    t_err[0] = 0;
+    Range nvtx_range("rubix_forward");
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !cube) return fail(RUBIX_ERR_NULL, "R or cube is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z,
+                                 ssp->n_lambda);
+    if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
+    const char *c0 = (const char *)cube, *w0 = (const char *)workspace;
+    if (c0 < w0 + L.bytes_total && w0 < c0 + (size_t)tel->n_x * tel->n_y * tel->n_channels * 4)
+        return fail(RUBIX_ERR_INVALID_ARG, "cube overlaps the workspace");
+    if ((s = forward_device(p, ssp, tel, R, cube, L, (char *)workspace, (cudaStream_t)stream)) != RUBIX_OK) return s;
     remember(workspace, L);
     return RUBIX_OK;
 }
@@ -207,6 +292,7 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
                                     void *workspace, size_t workspace_bytes, void *stream)
 {
     t_err[0] = 0;
+    Range nvtx_range("rubix_convolve_psf_lsf");
     g_launches = 0;
     rubix_status s;
     if ((s = check_tel(tel)) != RUBIX_OK) return s;
@@ -226,7 +312,7 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
     cudaError_t e;
     {
         StageTimer t(3, (cudaStream_t)stream);
-        e = launch_convolve(tel, cube_in, cube_out, tmp, taps, false, (cudaStream_t)stream);
+        e = launch_convolve(tel, cube_in, cube_out, tmp, taps, false, nullptr, nullptr, (cudaStream_t)stream);
     }
     if (e != cudaSuccess) return cuda_fail(e, "convolve");
     return RUBIX_OK;
@@ -238,6 +324,7 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
                                 void *stream)
 {
     t_err[0] = 0;
+    Range nvtx_range("rubix_cube_adjoint");
     g_launches = 0;
     rubix_status s;
     if ((s = check_particles(p)) != RUBIX_OK) return s;
@@ -265,7 +352,7 @@ rubix_status rubix_cube_adjoint(const rubix_particles *p, const rubix_ssp *ssp, 
         {
             StageTimer t(3, st);
             e = launch_convolve(tel, grad_cube, (float *)(ws + L.off_cube_a), (float *)(ws + L.off_cube_b),
-                                (float *)(ws + L.off_psftaps), true, st);
+                                (float *)(ws + L.off_psftaps), true, nullptr, nullptr, st);
         }
         if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
         gconv = (const float *)(ws + L.off_cube_a);
@@ -293,6 +380,7 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
                                  void *workspace, size_t workspace_bytes, void *stream)
 {
     t_err[0] = 0;
+    Range nvtx_range("rubix_loss_and_grad");
     g_launches = 0;
     rubix_status s;
     if ((s = check_particles(p)) != RUBIX_OK) return s;
@@ -323,14 +411,17 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
     if (e != cudaSuccess) return cuda_fail(e, "particle pass");
     // forward: raw cube, then PSF/LSF
     float *raw = conv ? buf_a : (cube_out ? cube_out : buf_a);
-    e = launch_accumulate(in, L, ws, raw, st);
+    float *fin = cube_out ? cube_out : buf_c;
+    const bool sparse = conv && convolve_fast_path(tel, raw, fin, buf_b);   // only occupied rows cross HBM
+    e = launch_accumulate(in, L, ws, raw, sparse, st);
     if (e != cudaSuccess) return cuda_fail(e, "accumulate");
     const float *final_cube = raw;
     if (conv) {
-        float *fin = cube_out ? cube_out : buf_c;
         {
             StageTimer t(3, st);
-            e = launch_convolve(tel, raw, fin, buf_b, (float *)(ws + L.off_psftaps), false, st);
+            e = launch_convolve(tel, raw, fin, buf_b, (float *)(ws + L.off_psftaps), false,
+                                sparse ? (const uint8_t *)(ws + L.off_occ[0]) : nullptr,
+                                sparse ? (uint8_t *)(ws + L.off_occ[1]) : nullptr, st);
         }
         if (e != cudaSuccess) return cuda_fail(e, "convolve");
         final_cube = fin;
@@ -343,7 +434,7 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
     if (conv) {                                            // G' = LSF^T PSF^T G (self-adjoint stencils)
         {
             StageTimer t(3, st);
-            e = launch_convolve(tel, grad, buf_c, buf_b, (float *)(ws + L.off_psftaps), true, st);   // buf_c is free
+            e = launch_convolve(tel, grad, buf_c, buf_b, (float *)(ws + L.off_psftaps), true, nullptr, nullptr, st);   // buf_c is free
         }
         if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
         gconv = buf_c;
@@ -361,6 +452,7 @@ rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_vo
                              uint64_t seed, void *stream)
 {
     t_err[0] = 0;
+    Range nvtx_range("rubix_add_noise");
     g_launches = 0;
     if (n_voxels < 0) return fail(RUBIX_ERR_INVALID_ARG, "n_voxels must be >= 0");
     if (n_voxels > 0 && (!cube_in || !cube_out)) return fail(RUBIX_ERR_NULL, "cube_in or cube_out is NULL");
@@ -419,8 +511,8 @@ HostLayout host_layout(int64_t n, const rubix_ssp *ssp, const rubix_telescope *t
 size_t rubix_forward_host_scratch_bytes(int64_t n, const rubix_ssp *ssp, const rubix_telescope *tel)
 {
     t_err[0] = 0;
-    if (n < 0 || n >= 2147483647LL || !ssp || check_tel(tel) != RUBIX_OK || ssp->n_age < 2 || ssp->n_z < 2 ||
-        ssp->n_lambda < 2) {
+    if (n < 0 || n >= 2147483647LL || !ssp || check_tel(tel) != RUBIX_OK || ssp->struct_size != sizeof(rubix_ssp) ||
+        ssp->n_age < 2 || ssp->n_z < 2 || ssp->n_lambda < 2) {
         if (!t_err[0]) fail(RUBIX_ERR_INVALID_ARG, "bad arguments");
         return 0;
     }
@@ -454,6 +546,7 @@ rubix_status forward_host_impl(const rubix_particles *hp, const rubix_ssp *hs, c
                                const float *R, float *h_cube, void *scratch, size_t scratch_bytes, void *stream,
                                bool pipelined)
 {
+    Range nvtx_range(pipelined ? "rubix_forward_host_pipelined" : "rubix_forward_host");
     t_err[0] = 0;
     rubix_status s;
     if ((s = check_particles(hp)) != RUBIX_OK) return s;
@@ -498,16 +591,9 @@ rubix_status forward_host_impl(const rubix_particles *hp, const rubix_ssp *hs, c
         if (g_pipe.used[slot] && (e = cudaStreamWaitEvent(st, g_pipe.copied[slot], 0)) != cudaSuccess)
             return cuda_fail(e, "pipeline wait");
     }
-    float *raw = conv ? (float *)(d + H.cube) : final_cube;
-    s = rubix_build_cube(&dp, &ds, tel, R, raw, d + H.ws, ws_bytes, stream);
+    // steps 1-8 in one call: with PSF/LSF on, the raw cube stays in the workspace and only occupied rows cross HBM
+    s = rubix_forward(&dp, &ds, tel, R, final_cube, d + H.ws, ws_bytes, stream);
     if (s != RUBIX_OK) return s;
-    int launches = g_launches;
-    if (conv) {
-        s = rubix_convolve_psf_lsf(tel, raw, final_cube, d + H.ws, ws_bytes, stream);
-        if (s != RUBIX_OK) return s;
-        launches += g_launches;
-    }
-    g_launches = launches;
     if (!pipelined) {
         e = cudaMemcpyAsync(h_cube, final_cube, cube_bytes, cudaMemcpyDeviceToHost, st);
         if (e != cudaSuccess) return cuda_fail(e, "device->host copy");

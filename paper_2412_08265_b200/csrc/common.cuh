@@ -73,7 +73,7 @@ struct Layout {
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,
-        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps, off_aux;
+        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps, off_aux, off_occ[2];
     int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
                                       // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
@@ -91,12 +91,18 @@ struct PassInputs {
 };
 
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
-cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube,
+// skip_empty: rows of spaxels without particles are NOT written (the masked PSF/LSF passes never read them)
+cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
                               cudaStream_t st);
 // taps_dev: device scratch of psf_taps_bytes(n_channels) for a wavelength-dependent PSF (reading R18), else unused.
 // transpose: apply LSF^T PSF^T (PSF first, then LSF) instead of PSF LSF; only differs when the PSF depends on lambda.
+// occ_in / occ_tmp (both or neither; forward order only): occ_in[s] != 0 marks the spaxel rows of `in` that hold data --
+// the others are taken as zeros WITHOUT being read (they may be unwritten); occ_tmp [n_s] receives the same
+// mask for the temporary after the first pass, so that all-zero rows cross HBM in neither direction.
 cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
-                            bool transpose, cudaStream_t st);
+                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st);
+// true when launch_convolve would take its marching (fast) path, the only one that honours the masks
+bool convolve_fast_path(const rubix_telescope *tel, const float *in, const float *out, const float *tmp);
 inline size_t psf_taps_bytes(int32_t n_c) { return align_up((size_t)15 * ((size_t)n_c + 2) * 4, 256); }
 cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, const float *gconv,
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st);

@@ -76,6 +76,12 @@ struct MarchParams {
     float h[9];                         // LSF taps along the channel, zero padded, centred, symmetric
     const float *taps;                  // VAR: per-channel PSF taps, tap-major [15][tstride] (reading R18)
     int32_t tstride;
+    // MASK: spaxel of (line, step) = line * sp_line + step * sp_step; mask_in[spaxel] == 0: the input row is taken
+    // as zeros without being read; mask_out (MASK == 1): 1 where the output row was written, 0 where it is all zero
+    // and was NOT written
+    const uint8_t *mask_in;
+    uint8_t *mask_out;
+    int32_t sp_line, sp_step;
 };
 
 __device__ __forceinline__ float2 shfl_up2(float2 v, int d)
@@ -102,6 +108,20 @@ __device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned 
     return o;
 }
 
+// predicated 8-byte streaming load / store (no branch: the marching loops stay straight-line)
+__device__ __forceinline__ float2 ldcs_pred(const float *p, uint32_t pred)
+{
+    float2 v;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\tmov.f32 %0, 0f00000000;\n\tmov.f32 %1, 0f00000000;\n\t"
+                 "@p ld.global.cs.v2.f32 {%0, %1}, [%2];\n\t}"
+                 : "=f"(v.x), "=f"(v.y) : "l"(p), "r"(pred));
+    return v;
+}
+__device__ __forceinline__ void stcs_pred(float *p, float2 v, uint32_t pred)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.cs.v2.f32 [%0], {%1, %2};\n\t}"
+                 :: "l"(p), "f"(v.x), "f"(v.y), "r"(pred) : "memory");
+}
 // steps prefetched per thread (divides 15) and resident CTAs per SM, for the pass with the fused LSF (1) and
 // for the plain passes (0)
 #ifndef RUBIX_MARCH_PF1
@@ -119,7 +139,12 @@ __device__ __forceinline__ unsigned long long lsf_pair(float2 v, const unsigned 
 
 // VAR: the stencil along the marching axis differs per channel (wavelength-dependent PSF, reading R18): the
 // thread loads the 15 taps of its two channels once; they then live in registers (two resident CTAs per SM).
-template <bool LSF, bool VAR = false>
+// MASK (occupancy-aware passes of the fused forward, where the sort knows which spaxels hold particles):
+//   1  first pass: rows with mask_in == 0 are not read; an output row whose 15 inputs are all unoccupied is NOT
+//      written and gets mask_out = 0 (else 1);  2  second pass: rows with mask_in == 0 are not read, every output is
+//      written.  A warp works on one line, so every mask decision is warp-uniform.  The mask bytes of the next 15
+//      steps are fetched one iteration ahead (one byte per lane + ballot).
+template <bool LSF, bool VAR = false, int MASK = 0>
 __global__ void __launch_bounds__(256, VAR ? 2 : (LSF ? RUBIX_MARCH_MINB1 : RUBIX_MARCH_MINB0))
 k_march(const __grid_constant__ MarchParams P)
 {
@@ -134,9 +159,10 @@ k_march(const __grid_constant__ MarchParams P)
     const size_t off = (size_t)line * P.line_stride + (size_t)(c_ok ? c : 0);
     const float *src = P.in + off;
     float *dst = P.out + off;
-    auto load = [&](int s) -> float2 {
-        if (c_ok && s < P.n_steps) return __ldcs(reinterpret_cast<const float2 *>(src + (size_t)s * P.step_stride));
-        return make_float2(0.0f, 0.0f);
+    const int64_t sp0 = MASK ? (int64_t)line * P.sp_line : 0;
+    auto mask_byte = [&](int base) -> uint32_t {           // lane i: occupancy of step base + i
+        const int s = base + lane;
+        return (lane < 15 && s < P.n_steps) ? (uint32_t)__ldg(P.mask_in + sp0 + (int64_t)s * P.sp_step) : 0u;
     };
     unsigned long long acc[15], g2[15], hp[5];
     float2 pf[kMarchPf];
@@ -152,25 +178,59 @@ k_march(const __grid_constant__ MarchParams P)
     }
 #pragma unroll
     for (int i = 0; i < 5; ++i) hp[i] = pack2(P.h[4 + i], P.h[4 + i]);
+    // the next row to load / to store, advanced by one step per step (no per-step 64-bit multiplies)
+    const float *lp = src;
+    float *op = dst;
+    // lane-dependent conditions as all-ones / zero words: a store predicate is then ONE and-with-uniform-bits test
+    const uint32_t st_word = st_ok ? ~0u : 0u, ld_word = c_ok ? ~0u : 0u;
+    // mq: occupancy shift register, bit 0 = the step loaded last, bit kMarchPf = the step consumed now,
+    // bits kMarchPf .. kMarchPf + 14 = the 15 inputs of the output that completes now
+    uint32_t mq = 0, mload = ~0u;
+    {
+        const uint32_t m0 = MASK ? __ballot_sync(0xffffffffu, mask_byte(0) != 0) : ~0u;
 #pragma unroll
-    for (int i = 0; i < kMarchPf; ++i) pf[i] = load(i);
+        for (int i = 0; i < kMarchPf; ++i) {
+            const uint32_t o = i < P.n_steps ? (m0 >> i) & 1u : 0u;
+            pf[i] = ldcs_pred(lp, ld_word & o);
+            lp += P.step_stride;
+            mq = (mq << 1) | o;
+        }
+        if (MASK) mload = __ballot_sync(0xffffffffu, mask_byte(kMarchPf) != 0);
+    }
     for (int s0 = 0; s0 < P.n_steps + 7; s0 += 15) {
+        const uint32_t mnext = MASK ? mask_byte(s0 + 15 + kMarchPf) : 0u;   // consumed at the end of this iteration
+        uint32_t wbits = 0;                                   // MASK == 1: bit u = the output completed at position u was written
 #pragma unroll
         for (int u = 0; u < 15; ++u) {
             const int s = s0 + u;
-            const float2 raw = pf[u % kMarchPf];
-            pf[u % kMarchPf] = load(s + kMarchPf);
-            const unsigned long long v = LSF ? lsf_pair(raw, hp) : pack2(raw.x, raw.y);
+            const int slot = u % kMarchPf;
+            const float2 raw = pf[slot];
+            const uint32_t lo = s + kMarchPf < P.n_steps ? (mload >> u) & 1u : 0u;
+            pf[slot] = ldcs_pred(lp, ld_word & lo);
+            lp += P.step_stride;
+            mq = (mq << 1) | lo;
+            if (!MASK || ((mq >> kMarchPf) & 1u)) {          // warp-uniform: an unoccupied step adds nothing
+                const unsigned long long v = LSF ? lsf_pair(raw, hp) : pack2(raw.x, raw.y);
 #pragma unroll
-            for (int d = -7; d <= 7; ++d) {
-                const int slot = (u - d + 15) % 15;           // output s - d
-                acc[slot] = ffma2(g2[d + 7], v, acc[slot]);
+                for (int d = -7; d <= 7; ++d) {
+                    const int sl = (u - d + 15) % 15;         // output s - d
+                    acc[sl] = ffma2(g2[d + 7], v, acc[sl]);
+                }
             }
-            const int o = s - 7, so = (u + 8) % 15;           // output o is complete
-            if (st_ok && o >= 0 && o < P.n_steps)
-                __stcs(reinterpret_cast<float2 *>(dst + (size_t)o * P.step_stride), unpack2(acc[so]));
+            const int so = (u + 8) % 15;                      // output s - 7 is complete
+            if (s >= 7) {
+                const uint32_t wr = (s - 7 < P.n_steps && (MASK != 1 || ((mq >> kMarchPf) & 0x7FFFu) != 0)) ? 1u : 0u;
+                stcs_pred(op, unpack2(acc[so]), st_word & wr);
+                op += P.step_stride;
+                if (MASK == 1) wbits |= wr << u;
+            }
             acc[so] = 0ull;
         }
+        if (MASK == 1 && cblock == 0) {                       // lane u records the output that completed at position u
+            const int o = s0 + lane - 7;
+            if (lane < 15 && o >= 0 && o < P.n_steps) P.mask_out[sp0 + (int64_t)o * P.sp_step] = (uint8_t)((wbits >> lane) & 1u);
+        }
+        if (MASK) mload = __ballot_sync(0xffffffffu, mnext != 0);
     }
 }
 
@@ -187,7 +247,8 @@ k_lsf_rows(const __grid_constant__ MarchParams P)
     const bool c_ok = c >= 0 && c + 1 < P.n_c;
     const size_t off = (size_t)row * P.n_c + (size_t)(c_ok ? c : 0);
     float2 v = make_float2(0.0f, 0.0f);
-    if (c_ok) v = __ldcs(reinterpret_cast<const float2 *>(P.in + off));
+    const bool occ = P.mask_in == nullptr || __ldg(P.mask_in + row) != 0;   // unoccupied rows are zeros, not read
+    if (c_ok && occ) v = __ldcs(reinterpret_cast<const float2 *>(P.in + off));
     unsigned long long hp[5];
 #pragma unroll
     for (int i = 0; i < 5; ++i) hp[i] = pack2(P.h[4 + i], P.h[4 + i]);
@@ -218,18 +279,30 @@ static void var_psf_taps(const rubix_telescope *tel, int tstride, float *dst)
     }
 }
 
-template <bool LSF, bool VAR>
+template <bool LSF, bool VAR, int MASK = 0>
 static cudaError_t march(MarchParams &P, cudaStream_t st)
 {
     P.cblocks = LSF ? (P.n_c + 55) / 56 : (P.n_c + 63) / 64;
     const int64_t warps = (int64_t)P.n_lines * P.cblocks;
-    k_march<LSF, VAR><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
+    k_march<LSF, VAR, MASK><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }
 
+static bool fast_path(const rubix_telescope *tel, const float *in, const float *out, const float *tmp)
+{
+    const bool aligned = (tel->n_channels % 2 == 0) && (((uintptr_t)in & 7u) == 0) && (((uintptr_t)out & 7u) == 0) &&
+                         (tmp == nullptr || ((uintptr_t)tmp & 7u) == 0);
+    return aligned && tel->psf_size <= 15 && tel->lsf_size <= 9;
+}
+
+bool convolve_fast_path(const rubix_telescope *tel, const float *in, const float *out, const float *tmp)
+{
+    return (tel->psf_size > 0 || tel->lsf_size > 0) && fast_path(tel, in, out, tmp);
+}
+
 cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
-                            bool transpose, cudaStream_t st)
+                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st)
 {
     const int32_t n_x = tel->n_x, n_y = tel->n_y, n_c = tel->n_channels;
     const int64_t n_vox = (int64_t)n_x * n_y * n_c;
@@ -241,12 +314,11 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
         return cudaMemcpyAsync(out, in, (size_t)n_vox * 4, cudaMemcpyDeviceToDevice, st);
 
     const bool var = psf.size > 0 && tel->psf_alpha != 0.0f;
-    const bool aligned = (n_c % 2 == 0) && (((uintptr_t)in & 7u) == 0) && (((uintptr_t)out & 7u) == 0) &&
-                         (tmp == nullptr || ((uintptr_t)tmp & 7u) == 0);
-    const bool fast = aligned && psf.size <= 15 && lsf.size <= 9;
+    const bool fast = fast_path(tel, in, out, tmp);
+    const bool masked = occ_in != nullptr && occ_tmp != nullptr && !transpose;
     cudaError_t e;
     if (!fast) {
-        if (var) return cudaErrorNotSupported;             // api.cu refuses this combination beforehand
+        if (var || masked) return cudaErrorNotSupported;   // api.cu refuses / avoids these combinations beforehand
         const float *src = in;
         if (lsf.size > 0) {
             if ((e = stencil_generic(src, out, n_vox, 1, n_c, lsf, st)) != cudaSuccess) return e;
@@ -263,10 +335,14 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     P.n_c = n_c;
     P.taps = nullptr;
     P.tstride = 0;
+    P.mask_in = nullptr;
+    P.mask_out = nullptr;
+    P.sp_line = P.sp_step = 0;
     centre_taps(psf, 15, P.g);
     centre_taps(lsf, 9, P.h);
     auto lsf_rows = [&](const float *src, float *dst) -> cudaError_t {
         P.in = src; P.out = dst;
+        P.mask_in = masked ? occ_in : nullptr;
         P.n_lines = n_x * n_y; P.n_steps = 1; P.line_stride = n_c; P.step_stride = 0;
         P.cblocks = (n_c + 55) / 56;
         const int64_t warps = (int64_t)P.n_lines * P.cblocks;
@@ -278,11 +354,13 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
         P.in = src; P.out = dst;
         P.n_lines = n_x; P.n_steps = n_y;
         P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
+        P.sp_line = n_y; P.sp_step = 1;
     };
     auto along_x = [&](const float *src, float *dst) {     // lines = y
         P.in = src; P.out = dst;
         P.n_lines = n_y; P.n_steps = n_x;
         P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
+        P.sp_line = 1; P.sp_step = n_y;
     };
     if (psf.size <= 0) return lsf_rows(in, out);           // LSF only
 
@@ -303,6 +381,14 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
             return lsf_rows(tmp, out);
         }
         along_y(in, tmp);                                  // PSF LSF: LSF fused into the pass along y
+        if (masked) {
+            P.mask_in = occ_in; P.mask_out = occ_tmp;
+            e = lsf.size > 0 ? march<true, true, 1>(P, st) : march<false, true, 1>(P, st);
+            if (e != cudaSuccess) return e;
+            along_x(tmp, out);
+            P.mask_in = occ_tmp; P.mask_out = nullptr;
+            return march<false, true, 2>(P, st);
+        }
         e = lsf.size > 0 ? march<true, true>(P, st) : march<false, true>(P, st);
         if (e != cudaSuccess) return e;
         along_x(tmp, out);
@@ -310,6 +396,14 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     }
     // pass 1: along y (lines = x), LSF fused when on; pass 2: along x (lines = y)
     along_y(in, tmp);
+    if (masked) {
+        P.mask_in = occ_in; P.mask_out = occ_tmp;
+        e = lsf.size > 0 ? march<true, false, 1>(P, st) : march<false, false, 1>(P, st);
+        if (e != cudaSuccess) return e;
+        along_x(tmp, out);
+        P.mask_in = occ_tmp; P.mask_out = nullptr;
+        return march<false, false, 2>(P, st);
+    }
     e = lsf.size > 0 ? march<true, false>(P, st) : march<false, false>(P, st);
     if (e != cudaSuccess) return e;
     along_x(tmp, out);

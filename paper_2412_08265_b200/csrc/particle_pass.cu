@@ -226,7 +226,7 @@ k_unit_tile_totals(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__restrict__ tile_tot,
              int32_t *__restrict__ unit_off, int32_t *__restrict__ part_off,
-             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals)
+             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals, uint8_t *__restrict__ occ)
 {
     __shared__ int32_t sm[3][kScanThreads / 32];
     __shared__ int32_t wsum[3][kScanThreads / 32];
@@ -264,6 +264,7 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__
             const int s = s0 + i;
             unit_off[s] = run[0];
             part_off[s] = run[1];
+            occ[s] = chunks[i] > 0 ? 1 : 0;             // occupancy mask of the masked PSF/LSF passes
             if (chunks[i] > 1) multi_list[run[2]] = s;
             run[0] += chunks[i] > 1 ? chunks[i] : 1;
             run[1] += chunks[i] > 1 ? chunks[i] : 0;
@@ -546,6 +547,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_xtab = take(((size_t)n_c + 1) * 8);           // Y[k] of the table mode (readings R15 / R16)
     L.off_lamobs = take(((size_t)n_c + 1) * 4);         // device copy of rubix_telescope.lambda_obs
     L.off_psftaps = take(psf_taps_bytes(n_c));          // per-channel PSF taps (reading R18)
+    for (int b = 0; b < 2; ++b) L.off_occ[b] = take((size_t)n_s + 64);   // occupancy of the raw cube / of the PSF temporary
     L.bytes_total = off;
     return L;
 }
@@ -619,7 +621,8 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
         k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot);
         RUBIX_LAUNCH_CHECK();
-        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot, unit_off, part_off, multi, totals);
+        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot, unit_off, part_off, multi, totals,
+                                                     (uint8_t *)(ws + L.off_occ[0]));
         RUBIX_LAUNCH_CHECK();
     }
     k_build_units<<<(unsigned)((L.max_units + 255) / 256), 256, 0, st>>>(seg, unit_off, part_off, n_s, units);

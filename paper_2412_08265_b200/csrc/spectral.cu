@@ -34,6 +34,7 @@ struct AccumParams {
     float *cube;
     float *partials;
     int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
+    int32_t skip_empty;      // 1: empty spaxels are left unwritten (the masked PSF/LSF passes never read them)
     const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
     cudaTextureObject_t tex;
 };
@@ -113,6 +114,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
     const int u = SINGLE ? blockIdx.x : blockIdx.x / P.n_tiles;
     if (u >= P.totals[0]) return;
     const Unit U = P.units[u];
+    if (U.count == 0 && P.skip_empty) return;
     constexpr int TC = CPT * kAccThreads;
     const int k0 = tile * TC;
     const int k_end = min(k0 + TC, P.n_c) - 1;              // last existing channel of this tile
@@ -439,7 +441,8 @@ int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
     return 0;
 }
 
-cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, cudaStream_t st)
+cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
+                              cudaStream_t st)
 {
     const bool logx = table_mode(in.ssp, in.tel);
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
@@ -463,6 +466,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     P.n_tiles = (L.n_c + tc - 1) / tc;
     P.wcap = wcap;
     P.n_lambda = in.ssp->n_lambda;
+    P.skip_empty = skip_empty ? 1 : 0;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.tex = 0;
 #if RUBIX_TEX_CORNERS > 0
