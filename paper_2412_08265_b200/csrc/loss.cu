@@ -26,11 +26,11 @@ __device__ __forceinline__ double block_sum(double v, double *sm)
 
 __global__ void __launch_bounds__(kLossThreads)
 k_residual_loss(const float *__restrict__ cube, const float *__restrict__ target, int64_t n_vox,
-                float *__restrict__ grad, double *__restrict__ partial)
+                float *__restrict__ grad, double *__restrict__ partial, int aligned)
 {
     __shared__ double sm[kLossThreads / 32];
     double acc = 0.0;
-    const int64_t n4 = n_vox >> 2;
+    const int64_t n4 = aligned ? n_vox >> 2 : 0;            // 16-byte accesses only when all three arrays allow them
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
         const float4 c = __ldcs(reinterpret_cast<const float4 *>(cube) + i);
@@ -63,7 +63,8 @@ size_t loss_scratch_bytes() { return align_up((size_t)kLossBlocks * sizeof(doubl
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
                                  double *partial, double *loss, cudaStream_t st)
 {
-    k_residual_loss<<<kLossBlocks, kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial);
+    const int aligned = ((((uintptr_t)cube) | ((uintptr_t)target) | ((uintptr_t)grad)) & 15u) == 0;
+    k_residual_loss<<<kLossBlocks, kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial, aligned);
     RUBIX_LAUNCH_CHECK();
     k_loss_final<<<1, kLossThreads, 0, st>>>(partial, kLossBlocks, loss);
     RUBIX_LAUNCH_CHECK();

@@ -29,9 +29,17 @@ __device__ __forceinline__ void normals4(uint64_t q, uint32_t k0, uint32_t k1, f
     float u[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) u[i] = ((float)(r[i] >> 9) + 0.5f) * (1.0f / 8388608.0f);
-    // hardware approximations (ex2/lg2/sin/cos units): |error| of a deviate stays below 1e-5, far inside the
-    // 1e-4 voxel tolerance, and the kernel stays bandwidth bound instead of transcendental bound
-    const float R0 = sqrtf(-2.0f * __logf(u[0])), R1 = sqrtf(-2.0f * __logf(u[2]));
+    // hardware approximations (lg2 / sin / cos units) keep the kernel bandwidth bound.  lg2.approx has an ABSOLUTE error of
+    // ~2^-21.4 on [0.5, 2], which is a large RELATIVE error of -ln u where u is close to 1: there (1 - u < 2^-6; 1 - u is
+    // exact in fp32) the series t + t^2/2 + t^3/3 + t^4/4 takes over (truncation t^5/5: < 2e-8 relative); the result is clamped at
+    // 0 so that the square root never sees a negative argument.  |error| of a deviate stays below 1e-5.
+    auto neg_log = [](float uu) -> float {
+        const float t = 1.0f - uu;
+        const float series = t * fmaf(t, fmaf(t, fmaf(t, 0.25f, 0.33333334f), 0.5f), 1.0f);
+        const float approx = fmaxf(-__logf(uu), 0.0f);
+        return t < 0.015625f ? series : approx;
+    };
+    const float R0 = sqrtf(2.0f * neg_log(u[0])), R1 = sqrtf(2.0f * neg_log(u[2]));
     // argument reduced to [-pi, pi): u in (0, 1) -> 2 pi (u - 0.5), cos / sin pick up a sign flip
     float s0, c0, s1, c1;
     __sincosf(6.283185307179586f * (u[1] - 0.5f), &s0, &c0);

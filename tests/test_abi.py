@@ -36,6 +36,27 @@ def test_struct_layouts_match_the_header():
     assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 56 and C.sizeof(B.CTelescope) == 72
 
 
+def test_abi_version_and_struct_size_are_checked(lib):
+    """A caller built against another rubix.h (other struct size, or the pre-struct_size layout, whose first field was a
+    small count) is refused before anything is read from the struct."""
+    header = open(os.path.join(ROOT, "include", "rubix.h")).read()
+    assert int(re.search(r"#define RUBIX_ABI_VERSION (\d+)", header).group(1)) == B.ABI_VERSION == lib.rubix_abi_version()
+    P = _fake_particles()
+    for which in ("ssp", "tel"):
+        for bad in (0, 50, 300, C.sizeof(B.CSSP if which == "ssp" else B.CTelescope) + 8):
+            ssp, tel = _structs()
+            (ssp if which == "ssp" else tel).struct.struct_size = bad
+            assert _call_build(lib, P, ssp, tel) == B.RUBIX_ERR_INVALID_ARG
+            assert "struct_size" in B.rubix_last_error()
+            assert lib.rubix_workspace_bytes(10, ssp.ref(), tel.ref()) == 0
+            assert lib.rubix_forward_host_scratch_bytes(10, ssp.ref(), tel.ref()) == 0
+            assert lib.rubix_forward(P.ref(), ssp.ref(), tel.ref(), np.eye(3, dtype=np.float32).ctypes.data, FAKE, FAKE,
+                                     1 << 40, None) == B.RUBIX_ERR_INVALID_ARG
+            if which == "tel":                             # (never reaches a launch: the addresses are fake)
+                assert lib.rubix_convolve_psf_lsf(tel.ref(), FAKE, FAKE + (1 << 33), FAKE + (1 << 34), 1 << 40,
+                                                  None) == B.RUBIX_ERR_INVALID_ARG
+
+
 def _structs(tel=None, ssp=None):
     tel = tel or synth.make_telescope("medium")
     ssp = ssp or synth.make_ssp(8, 4, 512, 3500.0, 9500.0, 1)

@@ -44,6 +44,27 @@ def test_noisy_cube_matches_the_oracle(B, n, sr, gain, seed):
         assert np.abs(dst[1:n].cpu().numpy() - ref1).max() <= 1e-4 * np.abs(ref1).max()
 
 
+def test_extreme_uniform_words(B):
+    """the largest uniform, u = 1 - 2^-24 (Philox word >> 9 = 0x7FFFFF), is where an approximate
+    log loses all relative accuracy of -ln u and may even return a positive value (NaN after the square root).  With
+    seed 4 the first 2^24 voxels contain that word three times (radius sqrt(-2 ln u) = 3.4527e-4; found with the oracle's
+    generator); the deviates there and everywhere else must match the fp64 oracle."""
+    n = 1 << 24
+    z = oracle.noise_normals(n, 4)
+    radius = np.hypot(z[0::2], z[1::2])
+    extreme = np.flatnonzero(radius < 3.5e-4)
+    assert extreme.size == 3 and abs(radius[extreme[0]] - np.sqrt(-2.0 * np.log(1.0 - 2.0 ** -24))) < 1e-12
+    zero = torch.zeros(n, device="cuda")
+    out = torch.empty_like(zero)
+    B.rubix_add_noise(zero, out, 1.0, 0.0, 4)                 # cube = 0, sigma_read = 1: the output IS the deviate
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    assert np.abs(got - z).max() <= 1e-5
+    pair = np.stack([got[2 * extreme], got[2 * extreme + 1]], 1)
+    ref = np.stack([z[2 * extreme], z[2 * extreme + 1]], 1)
+    assert np.abs(pair - ref).max() <= 2e-8                   # 1e-4 relative of the 3.45e-4 radius
+
+
 def test_zero_noise_is_the_identity_and_seeds_differ(B):
     cube = torch.from_numpy(synth.synthetic_cube(4, 4, 100, seed=1)).cuda()
     out = torch.empty_like(cube)
