@@ -54,6 +54,7 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-adjoint", action="store_true")
+    ap.add_argument("--no-batched", action="store_true")
     return ap.parse_args()
 
 
@@ -261,6 +262,75 @@ def time_adjoint(B, synth, dev, l2_peak, reps=10):
                          "algorithmic_bytes_per_launch": gather_b, "kernel_ms": k_ms,
                          "peak_source": "L2->SM read bandwidth measured in this run by rubix_measure_peaks (builder-measured: "
                                         "MEASURED_PEAKS.json has no L2 figure)"}}
+
+
+def time_batched(B, synth, dev, reps=20):
+    """cubes per second for the small cubes (launch-latency bound one at a time) with rubix_forward_batched
+    at B = 1, 16, 64 against B looped rubix_forward calls and against B replays of a CUDA graph of one call.  Each element is
+    the config's galaxy under its own rotation."""
+    import torch
+    out = {}
+    for name in ("tiny", "small"):
+        w = synth.make_workload(name)
+        dw = B.DeviceWorkload(w, device=dev)
+        t = w.telescope
+        res = {}
+        for batch in (1, 16, 64):
+            R = np.stack([synth.euler_rotation(*synth.random_euler(7000 + b)) for b in range(batch)]).astype(np.float32)
+            cubes = torch.empty((batch,) + dw.shape, dtype=torch.float32, device=dev)
+            ws = torch.empty(B.rubix_forward_batched_workspace_bytes(w.particles.n, None, batch, dw.ssp, dw.tel),
+                             dtype=torch.uint8, device=dev)
+
+            def batched():
+                B.rubix_forward_batched(dw.particles, None, batch, dw.ssp, dw.tel, R, cubes, ws)
+
+            def looped():
+                for b in range(batch):
+                    B.rubix_forward(dw.particles, dw.ssp, dw.tel, R[b], cubes[b], dw.workspace)
+
+            def timed(fn, n):
+                for _ in range(3):
+                    fn()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(n):
+                    fn()
+                e1.record()
+                torch.cuda.synchronize()
+                return e0.elapsed_time(e1) / n
+
+            ms_b = timed(batched, reps)
+            launches = B.rubix_last_launch_count()
+            ms_l = timed(looped, max(reps // 4, 2))
+            res[f"B={batch}"] = {"batched_ms": ms_b, "batched_cubes_per_s": batch / ms_b * 1e3, "launches": launches,
+                                 "looped_ms": ms_l, "looped_cubes_per_s": batch / ms_l * 1e3,
+                                 "speedup_over_loop": ms_l / ms_b}
+        # one captured rubix_forward replayed (the rotation is baked into the graph: a lower bound on the looped cost)
+        s = torch.cuda.Stream(device=dev)
+        one = torch.empty(dw.shape, dtype=torch.float32, device=dev)
+        with torch.cuda.stream(s):
+            B.rubix_forward(dw.particles, dw.ssp, dw.tel, dw.R, one, dw.workspace, stream=s.cuda_stream)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            B.rubix_forward(dw.particles, dw.ssp, dw.tel, dw.R, one, dw.workspace, stream=torch.cuda.current_stream().cuda_stream)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(64):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        res["graph_replay_ms_per_cube"] = e0.elapsed_time(e1) / 64
+        res["graph_replay_cubes_per_s"] = 64 / e0.elapsed_time(e1) * 1e3
+        res["speedup_over_graph_replay_at_B=64"] = res["B=64"]["batched_cubes_per_s"] / res["graph_replay_cubes_per_s"]
+        out[name] = res
+    out["what"] = ("rubix_forward_batched (one launch sequence for B cubes) vs B looped rubix_forward calls vs replays of a CUDA "
+                   "graph of one rubix_forward; BASELINE.json configs[0] (tiny) and configs[1] (small), one galaxy under B rotations")
+    return out
 
 
 # ------------------------------------------------------------------------------------- our arm
@@ -554,6 +624,8 @@ def run_ours(args):
             "two_calls": {"ms_per_step": two_call_ms,
                           "api": "rubix_build_cube + rubix_convolve_psf_lsf (dense raw cube, no masks; 5 steps)"}}
     line["roofline"]["whole_step"] = whole_step
+    if not args.no_batched:
+        line["batched"] = time_batched(B, synth, dev)
     line["flux_variant"] = flux_variant
     if table_variant is not None:
         line["log_grid_variant"] = table_variant

@@ -165,6 +165,25 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
 rubix_status rubix_forward(const rubix_particles *particles, const rubix_ssp *ssp, const rubix_telescope *tel,
                            const float *R, float *cube, void *workspace, size_t workspace_bytes, void *stream);
 
+/* Batched steps 1-8 ("produce a sufficient number of samples required for statistical
+ * analysis", L86 SBI): `batch` cubes per call with ONE launch sequence -- the detectors sit side by side in one key space
+ * of batch * N_s spaxels, so the sort, the work units, the accumulate kernel and the PSF/LSF passes each run once for all
+ * elements (small cubes are launch-latency bound one at a time).  Element b is computed exactly as rubix_forward would
+ * (bit-equal cubes).
+ *   particles  DEVICE arrays.  offsets != NULL: `batch` galaxies concatenated, element b = particles
+ *              offsets[b] .. offsets[b+1]) (HOST [batch+1], offsets[0] = 0, offsets[batch] = particles->n, non-decreasing).
+ *              offsets == NULL: the SAME particles->n particles for every element (one galaxy, `batch` orientations).
+ *   R          HOST [batch][9], one rotation per element
+ *   cubes      DEVICE [batch][n_x][n_y][n_channels] fp32, element-major; must not overlap the workspace
+ * Elements are processed in groups of 64 (the rotations travel as kernel parameters); the sort artefacts left in the
+ * workspace are those of the LAST group (keys are element * N_s + spaxel, dropped particles get group size * N_s).
+ * Workspace: rubix_forward_batched_workspace_bytes (returns 0 on invalid arguments). */
+size_t rubix_forward_batched_workspace_bytes(int64_t n, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                             const rubix_telescope *tel);
+rubix_status rubix_forward_batched(const rubix_particles *particles, const int64_t *offsets, int32_t batch,
+                                   const rubix_ssp *ssp, const rubix_telescope *tel, const float *R, float *cubes,
+                                   void *workspace, size_t workspace_bytes, void *stream);
+
 /* Step 9: gradients of a scalar loss L of the FINAL cube
  * (after PSF/LSF, if tel switches them on) with respect to each particle's mass, log age,
  * log Z and line-of-sight velocity.

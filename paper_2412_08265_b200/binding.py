@@ -19,6 +19,7 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf", "rubix_forward",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
+           "rubix_forward_batched_workspace_bytes", "rubix_forward_batched",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
@@ -76,6 +77,13 @@ def load():
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.rubix_forward.restype = C.c_int
         lib.rubix_forward.argtypes = lib.rubix_build_cube.argtypes
+        lib.rubix_forward_batched_workspace_bytes.restype = C.c_size_t
+        lib.rubix_forward_batched_workspace_bytes.argtypes = [C.c_int64, C.c_void_p, C.c_int32, C.POINTER(CSSP),
+                                                              C.POINTER(CTelescope)]
+        lib.rubix_forward_batched.restype = C.c_int
+        lib.rubix_forward_batched.argtypes = [C.POINTER(CParticles), C.c_void_p, C.c_int32, C.POINTER(CSSP),
+                                              C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
+                                              C.c_void_p]
         lib.rubix_convolve_psf_lsf.restype = C.c_int
         lib.rubix_convolve_psf_lsf.argtypes = [C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p,
                                                C.c_size_t, C.c_void_p]
@@ -210,6 +218,29 @@ def rubix_forward(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, 
     _check(load().rubix_forward(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
                                 _ptr(workspace), int(workspace.numel() * workspace.element_size()),
                                 _stream(stream)))
+
+
+def _offsets(offsets):
+    return None if offsets is None else np.ascontiguousarray(offsets, dtype=np.int64)
+
+
+def rubix_forward_batched_workspace_bytes(n, offsets, batch, ssp: _Keep, tel: _Keep) -> int:
+    off = _offsets(offsets)
+    b = int(load().rubix_forward_batched_workspace_bytes(int(n), _ptr(off), int(batch), ssp.ref(), tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_forward_batched(particles: _Keep, offsets, batch, ssp: _Keep, tel: _Keep, R, cubes, workspace, stream=None):
+    """``offsets``: int64 host array [batch + 1] (concatenated galaxies) or None (one galaxy, ``batch`` rotations);
+    ``R``: [batch, 3, 3]; ``cubes``: device tensor [batch, n_x, n_y, n_channels]."""
+    off = _offsets(offsets)
+    R = _host_f32(R).reshape(-1)
+    assert R.size == 9 * int(batch)
+    _check(load().rubix_forward_batched(particles.ref(), _ptr(off), int(batch), ssp.ref(), tel.ref(), R.ctypes.data,
+                                        _ptr(cubes), _ptr(workspace),
+                                        int(workspace.numel() * workspace.element_size()), _stream(stream)))
 
 
 def rubix_convolve_psf_lsf(tel: _Keep, cube_in, cube_out, workspace, stream=None):

@@ -236,9 +236,10 @@ rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, co
 // Steps 1-8 on device buffers.  With the marching PSF/LSF kernels the raw cube lives in the workspace and only the
 // rows of occupied spaxels are written and read (launch_convolve's masks); otherwise the two plain stages run.
 static rubix_status forward_device(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
-                                   const float *R, float *cube_out, const Layout &L, char *ws, cudaStream_t st)
+                                   const float *R, float *cube_out, const Layout &L, char *ws, cudaStream_t st,
+                                   int32_t batch = 1, const int64_t *offsets = nullptr)
 {
-    PassInputs in{p, ssp, tel, R};
+    PassInputs in{p, ssp, tel, R, batch, offsets};
     cudaError_t e;
     {
         StageTimer t(0, st);
@@ -259,9 +260,103 @@ static rubix_status forward_device(const rubix_particles *p, const rubix_ssp *ss
         StageTimer t(3, st);
         e = launch_convolve(tel, raw, cube_out, tmp, (float *)(ws + L.off_psftaps), false,
                             sparse ? (const uint8_t *)(ws + L.off_occ[0]) : nullptr,
-                            sparse ? (uint8_t *)(ws + L.off_occ[1]) : nullptr, st);
+                            sparse ? (uint8_t *)(ws + L.off_occ[1]) : nullptr, st, batch);
     }
     if (e != cudaSuccess) return cuda_fail(e, "convolve");
+    return RUBIX_OK;
+}
+
+// logical particles of the largest group of <= kMaxBatch elements, and that group's element count
+static void batch_groups(int64_t n, int32_t batch, const int64_t *offsets, int64_t *n_max, int32_t *b_max)
+{
+    *b_max = batch < kMaxBatch ? batch : kMaxBatch;
+    if (!offsets) { *n_max = n * *b_max; return; }
+    int64_t m = 0;
+    for (int32_t g0 = 0; g0 < batch; g0 += kMaxBatch) {
+        const int32_t g1 = g0 + kMaxBatch < batch ? g0 + kMaxBatch : batch;
+        if (offsets[g1] - offsets[g0] > m) m = offsets[g1] - offsets[g0];
+    }
+    *n_max = m;
+}
+
+static rubix_status check_batch(const rubix_particles *p, const int64_t *offsets, int32_t batch, const rubix_telescope *tel)
+{
+    if (batch < 1) return fail(RUBIX_ERR_INVALID_ARG, "batch must be >= 1");
+    const int32_t bg = batch < kMaxBatch ? batch : kMaxBatch;
+    if ((double)bg * tel->n_x * tel->n_y >= 2147483647.0 / 2)
+        return fail(RUBIX_ERR_UNSUPPORTED, "batch x spaxels too large for one key space");
+    if (offsets) {
+        if (offsets[0] != 0 || offsets[batch] != p->n)
+            return fail(RUBIX_ERR_INVALID_ARG, "offsets[0] must be 0 and offsets[batch] must equal particles->n");
+        for (int32_t b = 0; b < batch; ++b)
+            if (offsets[b + 1] < offsets[b]) return fail(RUBIX_ERR_INVALID_ARG, "offsets must be non-decreasing");
+    } else if ((double)p->n * bg >= 2147483647.0) {
+        return fail(RUBIX_ERR_UNSUPPORTED, "batch x particles must stay below 2^31 per group of %d elements", kMaxBatch);
+    }
+    return RUBIX_OK;
+}
+
+size_t rubix_forward_batched_workspace_bytes(int64_t n, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                             const rubix_telescope *tel)
+{
+    t_err[0] = 0;
+    if (n < 0 || n >= 2147483647LL) { fail(RUBIX_ERR_INVALID_ARG, "n out of range"); return 0; }
+    if (check_tel(tel) != RUBIX_OK || check_ssp(ssp, false) != RUBIX_OK) return 0;
+    rubix_particles fake{n, nullptr, nullptr, nullptr, nullptr, nullptr};
+    if (check_batch(&fake, offsets, batch, tel) != RUBIX_OK) return 0;
+    int64_t n_max; int32_t b_max;
+    batch_groups(n, batch, offsets, &n_max, &b_max);
+    return make_layout(n_max, b_max * tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda).bytes_total;
+}
+
+rubix_status rubix_forward_batched(const rubix_particles *p, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                   const rubix_telescope *tel, const float *R, float *cubes, void *workspace,
+                                   size_t workspace_bytes, void *stream)
+{
+    Range nvtx_range("rubix_forward_batched");
+    t_err[0] = 0;
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !cubes) return fail(RUBIX_ERR_NULL, "R or cubes is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    if ((s = check_batch(p, offsets, batch, tel)) != RUBIX_OK) return s;
+    int64_t n_max; int32_t b_max;
+    batch_groups(p->n, batch, offsets, &n_max, &b_max);
+    const int32_t n_s = tel->n_x * tel->n_y;
+    const Layout Lmax = make_layout(n_max, b_max * n_s, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda);
+    if ((s = check_ws(workspace, workspace_bytes, Lmax.bytes_total)) != RUBIX_OK) return s;
+    const size_t cube_elems = (size_t)n_s * tel->n_channels;
+    const char *c0 = (const char *)cubes, *w0 = (const char *)workspace;
+    if (c0 < w0 + Lmax.bytes_total && w0 < c0 + cube_elems * 4 * (size_t)batch)
+        return fail(RUBIX_ERR_INVALID_ARG, "cubes overlap the workspace");
+    int launches = 0;
+    for (int32_t g0 = 0; g0 < batch; g0 += kMaxBatch) {       // groups of <= kMaxBatch elements, one launch sequence each
+        const int32_t bg = g0 + kMaxBatch < batch ? kMaxBatch : batch - g0;
+        rubix_particles pg = *p;
+        int64_t off_local[kMaxBatch + 1];
+        if (offsets) {
+            const int64_t first = offsets[g0];
+            pg.n = offsets[g0 + bg] - first;
+            pg.pos = p->pos ? p->pos + 3 * first : nullptr;
+            pg.vel = p->vel ? p->vel + 3 * first : nullptr;
+            pg.mass = p->mass ? p->mass + first : nullptr;
+            pg.log_age = p->log_age ? p->log_age + first : nullptr;
+            pg.log_z = p->log_z ? p->log_z + first : nullptr;
+            for (int32_t b = 0; b <= bg; ++b) off_local[b] = offsets[g0 + b] - first;
+        }
+        const int64_t n_logical = offsets ? pg.n : p->n * bg;
+        const Layout L = make_layout(n_logical, bg * n_s, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda);
+        s = forward_device(&pg, ssp, tel, R + 9 * (size_t)g0, cubes + cube_elems * (size_t)g0, L, (char *)workspace,
+                           (cudaStream_t)stream, bg, offsets ? off_local : nullptr);
+        if (s != RUBIX_OK) return s;
+        launches += g_launches;
+        g_launches = 0;
+        remember(workspace, L);
+    }
+    g_launches = launches;
     return RUBIX_OK;
 }
 

@@ -83,11 +83,19 @@ struct Layout {
 Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t n_lambda);
 
 // ---- host launchers (each returns the CUDA status of its launches) ----------------------------
+constexpr int kMaxBatch = 64;              // batch elements per launch sequence (their rotations travel as kernel parameters)
+
 struct PassInputs {
     const rubix_particles *p;
     const rubix_ssp *ssp;
     const rubix_telescope *tel;
-    const float *R;
+    const float *R;                        // [batch][9]
+    // Batched forward: `batch` detectors side by side in one key space of batch * N_s spaxels.
+    // Logical particle i (0 <= i < Layout::n) belongs to element b with offsets[b] <= i < offsets[b+1] (concatenated
+    // galaxies), or, with offsets == nullptr and batch > 1, to element i / p->n and is physical particle i % p->n
+    // (the same galaxy seen under `batch` rotations).
+    int32_t batch = 1;
+    const int64_t *offsets = nullptr;      // HOST [batch + 1]
 };
 
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
@@ -100,7 +108,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
 // the others are taken as zeros WITHOUT being read (they may be unwritten); occ_tmp [n_s] receives the same
 // mask for the temporary after the first pass, so that all-zero rows cross HBM in neither direction.
 cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
-                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st);
+                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st, int32_t batch = 1);
 // true when launch_convolve would take its marching (fast) path, the only one that honours the masks
 bool convolve_fast_path(const rubix_telescope *tel, const float *in, const float *out, const float *tmp);
 inline size_t psf_taps_bytes(int32_t n_c) { return align_up((size_t)15 * ((size_t)n_c + 2) * 4, 256); }

@@ -82,6 +82,10 @@ struct MarchParams {
     const uint8_t *mask_in;
     uint8_t *mask_out;
     int32_t sp_line, sp_step;
+    // batched cubes: line = element * lines_per_batch + (line inside the element's cube); element b
+    // starts batch_stride floats / sp_batch spaxels after element b - 1; a stencil never crosses into the next cube
+    int32_t lines_per_batch, sp_batch;
+    int64_t batch_stride;
 };
 
 __device__ __forceinline__ float2 shfl_up2(float2 v, int d)
@@ -156,10 +160,11 @@ k_march(const __grid_constant__ MarchParams P)
     const int c = LSF ? cblock * 56 + 2 * (lane - 2) : cblock * 64 + 2 * lane;
     const bool c_ok = c >= 0 && c + 1 < P.n_c;
     const bool st_ok = c_ok && (!LSF || (lane >= 2 && lane < 30));
-    const size_t off = (size_t)line * P.line_stride + (size_t)(c_ok ? c : 0);
+    const int elem = line / P.lines_per_batch, lin = line - elem * P.lines_per_batch;
+    const size_t off = (size_t)elem * P.batch_stride + (size_t)lin * P.line_stride + (size_t)(c_ok ? c : 0);
     const float *src = P.in + off;
     float *dst = P.out + off;
-    const int64_t sp0 = MASK ? (int64_t)line * P.sp_line : 0;
+    const int64_t sp0 = MASK ? (int64_t)elem * P.sp_batch + (int64_t)lin * P.sp_line : 0;
     auto mask_byte = [&](int base) -> uint32_t {           // lane i: occupancy of step base + i
         const int s = base + lane;
         return (lane < 15 && s < P.n_steps) ? (uint32_t)__ldg(P.mask_in + sp0 + (int64_t)s * P.sp_step) : 0u;
@@ -302,10 +307,10 @@ bool convolve_fast_path(const rubix_telescope *tel, const float *in, const float
 }
 
 cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *out, float *tmp, float *taps_dev,
-                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st)
+                            bool transpose, const uint8_t *occ_in, uint8_t *occ_tmp, cudaStream_t st, int32_t batch)
 {
     const int32_t n_x = tel->n_x, n_y = tel->n_y, n_c = tel->n_channels;
-    const int64_t n_vox = (int64_t)n_x * n_y * n_c;
+    const int64_t n_vox = (int64_t)batch * n_x * n_y * n_c;   // `batch` cubes back to back
     if (n_vox == 0) return cudaSuccess;
     Taps lsf, psf;
     make_taps(tel->lsf_size, tel->lsf_sigma, &lsf);
@@ -338,12 +343,15 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     P.mask_in = nullptr;
     P.mask_out = nullptr;
     P.sp_line = P.sp_step = 0;
+    P.lines_per_batch = 1;
+    P.sp_batch = n_x * n_y;
+    P.batch_stride = (int64_t)n_x * n_y * n_c;
     centre_taps(psf, 15, P.g);
     centre_taps(lsf, 9, P.h);
     auto lsf_rows = [&](const float *src, float *dst) -> cudaError_t {
         P.in = src; P.out = dst;
         P.mask_in = masked ? occ_in : nullptr;
-        P.n_lines = n_x * n_y; P.n_steps = 1; P.line_stride = n_c; P.step_stride = 0;
+        P.n_lines = batch * n_x * n_y; P.n_steps = 1; P.line_stride = n_c; P.step_stride = 0;
         P.cblocks = (n_c + 55) / 56;
         const int64_t warps = (int64_t)P.n_lines * P.cblocks;
         k_lsf_rows<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
@@ -352,13 +360,13 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     };
     auto along_y = [&](const float *src, float *dst) {     // lines = x
         P.in = src; P.out = dst;
-        P.n_lines = n_x; P.n_steps = n_y;
+        P.n_lines = batch * n_x; P.n_steps = n_y; P.lines_per_batch = n_x;
         P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
         P.sp_line = n_y; P.sp_step = 1;
     };
     auto along_x = [&](const float *src, float *dst) {     // lines = y
         P.in = src; P.out = dst;
-        P.n_lines = n_y; P.n_steps = n_x;
+        P.n_lines = batch * n_y; P.n_steps = n_x; P.lines_per_batch = n_y;
         P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
         P.sp_line = 1; P.sp_step = n_y;
     };

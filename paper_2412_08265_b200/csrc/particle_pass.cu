@@ -43,6 +43,51 @@ k_rotate_bin(const float *__restrict__ pos, const float *__restrict__ vel, BinPa
     vlos[i] = vl;
 }
 
+// Batched variant: logical particle i belongs to batch element b (its own rotation) and gets the
+// key b * N_s + (key inside its detector); dropped particles get batch * N_s.  Same fp32 arithmetic.
+struct BinBatch {
+    float R[kMaxBatch][9];
+    int64_t off[kMaxBatch + 1];            // concatenated galaxies: element b = particles off[b] .. off[b+1]
+    int32_t batch;
+    int64_t n_phys;                        // > 0: shared galaxy, physical index = i % n_phys, element = i / n_phys
+};
+
+__global__ void __launch_bounds__(256)
+k_rotate_bin_batched(const float *__restrict__ pos, const float *__restrict__ vel, BinParams P,
+                     const __grid_constant__ BinBatch Bt, int32_t *__restrict__ key, float *__restrict__ vlos)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    int b;
+    int64_t ip = i;
+    if (Bt.n_phys > 0) {
+        b = (int)(i / Bt.n_phys);
+        ip = i - (int64_t)b * Bt.n_phys;
+    } else {
+        int lo = 0, hi = Bt.batch - 1;     // largest b with off[b] <= i
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (Bt.off[mid] <= i) lo = mid; else hi = mid - 1;
+        }
+        b = lo;
+    }
+    const float *R = Bt.R[b];
+    const float x = pos[3 * ip], y = pos[3 * ip + 1], z = pos[3 * ip + 2];
+    const float vx = vel[3 * ip], vy = vel[3 * ip + 1], vz = vel[3 * ip + 2];
+    const float xr = __fadd_rn(__fadd_rn(__fmul_rn(R[0], x), __fmul_rn(R[1], y)), __fmul_rn(R[2], z));
+    const float yr = __fadd_rn(__fadd_rn(__fmul_rn(R[3], x), __fmul_rn(R[4], y)), __fmul_rn(R[5], z));
+    const float vl = __fadd_rn(__fadd_rn(__fmul_rn(R[6], vx), __fmul_rn(R[7], vy)), __fmul_rn(R[8], vz));
+    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x), P.s);
+    const float hy = __fmul_rn(__fmul_rn(0.5f, (float)P.n_y), P.s);
+    const float u = __fdiv_rn(__fadd_rn(xr, hx), P.s);
+    const float v = __fdiv_rn(__fadd_rn(yr, hy), P.s);
+    const bool inside = (u >= 0.0f) && (u < (float)P.n_x) && (v >= 0.0f) && (v < (float)P.n_y) &&
+                        (fabsf(vl) <= kVcapKms);
+    const int32_t n_s = P.n_x * P.n_y;
+    key[i] = inside ? b * n_s + (int32_t)floorf(u) * P.n_y + (int32_t)floorf(v) : Bt.batch * n_s;
+    vlos[i] = vl;
+}
+
 // --------------------------------------------------------------------------------------------
 // K2.  Stable LSD radix sort.  Each WARP owns kSortItems consecutive keys ("warp chunk") and is
 // one column of the classic counting-sort histogram matrix histT[digit][warp chunk]; ranks
@@ -317,6 +362,7 @@ struct PrepParams {
     float redshift, flux_scale;         // DESIGN.md reading R14
     int32_t log_grid, table;            // table mode (R15 / R16): x_k = xtab[k] c + a
     const int64_t *xtab;
+    int64_t n_phys;                     // > 0: batched call on a shared galaxy, physical particle = perm value % n_phys
 };
 
 __device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *cell, double *t)
@@ -341,7 +387,8 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= seg_off[P.n_s]) return;            // dropped particles sort last and get no record
-    const int p = perm[i];
+    const int pl = perm[i];                       // logical particle: indexes v_los
+    const int p = P.n_phys > 0 ? (int)(pl % P.n_phys) : pl;   // physical particle: indexes the caller's arrays
     int ia, iz;
     double ta, tz;
     axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta);
@@ -364,7 +411,7 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     r.w[2] = (float)(m * (1.0 - ta) * tz);
     r.w[3] = (float)(m * ta * tz);
     r.cell = (ia * P.ax.n_z + iz) * P.pitch;
-    const double inv = 1.0 / ((1.0 + (double)vlos[p] / kCkms) * (1.0 + (double)P.redshift));
+    const double inv = 1.0 / ((1.0 + (double)vlos[pl] / kCkms) * (1.0 + (double)P.redshift));
     const double scale = (double)(1 << kFxFrac);
     const double A = ((double)P.l0_obs * inv - (double)P.l0_ssp) / (double)P.dl_ssp;
     const double B = (double)P.dl_obs * inv / (double)P.dl_ssp;
@@ -379,7 +426,7 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     if (P.table) {
         // x_k = llrint(Y[k] c) + a_fx, c quantised to 2.30 fixed point so that every kernel uses the same value;
         // Y is increasing, so the covered channels are found by bisection
-        const double opb = 1.0 + (double)vlos[p] / kCkms;
+        const double opb = 1.0 + (double)vlos[pl] / kCkms;
         c_fx = P.log_grid ? (1u << 30) : (uint32_t)__double2ll_rn((double)(1u << 30) / opb);
         const double c = (double)c_fx * (1.0 / (double)(1u << 30));
         a_fx = P.log_grid ? -__double2ll_rn(log10(opb) / (double)P.dl_ssp * scale)
@@ -584,7 +631,17 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         B.n_y = in.tel->n_y;
         B.s = in.tel->spaxel_size;
         B.n = n;
-        k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, key, vlos);
+        if (in.batch > 1 || in.offsets) {
+            BinBatch Bt;
+            Bt.batch = in.batch;
+            Bt.n_phys = in.offsets ? 0 : in.p->n;
+            for (int b = 0; b < in.batch; ++b)
+                for (int i = 0; i < 9; ++i) Bt.R[b][i] = in.R[9 * b + i];
+            for (int b = 0; b <= in.batch; ++b) Bt.off[b] = in.offsets ? in.offsets[b] : 0;
+            k_rotate_bin_batched<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, Bt, key, vlos);
+        } else {
+            k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, key, vlos);
+        }
         RUBIX_LAUNCH_CHECK();
 
         const int mask = (1 << L.digit_bits) - 1;
@@ -640,6 +697,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.mode = in.tel->resample;
         P.log_grid = in.ssp->log_lambda;
         P.table = table_mode(in.ssp, in.tel) ? 1 : 0;
+        P.n_phys = (in.batch > 1 && !in.offsets) ? in.p->n : 0;
         P.xtab = (const int64_t *)(ws + L.off_xtab);
         if (P.table) {
             const float *lam_dev = nullptr;
