@@ -55,31 +55,41 @@ def n_threads() -> int:
 
 
 def _mode(tel, ssp):
-    """bit 0: resampling rule (0 point-sampled, 1 flux-conserving); bit 1: log-sampled SSP grid."""
+    """bit 0: resampling rule (0 point-sampled, 1 bin average); bit 1: log-sampled SSP grid (R15);
+    bit 2: listed SSP wavelengths (R21, ``ssp.lambda_grid``)."""
     resample, log_grid = int(getattr(tel, "resample", 0)), int(getattr(ssp, "log_lambda", 0))
-    if resample == 1 and log_grid:
-        raise NotImplementedError("flux-conserving resampling is defined for linearly sampled SSP grids only")
-    return resample | (log_grid << 1)
+    listed = getattr(ssp, "lambda_grid", None) is not None
+    if listed and log_grid:
+        raise ValueError("an SSP grid is either log-sampled or listed, not both")
+    return resample | (log_grid << 1) | (4 if listed else 0)
 
 
-class _lambda_obs:
-    """Installs tel.lambda_obs (explicit observed wavelengths, reading R16) in the C oracle for one call."""
+class _grids:
+    """Installs tel.lambda_obs (explicit observed wavelengths, reading R16) and ssp.lambda_grid (listed SSP
+    wavelengths, reading R21) in the C oracle for one call."""
 
-    def __init__(self, tel):
+    def __init__(self, tel, ssp=None):
         arr = getattr(tel, "lambda_obs", None)
         self.arr = None if arr is None else np.ascontiguousarray(arr, dtype=np.float32)
         self.zp1 = 1.0 + float(getattr(tel, "redshift", 0.0))
-        if self.arr is not None and int(getattr(tel, "resample", 0)) != 0:
-            raise NotImplementedError("explicit observed wavelengths support the point-sampled rule only")
+        if self.arr is not None and int(getattr(tel, "resample", 0)) != 0 and self.arr.size < 2:
+            raise ValueError("the bin average on listed channel wavelengths needs at least two channels")
+        grid = None if ssp is None else getattr(ssp, "lambda_grid", None)
+        self.grid = None if grid is None else np.ascontiguousarray(grid, dtype=np.float32)
 
     def __enter__(self):
         if self.arr is not None:
             assert self.arr.size == 0 or np.all(np.diff(self.arr) > 0)
             _load().orc_set_lambda_obs(_pf(self.arr), C.c_double(self.zp1))
+        if self.grid is not None:
+            assert np.all(np.diff(self.grid) > 0)
+            _load().orc_set_lambda_ssp(_pf(self.grid))
 
     def __exit__(self, *exc):
         if self.arr is not None:
             _load().orc_set_lambda_obs(None, C.c_double(1.0))
+        if self.grid is not None:
+            _load().orc_set_lambda_ssp(None)
 
 
 def _f32(a):
@@ -141,7 +151,7 @@ def particle_spectrum(mass, log_age, log_z, vlos, ssp, tel):
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    with _lambda_obs(tel):
+    with _grids(tel, ssp):
         _load().orc_particle_spectrum_mode(
             C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
             C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_float(float(mass)), C.c_float(float(log_age)), C.c_float(float(log_z)),
@@ -158,7 +168,7 @@ def particle_spectrum_f64(mass, log_age, log_z, vlos, ia, iz, ssp, tel):
     na, nz, nl = flux.shape
     age_axis, z_axis = _f32(ssp.log_age_axis), _f32(ssp.log_z_axis)
     out = np.empty(tel.n_channels, np.float64)
-    with _lambda_obs(tel):
+    with _grids(tel, ssp):
         _load().orc_particle_spectrum_f64_mode(
             C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
             C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_double(float(mass)), C.c_double(float(log_age)), C.c_double(float(log_z)),
@@ -186,7 +196,7 @@ def build_cube(particles, R, ssp, tel, sel=None):
         sel_arr = np.ascontiguousarray(sel, dtype=np.int32)
         n_sel = sel_arr.size
         cube = np.empty((n_sel, n_c), np.float64)
-    with _lambda_obs(tel):
+    with _grids(tel, ssp):
         _load().orc_build_cube_mode(
             C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
             C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(mass.shape[0]), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R),
@@ -286,7 +296,7 @@ def adjoint(particles, R, ssp, tel, grad_cube):
     grad_cube = np.ascontiguousarray(grad_cube, dtype=np.float64)
     n = mass.shape[0]
     out = [np.empty(n, np.float64) for _ in range(4)]
-    with _lambda_obs(tel), _psf_sigma(psf_sigma_k(tel)):
+    with _grids(tel, ssp), _psf_sigma(psf_sigma_k(tel)):
         _load().orc_adjoint_mode(
             C.c_int32(_mode(tel, ssp)), C.c_double(float(getattr(tel, "redshift", 0.0))),
             C.c_double(float(getattr(tel, "flux_scale", 1.0))), C.c_int64(n), _pf(pos), _pf(vel), _pf(mass), _pf(la), _pf(lz), _pf(R), C.c_int32(na),
@@ -312,7 +322,11 @@ def knot_clearance(vlos, ssp, tel, chunk=4096):
     for a in range(0, vlos.shape[0], chunk):
         beta = vlos[a:a + chunk, None] / C_KMS
         rest = lam[None, :] / (1.0 + beta)
-        if int(getattr(ssp, "log_lambda", 0)):
+        if getattr(ssp, "lambda_grid", None) is not None:              # listed SSP wavelengths (R21)
+            knots = np.asarray(ssp.lambda_grid, np.float32).astype(np.float64)
+            x = np.interp(rest, knots, np.arange(knots.size, dtype=np.float64))
+            x = np.where((rest < knots[0]) | (rest > knots[-1]), 0.5, x)    # channels outside the coverage have no kink
+        elif int(getattr(ssp, "log_lambda", 0)):
             x = np.log10(rest / np.float64(ssp.lambda0)) / np.float64(ssp.dlambda)
         else:
             x = (rest - np.float64(ssp.lambda0)) / np.float64(ssp.dlambda)

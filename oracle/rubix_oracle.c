@@ -32,7 +32,11 @@
  * exact total-flux telescoping (flux-conserving resampling, tests/test_oracle_fluxcons.py);
  * numpy.interp at the doubly shifted wavelength, in log lambda, and at listed channel wavelengths
  * (redshift, log-sampled grids, explicit observed grids: tests/test_oracle_redshift.py,
- * test_oracle_loggrid.py, test_oracle_obsgrid.py), each with finite-difference and closed-form adjoint pins.
+ * test_oracle_loggrid.py, test_oracle_obsgrid.py), each with finite-difference and closed-form adjoint pins;
+ * the bin average on log-sampled grids / listed channel wavelengths and listed SSP wavelengths (readings R20, R21:
+ * particle_spectrum_general) against a prefix-integral restatement, numpy.interp on the knots, the telescoping sum,
+ * constant / linear-in-x closed forms, reduction to the uniform-grid functions and central finite differences
+ * (tests/test_oracle_gengrid.py).
  * No function here is "parity unpinned".
  *
  * No blocking, fusion or reordering beyond the definitions; the only parallelism is an
@@ -235,14 +239,161 @@ static void particle_spectrum_flux(double mass, int32_t ia, int32_t iz, double t
     }
 }
 
-/* mode bit 0: 0 = point-sampled linear interpolation, 1 = bin average (R13);
- * mode bit 1: SSP grid log-sampled (R15; point-sampled rule only) */
+/* ------------------------------------------------------------------------------------
+ * Step 5 on general grids ("Additional resampling is performed to match the
+ * wavelength grid of the observed telescope", L44 the experiment's library "Mastar_CB19_SLOG_1_5" is log-sampled;
+ * DESIGN.md readings R20, R21).  One definition covers every combination of
+ *   SSP grid       kind 0  lambda_j = l0 + j dl                 sampling coordinate x = (lambda - l0) / dl
+ *                  kind 1  lambda_j = l0 10^(j dl)  (R15)       x = log10(lambda / l0) / dl
+ *                  kind 2  lambda_j listed, increasing (R21)    x = j + (lambda - lambda_j) / (lambda_{j+1} - lambda_j)
+ *                          on knot interval j (continued linearly with the first / last interval outside the coverage)
+ *   observed grid  uniform l0_obs + k dl_obs, or listed lambda_obs[k] (R16)
+ *   rule           point:  F[k] = S~(x(lambda_k / (1+beta)))
+ *                  bin average (R20):  channel k is the bin [e_k, e_{k+1}] of OBSERVED wavelength -- e_k = lambda_k - dl_obs/2
+ *                          on a uniform grid; on a listed grid the midpoints of neighbouring channels, the first and last
+ *                          edge half a neighbouring spacing outside -- and
+ *                              F[k] = (1 / (x_hi - x_lo)) * integral_{x_lo}^{x_hi} S~(x) dx,   x_lo/hi = x(e / (1+beta)),
+ *                          the average of the interpolant over the bin IN THE SAMPLING COORDINATE x (S~ = 0 outside the
+ *                          coverage, the bin keeps its full width).  On a linearly sampled grid x is affine in lambda and
+ *                          this is R13 exactly; on a log-sampled grid it is the average per unit log lambda, which differs
+ *                          from the average per unit lambda by O((dl_obs / lambda)^2).  sum_k F[k] (x_hi - x_lo)_k telescopes
+ *                          to the integral of S~ over the covered part of the detector.
+ * S~(x) = S_j + (x - j)(S_{j+1} - S_j), j = floor(x), is the piecewise-linear interpolant of the blended samples in x
+ * for every kind (numpy.interp in lambda, in log lambda, or on the listed knots).
+ * If dF (length k_end) is non-NULL it receives dF[k] / d beta (analytic; edges clipped to the coverage do not move).
+ * ------------------------------------------------------------------------------------ */
+static const float *g_lambda_ssp = 0;      /* kind 2: listed SSP wavelengths [n_lambda], installed around one call */
+void orc_set_lambda_ssp(const float *lambda_ssp) { g_lambda_ssp = lambda_ssp; }
+
+/* sampling coordinate of rest wavelength lam and d x / d lambda there */
+static double sample_coord(double lam, int32_t kind, double l0, double dl, int32_t n_lambda, double *dxdlam)
+{
+    if (kind == 0) { *dxdlam = 1.0 / dl; return (lam - l0) / dl; }
+    if (kind == 1) { *dxdlam = 1.0 / (lam * dl * log(10.0)); return log10(lam / l0) / dl; }
+    const float *L = g_lambda_ssp;
+    int32_t j = 0;
+    if (lam >= (double)L[n_lambda - 1]) j = n_lambda - 2;
+    else if (lam > (double)L[0]) {
+        int32_t lo = 0, hi = n_lambda - 1;             /* largest j with L[j] <= lam */
+        while (lo < hi) { const int32_t mid = (lo + hi + 1) / 2; if ((double)L[mid] <= lam) lo = mid; else hi = mid - 1; }
+        j = lo > n_lambda - 2 ? n_lambda - 2 : lo;
+    }
+    const double w = (double)L[j + 1] - (double)L[j];
+    *dxdlam = 1.0 / w;
+    return (double)j + (lam - (double)L[j]) / w;
+}
+
+typedef struct { const float *T[4]; double w[4]; double mass; int32_t n_lambda; } blend_t;
+static double blend_sample(const blend_t *b, int32_t j)
+{
+    return b->mass * (b->w[0] * b->T[0][j] + b->w[1] * b->T[1][j] + b->w[2] * b->T[2][j] + b->w[3] * b->T[3][j]);
+}
+/* S~(x), 0 outside [0, n_lambda - 1] */
+static double interpolant(const blend_t *b, double x)
+{
+    if (x < 0.0 || x > (double)(b->n_lambda - 1)) return 0.0;
+    int32_t j = (int32_t)floor(x);
+    if (j > b->n_lambda - 2) j = b->n_lambda - 2;
+    const double s0 = blend_sample(b, j), s1 = blend_sample(b, j + 1);
+    return s0 + (x - (double)j) * (s1 - s0);
+}
+/* integral of S~ over [a, c] clipped to the coverage, one knot interval at a time (a trapezoid is exact) */
+static double interpolant_integral(const blend_t *b, double a, double c)
+{
+    const double x_last = (double)(b->n_lambda - 1);
+    if (a < 0.0) a = 0.0;
+    if (c > x_last) c = x_last;
+    double total = 0.0, pos = a;
+    while (pos < c) {
+        int32_t j = (int32_t)floor(pos);
+        if (j > b->n_lambda - 2) j = b->n_lambda - 2;
+        double next = (double)(j + 1);
+        if (next > c) next = c;
+        const double s0 = blend_sample(b, j), s1 = blend_sample(b, j + 1);
+        const double va = s0 + (pos - (double)j) * (s1 - s0), vb = s0 + (next - (double)j) * (s1 - s0);
+        total += 0.5 * (next - pos) * (va + vb);
+        pos = next;
+    }
+    return total;
+}
+
+/* observed bin edge e (0 <= e <= n_c) of reading R20, already divided by (1 + z) like observed_lambda */
+static double observed_edge(int32_t e, int32_t n_c, double l0_obs, double dl_obs)
+{
+    if (!g_lambda_obs) return l0_obs + dl_obs * ((double)e - 0.5);
+    if (n_c < 2) return 0.0;                                       /* refused by the wrapper */
+    if (e == 0) return observed_lambda(0, 0, 0) - 0.5 * (observed_lambda(1, 0, 0) - observed_lambda(0, 0, 0));
+    if (e == n_c) return observed_lambda(n_c - 1, 0, 0) + 0.5 * (observed_lambda(n_c - 1, 0, 0) - observed_lambda(n_c - 2, 0, 0));
+    return 0.5 * (observed_lambda(e - 1, 0, 0) + observed_lambda(e, 0, 0));
+}
+
+static void particle_spectrum_general(int32_t rule, int32_t kind, double mass, int32_t ia, int32_t iz, double ta, double tz,
+                                      double vlos, const float *flux, int32_t n_z, int32_t n_lambda, double l0_ssp,
+                                      double dl_ssp, int32_t k_begin, int32_t k_end, int32_t n_c, double l0_obs,
+                                      double dl_obs, double *F, double *dF)
+{
+    blend_t b;
+    b.T[0] = flux + ((int64_t)ia * n_z + iz) * n_lambda;
+    b.T[1] = flux + ((int64_t)(ia + 1) * n_z + iz) * n_lambda;
+    b.T[2] = flux + ((int64_t)ia * n_z + iz + 1) * n_lambda;
+    b.T[3] = flux + ((int64_t)(ia + 1) * n_z + iz + 1) * n_lambda;
+    b.w[0] = (1.0 - ta) * (1.0 - tz); b.w[1] = ta * (1.0 - tz); b.w[2] = (1.0 - ta) * tz; b.w[3] = ta * tz;
+    b.mass = mass;
+    b.n_lambda = n_lambda;
+    const double opb = 1.0 + vlos / ORC_C_KMS, x_last = (double)(n_lambda - 1);
+    for (int32_t k = k_begin; k < k_end; ++k) {
+        if (rule == 0) {
+            const double lam = observed_lambda(k, l0_obs, dl_obs) / opb;
+            double dxdl;
+            const double x = sample_coord(lam, kind, l0_ssp, dl_ssp, n_lambda, &dxdl);
+            F[k] = interpolant(&b, x);
+            if (dF) {                                              /* dF/dbeta = S~'(x) dx/dlambda dlambda/dbeta */
+                double slope = 0.0;
+                if (x >= 0.0 && x <= x_last) {
+                    int32_t j = (int32_t)floor(x);
+                    if (j > n_lambda - 2) j = n_lambda - 2;
+                    slope = blend_sample(&b, j + 1) - blend_sample(&b, j);
+                }
+                dF[k] = slope * dxdl * (-lam / opb);
+            }
+        } else {
+            const double lam_lo = observed_edge(k, n_c, l0_obs, dl_obs) / opb, lam_hi = observed_edge(k + 1, n_c, l0_obs, dl_obs) / opb;
+            double dlo, dhi;
+            const double x_lo = sample_coord(lam_lo, kind, l0_ssp, dl_ssp, n_lambda, &dlo);
+            const double x_hi = sample_coord(lam_hi, kind, l0_ssp, dl_ssp, n_lambda, &dhi);
+            const double W = x_hi - x_lo;
+            const double I = interpolant_integral(&b, x_lo, x_hi);
+            F[k] = I / W;
+            if (dF) {
+                /* F = I / W:  I' = S~(x_hi) x_hi' - S~(x_lo) x_lo'  (S~ = 0 at a clipped edge),  W' = x_hi' - x_lo' */
+                const double xlo_b = dlo * (-lam_lo / opb), xhi_b = dhi * (-lam_hi / opb);
+                const double Ip = interpolant(&b, x_hi) * xhi_b - interpolant(&b, x_lo) * xlo_b;
+                dF[k] = Ip / W - F[k] * (xhi_b - xlo_b) / W;
+            }
+        }
+    }
+}
+
+/* mode bit 0: 0 = point-sampled linear interpolation, 1 = bin average (R13 / R20);
+ * mode bit 1: SSP grid log-sampled (R15);  mode bit 2: SSP wavelengths listed (R21, orc_set_lambda_ssp).
+ * The combinations added by readings R20 / R21 (bin average on a log-sampled grid or on listed channel
+ * wavelengths; listed SSP wavelengths) go through particle_spectrum_general, the others through the
+ * functions above, whose arithmetic is unchanged. */
+static int32_t general_mode(int32_t mode)
+{
+    return (mode & 4) != 0 || ((mode & 1) != 0 && ((mode & 2) != 0 || g_lambda_obs != 0));
+}
+static int32_t grid_kind(int32_t mode) { return (mode & 4) ? 2 : ((mode & 2) ? 1 : 0); }
+
 static void particle_spectrum_mode(int32_t mode, double mass, int32_t ia, int32_t iz, double ta,
                                    double tz, double vlos, const float *flux, int32_t n_z,
                                    int32_t n_lambda, double l0_ssp, double dl_ssp, int32_t k_begin,
-                                   int32_t k_end, double l0_obs, double dl_obs, double *F)
+                                   int32_t k_end, int32_t n_c, double l0_obs, double dl_obs, double *F)
 {
-    if ((mode & 1) == 1)
+    if (general_mode(mode))
+        particle_spectrum_general(mode & 1, grid_kind(mode), mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp,
+                                  dl_ssp, k_begin, k_end, n_c, l0_obs, dl_obs, F, 0);
+    else if ((mode & 1) == 1)
         particle_spectrum_flux(mass, ia, iz, ta, tz, vlos, flux, n_z, n_lambda, l0_ssp, dl_ssp,
                                k_begin, k_end, l0_obs, dl_obs, F);
     else
@@ -265,7 +416,7 @@ void orc_particle_spectrum_mode(int32_t mode, double zc, double scale, float mas
     axis_cell(age_axis, n_age, log_age, &ia, &ta);
     axis_cell(z_axis, n_z, log_z, &iz, &tz);
     particle_spectrum_mode(mode, scale * (double)mass, ia, iz, ta, tz, (double)vlos, flux, n_z, n_lambda,
-                           (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs / (1.0 + zc),
+                           (double)l0_ssp, (double)dl_ssp, 0, n_c, n_c, (double)l0_obs / (1.0 + zc),
                            (double)dl_obs / (1.0 + zc), F);
 }
 
@@ -295,7 +446,7 @@ void orc_particle_spectrum_f64_mode(int32_t mode, double zc, double scale, doubl
     const double z0 = z_axis[iz], z1 = z_axis[iz + 1];
     (void)n_age;
     particle_spectrum_mode(mode, scale * mass, ia, iz, (log_age - a0) / (a1 - a0), (log_z - z0) / (z1 - z0),
-                           vlos, flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c,
+                           vlos, flux, n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c, n_c,
                            (double)l0_obs / (1.0 + zc), (double)dl_obs / (1.0 + zc), F);
 }
 
@@ -351,7 +502,7 @@ void orc_build_cube_mode(int32_t mode, double zc, double scale, int64_t n, const
                     axis_cell(age_axis, n_age, log_age[p], &ia, &ta);
                     axis_cell(z_axis, n_z, log_z[p], &iz, &tz);
                     particle_spectrum_mode(mode, scale * (double)mass[p], ia, iz, ta, tz, (double)vlos[p], flux,
-                                           n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke,
+                                           n_z, n_lambda, (double)l0_ssp, (double)dl_ssp, kb, ke, n_c,
                                            (double)l0_obs / (1.0 + zc), (double)dl_obs / (1.0 + zc), F);
                     for (int32_t k = kb; k < ke; ++k) row[k] += F[k];
                 }
@@ -578,14 +729,20 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
             for (int32_t c = 0; c < 4; ++c) {
                 const double cta = (c & 1) ? 1.0 : 0.0, ctz = (c & 2) ? 1.0 : 0.0;
                 particle_spectrum_mode(mode, 1.0, ia, iz, cta, ctz, (double)vlos[p], flux, n_z, n_lambda,
-                                       (double)l0_ssp, (double)dl_ssp, 0, n_c, (double)l0_obs,
+                                       (double)l0_ssp, (double)dl_ssp, 0, n_c, n_c, (double)l0_obs,
                                        (double)dl_obs, F);
                 double acc = 0.0;
                 for (int32_t k = 0; k < n_c; ++k) acc += g[k] * F[k];
                 D[c] = acc;  /* c = 0:(i,j) 1:(i+1,j) 2:(i,j+1) 3:(i+1,j+1) */
             }
             double E = 0.0;
-            if ((mode & 1) == 1) {
+            if (general_mode(mode)) {
+                /* readings R20 / R21: sum_k g[k] dF[k]/dbeta of the blended unit-mass spectrum, analytic */
+                particle_spectrum_general(mode & 1, grid_kind(mode), 1.0, ia, iz, ta, tz, (double)vlos[p], flux, n_z,
+                                          n_lambda, (double)l0_ssp, (double)dl_ssp, 0, n_c, n_c, (double)l0_obs,
+                                          (double)dl_obs, F, dS);
+                for (int32_t k = 0; k < n_c; ++k) E += g[k] * dS[k];
+            } else if ((mode & 1) == 1) {
                 /* Flux-conserving rule.  F[k] = (C(x_hi) - C(x_lo)) / B with C' = S~, the bin edges
                  * x(lambda_e) = (lambda_e/(1+beta) - l0_ssp)/dl_ssp and B = dl_obs/((1+beta) dl_ssp):
                  *   dF[k]/dbeta = F[k]/(1+beta) - (lambda_hi S~(x_hi) - lambda_lo S~(x_lo)) / (dl_obs (1+beta)),
@@ -629,7 +786,9 @@ void orc_adjoint_mode(int32_t mode, double zc, double scale, int64_t n, const fl
                                   : 0.0;
             g_log_z[p] = z_free ? m * (-(1 - ta) * D[0] - ta * D[1] + (1 - ta) * D[2] + ta * D[3]) / dZ
                                 : 0.0;
-            if ((mode & 1) == 1)
+            if (general_mode(mode))
+                g_vlos[p] = m * E / ORC_C_KMS;                     /* d/dv_los = (1/c) d/dbeta */
+            else if ((mode & 1) == 1)
                 g_vlos[p] = m * (g_mass[p] - E / (double)dl_obs) / (ORC_C_KMS * (1.0 + beta));
             else
                 g_vlos[p] = -m * E / (ORC_C_KMS * (1.0 + beta) * (1.0 + beta));

@@ -122,12 +122,15 @@ class SSPGrid:
     dlambda: np.float32       # uniform rest step: Angstrom, or dex (log10) when log_lambda = 1
     flux: np.ndarray          # [n_age, n_z, n_lambda] fp32, per unit mass, > 0
     log_lambda: int = 0       # 1: log-sampled grid, lambda_j = lambda0 * 10^(j dlambda)
+    lambda_grid: np.ndarray | None = None   # listed rest wavelengths [n_lambda] fp32, strictly increasing (irregular grid)
 
     @property
     def shape(self):
         return self.flux.shape
 
     def wavelengths(self) -> np.ndarray:
+        if self.lambda_grid is not None:
+            return np.asarray(self.lambda_grid, np.float32).astype(np.float64)
         j = np.arange(self.flux.shape[2])
         if self.log_lambda:
             return np.float64(self.lambda0) * 10.0 ** (np.float64(self.dlambda) * j)
@@ -143,9 +146,11 @@ def _jittered_axis(rng, lo, hi, n):
 
 
 def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
-             seed: int, n_lines: int = 10, log_lambda: bool = False) -> SSPGrid:
+             seed: int, n_lines: int = 10, log_lambda: bool = False, irregular: bool = False) -> SSPGrid:
     """Smooth positive continuum times ``n_lines`` Gaussian absorption lines whose depths vary
-    with age and Z (BASELINE.json configs[0]; recipe SURVEY.md §8(d))."""
+    with age and Z (BASELINE.json configs[0]; recipe SURVEY.md §8(d)).  ``irregular``: the same recipe sampled at
+    listed wavelengths -- the uniform knots with the interior ones moved by up to +-35 % of the spacing and a region
+    of doubled sampling density in the middle third (as merged / multi-arm libraries have)."""
     rng = np.random.Generator(np.random.PCG64(seed))
     age_ax = _jittered_axis(rng, math.log10(0.1), math.log10(13.5), n_age)
     z_ax = _jittered_axis(rng, -4.0, math.log10(0.03), n_z)
@@ -154,6 +159,15 @@ def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
     dlog = math.log10(lam_hi / lam_lo) / (n_lambda - 1)
     if log_lambda:                                         # same recipe on a log-sampled grid (MaStar "SLOG")
         lam = lam_lo * 10.0 ** (dlog * np.arange(n_lambda))
+    if irregular:                                          # own generator: the draws below stay those of the uniform grid
+        rj = np.random.Generator(np.random.PCG64(seed + 1_000_003))
+        t = np.linspace(0.0, 1.0, n_lambda)
+        dens = 1.0 + ((t > 1.0 / 3.0) & (t < 2.0 / 3.0))     # doubled density in the middle third
+        pos = np.concatenate([[0.0], np.cumsum(1.0 / (0.5 * (dens[1:] + dens[:-1])))])
+        lam = lam_lo + (lam_hi - lam_lo) * pos / pos[-1]
+        step = np.minimum(np.diff(lam)[1:], np.diff(lam)[:-1])
+        lam[1:-1] += rj.uniform(-0.35, 0.35, n_lambda - 2) * step
+        lam = lam.astype(np.float32).astype(np.float64)       # the knots the library sees
     u = ((age_ax - age_ax[0]) / (age_ax[-1] - age_ax[0]))[:, None, None]
     w = ((z_ax - z_ax[0]) / (z_ax[-1] - z_ax[0]))[None, :, None]
     ell = (lam / 5500.0)[None, None, :]
@@ -168,7 +182,8 @@ def make_ssp(n_age: int, n_z: int, n_lambda: int, lam_lo: float, lam_hi: float,
         flux = flux * (1.0 - d * np.exp(-0.5 * ((lam[None, None, :] - centre[l]) / width[l]) ** 2))
     return SSPGrid(age_ax.astype(np.float32), z_ax.astype(np.float32),
                    np.float32(lam_lo), np.float32(dlog if log_lambda else dlam),
-                   np.ascontiguousarray(flux, dtype=np.float32), 1 if log_lambda else 0)
+                   np.ascontiguousarray(flux, dtype=np.float32), 1 if log_lambda else 0,
+                   lam.astype(np.float32) if irregular else None)
 
 
 # --------------------------------------------------------------------------------------
