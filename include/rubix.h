@@ -21,7 +21,7 @@
  *     Consequently a sequence of calls can be captured in a CUDA graph (stage timing of
  *     rubix_peaks.h off) and replayed; the kernels read their sizes from the workspace, not
  *     from the host, after the call has returned.  NOT capturable: calls with rubix_telescope.lambda_obs
- *     (the host array is copied to the workspace) and calls that apply a wavelength-dependent PSF
+ *     or rubix_ssp.lambda_grid (the host arrays are copied to the workspace) and calls that apply a wavelength-dependent PSF
  *     (psf_alpha != 0 with psf_size > 0: the per-channel taps are computed on the host and copied from
  *     pageable memory); the rubix_forward_host* entries (host buffers).
  *   - Every compute call is bracketed by an NVTX range carrying its name (visible in Nsight timelines).
@@ -77,7 +77,12 @@ typedef struct {
                                     /* 1: log-sampled grid (e.g. MaStar "SLOG"): */
                                     /*    lambda_j = lambda0 * 10^(j dlambda), dlambda in dex; */
                                     /*    the interpolant is then linear in log lambda between */
-                                    /*    knots; RUBIX_RESAMPLE_POINT only                     */
+                                    /*    knots                                                */
+    const float *lambda_grid;       /* HOST [n_lambda] or NULL.  Non-NULL: LISTED rest wavelengths   */
+                                    /* (Angstrom, > 0, strictly increasing; irregular sampling as in */
+                                    /* merged libraries) replace lambda0 / dlambda / log_lambda (which */
+                                    /* must be 0); the interpolant is linear between the listed knots. */
+                                    /* Read and copied to the workspace before the call returns.       */
 } rubix_ssp;
 
 /* Detector ("telescope-specific configurations", L44 Gaussian PSF and LSF). */
@@ -98,8 +103,10 @@ typedef struct {
                                     /* dimming / unit conversion chosen by the caller); 1 = off */
     const float *lambda_obs;        /* HOST [n_channels] or NULL.  Non-NULL: explicit channel   */
                                     /* wavelengths (Angstrom, > 0, strictly increasing) replace  */
-                                    /* lambda0 + k dlambda; RUBIX_RESAMPLE_POINT only.  Read (and */
-                                    /* copied to the workspace) before the call returns.         */
+                                    /* lambda0 + k dlambda.  With RUBIX_RESAMPLE_FLUX (needs       */
+                                    /* n_channels >= 2) channel k is the bin between the midpoints  */
+                                    /* to its neighbours (outer edges half a spacing outside).  Read */
+                                    /* (and copied to the workspace) before the call returns.       */
     float psf_alpha;                /* wavelength-dependent PSF: channel k uses the width         */
     float psf_lambda_ref;           /* psf_sigma (lambda_k / psf_lambda_ref)^psf_alpha (e.g. -0.2 */
                                     /* for seeing); 0 = the same PSF for every channel.  Needs    */
@@ -109,7 +116,7 @@ typedef struct {
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 3
+#define RUBIX_ABI_VERSION 4
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -121,7 +128,11 @@ uint32_t rubix_abi_version(void);
  *                         [lambda_k - dlambda_obs/2, lambda_k + dlambda_obs/2], S~ = 0 outside the
  *                         SSP coverage (sum_k F[k] dlambda_obs telescopes to the
  *                         total flux exactly).  rubix_cube_adjoint differentiates whichever rule
- *                         the telescope selects. */
+ *                         the telescope selects.  On a log-sampled SSP grid, on listed channel
+ *                         wavelengths and on listed SSP wavelengths the bin [e_k, e_{k+1}] of observed
+ *                         wavelength is averaged IN THE SAMPLING COORDINATE x of the SSP grid,
+ *                         F[k] = (1/(x_hi - x_lo)) * integral of S~(x) dx  (reading R20: identical
+ *                         to the above on a linearly sampled grid; per unit log lambda on a log-sampled one). */
 #define RUBIX_RESAMPLE_POINT 0
 #define RUBIX_RESAMPLE_FLUX 1
 

@@ -25,7 +25,7 @@ EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf"
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 3          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 4          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -45,7 +45,7 @@ class CSSP(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_age", C.c_int32), ("n_z", C.c_int32), ("n_lambda", C.c_int32),
                 ("log_age_axis", C.c_void_p), ("log_z_axis", C.c_void_p),
                 ("lambda0", C.c_float), ("dlambda", C.c_float), ("flux", C.c_void_p),
-                ("log_lambda", C.c_int32)]
+                ("log_lambda", C.c_int32), ("lambda_grid", C.c_void_p)]
 
 
 class CTelescope(C.Structure):
@@ -182,8 +182,11 @@ def c_ssp(ssp, flux) -> _Keep:
     rubix_forward_host)."""
     age, zed = _host_f32(ssp.log_age_axis), _host_f32(ssp.log_z_axis)
     n_age, n_z, n_lambda = (int(v) for v in flux.shape)
+    grid = getattr(ssp, "lambda_grid", None)
+    grid = None if grid is None else _host_f32(grid)
     return _Keep(CSSP(C.sizeof(CSSP), n_age, n_z, n_lambda, age.ctypes.data, zed.ctypes.data, float(ssp.lambda0),
-                      float(ssp.dlambda), _ptr(flux), int(getattr(ssp, "log_lambda", 0))), age, zed, flux)
+                      float(ssp.dlambda), _ptr(flux), int(getattr(ssp, "log_lambda", 0)),
+                      None if grid is None else grid.ctypes.data), age, zed, flux, grid)
 
 
 def c_particles(pos, vel, mass, log_age, log_z) -> _Keep:

@@ -57,8 +57,15 @@ rubix_status check_ssp(const rubix_ssp *s, bool flux_required)
         return fail(RUBIX_ERR_NULL, "ssp axis / flux pointer is NULL");
     if (s->n_age < 2 || s->n_z < 2 || s->n_lambda < 2)
         return fail(RUBIX_ERR_INVALID_ARG, "ssp grid needs n_age, n_z, n_lambda >= 2");
-    if (!(s->dlambda > 0.0f) || !isfinite(s->dlambda) || !isfinite(s->lambda0))
+    if (s->lambda_grid) {                                  // listed rest wavelengths replace lambda0 / dlambda
+        if (s->log_lambda != 0)
+            return fail(RUBIX_ERR_INVALID_ARG, "ssp lambda_grid (listed wavelengths) and log_lambda = 1 exclude each other");
+        for (int j = 0; j < s->n_lambda; ++j)
+            if (!(s->lambda_grid[j] > 0.0f) || !isfinite(s->lambda_grid[j]) || (j > 0 && !(s->lambda_grid[j] > s->lambda_grid[j - 1])))
+                return fail(RUBIX_ERR_INVALID_ARG, "ssp lambda_grid must be positive, finite and strictly increasing");
+    } else if (!(s->dlambda > 0.0f) || !isfinite(s->dlambda) || !isfinite(s->lambda0)) {
         return fail(RUBIX_ERR_INVALID_ARG, "ssp dlambda must be > 0 and finite");
+    }
     if (s->log_lambda != 0 && s->log_lambda != 1)
         return fail(RUBIX_ERR_INVALID_ARG, "ssp log_lambda must be 0 or 1");
     if (s->log_lambda == 1 && !(s->lambda0 > 0.0f))
@@ -107,8 +114,8 @@ rubix_status check_tel(const rubix_telescope *t)
             return fail(RUBIX_ERR_INVALID_ARG, "a wavelength-dependent PSF needs positive channel wavelengths");
     }
     if (t->lambda_obs) {
-        if (t->resample != RUBIX_RESAMPLE_POINT)
-            return fail(RUBIX_ERR_UNSUPPORTED, "explicit channel wavelengths support RUBIX_RESAMPLE_POINT only");
+        if (t->resample == RUBIX_RESAMPLE_FLUX && t->n_channels < 2)
+            return fail(RUBIX_ERR_INVALID_ARG, "the bin average on listed channel wavelengths needs n_channels >= 2");
         for (int k = 0; k < t->n_channels; ++k)
             if (!(t->lambda_obs[k] > 0.0f) || !isfinite(t->lambda_obs[k]) || (k > 0 && !(t->lambda_obs[k] > t->lambda_obs[k - 1])))
                 return fail(RUBIX_ERR_INVALID_ARG, "lambda_obs must be positive, finite and strictly increasing");
@@ -137,10 +144,17 @@ rubix_status check_particles(const rubix_particles *p)
 
 rubix_status check_resampler(const rubix_ssp *s, const rubix_telescope *t)
 {
+    if (gen_mode(s, t)) {                                  // readings R20 / R21: positions per sample in fp64
+        const bool fl = t->resample == RUBIX_RESAMPLE_FLUX;
+        const double first = t->lambda_obs ? (double)t->lambda_obs[0] - (fl ? 0.5 * ((double)t->lambda_obs[1] - (double)t->lambda_obs[0]) : 0.0)
+                                           : (double)t->lambda0 - (fl ? 0.5 * (double)t->dlambda : 0.0);
+        if (!(first > 0.0)) return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths (bin edges included) must be > 0");
+        const double b0 = gen_step_max(s, t);
+        if (!(b0 < 14.25))
+            return fail(RUBIX_ERR_UNSUPPORTED, "one channel spans %.3f SSP samples: outside the resampler range (< 14.25)", b0);
+        return RUBIX_OK;
+    }
     if (table_mode(s, t)) {
-        if (t->resample != RUBIX_RESAMPLE_POINT)
-            return fail(RUBIX_ERR_UNSUPPORTED,
-                        "log-sampled ssp grids and explicit channel wavelengths support RUBIX_RESAMPLE_POINT only");
         if (!t->lambda_obs && !((double)t->lambda0 > 0.0))
             return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths must be > 0 for a log-sampled ssp grid");
         const double b0 = table_step_max(s, t);

@@ -73,7 +73,8 @@ struct Layout {
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,
-        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps, off_aux, off_occ[2];
+        off_partials, off_cube_a, off_cube_b, off_flux, off_xtab, off_lamobs, off_psftaps, off_aux, off_occ[2],
+        off_gtab, off_gknots, off_ginvw, off_glut, off_glam;   // general-grid mode (gen_coord.cuh)
     int32_t n_rows, n_lambda, pitch;  // workspace copy of the SSP grid: n_rows = N_a*N_z rows of
                                       // `pitch` floats (zero padded), then kFluxPad zeros
     size_t bytes_total;           // two cube-sized buffers (convolve temp, adjoint G') + pass scratch
@@ -123,7 +124,25 @@ cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t
 
 // Table mode (readings R15 / R16): the rest position of channel k is x_k = Y[k] c + a with a per-launch
 // table Y and per-particle (c, a); used for log-sampled SSP grids and for explicit channel wavelengths.
-inline bool table_mode(const rubix_ssp *s, const rubix_telescope *t) { return s->log_lambda != 0 || t->lambda_obs != nullptr; }
+// General-grid mode (readings R20 / R21, gen_coord.cuh): listed SSP wavelengths, or the bin average on a log-sampled grid
+// or on listed channel wavelengths; positions per sample in fp64.  It takes precedence over the table mode.
+inline bool gen_mode(const rubix_ssp *s, const rubix_telescope *t)
+{
+    return s->lambda_grid != nullptr ||
+           (t->resample == RUBIX_RESAMPLE_FLUX && (s->log_lambda != 0 || t->lambda_obs != nullptr));
+}
+inline bool table_mode(const rubix_ssp *s, const rubix_telescope *t)
+{
+    return !gen_mode(s, t) && (s->log_lambda != 0 || t->lambda_obs != nullptr);
+}
+struct GenGrid;
+int gen_kind(const rubix_ssp *s);
+// largest span of one channel (point rule: channel to channel; bin average: one bin) in SSP samples, Doppler cap included
+double gen_step_max(const rubix_ssp *s, const rubix_telescope *t);
+void gen_grid_params(const PassInputs &in, const Layout &L, char *ws, GenGrid *G);          // host only
+cudaError_t launch_adjoint_general(const PassInputs &in, const Layout &L, char *ws, const float *gconv, float *g_mass,
+                                   float *g_age, float *g_z, float *g_v, cudaStream_t st);
+cudaError_t launch_gen_setup(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st, GenGrid *G);   // + tables
 // largest d x / d channel over the detector, including the largest Doppler stretch (host, fp64)
 double table_step_max(const rubix_ssp *s, const rubix_telescope *t);
 

@@ -7,6 +7,7 @@
 //       k_build_units       unit descriptors
 //   K2c k_prepare_records   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
 #include "common.cuh"
+#include "gen_coord.cuh"
 
 namespace rubix {
 
@@ -363,6 +364,8 @@ struct PrepParams {
     int32_t log_grid, table;            // table mode (R15 / R16): x_k = xtab[k] c + a
     const int64_t *xtab;
     int64_t n_phys;                     // > 0: batched call on a shared galaxy, physical particle = perm value % n_phys
+    int32_t gen_on;                     // general-grid mode (gen_coord.cuh): positions per sample in fp64
+    GenGrid gen;
 };
 
 __device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *cell, double *t)
@@ -461,6 +464,42 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
         if (k_lo > P.n_c) k_lo = P.n_c;
         x_first = a_fx + b * k_lo;
         x_last = a_fx + b * k_hi;
+    }
+    if (P.gen_on) {
+        // general-grid mode: x = gen_coord(tab[e], g) in fp64; the record carries g; the covered channels / bins are
+        // found by bisection on the (increasing) table, the window gets a 1e-6-sample margin on either side
+        const double g = gen_doppler(P.gen, 1.0 + (double)vlos[pl] / kCkms);
+        const double x_top = (double)(P.n_lambda - 1);
+        auto xe = [&](int e) { return gen_coord(P.gen, P.gen.tab[e], g); };
+        const int fl = P.gen.flux;
+        int lo = 0, hi = P.n_c;                            // point: first k with x_k >= 0; bins: first k with x_{k+1} > 0
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const bool ok = fl ? xe(mid + 1) > 0.0 : xe(mid) >= 0.0;
+            if (ok) hi = mid; else lo = mid + 1;
+        }
+        k_lo = lo;
+        lo = -1; hi = P.n_c - 1;                           // point: last k with x_k <= top; bins: last k with x_k < top
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            const bool ok = fl ? xe(mid) < x_top : xe(mid) <= x_top;
+            if (ok) lo = mid; else hi = mid - 1;
+        }
+        k_hi = lo;
+        r.a_fx = __double_as_longlong(g);
+        r.b_fx = 0;
+        r.k_lo = (int32_t)k_lo;
+        r.k_hi = (int32_t)k_hi;
+        r.j0 = 0;
+        r.nw = 0;
+        if (k_lo <= k_hi) {
+            const double xa = fmin(fmax(xe((int)k_lo) - 1e-6, 0.0), x_top);
+            const double xb = fmin(fmax(xe((int)k_hi + fl) + 1e-6, 0.0), x_top);
+            r.j0 = (int32_t)xa & ~(kRowAlign - 1);
+            r.nw = (int32_t)xb - r.j0 + 2;
+        }
+        rec[i] = r;
+        return;
     }
     r.a_fx = a_fx;
     r.b_fx = P.table ? c_fx : b_fx;            // table mode: the Doppler factor c (2.30) takes B's slot
@@ -595,6 +634,12 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_lamobs = take(((size_t)n_c + 1) * 4);         // device copy of rubix_telescope.lambda_obs
     L.off_psftaps = take(psf_taps_bytes(n_c));          // per-channel PSF taps (reading R18)
     for (int b = 0; b < 2; ++b) L.off_occ[b] = take((size_t)n_s + 64);   // occupancy of the raw cube / of the PSF temporary
+    // general-grid mode (gen_coord.cuh): table over channel centres / bin edges, knots, inverse widths, look-up table
+    L.off_gtab = take(((size_t)n_c + 2) * 8);
+    L.off_gknots = take(((size_t)n_lambda + 1) * 8);
+    L.off_ginvw = take(((size_t)n_lambda + 1) * 8);
+    L.off_glut = take(((size_t)kGenLutPerKnot * n_lambda + 8) * 4);
+    L.off_glam = take(((size_t)n_lambda + 1) * 4);
     L.bytes_total = off;
     return L;
 }
@@ -697,6 +742,11 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.mode = in.tel->resample;
         P.log_grid = in.ssp->log_lambda;
         P.table = table_mode(in.ssp, in.tel) ? 1 : 0;
+        P.gen_on = gen_mode(in.ssp, in.tel) ? 1 : 0;
+        if (P.gen_on) {
+            cudaError_t eg = launch_gen_setup(in, L, ws, st, &P.gen);
+            if (eg != cudaSuccess) return eg;
+        }
         P.n_phys = (in.batch > 1 && !in.offsets) ? in.p->n : 0;
         P.xtab = (const int64_t *)(ws + L.off_xtab);
         if (P.table) {

@@ -23,6 +23,7 @@
 // Single-chunk spaxels write their cube row directly (each voxel exactly once, coalesced);
 // spaxels with more particles write partial rows that k_reduce_partials sums in fixed order.
 #include "common.cuh"
+#include "gen_coord.cuh"
 
 namespace rubix {
 
@@ -37,6 +38,7 @@ struct AccumParams {
     int32_t skip_empty;      // 1: empty spaxels are left unwritten (the masked PSF/LSF passes never read them)
     const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
     cudaTextureObject_t tex;
+    GenGrid gen;             // GEN: general-grid mode (gen_coord.cuh)
 };
 
 constexpr int kPass = 128;                           // table samples produced per warp per pass
@@ -93,6 +95,7 @@ struct Win {                 // one particle's window in one channel tile
     int32_t first, nw;       // flux index of (corner (i,j), sample j0); samples needed
     int32_t j0;              // first table sample (multiple of 32)
     float w0, w1, w2, w3;
+    double g;                // GEN: the particle's Doppler value (gen_coord.cuh)
 };
 
 struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
@@ -104,7 +107,9 @@ struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 // LOGX: table mode (readings R15 / R16: log-sampled SSP grid, explicit channel wavelengths):
 // x_k = Y[k] c + a with the per-launch table Y = xtab and the particle's (c, a); c (2.30 fixed point) travels in
 // the record's b slot.  The thread keeps Y of its CPT channels relative to the tile start in registers (12.20).
-template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX>
+// GEN: general-grid mode (readings R20 / R21, gen_coord.cuh): x = gen_coord(tab[e], g) per sample in fp64, e = channel
+// (point rule) or bin edge (FLUX: channel k is the bin between edges k and k + 1, averaged over its FULL width in x).
+template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX, bool GEN = false>
 __global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
@@ -151,10 +156,22 @@ k_accumulate(const __grid_constant__ AccumParams P)
             W.w2 = __int_as_float(ra.z); W.w3 = __int_as_float(ra.w);
             W.b = (uint32_t)rb.y;
             const int64_t a = (int64_t)(((uint64_t)(uint32_t)rb.w << 32) | (uint32_t)rb.z);
+            W.g = GEN ? __longlong_as_double(a) : 0.0;
             int j0;
             if (SINGLE) {                                   // k0 = 0, k_end = n_c - 1 >= k_hi
                 W.ka = rc.x; W.kb = rc.y;
                 j0 = rc.z; W.nw = rc.w;
+            } else if (GEN) {
+                W.ka = max(k0, rc.x);
+                W.kb = min(k_end, rc.y);
+                j0 = 0; W.nw = 0;
+                if (W.ka <= W.kb) {                         // as k_prepare_records, for this tile's channels
+                    const double x_top = (double)(P.n_lambda - 1);
+                    const double xa = fmin(fmax(gen_coord(P.gen, P.gen.tab[W.ka], W.g) - 1e-6, 0.0), x_top);
+                    const double xb = fmin(fmax(gen_coord(P.gen, P.gen.tab[W.kb + (FLUX ? 1 : 0)], W.g) + 1e-6, 0.0), x_top);
+                    j0 = (int)xa & ~(kRowAlign - 1);
+                    W.nw = (int)xb - j0 + 2;
+                }
             } else {
                 W.ka = max(k0, rc.x);
                 W.kb = min(k_end, rc.y);
@@ -178,7 +195,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
             W.first = rb.x + j0;
             W.j0 = j0;
-            W.base = a + (LOGX ? __double2ll_rn((double)x_tile0 * ((double)W.b * (1.0 / (double)(1u << 30))))
+            W.base = GEN ? 0 : a + (LOGX ? __double2ll_rn((double)x_tile0 * ((double)W.b * (1.0 / (double)(1u << 30))))
                                : (int64_t)W.b * k0) - ((int64_t)j0 << kFxFrac);
             return W;
         };
@@ -255,8 +272,44 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
             acc[i] = fmaf(tot, inv_b, acc[i]);
         };
+        // GEN: integral of the table's interpolant over [a, b] (sample coordinates relative to the table start, a < b)
+        auto gen_integral = [&](const float *tabp, double a, double b) -> float {
+            const int ja = (int)a, jb = (int)b;
+            const float fa = (float)(a - (double)ja), fb = (float)(b - (double)jb);
+            const float a0 = tabp[ja], a1 = tabp[ja + 1];
+            if (ja == jb) return (fb - fa) * fmaf(0.5f * (fa + fb), a1 - a0, a0);
+            const float c0 = tabp[jb], c1 = tabp[jb + 1];
+            float tot = 0.5f * (1.0f - fa) * (fmaf(fa, a1 - a0, a0) + a1);
+            tot = fmaf(0.5f * fb, c0 + fmaf(fb, c1 - c0, c0), tot);
+            for (int j = ja + 1; j < jb; ++j) tot = fmaf(0.5f, tabp[j] + tabp[j + 1], tot);
+            return tot;
+        };
         auto resample = [&](const Win &W, const float *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
+            if (GEN) {
+                const double x_top = (double)(P.n_lambda - 1), j0d = (double)W.j0;
+#pragma unroll 1
+                for (int i = 0; i < CPT; ++i) {
+                    const int k = k0 + tid + i * kAccThreads;
+                    if (k < W.ka || k > W.kb) continue;
+                    if (!FLUX) {
+                        const double x = gen_coord(P.gen, __ldg(P.gen.tab + k), W.g);
+                        if (x >= 0.0 && x <= x_top) {
+                            const double xl = x - j0d;
+                            const int j = (int)xl;
+                            const float f = (float)(xl - (double)j);
+                            const float s0 = buf[j], s1 = buf[j + 1];
+                            acc[i] += fmaf(f, s1 - s0, s0);
+                        }
+                    } else {
+                        const double xlo = gen_coord(P.gen, __ldg(P.gen.tab + k), W.g);
+                        const double xhi = gen_coord(P.gen, __ldg(P.gen.tab + k + 1), W.g);
+                        const double cl = fmax(xlo, 0.0), ch = fmin(xhi, x_top);
+                        if (ch > cl) acc[i] = fmaf(gen_integral(buf, cl - j0d, ch - j0d), (float)(1.0 / (xhi - xlo)), acc[i]);
+                    }
+                }
+                return;
+            }
             if (FLUX) {
                 const float inv_b = (float)(1 << kFxFrac) / (float)W.b;
                 // coverage in local coordinates; W.base = x(k0) - (j0 << 28)
@@ -397,10 +450,10 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
-template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false>
+template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false, bool GEN = false>
 static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, LOGX ? 3 : kAccMinBlocks, FLUX, LOGX>;
+    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, (LOGX || GEN) ? 3 : kAccMinBlocks, FLUX, LOGX, GEN>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kAccThreads, smem, st>>>(P);
@@ -409,8 +462,15 @@ static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem,
 }
 
 template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsigned grid, size_t smem, cudaStream_t st)
+static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, bool gen, unsigned grid, size_t smem, cudaStream_t st)
 {
+    if (gen) {
+        if (P.n_tiles == 1)
+            return flux ? launch_acc2<CPT, true, true, false, true>(P, grid, smem, st)
+                        : launch_acc2<CPT, true, false, false, true>(P, grid, smem, st);
+        return flux ? launch_acc2<CPT, false, true, false, true>(P, grid, smem, st)
+                    : launch_acc2<CPT, false, false, false, true>(P, grid, smem, st);
+    }
     if (logx)
         return P.n_tiles == 1 ? launch_acc2<CPT, true, false, true>(P, grid, smem, st)
                               : launch_acc2<CPT, false, false, true>(P, grid, smem, st);
@@ -444,10 +504,10 @@ int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
                               cudaStream_t st)
 {
-    const bool logx = table_mode(in.ssp, in.tel);
+    const bool logx = table_mode(in.ssp, in.tel), gen = gen_mode(in.ssp, in.tel);
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
-    // table mode: the steepest d x / d k of the detector, largest Doppler stretch included
-    const double b_max = logx ? table_step_max(in.ssp, in.tel) : b0 / (1.0 - kBetaCap);
+    // table / general-grid mode: the steepest d x / d k of the detector, largest Doppler stretch included
+    const double b_max = gen ? gen_step_max(in.ssp, in.tel) : (logx ? table_step_max(in.ssp, in.tel) : b0 / (1.0 - kBetaCap));
     int wcap = 0;
     const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
     const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap);
@@ -469,6 +529,8 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     P.skip_empty = skip_empty ? 1 : 0;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.tex = 0;
+    P.gen = GenGrid{};
+    if (gen) gen_grid_params(in, L, ws, &P.gen);            // the tables the particle pass wrote
 #if RUBIX_TEX_CORNERS > 0
     {
         static thread_local const void *cached_ptr = nullptr;
@@ -495,12 +557,12 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     {
         StageTimer t(1, st);
         switch (cpt) {
-            case 29: e = launch_acc<29>(P, flux, logx, grid, smem, st); break;
-            case 15: e = launch_acc<15>(P, flux, logx, grid, smem, st); break;
-            case 8: e = launch_acc<8>(P, flux, logx, grid, smem, st); break;
-            case 4: e = launch_acc<4>(P, flux, logx, grid, smem, st); break;
-            case 2: e = launch_acc<2>(P, flux, logx, grid, smem, st); break;
-            default: e = launch_acc<1>(P, flux, logx, grid, smem, st); break;
+            case 29: e = launch_acc<29>(P, flux, logx, gen, grid, smem, st); break;
+            case 15: e = launch_acc<15>(P, flux, logx, gen, grid, smem, st); break;
+            case 8: e = launch_acc<8>(P, flux, logx, gen, grid, smem, st); break;
+            case 4: e = launch_acc<4>(P, flux, logx, gen, grid, smem, st); break;
+            case 2: e = launch_acc<2>(P, flux, logx, gen, grid, smem, st); break;
+            default: e = launch_acc<1>(P, flux, logx, gen, grid, smem, st); break;
         }
     }
     if (e != cudaSuccess) return e;

@@ -37,7 +37,8 @@ def assert_gradients(g, ref, key, vlos, ssp, tel, what="", tol=1e-3, floor=1e-3)
         rel = (np.abs(got - want) / scale)[inside]
         excluded = np.zeros(rel.shape, bool)
         if q == 3 and int(getattr(tel, "resample", 0)) == 0:
-            table = int(getattr(ssp, "log_lambda", 0)) or getattr(tel, "lambda_obs", None) is not None
+            listed = getattr(ssp, "lambda_grid", None) is not None       # general-grid mode: fp64 positions
+            table = (int(getattr(ssp, "log_lambda", 0)) or getattr(tel, "lambda_obs", None) is not None) and not listed
             clr = oracle.knot_clearance(vlos[inside], ssp, tel)
             excluded = clr < (X_TOL_TABLE if table else X_TOL_UNIFORM)
             assert excluded.mean() < 5e-3, (what, "too many particles within the position resolution of a knot",

@@ -103,13 +103,16 @@ def test_adjoint(B, log_grid):
     assert_gradients(g, ana, key, vlos, w.ssp, t, "test_gpu_obsgrid.py")
 
 
-def test_bad_arrays_and_the_flux_rule_are_refused(B):
+def test_bad_arrays_are_refused(B):
     w = synth.make_workload("tiny")
     lam = w.telescope.wavelengths().astype(np.float32)
     bad = lam.copy()
     bad[10] = bad[9]
-    for arr, rs, msg in ((bad, 0, "increasing"), (lam, 1, "RUBIX_RESAMPLE_POINT")):
-        w2 = dataclasses.replace(w, telescope=dataclasses.replace(w.telescope, lambda_obs=arr, resample=rs))
-        with pytest.raises(B.RubixError):
-            B.DeviceWorkload(w2).build_cube()
-        assert msg in B.rubix_last_error()
+    w2 = dataclasses.replace(w, telescope=dataclasses.replace(w.telescope, lambda_obs=bad))
+    with pytest.raises(B.RubixError):
+        B.DeviceWorkload(w2).build_cube()
+    assert "increasing" in B.rubix_last_error()
+    one = dataclasses.replace(w, telescope=dataclasses.replace(w.telescope, n_channels=1, lambda_obs=lam[:1], resample=1))
+    with pytest.raises(B.RubixError):                           # a bin needs a neighbour to define its edges (R20)
+        B.DeviceWorkload(one).build_cube()
+    assert "n_channels >= 2" in B.rubix_last_error()
