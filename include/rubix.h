@@ -112,11 +112,16 @@ typedef struct {
                                     /* for seeing); 0 = the same PSF for every channel.  Needs    */
                                     /* psf_size <= 15, lsf_size <= 9 and an even n_channels.      */
                                     /* The PSF then acts AFTER the LSF (they no longer commute).  */
+    int32_t n_x_full, x_first;      /* Row window for spaxel-sharded runs:  */
+                                    /* n_x_full > 0: the detector has n_x_full rows along x, binning  */
+                                    /* uses THAT geometry (bit-equal keys), and this call owns the    */
+                                    /* n_x rows x_first .. x_first + n_x - 1 (key = (ix - x_first)    */
+                                    /* n_y + iy; particles in other rows are dropped).  0 = off.      */
 } rubix_telescope;
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 4
+#define RUBIX_ABI_VERSION 5
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -163,6 +168,13 @@ rubix_status rubix_build_cube(const rubix_particles *particles, const rubix_ssp 
 rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cube_in,
                                     float *cube_out, void *workspace, size_t workspace_bytes,
                                     void *stream);
+
+/* Steps 1-2 alone: the spaxel key and the line-of-sight velocity of every particle, in the
+ * caller's order, with the fp32 fixed-order arithmetic of rubix_build_cube (bit-equal keys).  Used by the spaxel-sharded
+ * multi-GPU path (paper_2412_08265_b200/sharded.py) to route particles to the rank that owns their detector row.
+ *   pos, vel  DEVICE [n][3];  key DEVICE [n] int32 (n_x*n_y = dropped);  vlos DEVICE [n] fp32 or NULL */
+rubix_status rubix_bin_particles(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
+                                 int32_t *key, float *vlos, void *stream);
 
 /* Steps 1-8 in one call on DEVICE buffers (the whole forward model: rubix_build_cube followed by
  * rubix_convolve_psf_lsf, same arithmetic, same results bit for bit).  The raw cube of step 6 lives in the workspace; with

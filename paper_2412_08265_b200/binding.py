@@ -19,13 +19,13 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf", "rubix_forward",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
-           "rubix_forward_batched_workspace_bytes", "rubix_forward_batched",
+           "rubix_forward_batched_workspace_bytes", "rubix_forward_batched", "rubix_bin_particles",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 4          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 5          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -54,7 +54,7 @@ class CTelescope(C.Structure):
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
                 ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
                 ("redshift", C.c_float), ("flux_scale", C.c_float), ("lambda_obs", C.c_void_p),
-                ("psf_alpha", C.c_float), ("psf_lambda_ref", C.c_float)]
+                ("psf_alpha", C.c_float), ("psf_lambda_ref", C.c_float), ("n_x_full", C.c_int32), ("x_first", C.c_int32)]
 
 
 _lib = None
@@ -84,6 +84,9 @@ def load():
         lib.rubix_forward_batched.argtypes = [C.POINTER(CParticles), C.c_void_p, C.c_int32, C.POINTER(CSSP),
                                               C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                               C.c_void_p]
+        lib.rubix_bin_particles.restype = C.c_int
+        lib.rubix_bin_particles.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(CTelescope), C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p]
         lib.rubix_convolve_psf_lsf.restype = C.c_int
         lib.rubix_convolve_psf_lsf.argtypes = [C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p,
                                                C.c_size_t, C.c_void_p]
@@ -173,7 +176,8 @@ def c_telescope(tel) -> _Keep:
                             int(getattr(tel, "resample", 0)), float(getattr(tel, "redshift", 0.0)),
                             float(getattr(tel, "flux_scale", 1.0)),
                             None if lam is None else lam.ctypes.data, float(getattr(tel, "psf_alpha", 0.0)),
-                            float(getattr(tel, "psf_lambda_ref", 1.0))), lam)
+                            float(getattr(tel, "psf_lambda_ref", 1.0)), int(getattr(tel, "n_x_full", 0)),
+                            int(getattr(tel, "x_first", 0))), lam)
 
 
 def c_ssp(ssp, flux) -> _Keep:
@@ -221,6 +225,12 @@ def rubix_forward(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, 
     _check(load().rubix_forward(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
                                 _ptr(workspace), int(workspace.numel() * workspace.element_size()),
                                 _stream(stream)))
+
+
+def rubix_bin_particles(pos, vel, tel: _Keep, R, key, vlos=None, stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_bin_particles(int(pos.shape[0]), _ptr(pos), _ptr(vel), tel.ref(), R.ctypes.data, _ptr(key), _ptr(vlos),
+                                      _stream(stream)))
 
 
 def _offsets(offsets):

@@ -96,6 +96,10 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_UNSUPPORTED, "detector too large");
     if (!(t->spaxel_size > 0.0f) || !isfinite(t->spaxel_size))
         return fail(RUBIX_ERR_INVALID_ARG, "spaxel_size must be > 0");
+    if (t->n_x_full < 0 || (t->n_x_full > 0 && (t->x_first < 0 || (int64_t)t->x_first + t->n_x > t->n_x_full)))
+        return fail(RUBIX_ERR_INVALID_ARG, "row window: need 0 <= x_first and x_first + n_x <= n_x_full");
+    if (t->n_x_full == 0 && t->x_first != 0)
+        return fail(RUBIX_ERR_INVALID_ARG, "x_first needs n_x_full > 0");
     if (!(t->dlambda > 0.0f) || !isfinite(t->dlambda) || !isfinite(t->lambda0))
         return fail(RUBIX_ERR_INVALID_ARG, "telescope dlambda must be > 0 and finite");
     if (t->resample != RUBIX_RESAMPLE_POINT && t->resample != RUBIX_RESAMPLE_FLUX)
@@ -244,6 +248,21 @@ rubix_status rubix_build_cube(const rubix_particles *p, const rubix_ssp *ssp, co
     e = launch_accumulate(in, L, (char *)workspace, cube, false, st);
     if (e != cudaSuccess) return cuda_fail(e, "accumulate");
     remember(workspace, L);
+    return RUBIX_OK;
+}
+
+rubix_status rubix_bin_particles(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
+                                 int32_t *key, float *vlos, void *stream)
+{
+    t_err[0] = 0;
+    Range nvtx_range("rubix_bin_particles");
+    g_launches = 0;
+    rubix_status s;
+    if (n < 0 || n >= 2147483647LL) return fail(RUBIX_ERR_INVALID_ARG, "n out of range");
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || (n > 0 && (!pos || !vel || !key))) return fail(RUBIX_ERR_NULL, "R, pos, vel or key is NULL");
+    cudaError_t e = launch_bin_only(n, pos, vel, tel, R, key, vlos, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "bin");
     return RUBIX_OK;
 }
 
@@ -413,10 +432,12 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
     float *tmp = nullptr, *taps = nullptr;
     if (tel->psf_size > 0) {
         const bool var = tel->psf_alpha != 0.0f;
-        const size_t need = align_up(cube_bytes, 256) + (var ? psf_taps_bytes(tel->n_channels) : 0);
+        // first cube buffer = the temporary; the per-channel taps live behind BOTH cube buffers (make_layout), so a
+        // workspace shared with rubix_build_cube keeps its sort artefacts
+        const size_t need = var ? 2 * align_up(cube_bytes, 256) + psf_taps_bytes(tel->n_channels) : align_up(cube_bytes, 256);
         if ((s = check_ws(workspace, workspace_bytes, need)) != RUBIX_OK) return s;
         tmp = (float *)workspace;
-        if (var) taps = (float *)((char *)workspace + align_up(cube_bytes, 256));   // start of the second cube buffer
+        if (var) taps = (float *)((char *)workspace + 2 * align_up(cube_bytes, 256));
     }
     cudaError_t e;
     {

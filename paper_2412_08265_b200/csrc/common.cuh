@@ -100,6 +100,8 @@ struct PassInputs {
 };
 
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
+cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
+                            int32_t *key, float *vlos, cudaStream_t st);
 // skip_empty: rows of spaxels without particles are NOT written (the masked PSF/LSF passes never read them)
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
                               cudaStream_t st);

@@ -238,7 +238,10 @@ k_adjoint_general(const __grid_constant__ AdjGenParams P)
         const uint32_t ju = (uint32_t)j;
         auto mix = [&](uint32_t q) -> double {
             const float t0 = __ldg(T0 + q), t1 = __ldg(T1 + q), t2 = __ldg(T2 + q), t3 = __ldg(T3 + q);
-            return (double)t0 + ta * (double)(t1 - t0) + tz * (double)(t2 - t0) + ta * tz * (double)((t3 - t2) - (t1 - t0));
+            // promoted BEFORE subtracting: corners may differ by far more than a factor of two, where an fp32 difference
+            // rounds at the level of the larger sample -- and the derivative below is a difference of such blends
+            const double d0 = t0, d1 = t1, d2 = t2, d3 = t3;
+            return d0 + ta * (d1 - d0) + tz * (d2 - d0) + ta * tz * ((d3 - d2) - (d1 - d0));
         };
         const double a = mix(ju), b = mix(ju + 1);
         return a + f * (b - a);
@@ -278,11 +281,11 @@ k_adjoint_general(const __grid_constant__ AdjGenParams P)
             for (int j = jl; j <= ju_; ++j) {
                 const double w = gen_hat_integral(ch - (double)j) - gen_hat_integral(cl - (double)j);
                 const uint32_t j32 = (uint32_t)j;
-                const float t0 = __ldg(T0 + j32), t1 = __ldg(T1 + j32), t2 = __ldg(T2 + j32), t3 = __ldg(T3 + j32);
-                v0 += w * (double)t0;
-                da += w * (double)(t1 - t0);
-                dz += w * (double)(t2 - t0);
-                dq += w * (double)((t3 - t2) - (t1 - t0));
+                const double t0 = __ldg(T0 + j32), t1 = __ldg(T1 + j32), t2 = __ldg(T2 + j32), t3 = __ldg(T3 + j32);
+                v0 += w * t0;
+                da += w * (t1 - t0);
+                dz += w * (t2 - t0);
+                dq += w * ((t3 - t2) - (t1 - t0));
             }
             const double gw = (double)gk * inv_w;
             P0 += gw * v0; Pa += gw * da; Pz += gw * dz; Pq += gw * dq;

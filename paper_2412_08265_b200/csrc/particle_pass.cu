@@ -18,10 +18,20 @@ namespace rubix {
 // --------------------------------------------------------------------------------------------
 struct BinParams {
     float R[9];
-    int32_t n_x, n_y;
+    int32_t n_x, n_y;                      // rows owned by this call
+    int32_t n_x_full, x_first;             // geometry of the whole detector along x and the first owned row (row window)
     float s;
     int64_t n;
 };
+
+// key of (u, v) = detector coordinates in spaxels, or the sentinel n_x * n_y
+__device__ __forceinline__ int32_t bin_key(const BinParams &P, float u, float v, float vl)
+{
+    const bool inside = (u >= 0.0f) && (u < (float)P.n_x_full) && (v >= 0.0f) && (v < (float)P.n_y) &&
+                        (fabsf(vl) <= kVcapKms);
+    const int32_t ix = (int32_t)floorf(u) - P.x_first;
+    return (inside && ix >= 0 && ix < P.n_x) ? ix * P.n_y + (int32_t)floorf(v) : P.n_x * P.n_y;
+}
 
 __global__ void __launch_bounds__(256)
 k_rotate_bin(const float *__restrict__ pos, const float *__restrict__ vel, BinParams P,
@@ -34,14 +44,12 @@ k_rotate_bin(const float *__restrict__ pos, const float *__restrict__ vel, BinPa
     const float xr = __fadd_rn(__fadd_rn(__fmul_rn(P.R[0], x), __fmul_rn(P.R[1], y)), __fmul_rn(P.R[2], z));
     const float yr = __fadd_rn(__fadd_rn(__fmul_rn(P.R[3], x), __fmul_rn(P.R[4], y)), __fmul_rn(P.R[5], z));
     const float vl = __fadd_rn(__fadd_rn(__fmul_rn(P.R[6], vx), __fmul_rn(P.R[7], vy)), __fmul_rn(P.R[8], vz));
-    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x), P.s);
+    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x_full), P.s);
     const float hy = __fmul_rn(__fmul_rn(0.5f, (float)P.n_y), P.s);
     const float u = __fdiv_rn(__fadd_rn(xr, hx), P.s);
     const float v = __fdiv_rn(__fadd_rn(yr, hy), P.s);
-    const bool inside = (u >= 0.0f) && (u < (float)P.n_x) && (v >= 0.0f) && (v < (float)P.n_y) &&
-                        (fabsf(vl) <= kVcapKms);
-    key[i] = inside ? (int32_t)floorf(u) * P.n_y + (int32_t)floorf(v) : P.n_x * P.n_y;
-    vlos[i] = vl;
+    key[i] = bin_key(P, u, v, vl);
+    if (vlos) vlos[i] = vl;
 }
 
 // Batched variant: logical particle i belongs to batch element b (its own rotation) and gets the
@@ -78,14 +86,13 @@ k_rotate_bin_batched(const float *__restrict__ pos, const float *__restrict__ ve
     const float xr = __fadd_rn(__fadd_rn(__fmul_rn(R[0], x), __fmul_rn(R[1], y)), __fmul_rn(R[2], z));
     const float yr = __fadd_rn(__fadd_rn(__fmul_rn(R[3], x), __fmul_rn(R[4], y)), __fmul_rn(R[5], z));
     const float vl = __fadd_rn(__fadd_rn(__fmul_rn(R[6], vx), __fmul_rn(R[7], vy)), __fmul_rn(R[8], vz));
-    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x), P.s);
+    const float hx = __fmul_rn(__fmul_rn(0.5f, (float)P.n_x_full), P.s);
     const float hy = __fmul_rn(__fmul_rn(0.5f, (float)P.n_y), P.s);
     const float u = __fdiv_rn(__fadd_rn(xr, hx), P.s);
     const float v = __fdiv_rn(__fadd_rn(yr, hy), P.s);
-    const bool inside = (u >= 0.0f) && (u < (float)P.n_x) && (v >= 0.0f) && (v < (float)P.n_y) &&
-                        (fabsf(vl) <= kVcapKms);
     const int32_t n_s = P.n_x * P.n_y;
-    key[i] = inside ? b * n_s + (int32_t)floorf(u) * P.n_y + (int32_t)floorf(v) : Bt.batch * n_s;
+    const int32_t kk = bin_key(P, u, v, vl);
+    key[i] = kk < n_s ? b * n_s + kk : Bt.batch * n_s;
     vlos[i] = vl;
 }
 
@@ -535,6 +542,23 @@ k_positions(int32_t n_c, const float *__restrict__ lam, double l0_obs, double dl
     ytab[k] = __double2ll_rn(y * (double)(1 << kFxFrac));
 }
 
+cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
+                            int32_t *key, float *vlos, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    BinParams B;
+    for (int i = 0; i < 9; ++i) B.R[i] = R[i];
+    B.n_x = tel->n_x;
+    B.n_y = tel->n_y;
+    B.n_x_full = tel->n_x_full > 0 ? tel->n_x_full : tel->n_x;
+    B.x_first = tel->n_x_full > 0 ? tel->x_first : 0;
+    B.s = tel->spaxel_size;
+    B.n = n;
+    k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, vel, B, key, vlos);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
 double table_step_max(const rubix_ssp *s, const rubix_telescope *t)
 {
     const double zp1 = 1.0 + (double)t->redshift;
@@ -606,6 +630,9 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     const size_t cube = (size_t)n_s * (size_t)n_c * 4;
     L.off_cube_a = take(cube);
     L.off_cube_b = take(cube);
+    // per-channel PSF taps (reading R18) sit right behind the two cubes, at an offset that depends on the detector
+    // only: rubix_convolve_psf_lsf finds them without knowing n, and never touches the sort artefacts behind them
+    L.off_psftaps = take(psf_taps_bytes(n_c));
     L.off_key = take(nn * 4);
     L.off_vlos = take(nn * 4);
     L.off_seg = take(((size_t)n_s + 2) * 4);
@@ -632,7 +659,6 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     L.off_flux = take(((size_t)n_rows * L.pitch + kFluxPad) * 4);
     L.off_xtab = take(((size_t)n_c + 1) * 8);           // Y[k] of the table mode (readings R15 / R16)
     L.off_lamobs = take(((size_t)n_c + 1) * 4);         // device copy of rubix_telescope.lambda_obs
-    L.off_psftaps = take(psf_taps_bytes(n_c));          // per-channel PSF taps (reading R18)
     for (int b = 0; b < 2; ++b) L.off_occ[b] = take((size_t)n_s + 64);   // occupancy of the raw cube / of the PSF temporary
     // general-grid mode (gen_coord.cuh): table over channel centres / bin edges, knots, inverse widths, look-up table
     L.off_gtab = take(((size_t)n_c + 2) * 8);
@@ -674,6 +700,8 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         for (int i = 0; i < 9; ++i) B.R[i] = in.R[i];
         B.n_x = in.tel->n_x;
         B.n_y = in.tel->n_y;
+        B.n_x_full = in.tel->n_x_full > 0 ? in.tel->n_x_full : in.tel->n_x;
+        B.x_first = in.tel->n_x_full > 0 ? in.tel->x_first : 0;
         B.s = in.tel->spaxel_size;
         B.n = n;
         if (in.batch > 1 || in.offsets) {

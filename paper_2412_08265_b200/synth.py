@@ -207,6 +207,8 @@ class Telescope:
     lambda_obs: np.ndarray | None = None       # explicit, increasing channel wavelengths [n_channels] fp32 (else uniform)
     psf_alpha: np.float32 = np.float32(0.0)    # PSF width ~ (lambda / psf_lambda_ref)^psf_alpha; 0 = the same for every channel
     psf_lambda_ref: np.float32 = np.float32(1.0)
+    n_x_full: int = 0         # row window of a spaxel-sharded run: the whole detector has n_x_full rows and this
+    x_first: int = 0          # telescope owns rows x_first .. x_first + n_x - 1 (0 / 0 = the whole detector)
 
     @property
     def n_spaxels(self) -> int:

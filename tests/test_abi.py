@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 
 def test_struct_layouts_match_the_header():
-    assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 64 and C.sizeof(B.CTelescope) == 72
+    assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 64 and C.sizeof(B.CTelescope) == 80
 
 
 def test_abi_version_and_struct_size_are_checked(lib):

@@ -25,17 +25,19 @@ def B():
 
 def random_case(seed):
     rng = np.random.default_rng(seed)
-    log_grid = bool(rng.integers(0, 3) == 0)
+    kind = str(rng.choice(["lin", "lin", "log", "irr"]))           # SSP grid: linear, log-sampled (R15), listed knots (R21)
+    log_grid = kind == "log"
     n_l = int(rng.integers(40, 900))
     ssp = synth.make_ssp(int(rng.integers(2, 7)), int(rng.integers(2, 5)), n_l, 3500.0, 9500.0,
-                         int(rng.integers(1, 10 ** 6)), log_lambda=log_grid)
-    resample = 0 if log_grid else int(rng.integers(0, 2))
+                         int(rng.integers(1, 10 ** 6)), log_lambda=log_grid, irregular=kind == "irr")
+    resample = int(rng.integers(0, 2))                              # either rule on every grid (R13 / R20)
     n_c = int(rng.integers(1, 700))
     span = float(rng.uniform(500.0, 7000.0))
     l0 = float(rng.uniform(3000.0, 9000.0))
     dl = span / max(n_c, 2)
     step_ssp = 6000.0 / (n_l - 1)
-    dl = float(np.clip(dl, 0.05 * step_ssp, 8.0 * step_ssp))       # keep d x / d k inside the resampler range
+    # keep one channel's span inside the resampler range (listed knots are up to twice as dense as the average)
+    dl = float(np.clip(dl, 0.05 * step_ssp, (3.5 if kind == "irr" else 8.0) * step_ssp))
     z = float(rng.choice([0.0, 0.0, 0.07, 0.5]))
     psf = int(rng.choice([0, 0, 3, 7, 15, 21]))
     lsf = int(rng.choice([0, 0, 3, 9, 13]))
@@ -43,7 +45,7 @@ def random_case(seed):
                           np.float32(l0 * (1 + z)), np.float32(dl * (1 + z)), psf, np.float32(rng.uniform(0.6, 3.0)),
                           lsf, np.float32(rng.uniform(0.6, 3.0)), resample, np.float32(z),
                           np.float32(rng.choice([1.0, 3.0e-3, 40.0])))
-    if resample == 0 and rng.integers(0, 3) == 0 and n_c >= 1:      # explicit, irregular channel wavelengths (R16)
+    if rng.integers(0, 3) == 0 and n_c >= (2 if resample else 1):  # explicit, irregular channel wavelengths (R16, R20)
         steps = rng.uniform(0.4, 1.6, n_c)
         lam = (float(tel.lambda0) + float(tel.dlambda) * (np.cumsum(steps) - steps[0])).astype(np.float32)
         if np.all(np.diff(lam) > 0):
@@ -61,12 +63,12 @@ def random_case(seed):
     return w
 
 
-@pytest.mark.parametrize("seed", range(80))
+@pytest.mark.parametrize("seed", range(120))
 def test_random_configuration(B, seed):
     w = random_case(1234 + seed)
     t = w.telescope
     what = f"seed {seed}: n={w.particles.n} {t.n_x}x{t.n_y}x{t.n_channels} psf={t.psf_size} lsf={t.lsf_size} " \
-           f"resample={t.resample} log={w.ssp.log_lambda} z={float(t.redshift)} listed={t.lambda_obs is not None} alpha={float(t.psf_alpha)}"
+           f"resample={t.resample} log={w.ssp.log_lambda} listed_ssp={w.ssp.lambda_grid is not None} z={float(t.redshift)} listed={t.lambda_obs is not None} alpha={float(t.psf_alpha)}"
     dw = B.DeviceWorkload(w)
     cube = dw.build_cube(out=torch.full(dw.shape, float("nan"), device="cuda"))
     final = dw.convolve(cube)

@@ -84,3 +84,22 @@ def test_unsupported_and_invalid_combinations(B):
         with pytest.raises(B.RubixError):
             B.DeviceWorkload(w2).forward()
         assert msg in B.rubix_last_error(), B.rubix_last_error()
+
+
+def test_convolve_on_a_tiny_detector_keeps_the_sort_artefacts(B):
+    """The per-channel taps (15 x (n_c + 2) floats) are larger than a cube of fewer than 15 spaxels: they must not land on
+    the sort artefacts that rubix_build_cube left in the shared workspace (found by the r02 fuzz run, seed 118)."""
+    w = synth.make_workload("tiny", n=200)
+    w.telescope = dataclasses.replace(synth.Telescope(2, 3, np.float32(6.0), 88, np.float32(4700.0), np.float32(50.0)).with_psf_lsf(lsf_size=0),
+                                      psf_alpha=np.float32(-0.2), psf_lambda_ref=np.float32(6000.0))
+    dw = B.DeviceWorkload(w)
+    cube = dw.build_cube()
+    before = [a.clone() for a in dw.sort_artifacts()]
+    final = dw.convolve(cube)
+    torch.cuda.synchronize()
+    for a, b in zip(before, dw.sort_artifacts()):
+        assert torch.equal(a, b)
+    t = w.telescope
+    ref = oracle.convolve(oracle.build_cube(w.particles, w.rotation, w.ssp, t), t.psf_size, t.psf_sigma, t.lsf_size, t.lsf_sigma,
+                          oracle.psf_sigma_k(t))
+    assert np.abs(final.cpu().numpy() - ref).max() <= 1e-4 * ref.max()
