@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-adjoint", action="store_true")
     ap.add_argument("--no-batched", action="store_true")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
+                    help="replicas (default, BASELINE.json north_star: one galaxy per GPU, weak scaling) or sharded: ONE galaxy "
+                         "over all GPUs by detector rows (paper_2412_08265_b200/sharded.py, SURVEY.md 8(f)-4, strong scaling)")
     return ap.parse_args()
 
 
@@ -331,6 +334,74 @@ def time_batched(B, synth, dev, reps=20):
     out["what"] = ("rubix_forward_batched (one launch sequence for B cubes) vs B looped rubix_forward calls vs replays of a CUDA "
                    "graph of one rubix_forward; BASELINE.json configs[0] (tiny) and configs[1] (small), one galaxy under B rotations")
     return out
+
+
+def run_sharded(args):
+    """ONE galaxy over all ranks, sharded by detector rows: all-to-all of particle records, halo
+    exchange of raw rows, no cube exchange.  Strong scaling: value = the galaxy's samples / slowest rank's time.  Every rank
+    keeps its slice of the particle arrays resident; the step includes the binning, both exchanges and the PSF/LSF."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2412_08265_b200 import replicas, sharded, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    own_group = False
+    if not dist.is_initialized():
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29517")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+        own_group = True
+    w = synth.make_workload(args.workload)
+    t, p = w.telescope, w.particles
+    backend = sharded.CudaBackend(dev)
+    comm = sharded.DistComm()
+    sl = sharded.slice_for_rank(p.n, rank, world)
+    rec = sharded.pack_records(p.subset(np.arange(p.n)[sl]), dev)
+    flux = backend.upload_flux(w.ssp)
+
+    def step():
+        return sharded.forward_sharded(comm, backend, rec, w.rotation, w.ssp, t, flux_dev=flux)
+
+    for _ in range(max(args.warmup, 3)):
+        slab = step()
+    torch.cuda.synchronize()
+    dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        slab = step()
+    e1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    ms = replicas.max_over_ranks(e0.elapsed_time(e1), dev) / args.steps
+    rows = torch.tensor([float(slab.x1 - slab.x0), float(slab.n_received)], dtype=torch.float64, device=dev)
+    allr = [torch.zeros_like(rows) for _ in range(world)]
+    dist.all_gather(allr, rows)
+    if rank == 0:
+        line = {"metric": METRIC, "value": p.n * t.n_channels / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": dict(workload_config(w), parallelism=f"one galaxy sharded by detector rows over {world} GPUs "
+                               "(all-to-all of particle records + halo exchange of raw rows; no cube exchange)"),
+                "clocks": sampler.result(),
+                "rows_per_rank": [int(v[0].item()) for v in allr], "particles_per_rank": [int(v[1].item()) for v in allr],
+                "note": "host-orchestrated steps (routing with torch ops, per-step workspace allocation): a functional "
+                        "strong-scaling path, not the tuned single-GPU step of the default run"}
+        print(json.dumps(line))
+    if own_group:
+        dist.destroy_process_group()
 
 
 # ------------------------------------------------------------------------------------- our arm
@@ -649,5 +720,7 @@ if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.parallelism == "sharded":
+        run_sharded(a)
     else:
         run_ours(a)
