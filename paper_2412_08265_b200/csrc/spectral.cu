@@ -419,6 +419,160 @@ k_accumulate(const __grid_constant__ AccumParams P)
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Experimental variant (kept for the measurement in profiles/r02_accumulate_async.md): the four corner
+// windows of particle q + 1 are staged in shared memory by 1-D bulk async copies (cp.async.bulk, mbarrier completion)
+// while particle q is resampled; the blend then reads shared memory instead of waiting on LDG results in registers.
+// Point rule, uniform grids, one channel tile.  Built only with -DRUBIX_ACC_ASYNC=1.
+// ------------------------------------------------------------------------------------------
+#ifndef RUBIX_ACC_ASYNC
+#define RUBIX_ACC_ASYNC 0
+#endif
+#ifndef RUBIX_ACC_ASYNC_TABLES
+#define RUBIX_ACC_ASYNC_TABLES 2                     // 2: double-buffered table, one barrier per particle; 1: single table, two
+#endif
+#ifndef RUBIX_ACC_ASYNC_MINB
+#define RUBIX_ACC_ASYNC_MINB 2
+#endif
+#if RUBIX_ACC_ASYNC
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\t"
+                 "bra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ Quad lds_quad(const float *p)
+{
+    Quad q;
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "r"(smem_addr(p)));
+    return q;
+}
+
+template <int CPT>
+__global__ void __launch_bounds__(kAccThreads, RUBIX_ACC_ASYNC_MINB)
+k_accumulate_async(const __grid_constant__ AccumParams P)
+{
+    extern __shared__ __align__(128) float sm[];            // stage[4][wcap] | tab[NT][wcap] | records | mbarrier
+    constexpr int NT = RUBIX_ACC_ASYNC_TABLES;
+    const int tid = threadIdx.x;
+    const int u = blockIdx.x;
+    if (u >= P.totals[0]) return;
+    const Unit U = P.units[u];
+    if (U.count == 0 && P.skip_empty) return;
+    const int k_end = P.n_c - 1;
+    float *out = U.part_row >= 0 ? P.partials + (size_t)U.part_row * P.n_c : P.cube + (size_t)U.spaxel * P.n_c;
+    float acc[CPT];
+#pragma unroll
+    for (int i = 0; i < CPT; ++i) acc[i] = 0.0f;
+    if (U.count > 0) {
+        float *stage = sm, *tab = sm + 4 * (size_t)P.wcap;
+        int4 *srec = reinterpret_cast<int4 *>(tab + NT * (size_t)P.wcap);
+        const uint32_t bar = smem_addr(srec + 3 * kChunk);
+        {
+            const int4 *g = reinterpret_cast<const int4 *>(P.rec + U.start);
+            for (int i = tid; i < U.count * 3; i += kAccThreads) srec[i] = __ldg(g + i);
+        }
+        if (tid == 0) {
+            mbar_init(bar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        const int row_a = P.n_z * P.pitch, row_z = P.pitch;
+        // thread 0: start the copies of particle q's four corner windows (whole 128-sample groups; the padded grid copy
+        // absorbs the overshoot); returns nothing -- every thread derives "has a window" from the record itself
+        auto issue = [&](int q) {
+            const int4 rb = srec[3 * q + 1], rc = srec[3 * q + 2];
+            if (rc.x > rc.y) return;                          // no covered channel: no window
+            const uint32_t bytes = (uint32_t)((rc.w + kPass - 1) / kPass * kPass) * 4u;
+            const float *t0 = P.flux + (rb.x + rc.z);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the stage precede the async writes
+            mbar_expect_tx(bar, 4u * bytes);
+            bulk_g2s(smem_addr(stage), t0, bytes, bar);
+            bulk_g2s(smem_addr(stage + P.wcap), t0 + row_a, bytes, bar);
+            bulk_g2s(smem_addr(stage + 2 * (size_t)P.wcap), t0 + row_z, bytes, bar);
+            bulk_g2s(smem_addr(stage + 3 * (size_t)P.wcap), t0 + row_a + row_z, bytes, bar);
+        };
+        auto blend = [&](int q, float *buf) {
+            const int4 ra = srec[3 * q], rc = srec[3 * q + 2];
+            const float f0 = __int_as_float(ra.x), f1 = __int_as_float(ra.y), f2 = __int_as_float(ra.z), f3 = __int_as_float(ra.w);
+            const unsigned long long w0 = pack2(f0, f0), w1 = pack2(f1, f1), w2 = pack2(f2, f2), w3 = pack2(f3, f3);
+            const int n = (rc.w + kPass - 1) / kPass * kPass;
+            for (int s0 = 4 * tid; s0 < n; s0 += 4 * kAccThreads) {
+                const Quad c0 = lds_quad(stage + s0), c1 = lds_quad(stage + P.wcap + s0);
+                const Quad c2 = lds_quad(stage + 2 * (size_t)P.wcap + s0), c3 = lds_quad(stage + 3 * (size_t)P.wcap + s0);
+                const unsigned long long lo = ffma2(w3, c3.lo, ffma2(w2, c2.lo, ffma2(w1, c1.lo, fmul2(w0, c0.lo))));
+                const unsigned long long hi = ffma2(w3, c3.hi, ffma2(w2, c2.hi, ffma2(w1, c1.hi, fmul2(w0, c0.hi))));
+                sts_quad(buf + s0, lo, hi);
+            }
+        };
+        const uint32_t m_addr = 0x3FFCu, m_frac = 0x7FFFF8u, one_bits = 0x3F800000u;
+        auto resample = [&](int q, const float *buf) {
+            const int4 rb = srec[3 * q + 1], rc = srec[3 * q + 2];
+            if (rc.x > rc.y) return;
+            const char *bytes = reinterpret_cast<const char *>(buf);
+            const uint32_t b = (uint32_t)rb.y;
+            const int64_t a = (int64_t)(((uint64_t)(uint32_t)rb.w << 32) | (uint32_t)rb.z);
+            const int64_t base = a - ((int64_t)rc.z << kFxFrac);
+            const uint32_t x0 = (uint32_t)((base + (int64_t)b * tid) >> 8);
+            auto sample = [&](int i, uint32_t x) {
+                const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
+                const float s0 = e[0], s1 = e[1];
+                const float f = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;
+                acc[i] += fmaf(f, s1 - s0, s0);
+            };
+            if (rc.x == 0 && rc.y == k_end) {
+#pragma unroll
+                for (int i = 0; i < CPT; ++i) sample(i, x0 + (uint32_t)i * (b >> 1));
+            } else {
+#pragma unroll
+                for (int i = 0; i < CPT; ++i) {
+                    const int k = tid + i * kAccThreads;
+                    if (k >= rc.x && k <= rc.y) sample(i, x0 + (uint32_t)i * (b >> 1));
+                }
+            }
+        };
+        auto has_window = [&](int q) { const int4 rc = srec[3 * q + 2]; return rc.x <= rc.y; };
+        uint32_t parity = 0;
+        if (tid == 0) issue(0);
+        if (has_window(0)) { mbar_wait(bar, parity); parity ^= 1u; blend(0, tab); }
+        __syncthreads();
+        for (int q = 0; q < U.count; ++q) {
+            const bool more = q + 1 < U.count;
+            if (more && tid == 0) issue(q + 1);               // the stage is free: its last reader passed the barrier
+            resample(q, tab + (NT == 2 ? (size_t)(q & 1) * P.wcap : 0));
+            if (NT == 1) __syncthreads();                     // single table: every thread is done reading it
+            if (more && has_window(q + 1)) {
+                mbar_wait(bar, parity);
+                parity ^= 1u;
+                blend(q + 1, tab + (NT == 2 ? (size_t)((q + 1) & 1) * P.wcap : 0));
+            }
+            __syncthreads();
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < CPT; ++i) {
+        const int k = tid + i * kAccThreads;
+        if (k <= k_end) {
+            if (U.part_row >= 0) out[k] = acc[i];
+            else __stcs(out + k, acc[i]);
+        }
+    }
+}
+#endif  // RUBIX_ACC_ASYNC
+
 // Fixed-order second level for spaxels with more than kChunk particles: fp64 running sum over the
 // chunk rows (the kernel is bandwidth bound; the fp64 adds are free and keep 1e6-term sums exact
 // to fp32 rounding).
@@ -554,6 +708,19 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const size_t smem = (size_t)2 * wcap * sizeof(float) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
+#if RUBIX_ACC_ASYNC
+    if (!flux && !logx && !gen && P.n_tiles == 1 && cpt == 29) {     // the experimental staged variant (headline shape only)
+        const size_t sm_async = (size_t)(4 + RUBIX_ACC_ASYNC_TABLES) * wcap * sizeof(float) + (size_t)kChunk * sizeof(Rec) + 16;
+        {
+            StageTimer t(1, st);
+            auto kern = k_accumulate_async<29>;
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_async);
+            if (e != cudaSuccess) return e;
+            kern<<<grid, kAccThreads, sm_async, st>>>(P);
+            RUBIX_LAUNCH_CHECK();
+        }
+    } else
+#endif
     {
         StageTimer t(1, st);
         switch (cpt) {
