@@ -22,7 +22,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rubix_oracle.c")
-_LIB = os.path.join(_HERE, "librubix_oracle.so")
+# RUBIX_ORACLE_SANITIZE=1: a second build with -fsanitize=address,undefined (the process must then
+# be started with LD_PRELOAD=libasan, as tests/test_oracle_sanitizers.py does)
+_SANITIZE = os.environ.get("RUBIX_ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "librubix_oracle_san.so" if _SANITIZE else "librubix_oracle.so")
 _lock = threading.Lock()
 _lib = None
 
@@ -33,7 +36,8 @@ def build(force: bool = False) -> str:
     """gcc -O2, fp contraction off (the fp32 binning must round every op), OpenMP."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+        san = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-g", "-O1"] if _SANITIZE else ["-O2"]
+        subprocess.check_call(["gcc"] + san + ["-std=c11", "-fPIC", "-shared", "-fopenmp",
                                "-ffp-contract=off", "-fno-fast-math", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
