@@ -37,11 +37,11 @@ METRIC = "particle_channel_samples_per_s"
 UNIT = "G particle*channel/s"
 # four corner templates x 4 B x (dl_obs / dl_ssp) SSP samples per channel
 GATHER_BYTES_PER_SAMPLE = lambda tel, ssp: 16.0 * float(tel.dlambda) / float(ssp.dlambda)
-# DRAM bytes of one k_accumulate launch on the medium workload, from the committed ncu --set full
-# capture (profiles/r01_full_medium.md): 0.053 GB read + 1.347 GB written
-NCU_DRAM_BYTES_K_ACCUMULATE = 1.400e9
+# DRAM bytes of one k_accumulate launch on the medium workload inside rubix_forward, from the committed ncu --set full
+# capture (profiles/r02_full_medium.md): 0.0531 GB read + 0.3327 GB written (rows of empty spaxels are not written)
+NCU_DRAM_BYTES_K_ACCUMULATE = 0.3858e9
 NCU_TRAFFIC_SOURCE = ("STATIC: dram__bytes_read.sum + dram__bytes_write.sum of one k_accumulate launch in the committed "
-                      "ncu --set full capture profiles/r01_full_medium.md; not measured in this run")
+                      "ncu --set full capture profiles/r02_full_medium.md; not measured in this run")
 
 
 def parse():
@@ -486,6 +486,29 @@ def run_ours(args):
     two_call_ms = e0.elapsed_time(e1) / 5
     step()                                                    # `final` holds the fused call's cube again
 
+    # ---- the same step replayed from a CUDA graph (the call is capturable: no launch gaps between its 19 kernels)
+    graph_ms = None
+    try:
+        gs = torch.cuda.Stream(device=dev)
+        with torch.cuda.stream(gs):
+            B.rubix_forward(dw.particles, dw.ssp, dw.tel, dw.R, final, dw.workspace, stream=gs.cuda_stream)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=gs):
+            B.rubix_forward(dw.particles, dw.ssp, dw.tel, dw.R, final, dw.workspace, stream=torch.cuda.current_stream().cuda_stream)
+        for _ in range(3):
+            graph.replay()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(10):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        graph_ms = e0.elapsed_time(e1) / 10
+        del graph
+    except Exception as exc:                                  # reported, never fatal for the bench line
+        graph_ms = f"failed: {exc}"
+
     # ---- step 9 on the bench workload itself (outside the timed step): rubix_cube_adjoint with the final cube as the
     #      upstream gradient; the kernel's time per 1e6 in-FoV particles
     adjoint_workload = None
@@ -655,6 +678,33 @@ def run_ours(args):
                          "particle_pass_ms": st_l["particle_pass"]["ms"] / max(st_l["particle_pass"]["calls"], 1)}
         del dwl, cube_l
 
+    # ---- general-grid mode (readings R20 / R21): fp64 positions per sample
+    gen_variant = None
+    if args.workload in ("small", "medium", "contention"):
+        na, nz, nl = w.ssp.flux.shape
+        gen_variant = {"what": "rubix_build_cube in the general-grid mode (gen_coord.cuh: positions per sample in fp64), same "
+                               "particles and detector; k_accumulate<GEN> ms"}
+        cases = {"bin_average_on_log_grid": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, log_lambda=True), 1),
+                 "listed_ssp_wavelengths_point_rule": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, irregular=True), 0),
+                 "listed_ssp_wavelengths_bin_average": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, irregular=True), 1)}
+        for name, (ssp_g, rule) in cases.items():
+            wg = dataclasses.replace(w, ssp=ssp_g, telescope=dataclasses.replace(t, resample=rule))
+            dwg = B.DeviceWorkload(wg, device=dev)
+            cube_g = torch.empty(dw.shape, dtype=torch.float32, device=dev)
+            for _ in range(2):
+                dwg.build_cube(out=cube_g)
+            torch.cuda.synchronize()
+            B.rubix_stage_timing_enable(True)
+            B.rubix_stage_timing_read()
+            for _ in range(5):
+                dwg.build_cube(out=cube_g)
+            torch.cuda.synchronize()
+            st_g = B.rubix_stage_timing_read()
+            B.rubix_stage_timing_enable(False)
+            gen_variant[name] = {"k_accumulate_ms": st_g["accumulate"]["ms"] / max(st_g["accumulate"]["calls"], 1),
+                                 "particle_pass_ms": st_g["particle_pass"]["ms"] / max(st_g["particle_pass"]["calls"], 1)}
+            del dwg, cube_g
+
     # ---- noise stage (reading R17): elementwise, read + write of the cube
     noise_info = None
     if has_conv:
@@ -692,6 +742,7 @@ def run_ours(args):
             "gpu_launches": launches_per_step[0] * args.steps, "gpu_launches_per_step": launches_per_step[0],
             "stage_ms": stage_ms, "roofline": roofline,
             "api": "rubix_forward (steps 1-8 in one device call; occupancy-masked PSF/LSF passes)",
+            "graph_replay_ms_per_step": graph_ms,
             "two_calls": {"ms_per_step": two_call_ms,
                           "api": "rubix_build_cube + rubix_convolve_psf_lsf (dense raw cube, no masks; 5 steps)"}}
     line["roofline"]["whole_step"] = whole_step
@@ -700,6 +751,8 @@ def run_ours(args):
     line["flux_variant"] = flux_variant
     if table_variant is not None:
         line["log_grid_variant"] = table_variant
+    if gen_variant is not None:
+        line["general_grid_variant"] = gen_variant
     if noise_info is not None:
         line["noise_stage"] = noise_info
     if adjoint_info is not None:

@@ -338,7 +338,13 @@ constexpr int kAdjUSplit = 4;               // CTAs per unit: each takes kChunk 
 // lattice point: k >= -32/B - 2) and `back` behind it (a pass overshoots the last one by < 128/B + 8 points); both are
 // multiples of 4, chosen by the host from the smallest B the velocity cap allows.
 constexpr int kAdjUFrac = 44;               // fractional bits of x_k in this kernel
-constexpr int kAdjUFlush = 4;               // passes accumulated in fp32 before the fp64 flush
+#ifndef RUBIX_ADJU_FLUSH
+#define RUBIX_ADJU_FLUSH 8
+#endif
+#ifndef RUBIX_ADJU_DB
+#define RUBIX_ADJU_DB 0                      // 1: the next pass's corner quads are loaded into a second register set before this pass is worked on
+#endif
+constexpr int kAdjUFlush = RUBIX_ADJU_FLUSH;  // passes accumulated in fp32 before the fp64 flush
 
 struct AdjUParams {
     const int32_t *perm, *totals, *seg_off;
@@ -394,7 +400,8 @@ __device__ __forceinline__ void adj_add64(uint32_t &lo, uint32_t &hi, uint32_t b
 
 // One pass (one sample quad per lane) of one particle.  sg_bytes: byte address (shared window) of sg[0].
 template <int NA, int NB, bool MASK>
-__device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32_t sg_addr, int lane, int lim)
+__device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32_t sg_addr, int lane, int lim,
+                                         const AdjCorners *N = nullptr)
 {
     // ---- channels of the quad, interval by interval: sigma_i = sum g, b1_i = sum g (1 + frac)
     uint32_t addr = sg_addr + ((uint32_t)L.k << 2);
@@ -454,8 +461,14 @@ __device__ __forceinline__ void adj_pass(const AdjCorners &C, AdjLane &L, uint32
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const float2 a = unpack2(C.c[c].lo), bq = unpack2(C.c[c].hi);
-            float nx = __shfl_down_sync(0xffffffffu, a.x, 1);
-            if (lane == 31) nx = C.e[c];
+            float nx;
+            if (N) {                                        // lane 0 publishes the NEXT pass's first sample for lane 31
+                const float pub = lane == 0 ? unpack2(N->c[c].lo).x : a.x;
+                nx = __shfl_sync(0xffffffffu, pub, (lane + 1) & 31);
+            } else {
+                nx = __shfl_down_sync(0xffffffffu, a.x, 1);
+                if (lane == 31) nx = C.e[c];
+            }
             q[c] = fmaf(gm3, nx - bq.y, fmaf(gm2, bq.y - bq.x, fmaf(gm1, bq.x - a.y, fmaf(gm0, a.y - a.x, q[c]))));
         }
         L.q0 = q[0]; L.q1 = q[1]; L.q2 = q[2]; L.q3 = q[3];
@@ -684,6 +697,29 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
             int jp = j_begin;
             AdjCorners A;
             A.e[0] = A.e[1] = A.e[2] = A.e[3] = 0.0f;
+#if RUBIX_ADJU_DB
+            if (!FLUX) {
+                // two register sets: the quads of pass p + 1 are in flight while pass p is worked on (no L1 prefetch), and
+                // lane 31's fifth sample is lane 0's first sample of the next set (no extra loads); the padded grid copy
+                // makes the load behind the last pass harmless
+                auto load4 = [&](AdjCorners &C, const float *tt) {
+                    C.c[0] = adj_ldg_quad(tt); C.c[1] = adj_ldg_quad(tt + row_a);
+                    C.c[2] = adj_ldg_quad(tt + row_z); C.c[3] = adj_ldg_quad(tt + row_a + row_z);
+                };
+                AdjCorners Bn;
+                load4(A, t);
+                for (; jp <= j_last; jp += 128) {
+                    load4(Bn, t + 128);
+                    L.d_lo = (uint32_t)d; L.d_hi = (uint32_t)((uint64_t)d >> 32);
+                    if (jp <= j_main) adj_pass<NA, NB, false>(A, L, sg_addr, lane, 0, &Bn);
+                    else adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0, &Bn);
+                    advance();
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) A.c[c] = Bn.c[c];
+                }
+            } else
+#endif
+            {
             for (; jp <= j_main; jp += 128) {
                 load(A, t);
                 prefetch(t + 128);
@@ -698,6 +734,7 @@ k_adjoint_units(const __grid_constant__ AdjUParams P)
                 if (FLUX) adj_pass_flux<NA, NB, true>(A, L, c_carry, sg_addr, lane, P.n_lambda - 1 - j0);
                 else adj_pass<NA, NB, true>(A, L, sg_addr, lane, P.n_lambda - 1 - j0);
                 advance();
+            }
             }
             flush();
         }
