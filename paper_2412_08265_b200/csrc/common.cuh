@@ -141,6 +141,8 @@ struct GenGrid;
 int gen_kind(const rubix_ssp *s);
 // largest span of one channel (point rule: channel to channel; bin average: one bin) in SSP samples, Doppler cap included
 double gen_step_max(const rubix_ssp *s, const rubix_telescope *t);
+// samples spanned by tc consecutive channels (the table one channel tile needs)
+double gen_window_max(const rubix_ssp *s, const rubix_telescope *t, int tc);
 void gen_grid_params(const PassInputs &in, const Layout &L, char *ws, GenGrid *G);          // host only
 cudaError_t launch_adjoint_general(const PassInputs &in, const Layout &L, char *ws, const float *gconv, float *g_mass,
                                    float *g_age, float *g_z, float *g_v, cudaStream_t st);

@@ -4,23 +4,25 @@
 //   k_adjoint_general         step 9 for these modes: one warp per particle, lanes over the channels, fp64 positions
 #include <math.h>
 
+#include <vector>
+
 #include "common.cuh"
 #include "gen_coord.cuh"
 
 namespace rubix {
 
 __global__ void __launch_bounds__(256)
-k_gen_knots(int32_t n_lambda, const float *__restrict__ lam, double *__restrict__ knots, double *__restrict__ inv_w)
+k_gen_knots(int32_t n_lambda, const float *__restrict__ lam, double2 *__restrict__ kw)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_lambda) return;
-    knots[j] = (double)lam[j];
-    if (j + 1 < n_lambda) inv_w[j] = 1.0 / ((double)lam[j + 1] - (double)lam[j]);
+    const int i = j + 1 < n_lambda ? j : n_lambda - 2;      // the last entry repeats the last interval's width
+    kw[j] = make_double2((double)lam[j], 1.0 / ((double)lam[i + 1] - (double)lam[i]));
 }
 
 // lut[m] = largest j <= n_lambda - 2 with knots[j] <= start of cell m (0 for cells that start below the first knot)
 __global__ void __launch_bounds__(256)
-k_gen_lut(int32_t lut_n, double l0, double h, const double *__restrict__ knots, int32_t n_lambda, int32_t *__restrict__ lut)
+k_gen_lut(int32_t lut_n, double l0, double h, const double2 *__restrict__ kw, int32_t n_lambda, int32_t *__restrict__ lut)
 {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= lut_n) return;
@@ -28,7 +30,7 @@ k_gen_lut(int32_t lut_n, double l0, double h, const double *__restrict__ knots, 
     int lo = 0, hi = n_lambda - 2;
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if (knots[mid] <= start) lo = mid; else hi = mid - 1;
+        if (kw[mid].x <= start) lo = mid; else hi = mid - 1;
     }
     lut[m] = lo;
 }
@@ -112,6 +114,29 @@ double gen_step_max(const rubix_ssp *s, const rubix_telescope *t)
     return m * 1.001 + 1e-6;
 }
 
+// Largest number of SSP samples spanned by `tc` consecutive channels (point rule: channel k .. k + tc - 1; bin average:
+// edges k .. k + tc), inside the coverage, over the three Doppler factors that bound the velocity cap: what one channel
+// tile's table has to hold.  (gen_step_max x tc would charge the densest stretch of a listed grid to the whole tile.)
+double gen_window_max(const rubix_ssp *s, const rubix_telescope *t, int tc)
+{
+    const bool flux = t->resample == RUBIX_RESAMPLE_FLUX;
+    const int n_e = t->n_channels + (flux ? 1 : 0);
+    const int reach = flux ? tc : tc - 1;
+    const double betas[3] = {-kBetaCap, 0.0, kBetaCap};
+    const double x_top = (double)(s->n_lambda - 1);
+    std::vector<double> x((size_t)n_e);
+    double m = 0.0;
+    for (int b = 0; b < 3; ++b) {
+        const double c = 1.0 / (1.0 + betas[b]);
+        for (int e = 0; e < n_e; ++e) x[e] = fmin(fmax(host_coord(s, host_edge(t, e, flux) * c), 0.0), x_top);
+        for (int e = 0; e < n_e; ++e) {
+            const int hi = e + reach < n_e ? e + reach : n_e - 1;
+            m = fmax(m, x[hi] - x[e]);
+        }
+    }
+    return m * 1.001 + 1e-3;
+}
+
 // the GenGrid of a launch: pointers into the workspace and constants (host only, no launch)
 void gen_grid_params(const PassInputs &in, const Layout &L, char *ws, GenGrid *G)
 {
@@ -122,14 +147,22 @@ void gen_grid_params(const PassInputs &in, const Layout &L, char *ws, GenGrid *G
     G->a0 = -(double)s->lambda0 / (double)s->dlambda;
     G->log_scale = 1.0 / (double)s->dlambda;
     G->tab = (const double *)(ws + L.off_gtab);
-    G->knots = (const double *)(ws + L.off_gknots);
-    G->inv_w = (const double *)(ws + L.off_ginvw);
+    G->kw = (const double2 *)(ws + L.off_gknots);
     G->lut = (const int32_t *)(ws + L.off_glut);
     G->lut_n = kGenLutPerKnot * s->n_lambda;
     G->lut_l0 = 0.0;
     G->lut_inv_h = 0.0;
+    G->walk = 0;
     if (G->kind == 2) {
         const double first = (double)s->lambda_grid[0], last = (double)s->lambda_grid[s->n_lambda - 1];
+        double narrowest = last - first;
+        for (int j = 1; j < s->n_lambda; ++j)
+            narrowest = fmin(narrowest, (double)s->lambda_grid[j] - (double)s->lambda_grid[j - 1]);
+        // cells narrower than two of the narrowest intervals => the interval is the cell's or one of the next two
+        const double want = ceil((last - first) / (2.0 * narrowest) * (1.0 + 1e-6)) + 1.0;
+        const double cap = (double)kGenLutMaxPerKnot * s->n_lambda;
+        if (want > (double)G->lut_n) G->lut_n = (int32_t)(want < cap ? want : cap);
+        G->walk = want > cap ? 1 : 0;
         G->lut_l0 = first;
         G->lut_inv_h = (double)G->lut_n / (last - first);
     }
@@ -145,11 +178,10 @@ cudaError_t launch_gen_setup(const PassInputs &in, const Layout &L, char *ws, cu
         float *lam_dev = (float *)(ws + L.off_glam);
         e = cudaMemcpyAsync(lam_dev, s->lambda_grid, (size_t)s->n_lambda * 4, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return e;
-        k_gen_knots<<<(unsigned)((s->n_lambda + 255) / 256), 256, 0, st>>>(s->n_lambda, lam_dev, (double *)(ws + L.off_gknots),
-                                                                           (double *)(ws + L.off_ginvw));
+        k_gen_knots<<<(unsigned)((s->n_lambda + 255) / 256), 256, 0, st>>>(s->n_lambda, lam_dev, (double2 *)(ws + L.off_gknots));
         RUBIX_LAUNCH_CHECK();
         const double first = G->lut_l0, h = 1.0 / G->lut_inv_h;
-        k_gen_lut<<<(unsigned)((G->lut_n + 255) / 256), 256, 0, st>>>(G->lut_n, first, h, G->knots, s->n_lambda,
+        k_gen_lut<<<(unsigned)((G->lut_n + 255) / 256), 256, 0, st>>>(G->lut_n, first, h, G->kw, s->n_lambda,
                                                                       (int32_t *)(ws + L.off_glut));
         RUBIX_LAUNCH_CHECK();
     }

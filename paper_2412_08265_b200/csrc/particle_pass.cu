@@ -662,9 +662,9 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     for (int b = 0; b < 2; ++b) L.off_occ[b] = take((size_t)n_s + 64);   // occupancy of the raw cube / of the PSF temporary
     // general-grid mode (gen_coord.cuh): table over channel centres / bin edges, knots, inverse widths, look-up table
     L.off_gtab = take(((size_t)n_c + 2) * 8);
-    L.off_gknots = take(((size_t)n_lambda + 1) * 8);
-    L.off_ginvw = take(((size_t)n_lambda + 1) * 8);
-    L.off_glut = take(((size_t)kGenLutPerKnot * n_lambda + 8) * 4);
+    L.off_gknots = take(((size_t)n_lambda + 1) * 16);    // (knot, inverse interval width) pairs
+    L.off_ginvw = L.off_gknots;
+    L.off_glut = take(((size_t)kGenLutMaxPerKnot * n_lambda + 8) * 4);
     L.off_glam = take(((size_t)n_lambda + 1) * 4);
     L.bytes_total = off;
     return L;

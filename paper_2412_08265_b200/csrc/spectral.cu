@@ -68,9 +68,16 @@ __device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c)
 
 struct Quad { unsigned long long lo, hi; };          // four consecutive samples as two packed pairs
 
+// NOALLOC: the corner windows stream past L1 (listed-knot mode: L1 then keeps the look-up table and the knots, which every
+// sample reads; measured 37.7 -> 27.7 ms on the medium workload)
+template <bool NOALLOC = false>
 __device__ __forceinline__ Quad ldg_quad(const float *p)
 {
     Quad q;
+    if (NOALLOC) {
+        asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
+        return q;
+    }
 #if RUBIX_LDG_MODE == 1
     asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
 #elif RUBIX_LDG_MODE == 2
@@ -109,7 +116,10 @@ struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 // the record's b slot.  The thread keeps Y of its CPT channels relative to the tile start in registers (12.20).
 // GEN: general-grid mode (readings R20 / R21, gen_coord.cuh): x = gen_coord(tab[e], g) per sample in fp64, e = channel
 // (point rule) or bin edge (FLUX: channel k is the bin between edges k and k + 1, averaged over its FULL width in x).
-template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX, bool GEN = false>
+// NARROW (GEN + FLUX): no bin is wider than one SSP sample, so a bin touches at most two knot intervals and is integrated
+// through three samples without a branch (as the fixed-point kernel does for B <= 1).
+// GEN = 0: off; 1 + kind of gen_coord.cuh otherwise (1 linear, 2 log-sampled, 3 listed SSP wavelengths).
+template <int CPT, bool SINGLE, int DEPTH, int MINB, bool FLUX, bool LOGX, int GEN = 0, bool NARROW = false>
 __global__ void __launch_bounds__(kAccThreads, MINB)
 k_accumulate(const __grid_constant__ AccumParams P)
 {
@@ -167,8 +177,8 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 j0 = 0; W.nw = 0;
                 if (W.ka <= W.kb) {                         // as k_prepare_records, for this tile's channels
                     const double x_top = (double)(P.n_lambda - 1);
-                    const double xa = fmin(fmax(gen_coord(P.gen, P.gen.tab[W.ka], W.g) - 1e-6, 0.0), x_top);
-                    const double xb = fmin(fmax(gen_coord(P.gen, P.gen.tab[W.kb + (FLUX ? 1 : 0)], W.g) + 1e-6, 0.0), x_top);
+                    const double xa = fmin(fmax(gen_coord_k<GEN - 1>(P.gen, P.gen.tab[W.ka], W.g) - 1e-6, 0.0), x_top);
+                    const double xb = fmin(fmax(gen_coord_k<GEN - 1>(P.gen, P.gen.tab[W.kb + (FLUX ? 1 : 0)], W.g) + 1e-6, 0.0), x_top);
                     j0 = (int)xa & ~(kRowAlign - 1);
                     W.nw = (int)xb - j0 + 2;
                 }
@@ -213,10 +223,11 @@ k_accumulate(const __grid_constant__ AccumParams P)
             return q;
         };
         auto issue = [&](LoadSet &L, const float *t0) {
-            L.c[0] = RUBIX_TEX_CORNERS >= 4 ? tex_quad(t0) : ldg_quad(t0);
-            L.c[1] = RUBIX_TEX_CORNERS >= 3 ? tex_quad(t0 + row_a) : ldg_quad(t0 + row_a);
-            L.c[2] = RUBIX_TEX_CORNERS >= 2 ? tex_quad(t0 + row_z) : ldg_quad(t0 + row_z);
-            L.c[3] = RUBIX_TEX_CORNERS >= 1 ? tex_quad(t0 + row_a + row_z) : ldg_quad(t0 + row_a + row_z);
+            constexpr bool NA = GEN == 3;
+            L.c[0] = RUBIX_TEX_CORNERS >= 4 ? tex_quad(t0) : ldg_quad<NA>(t0);
+            L.c[1] = RUBIX_TEX_CORNERS >= 3 ? tex_quad(t0 + row_a) : ldg_quad<NA>(t0 + row_a);
+            L.c[2] = RUBIX_TEX_CORNERS >= 2 ? tex_quad(t0 + row_z) : ldg_quad<NA>(t0 + row_z);
+            L.c[3] = RUBIX_TEX_CORNERS >= 1 ? tex_quad(t0 + row_a + row_z) : ldg_quad<NA>(t0 + row_a + row_z);
         };
         auto consume = [&](const LoadSet &L, const Win &W, float *dst) {
             const unsigned long long w0 = pack2(W.w0, W.w0), w1 = pack2(W.w1, W.w1);
@@ -272,40 +283,65 @@ k_accumulate(const __grid_constant__ AccumParams P)
             }
             acc[i] = fmaf(tot, inv_b, acc[i]);
         };
-        // GEN: integral of the table's interpolant over [a, b] (sample coordinates relative to the table start, a < b)
-        auto gen_integral = [&](const float *tabp, double a, double b) -> float {
-            const int ja = (int)a, jb = (int)b;
-            const float fa = (float)(a - (double)ja), fb = (float)(b - (double)jb);
-            const float a0 = tabp[ja], a1 = tabp[ja + 1];
-            if (ja == jb) return (fb - fa) * fmaf(0.5f * (fa + fb), a1 - a0, a0);
-            const float c0 = tabp[jb], c1 = tabp[jb + 1];
-            float tot = 0.5f * (1.0f - fa) * (fmaf(fa, a1 - a0, a0) + a1);
-            tot = fmaf(0.5f * fb, c0 + fmaf(fb, c1 - c0, c0), tot);
-            for (int j = ja + 1; j < jb; ++j) tot = fmaf(0.5f, tabp[j] + tabp[j + 1], tot);
-            return tot;
-        };
         auto resample = [&](const Win &W, const float *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
             if (GEN) {
+                // Branch-free per sample (a channel outside [ka, kb] or outside the coverage is computed on a clamped
+                // position and masked), so that the unrolled iterations overlap their table loads and fp64 chains.
                 const double x_top = (double)(P.n_lambda - 1), j0d = (double)W.j0;
-#pragma unroll 1
+                const int e_max = P.n_c - (FLUX ? 0 : 1);
+                // local position -> (table index, fraction); one fp64 subtraction, then everything in fp32
+                auto split = [&](double x, int &j, float &f) {
+                    const double xl = x - j0d;
+                    j = (int)xl;
+                    f = (float)(xl - (double)j);
+                };
+#pragma unroll                                              // fully: acc[i] must stay in registers
                 for (int i = 0; i < CPT; ++i) {
                     const int k = k0 + tid + i * kAccThreads;
-                    if (k < W.ka || k > W.kb) continue;
+                    const bool in_k = k >= W.ka && k <= W.kb;
+                    const int kc = min(k, e_max);
                     if (!FLUX) {
-                        const double x = gen_coord(P.gen, __ldg(P.gen.tab + k), W.g);
-                        if (x >= 0.0 && x <= x_top) {
-                            const double xl = x - j0d;
-                            const int j = (int)xl;
-                            const float f = (float)(xl - (double)j);
-                            const float s0 = buf[j], s1 = buf[j + 1];
-                            acc[i] += fmaf(f, s1 - s0, s0);
-                        }
+                        const double x = gen_coord_k<GEN - 1>(P.gen, __ldg(P.gen.tab + kc), W.g);
+                        const bool ok = in_k && x >= 0.0 && x <= x_top;
+                        int j; float f;
+                        split(ok ? x : j0d, j, f);
+                        const float s0 = buf[j], s1 = buf[j + 1];
+                        acc[i] += ok ? fmaf(f, s1 - s0, s0) : 0.0f;
                     } else {
-                        const double xlo = gen_coord(P.gen, __ldg(P.gen.tab + k), W.g);
-                        const double xhi = gen_coord(P.gen, __ldg(P.gen.tab + k + 1), W.g);
+                        const double xlo = gen_coord_k<GEN - 1>(P.gen, __ldg(P.gen.tab + kc), W.g);
+                        const double xhi = gen_coord_k<GEN - 1>(P.gen, __ldg(P.gen.tab + min(kc + 1, e_max)), W.g);
                         const double cl = fmax(xlo, 0.0), ch = fmin(xhi, x_top);
-                        if (ch > cl) acc[i] = fmaf(gen_integral(buf, cl - j0d, ch - j0d), (float)(1.0 / (xhi - xlo)), acc[i]);
+                        const bool ok = in_k && ch > cl;
+                        float tot;
+                        if (NARROW) {
+                            // I(u) = integral of the interpolant from knot ja to ja + u (u < 2) through a0, a1, a2
+                            int ja; float fa;
+                            split(ok ? cl : j0d, ja, fa);
+                            const float u = fa + (ok ? (float)(ch - cl) : 0.0f);
+                            const float u1 = fminf(u, 1.0f), u2 = fmaxf(u - 1.0f, 0.0f);
+                            const float a0 = buf[ja], a1 = buf[ja + 1], a2r = buf[ja + 2];
+                            const float a2 = u > 1.0f ? a2r : a1;         // buf[ja + 2] may lie beyond the blended window
+                            const float d1 = a1 - a0, d2 = a2 - a1;
+                            const float il = fa * fmaf(0.5f * fa, d1, a0);
+                            float iu = u1 * fmaf(0.5f * u1, d1, a0);
+                            iu = fmaf(u2, fmaf(0.5f * u2, d2, a1), iu);
+                            tot = iu - il;
+                        } else {
+                            int ja, jb; float fa, fb;
+                            split(ok ? cl : j0d, ja, fa);
+                            split(ok ? ch : j0d, jb, fb);
+                            const float a0 = buf[ja], a1 = buf[ja + 1], c0 = buf[jb], c1 = buf[jb + 1];
+                            // same interval: (fb - fa) * value at the midpoint; else the two partial trapezoids + whole intervals
+                            tot = (fb - fa) * fmaf(0.5f * (fa + fb), a1 - a0, a0);
+                            if (ja != jb) {
+                                tot = 0.5f * (1.0f - fa) * (fmaf(fa, a1 - a0, a0) + a1);
+                                tot = fmaf(0.5f * fb, c0 + fmaf(fb, c1 - c0, c0), tot);
+                                for (int j = ja + 1; j < jb; ++j) tot = fmaf(0.5f, buf[j] + buf[j + 1], tot);
+                            }
+                        }
+                        const float inv_w = __fdividef(1.0f, (float)(xhi - xlo));   // the FULL width of the bin
+                        acc[i] = ok ? fmaf(tot, inv_w, acc[i]) : acc[i];
                     }
                 }
                 return;
@@ -604,10 +640,10 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
     }
 }
 
-template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false, bool GEN = false>
+template <int CPT, bool SINGLE, bool FLUX, bool LOGX = false, int GEN = 0, bool NARROW = false>
 static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem, cudaStream_t st)
 {
-    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, (LOGX || GEN) ? 3 : kAccMinBlocks, FLUX, LOGX, GEN>;
+    auto kern = k_accumulate<CPT, SINGLE, kAccDepth, (LOGX || GEN) ? 3 : kAccMinBlocks, FLUX, LOGX, GEN, NARROW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kAccThreads, smem, st>>>(P);
@@ -616,15 +652,8 @@ static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem,
 }
 
 template <int CPT>
-static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, bool gen, unsigned grid, size_t smem, cudaStream_t st)
+static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsigned grid, size_t smem, cudaStream_t st)
 {
-    if (gen) {
-        if (P.n_tiles == 1)
-            return flux ? launch_acc2<CPT, true, true, false, true>(P, grid, smem, st)
-                        : launch_acc2<CPT, true, false, false, true>(P, grid, smem, st);
-        return flux ? launch_acc2<CPT, false, true, false, true>(P, grid, smem, st)
-                    : launch_acc2<CPT, false, false, false, true>(P, grid, smem, st);
-    }
     if (logx)
         return P.n_tiles == 1 ? launch_acc2<CPT, true, false, true>(P, grid, smem, st)
                               : launch_acc2<CPT, false, false, true>(P, grid, smem, st);
@@ -633,19 +662,46 @@ static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, bool g
     return flux ? launch_acc2<CPT, false, true>(P, grid, smem, st) : launch_acc2<CPT, false, false>(P, grid, smem, st);
 }
 
+// general-grid mode: instantiated for CPT in {29, 8, 1} only (choose_cpt draws from that list then)
+template <int CPT, int GEN>
+static cudaError_t launch_acc_gen2(const AccumParams &P, bool flux, bool narrow, unsigned grid, size_t smem, cudaStream_t st)
+{
+    if (flux && narrow)
+        return P.n_tiles == 1 ? launch_acc2<CPT, true, true, false, GEN, true>(P, grid, smem, st)
+                              : launch_acc2<CPT, false, true, false, GEN, true>(P, grid, smem, st);
+    if (P.n_tiles == 1)
+        return flux ? launch_acc2<CPT, true, true, false, GEN>(P, grid, smem, st)
+                    : launch_acc2<CPT, true, false, false, GEN>(P, grid, smem, st);
+    return flux ? launch_acc2<CPT, false, true, false, GEN>(P, grid, smem, st)
+                : launch_acc2<CPT, false, false, false, GEN>(P, grid, smem, st);
+}
+template <int CPT>
+static cudaError_t launch_acc_gen(const AccumParams &P, bool flux, bool narrow, unsigned grid, size_t smem, cudaStream_t st)
+{
+    switch (P.gen.kind) {
+        case 0: return launch_acc_gen2<CPT, 1>(P, flux, narrow, grid, smem, st);
+        case 1: return launch_acc_gen2<CPT, 2>(P, flux, narrow, grid, smem, st);
+        default: return launch_acc_gen2<CPT, 3>(P, flux, narrow, grid, smem, st);
+    }
+}
+
 // Largest CPT in {29, 15, 8, 4, 2, 1} whose table fits the 12.20 format; returns the table capacity
 // (samples, a whole number of passes).
-int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out)
+int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out, const rubix_ssp *gen_ssp = nullptr,
+               const rubix_telescope *gen_tel = nullptr)
 {
     const int cand[6] = {29, 15, 8, 4, 2, 1};
     for (int c = 0; c < 6; ++c) {
         const int cpt = cand[c];
+        if (gen_ssp && cpt != 29 && cpt != 8 && cpt != 1) continue;   // the instantiated general-grid kernels
         const int tc = cpt * kAccThreads;
         const int tiles = (n_c + tc - 1) / tc;
         // skip tilings that leave a whole 256-channel group of lanes idle (unless the smallest)
         if (cpt > 1 && (long long)tiles * tc - n_c >= kAccThreads) continue;
         // samples j0 .. j_max + 1 with j0 rounded down to a multiple of kRowAlign
-        const int need = (int)(b_max * (tc + (flux ? 1 : 0))) + kRowAlign + 4;
+        // general-grid mode: the exact span of the widest tile (a listed grid is not equally dense everywhere)
+        const int need = gen_ssp ? (int)gen_window_max(gen_ssp, gen_tel, tc < n_c ? tc : n_c) + kRowAlign + 6
+                                 : (int)(b_max * (tc + (flux ? 1 : 0))) + kRowAlign + 4;
         const int wcap = (need + kPass - 1) / kPass * kPass;
         if (wcap > kTabMax) continue;
         *wcap_out = wcap;
@@ -664,7 +720,8 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const double b_max = gen ? gen_step_max(in.ssp, in.tel) : (logx ? table_step_max(in.ssp, in.tel) : b0 / (1.0 - kBetaCap));
     int wcap = 0;
     const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
-    const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap);
+    const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap, gen ? in.ssp : nullptr, gen ? in.tel : nullptr);
+    const bool narrow = gen && flux && b_max <= 1.0;        // no bin wider than one SSP sample
     if (cpt == 0) return cudaErrorInvalidConfiguration;
     AccumParams P;
     P.flux = (const float *)(ws + L.off_flux);
@@ -723,13 +780,21 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
 #endif
     {
         StageTimer t(1, st);
-        switch (cpt) {
-            case 29: e = launch_acc<29>(P, flux, logx, gen, grid, smem, st); break;
-            case 15: e = launch_acc<15>(P, flux, logx, gen, grid, smem, st); break;
-            case 8: e = launch_acc<8>(P, flux, logx, gen, grid, smem, st); break;
-            case 4: e = launch_acc<4>(P, flux, logx, gen, grid, smem, st); break;
-            case 2: e = launch_acc<2>(P, flux, logx, gen, grid, smem, st); break;
-            default: e = launch_acc<1>(P, flux, logx, gen, grid, smem, st); break;
+        if (gen) {
+            switch (cpt) {
+                case 29: e = launch_acc_gen<29>(P, flux, narrow, grid, smem, st); break;
+                case 8: e = launch_acc_gen<8>(P, flux, narrow, grid, smem, st); break;
+                default: e = launch_acc_gen<1>(P, flux, narrow, grid, smem, st); break;
+            }
+        } else {
+            switch (cpt) {
+                case 29: e = launch_acc<29>(P, flux, logx, grid, smem, st); break;
+                case 15: e = launch_acc<15>(P, flux, logx, grid, smem, st); break;
+                case 8: e = launch_acc<8>(P, flux, logx, grid, smem, st); break;
+                case 4: e = launch_acc<4>(P, flux, logx, grid, smem, st); break;
+                case 2: e = launch_acc<2>(P, flux, logx, grid, smem, st); break;
+                default: e = launch_acc<1>(P, flux, logx, grid, smem, st); break;
+            }
         }
     }
     if (e != cudaSuccess) return e;
