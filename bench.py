@@ -682,8 +682,9 @@ def run_ours(args):
     gen_variant = None
     if args.workload in ("small", "medium", "contention"):
         na, nz, nl = w.ssp.flux.shape
-        gen_variant = {"what": "rubix_build_cube in the general-grid mode (gen_coord.cuh: positions per sample in fp64), same "
-                               "particles and detector; k_accumulate<GEN> ms"}
+        gen_variant = {"what": "rubix_build_cube under readings R20 / R21, same particles and detector, k_accumulate ms: the bin average "
+                               "on a log-sampled grid (table mode, fixed point) and listed SSP wavelengths (general-grid mode, "
+                               "positions per sample in fp64)"}
         cases = {"bin_average_on_log_grid": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, log_lambda=True), 1),
                  "listed_ssp_wavelengths_point_rule": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, irregular=True), 0),
                  "listed_ssp_wavelengths_bin_average": (synth.make_ssp(na, nz, nl, 3000.0, 10000.0, 2101, irregular=True), 1)}

@@ -845,7 +845,8 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
                            float *g_mass, float *g_age, float *g_z, float *g_v, cudaStream_t st)
 {
     if (L.n == 0) return cudaSuccess;
-    if (gen_mode(in.ssp, in.tel)) return launch_adjoint_general(in, L, ws, gconv, g_mass, g_age, g_z, g_v, st);
+    if (gen_mode(in.ssp, in.tel) || table_flux(in.ssp, in.tel))
+        return launch_adjoint_general(in, L, ws, gconv, g_mass, g_age, g_z, g_v, st);
     AdjParams P;
     P.ax.n_age = in.ssp->n_age;
     P.ax.n_z = in.ssp->n_z;

@@ -159,8 +159,10 @@ rubix_status check_resampler(const rubix_ssp *s, const rubix_telescope *t)
         return RUBIX_OK;
     }
     if (table_mode(s, t)) {
-        if (!t->lambda_obs && !((double)t->lambda0 > 0.0))
-            return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths must be > 0 for a log-sampled ssp grid");
+        const bool fl = t->resample == RUBIX_RESAMPLE_FLUX;
+        const double first = t->lambda_obs ? (double)t->lambda_obs[0] - (fl ? 0.5 * ((double)t->lambda_obs[1] - (double)t->lambda_obs[0]) : 0.0)
+                                           : (double)t->lambda0 - (fl ? 0.5 * (double)t->dlambda : 0.0);
+        if (!(first > 0.0)) return fail(RUBIX_ERR_INVALID_ARG, "observed wavelengths (bin edges included) must be > 0");
         const double b0 = table_step_max(s, t);
         if (!(b0 < 14.25))
             return fail(RUBIX_ERR_UNSUPPORTED, "d x / d channel = %.3f is outside the resampler range (< 14.25)", b0);

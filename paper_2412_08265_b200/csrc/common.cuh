@@ -126,16 +126,22 @@ cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t
 
 // Table mode (readings R15 / R16): the rest position of channel k is x_k = Y[k] c + a with a per-launch
 // table Y and per-particle (c, a); used for log-sampled SSP grids and for explicit channel wavelengths.
-// General-grid mode (readings R20 / R21, gen_coord.cuh): listed SSP wavelengths, or the bin average on a log-sampled grid
-// or on listed channel wavelengths; positions per sample in fp64.  It takes precedence over the table mode.
+// General-grid mode (reading R21, gen_coord.cuh): listed SSP wavelengths; positions per sample in fp64.  Takes precedence
+// over the table mode.
 inline bool gen_mode(const rubix_ssp *s, const rubix_telescope *t)
 {
-    return s->lambda_grid != nullptr ||
-           (t->resample == RUBIX_RESAMPLE_FLUX && (s->log_lambda != 0 || t->lambda_obs != nullptr));
+    (void)t;
+    return s->lambda_grid != nullptr;
 }
+// Table mode (readings R15 / R16, and R20 for the bin average): log-sampled SSP grid and / or listed channel wavelengths.
 inline bool table_mode(const rubix_ssp *s, const rubix_telescope *t)
 {
     return !gen_mode(s, t) && (s->log_lambda != 0 || t->lambda_obs != nullptr);
+}
+// table mode under the bin average: the per-launch table holds the n_c + 1 bin edges; the adjoint is k_adjoint_general
+inline bool table_flux(const rubix_ssp *s, const rubix_telescope *t)
+{
+    return table_mode(s, t) && t->resample == RUBIX_RESAMPLE_FLUX;
 }
 struct GenGrid;
 int gen_kind(const rubix_ssp *s);

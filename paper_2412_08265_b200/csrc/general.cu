@@ -245,8 +245,8 @@ k_adjoint_general(const __grid_constant__ AdjGenParams P)
     const Rec r = P.rec[i];
     const AdjAux ax = P.aux[i];
     const GenGrid &G = P.gen;
-    const double g = __longlong_as_double(r.a_fx);
     const double opb = 1.0 + (double)P.vlos[p] / kCkms, inv_opb = 1.0 / opb;
+    const double g = gen_doppler(G, opb);                   // (the table mode's records carry fixed-point values instead)
     const float *gr = P.gconv + (size_t)P.key[p] * P.n_c;
     const float *T0 = P.flux + r.cell;
     const float *T1 = T0 + (size_t)P.n_z * P.pitch, *T2 = T0 + P.pitch, *T3 = T1 + P.pitch;

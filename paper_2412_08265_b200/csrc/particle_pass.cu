@@ -442,14 +442,23 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
         a_fx = P.log_grid ? -__double2ll_rn(log10(opb) / (double)P.dl_ssp * scale)
                           : -__double2ll_rn((double)P.l0_ssp / (double)P.dl_ssp * scale);
         auto xk = [&](int k) { return __double2ll_rn((double)P.xtab[k] * c) + a_fx; };
-        int lo = 0, hi = P.n_c;                            // first k with x_k >= 0
-        while (lo < hi) { const int mid = (lo + hi) >> 1; if (xk(mid) >= 0) hi = mid; else lo = mid + 1; }
+        const bool fl = P.mode == RUBIX_RESAMPLE_FLUX;     // the table then holds bin edges: bin k = [x_k, x_{k+1}]
+        int lo = 0, hi = P.n_c;                            // point: first k with x_k >= 0; bins: first k with x_{k+1} > 0
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (fl ? xk(mid + 1) > 0 : xk(mid) >= 0) hi = mid; else lo = mid + 1;
+        }
         k_lo = lo;
-        lo = -1; hi = P.n_c - 1;                           // last k with x_k <= x_max
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (xk(mid) <= x_max) lo = mid; else hi = mid - 1; }
+        lo = -1; hi = P.n_c - 1;                           // point: last k with x_k <= x_max; bins: last k with x_k < x_max
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (fl ? xk(mid) < x_max : xk(mid) <= x_max) lo = mid; else hi = mid - 1;
+        }
         k_hi = lo;
         x_first = k_lo <= k_hi ? xk((int)k_lo) : 0;
-        x_last = k_lo <= k_hi ? xk((int)k_hi) : 0;
+        x_last = k_lo <= k_hi ? xk((int)k_hi + (fl ? 1 : 0)) : 0;
+        if (x_first < 0) x_first = 0;
+        if (x_last > x_max) x_last = x_max;
     } else if (P.mode == RUBIX_RESAMPLE_FLUX) {
         // x_k = a_fx + b k is the LOWER EDGE of bin k (upper edge = lower edge of bin k + 1);
         // [k_lo, k_hi] = bins that overlap the coverage [0, N_l - 1]
@@ -533,11 +542,23 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_positions(int32_t n_c, const float *__restrict__ lam, double l0_obs, double dl_obs, double zp1, int32_t log_grid,
-            double l0_ssp, double dl_ssp, int64_t *__restrict__ ytab)
+            double l0_ssp, double dl_ssp, int32_t edges, int64_t *__restrict__ ytab)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > n_c) return;
-    const double l = (lam ? (double)lam[min(k, n_c - 1)] : l0_obs + dl_obs * (double)k) / zp1;
+    double l;
+    if (!edges) {
+        l = lam ? (double)lam[min(k, n_c - 1)] : l0_obs + dl_obs * (double)k;
+    } else if (!lam) {                                     // bin average (reading R20): entry e = lower edge of bin e
+        l = l0_obs + dl_obs * ((double)k - 0.5);
+    } else if (k == 0) {
+        l = (double)lam[0] - 0.5 * ((double)lam[1] - (double)lam[0]);
+    } else if (k == n_c) {
+        l = (double)lam[n_c - 1] + 0.5 * ((double)lam[n_c - 1] - (double)lam[n_c - 2]);
+    } else {
+        l = 0.5 * ((double)lam[k - 1] + (double)lam[k]);
+    }
+    l /= zp1;
     const double y = log_grid ? log10(l / l0_ssp) / dl_ssp : l / dl_ssp;
     ytab[k] = __double2ll_rn(y * (double)(1 << kFxFrac));
 }
@@ -562,16 +583,26 @@ cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const
 double table_step_max(const rubix_ssp *s, const rubix_telescope *t)
 {
     const double zp1 = 1.0 + (double)t->redshift;
+    const bool edges = t->resample == RUBIX_RESAMPLE_FLUX;  // bin average: the table holds the n_c + 1 bin edges
+    const int n_c = t->n_channels;
     auto y = [&](int k) {
-        const double l = (t->lambda_obs ? (double)t->lambda_obs[k] : (double)t->lambda0 + (double)t->dlambda * k) / zp1;
+        const float *lam = t->lambda_obs;
+        double l;
+        if (!edges) l = lam ? (double)lam[k] : (double)t->lambda0 + (double)t->dlambda * k;
+        else if (!lam) l = (double)t->lambda0 + (double)t->dlambda * ((double)k - 0.5);
+        else if (k == 0) l = (double)lam[0] - 0.5 * ((double)lam[1] - (double)lam[0]);
+        else if (k == n_c) l = (double)lam[n_c - 1] + 0.5 * ((double)lam[n_c - 1] - (double)lam[n_c - 2]);
+        else l = 0.5 * ((double)lam[k - 1] + (double)lam[k]);
+        l /= zp1;
         return s->log_lambda ? log10(l / (double)s->lambda0) / (double)s->dlambda : l / (double)s->dlambda;
     };
     double m = 0.0;
-    if (t->n_channels < 2) return 0.0;
+    const int n_e = n_c + (edges ? 1 : 0);
+    if (n_e < 2) return 0.0;
     if (!t->lambda_obs) {                                  // uniform grid: steepest at one of the two ends
-        m = fmax(y(1) - y(0), y(t->n_channels - 1) - y(t->n_channels - 2));
+        m = fmax(y(1) - y(0), y(n_e - 1) - y(n_e - 2));
     } else {
-        for (int k = 1; k < t->n_channels; ++k) m = fmax(m, y(k) - y(k - 1));
+        for (int k = 1; k < n_e; ++k) m = fmax(m, y(k) - y(k - 1));
     }
     return s->log_lambda ? m : m / (1.0 - kBetaCap);
 }
@@ -787,8 +818,14 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
             }
             k_positions<<<(unsigned)((L.n_c + 256) / 256), 256, 0, st>>>(
                 L.n_c, lam_dev, (double)in.tel->lambda0, (double)in.tel->dlambda, 1.0 + (double)in.tel->redshift,
-                P.log_grid, (double)in.ssp->lambda0, (double)in.ssp->dlambda, (int64_t *)(ws + L.off_xtab));
+                P.log_grid, (double)in.ssp->lambda0, (double)in.ssp->dlambda, P.mode == RUBIX_RESAMPLE_FLUX ? 1 : 0,
+                (int64_t *)(ws + L.off_xtab));
             RUBIX_LAUNCH_CHECK();
+            if (P.mode == RUBIX_RESAMPLE_FLUX) {           // the adjoint of this combination is k_adjoint_general: its tables
+                GenGrid Gt;
+                cudaError_t eg = launch_gen_setup(in, L, ws, st, &Gt);
+                if (eg != cudaSuccess) return eg;
+            }
         }
         P.redshift = in.tel->redshift;
         P.flux_scale = in.tel->flux_scale;

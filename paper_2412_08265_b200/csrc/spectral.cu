@@ -36,6 +36,7 @@ struct AccumParams {
     float *partials;
     int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
     int32_t skip_empty;      // 1: empty spaxels are left unwritten (the masked PSF/LSF passes never read them)
+    int32_t narrow;          // bin average in table / general-grid mode: no bin is wider than one SSP sample
     const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
     cudaTextureObject_t tex;
     GenGrid gen;             // GEN: general-grid mode (gen_coord.cuh)
@@ -137,6 +138,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                                  : P.cube + (size_t)U.spaxel * P.n_c;
     float acc[CPT];
     uint32_t xl[LOGX ? CPT : 1];
+    uint32_t wd[(LOGX && FLUX) ? CPT : 1];                  // LOGX + FLUX: width of the thread's bins at beta = 0 (2^-20 samples)
     int64_t x_tile0 = 0;                                    // LOGX: xtab[k0]
 #pragma unroll
     for (int i = 0; i < CPT; ++i) acc[i] = 0.0f;
@@ -148,6 +150,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
             for (int i = 0; i < CPT; ++i) {
                 const int k = k0 + tid + i * kAccThreads;
                 xl[i] = (uint32_t)((P.xtab[min(k, P.n_c)] - x_tile0) >> 8);
+                if (FLUX) wd[i] = (uint32_t)((P.xtab[min(k + 1, P.n_c)] - P.xtab[min(k, P.n_c)]) >> 8);
             }
         }
         int4 *srec = reinterpret_cast<int4 *>(tab + 2 * (size_t)P.wcap);
@@ -191,7 +194,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                     if (LOGX) {
                         const double c = (double)W.b * (1.0 / (double)(1u << 30));
                         xa = a + __double2ll_rn((double)P.xtab[W.ka] * c);
-                        xb = a + __double2ll_rn((double)P.xtab[W.kb] * c);
+                        xb = a + __double2ll_rn((double)P.xtab[W.kb + (FLUX ? 1 : 0)] * c);
                     }
                     if (FLUX) {                             // bins are clipped to the coverage
                         xa = max(xa, (int64_t)0);
@@ -342,6 +345,48 @@ k_accumulate(const __grid_constant__ AccumParams P)
                         }
                         const float inv_w = __fdividef(1.0f, (float)(xhi - xlo));   // the FULL width of the bin
                         acc[i] = ok ? fmaf(tot, inv_w, acc[i]) : acc[i];
+                    }
+                }
+                return;
+            }
+            if (FLUX && LOGX) {
+                // Bin average in table mode (reading R20): the table holds the bin edges, x_e = Y[e] c + a; the thread keeps
+                // the lower edge and the width of its bins at beta = 0 (12.20), both scale with c.  Lower edge and width
+                // are truncated separately, so neighbouring bins share their edge to 2^-20 samples (not bit for bit).
+                const int64_t j0s = (int64_t)W.j0 << kFxFrac;
+                const int64_t cov_lo = -j0s >> 8, cov_hi = (((int64_t)(P.n_lambda - 1) << kFxFrac) - j0s) >> 8;   // 2^-20
+                const double cd = (double)W.b * (1.0 / (double)(1u << 30));
+                const int64_t base20 = W.base >> 8;
+                const int64_t last20 = base20 + (__double2ll_rn((double)(P.xtab[min(k_end + 1, P.n_c)] - x_tile0) * cd) >> 8);
+                const bool interior = W.ka == k0 && W.kb == k_end && base20 >= cov_lo + 4 && last20 + 4 <= cov_hi;
+                const uint32_t x0 = (uint32_t)base20;
+                if (interior && P.narrow) {
+#pragma unroll
+                    for (int i = 0; i < CPT; ++i) {
+                        const uint32_t x = x0 + (uint32_t)(((uint64_t)xl[i] * W.b) >> 30);
+                        const float width = (float)(uint32_t)(((uint64_t)wd[i] * W.b) >> 30) * (1.0f / 1048576.0f);
+                        const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
+                        const float a0 = e[0], a1 = e[1], a2r = e[2];
+                        const float fl = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;
+                        const float u = fl + width;
+                        const float u1 = fminf(u, 1.0f), u2 = fmaxf(u - 1.0f, 0.0f);
+                        const float a2 = u > 1.0f ? a2r : a1;     // e[2] may lie beyond the table
+                        const float d1 = a1 - a0, d2 = a2 - a1;
+                        const float il = fl * fmaf(0.5f * fl, d1, a0);
+                        float iu = u1 * fmaf(0.5f * u1, d1, a0);
+                        iu = fmaf(u2, fmaf(0.5f * u2, d2, a1), iu);
+                        acc[i] = fmaf(iu - il, __fdividef(1.0f, width), acc[i]);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < CPT; ++i) {
+                        const int k = k0 + tid + i * kAccThreads;
+                        if (k >= W.ka && k <= W.kb) {
+                            const int64_t lo = base20 + (int64_t)(((uint64_t)xl[i] * W.b) >> 30);
+                            const uint32_t wx = (uint32_t)(((uint64_t)wd[i] * W.b) >> 30);
+                            const int64_t cl = max(lo, cov_lo), ch = min(lo + (int64_t)wx, cov_hi);
+                            if (ch > cl) flux_sample(i, (uint32_t)cl, (uint32_t)ch, 1048576.0f / (float)wx, buf);
+                        }
                     }
                 }
                 return;
@@ -654,6 +699,9 @@ static cudaError_t launch_acc2(const AccumParams &P, unsigned grid, size_t smem,
 template <int CPT>
 static cudaError_t launch_acc(const AccumParams &P, bool flux, bool logx, unsigned grid, size_t smem, cudaStream_t st)
 {
+    if (logx && flux)
+        return P.n_tiles == 1 ? launch_acc2<CPT, true, true, true>(P, grid, smem, st)
+                              : launch_acc2<CPT, false, true, true>(P, grid, smem, st);
     if (logx)
         return P.n_tiles == 1 ? launch_acc2<CPT, true, false, true>(P, grid, smem, st)
                               : launch_acc2<CPT, false, false, true>(P, grid, smem, st);
@@ -721,7 +769,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     int wcap = 0;
     const bool flux = in.tel->resample == RUBIX_RESAMPLE_FLUX;
     const int cpt = choose_cpt(L.n_c, b_max, flux, &wcap, gen ? in.ssp : nullptr, gen ? in.tel : nullptr);
-    const bool narrow = gen && flux && b_max <= 1.0;        // no bin wider than one SSP sample
+    const bool narrow = (gen || logx) && flux && b_max <= 1.0;   // no bin wider than one SSP sample
     if (cpt == 0) return cudaErrorInvalidConfiguration;
     AccumParams P;
     P.flux = (const float *)(ws + L.off_flux);
@@ -738,6 +786,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     P.wcap = wcap;
     P.n_lambda = in.ssp->n_lambda;
     P.skip_empty = skip_empty ? 1 : 0;
+    P.narrow = narrow ? 1 : 0;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.tex = 0;
     P.gen = GenGrid{};
