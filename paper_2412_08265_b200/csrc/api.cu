@@ -275,20 +275,21 @@ static rubix_status forward_device(const rubix_particles *p, const rubix_ssp *ss
                                    int32_t batch = 1, const int64_t *offsets = nullptr)
 {
     PassInputs in{p, ssp, tel, R, batch, offsets};
+    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
+    float *raw = (float *)(ws + L.off_cube_a), *tmp = (float *)(ws + L.off_cube_b);
+    const bool sparse = conv && convolve_fast_path(tel, raw, cube_out, tmp);
+    in.compact_units = sparse;                             // empty spaxels then need no work unit at all
     cudaError_t e;
     {
         StageTimer t(0, st);
         e = launch_particle_pass(in, L, ws, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "particle pass");
-    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
     if (!conv) {
         e = launch_accumulate(in, L, ws, cube_out, false, st);
         if (e != cudaSuccess) return cuda_fail(e, "accumulate");
         return RUBIX_OK;
     }
-    float *raw = (float *)(ws + L.off_cube_a), *tmp = (float *)(ws + L.off_cube_b);
-    const bool sparse = convolve_fast_path(tel, raw, cube_out, tmp);
     e = launch_accumulate(in, L, ws, raw, sparse, st);
     if (e != cudaSuccess) return cuda_fail(e, "accumulate");
     {

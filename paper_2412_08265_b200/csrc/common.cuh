@@ -97,6 +97,8 @@ struct PassInputs {
     // (the same galaxy seen under `batch` rotations).
     int32_t batch = 1;
     const int64_t *offsets = nullptr;      // HOST [batch + 1]
+    // true: empty spaxels get NO work unit (the caller runs k_accumulate with skip_empty: nothing is written for them)
+    bool compact_units = false;
 };
 
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);

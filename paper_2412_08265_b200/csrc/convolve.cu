@@ -82,9 +82,9 @@ struct MarchParams {
     const uint8_t *mask_in;
     uint8_t *mask_out;
     int32_t sp_line, sp_step;
-    // batched cubes: line = element * lines_per_batch + (line inside the element's cube); element b
-    // starts batch_stride floats / sp_batch spaxels after element b - 1; a stencil never crosses into the next cube
-    int32_t lines_per_batch, sp_batch;
+    // batched cubes: gridDim.y = elements; element b starts batch_stride floats / sp_batch spaxels after
+    // element b - 1; n_lines counts the lines of ONE cube, so a stencil never crosses into the next cube
+    int32_t n_batch, sp_batch;
     int64_t batch_stride;
 };
 
@@ -148,8 +148,11 @@ __device__ __forceinline__ void stcs_pred(float *p, float2 v, uint32_t pred)
 //      written and gets mask_out = 0 (else 1);  2  second pass: rows with mask_in == 0 are not read, every output is
 //      written.  A warp works on one line, so every mask decision is warp-uniform.  The mask bytes of the next 15
 //      steps are fetched one iteration ahead (one byte per lane + ballot).
+#ifndef RUBIX_MARCH_MINB2
+#define RUBIX_MARCH_MINB2 4                  // the masked plain pass (second pass of rubix_forward)
+#endif
 template <bool LSF, bool VAR = false, int MASK = 0>
-__global__ void __launch_bounds__(256, VAR ? 2 : (LSF ? RUBIX_MARCH_MINB1 : RUBIX_MARCH_MINB0))
+__global__ void __launch_bounds__(256, VAR ? 2 : (LSF ? RUBIX_MARCH_MINB1 : (MASK == 2 ? RUBIX_MARCH_MINB2 : RUBIX_MARCH_MINB0)))
 k_march(const __grid_constant__ MarchParams P)
 {
     constexpr int kMarchPf = LSF ? RUBIX_MARCH_PF1 : RUBIX_MARCH_PF0;
@@ -160,7 +163,8 @@ k_march(const __grid_constant__ MarchParams P)
     const int c = LSF ? cblock * 56 + 2 * (lane - 2) : cblock * 64 + 2 * lane;
     const bool c_ok = c >= 0 && c + 1 < P.n_c;
     const bool st_ok = c_ok && (!LSF || (lane >= 2 && lane < 30));
-    const int elem = line / P.lines_per_batch, lin = line - elem * P.lines_per_batch;
+    // batched cubes: blockIdx.y = element (no per-thread division: it cost the masked x pass 66 us in registers / spills)
+    const int elem = blockIdx.y, lin = line;
     const size_t off = (size_t)elem * P.batch_stride + (size_t)lin * P.line_stride + (size_t)(c_ok ? c : 0);
     const float *src = P.in + off;
     float *dst = P.out + off;
@@ -289,7 +293,7 @@ static cudaError_t march(MarchParams &P, cudaStream_t st)
 {
     P.cblocks = LSF ? (P.n_c + 55) / 56 : (P.n_c + 63) / 64;
     const int64_t warps = (int64_t)P.n_lines * P.cblocks;
-    k_march<LSF, VAR, MASK><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P);
+    k_march<LSF, VAR, MASK><<<dim3((unsigned)((warps + 7) / 8), (unsigned)P.n_batch), 256, 0, st>>>(P);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }
@@ -343,7 +347,7 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     P.mask_in = nullptr;
     P.mask_out = nullptr;
     P.sp_line = P.sp_step = 0;
-    P.lines_per_batch = 1;
+    P.n_batch = batch;
     P.sp_batch = n_x * n_y;
     P.batch_stride = (int64_t)n_x * n_y * n_c;
     centre_taps(psf, 15, P.g);
@@ -360,13 +364,13 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
     };
     auto along_y = [&](const float *src, float *dst) {     // lines = x
         P.in = src; P.out = dst;
-        P.n_lines = batch * n_x; P.n_steps = n_y; P.lines_per_batch = n_x;
+        P.n_lines = n_x; P.n_steps = n_y;
         P.line_stride = (int64_t)n_y * n_c; P.step_stride = n_c;
         P.sp_line = n_y; P.sp_step = 1;
     };
     auto along_x = [&](const float *src, float *dst) {     // lines = y
         P.in = src; P.out = dst;
-        P.n_lines = batch * n_y; P.n_steps = n_x; P.lines_per_batch = n_y;
+        P.n_lines = n_y; P.n_steps = n_x;
         P.line_stride = n_c; P.step_stride = (int64_t)n_y * n_c;
         P.sp_line = 1; P.sp_step = n_y;
     };

@@ -227,7 +227,8 @@ constexpr int kScanItems = 4;
 constexpr int kScanThreads = 256;
 constexpr int kScanTile = kScanItems * kScanThreads;
 
-__device__ __forceinline__ void unit_counts(const int32_t *__restrict__ seg_off, int32_t n_s, int s0,
+// compact: an empty spaxel gets no unit (else one, which zero-fills its cube row)
+__device__ __forceinline__ void unit_counts(const int32_t *__restrict__ seg_off, int32_t n_s, int s0, int compact,
                                             int32_t (&chunks)[kScanItems], int32_t (&tot)[3])
 {
     tot[0] = tot[1] = tot[2] = 0;
@@ -240,7 +241,7 @@ __device__ __forceinline__ void unit_counts(const int32_t *__restrict__ seg_off,
             const int32_t next = seg_off[s + 1];
             chunks[i] = (next - prev + kChunk - 1) / kChunk;
             prev = next;
-            tot[0] += chunks[i] > 1 ? chunks[i] : 1;
+            tot[0] += chunks[i] > 1 ? chunks[i] : ((compact && chunks[i] == 0) ? 0 : 1);
             tot[1] += chunks[i] > 1 ? chunks[i] : 0;
             tot[2] += chunks[i] > 1 ? 1 : 0;
         }
@@ -267,17 +268,17 @@ __device__ __forceinline__ void block_sum3(int32_t (&v)[3], int32_t (*sm)[kScanT
 }
 
 __global__ void __launch_bounds__(kScanThreads)
-k_unit_tile_totals(const int32_t *__restrict__ seg_off, int32_t n_s, int32_t *__restrict__ tile_tot)
+k_unit_tile_totals(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, int32_t *__restrict__ tile_tot)
 {
     __shared__ int32_t sm[3][kScanThreads / 32];
     int32_t chunks[kScanItems], tot[3];
-    unit_counts(seg_off, n_s, blockIdx.x * kScanTile + threadIdx.x * kScanItems, chunks, tot);
+    unit_counts(seg_off, n_s, blockIdx.x * kScanTile + threadIdx.x * kScanItems, compact, chunks, tot);
     block_sum3(tot, sm);
     if (threadIdx.x < 3) tile_tot[3 * blockIdx.x + threadIdx.x] = tot[threadIdx.x];
 }
 
 __global__ void __launch_bounds__(kScanThreads)
-k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__restrict__ tile_tot,
+k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, const int32_t *__restrict__ tile_tot,
              int32_t *__restrict__ unit_off, int32_t *__restrict__ part_off,
              int32_t *__restrict__ multi_list, int32_t *__restrict__ totals, uint8_t *__restrict__ occ)
 {
@@ -293,7 +294,7 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__
     block_sum3(before, sm);
     const int s0 = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
     int32_t chunks[kScanItems], tot[3], inc[3];
-    unit_counts(seg_off, n_s, s0, chunks, tot);
+    unit_counts(seg_off, n_s, s0, compact, chunks, tot);
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         inc[q] = tot[q];
@@ -319,7 +320,7 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, const int32_t *__
             part_off[s] = run[1];
             occ[s] = chunks[i] > 0 ? 1 : 0;             // occupancy mask of the masked PSF/LSF passes
             if (chunks[i] > 1) multi_list[run[2]] = s;
-            run[0] += chunks[i] > 1 ? chunks[i] : 1;
+            run[0] += chunks[i] > 1 ? chunks[i] : ((compact && chunks[i] == 0) ? 0 : 1);
             run[1] += chunks[i] > 1 ? chunks[i] : 0;
             run[2] += chunks[i] > 1 ? 1 : 0;
         }
@@ -780,9 +781,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     {
         int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
         const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
-        k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot);
+        const int compact = in.compact_units ? 1 : 0;
+        k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot);
         RUBIX_LAUNCH_CHECK();
-        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, tile_tot, unit_off, part_off, multi, totals,
+        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot, unit_off, part_off, multi, totals,
                                                      (uint8_t *)(ws + L.off_occ[0]));
         RUBIX_LAUNCH_CHECK();
     }
