@@ -121,7 +121,7 @@ typedef struct {
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 5
+#define RUBIX_ABI_VERSION 6
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -175,6 +175,17 @@ rubix_status rubix_convolve_psf_lsf(const rubix_telescope *tel, const float *cub
  *   pos, vel  DEVICE [n][3];  key DEVICE [n] int32 (n_x*n_y = dropped);  vlos DEVICE [n] fp32 or NULL */
 rubix_status rubix_bin_particles(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
                                  int32_t *key, float *vlos, void *stream);
+
+/* rubix_build_cube with the halo exchange of a spaxel-sharded run FUSED into the producing kernels (
+ * paper_2412_08265_b200/sharded.py): besides `cube`, the first `mirror_rows` detector rows (x < mirror_rows) are stored at
+ * mirror_lo [mirror_rows][n_y][n_channels] and the last `mirror_rows` rows at mirror_hi, row by row as k_accumulate /
+ * k_reduce_partials produce them.  The mirrors are the halo regions of the neighbouring ranks' buffers: any DEVICE address the
+ * calling GPU can store to -- memory of the same GPU, or PEER memory of another GPU mapped into this process (NVLink stores);
+ * NULL = no mirror on that side.  The neighbour may read its halo once this call's stream has completed (the caller
+ * synchronises across ranks).  Everything else as rubix_build_cube. */
+rubix_status rubix_build_cube_mirrored(const rubix_particles *particles, const rubix_ssp *ssp, const rubix_telescope *tel,
+                                       const float *R, float *cube, float *mirror_lo, float *mirror_hi, int32_t mirror_rows,
+                                       void *workspace, size_t workspace_bytes, void *stream);
 
 /* Steps 1-8 in one call on DEVICE buffers (the whole forward model: rubix_build_cube followed by
  * rubix_convolve_psf_lsf, same arithmetic, same results bit for bit).  The raw cube of step 6 lives in the workspace; with

@@ -19,13 +19,13 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf", "rubix_forward",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
-           "rubix_forward_batched_workspace_bytes", "rubix_forward_batched", "rubix_bin_particles",
+           "rubix_forward_batched_workspace_bytes", "rubix_forward_batched", "rubix_bin_particles", "rubix_build_cube_mirrored",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 5          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 6          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -84,6 +84,9 @@ def load():
         lib.rubix_forward_batched.argtypes = [C.POINTER(CParticles), C.c_void_p, C.c_int32, C.POINTER(CSSP),
                                               C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                               C.c_void_p]
+        lib.rubix_build_cube_mirrored.restype = C.c_int
+        lib.rubix_build_cube_mirrored.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope), C.c_void_p,
+                                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.rubix_bin_particles.restype = C.c_int
         lib.rubix_bin_particles.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(CTelescope), C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p]
@@ -225,6 +228,14 @@ def rubix_forward(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, 
     _check(load().rubix_forward(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
                                 _ptr(workspace), int(workspace.numel() * workspace.element_size()),
                                 _stream(stream)))
+
+
+def rubix_build_cube_mirrored(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, mirror_lo, mirror_hi, mirror_rows, workspace,
+                              stream=None):
+    R = _host_f32(R).reshape(9)
+    _check(load().rubix_build_cube_mirrored(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube), _ptr(mirror_lo),
+                                            _ptr(mirror_hi), int(mirror_rows), _ptr(workspace),
+                                            int(workspace.numel() * workspace.element_size()), _stream(stream)))
 
 
 def rubix_bin_particles(pos, vel, tel: _Keep, R, key, vlos=None, stream=None):

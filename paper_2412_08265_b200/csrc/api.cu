@@ -268,6 +268,38 @@ rubix_status rubix_bin_particles(int64_t n, const float *pos, const float *vel, 
     return RUBIX_OK;
 }
 
+rubix_status rubix_build_cube_mirrored(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,
+                                       const float *R, float *cube, float *mirror_lo, float *mirror_hi, int32_t mirror_rows,
+                                       void *workspace, size_t workspace_bytes, void *stream)
+{
+    t_err[0] = 0;
+    Range nvtx_range("rubix_build_cube_mirrored");
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !cube) return fail(RUBIX_ERR_NULL, "R or cube is NULL");
+    if ((mirror_lo || mirror_hi) && (mirror_rows < 1 || mirror_rows > tel->n_x))
+        return fail(RUBIX_ERR_INVALID_ARG, "mirror_rows must be in [1, n_x] when a mirror is given");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    const Layout L = make_layout(p->n, tel->n_x * tel->n_y, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda);
+    if ((s = check_ws(workspace, workspace_bytes, L.bytes_total)) != RUBIX_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    PassInputs in{p, ssp, tel, R};
+    cudaError_t e;
+    {
+        StageTimer t(0, st);
+        e = launch_particle_pass(in, L, (char *)workspace, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+    const Mirrors m{mirror_lo, mirror_hi, mirror_rows};
+    e = launch_accumulate(in, L, (char *)workspace, cube, false, st, (mirror_lo || mirror_hi) ? &m : nullptr);
+    if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+    remember(workspace, L);
+    return RUBIX_OK;
+}
+
 // Steps 1-8 on device buffers.  With the marching PSF/LSF kernels the raw cube lives in the workspace and only the
 // rows of occupied spaxels are written and read (launch_convolve's masks); otherwise the two plain stages run.
 static rubix_status forward_device(const rubix_particles *p, const rubix_ssp *ssp, const rubix_telescope *tel,

@@ -105,8 +105,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
 cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
                             int32_t *key, float *vlos, cudaStream_t st);
 // skip_empty: rows of spaxels without particles are NOT written (the masked PSF/LSF passes never read them)
+// Mirrors of a spaxel-sharded run: the first / last `rows` detector rows are also stored at lo / hi (nullptr = none)
+struct Mirrors { float *lo, *hi; int32_t rows; };
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
-                              cudaStream_t st);
+                              cudaStream_t st, const Mirrors *mirrors = nullptr);
 // taps_dev: device scratch of psf_taps_bytes(n_channels) for a wavelength-dependent PSF (reading R18), else unused.
 // transpose: apply LSF^T PSF^T (PSF first, then LSF) instead of PSF LSF; only differs when the PSF depends on lambda.
 // occ_in / occ_tmp (both or neither; forward order only): occ_in[s] != 0 marks the spaxel rows of `in` that hold data --

@@ -37,6 +37,10 @@ struct AccumParams {
     int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
     int32_t skip_empty;      // 1: empty spaxels are left unwritten (the masked PSF/LSF passes never read them)
     int32_t narrow;          // bin average in table / general-grid mode: no bin is wider than one SSP sample
+    // Mirrors (spaxel-sharded runs, rubix_build_cube_mirrored): rows of spaxels < mirror_lo_n are ALSO stored at mirror_lo,
+    // rows of spaxels >= mirror_hi_first at mirror_hi -- a neighbour's halo, possibly peer memory of another GPU.
+    float *mirror_lo, *mirror_hi;
+    int32_t mirror_lo_n, mirror_hi_first;
     const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
     cudaTextureObject_t tex;
     GenGrid gen;             // GEN: general-grid mode (gen_coord.cuh)
@@ -490,12 +494,24 @@ k_accumulate(const __grid_constant__ AccumParams P)
             __syncthreads();
         }
     }
+    // (derived here, not before the particle loop: the pointer must not occupy registers while the loop runs)
+    // (a slab of fewer than two halos has rows that go to BOTH neighbours)
+    float *mirror = nullptr, *mirror2 = nullptr;
+    if (U.part_row < 0) {
+        const int sp = P.units[u].spaxel;
+        if (P.mirror_lo && sp < P.mirror_lo_n) mirror = P.mirror_lo + (size_t)sp * P.n_c;
+        if (P.mirror_hi && sp >= P.mirror_hi_first) mirror2 = P.mirror_hi + (size_t)(sp - P.mirror_hi_first) * P.n_c;
+    }
 #pragma unroll
     for (int i = 0; i < CPT; ++i) {
         const int k = k0 + tid + i * kAccThreads;
         if (k <= k_end) {
             if (U.part_row >= 0) out[k] = acc[i];
-            else __stcs(out + k, acc[i]);                   // cube is written once, streamed
+            else {
+                __stcs(out + k, acc[i]);                    // cube is written once, streamed
+                if (mirror) mirror[k] = acc[i];             // ... and once more into the neighbour's halo, as it is produced
+                if (mirror2) mirror2[k] = acc[i];
+            }
         }
     }
 }
@@ -660,7 +676,8 @@ k_accumulate_async(const __grid_constant__ AccumParams P)
 __global__ void __launch_bounds__(256)
 k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict__ seg_off,
                   const int32_t *__restrict__ part_off, const int32_t *__restrict__ multi_list,
-                  const int32_t *__restrict__ totals, int32_t n_c, float *__restrict__ cube)
+                  const int32_t *__restrict__ totals, int32_t n_c, float *__restrict__ cube, float *mirror_lo,
+                  float *mirror_hi, int32_t mirror_lo_n, int32_t mirror_hi_first)
 {
     for (int m = blockIdx.x; m < totals[2]; m += gridDim.x) {
     const int s = multi_list[m];
@@ -681,6 +698,8 @@ k_reduce_partials(const float *__restrict__ partials, const int32_t *__restrict_
         }
         for (; c < chunks; ++c) a += (double)__ldcs(col + (size_t)c * n_c);
         __stcs(cube + (size_t)s * n_c + k, (float)a);
+        if (mirror_lo && s < mirror_lo_n) mirror_lo[(size_t)s * n_c + k] = (float)a;
+        if (mirror_hi && s >= mirror_hi_first) mirror_hi[(size_t)(s - mirror_hi_first) * n_c + k] = (float)a;
     }
     }
 }
@@ -760,7 +779,7 @@ int choose_cpt(int n_c, double b_max, bool flux, int *wcap_out, const rubix_ssp 
 }
 
 cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, float *cube, bool skip_empty,
-                              cudaStream_t st)
+                              cudaStream_t st, const Mirrors *mirrors)
 {
     const bool logx = table_mode(in.ssp, in.tel), gen = gen_mode(in.ssp, in.tel);
     const double b0 = (double)in.tel->dlambda / (double)in.ssp->dlambda;
@@ -787,6 +806,10 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     P.n_lambda = in.ssp->n_lambda;
     P.skip_empty = skip_empty ? 1 : 0;
     P.narrow = narrow ? 1 : 0;
+    P.mirror_lo = mirrors ? mirrors->lo : nullptr;
+    P.mirror_hi = mirrors ? mirrors->hi : nullptr;
+    P.mirror_lo_n = mirrors ? mirrors->rows * in.tel->n_y : 0;
+    P.mirror_hi_first = mirrors ? (in.tel->n_x - mirrors->rows) * in.tel->n_y : 0;
     P.xtab = (const int64_t *)(ws + L.off_xtab);
     P.tex = 0;
     P.gen = GenGrid{};
@@ -852,7 +875,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     const unsigned gx = (unsigned)(L.max_multi < 1184 ? L.max_multi : 1184);   // grid-stride over the multi-chunk spaxels
     k_reduce_partials<<<dim3(gx, gy), 256, 0, st>>>(
         P.partials, (const int32_t *)(ws + L.off_seg), (const int32_t *)(ws + L.off_partoff),
-        (const int32_t *)(ws + L.off_multi), P.totals, L.n_c, cube);
+        (const int32_t *)(ws + L.off_multi), P.totals, L.n_c, cube, P.mirror_lo, P.mirror_hi, P.mirror_lo_n, P.mirror_hi_first);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }

@@ -11,7 +11,9 @@ whole spaxels locally and the cube is never exchanged -- only 36-byte particle r
   4  all-to-all of the particle records, source order kept: ranks hold contiguous slices of the original arrays, so a
      rank receives its particles in ORIGINAL order and the stable (key, index) order of step 3 is the single-GPU one
   5  rubix_build_cube on the rank's row window (rubix_telescope.n_x_full / x_first) into a buffer with room for the halos
-  6  halo exchange of raw rows with the neighbouring ranks
+  6  halo exchange of raw rows with the neighbouring ranks -- or, where a rank can store into its neighbours' buffers
+     (ranks of one process; peer-mapped memory), steps 5 + 6 FUSED: rubix_build_cube_mirrored lets the kernels that produce
+     the boundary rows write them into the neighbours' halos as well, and the exchange shrinks to a barrier
   7  rubix_convolve_psf_lsf on rows + halos; the rank keeps its own rows of the final cube
 Every spaxel is summed by one rank over the same particles in the same order and chunks as on one GPU, and the stencils see
 the same neighbours, so the slabs equal the single-GPU cube bit for bit.
@@ -83,6 +85,14 @@ class DistComm:
         self.dist.all_gather(out, t)
         return out
 
+    def share(self, obj):
+        """Ranks are separate processes: no rank can store into another rank's buffer through this communicator (peer
+        pointers would need CUDA IPC handles), so the halo goes through `exchange`."""
+        return None
+
+    def barrier(self):
+        self.dist.barrier()
+
     def exchange(self, sends: dict, recv_shapes: dict, like):
         """sends: {peer: tensor}; recv_shapes: {peer: shape}.  Returns {peer: tensor}."""
         import torch
@@ -125,6 +135,14 @@ class ThreadComm:
 
     def all_gather_counts(self, t):
         return [v.clone() for v in self._gather("cnt", t.clone())]
+
+    def share(self, obj):
+        """The ranks live in one address space: every rank gets every rank's object (here: its raw-row buffer), so a
+        rank's kernels can store straight into a neighbour's halo."""
+        return self._gather("share", obj)
+
+    def barrier(self):
+        self._gather("bar", None)
 
     def exchange(self, sends: dict, recv_shapes: dict, like):
         import torch
@@ -177,14 +195,18 @@ class CudaBackend:
         B.rubix_bin_particles(pos, vel, B.c_telescope(tel), R, key)
         return key
 
-    def build_rows(self, records, R, ssp, flux_dev, tel, x0, x1, out):
-        """Raw cube rows x0 .. x1 - 1 of the whole detector ``tel`` from ``records`` into ``out`` [x1 - x0, n_y, n_c]."""
+    def build_rows(self, records, R, ssp, flux_dev, tel, x0, x1, out, mirror_lo=None, mirror_hi=None, mirror_rows=0):
+        """Raw cube rows x0 .. x1 - 1 of the whole detector ``tel`` from ``records`` into ``out`` [x1 - x0, n_y, n_c]; with
+        mirrors, the first / last ``mirror_rows`` rows are also stored there by the producing kernels (the fused halo write)."""
         B, torch = self.B, self.torch
         sub = dataclasses.replace(tel, n_x=int(x1 - x0), n_x_full=int(tel.n_x), x_first=int(x0))
         cols = [records[:, 0:3].contiguous(), records[:, 3:6].contiguous()] + [records[:, c].contiguous() for c in (6, 7, 8)]
         cp, cs, ct = B.c_particles(*cols), B.c_ssp(ssp, flux_dev), B.c_telescope(sub)
         ws = torch.empty(B.rubix_workspace_bytes(records.shape[0], cs, ct), dtype=torch.uint8, device=self.device)
-        B.rubix_build_cube(cp, cs, ct, R, out, ws)
+        if mirror_lo is not None or mirror_hi is not None:
+            B.rubix_build_cube_mirrored(cp, cs, ct, R, out, mirror_lo, mirror_hi, mirror_rows, ws)
+        else:
+            B.rubix_build_cube(cp, cs, ct, R, out, ws)
         return ws                                           # kept alive by the caller until the stream has run
 
     def convolve_rows(self, rows, tel):
@@ -218,9 +240,10 @@ class Slab:
     n_received: int
 
 
-def forward_sharded(comm, backend, records, R, ssp, tel, flux_dev=None, row_cost=None) -> Slab:
+def forward_sharded(comm, backend, records, R, ssp, tel, flux_dev=None, row_cost=None, fuse_halo=True) -> Slab:
     """SPMD: every rank calls this with ITS slice of the particle records (contiguous slices of the original arrays in rank
-    order).  Returns the rank's slab of the final cube.  ``tel`` is the whole detector."""
+    order).  Returns the rank's slab of the final cube.  ``tel`` is the whole detector.  ``fuse_halo``: use the fused halo write
+    (rubix_build_cube_mirrored) where the communicator lets ranks store into each other's buffers."""
     import torch
     n_x, n_y, n_c = int(tel.n_x), int(tel.n_y), int(tel.n_channels)
     rank, world = comm.rank, comm.world
@@ -250,15 +273,34 @@ def forward_sharded(comm, backend, records, R, ssp, tel, flux_dev=None, row_cost
     buf = torch.zeros((h_lo + n_own + h_hi, n_y, n_c), dtype=getattr(backend, "dtype", torch.float32), device=records.device)
     if flux_dev is None:
         flux_dev = backend.upload_flux(ssp)
-    keep = backend.build_rows(mine, R, ssp, flux_dev, tel, x0, x1, buf[h_lo:h_lo + n_own])
     conv = int(tel.psf_size) > 0 or int(tel.lsf_size) > 0
+    # 5 + 6 fused where the ranks can store into each other's buffers (one address space / mapped peer memory): the kernels
+    # that produce my boundary rows also write them into the neighbours' halos, and the exchange shrinks to a barrier
+    peers = None
+    if fuse_halo and conv and halo > 0 and world > 1:
+        if records.is_cuda:
+            torch.cuda.current_stream().synchronize()      # my buffer is zero-filled before a neighbour may store into it
+        peers = comm.share(buf)
+    if peers is not None:
+        lo_peer = hi_peer = None
+        if rank > 0:                                        # my first rows are the UPPER halo of rank - 1
+            b_lo = peers[rank - 1]
+            lo_peer = b_lo[b_lo.shape[0] - halo:]
+        if rank < world - 1:                                # my last rows are the LOWER halo of rank + 1
+            hi_peer = peers[rank + 1][0:halo]
+        keep = backend.build_rows(mine, R, ssp, flux_dev, tel, x0, x1, buf[h_lo:h_lo + n_own], lo_peer, hi_peer, halo)
+        if records.is_cuda:
+            torch.cuda.current_stream().synchronize()
+        comm.barrier()                                      # every rank's rows (and mirrors) are complete
+    else:
+        keep = backend.build_rows(mine, R, ssp, flux_dev, tel, x0, x1, buf[h_lo:h_lo + n_own])
     if not conv:
         if records.is_cuda:
             torch.cuda.current_stream().synchronize()
         del keep
         return Slab(x0, x1, buf, bounds, int(mine.shape[0]))
     # 6  halo exchange: my first / last `halo` rows are the neighbours' upper / lower halo
-    if halo > 0 and world > 1:
+    if peers is None and halo > 0 and world > 1:
         if records.is_cuda:
             torch.cuda.current_stream().synchronize()      # the rows must be complete before a peer reads them
         sends, recvs = {}, {}

@@ -26,12 +26,16 @@ class OracleBackend:
     def upload_flux(self, ssp):
         return None
 
-    def build_rows(self, records, R, ssp, flux_dev, tel, x0, x1, out):
+    def build_rows(self, records, R, ssp, flux_dev, tel, x0, x1, out, mirror_lo=None, mirror_hi=None, mirror_rows=0):
         n_y, n_c = tel.n_y, tel.n_channels
         sel = np.arange(x0 * n_y, x1 * n_y, dtype=np.int32)
         if sel.size:
             cube = oracle.build_cube(particles_of(records), R, ssp, tel, sel=sel)
             out.copy_(torch.from_numpy(cube.reshape(x1 - x0, n_y, n_c)))
+        if mirror_lo is not None:                              # the fused halo write of rubix_build_cube_mirrored
+            mirror_lo.copy_(out[:mirror_rows])
+        if mirror_hi is not None:
+            mirror_hi.copy_(out[out.shape[0] - mirror_rows:])
         return None
 
     def convolve_rows(self, rows, tel):

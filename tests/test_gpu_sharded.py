@@ -43,8 +43,34 @@ def test_bin_particles_and_row_window(B):
         B.DeviceWorkload(bad).build_cube()
 
 
+def test_mirrored_build_writes_the_boundary_rows_twice(B):
+    """rubix_build_cube_mirrored: the cube equals rubix_build_cube's, and the first / last rows also land in the mirrors
+    (single- and multi-chunk spaxels: direct stores of k_accumulate and the sums of k_reduce_partials)."""
+    w = synth.make_workload("small", n=60000)
+    w.particles.pos[:4000, :2] *= np.float32(0.02)                       # a pile-up in the centre and ...
+    w.particles.pos[4000:8000, 0] = np.float32(-14.5)                    # ... one in the first detector row (multi-chunk there)
+    t = w.telescope
+    dw = B.DeviceWorkload(w)
+    plain = dw.build_cube()
+    for rows in (1, 7, t.n_x):
+        cube = torch.full(dw.shape, float("nan"), device="cuda")
+        lo = torch.full((rows, t.n_y, t.n_channels), float("nan"), device="cuda")
+        hi = torch.full((rows, t.n_y, t.n_channels), float("nan"), device="cuda")
+        B.rubix_build_cube_mirrored(dw.particles, dw.ssp, dw.tel, dw.R, cube, lo, hi, rows, dw.workspace)
+        torch.cuda.synchronize()
+        assert torch.equal(cube, plain) and torch.equal(lo, plain[:rows]) and torch.equal(hi, plain[t.n_x - rows:])
+    cube = torch.full(dw.shape, float("nan"), device="cuda")
+    hi = torch.full((3, t.n_y, t.n_channels), float("nan"), device="cuda")
+    B.rubix_build_cube_mirrored(dw.particles, dw.ssp, dw.tel, dw.R, cube, None, hi, 3, dw.workspace)
+    torch.cuda.synchronize()
+    assert torch.equal(cube, plain) and torch.equal(hi, plain[t.n_x - 3:])
+    with pytest.raises(B.RubixError):
+        B.rubix_build_cube_mirrored(dw.particles, dw.ssp, dw.tel, dw.R, cube, None, hi, 0, dw.workspace)
+
+
+@pytest.mark.parametrize("fuse_halo", [True, False])
 @pytest.mark.parametrize("name,world,psf_size", [("tiny", 2, 15), ("tiny", 4, 7), ("small", 3, 15), ("small", 5, 9), ("tiny", 3, 0)])
-def test_sharded_slabs_equal_the_single_gpu_cube(B, name, world, psf_size):
+def test_sharded_slabs_equal_the_single_gpu_cube(B, name, world, psf_size, fuse_halo):
     w = synth.make_workload(name, n=None if name == "tiny" else 40000)
     if psf_size:
         w.telescope = w.telescope.with_psf_lsf(psf_size=psf_size)
@@ -56,7 +82,7 @@ def test_sharded_slabs_equal_the_single_gpu_cube(B, name, world, psf_size):
     def rank_fn(comm):
         sl = sharded.slice_for_rank(p.n, comm.rank, comm.world)
         rec = sharded.pack_records(p.subset(np.arange(p.n)[sl]), "cuda")
-        return sharded.forward_sharded(comm, backend, rec, w.rotation, w.ssp, t)
+        return sharded.forward_sharded(comm, backend, rec, w.rotation, w.ssp, t, fuse_halo=fuse_halo)
 
     slabs = sharded.run_threads(world, rank_fn)
     assert slabs[0].x0 == 0 and slabs[-1].x1 == t.n_x

@@ -25,11 +25,11 @@ def workload(n=900, psf=True):
     return w
 
 
-def run_rank(comm, w):
+def run_rank(comm, w, fuse_halo=True):
     p = w.particles
     sl = sharded.slice_for_rank(p.n, comm.rank, comm.world)
     rec = sharded.pack_records(p.subset(np.arange(p.n)[sl]), "cpu")
-    return sharded.forward_sharded(comm, OracleBackend(), rec, w.rotation, w.ssp, w.telescope)
+    return sharded.forward_sharded(comm, OracleBackend(), rec, w.rotation, w.ssp, w.telescope, fuse_halo=fuse_halo)
 
 
 def check_slabs(slabs, w):
@@ -78,11 +78,14 @@ def test_owner_of_rows():
 # ------------------------------------------------------------------------------------------ ranks as threads
 @pytest.mark.parametrize("world", [1, 2, 3, 5])
 @pytest.mark.parametrize("psf", [True, False])
-def test_thread_ranks_reproduce_the_single_rank_cube(world, psf):
+@pytest.mark.parametrize("fuse_halo", [True, False])
+def test_thread_ranks_reproduce_the_single_rank_cube(world, psf, fuse_halo):
+    """fuse_halo: the boundary rows reach the neighbours through mirror stores of the build (thread ranks share an address
+    space) or through the explicit halo exchange (what separate processes do)."""
     w = workload(psf=psf)
     if psf and world == 5:
         w.telescope = dataclasses.replace(w.telescope, psf_size=5)           # 16 rows / 5 ranks: halo of 2 rows
-    slabs = sharded.run_threads(world, lambda comm: run_rank(comm, w))
+    slabs = sharded.run_threads(world, lambda comm: run_rank(comm, w, fuse_halo))
     check_slabs(slabs, w)
 
 
