@@ -193,3 +193,42 @@ def test_no_cpu_fallback_without_the_library(monkeypatch):
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/librubix_b200.so")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         B.load()
+
+
+def test_batched_sharded_and_mirrored_entries_validate_on_the_host(lib):
+    """rubix_forward_batched / rubix_bin_particles / rubix_build_cube_mirrored / the row window: bad arguments are refused
+    before any launch (fake device addresses, no GPU needed)."""
+    ssp, tel = _structs(tel=synth.make_telescope("tiny"))
+    P = _fake_particles(100)
+    R = np.tile(np.eye(3, dtype=np.float32).reshape(1, 9), (3, 1))
+
+    def batched(offsets, batch, ws_bytes=1 << 40):
+        off = None if offsets is None else np.asarray(offsets, np.int64)
+        return lib.rubix_forward_batched(P.ref(), None if off is None else off.ctypes.data, batch, ssp.ref(), tel.ref(),
+                                         R.ctypes.data, FAKE + (1 << 41), FAKE, ws_bytes, None)
+
+    assert batched(None, 0) == B.RUBIX_ERR_INVALID_ARG and "batch" in B.rubix_last_error()
+    assert batched([0, 50, 40, 100], 3) == B.RUBIX_ERR_INVALID_ARG and "non-decreasing" in B.rubix_last_error()
+    assert batched([0, 50, 60, 99], 3) == B.RUBIX_ERR_INVALID_ARG
+    assert batched([1, 50, 60, 100], 3) == B.RUBIX_ERR_INVALID_ARG
+    assert batched([0, 50, 60, 100], 3, ws_bytes=1024) == B.RUBIX_ERR_WORKSPACE
+    assert lib.rubix_forward_batched_workspace_bytes(100, None, 3, ssp.ref(), tel.ref()) > \
+        lib.rubix_forward_batched_workspace_bytes(100, None, 1, ssp.ref(), tel.ref()) > 0
+    assert lib.rubix_forward_batched_workspace_bytes(100, None, 0, ssp.ref(), tel.ref()) == 0
+    # row window of a sharded run
+    for n_x, n_full, first, ok in ((4, 16, 12, True), (4, 16, 13, False), (4, 0, 2, False), (4, 16, -1, False)):
+        _, t2 = _structs(tel=synth.make_telescope("tiny"))
+        t2.struct.n_x, t2.struct.n_x_full, t2.struct.x_first = n_x, n_full, first
+        st = lib.rubix_workspace_bytes(10, ssp.ref(), t2.ref())
+        assert (st > 0) == ok, (n_x, n_full, first)
+    assert lib.rubix_bin_particles(10, None, FAKE, tel.ref(), R.ctypes.data, FAKE, None, None) == B.RUBIX_ERR_NULL
+    assert lib.rubix_bin_particles(-1, FAKE, FAKE, tel.ref(), R.ctypes.data, FAKE, None, None) == B.RUBIX_ERR_INVALID_ARG
+    assert lib.rubix_build_cube_mirrored(P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, FAKE + (1 << 41), FAKE + (1 << 42), None, 0,
+                                         FAKE, 1 << 40, None) == B.RUBIX_ERR_INVALID_ARG
+    assert lib.rubix_build_cube_mirrored(P.ref(), ssp.ref(), tel.ref(), R.ctypes.data, FAKE + (1 << 41), None, FAKE + (1 << 42), 17,
+                                         FAKE, 1 << 40, None) == B.RUBIX_ERR_INVALID_ARG
+    # listed SSP wavelengths: validated on the host like the axes
+    base = synth.make_ssp(8, 4, 64, 3500.0, 9500.0, 1, irregular=True)
+    bad = synth.SSPGrid(base.log_age_axis, base.log_z_axis, base.lambda0, base.dlambda, base.flux, 0, base.lambda_grid[::-1].copy())
+    s_bad, _ = _structs(ssp=bad)
+    assert _call_build(lib, P, s_bad, tel) == B.RUBIX_ERR_INVALID_ARG and "lambda_grid" in B.rubix_last_error()
