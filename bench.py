@@ -331,6 +331,46 @@ def time_batched(B, synth, dev, reps=20):
         res["graph_replay_cubes_per_s"] = 64 / e0.elapsed_time(e1) * 1e3
         res["speedup_over_graph_replay_at_B=64"] = res["B=64"]["batched_cubes_per_s"] / res["graph_replay_cubes_per_s"]
         out[name] = res
+    # the fused forward + loss + adjoint for 64 concatenated galaxies (rubix_loss_and_grad_batched) against 64 looped calls
+    w = synth.make_workload("tiny")
+    dw = B.DeviceWorkload(w, device=dev)
+    batch, n = 64, w.particles.n
+    rep = lambda a: a.repeat(batch, *([1] * (a.dim() - 1))).contiguous()
+    arrays = [rep(getattr(dw, f)) for f in ("pos", "vel", "mass", "log_age", "log_z")]
+    cp = B.c_particles(*arrays)
+    offsets = np.arange(batch + 1, dtype=np.int64) * n
+    R = np.stack([synth.euler_rotation(*synth.random_euler(7000 + b)) for b in range(batch)]).astype(np.float32)
+    targets = torch.zeros((batch,) + dw.shape, dtype=torch.float32, device=dev)
+    loss = torch.zeros(batch, dtype=torch.float64, device=dev)
+    g = [torch.empty(batch * n, dtype=torch.float32, device=dev) for _ in range(4)]
+    ws = torch.empty(B.rubix_loss_and_grad_batched_workspace_bytes(batch * n, offsets, batch, dw.ssp, dw.tel),
+                     dtype=torch.uint8, device=dev)
+    g1 = [torch.empty(n, dtype=torch.float32, device=dev) for _ in range(4)]
+    ws1 = torch.empty(B.rubix_loss_and_grad_workspace_bytes(n, dw.ssp, dw.tel), dtype=torch.uint8, device=dev)
+
+    def lg_batched():
+        B.rubix_loss_and_grad_batched(cp, offsets, batch, dw.ssp, dw.tel, R, targets, loss, None, *g, ws)
+
+    def lg_looped():
+        for b in range(batch):
+            B.rubix_loss_and_grad(dw.particles, dw.ssp, dw.tel, R[b], targets[b], loss[b:b + 1], None, *g1, ws1)
+
+    def timed2(fn, k):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(k):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / k
+
+    ms_b, ms_l = timed2(lg_batched, reps), timed2(lg_looped, max(reps // 4, 2))
+    out["loss_and_grad_tiny_B=64"] = {"batched_ms": ms_b, "batched_galaxies_per_s": batch / ms_b * 1e3, "looped_ms": ms_l,
+                                      "looped_galaxies_per_s": batch / ms_l * 1e3, "speedup_over_loop": ms_l / ms_b,
+                                      "what": "rubix_loss_and_grad_batched, 64 copies of configs[0] under 64 rotations, zero targets"}
     out["what"] = ("rubix_forward_batched (one launch sequence for B cubes) vs B looped rubix_forward calls vs replays of a CUDA "
                    "graph of one rubix_forward; BASELINE.json configs[0] (tiny) and configs[1] (small), one galaxy under B rotations")
     return out

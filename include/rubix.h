@@ -121,7 +121,7 @@ typedef struct {
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 6
+#define RUBIX_ABI_VERSION 7
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -250,6 +250,23 @@ rubix_status rubix_loss_and_grad(const rubix_particles *particles, const rubix_s
                                  double *loss, float *cube_out, float *g_mass, float *g_log_age,
                                  float *g_log_z, float *g_vlos, void *workspace, size_t workspace_bytes,
                                  void *stream);
+
+/* rubix_loss_and_grad for `batch` concatenated galaxies per call ("gradient based
+ * optimization", L32): one launch sequence per group of 64 elements runs steps 1-8, the per-element losses
+ *     loss[b] = sum over the voxels of element b of (final cube_b - target_b)^2
+ * and step 9 for every particle, with one particle pass shared by forward and adjoint.  Element b gets the cube, the loss (when
+ * n_x n_y n_channels is a multiple of 4: bit-equal; else equal to rounding of the fp64 sum) and the gradients of a single
+ * rubix_loss_and_grad call on that galaxy.
+ *   offsets    HOST [batch+1], required (the same-galaxy mode of rubix_forward_batched has no gradient counterpart)
+ *   targets    DEVICE [batch][n_x][n_y][n_channels];  loss DEVICE [batch] doubles;  cubes_out DEVICE like targets, or NULL
+ *   g_*        DEVICE [particles->n] in the order of the concatenated arrays
+ * When cubes_out is NULL and PSF / LSF are on, the final cubes live in the workspace only. */
+size_t rubix_loss_and_grad_batched_workspace_bytes(int64_t n, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                                   const rubix_telescope *tel);
+rubix_status rubix_loss_and_grad_batched(const rubix_particles *particles, const int64_t *offsets, int32_t batch,
+                                         const rubix_ssp *ssp, const rubix_telescope *tel, const float *R, const float *targets,
+                                         double *loss, float *cubes_out, float *g_mass, float *g_log_age, float *g_log_z,
+                                         float *g_vlos, void *workspace, size_t workspace_bytes, void *stream);
 
 /* Noise stage ("add realistic noise"; the paper names no model -- DESIGN.md reading R17):
  *     cube_out[v] = cube_in[v] + sqrt(sigma_read^2 + gain * max(cube_in[v], 0)) * n_v ,   n_v ~ N(0, 1)

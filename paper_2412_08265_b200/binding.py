@@ -20,12 +20,13 @@ RUBIX_OK, RUBIX_ERR_NULL, RUBIX_ERR_INVALID_ARG, RUBIX_ERR_UNSUPPORTED, RUBIX_ER
 EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf", "rubix_forward",
            "rubix_cube_adjoint", "rubix_get_sort_artifacts", "rubix_forward_host_scratch_bytes",
            "rubix_forward_batched_workspace_bytes", "rubix_forward_batched", "rubix_bin_particles", "rubix_build_cube_mirrored",
+           "rubix_loss_and_grad_batched_workspace_bytes", "rubix_loss_and_grad_batched",
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 6          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 7          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -84,6 +85,11 @@ def load():
         lib.rubix_forward_batched.argtypes = [C.POINTER(CParticles), C.c_void_p, C.c_int32, C.POINTER(CSSP),
                                               C.POINTER(CTelescope), C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                               C.c_void_p]
+        lib.rubix_loss_and_grad_batched_workspace_bytes.restype = C.c_size_t
+        lib.rubix_loss_and_grad_batched_workspace_bytes.argtypes = lib.rubix_forward_batched_workspace_bytes.argtypes
+        lib.rubix_loss_and_grad_batched.restype = C.c_int
+        lib.rubix_loss_and_grad_batched.argtypes = [C.POINTER(CParticles), C.c_void_p, C.c_int32, C.POINTER(CSSP),
+                                                    C.POINTER(CTelescope)] + [C.c_void_p] * 9 + [C.c_size_t, C.c_void_p]
         lib.rubix_build_cube_mirrored.restype = C.c_int
         lib.rubix_build_cube_mirrored.argtypes = [C.POINTER(CParticles), C.POINTER(CSSP), C.POINTER(CTelescope), C.c_void_p,
                                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -228,6 +234,26 @@ def rubix_forward(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, workspace, 
     _check(load().rubix_forward(particles.ref(), ssp.ref(), tel.ref(), R.ctypes.data, _ptr(cube),
                                 _ptr(workspace), int(workspace.numel() * workspace.element_size()),
                                 _stream(stream)))
+
+
+def rubix_loss_and_grad_batched_workspace_bytes(n, offsets, batch, ssp: _Keep, tel: _Keep) -> int:
+    off = _offsets(offsets)
+    b = int(load().rubix_loss_and_grad_batched_workspace_bytes(int(n), _ptr(off), int(batch), ssp.ref(), tel.ref()))
+    if b == 0:
+        raise RubixError(RUBIX_ERR_INVALID_ARG, rubix_last_error())
+    return b
+
+
+def rubix_loss_and_grad_batched(particles: _Keep, offsets, batch, ssp: _Keep, tel: _Keep, R, targets, loss, cubes_out, g_mass,
+                                g_log_age, g_log_z, g_vlos, workspace, stream=None):
+    """``loss``: float64 device tensor [batch]; ``cubes_out``: device tensor [batch, n_x, n_y, n_channels] or None."""
+    off = _offsets(offsets)
+    R = _host_f32(R).reshape(-1)
+    assert R.size == 9 * int(batch)
+    _check(load().rubix_loss_and_grad_batched(particles.ref(), _ptr(off), int(batch), ssp.ref(), tel.ref(), R.ctypes.data,
+                                              _ptr(targets), _ptr(loss), _ptr(cubes_out), _ptr(g_mass), _ptr(g_log_age),
+                                              _ptr(g_log_z), _ptr(g_vlos), _ptr(workspace),
+                                              int(workspace.numel() * workspace.element_size()), _stream(stream)))
 
 
 def rubix_build_cube_mirrored(particles: _Keep, ssp: _Keep, tel: _Keep, R, cube, mirror_lo, mirror_hi, mirror_rows, workspace,

@@ -613,6 +613,113 @@ rubix_status rubix_loss_and_grad(const rubix_particles *p, const rubix_ssp *ssp,
     return RUBIX_OK;
 }
 
+size_t rubix_loss_and_grad_batched_workspace_bytes(int64_t n, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                                   const rubix_telescope *tel)
+{
+    const size_t base = rubix_forward_batched_workspace_bytes(n, offsets, batch, ssp, tel);
+    if (base == 0) return 0;
+    if (!offsets) { fail(RUBIX_ERR_INVALID_ARG, "rubix_loss_and_grad_batched needs offsets (concatenated galaxies)"); return 0; }
+    const int32_t bg = batch < kMaxBatch ? batch : kMaxBatch;
+    const size_t cube_bytes = (size_t)bg * tel->n_x * tel->n_y * tel->n_channels * 4;
+    return base + align_up(cube_bytes, 256) + loss_scratch_bytes(bg);
+}
+
+rubix_status rubix_loss_and_grad_batched(const rubix_particles *p, const int64_t *offsets, int32_t batch, const rubix_ssp *ssp,
+                                         const rubix_telescope *tel, const float *R, const float *targets, double *loss,
+                                         float *cubes_out, float *g_mass, float *g_log_age, float *g_log_z, float *g_vlos,
+                                         void *workspace, size_t workspace_bytes, void *stream)
+{
+    t_err[0] = 0;
+    Range nvtx_range("rubix_loss_and_grad_batched");
+    g_launches = 0;
+    rubix_status s;
+    if ((s = check_particles(p)) != RUBIX_OK) return s;
+    if ((s = check_ssp(ssp, true)) != RUBIX_OK) return s;
+    if ((s = check_tel(tel)) != RUBIX_OK) return s;
+    if (!R || !targets || !loss) return fail(RUBIX_ERR_NULL, "R, targets or loss is NULL");
+    if (!offsets) return fail(RUBIX_ERR_INVALID_ARG, "rubix_loss_and_grad_batched needs offsets (concatenated galaxies)");
+    if (p->n > 0 && (!g_mass || !g_log_age || !g_log_z || !g_vlos))
+        return fail(RUBIX_ERR_NULL, "a gradient output is NULL");
+    if ((s = check_resampler(ssp, tel)) != RUBIX_OK) return s;
+    if ((s = check_batch(p, offsets, batch, tel)) != RUBIX_OK) return s;
+    int64_t n_max; int32_t b_max;
+    batch_groups(p->n, batch, offsets, &n_max, &b_max);
+    const int32_t n_s = tel->n_x * tel->n_y;
+    const Layout Lmax = make_layout(n_max, b_max * n_s, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda);
+    const int64_t n_vox = (int64_t)n_s * tel->n_channels;
+    const size_t cube_al = align_up((size_t)b_max * n_vox * 4, 256);
+    if ((s = check_ws(workspace, workspace_bytes, Lmax.bytes_total + cube_al + loss_scratch_bytes(b_max))) != RUBIX_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    const bool conv = tel->psf_size > 0 || tel->lsf_size > 0;
+    int launches = 0;
+    for (int32_t g0 = 0; g0 < batch; g0 += kMaxBatch) {       // groups of <= kMaxBatch elements, one launch sequence each
+        const int32_t bg = g0 + kMaxBatch < batch ? kMaxBatch : batch - g0;
+        const int64_t first = offsets[g0];
+        rubix_particles pg = *p;
+        pg.n = offsets[g0 + bg] - first;
+        pg.pos = p->pos ? p->pos + 3 * first : nullptr;
+        pg.vel = p->vel ? p->vel + 3 * first : nullptr;
+        pg.mass = p->mass ? p->mass + first : nullptr;
+        pg.log_age = p->log_age ? p->log_age + first : nullptr;
+        pg.log_z = p->log_z ? p->log_z + first : nullptr;
+        int64_t off_local[kMaxBatch + 1];
+        for (int32_t b = 0; b <= bg; ++b) off_local[b] = offsets[g0 + b] - first;
+        const Layout L = make_layout(pg.n, bg * n_s, tel->n_channels, ssp->n_age * ssp->n_z, ssp->n_lambda);
+        float *buf_a = (float *)(ws + L.off_cube_a), *buf_b = (float *)(ws + L.off_cube_b);
+        float *buf_c = (float *)(ws + Lmax.bytes_total);
+        double *partial = (double *)(ws + Lmax.bytes_total + cube_al);
+        PassInputs in{&pg, ssp, tel, R + 9 * (size_t)g0, bg, off_local};
+        const float *target = targets + (size_t)g0 * n_vox;
+        float *cube_g = cubes_out ? cubes_out + (size_t)g0 * n_vox : nullptr;
+        float *raw = conv ? buf_a : (cube_g ? cube_g : buf_a);
+        float *fin = cube_g ? cube_g : buf_c;
+        const bool sparse = conv && convolve_fast_path(tel, raw, fin, buf_b);
+        in.compact_units = false;                          // the adjoint kernels walk the same units
+        cudaError_t e;
+        {
+            StageTimer t(0, st);
+            e = launch_particle_pass(in, L, ws, st);       // ONE particle pass serves forward and adjoint of every element
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "particle pass");
+        e = launch_accumulate(in, L, ws, raw, sparse, st);
+        if (e != cudaSuccess) return cuda_fail(e, "accumulate");
+        const float *final_cube = raw;
+        if (conv) {
+            {
+                StageTimer t(3, st);
+                e = launch_convolve(tel, raw, fin, buf_b, (float *)(ws + L.off_psftaps), false,
+                                    sparse ? (const uint8_t *)(ws + L.off_occ[0]) : nullptr,
+                                    sparse ? (uint8_t *)(ws + L.off_occ[1]) : nullptr, st, bg);
+            }
+            if (e != cudaSuccess) return cuda_fail(e, "convolve");
+            final_cube = fin;
+        }
+        float *grad = conv ? buf_a : buf_b;
+        e = launch_residual_loss(final_cube, target, n_vox, grad, partial, loss + g0, st, bg);
+        if (e != cudaSuccess) return cuda_fail(e, "loss");
+        const float *gconv = grad;
+        if (conv) {
+            {
+                StageTimer t(3, st);
+                e = launch_convolve(tel, grad, buf_c, buf_b, (float *)(ws + L.off_psftaps), true, nullptr, nullptr, st, bg);
+            }
+            if (e != cudaSuccess) return cuda_fail(e, "adjoint convolve");
+            gconv = buf_c;
+        }
+        {
+            StageTimer t(4, st);
+            e = launch_adjoint(in, L, ws, gconv, g_mass + first, g_log_age + first, g_log_z + first, g_vlos + first, st);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "adjoint");
+        launches += g_launches;
+        g_launches = 0;
+        remember(workspace, L);
+    }
+    g_launches = launches;
+    return RUBIX_OK;
+}
+
 rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_voxels, float sigma_read, float gain,
                              uint64_t seed, void *stream)
 {

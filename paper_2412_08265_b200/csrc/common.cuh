@@ -124,9 +124,9 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
 
 cudaError_t launch_add_noise(const float *in, float *out, int64_t n, float sigma_read, float gain, uint64_t seed,
                              cudaStream_t st);
-size_t loss_scratch_bytes();
+size_t loss_scratch_bytes(int32_t batch = 1);
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
-                                 double *partial, double *loss, cudaStream_t st);
+                                 double *partial, double *loss, cudaStream_t st, int32_t batch = 1);
 
 // Table mode (readings R15 / R16): the rest position of channel k is x_k = Y[k] c + a with a per-launch
 // table Y and per-particle (c, a); used for log-sampled SSP grids and for explicit channel wavelengths.

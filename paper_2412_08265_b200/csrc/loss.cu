@@ -24,11 +24,15 @@ __device__ __forceinline__ double block_sum(double v, double *sm)
     return t;                               // valid in thread 0
 }
 
+// blockIdx.y = batch element (cubes back to back, n_vox voxels each; one row of partials per element)
 __global__ void __launch_bounds__(kLossThreads)
-k_residual_loss(const float *__restrict__ cube, const float *__restrict__ target, int64_t n_vox,
-                float *__restrict__ grad, double *__restrict__ partial, int aligned)
+k_residual_loss(const float *__restrict__ cube0, const float *__restrict__ target0, int64_t n_vox,
+                float *__restrict__ grad0, double *__restrict__ partial0, int aligned)
 {
     __shared__ double sm[kLossThreads / 32];
+    const float *cube = cube0 + (size_t)blockIdx.y * n_vox, *target = target0 + (size_t)blockIdx.y * n_vox;
+    float *grad = grad0 + (size_t)blockIdx.y * n_vox;
+    double *partial = partial0 + (size_t)blockIdx.y * gridDim.x;
     double acc = 0.0;
     const int64_t n4 = aligned ? n_vox >> 2 : 0;            // 16-byte accesses only when all three arrays allow them
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -49,24 +53,27 @@ k_residual_loss(const float *__restrict__ cube, const float *__restrict__ target
 }
 
 __global__ void __launch_bounds__(kLossThreads)
-k_loss_final(const double *__restrict__ partial, int n, double *__restrict__ loss)
+k_loss_final(const double *__restrict__ partial0, int n, double *__restrict__ loss)
 {
     __shared__ double sm[kLossThreads / 32];
+    const double *partial = partial0 + (size_t)blockIdx.x * n;   // blockIdx.x = batch element
     double acc = 0.0;
     for (int i = threadIdx.x; i < n; i += kLossThreads) acc += partial[i];
     const double tot = block_sum(acc, sm);
-    if (threadIdx.x == 0) *loss = tot;
+    if (threadIdx.x == 0) loss[blockIdx.x] = tot;
 }
 
-size_t loss_scratch_bytes() { return align_up((size_t)kLossBlocks * sizeof(double), 256); }
+size_t loss_scratch_bytes(int32_t batch) { return align_up((size_t)batch * kLossBlocks * sizeof(double), 256); }
 
+// `batch` cubes of n_vox voxels back to back: loss[b] and grad of every element, each summed exactly as a single call would
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
-                                 double *partial, double *loss, cudaStream_t st)
+                                 double *partial, double *loss, cudaStream_t st, int32_t batch)
 {
-    const int aligned = ((((uintptr_t)cube) | ((uintptr_t)target) | ((uintptr_t)grad)) & 15u) == 0;
-    k_residual_loss<<<kLossBlocks, kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial, aligned);
+    const int aligned = ((((uintptr_t)cube) | ((uintptr_t)target) | ((uintptr_t)grad)) & 15u) == 0 &&
+                        (batch == 1 || (n_vox & 3) == 0);
+    k_residual_loss<<<dim3(kLossBlocks, (unsigned)batch), kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial, aligned);
     RUBIX_LAUNCH_CHECK();
-    k_loss_final<<<1, kLossThreads, 0, st>>>(partial, kLossBlocks, loss);
+    k_loss_final<<<(unsigned)batch, kLossThreads, 0, st>>>(partial, kLossBlocks, loss);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
 }

@@ -215,6 +215,21 @@ def test_batched_sharded_and_mirrored_entries_validate_on_the_host(lib):
     assert lib.rubix_forward_batched_workspace_bytes(100, None, 3, ssp.ref(), tel.ref()) > \
         lib.rubix_forward_batched_workspace_bytes(100, None, 1, ssp.ref(), tel.ref()) > 0
     assert lib.rubix_forward_batched_workspace_bytes(100, None, 0, ssp.ref(), tel.ref()) == 0
+    # the fused forward + loss + adjoint of many galaxies: offsets are required, the same checks apply
+    def lg_batched(offsets, batch, ws_bytes=1 << 40, loss=FAKE):
+        off = None if offsets is None else np.asarray(offsets, np.int64)
+        return lib.rubix_loss_and_grad_batched(P.ref(), None if off is None else off.ctypes.data, batch, ssp.ref(), tel.ref(),
+                                               R.ctypes.data, FAKE + (1 << 41), loss, None, FAKE, FAKE, FAKE, FAKE,
+                                               FAKE + (1 << 42), ws_bytes, None)
+
+    assert lg_batched(None, 3) == B.RUBIX_ERR_INVALID_ARG and "offsets" in B.rubix_last_error()
+    assert lg_batched([0, 50, 40, 100], 3) == B.RUBIX_ERR_INVALID_ARG
+    assert lg_batched([0, 50, 60, 100], 3, loss=None) == B.RUBIX_ERR_NULL
+    assert lg_batched([0, 50, 60, 100], 3, ws_bytes=1024) == B.RUBIX_ERR_WORKSPACE
+    off3 = np.asarray([0, 50, 60, 100], np.int64)
+    assert lib.rubix_loss_and_grad_batched_workspace_bytes(100, off3.ctypes.data, 3, ssp.ref(), tel.ref()) > \
+        lib.rubix_forward_batched_workspace_bytes(100, off3.ctypes.data, 3, ssp.ref(), tel.ref())
+    assert lib.rubix_loss_and_grad_batched_workspace_bytes(100, None, 3, ssp.ref(), tel.ref()) == 0
     # row window of a sharded run
     for n_x, n_full, first, ok in ((4, 16, 12, True), (4, 16, 13, False), (4, 0, 2, False), (4, 16, -1, False)):
         _, t2 = _structs(tel=synth.make_telescope("tiny"))
