@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-adjoint", action="store_true")
     ap.add_argument("--no-batched", action="store_true")
+    ap.add_argument("--cell-order", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="rubix_telescope.cell_order: 0 auto (the library decides), 1 off, 2 on, 3 on for every spaxel")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
                     help="replicas (default, BASELINE.json north_star: one galaxy per GPU, weak scaling) or sharded: ONE galaxy "
                          "over all GPUs by detector rows (paper_2412_08265_b200/sharded.py, SURVEY.md 8(f)-4, strong scaling)")
@@ -71,6 +73,7 @@ def workload_config(w):
             "euler_deg": [round(float(v), 4) for v in w.euler_deg],
             "l2_policy": "cube (%.2f GB) and workspace exceed the 126 MB L2: no flush needed"
                          % (t.n_spaxels * t.n_channels * 4 / 1e9),
+            "cell_order": int(getattr(t, "cell_order", 0)),
             "parallelism": "replicas only (one galaxy per GPU, no collective)"}
 
 
@@ -467,6 +470,9 @@ def run_ours(args):
     base = synth.make_workload(args.workload)
     widx = ["tiny", "small", "medium", "contention"].index(args.workload)
     w = base if rank == 0 else synth.make_workload(args.workload, seed=replicas.replica_seed(widx, rank))
+    if args.cell_order:
+        import dataclasses
+        w = dataclasses.replace(w, telescope=dataclasses.replace(w.telescope, cell_order=args.cell_order))
     t, n = w.telescope, w.particles.n
     dw = B.DeviceWorkload(w, device=dev)
     cube = torch.empty(dw.shape, dtype=torch.float32, device=dev)

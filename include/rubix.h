@@ -117,11 +117,29 @@ typedef struct {
                                     /* uses THAT geometry (bit-equal keys), and this call owns the    */
                                     /* n_x rows x_first .. x_first + n_x - 1 (key = (ix - x_first)    */
                                     /* n_y + iy; particles in other rows are dropped).  0 = off.      */
+    int32_t cell_order;             /* Per-cell template reuse in piled-up spaxels: */
+                                    /* the particles of a spaxel are accumulated in the order (SSP    */
+                                    /* cell, original index) and spaxels with >= 2 N_a N_z particles  */
+                                    /* go to a kernel that keeps the corner templates of a cell in    */
+                                    /* registers.  RUBIX_CELL_ORDER_AUTO (0): on when n >= 10^6 and   */
+                                    /* n >= 64 x the spaxels of the whole detector (times the batch);  */
+                                    /* _OFF (1); _ON (2); _ALL (3): on,                                */
+                                    /* and EVERY spaxel goes to that kernel.  Uniform grids only      */
+                                    /* (otherwise off).  Changes the fp32 summation order inside a    */
+                                    /* spaxel and the exported `perm` (rubix_get_sort_artifacts),     */
+                                    /* nothing else; calls that must agree bit for bit (the ranks of  */
+                                    /* a spaxel-sharded run) pass the same explicit value.             */
+    int32_t reserved0;              /* 0 */
 } rubix_telescope;
+
+#define RUBIX_CELL_ORDER_AUTO 0
+#define RUBIX_CELL_ORDER_OFF 1
+#define RUBIX_CELL_ORDER_ON 2
+#define RUBIX_CELL_ORDER_ALL 3
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 7
+#define RUBIX_ABI_VERSION 8
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -281,7 +299,8 @@ rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_vo
 /* DEVICE pointers into the workspace last used by rubix_build_cube / rubix_forward / rubix_cube_adjoint /
  * rubix_loss_and_grad on this workspace address (the library remembers the 256 most recently used addresses) (compared bit for bit with the oracle):
  *   key     [n]      spaxel key of each particle in original order (n_s = dropped)
- *   perm    [n]      stable order by (key, original index)
+ *   perm    [n]      stable order by (key, original index); with the cell order active (rubix_telescope.cell_order)
+ *                    by (key, SSP cell, original index): the same segments, each holding the same particles
  *   seg_off [n_s+2]  segment s is perm[seg_off[s] .. seg_off[s+1]); s = n_s: dropped particles
  * Valid once the stream of that call has completed. */
 rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key,

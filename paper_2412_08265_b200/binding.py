@@ -26,7 +26,7 @@ EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf"
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 7          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 8          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -55,7 +55,8 @@ class CTelescope(C.Structure):
                 ("psf_size", C.c_int32), ("psf_sigma", C.c_float),
                 ("lsf_size", C.c_int32), ("lsf_sigma", C.c_float), ("resample", C.c_int32),
                 ("redshift", C.c_float), ("flux_scale", C.c_float), ("lambda_obs", C.c_void_p),
-                ("psf_alpha", C.c_float), ("psf_lambda_ref", C.c_float), ("n_x_full", C.c_int32), ("x_first", C.c_int32)]
+                ("psf_alpha", C.c_float), ("psf_lambda_ref", C.c_float), ("n_x_full", C.c_int32), ("x_first", C.c_int32),
+                ("cell_order", C.c_int32), ("reserved0", C.c_int32)]
 
 
 _lib = None
@@ -186,7 +187,7 @@ def c_telescope(tel) -> _Keep:
                             float(getattr(tel, "flux_scale", 1.0)),
                             None if lam is None else lam.ctypes.data, float(getattr(tel, "psf_alpha", 0.0)),
                             float(getattr(tel, "psf_lambda_ref", 1.0)), int(getattr(tel, "n_x_full", 0)),
-                            int(getattr(tel, "x_first", 0))), lam)
+                            int(getattr(tel, "x_first", 0)), int(getattr(tel, "cell_order", 0)), 0), lam)
 
 
 def c_ssp(ssp, flux) -> _Keep:

@@ -100,6 +100,7 @@ rubix_status check_tel(const rubix_telescope *t)
         return fail(RUBIX_ERR_INVALID_ARG, "row window: need 0 <= x_first and x_first + n_x <= n_x_full");
     if (t->n_x_full == 0 && t->x_first != 0)
         return fail(RUBIX_ERR_INVALID_ARG, "x_first needs n_x_full > 0");
+    if (t->cell_order < 0 || t->cell_order > 3) return fail(RUBIX_ERR_INVALID_ARG, "cell_order must be 0 (auto), 1 (off), 2 (on) or 3 (all)");
     if (!(t->dlambda > 0.0f) || !isfinite(t->dlambda) || !isfinite(t->lambda0))
         return fail(RUBIX_ERR_INVALID_ARG, "telescope dlambda must be > 0 and finite");
     if (t->resample != RUBIX_RESAMPLE_POINT && t->resample != RUBIX_RESAMPLE_FLUX)

@@ -27,6 +27,9 @@ constexpr int kSortWarps = 8;               // warps per CTA in the radix passes
 constexpr int kSortItems = 1024;            // keys per warp per radix pass
 constexpr int kSortMaxDigitBits = 9;
 constexpr int kFluxPad = 2048;              // zero floats behind the workspace copy of the SSP grid
+constexpr int kCellAutoMean = 64;           // cell order, auto: on when the detector holds >= this many particles per spaxel ...
+constexpr int64_t kCellAutoMinN = 1000000;  // ... and at least this many particles (several waves of work units for BOTH kernels);
+constexpr int kCellAutoRuns = 2;            // ... and a spaxel goes to k_accumulate_cell from this many particles per SSP cell
 constexpr int kRowAlign = 32;               // rows of that copy are padded to 32 floats (128 B)
 
 // Sorted-order particle record consumed by the accumulate kernel (48 B, 16-B aligned).
@@ -101,6 +104,11 @@ struct PassInputs {
     bool compact_units = false;
 };
 
+// Cell order (rubix_telescope.cell_order, spectral_cell.cu): > 0 when the particle pass sorts by (spaxel, SSP cell) -- the
+// number of cells, i.e. the multiplier of the composite sort key -- else 0.  *threshold (if given) receives the particle
+// count from which a spaxel goes to k_accumulate_cell (0 = every spaxel).
+int32_t cell_order_cells(const PassInputs &in, const Layout &L, int32_t *threshold = nullptr);
+bool cell_kernel_fits(int32_t n_c, double b_max, bool flux);   // spectral_cell.cu
 cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws, cudaStream_t st);
 cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const rubix_telescope *tel, const float *R,
                             int32_t *key, float *vlos, cudaStream_t st);

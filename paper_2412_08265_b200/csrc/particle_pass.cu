@@ -204,16 +204,18 @@ k_sort_scatter(const int32_t *__restrict__ key_in, const int32_t *__restrict__ p
 }
 
 // seg_off[s] = first sorted position whose key is >= s   (s = 0 .. n_s+1)
+// (cell order: the sorted keys are spaxel * mult + cell, dropped particles carry n_s * mult)
 __global__ void __launch_bounds__(256)
-k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s,
+k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s, int32_t mult,
                   int32_t *__restrict__ seg_off)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s > n_s + 1) return;
+    const int64_t want = (int64_t)s * mult;
     int64_t lo = 0, hi = n;
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
-        if (key_sorted[mid] < s) lo = mid + 1; else hi = mid;
+        if ((int64_t)key_sorted[mid] < want) lo = mid + 1; else hi = mid;
     }
     seg_off[s] = (int32_t)lo;
 }
@@ -421,6 +423,9 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     r.w[1] = (float)(m * ta * (1.0 - tz));
     r.w[2] = (float)(m * (1.0 - ta) * tz);
     r.w[3] = (float)(m * ta * tz);
+#ifdef RUBIX_EXP_ONECELL
+    ia = 3; iz = 2;                                     // timing experiment only: every particle in one SSP cell
+#endif
     r.cell = (ia * P.ax.n_z + iz) * P.pitch;
     const double inv = 1.0 / ((1.0 + (double)vlos[pl] / kCkms) * (1.0 + (double)P.redshift));
     const double scale = (double)(1 << kFxFrac);
@@ -630,6 +635,32 @@ k_pad_flux(const float *__restrict__ flux, int32_t n_lambda, int32_t pitch, int6
     }
 }
 
+// Cell order (spectral_cell.cu): composite sort key spaxel * cells + (i_age * n_z + i_z), so that the particles of a spaxel
+// come grouped by SSP cell.  The cell found here only ORDERS the particles (k_prepare_records finds the cell it uses with the
+// same search); dropped particles keep the last key.
+struct CellKeyParams {
+    AxisParams ax;
+    int64_t n;
+    int32_t n_s, cells;
+    int64_t n_phys;
+};
+
+__global__ void __launch_bounds__(256)
+k_cell_keys(const int32_t *__restrict__ key, const float *__restrict__ log_age, const float *__restrict__ log_z,
+            const __grid_constant__ CellKeyParams P, int32_t *__restrict__ ckey)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const int32_t k = key[i];
+    if (k >= P.n_s) { ckey[i] = P.n_s * P.cells; return; }
+    const int64_t p = P.n_phys > 0 ? i % P.n_phys : i;
+    int ia, iz;
+    double ta, tz;
+    axis_cell(P.ax.age, P.ax.n_age, log_age[p], &ia, &ta);
+    axis_cell(P.ax.z, P.ax.n_z, log_z[p], &iz, &tz);
+    ckey[i] = k * P.cells + ia * P.ax.n_z + iz;
+}
+
 // --------------------------------------------------------------------------------------------
 // host side
 // --------------------------------------------------------------------------------------------
@@ -640,20 +671,39 @@ static int bits_for(int32_t max_value)
     return b;
 }
 
+int32_t cell_order_cells(const PassInputs &in, const Layout &L, int32_t *threshold)
+{
+    if (threshold) *threshold = 0;
+    const rubix_telescope *t = in.tel;
+    if (t->cell_order == RUBIX_CELL_ORDER_OFF || L.n <= 0 || !in.ssp) return 0;
+    if (table_mode(in.ssp, t) || gen_mode(in.ssp, t)) return 0;                  // uniform grids only
+    const int32_t cells = in.ssp->n_age * in.ssp->n_z;
+    if ((double)(L.n_s + 2) * cells >= 2147483647.0) return 0;                   // composite key space
+    const double b_max = (double)t->dlambda / (double)in.ssp->dlambda / (1.0 - kBetaCap);
+    if (!cell_kernel_fits(L.n_c, b_max, t->resample == RUBIX_RESAMPLE_FLUX)) return 0;
+    if (t->cell_order == RUBIX_CELL_ORDER_ALL) return cells;                     // every spaxel
+    if (t->cell_order == RUBIX_CELL_ORDER_AUTO) {                                // piled-up detectors only
+        const int64_t n_s_full = (int64_t)(t->n_x_full > 0 ? t->n_x_full : t->n_x) * t->n_y * (in.batch > 0 ? in.batch : 1);
+        if (L.n < kCellAutoMinN || L.n < (int64_t)kCellAutoMean * n_s_full) return 0;
+    }
+    if (threshold) *threshold = kCellAutoRuns * cells;
+    return cells;
+}
+
 Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t n_lambda)
 {
     Layout L{};
     L.n = n;
     L.n_s = n_s;
     L.n_c = n_c;
-    const int bits = bits_for(n_s);                      // keys are 0 .. n_s
-    L.sort_passes = (bits + kSortMaxDigitBits - 1) / kSortMaxDigitBits;
+    const int bits = bits_for(n_s);                      // keys are 0 .. n_s  (the cell order sorts wider keys: the pass
+    L.sort_passes = (bits + kSortMaxDigitBits - 1) / kSortMaxDigitBits;   // count is then fixed in launch_particle_pass)
     L.digit_bits = (bits + L.sort_passes - 1) / L.sort_passes;
     L.n_wchunks = (int32_t)((n + kSortItems - 1) / kSortItems);
     L.max_units = (int64_t)n_s + n / kChunk + 1;
     L.max_part_rows = 2 * (n / kChunk) + 2;
     L.max_multi = n / kChunk + 1;
-    L.final_buf = (L.sort_passes - 1) & 1;
+    L.final_buf = 0;                                     // the LAST radix pass always writes buffer 0
     const size_t nn = (size_t)(n > 0 ? n : 1);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
@@ -672,7 +722,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
         L.off_keybuf[b] = take(nn * 4);
         L.off_permbuf[b] = take(nn * 4);
     }
-    L.off_hist = take((size_t)(1 << L.digit_bits) * (size_t)(L.n_wchunks > 0 ? L.n_wchunks : 1) * 4);
+    L.off_hist = take((size_t)(1 << kSortMaxDigitBits) * (size_t)(L.n_wchunks > 0 ? L.n_wchunks : 1) * 4);
     L.off_dtot = take((size_t)(1 << kSortMaxDigitBits) * 4);
     L.off_dbase = take((size_t)(1 << kSortMaxDigitBits) * 4);
     L.off_unitoff = take(((size_t)n_s + 1) * 4);
@@ -749,14 +799,38 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         }
         RUBIX_LAUNCH_CHECK();
 
-        const int mask = (1 << L.digit_bits) - 1;
-        const int n_digits = 1 << L.digit_bits;
-        const unsigned sort_grid = (unsigned)((L.n_wchunks + kSortWarps - 1) / kSortWarps);
+        // cell order: sort by spaxel * n_cells + cell instead (the composite keys go to the buffer the first pass does not write)
+        const int32_t cells = cell_order_cells(in, L);
+        int sort_passes = L.sort_passes, digit_bits = L.digit_bits;
+        if (cells > 0) {
+            const int bits = bits_for((int32_t)((int64_t)n_s * cells));
+            sort_passes = (bits + kSortMaxDigitBits - 1) / kSortMaxDigitBits;
+            digit_bits = (bits + sort_passes - 1) / sort_passes;
+        }
         const int32_t *kin = key;
+        if (cells > 0) {
+            CellKeyParams C;
+            C.ax.n_age = in.ssp->n_age;
+            C.ax.n_z = in.ssp->n_z;
+            for (int i = 0; i < in.ssp->n_age; ++i) C.ax.age[i] = in.ssp->log_age_axis[i];
+            for (int i = 0; i < in.ssp->n_z; ++i) C.ax.z[i] = in.ssp->log_z_axis[i];
+            C.n = n;
+            C.n_s = n_s;
+            C.cells = cells;
+            C.n_phys = (in.batch > 1 && !in.offsets) ? in.p->n : 0;
+            int32_t *ckey = kbuf[sort_passes & 1];
+            k_cell_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(key, in.p->log_age, in.p->log_z, C, ckey);
+            RUBIX_LAUNCH_CHECK();
+            kin = ckey;
+        }
+        const int mask = (1 << digit_bits) - 1;
+        const int n_digits = 1 << digit_bits;
+        const unsigned sort_grid = (unsigned)((L.n_wchunks + kSortWarps - 1) / kSortWarps);
         const int32_t *pin = nullptr;
-        for (int pass = 0; pass < L.sort_passes; ++pass) {
-            const int shift = pass * L.digit_bits;
-            int32_t *kout = kbuf[pass & 1], *pout = pbuf[pass & 1];
+        for (int pass = 0; pass < sort_passes; ++pass) {
+            const int shift = pass * digit_bits;
+            const int ob = (sort_passes - 1 - pass) & 1;   // the last pass writes buffer 0 = Layout::final_buf
+            int32_t *kout = kbuf[ob], *pout = pbuf[ob];
             k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, histT);
             RUBIX_LAUNCH_CHECK();
             k_sort_rowscan<<<n_digits, 256, 0, st>>>(histT, L.n_wchunks, dtot);
@@ -776,7 +850,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     }
     const int32_t *key_sorted = kbuf[L.final_buf];
     const int32_t *perm = pbuf[L.final_buf];
-    k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, seg);
+    {
+        const int32_t cells = n > 0 ? cell_order_cells(in, L) : 0;
+        k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, cells > 0 ? cells : 1, seg);
+    }
     RUBIX_LAUNCH_CHECK();
     {
         int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);

@@ -22,83 +22,9 @@
 // The unit's records are staged in shared memory once.
 // Single-chunk spaxels write their cube row directly (each voxel exactly once, coalesced);
 // spaxels with more particles write partial rows that k_reduce_partials sums in fixed order.
-#include "common.cuh"
-#include "gen_coord.cuh"
+#include "accumulate.cuh"
 
 namespace rubix {
-
-struct AccumParams {
-    const float *flux;       // padded workspace copy of the SSP grid (Layout::pitch)
-    const Rec *rec;
-    const Unit *units;
-    const int32_t *totals;
-    float *cube;
-    float *partials;
-    int32_t pitch, n_z, n_c, n_tiles, wcap, n_lambda;
-    int32_t skip_empty;      // 1: empty spaxels are left unwritten (the masked PSF/LSF passes never read them)
-    int32_t narrow;          // bin average in table / general-grid mode: no bin is wider than one SSP sample
-    // Mirrors (spaxel-sharded runs, rubix_build_cube_mirrored): rows of spaxels < mirror_lo_n are ALSO stored at mirror_lo,
-    // rows of spaxels >= mirror_hi_first at mirror_hi -- a neighbour's halo, possibly peer memory of another GPU.
-    float *mirror_lo, *mirror_hi;
-    int32_t mirror_lo_n, mirror_hi_first;
-    const int64_t *xtab;     // LOGX: rest position of channel k at beta = 0 (36.28), see k_log_positions
-    cudaTextureObject_t tex;
-    GenGrid gen;             // GEN: general-grid mode (gen_coord.cuh)
-};
-
-constexpr int kPass = 128;                           // table samples produced per warp per pass
-constexpr int kAccWarps = kAccThreads / 32;
-#ifndef RUBIX_LDG_MODE
-#define RUBIX_LDG_MODE 0
-#endif
-#ifndef RUBIX_TEX_CORNERS
-#define RUBIX_TEX_CORNERS 0
-#endif
-#ifndef RUBIX_ACC_DEPTH
-#define RUBIX_ACC_DEPTH 1
-#endif
-#ifndef RUBIX_ACC_MINB
-#define RUBIX_ACC_MINB 5
-#endif
-constexpr int kAccDepth = RUBIX_ACC_DEPTH;           // load sets (passes) in flight per warp
-constexpr int kAccMinBlocks = RUBIX_ACC_MINB;
-
-// (a & b) | c in one LOP3 (b, c stay in registers)
-__device__ __forceinline__ uint32_t and_or(uint32_t a, uint32_t b, uint32_t c)
-{
-    uint32_t d;
-    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
-    return d;
-}
-
-struct Quad { unsigned long long lo, hi; };          // four consecutive samples as two packed pairs
-
-// NOALLOC: the corner windows stream past L1 (listed-knot mode: L1 then keeps the look-up table and the knots, which every
-// sample reads; measured 37.7 -> 27.7 ms on the medium workload)
-template <bool NOALLOC = false>
-__device__ __forceinline__ Quad ldg_quad(const float *p)
-{
-    Quad q;
-    if (NOALLOC) {
-        asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
-        return q;
-    }
-#if RUBIX_LDG_MODE == 1
-    asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
-#elif RUBIX_LDG_MODE == 2
-    asm volatile("ld.global.cg.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
-#elif RUBIX_LDG_MODE == 3
-    asm volatile("ld.global.nc.L1::evict_first.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
-#else
-    asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(q.lo), "=l"(q.hi) : "l"(p));
-#endif
-    return q;
-}
-__device__ __forceinline__ void sts_quad(float *p, unsigned long long lo, unsigned long long hi)
-{
-    asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"((uint32_t)__cvta_generic_to_shared(p)), "l"(lo), "l"(hi)
-                 : "memory");
-}
 
 struct Win {                 // one particle's window in one channel tile
     int64_t base;            // x(k0) - j0 in 36.28 fixed point
@@ -109,8 +35,6 @@ struct Win {                 // one particle's window in one channel tile
     float w0, w1, w2, w3;
     double g;                // GEN: the particle's Doppler value (gen_coord.cuh)
 };
-
-struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 
 // SINGLE: the whole spectrum is one tile (n_tiles == 1): window (j0, nw) comes from the record.
 // FLUX: flux-conserving resampling (RUBIX_RESAMPLE_FLUX): x_k is the lower edge of bin k and the
@@ -135,6 +59,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
     if (u >= P.totals[0]) return;
     const Unit U = P.units[u];
     if (U.count == 0 && P.skip_empty) return;
+    if (P.cell_split && cell_kernel_owns(P, U.spaxel)) return;
     constexpr int TC = CPT * kAccThreads;
     const int k0 = tile * TC;
     const int k_end = min(k0 + TC, P.n_c) - 1;              // last existing channel of this tile
@@ -834,6 +759,11 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
         P.tex = cached_tex;
     }
 #endif
+    int32_t cell_threshold = 0;
+    const bool cell = cell_order_cells(in, L, &cell_threshold) > 0;    // as the particle pass decided
+    P.seg = (const int32_t *)(ws + L.off_seg);
+    P.cell_threshold = cell_threshold;
+    P.cell_split = cell && cell_threshold > 0 ? 1 : 0;
     const size_t smem = (size_t)2 * wcap * sizeof(float) + (size_t)kChunk * sizeof(Rec);
     const unsigned grid = (unsigned)(L.max_units * P.n_tiles);
     cudaError_t e = cudaSuccess;
@@ -851,7 +781,12 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     } else
 #endif
     {
-        StageTimer t(1, st);
+    StageTimer t(1, st);
+    if (cell) {                                             // piled-up spaxels (all of them with RUBIX_CELL_ORDER_ALL)
+        e = launch_accumulate_cell(P, b_max, flux, (unsigned)L.max_units, st);
+        if (e != cudaSuccess) return e;
+    }
+    if (!cell || P.cell_split) {
         if (gen) {
             switch (cpt) {
                 case 29: e = launch_acc_gen<29>(P, flux, narrow, grid, smem, st); break;
@@ -868,6 +803,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
                 default: e = launch_acc<1>(P, flux, logx, grid, smem, st); break;
             }
         }
+    }
     }
     if (e != cudaSuccess) return e;
     StageTimer t2(2, st);

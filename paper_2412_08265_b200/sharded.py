@@ -31,6 +31,8 @@ import threading
 import numpy as np
 
 RECORD_FLOATS = 9        # pos[3], vel[3], mass, log_age, log_z
+CELL_AUTO_MEAN = 64      # rubix.h: RUBIX_CELL_ORDER_AUTO turns the cell order on from this many particles per spaxel ...
+CELL_AUTO_MIN_N = 1_000_000   # ... and this many particles
 
 
 # ------------------------------------------------------------------------------------------ partitioning
@@ -254,6 +256,11 @@ def forward_sharded(comm, backend, records, R, ssp, tel, flux_dev=None, row_cost
     rows = torch.div(key, n_y, rounding_mode="floor")
     counts = torch.bincount(rows[inside], minlength=n_x).to(torch.int64)
     counts = comm.all_reduce_sum(counts)
+    # the order of summation inside a spaxel (rubix_telescope.cell_order) is decided ONCE, from the whole galaxy, as a
+    # single-GPU call on it would decide: every rank then accumulates its spaxels in that order
+    if int(getattr(tel, "cell_order", 0)) == 0:
+        n_total = int(comm.all_reduce_sum(torch.tensor([records.shape[0]], dtype=torch.int64, device=key.device))[0].item())
+        tel = dataclasses.replace(tel, cell_order=2 if n_total >= max(CELL_AUTO_MIN_N, CELL_AUTO_MEAN * n_x * n_y) else 1)
     # 3  the same partition on every rank
     bounds = partition_rows(counts.cpu().numpy(), world, min_rows=max(1, halo),
                             row_cost=float(n_y) if row_cost is None else row_cost)

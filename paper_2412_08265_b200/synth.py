@@ -209,6 +209,7 @@ class Telescope:
     psf_lambda_ref: np.float32 = np.float32(1.0)
     n_x_full: int = 0         # row window of a spaxel-sharded run: the whole detector has n_x_full rows and this
     x_first: int = 0          # telescope owns rows x_first .. x_first + n_x - 1 (0 / 0 = the whole detector)
+    cell_order: int = 0       # per-cell template reuse in piled-up spaxels: 0 = auto, 1 = off, 2 = on, 3 = on for every spaxel
 
     @property
     def n_spaxels(self) -> int:

@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 
 def test_struct_layouts_match_the_header():
-    assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 64 and C.sizeof(B.CTelescope) == 80
+    assert C.sizeof(B.CParticles) == 48 and C.sizeof(B.CSSP) == 64 and C.sizeof(B.CTelescope) == 88
 
 
 def test_abi_version_and_struct_size_are_checked(lib):
@@ -230,6 +230,10 @@ def test_batched_sharded_and_mirrored_entries_validate_on_the_host(lib):
     assert lib.rubix_loss_and_grad_batched_workspace_bytes(100, off3.ctypes.data, 3, ssp.ref(), tel.ref()) > \
         lib.rubix_forward_batched_workspace_bytes(100, off3.ctypes.data, 3, ssp.ref(), tel.ref())
     assert lib.rubix_loss_and_grad_batched_workspace_bytes(100, None, 3, ssp.ref(), tel.ref()) == 0
+    # cell order: 0 .. 3
+    _, t3 = _structs(tel=synth.make_telescope("tiny"))
+    t3.struct.cell_order = 4
+    assert lib.rubix_workspace_bytes(10, ssp.ref(), t3.ref()) == 0 and "cell_order" in B.rubix_last_error()
     # row window of a sharded run
     for n_x, n_full, first, ok in ((4, 16, 12, True), (4, 16, 13, False), (4, 0, 2, False), (4, 16, -1, False)):
         _, t2 = _structs(tel=synth.make_telescope("tiny"))

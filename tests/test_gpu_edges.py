@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
+from sortcheck import check_perm
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -29,7 +30,8 @@ def run_and_check(B, w, what):
     key, perm, seg = (a.cpu().numpy() for a in dw.sort_artifacts())
     okey, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
     operm, oseg = oracle.sort(okey, t.n_spaxels)
-    assert np.array_equal(key, okey) and np.array_equal(perm, operm) and np.array_equal(seg, oseg), what
+    assert np.array_equal(key, okey) and np.array_equal(seg, oseg), what
+    check_perm(perm, operm, oseg, w.particles, w.ssp, t.n_spaxels, None)
     ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t)
     got = cube.cpu().numpy().astype(np.float64)
     assert np.isfinite(got).all(), what

@@ -9,6 +9,7 @@ import numpy as np
 import pytest
 
 import oracle
+from sortcheck import check_perm
 from paper_2412_08265_b200 import synth
 
 torch = pytest.importorskip("torch")
@@ -39,7 +40,8 @@ def check(B, w, what, oracle_too=True):
     key, perm, seg = (a.cpu().numpy() for a in dw.sort_artifacts())
     okey, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
     operm, oseg = oracle.sort(okey, t.n_spaxels)
-    assert np.array_equal(key, okey) and np.array_equal(perm, operm) and np.array_equal(seg, oseg), what
+    assert np.array_equal(key, okey) and np.array_equal(seg, oseg), what
+    check_perm(perm, operm, oseg, w.particles, w.ssp, t.n_spaxels, None)
     assert torch.isfinite(got).all(), what
     two = dw.forward_two_calls()
     torch.cuda.synchronize()

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
+from sortcheck import check_perm
 from gradcheck import assert_gradients, upstream_gradient
 from paper_2412_08265_b200 import synth
 
@@ -59,7 +60,8 @@ def run_and_check(B, w, what):
     key, perm, seg = (a.cpu().numpy() for a in dw.sort_artifacts())
     okey, _ = oracle.rotate_bin(w.particles.pos, w.particles.vel, w.rotation, t.n_x, t.n_y, t.spaxel_size)
     operm, oseg = oracle.sort(okey, t.n_spaxels)
-    assert np.array_equal(key, okey) and np.array_equal(perm, operm) and np.array_equal(seg, oseg), what
+    assert np.array_equal(key, okey) and np.array_equal(seg, oseg), what
+    check_perm(perm, operm, oseg, w.particles, w.ssp, t.n_spaxels, None)
     got = cube.cpu().numpy().astype(np.float64)
     assert np.isfinite(got).all(), what
     ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t)
