@@ -117,18 +117,18 @@ typedef struct {
                                     /* uses THAT geometry (bit-equal keys), and this call owns the    */
                                     /* n_x rows x_first .. x_first + n_x - 1 (key = (ix - x_first)    */
                                     /* n_y + iy; particles in other rows are dropped).  0 = off.      */
-    int32_t cell_order;             /* Per-cell template reuse in piled-up spaxels: */
-                                    /* the particles of a spaxel are accumulated in the order (SSP    */
-                                    /* cell, original index) and spaxels with >= 2 N_a N_z particles  */
-                                    /* go to a kernel that keeps the corner templates of a cell in    */
-                                    /* registers.  RUBIX_CELL_ORDER_AUTO (0): on when n >= 10^6 and   */
-                                    /* n >= 64 x the spaxels of the whole detector (times the batch);  */
-                                    /* _OFF (1); _ON (2); _ALL (3): on,                                */
-                                    /* and EVERY spaxel goes to that kernel.  Uniform grids only      */
-                                    /* (otherwise off).  Changes the fp32 summation order inside a    */
-                                    /* spaxel and the exported `perm` (rubix_get_sort_artifacts),     */
+    int32_t cell_order;             /* Per-cell template reuse in piled-up spaxels (SURVEY.md 8(d)    */
+                                    /* K3): the particles of a spaxel are accumulated in the order    */
+                                    /* (SSP cell, original index) and spaxels with >= 2 N_a N_z       */
+                                    /* particles go to a kernel that keeps the corner templates of a  */
+                                    /* cell in registers.  RUBIX_CELL_ORDER_AUTO (0): on when         */
+                                    /* n >= 10^6 and n >= 64 x the spaxels of the whole detector      */
+                                    /* (times the batch); _OFF (1); _ON (2); _ALL (3): on, and EVERY  */
+                                    /* spaxel goes to that kernel.  Uniform grids and the point rule  */
+                                    /* only (otherwise off).  Changes the fp32 summation order inside */
+                                    /* a spaxel and the exported `perm` (rubix_get_sort_artifacts),   */
                                     /* nothing else; calls that must agree bit for bit (the ranks of  */
-                                    /* a spaxel-sharded run) pass the same explicit value.             */
+                                    /* a spaxel-sharded run) pass the same explicit value.            */
     int32_t reserved0;              /* 0 */
 } rubix_telescope;
 

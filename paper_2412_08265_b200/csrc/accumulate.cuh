@@ -92,6 +92,6 @@ __device__ __forceinline__ void sts_quad(float *p, unsigned long long lo, unsign
 struct LoadSet { Quad c[4]; };                       // 4 corners x 4 samples
 
 // spectral_cell.cu: the variant for piled-up spaxels (corner windows kept in registers across particles of one SSP cell)
-cudaError_t launch_accumulate_cell(const AccumParams &P, double b_max, bool flux, unsigned grid, cudaStream_t st);
+cudaError_t launch_accumulate_cell(const AccumParams &P, double b_max, unsigned grid, cudaStream_t st);
 
 }  // namespace rubix

@@ -783,7 +783,7 @@ cudaError_t launch_accumulate(const PassInputs &in, const Layout &L, char *ws, f
     {
     StageTimer t(1, st);
     if (cell) {                                             // piled-up spaxels (all of them with RUBIX_CELL_ORDER_ALL)
-        e = launch_accumulate_cell(P, b_max, flux, (unsigned)L.max_units, st);
+        e = launch_accumulate_cell(P, b_max, (unsigned)L.max_units, st);
         if (e != cudaSuccess) return e;
     }
     if (!cell || P.cell_split) {

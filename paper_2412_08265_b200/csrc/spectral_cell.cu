@@ -10,7 +10,7 @@
 // pass and lane, no global load at all; the resample phase is k_accumulate's.  The decision is taken per particle from the
 // records, so the kernel is correct for any order; the order only decides how often it reloads.
 //
-// 256 threads (thread t owns channels t + 256 i, i < CPT), two CTAs per SM; uniform grids, one channel tile.
+// 256 threads (thread t owns channels t + 256 i, i < CPT), two CTAs per SM; uniform grids, point rule, one channel tile.
 #include <type_traits>
 
 #include "accumulate.cuh"
@@ -33,7 +33,7 @@ struct WinC {
     bool reload, interior;
 };
 
-template <int CPT, int NPASS, bool FLUX>
+template <int CPT, int NPASS>
 __global__ void __launch_bounds__(kCellThreads, 2)
 k_accumulate_cell(const __grid_constant__ AccumParams P)
 {
@@ -91,11 +91,7 @@ k_accumulate_cell(const __grid_constant__ AccumParams P)
                 const int lo = covered ? rc.z - J0 : 0, hi = covered ? lo + rc.w : 0;
                 const int64_t base = a - ((int64_t)J0 << kFxFrac);
                 const uint32_t b = (uint32_t)rb.y;
-                bool interior = covered && rc.x == 0 && rc.y == k_end;
-                if (FLUX) {
-                    const int64_t j0s = (int64_t)J0 << kFxFrac;
-                    interior = interior && base >= -j0s && base + (int64_t)b * (k_end + 1) <= ((int64_t)(P.n_lambda - 1) << kFxFrac) - j0s;
-                }
+                const bool interior = covered && rc.x == 0 && rc.y == k_end;
                 const bool reload = covered && (!common || prev_cell != rb.x);
                 srec[3 * tid + 1] = make_int4((int)(uint32_t)base, (int)(base >> 32), rb.y, rb.x + J0);
                 srec[3 * tid + 2] = make_int4(covered ? rc.x : 1, covered ? rc.y : 0,
@@ -175,68 +171,9 @@ k_accumulate_cell(const __grid_constant__ AccumParams P)
             const unsigned long long d = ffma2(s0, minus1, s1);
             acc2[m] = fadd2(acc2[m], ffma2(f, d, s0));
         };
-        // exact integral of the table's interpolant over local positions [xl, xh] (12.20), times inv_b
-        auto flux_sample = [&](int i, uint32_t xl, uint32_t xh, float inv_b, const float *tabp) {
-            const uint32_t jl = xl >> 20, jh = xh >> 20;
-            const float fl = (float)(xl & 0xFFFFFu) * (1.0f / 1048576.0f);
-            const float fh = (float)(xh & 0xFFFFFu) * (1.0f / 1048576.0f);
-            const float a0 = tabp[jl], a1 = tabp[jl + 1];
-            float tot;
-            if (jl == jh) {
-                tot = (fh - fl) * fmaf(0.5f * (fl + fh), a1 - a0, a0);
-            } else {
-                const float c0 = tabp[jh], c1 = tabp[jh + 1];
-                tot = 0.5f * (1.0f - fl) * (fmaf(fl, a1 - a0, a0) + a1);
-                tot = fmaf(0.5f * fh, c0 + fmaf(fh, c1 - c0, c0), tot);
-                for (uint32_t j = jl + 1; j < jh; ++j) tot = fmaf(0.5f, tabp[j] + tabp[j + 1], tot);
-            }
-            add_to(i, tot * inv_b);
-        };
         // channel stride 256 b / 256 = b in the 2^-20 local format: exact for every b
         auto resample = [&](const WinC &W, const float *buf) {
             const char *bytes = reinterpret_cast<const char *>(buf);
-            if (FLUX) {
-                const float inv_b = (float)(1 << kFxFrac) / (float)W.b;
-                const int64_t j0s = (int64_t)W.J0 << kFxFrac;
-                const int64_t cov_lo = -j0s, cov_hi = ((int64_t)(P.n_lambda - 1) << kFxFrac) - j0s;
-                const int64_t e0 = W.base + (int64_t)W.b * tid;          // lower edge of channel tid
-                if (W.interior) {
-                    const uint32_t xl0 = (uint32_t)(e0 >> 8), xh0 = (uint32_t)((e0 + (int64_t)W.b) >> 8);
-                    if (W.b <= (1u << kFxFrac)) {           // bins no wider than one SSP sample: three samples, no branch
-                        const float width = (float)(xh0 - xl0) * (1.0f / 1048576.0f);
-#pragma unroll
-                        for (int i = 0; i < CPT; ++i) {
-                            const uint32_t x = xl0 + (uint32_t)i * W.b;
-                            const float *e = reinterpret_cast<const float *>(bytes + ((x >> 18) & m_addr));
-                            const float a0 = e[0], a1 = e[1], a2r = e[2];
-                            const float fl = __uint_as_float(and_or(x << 3, m_frac, one_bits)) - 1.0f;
-                            const float uu = fl + width;
-                            const float u1 = fminf(uu, 1.0f), u2 = fmaxf(uu - 1.0f, 0.0f);
-                            const float a2 = uu > 1.0f ? a2r : a1;
-                            const float d1 = a1 - a0, d2 = a2 - a1;
-                            const float il = fl * fmaf(0.5f * fl, d1, a0);
-                            float iu = u1 * fmaf(0.5f * u1, d1, a0);
-                            iu = fmaf(u2, fmaf(0.5f * u2, d2, a1), iu);
-                            add_to(i, (iu - il) * inv_b);
-                        }
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < CPT; ++i)
-                            flux_sample(i, xl0 + (uint32_t)i * W.b, xh0 + (uint32_t)i * W.b, inv_b, buf);
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < CPT; ++i) {
-                        const int k = tid + i * kCellThreads;
-                        if (k >= W.ka && k <= W.kb) {
-                            const int64_t lo = e0 + (int64_t)W.b * (i * kCellThreads);
-                            const int64_t cl = max(lo, cov_lo), ch = min(lo + (int64_t)W.b, cov_hi);
-                            if (ch > cl) flux_sample(i, (uint32_t)(cl >> 8), (uint32_t)(ch >> 8), inv_b, buf);
-                        }
-                    }
-                }
-                return;
-            }
             const uint32_t x0 = (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             if (W.interior) {                               // the whole spectrum inside the SSP coverage
 #pragma unroll
@@ -300,24 +237,26 @@ k_accumulate_cell(const __grid_constant__ AccumParams P)
 // ---- host --------------------------------------------------------------------------------------
 static int cell_cpt(int32_t n_c) { return n_c <= 2 * kCellThreads ? 2 : (n_c <= 8 * kCellThreads ? 8 : 15); }
 
-// samples the table must hold: every channel a thread may address (CPT x 256 of them) plus the reload margin
-static int cell_need(int32_t n_c, double b_max, bool flux)
+// samples the table must hold: every channel a thread may address (CPT x 256 of them) plus the spread of the window starts
+static int cell_need(int32_t n_c, double b_max)
 {
     const int tc = cell_cpt(n_c) * kCellThreads;
-    return (int)(b_max * (tc + (flux ? 1 : 0))) + kRowAlign + 4 + kCellMargin;
+    return (int)(b_max * tc) + kRowAlign + 4 + kCellMargin;
 }
 
+// point rule only: under the bin average the kernel would be bound by its instruction count even harder (measured on the
+// contention workload: 48.2 ms with the heavy spaxels here against 44 ms with k_accumulate<FLUX> alone)
 bool cell_kernel_fits(int32_t n_c, double b_max, bool flux)
 {
-    return n_c <= 15 * kCellThreads && cell_need(n_c, b_max, flux) <= kTabMax;
+    return !flux && n_c <= 15 * kCellThreads && cell_need(n_c, b_max) <= kTabMax;
 }
 
-template <int CPT, int NPASS, bool FLUX>
+template <int CPT, int NPASS>
 static cudaError_t launch_cell3(const AccumParams &P, unsigned grid, cudaStream_t st)
 {
     // the masked 12.20 address of a lane beyond the last channel may point up to 16 KB past a table: pad
     const size_t smem = (size_t)2 * NPASS * kCellStep * sizeof(float) + (size_t)kChunk * sizeof(Rec) + (NPASS < 4 ? 16384 : 0);
-    auto kern = k_accumulate_cell<CPT, NPASS, FLUX>;
+    auto kern = k_accumulate_cell<CPT, NPASS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kCellThreads, smem, st>>>(P);
@@ -326,19 +265,18 @@ static cudaError_t launch_cell3(const AccumParams &P, unsigned grid, cudaStream_
 }
 
 template <int CPT>
-static cudaError_t launch_cell2(const AccumParams &P, int npass, bool flux, unsigned grid, cudaStream_t st)
+static cudaError_t launch_cell2(const AccumParams &P, int npass, unsigned grid, cudaStream_t st)
 {
-    if (npass <= 2) return flux ? launch_cell3<CPT, 2, true>(P, grid, st) : launch_cell3<CPT, 2, false>(P, grid, st);
-    return flux ? launch_cell3<CPT, 4, true>(P, grid, st) : launch_cell3<CPT, 4, false>(P, grid, st);
+    return npass <= 2 ? launch_cell3<CPT, 2>(P, grid, st) : launch_cell3<CPT, 4>(P, grid, st);
 }
 
-cudaError_t launch_accumulate_cell(const AccumParams &P, double b_max, bool flux, unsigned grid, cudaStream_t st)
+cudaError_t launch_accumulate_cell(const AccumParams &P, double b_max, unsigned grid, cudaStream_t st)
 {
-    const int npass = (cell_need(P.n_c, b_max, flux) + kCellStep - 1) / kCellStep;
+    const int npass = (cell_need(P.n_c, b_max) + kCellStep - 1) / kCellStep;
     switch (cell_cpt(P.n_c)) {
-        case 2: return launch_cell2<2>(P, npass, flux, grid, st);
-        case 8: return launch_cell2<8>(P, npass, flux, grid, st);
-        default: return launch_cell2<15>(P, npass, flux, grid, st);
+        case 2: return launch_cell2<2>(P, npass, grid, st);
+        case 8: return launch_cell2<8>(P, npass, grid, st);
+        default: return launch_cell2<15>(P, npass, grid, st);
     }
 }
 
