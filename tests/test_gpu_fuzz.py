@@ -58,6 +58,9 @@ def random_case(seed):
     w = synth.make_workload("tiny", n=max(n, 1), seed=int(rng.integers(1, 10 ** 6)))
     if n == 0:
         w.particles = w.particles.subset(slice(0, 0))
+    # (drawn from a stream of its own so that the cases above stay what they were) order inside a spaxel: auto / off / cell
+    # order with every spaxel through k_accumulate_cell (R22; silently off where that kernel does not apply)
+    tel = dataclasses.replace(tel, cell_order=int(np.random.default_rng(77_000 + seed).choice([0, 1, 3, 3])))
     w.ssp, w.telescope = ssp, tel
     if rng.integers(0, 4) == 0 and n > 0:                          # pile everything into a few spaxels
         w.particles.pos[:] *= np.float32(0.05)
