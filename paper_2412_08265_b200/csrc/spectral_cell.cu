@@ -90,7 +90,6 @@ k_accumulate_cell(const __grid_constant__ AccumParams P)
                 const int J0 = common ? s_jmin : rc.z;
                 const int lo = covered ? rc.z - J0 : 0, hi = covered ? lo + rc.w : 0;
                 const int64_t base = a - ((int64_t)J0 << kFxFrac);
-                const uint32_t b = (uint32_t)rb.y;
                 const bool interior = covered && rc.x == 0 && rc.y == k_end;
                 const bool reload = covered && (!common || prev_cell != rb.x);
                 srec[3 * tid + 1] = make_int4((int)(uint32_t)base, (int)(base >> 32), rb.y, rb.x + J0);
