@@ -139,7 +139,7 @@ typedef struct {
 
 /* Version of this header's ABI (struct layouts and call signatures); bumped whenever either changes.
  * rubix_abi_version() returns the value the LIBRARY was built with. */
-#define RUBIX_ABI_VERSION 8
+#define RUBIX_ABI_VERSION 9
 uint32_t rubix_abi_version(void);
 
 /* Resampling rule of step 5 ("Additional resampling is performed to match the
@@ -285,6 +285,22 @@ rubix_status rubix_loss_and_grad_batched(const rubix_particles *particles, const
                                          const rubix_ssp *ssp, const rubix_telescope *tel, const float *R, const float *targets,
                                          double *loss, float *cubes_out, float *g_mass, float *g_log_age, float *g_log_z,
                                          float *g_vlos, void *workspace, size_t workspace_bytes, void *stream);
+
+/* The loss step of rubix_loss_and_grad on its own, WITHOUT any workspace or allocation (for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ *     grads[b][v] = 2 (cubes[b][v] - targets[b][v]),   loss[b] = sum_v (cubes[b][v] - targets[b][v])^2   (fp64, fixed order)
+ * for `batch` cubes of n_voxels voxels back to back -- the upstream gradient rubix_cube_adjoint takes (
+ * SURVEY.md 8(f)-3).  Same kernels and summation order as inside rubix_loss_and_grad(_batched): the same values bit for bit.
+ *   cubes, targets, grads  DEVICE [batch][n_voxels] fp32, three distinct arrays;  loss  DEVICE [batch] doubles
+ * The per-block partial sums live in a file-scope device array of the library: 64 x 1184 doubles = 606 208 bytes, held by
+ * every GPU that loads the library until the process exits.  LIMIT: batch <= RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH (64);
+ * more is refused with RUBIX_ERR_UNSUPPORTED.  All calls on one device share that array: calls that may overlap on the GPU
+ * (different streams without an ordering between them) race on it and return wrong losses -- order them on one stream or
+ * with events.  Nothing in it has to be cleared between calls (every slot is written before it is read).  The call
+ * launches two kernels on `stream`, never synchronises and calls no cudaMalloc / cudaFree. */
+#define RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH 64
+rubix_status rubix_residual_loss_static(const float *cubes, const float *targets, int64_t n_voxels, int32_t batch,
+                                        float *grads, double *loss, void *stream);
 
 /* Noise stage ("add realistic noise"; the paper names no model -- DESIGN.md reading R17):
  *     cube_out[v] = cube_in[v] + sqrt(sigma_read^2 + gain * max(cube_in[v], 0)) * n_v ,   n_v ~ N(0, 1)

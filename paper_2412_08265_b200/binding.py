@@ -24,9 +24,10 @@ EXPORTS = ("rubix_workspace_bytes", "rubix_build_cube", "rubix_convolve_psf_lsf"
            "rubix_forward_host", "rubix_last_launch_count", "rubix_last_error", "rubix_abi_version",
            "rubix_forward_host_pipelined_scratch_bytes", "rubix_forward_host_pipelined", "rubix_forward_host_drain",
            "rubix_loss_and_grad_workspace_bytes", "rubix_loss_and_grad", "rubix_add_noise",
+           "rubix_residual_loss_static",
            # include/rubix_peaks.h (measurement helpers)
            "rubix_measure_peaks", "rubix_stage_timing_enable", "rubix_stage_timing_read")
-ABI_VERSION = 8          # RUBIX_ABI_VERSION of include/rubix.h
+ABI_VERSION = 9          # RUBIX_ABI_VERSION of include/rubix.h
 N_STAGES = 5
 STAGES = ("particle_pass", "accumulate", "reduce_partials", "psf_lsf", "adjoint")
 
@@ -111,6 +112,8 @@ def load():
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                             C.c_void_p]
+        lib.rubix_residual_loss_static.restype = C.c_int
+        lib.rubix_residual_loss_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.rubix_add_noise.restype = C.c_int
         lib.rubix_add_noise.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float, C.c_uint64, C.c_void_p]
         lib.rubix_get_sort_artifacts.restype = C.c_int
@@ -324,6 +327,17 @@ def rubix_loss_and_grad(particles: _Keep, ssp: _Keep, tel: _Keep, R, target, los
                                       _ptr(loss), _ptr(cube_out), _ptr(g_mass), _ptr(g_log_age),
                                       _ptr(g_log_z), _ptr(g_vlos), _ptr(workspace),
                                       int(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
+RESIDUAL_LOSS_STATIC_MAX_BATCH = 64      # RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH of include/rubix.h
+
+
+def rubix_residual_loss_static(cubes, targets, grads, loss, batch=1, stream=None):
+    """grads = 2 (cubes - targets), loss[b] = sum (cubes[b] - targets[b])^2; no workspace, no allocation (batch <= 64)."""
+    n_vox = int(cubes.numel()) // int(batch)
+    assert int(cubes.numel()) == n_vox * int(batch) == int(targets.numel()) == int(grads.numel())
+    _check(load().rubix_residual_loss_static(_ptr(cubes), _ptr(targets), n_vox, int(batch), _ptr(grads), _ptr(loss),
+                                             _stream(stream)))
 
 
 def rubix_add_noise(cube_in, cube_out, sigma_read, gain, seed, stream=None):

@@ -741,6 +741,26 @@ rubix_status rubix_add_noise(const float *cube_in, float *cube_out, int64_t n_vo
     return RUBIX_OK;
 }
 
+rubix_status rubix_residual_loss_static(const float *cubes, const float *targets, int64_t n_voxels, int32_t batch,
+                                        float *grads, double *loss, void *stream)
+{
+    t_err[0] = 0;
+    Range nvtx_range("rubix_residual_loss_static");
+    g_launches = 0;
+    if (n_voxels < 0) return fail(RUBIX_ERR_INVALID_ARG, "n_voxels must be >= 0");
+    if (batch < 1) return fail(RUBIX_ERR_INVALID_ARG, "batch must be >= 1");
+    if (batch > RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH)
+        return fail(RUBIX_ERR_UNSUPPORTED, "batch = %d exceeds the %d cubes the static scratch of rubix_residual_loss_static holds "
+                    "(split the call, or use rubix_loss_and_grad_batched with a workspace)", batch,
+                    RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH);
+    if (!loss) return fail(RUBIX_ERR_NULL, "loss is NULL");
+    if (n_voxels > 0 && (!cubes || !targets || !grads)) return fail(RUBIX_ERR_NULL, "cubes, targets or grads is NULL");
+    static_assert(RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH == kLossStaticMaxBatch, "header and scratch size disagree");
+    cudaError_t e = launch_residual_loss_static(cubes, targets, n_voxels, grads, loss, (cudaStream_t)stream, batch);
+    if (e != cudaSuccess) return cuda_fail(e, "residual loss (static scratch)");
+    return RUBIX_OK;
+}
+
 rubix_status rubix_get_sort_artifacts(const void *workspace, const int32_t **key, const int32_t **perm,
                                       const int32_t **seg_off)
 {

@@ -132,6 +132,10 @@ cudaError_t launch_adjoint(const PassInputs &in, const Layout &L, char *ws, cons
 
 cudaError_t launch_add_noise(const float *in, float *out, int64_t n, float sigma_read, float gain, uint64_t seed,
                              cudaStream_t st);
+constexpr int kLossStaticMaxBatch = 64;    // cubes per rubix_residual_loss_static call (size of its file-scope scratch)
+// launch_residual_loss with the partials in a file-scope device array (loss.cu): no workspace, no allocation; batch <= 64
+cudaError_t launch_residual_loss_static(const float *cube, const float *target, int64_t n_vox, float *grad, double *loss,
+                                        cudaStream_t st, int32_t batch);
 size_t loss_scratch_bytes(int32_t batch = 1);
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
                                  double *partial, double *loss, cudaStream_t st, int32_t batch = 1);

@@ -4,6 +4,8 @@
 //   L       = sum_v (cube[v] - target[v])^2                    in fp64, FIXED order: per-thread
 //             grid-stride partial -> warp shuffle tree -> block tree -> one partial per CTA, then a
 //             single CTA adds the partials in index order, so the value is bit-reproducible.
+#include <mutex>
+
 #include "common.cuh"
 
 namespace rubix {
@@ -69,6 +71,54 @@ size_t loss_scratch_bytes(int32_t batch) { return align_up((size_t)batch * kLoss
 cudaError_t launch_residual_loss(const float *cube, const float *target, int64_t n_vox, float *grad,
                                  double *partial, double *loss, cudaStream_t st, int32_t batch)
 {
+    const int aligned = ((((uintptr_t)cube) | ((uintptr_t)target) | ((uintptr_t)grad)) & 15u) == 0 &&
+                        (batch == 1 || (n_vox & 3) == 0);
+    k_residual_loss<<<dim3(kLossBlocks, (unsigned)batch), kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial, aligned);
+    RUBIX_LAUNCH_CHECK();
+    k_loss_final<<<(unsigned)batch, kLossThreads, 0, st>>>(partial, kLossBlocks, loss);
+    RUBIX_LAUNCH_CHECK();
+    return cudaSuccess;
+}
+
+// ------------------------------------------------------------------------------------------
+// No-allocation variant (rubix_residual_loss_static, include/rubix.h): the per-CTA partial sums of up to
+// kLossStaticMaxBatch cubes live in a file-scope device array instead of a caller-provided workspace, for callers that
+// cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU that loads the library
+// holds the array (kLossStaticMaxBatch x 1184 doubles = 606 208 bytes) until the process exits.
+//
+// In HOST code the name `s_loss_partials` is a stand-in for the symbol, not a device address: the address the kernels get
+// comes from cudaGetSymbolAddress, asked once per device with that device current (each device has its own copy).
+// Every block of k_residual_loss overwrites its slot before k_loss_final reads it, so nothing has to start at zero and the
+// contents a previous call left behind are never read.  All calls on a device SHARE the array: calls that overlap on the
+// GPU (different streams, no ordering between them) race on it.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) double s_loss_partials[(size_t)kLossStaticMaxBatch * kLossBlocks];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex s_mu;
+double *s_partials_addr[kMaxDevices] = {};                  // device address of s_loss_partials, per device ordinal
+}  // namespace
+
+cudaError_t launch_residual_loss_static(const float *cube, const float *target, int64_t n_vox, float *grad, double *loss,
+                                        cudaStream_t st, int32_t batch)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    double *partial = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(s_mu);
+        if (!s_partials_addr[dev]) {                        // set-up, once per device, with that device current
+            double *ptr = nullptr;
+            e = cudaGetSymbolAddress((void **)&ptr, s_loss_partials);
+            if (e != cudaSuccess) return e;
+            if (!ptr) return cudaErrorInvalidSymbol;
+            s_partials_addr[dev] = ptr;
+        }
+        partial = s_partials_addr[dev];
+    }
     const int aligned = ((((uintptr_t)cube) | ((uintptr_t)target) | ((uintptr_t)grad)) & 15u) == 0 &&
                         (batch == 1 || (n_vox & 3) == 0);
     k_residual_loss<<<dim3(kLossBlocks, (unsigned)batch), kLossThreads, 0, st>>>(cube, target, n_vox, grad, partial, aligned);
