@@ -21,9 +21,9 @@
  *     Consequently a sequence of calls can be captured in a CUDA graph (stage timing of
  *     rubix_peaks.h off) and replayed; the kernels read their sizes from the workspace, not
  *     from the host, after the call has returned.  NOT capturable: calls with rubix_telescope.lambda_obs
- *     or rubix_ssp.lambda_grid (the host arrays are copied to the workspace) and calls that apply a wavelength-dependent PSF
- *     (psf_alpha != 0 with psf_size > 0: the per-channel taps are computed on the host and copied from
- *     pageable memory); the rubix_forward_host* entries (host buffers).
+ *     or rubix_ssp.lambda_grid (the host arrays are copied to the workspace; with lambda_obs the per-channel taps of a
+ *     wavelength-dependent PSF are also computed on the host and copied from pageable memory -- on a uniform channel grid
+ *     they are computed by a kernel and the call stays capturable); the rubix_forward_host* entries (host buffers).
  *   - Every compute call is bracketed by an NVTX range carrying its name (visible in Nsight timelines).
  *   - Device arrays are dense, row-major, fp32 / int32 as stated, 16-byte aligned.
  *   - Errors: every call validates its arguments on the host BEFORE any launch and returns a

@@ -288,6 +288,26 @@ static void var_psf_taps(const rubix_telescope *tel, int tstride, float *dst)
     }
 }
 
+// The same on the device for a uniform channel grid (no host array to read): the call stays asynchronous and can be captured
+// in a CUDA graph.  One thread per channel, fp64 like the host version (its values can differ from the host's in the last bit
+// of an fp32 tap where the two exp / pow implementations round differently).
+__global__ void __launch_bounds__(256)
+k_var_psf_taps(int n_c, int psf_size, int tstride, double lambda0, double dlambda, double sigma0, double lambda_ref, double alpha,
+               float *__restrict__ dst)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= tstride) return;
+    const int h = (psf_size - 1) / 2, shift = (15 - psf_size) / 2;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) dst[(size_t)i * tstride + k] = 0.0f;
+    if (k >= n_c) return;
+    const double lam = lambda0 + dlambda * k;
+    const double sigma = sigma0 * pow(lam / lambda_ref, alpha);
+    double w[15], sum = 0.0;
+    for (int i = -h; i <= h; ++i) { w[i + h] = exp(-((double)i * i) / (2.0 * sigma * sigma)); sum += w[i + h]; }
+    for (int i = 0; i < psf_size; ++i) dst[(size_t)(shift + i) * tstride + k] = (float)(w[i] / sum);
+}
+
 template <bool LSF, bool VAR, int MASK = 0>
 static cudaError_t march(MarchParams &P, cudaStream_t st)
 {
@@ -380,11 +400,18 @@ cudaError_t launch_convolve(const rubix_telescope *tel, const float *in, float *
         // wavelength-dependent PSF: per-channel taps go to the device once per call
         P.tstride = n_c + 2;
         P.taps = taps_dev;
-        static thread_local std::vector<float> host_taps;
-        host_taps.resize((size_t)15 * P.tstride);
-        var_psf_taps(tel, P.tstride, host_taps.data());
-        e = cudaMemcpyAsync(taps_dev, host_taps.data(), host_taps.size() * 4, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return e;
+        if (!tel->lambda_obs) {                            // uniform channel grid: taps on the device (asynchronous, capturable)
+            k_var_psf_taps<<<(unsigned)((P.tstride + 255) / 256), 256, 0, st>>>(
+                n_c, tel->psf_size, P.tstride, (double)tel->lambda0, (double)tel->dlambda, (double)tel->psf_sigma,
+                (double)tel->psf_lambda_ref, (double)tel->psf_alpha, taps_dev);
+            RUBIX_LAUNCH_CHECK();
+        } else {                                           // listed channel wavelengths are a HOST array: taps on the host
+            static thread_local std::vector<float> host_taps;
+            host_taps.resize((size_t)15 * P.tstride);
+            var_psf_taps(tel, P.tstride, host_taps.data());
+            e = cudaMemcpyAsync(taps_dev, host_taps.data(), host_taps.size() * 4, cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return e;
+        }
         if (transpose && lsf.size > 0) {                   // LSF^T PSF^T: PSF first (y, x), then the LSF
             along_y(in, out);
             if ((e = march<false, true>(P, st)) != cudaSuccess) return e;

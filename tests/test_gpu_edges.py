@@ -2,6 +2,8 @@
 view, one spaxel holding every particle (multi-chunk partial rows), multi-tile spectra, SSP grids
 whose row length is not a multiple of 4 (scalar blend path), observed grids sticking out of the
 SSP coverage (predicated resampling), non-square detectors, the host-buffer entry point."""
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -153,11 +155,15 @@ def test_gpu_error_paths(B):
         B.rubix_convolve_psf_lsf(B.c_telescope(w.telescope.with_psf_lsf()), cube, cube, dw.workspace)
 
 
-def test_calls_can_be_captured_in_a_cuda_graph(B):
+@pytest.mark.parametrize("var_psf", [False, True])
+def test_calls_can_be_captured_in_a_cuda_graph(B, var_psf):
     """The library enqueues on the caller's stream, never synchronises and never allocates, so a
-    build + PSF/LSF step is capturable and replays bit-identically (launch-bound small cubes gain)."""
+    build + PSF/LSF step is capturable and replays bit-identically (launch-bound small cubes gain).  Also with a
+    wavelength-dependent PSF on a uniform channel grid (its per-channel taps come from a kernel)."""
     w = synth.make_workload("tiny")
     w.telescope = w.telescope.with_psf_lsf()
+    if var_psf:
+        w.telescope = dataclasses.replace(w.telescope, psf_alpha=np.float32(-0.2), psf_lambda_ref=np.float32(6000.0))
     dw = B.DeviceWorkload(w)
     cube = torch.empty(dw.shape, device="cuda")
     final = torch.empty_like(cube)
