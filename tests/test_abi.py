@@ -188,6 +188,21 @@ def test_add_noise_validation(lib):
     assert f(None, None, 0, 1.0, 0.0, 1, None) == B.RUBIX_OK                          # nothing to do
 
 
+def test_residual_loss_static_validation(lib):
+    """The no-allocation loss entry refuses bad arguments, and batches beyond its static scratch, before any launch."""
+    f = lib.rubix_residual_loss_static
+    a, b, c, d = FAKE, FAKE + (1 << 30), FAKE + (2 << 30), FAKE + (3 << 30)
+    assert f(a, b, 16, B.RESIDUAL_LOSS_STATIC_MAX_BATCH + 1, c, d, None) == B.RUBIX_ERR_UNSUPPORTED
+    assert "exceeds" in B.rubix_last_error() and str(B.RESIDUAL_LOSS_STATIC_MAX_BATCH) in B.rubix_last_error()
+    assert f(a, b, 16, 0, c, d, None) == B.RUBIX_ERR_INVALID_ARG
+    assert f(a, b, -1, 1, c, d, None) == B.RUBIX_ERR_INVALID_ARG
+    assert f(a, b, 16, 1, c, None, None) == B.RUBIX_ERR_NULL
+    assert f(None, b, 16, 1, c, d, None) == B.RUBIX_ERR_NULL
+    assert f(a, b, 16, 1, None, d, None) == B.RUBIX_ERR_NULL
+    header = open(os.path.join(ROOT, "include", "rubix.h")).read()
+    assert f"#define RUBIX_RESIDUAL_LOSS_STATIC_MAX_BATCH {B.RESIDUAL_LOSS_STATIC_MAX_BATCH}" in header
+
+
 def test_no_cpu_fallback_without_the_library(monkeypatch):
     monkeypatch.setattr(B, "_lib", None)
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/librubix_b200.so")
