@@ -164,3 +164,42 @@ def test_batched_and_fused_calls_under_the_cell_order(B):
         assert torch.equal(cubes[b], B.DeviceWorkload(w1).forward()), b
     ref = oracle.forward(p, R[2], base.ssp, tel)
     assert np.abs(cubes[2].cpu().numpy() - ref).max() <= VOXEL_TOL * ref.max()
+
+
+@pytest.mark.parametrize("order", [2, 3])
+def test_mirrored_build_and_sharded_run_under_the_cell_order(B, order):
+    """rubix_build_cube_mirrored through k_accumulate_cell (its own epilogue stores the mirrors) and the split between the two
+    kernels (order 2: spaxels of >= 2 N_a N_z particles only); then the spaxel-sharded run, which fixes the order once for
+    all ranks: slabs bit-equal to the single-GPU cube of the same order."""
+    from paper_2412_08265_b200 import sharded
+    base = synth.make_workload("tiny", n=6000)
+    base.particles.pos[:2500, :2] *= np.float32(0.03)                    # a pile-up: multi-chunk spaxels above the threshold of order 2
+    base.particles.pos[2500:3200, 0] = np.float32(-7.5)                  # ... and some in the first detector row
+    w = with_order(base, order)
+    t = w.telescope
+    dw = B.DeviceWorkload(w)
+    plain = dw.build_cube()
+    ref = oracle.build_cube(w.particles, w.rotation, w.ssp, t)
+    assert np.abs(plain.cpu().numpy() - ref).max() <= VOXEL_TOL * ref.max()
+    for rows in (1, 5, t.n_x):
+        cube = torch.full(dw.shape, float("nan"), device="cuda")
+        lo = torch.full((rows, t.n_y, t.n_channels), float("nan"), device="cuda")
+        hi = torch.full((rows, t.n_y, t.n_channels), float("nan"), device="cuda")
+        B.rubix_build_cube_mirrored(dw.particles, dw.ssp, dw.tel, dw.R, cube, lo, hi, rows, dw.workspace)
+        torch.cuda.synchronize()
+        assert torch.equal(cube, plain) and torch.equal(lo, plain[:rows]) and torch.equal(hi, plain[t.n_x - rows:])
+    wc = dataclasses.replace(w, telescope=t.with_psf_lsf(psf_size=7))
+    single = B.DeviceWorkload(wc).forward()
+    backend = sharded.CudaBackend()
+    p = wc.particles
+    world = 3
+
+    def rank_fn(comm):
+        sl = sharded.slice_for_rank(p.n, comm.rank, comm.world)
+        rec = sharded.pack_records(p.subset(np.arange(p.n)[sl]), "cuda")
+        return sharded.forward_sharded(comm, backend, rec, wc.rotation, wc.ssp, wc.telescope)
+
+    slabs = sharded.run_threads(world, rank_fn)
+    torch.cuda.synchronize()
+    for s in slabs:
+        assert torch.equal(s.cube, single[s.x0:s.x1]), (s.x0, s.x1)
