@@ -24,7 +24,7 @@ constexpr int kMaxTaps = 63;
 constexpr int kAccThreads = 128;            // threads per CTA of the accumulate kernel (the 12.20 stride trick needs 128)
 constexpr int kTabMax = 4096;               // table entries addressable by the 12.20 local format
 constexpr int kSortWarps = 8;               // warps per CTA in the radix passes
-constexpr int kSortItems = 1024;            // keys per warp per radix pass
+constexpr int kSortItemsMax = 1024;         // keys per warp per radix pass: 128 .. 1024, chosen from n (Layout::sort_items)
 constexpr int kSortMaxDigitBits = 9;
 constexpr int kFluxPad = 2048;              // zero floats behind the workspace copy of the SSP grid
 constexpr int kCellAutoMean = 64;           // cell order, auto: on when the detector holds >= this many particles per spaxel ...
@@ -72,7 +72,7 @@ struct Taps {
 struct Layout {
     int64_t n;
     int32_t n_s, n_c;
-    int32_t sort_passes, digit_bits, n_wchunks;
+    int32_t sort_passes, digit_bits, n_wchunks, sort_items;   // sort_items: keys per warp chunk (multiple of 32)
     int64_t max_units, max_part_rows, max_multi;
     size_t off_key, off_vlos, off_seg, off_keybuf[2], off_permbuf[2], off_hist, off_dtot,
         off_dbase, off_unitoff, off_partoff, off_multi, off_totals, off_tiletot, off_units, off_rec,

@@ -97,12 +97,12 @@ k_rotate_bin_batched(const float *__restrict__ pos, const float *__restrict__ ve
 }
 
 // --------------------------------------------------------------------------------------------
-// K2.  Stable LSD radix sort.  Each WARP owns kSortItems consecutive keys ("warp chunk") and is
+// K2.  Stable LSD radix sort.  Each WARP owns `items` consecutive keys ("warp chunk", Layout::sort_items) and is
 // one column of the classic counting-sort histogram matrix histT[digit][warp chunk]; ranks
 // inside a 32-key round come from __match_any_sync, so equal keys keep their index order.
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kSortWarps * 32)
-k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, int n_wchunks,
+k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, int n_wchunks, int items,
             int32_t *__restrict__ histT)
 {
     __shared__ int32_t cnt[kSortWarps][1 << kSortMaxDigitBits];
@@ -111,8 +111,8 @@ k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, 
     if (wc >= n_wchunks) return;
     for (int d = lane; d <= mask; d += 32) cnt[warp][d] = 0;
     __syncwarp();
-    const int64_t base = (int64_t)wc * kSortItems;
-    for (int r = 0; r < kSortItems; r += 32) {
+    const int64_t base = (int64_t)wc * items;
+    for (int r = 0; r < items; r += 32) {
         const int64_t i = base + r + lane;
         if (i < n) atomicAdd(&cnt[warp][(key_in[i] >> shift) & mask], 1);
     }
@@ -170,7 +170,7 @@ k_sort_digitscan(const int32_t *__restrict__ digit_total, int n_digits, int32_t 
 template <bool FIRST>
 __global__ void __launch_bounds__(kSortWarps * 32)
 k_sort_scatter(const int32_t *__restrict__ key_in, const int32_t *__restrict__ perm_in, int64_t n,
-               int shift, int mask, int n_wchunks, const int32_t *__restrict__ histT,
+               int shift, int mask, int n_wchunks, int items, const int32_t *__restrict__ histT,
                const int32_t *__restrict__ digit_base, int32_t *__restrict__ key_out,
                int32_t *__restrict__ perm_out)
 {
@@ -181,9 +181,9 @@ k_sort_scatter(const int32_t *__restrict__ key_in, const int32_t *__restrict__ p
     for (int d = lane; d <= mask; d += 32)
         cur[warp][d] = digit_base[d] + histT[(int64_t)d * n_wchunks + wc];
     __syncwarp();
-    const int64_t base = (int64_t)wc * kSortItems;
+    const int64_t base = (int64_t)wc * items;
     const unsigned lt = (1u << lane) - 1u;
-    for (int r = 0; r < kSortItems; r += 32) {
+    for (int r = 0; r < items; r += 32) {
         const int64_t i = base + r + lane;
         const bool valid = i < n;
         const int32_t k = valid ? key_in[i] : 0;
@@ -699,7 +699,11 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
     const int bits = bits_for(n_s);                      // keys are 0 .. n_s  (the cell order sorts wider keys: the pass
     L.sort_passes = (bits + kSortMaxDigitBits - 1) / kSortMaxDigitBits;   // count is then fixed in launch_particle_pass)
     L.digit_bits = (bits + L.sort_passes - 1) / L.sort_passes;
-    L.n_wchunks = (int32_t)((n + kSortItems - 1) / kSortItems);
+    // keys per warp chunk: about 2048 warps per radix pass, 128 .. 1024 keys each (measured: 10^5 particles are fastest at
+    // 128, 10^6 at 512, 10^7 at 1024; the stable order does not depend on it)
+    L.sort_items = 128;
+    while (L.sort_items < kSortItemsMax && (int64_t)L.sort_items * 2048 < n) L.sort_items *= 2;
+    L.n_wchunks = (int32_t)((n + L.sort_items - 1) / L.sort_items);
     L.max_units = (int64_t)n_s + n / kChunk + 1;
     L.max_part_rows = 2 * (n / kChunk) + 2;
     L.max_multi = n / kChunk + 1;
@@ -831,7 +835,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
             const int shift = pass * digit_bits;
             const int ob = (sort_passes - 1 - pass) & 1;   // the last pass writes buffer 0 = Layout::final_buf
             int32_t *kout = kbuf[ob], *pout = pbuf[ob];
-            k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, histT);
+            k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, L.sort_items, histT);
             RUBIX_LAUNCH_CHECK();
             k_sort_rowscan<<<n_digits, 256, 0, st>>>(histT, L.n_wchunks, dtot);
             RUBIX_LAUNCH_CHECK();
@@ -839,10 +843,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
             RUBIX_LAUNCH_CHECK();
             if (pass == 0)
                 k_sort_scatter<true><<<sort_grid, kSortWarps * 32, 0, st>>>(
-                    kin, pin, n, shift, mask, L.n_wchunks, histT, dbase, kout, pout);
+                    kin, pin, n, shift, mask, L.n_wchunks, L.sort_items, histT, dbase, kout, pout);
             else
                 k_sort_scatter<false><<<sort_grid, kSortWarps * 32, 0, st>>>(
-                    kin, pin, n, shift, mask, L.n_wchunks, histT, dbase, kout, pout);
+                    kin, pin, n, shift, mask, L.n_wchunks, L.sort_items, histT, dbase, kout, pout);
             RUBIX_LAUNCH_CHECK();
             kin = kout;
             pin = pout;
