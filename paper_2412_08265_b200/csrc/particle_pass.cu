@@ -1,7 +1,8 @@
 // Particle pass: steps 1-3 of the hot path plus the per-particle records for steps 4-5.
 //   K1  k_rotate_bin        rotate, project, bin  (fp32, fixed order)
 //   K2  k_sort_*            stable LSD radix sort of (key, index)            (8(a) row 3)
-//       k_segment_offsets   seg_off[s] = lower_bound(sorted keys, s)  -- no atomics anywhere
+//       k_segment_offsets   seg_off[s] = lower_bound(sorted keys, s)  -- no atomics on data anywhere (k_sort_rowscan counts
+//                           its finished CTAs to pick the one that scans the digit totals: the result does not depend on it)
 //       k_unit_tile_totals, k_scan_units   work units (chunks of <= kChunk particles) per spaxel,
 //                           partial rows: tiled three-way exclusive scan
 //       k_build_units       unit descriptors
@@ -103,11 +104,12 @@ k_rotate_bin_batched(const float *__restrict__ pos, const float *__restrict__ ve
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kSortWarps * 32)
 k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, int n_wchunks, int items,
-            int32_t *__restrict__ histT)
+            int32_t *__restrict__ histT, int32_t *__restrict__ arrived)
 {
     __shared__ int32_t cnt[kSortWarps][1 << kSortMaxDigitBits];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = blockIdx.x * kSortWarps + warp;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *arrived = 0;  // arrival counter of k_sort_rowscan (the next kernel on the stream)
     if (wc >= n_wchunks) return;
     for (int d = lane; d <= mask; d += 32) cnt[warp][d] = 0;
     __syncwarp();
@@ -121,11 +123,16 @@ k_sort_hist(const int32_t *__restrict__ key_in, int64_t n, int shift, int mask, 
 }
 
 // one CTA per digit: exclusive scan of its row of histT, row total to digit_total
+// ... and the CTA that finishes last turns the row totals into the exclusive digit bases (one launch less per radix pass than a
+// scan kernel of its own; `arrived` was zeroed by k_sort_hist)
 __global__ void __launch_bounds__(256)
-k_sort_rowscan(int32_t *__restrict__ histT, int n_wchunks, int32_t *__restrict__ digit_total)
+k_sort_rowscan(int32_t *__restrict__ histT, int n_wchunks, int32_t *digit_total, int n_digits, int32_t *__restrict__ digit_base,
+               int32_t *arrived)
 {
     __shared__ int32_t warp_sum[8];
     __shared__ int32_t carry_s;
+    __shared__ int32_t s_last;
+    __shared__ int32_t s_scan[1 << kSortMaxDigitBits];
     int32_t *row = histT + (int64_t)blockIdx.x * n_wchunks;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) carry_s = 0;
@@ -148,23 +155,28 @@ k_sort_rowscan(int32_t *__restrict__ histT, int n_wchunks, int32_t *__restrict__
         if (threadIdx.x == 255) carry_s = carry + wpre + inc;
         __syncthreads();
     }
-    if (threadIdx.x == 0) digit_total[blockIdx.x] = carry_s;
-}
-
-__global__ void __launch_bounds__(1 << kSortMaxDigitBits)
-k_sort_digitscan(const int32_t *__restrict__ digit_total, int n_digits, int32_t *__restrict__ digit_base)
-{
-    __shared__ int32_t s[1 << kSortMaxDigitBits];
-    const int t = threadIdx.x;
-    s[t] = t < n_digits ? digit_total[t] : 0;
+    if (threadIdx.x == 0) {
+        digit_total[blockIdx.x] = carry_s;
+        __threadfence();                                    // the total is visible before the arrival is counted
+        s_last = atomicAdd(arrived, 1) == (int32_t)gridDim.x - 1;
+    }
     __syncthreads();
-    for (int o = 1; o < (1 << kSortMaxDigitBits); o <<= 1) {
-        const int32_t v = t >= o ? s[t - o] : 0;
+    if (!s_last) return;
+    __threadfence();
+    constexpr int kD = 1 << kSortMaxDigitBits;
+    const volatile int32_t *dt = digit_total;               // written by the other CTAs: read past L1
+    for (int t = threadIdx.x; t < kD; t += 256) s_scan[t] = t < n_digits ? dt[t] : 0;
+    __syncthreads();
+    for (int o = 1; o < kD; o <<= 1) {                      // inclusive scan, two entries per thread
+        int32_t v[kD / 256];
+#pragma unroll
+        for (int i = 0; i < kD / 256; ++i) { const int t = threadIdx.x + 256 * i; v[i] = t >= o ? s_scan[t - o] : 0; }
         __syncthreads();
-        s[t] += v;
+#pragma unroll
+        for (int i = 0; i < kD / 256; ++i) s_scan[threadIdx.x + 256 * i] += v[i];
         __syncthreads();
     }
-    if (t < n_digits) digit_base[t] = s[t] - digit_total[t];
+    for (int t = threadIdx.x; t < n_digits; t += 256) digit_base[t] = s_scan[t] - dt[t];
 }
 
 template <bool FIRST>
@@ -727,7 +739,7 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
         L.off_permbuf[b] = take(nn * 4);
     }
     L.off_hist = take((size_t)(1 << kSortMaxDigitBits) * (size_t)(L.n_wchunks > 0 ? L.n_wchunks : 1) * 4);
-    L.off_dtot = take((size_t)(1 << kSortMaxDigitBits) * 4);
+    L.off_dtot = take(((size_t)(1 << kSortMaxDigitBits) + 1) * 4);   // + the arrival counter of k_sort_rowscan
     L.off_dbase = take((size_t)(1 << kSortMaxDigitBits) * 4);
     L.off_unitoff = take(((size_t)n_s + 1) * 4);
     L.off_partoff = take(((size_t)n_s + 1) * 4);
@@ -768,6 +780,7 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     int32_t *histT = (int32_t *)(ws + L.off_hist);
     int32_t *dtot = (int32_t *)(ws + L.off_dtot);
     int32_t *dbase = (int32_t *)(ws + L.off_dbase);
+    int32_t *arrived = dtot + (1 << kSortMaxDigitBits);   // behind the digit totals (Layout reserves one more word)
     int32_t *unit_off = (int32_t *)(ws + L.off_unitoff);
     int32_t *part_off = (int32_t *)(ws + L.off_partoff);
     int32_t *multi = (int32_t *)(ws + L.off_multi);
@@ -835,11 +848,9 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
             const int shift = pass * digit_bits;
             const int ob = (sort_passes - 1 - pass) & 1;   // the last pass writes buffer 0 = Layout::final_buf
             int32_t *kout = kbuf[ob], *pout = pbuf[ob];
-            k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, L.sort_items, histT);
+            k_sort_hist<<<sort_grid, kSortWarps * 32, 0, st>>>(kin, n, shift, mask, L.n_wchunks, L.sort_items, histT, arrived);
             RUBIX_LAUNCH_CHECK();
-            k_sort_rowscan<<<n_digits, 256, 0, st>>>(histT, L.n_wchunks, dtot);
-            RUBIX_LAUNCH_CHECK();
-            k_sort_digitscan<<<1, 1 << kSortMaxDigitBits, 0, st>>>(dtot, n_digits, dbase);
+            k_sort_rowscan<<<n_digits, 256, 0, st>>>(histT, L.n_wchunks, dtot, n_digits, dbase, arrived);
             RUBIX_LAUNCH_CHECK();
             if (pass == 0)
                 k_sort_scatter<true><<<sort_grid, kSortWarps * 32, 0, st>>>(
@@ -863,8 +874,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
         const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
         const int compact = in.compact_units ? 1 : 0;
-        k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot);
-        RUBIX_LAUNCH_CHECK();
+        if (tiles > 1) {                                   // a single tile has nothing before it: k_scan_units reads no tile sums
+            k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot);
+            RUBIX_LAUNCH_CHECK();
+        }
         k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot, unit_off, part_off, multi, totals,
                                                      (uint8_t *)(ws + L.off_occ[0]));
         RUBIX_LAUNCH_CHECK();
