@@ -1,11 +1,10 @@
 // Particle pass: steps 1-3 of the hot path plus the per-particle records for steps 4-5.
 //   K1  k_rotate_bin        rotate, project, bin  (fp32, fixed order)
 //   K2  k_sort_*            stable LSD radix sort of (key, index)            (8(a) row 3)
-//       k_segment_offsets   seg_off[s] = lower_bound(sorted keys, s)  -- no atomics on data anywhere (k_sort_rowscan counts
-//                           its finished CTAs to pick the one that scans the digit totals: the result does not depend on it)
-//       k_unit_tile_totals, k_scan_units   work units (chunks of <= kChunk particles) per spaxel,
-//                           partial rows: tiled three-way exclusive scan
-//       k_build_units       unit descriptors
+//       k_unit_tile_totals, k_scan_units   seg_off[s] = lower_bound(sorted keys, s); work units (chunks of <= kChunk
+//                           particles) per spaxel, partial rows: tiled three-way exclusive scan; unit descriptors
+//                           -- no atomics on data anywhere (k_sort_rowscan counts its finished CTAs to pick the one that scans
+//                           the digit totals, k_scan_units numbers the slots of a shared-memory list: neither changes a result)
 //   K2c k_prepare_records   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
 #include "common.cuh"
 #include "gen_coord.cuh"
@@ -217,6 +216,12 @@ k_sort_scatter(const int32_t *__restrict__ key_in, const int32_t *__restrict__ p
 
 // seg_off[s] = first sorted position whose key is >= s   (s = 0 .. n_s+1)
 // (cell order: the sorted keys are spaxel * mult + cell, dropped particles carry n_s * mult)
+struct SegSource {
+    const int32_t *key_sorted;         // non-null: seg_off is COMPUTED here (binary search) and written; null: read
+    int64_t n;
+    int32_t mult;
+};
+
 __global__ void __launch_bounds__(256)
 k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s, int32_t mult,
                   int32_t *__restrict__ seg_off)
@@ -232,29 +237,53 @@ k_segment_offsets(const int32_t *__restrict__ key_sorted, int64_t n, int32_t n_s
     seg_off[s] = (int32_t)lo;
 }
 
-// Three exclusive scans over the spaxels, two small kernels, kScanTile spaxels per CTA:
+constexpr int64_t kFusedSegMaxN = 16384;   // up to this many particles a one-tile detector finds its segment offsets inside k_scan_units
+
+// Three exclusive scans over the spaxels, kScanTile spaxels per CTA:
 //   unit_off: max(1, chunks(s))     part_off: chunks(s) if > 1 else 0     multi index: chunks(s) > 1
-// k_unit_tile_totals writes the three sums of every tile; k_scan_units adds the sums of the tiles
-// before its own (a few hundred values at most) and scans its tile.  totals = { n_units,
+// Detectors of more than one tile: k_unit_tile_totals writes the three sums of every tile; k_scan_units adds the sums of the
+// tiles before its own (a few hundred values at most), scans its tile and writes the unit descriptors.  A single tile needs no
+// pre-pass, and with few particles k_scan_units also finds the segment offsets itself (SegSource).  totals = { n_units,
 // n_part_rows, n_multi }.
 constexpr int kScanItems = 4;
 constexpr int kScanThreads = 256;
 constexpr int kScanTile = kScanItems * kScanThreads;
 
-// compact: an empty spaxel gets no unit (else one, which zero-fills its cube row)
-__device__ __forceinline__ void unit_counts(const int32_t *__restrict__ seg_off, int32_t n_s, int s0, int compact,
-                                            int32_t (&chunks)[kScanItems], int32_t (&tot)[3])
+// compact: an empty spaxel gets no unit (else one, which zero-fills its cube row).  first[i] = seg_off[s0 + i], i <= kScanItems
+__device__ __forceinline__ void unit_counts(int32_t *__restrict__ seg_off, const SegSource &S, int32_t n_s, int s0, int compact,
+                                            int32_t (&chunks)[kScanItems], int32_t (&first)[kScanItems + 1], int32_t (&tot)[3])
 {
     tot[0] = tot[1] = tot[2] = 0;
-    int32_t prev = s0 <= n_s ? seg_off[s0] : 0;
+    if (S.key_sorted) {
+        // kScanItems + 1 binary searches in lockstep (one load of each per step: the chains overlap): first[i] = number of
+        // sorted keys below (s0 + i) mult
+        int64_t want[kScanItems + 1], pos[kScanItems + 1];
+#pragma unroll
+        for (int i = 0; i <= kScanItems; ++i) { want[i] = (int64_t)(s0 + i) * S.mult; pos[i] = 0; }
+        int64_t step = 1;
+        while (step * 2 <= S.n) step *= 2;
+        for (; step > 0 && S.n > 0; step >>= 1) {
+#pragma unroll
+            for (int i = 0; i <= kScanItems; ++i) {
+                const int64_t probe = pos[i] + step;
+                if (probe <= S.n && (int64_t)__ldg(S.key_sorted + (probe - 1)) < want[i]) pos[i] = probe;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i <= kScanItems; ++i) {
+            first[i] = (int32_t)pos[i];
+            if (s0 + i <= n_s + 1) seg_off[s0 + i] = first[i];   // (the entry shared with the next thread is written twice: same value)
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i <= kScanItems; ++i) first[i] = s0 + i <= n_s + 1 ? seg_off[s0 + i] : 0;
+    }
 #pragma unroll
     for (int i = 0; i < kScanItems; ++i) {
         const int s = s0 + i;
         chunks[i] = -1;
         if (s < n_s) {
-            const int32_t next = seg_off[s + 1];
-            chunks[i] = (next - prev + kChunk - 1) / kChunk;
-            prev = next;
+            chunks[i] = (first[i + 1] - first[i] + kChunk - 1) / kChunk;
             tot[0] += chunks[i] > 1 ? chunks[i] : ((compact && chunks[i] == 0) ? 0 : 1);
             tot[1] += chunks[i] > 1 ? chunks[i] : 0;
             tot[2] += chunks[i] > 1 ? 1 : 0;
@@ -282,23 +311,29 @@ __device__ __forceinline__ void block_sum3(int32_t (&v)[3], int32_t (*sm)[kScanT
 }
 
 __global__ void __launch_bounds__(kScanThreads)
-k_unit_tile_totals(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, int32_t *__restrict__ tile_tot)
+k_unit_tile_totals(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int compact, int32_t *__restrict__ tile_tot)
 {
     __shared__ int32_t sm[3][kScanThreads / 32];
-    int32_t chunks[kScanItems], tot[3];
-    unit_counts(seg_off, n_s, blockIdx.x * kScanTile + threadIdx.x * kScanItems, compact, chunks, tot);
+    int32_t chunks[kScanItems], first[kScanItems + 1], tot[3];
+    unit_counts(seg_off, S, n_s, blockIdx.x * kScanTile + threadIdx.x * kScanItems, compact, chunks, first, tot);
     block_sum3(tot, sm);
     if (threadIdx.x < 3) tile_tot[3 * blockIdx.x + threadIdx.x] = tot[threadIdx.x];
 }
 
+// (one descriptor per unit; a spaxel of more than kChunk particles has several: the CTA writes those together)
 __global__ void __launch_bounds__(kScanThreads)
-k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, const int32_t *__restrict__ tile_tot,
+k_scan_units(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int compact, const int32_t *__restrict__ tile_tot,
              int32_t *__restrict__ unit_off, int32_t *__restrict__ part_off,
-             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals, uint8_t *__restrict__ occ)
+             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals, uint8_t *__restrict__ occ,
+             Unit *__restrict__ units)
 {
     __shared__ int32_t sm[3][kScanThreads / 32];
     __shared__ int32_t wsum[3][kScanThreads / 32];
+    __shared__ int4 s_multi[kScanTile];                     // multi-chunk spaxels of this tile: (first, count, unit_off, part_off)
+    __shared__ int32_t s_multi_s[kScanTile];
+    __shared__ int32_t s_n_multi;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_n_multi = 0;
     // sums of the tiles before this one (and, in the last CTA, of all tiles)
     int32_t before[3] = {0, 0, 0};
     for (int t = threadIdx.x; t < (int)blockIdx.x; t += kScanThreads) {
@@ -307,8 +342,8 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, cons
     }
     block_sum3(before, sm);
     const int s0 = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-    int32_t chunks[kScanItems], tot[3], inc[3];
-    unit_counts(seg_off, n_s, s0, compact, chunks, tot);
+    int32_t chunks[kScanItems], first[kScanItems + 1], tot[3], inc[3];
+    unit_counts(seg_off, S, n_s, s0, compact, chunks, first, tot);
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         inc[q] = tot[q];
@@ -330,10 +365,20 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, cons
     for (int i = 0; i < kScanItems; ++i) {
         if (chunks[i] >= 0) {
             const int s = s0 + i;
+            const int32_t cnt = first[i + 1] - first[i];
             unit_off[s] = run[0];
             part_off[s] = run[1];
             occ[s] = chunks[i] > 0 ? 1 : 0;             // occupancy mask of the masked PSF/LSF passes
-            if (chunks[i] > 1) multi_list[run[2]] = s;
+            if (chunks[i] > 1) {
+                multi_list[run[2]] = s;
+                const int slot = atomicAdd(&s_n_multi, 1);  // (shared memory, order irrelevant: every entry is written out below)
+                s_multi[slot] = make_int4(first[i], cnt, run[0], run[1]);
+                s_multi_s[slot] = s;
+            } else if (!(compact && chunks[i] == 0)) {
+                Unit U;
+                U.start = first[i]; U.count = cnt; U.spaxel = s; U.part_row = -1;
+                units[run[0]] = U;
+            }
             run[0] += chunks[i] > 1 ? chunks[i] : ((compact && chunks[i] == 0) ? 0 : 1);
             run[1] += chunks[i] > 1 ? chunks[i] : 0;
             run[2] += chunks[i] > 1 ? 1 : 0;
@@ -346,27 +391,28 @@ k_scan_units(const int32_t *__restrict__ seg_off, int32_t n_s, int compact, cons
         totals[1] = run[1];
         totals[2] = run[2];
     }
-}
-
-__global__ void __launch_bounds__(256)
-k_build_units(const int32_t *__restrict__ seg_off, const int32_t *__restrict__ unit_off,
-              const int32_t *__restrict__ part_off, int32_t n_s, Unit *__restrict__ units)
-{
-    const int u = blockIdx.x * blockDim.x + threadIdx.x;
-    if (u >= unit_off[n_s]) return;
-    int lo = 0, hi = n_s - 1;          // largest s with unit_off[s] <= u
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (unit_off[mid] <= u) lo = mid; else hi = mid - 1;
+    __syncthreads();
+    // the units of the multi-chunk spaxels: a thread per spaxel of up to 32 chunks, then a warp per heavier spaxel
+    const int n_multi = s_n_multi;
+    auto write_units = [&](const int4 e, int32_t sp, int c0, int c_step) {
+        const int32_t n_chunks = (e.y + kChunk - 1) / kChunk;
+        for (int c = c0; c < n_chunks; c += c_step) {
+            Unit U;
+            U.start = e.x + c * kChunk;
+            U.count = min(kChunk, e.y - c * kChunk);
+            U.spaxel = sp;
+            U.part_row = e.w + c;
+            units[e.z + c] = U;
+        }
+    };
+    for (int m = threadIdx.x; m < n_multi; m += kScanThreads) {
+        const int4 e = s_multi[m];
+        if (e.y <= 32 * kChunk) write_units(e, s_multi_s[m], 0, 1);
     }
-    const int s = lo, c = u - unit_off[s];
-    const int32_t first = seg_off[s], cnt = seg_off[s + 1] - first;
-    Unit U;
-    U.spaxel = s;
-    U.start = first + c * kChunk;
-    U.count = cnt > 0 ? min(kChunk, cnt - c * kChunk) : 0;
-    U.part_row = cnt > kChunk ? part_off[s] + c : -1;
-    units[u] = U;
+    for (int m = warp; m < n_multi; m += kScanThreads / 32) {
+        const int4 e = s_multi[m];
+        if (e.y > 32 * kChunk) write_units(e, s_multi_s[m], lane, 32);
+    }
 }
 
 // --------------------------------------------------------------------------------------------
@@ -867,23 +913,25 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     const int32_t *perm = pbuf[L.final_buf];
     {
         const int32_t cells = n > 0 ? cell_order_cells(in, L) : 0;
-        k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, cells > 0 ? cells : 1, seg);
-    }
-    RUBIX_LAUNCH_CHECK();
-    {
         int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
         const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
         const int compact = in.compact_units ? 1 : 0;
-        if (tiles > 1) {                                   // a single tile has nothing before it: k_scan_units reads no tile sums
-            k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot);
+        const SegSource compute{key_sorted, n, cells > 0 ? cells : 1}, read{nullptr, 0, 1};
+        // the segment offsets: inside the unit scan where that is one CTA and the searches are short, else a kernel of their own
+        // (one search per thread; measured: five searches per thread in the 88 CTAs of the medium detector cost 40 us more)
+        const bool fused_seg = tiles == 1 && n <= kFusedSegMaxN;
+        if (!fused_seg) {
+            k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, compute.mult, seg);
             RUBIX_LAUNCH_CHECK();
         }
-        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, n_s, compact, tile_tot, unit_off, part_off, multi, totals,
-                                                     (uint8_t *)(ws + L.off_occ[0]));
+        if (tiles > 1) {                                   // a single tile has nothing before it: k_scan_units reads no tile sums
+            k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, read, n_s, compact, tile_tot);
+            RUBIX_LAUNCH_CHECK();
+        }
+        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, fused_seg ? compute : read, n_s, compact, tile_tot, unit_off, part_off,
+                                                     multi, totals, (uint8_t *)(ws + L.off_occ[0]), units);
         RUBIX_LAUNCH_CHECK();
     }
-    k_build_units<<<(unsigned)((L.max_units + 255) / 256), 256, 0, st>>>(seg, unit_off, part_off, n_s, units);
-    RUBIX_LAUNCH_CHECK();
     if (n > 0) {
         PrepParams P;
         P.ax.n_age = in.ssp->n_age;
