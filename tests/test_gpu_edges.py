@@ -91,6 +91,19 @@ def test_multi_tile_and_ragged_channel_counts(B, n_c, dl):
     run_and_check(B, w, f"n_c={n_c}")
 
 
+@pytest.mark.parametrize("n_x,n_y", [(33, 31), (32, 32), (41, 25), (64, 33)])
+@pytest.mark.parametrize("n", [3000, 16384, 16385, 40000])
+def test_unit_scan_around_the_tile_and_size_limits(B, n_x, n_y, n):
+    """1023 / 1024 / 1025 / 2112 spaxels (one scan tile holds 1024) and particle counts either side of the limit up to which
+    k_scan_units finds the segment offsets itself; a pile-up gives multi-chunk spaxels of more than 32 chunks (the warp path of
+    the unit descriptors) next to ones of two or three."""
+    w = synth.make_workload("tiny", n=n, seed=77)
+    w.particles.pos[: n // 3, :2] *= np.float32(0.02)            # > 32 chunks of 128 in the central spaxels from n = 16384 on
+    w.particles.pos[n // 3: n // 2, :2] *= np.float32(0.2)
+    w.telescope = dataclasses.replace(w.telescope, n_x=n_x, n_y=n_y, spaxel_size=np.float32(0.5), n_channels=64)
+    run_and_check(B, w, f"{n_x}x{n_y} n={n}")
+
+
 def test_row_length_not_multiple_of_four_uses_scalar_blend(B):
     w = synth.make_workload("tiny", n=600)
     w.ssp = synth.make_ssp(6, 3, 511, 3500.0, 9500.0, seed=77)
