@@ -784,7 +784,12 @@ Layout make_layout(int64_t n, int32_t n_s, int32_t n_c, int32_t n_rows, int32_t 
         L.off_keybuf[b] = take(nn * 4);
         L.off_permbuf[b] = take(nn * 4);
     }
-    L.off_hist = take((size_t)(1 << kSortMaxDigitBits) * (size_t)(L.n_wchunks > 0 ? L.n_wchunks : 1) * 4);
+    // rows reserved for the histogram matrix: n_wchunks itself DROPS where sort_items doubles, and a batched call carves the
+    // layouts of its smaller groups out of the workspace sized for the largest -- so reserve a count that never decreases with n
+    // (<= 2048 rows up to 262 144 particles, 4096 up to 4 M, then n / 1024)
+    int64_t hist_rows = L.n_wchunks > 0 ? L.n_wchunks : 1;
+    if (n > (int64_t)128 * 2048 && hist_rows < 4096) hist_rows = 4096;
+    L.off_hist = take((size_t)(1 << kSortMaxDigitBits) * (size_t)hist_rows * 4);
     L.off_dtot = take(((size_t)(1 << kSortMaxDigitBits) + 1) * 4);   // + the arrival counter of k_sort_rowscan
     L.off_dbase = take((size_t)(1 << kSortMaxDigitBits) * 4);
     L.off_unitoff = take(((size_t)n_s + 1) * 4);

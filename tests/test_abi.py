@@ -188,6 +188,22 @@ def test_add_noise_validation(lib):
     assert f(None, None, 0, 1.0, 0.0, 1, None) == B.RUBIX_OK                          # nothing to do
 
 
+def test_workspace_bytes_never_decrease_with_n(lib):
+    """A batched call carves the layouts of its smaller groups out of the workspace sized for the largest group: every
+    buffer must be monotone in n, also where the sort switches to larger warp chunks (fewer histogram rows)."""
+    ssp, tel = _structs(tel=synth.make_telescope("tiny"))
+    prev = 0
+    for n in [0, 1, 127, 128, 129, 1000, 100_000, 262_143, 262_144, 262_145, 300_000, 524_288, 524_289, 1_048_576, 1_048_577,
+              2_097_152, 2_097_153, 4_194_304, 4_194_305, 10_000_000]:
+        b = lib.rubix_workspace_bytes(n, ssp.ref(), tel.ref())
+        assert b >= prev > -1, n
+        prev = b
+    rng = np.random.default_rng(0)
+    for _ in range(300):
+        a, c = sorted(int(v) for v in rng.integers(1, 6_000_000, size=2))
+        assert lib.rubix_workspace_bytes(a, ssp.ref(), tel.ref()) <= lib.rubix_workspace_bytes(c, ssp.ref(), tel.ref()), (a, c)
+
+
 def test_residual_loss_static_validation(lib):
     """The no-allocation loss entry refuses bad arguments, and batches beyond its static scratch, before any launch."""
     f = lib.rubix_residual_loss_static

@@ -116,3 +116,21 @@ def test_variants_and_bad_arguments(B):
         run_batched(B, base.particles, np.array([0, 500, 700, 801]), 3, base.ssp, base.telescope, R)
     with pytest.raises(B.RubixError):
         run_batched(B, base.particles, None, 0, base.ssp, base.telescope, R[:0])
+
+
+def test_groups_either_side_of_a_sort_chunk_threshold(B):
+    """65 elements = two launch sequences whose particle counts (262 208 and 262 000) sit either side of the count at which the
+    radix sort doubles its warp chunks: the smaller group needs MORE histogram rows than the larger one, and both layouts are
+    carved out of one workspace sized for the larger group (the layout must be monotone in n)."""
+    base = synth.make_workload("tiny")
+    tel = base.telescope
+    sizes = [4097] * 64 + [262_000]
+    big = synth.make_particles_for("tiny", n=262_000, seed=910)
+    gals = [big.subset(np.arange(i * 4097, (i + 1) * 4097)) for i in range(63)] + \
+           [synth.make_particles_for("tiny", n=4097, seed=911), big]
+    offsets = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    R = rotations(len(sizes), 123)
+    cubes, _ = run_batched(B, concat(gals), offsets, len(sizes), base.ssp, tel, R)
+    assert torch.isfinite(cubes).all()
+    for b in (0, 17, 63, 64):
+        assert torch.equal(cubes[b], single(B, gals[b], base.ssp, tel, R[b])), b
