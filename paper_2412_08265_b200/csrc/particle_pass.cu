@@ -22,7 +22,27 @@ struct BinParams {
     int32_t n_x_full, x_first;             // geometry of the whole detector along x and the first owned row (row window)
     float s;
     int64_t n;
+    // the first pad_blocks CTAs of the launch write the padded workspace copy of the SSP grid instead (k_pad_flux's job: the
+    // two tasks are independent and both come first, so they share a launch); 0 = binning only
+    const float *pad_src;
+    float *pad_dst;
+    int64_t pad_total, pad_grid;
+    int32_t pad_blocks, pad_n_lambda, pad_pitch;
 };
+
+// rows of n_lambda samples -> rows of `pitch` floats (zero padded), then zeros up to pad_total
+__device__ __forceinline__ void pad_flux_part(const BinParams &P)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < P.pad_total; e += (int64_t)P.pad_blocks * blockDim.x) {
+        float v = 0.0f;
+        if (e < P.pad_grid) {
+            const int64_t row = e / P.pad_pitch;
+            const int32_t j = (int32_t)(e - row * P.pad_pitch);
+            if (j < P.pad_n_lambda) v = __ldg(P.pad_src + row * P.pad_n_lambda + j);
+        }
+        P.pad_dst[e] = v;
+    }
+}
 
 // key of (u, v) = detector coordinates in spaxels, or the sentinel n_x * n_y
 __device__ __forceinline__ int32_t bin_key(const BinParams &P, float u, float v, float vl)
@@ -37,7 +57,8 @@ __global__ void __launch_bounds__(256)
 k_rotate_bin(const float *__restrict__ pos, const float *__restrict__ vel, BinParams P,
              int32_t *__restrict__ key, float *__restrict__ vlos)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if ((int)blockIdx.x < P.pad_blocks) { pad_flux_part(P); return; }
+    const int64_t i = (int64_t)(blockIdx.x - P.pad_blocks) * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
     const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
     const float vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
@@ -65,7 +86,8 @@ __global__ void __launch_bounds__(256)
 k_rotate_bin_batched(const float *__restrict__ pos, const float *__restrict__ vel, BinParams P,
                      const __grid_constant__ BinBatch Bt, int32_t *__restrict__ key, float *__restrict__ vlos)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if ((int)blockIdx.x < P.pad_blocks) { pad_flux_part(P); return; }
+    const int64_t i = (int64_t)(blockIdx.x - P.pad_blocks) * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
     int b;
     int64_t ip = i;
@@ -639,6 +661,7 @@ cudaError_t launch_bin_only(int64_t n, const float *pos, const float *vel, const
     B.x_first = tel->n_x_full > 0 ? tel->x_first : 0;
     B.s = tel->spaxel_size;
     B.n = n;
+    B.pad_src = nullptr; B.pad_dst = nullptr; B.pad_total = B.pad_grid = 0; B.pad_blocks = 0; B.pad_n_lambda = B.pad_pitch = 0;
     k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, vel, B, key, vlos);
     RUBIX_LAUNCH_CHECK();
     return cudaSuccess;
@@ -839,14 +862,18 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     Unit *units = (Unit *)(ws + L.off_units);
     Rec *rec = (Rec *)(ws + L.off_rec);
 
-    if (L.n_rows > 0) {
-        const int64_t n_grid = (int64_t)L.n_rows * L.pitch, n_total = n_grid + kFluxPad;
-        k_pad_flux<<<(unsigned)((n_total + 1023) / 1024), 256, 0, st>>>(
-            in.ssp->flux, L.n_lambda, L.pitch, n_total, n_grid, (float *)(ws + L.off_flux));
+    const int64_t n_grid = (int64_t)L.n_rows * L.pitch, n_total = n_grid + kFluxPad;
+    const unsigned pad_blocks = L.n_rows > 0 ? (unsigned)((n_total + 1023) / 1024) : 0u;
+    if (pad_blocks > 0 && n == 0) {                         // no particles: the copy alone (the adjoint of an empty set reads nothing)
+        k_pad_flux<<<pad_blocks, 256, 0, st>>>(in.ssp->flux, L.n_lambda, L.pitch, n_total, n_grid, (float *)(ws + L.off_flux));
         RUBIX_LAUNCH_CHECK();
     }
     if (n > 0) {
         BinParams B;
+        B.pad_src = L.n_rows > 0 ? in.ssp->flux : nullptr;
+        B.pad_dst = (float *)(ws + L.off_flux);
+        B.pad_total = n_total; B.pad_grid = n_grid;
+        B.pad_blocks = (int32_t)pad_blocks; B.pad_n_lambda = L.n_lambda; B.pad_pitch = L.pitch;
         for (int i = 0; i < 9; ++i) B.R[i] = in.R[i];
         B.n_x = in.tel->n_x;
         B.n_y = in.tel->n_y;
@@ -861,9 +888,9 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
             for (int b = 0; b < in.batch; ++b)
                 for (int i = 0; i < 9; ++i) Bt.R[b][i] = in.R[9 * b + i];
             for (int b = 0; b <= in.batch; ++b) Bt.off[b] = in.offsets ? in.offsets[b] : 0;
-            k_rotate_bin_batched<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, Bt, key, vlos);
+            k_rotate_bin_batched<<<pad_blocks + (unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, Bt, key, vlos);
         } else {
-            k_rotate_bin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, key, vlos);
+            k_rotate_bin<<<pad_blocks + (unsigned)((n + 255) / 256), 256, 0, st>>>(in.p->pos, in.p->vel, B, key, vlos);
         }
         RUBIX_LAUNCH_CHECK();
 
