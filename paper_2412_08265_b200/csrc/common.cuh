@@ -43,7 +43,7 @@ struct __align__(16) Rec {
 };
 static_assert(sizeof(Rec) == 48, "Rec layout");
 
-// Per in-FoV particle, sorted order: what the adjoint kernel needs of the SSP cell (written by k_prepare_records).
+// Per in-FoV particle, sorted order: what the adjoint kernel needs of the SSP cell (written by prepare_records_body).
 struct __align__(16) AdjAux {
     float ta, tz;          // position inside the (log age, log Z) cell, in [0, 1]
     float inv_wa, inv_wz;  // 1 / cell width along each axis, 0 where the particle is clamped to the grid edge

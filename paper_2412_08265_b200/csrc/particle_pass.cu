@@ -5,7 +5,7 @@
 //                           particles) per spaxel, partial rows: tiled three-way exclusive scan; unit descriptors
 //                           -- no atomics on data anywhere (k_sort_rowscan counts its finished CTAs to pick the one that scans
 //                           the digit totals, k_scan_units numbers the slots of a shared-memory list: neither changes a result)
-//   K2c k_prepare_records   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
+//   K2c prepare_records_body (in k_scan_units_and_records)   SSP cell + bilinear weights x mass, fixed-point Doppler map (rows 4-5)
 #include "common.cuh"
 #include "gen_coord.cuh"
 
@@ -343,12 +343,27 @@ k_unit_tile_totals(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s
 }
 
 // (one descriptor per unit; a spaxel of more than kChunk particles has several: the CTA writes those together)
-__global__ void __launch_bounds__(kScanThreads)
-k_scan_units(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int compact, const int32_t *__restrict__ tile_tot,
-             int32_t *__restrict__ unit_off, int32_t *__restrict__ part_off,
-             int32_t *__restrict__ multi_list, int32_t *__restrict__ totals, uint8_t *__restrict__ occ,
-             Unit *__restrict__ units)
+struct ScanArgs {
+    int32_t *seg_off;
+    SegSource S;
+    int32_t n_s, compact, n_tiles;
+    const int32_t *tile_tot;
+    int32_t *unit_off, *part_off, *multi_list, *totals;
+    uint8_t *occ;
+    Unit *units;
+};
+
+__device__ __forceinline__ void scan_units_body(const ScanArgs &A, const int tile)
 {
+    int32_t *__restrict__ seg_off = A.seg_off;
+    const SegSource S = A.S;
+    const int32_t n_s = A.n_s;
+    const int compact = A.compact;
+    const int32_t *__restrict__ tile_tot = A.tile_tot;
+    int32_t *__restrict__ unit_off = A.unit_off, *__restrict__ part_off = A.part_off;
+    int32_t *__restrict__ multi_list = A.multi_list, *__restrict__ totals = A.totals;
+    uint8_t *__restrict__ occ = A.occ;
+    Unit *__restrict__ units = A.units;
     __shared__ int32_t sm[3][kScanThreads / 32];
     __shared__ int32_t wsum[3][kScanThreads / 32];
     __shared__ int4 s_multi[kScanTile];                     // multi-chunk spaxels of this tile: (first, count, unit_off, part_off)
@@ -358,12 +373,12 @@ k_scan_units(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int 
     if (threadIdx.x == 0) s_n_multi = 0;
     // sums of the tiles before this one (and, in the last CTA, of all tiles)
     int32_t before[3] = {0, 0, 0};
-    for (int t = threadIdx.x; t < (int)blockIdx.x; t += kScanThreads) {
+    for (int t = threadIdx.x; t < tile; t += kScanThreads) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) before[q] += tile_tot[3 * t + q];
     }
     block_sum3(before, sm);
-    const int s0 = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+    const int s0 = tile * kScanTile + threadIdx.x * kScanItems;
     int32_t chunks[kScanItems], first[kScanItems + 1], tot[3], inc[3];
     unit_counts(seg_off, S, n_s, s0, compact, chunks, first, tot);
 #pragma unroll
@@ -406,7 +421,7 @@ k_scan_units(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int 
             run[2] += chunks[i] > 1 ? 1 : 0;
         }
     }
-    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == kScanThreads - 1) {   // holds the grand totals
+    if (tile == A.n_tiles - 1 && threadIdx.x == kScanThreads - 1) {   // holds the grand totals
         unit_off[n_s] = run[0];
         part_off[n_s] = run[1];
         totals[0] = run[0];
@@ -435,6 +450,12 @@ k_scan_units(int32_t *__restrict__ seg_off, const SegSource S, int32_t n_s, int 
         const int4 e = s_multi[m];
         if (e.y > 32 * kChunk) write_units(e, s_multi_s[m], lane, 32);
     }
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_units(const ScanArgs A)
+{
+    scan_units_body(A, (int)blockIdx.x);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -472,14 +493,25 @@ __device__ __forceinline__ void axis_cell(const float *A, int n, float q, int *c
     *t = tt;
 }
 
-__global__ void __launch_bounds__(256)
-k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ seg_off,
-                  const float *__restrict__ vlos, const float *__restrict__ mass,
-                  const float *__restrict__ log_age, const float *__restrict__ log_z,
-                  const __grid_constant__ PrepParams P, Rec *__restrict__ rec, AdjAux *__restrict__ aux)
+struct PrepArgs {
+    const int32_t *perm, *key_sorted;
+    const float *vlos, *mass, *log_age, *log_z;
+    Rec *rec;
+    AdjAux *aux;
+    int64_t n;
+    int32_t drop_key;                           // sorted keys from here on belong to dropped particles
+};
+
+__device__ __forceinline__ void prepare_records_body(const PrepArgs &Q, const PrepParams &P, const int64_t i64)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= seg_off[P.n_s]) return;            // dropped particles sort last and get no record
+    if (i64 >= Q.n) return;
+    const int i = (int)i64;
+    if (__ldg(Q.key_sorted + i) >= Q.drop_key) return;   // dropped particles sort last and get no record
+    const int32_t *__restrict__ perm = Q.perm;
+    const float *__restrict__ vlos = Q.vlos, *__restrict__ mass = Q.mass;
+    const float *__restrict__ log_age = Q.log_age, *__restrict__ log_z = Q.log_z;
+    Rec *__restrict__ rec = Q.rec;
+    AdjAux *__restrict__ aux = Q.aux;
     const int pl = perm[i];                       // logical particle: indexes v_los
     const int p = P.n_phys > 0 ? (int)(pl % P.n_phys) : pl;   // physical particle: indexes the caller's arrays
     int ia, iz;
@@ -620,6 +652,14 @@ k_prepare_records(const int32_t *__restrict__ perm, const int32_t *__restrict__ 
     rec[i] = r;
 }
 
+// The unit scan and the records are independent (both read the sorted keys): one launch, the first n_tiles CTAs scan
+__global__ void __launch_bounds__(256)
+k_scan_units_and_records(const ScanArgs S, const PrepArgs A, const __grid_constant__ PrepParams P)
+{
+    if ((int)blockIdx.x < S.n_tiles) { scan_units_body(S, (int)blockIdx.x); return; }
+    prepare_records_body(A, P, (int64_t)(blockIdx.x - S.n_tiles) * blockDim.x + threadIdx.x);
+}
+
 // --------------------------------------------------------------------------------------------
 // Table mode (readings R15 / R16): x_k = Y[k] c + a with (c, a) per particle and
 //   log-sampled SSP grid:   Y[k] = log10(lambda_k / ((1+z) lambda0_ssp)) / dlog,   c = 1,  a = -log10(1+beta)/dlog
@@ -717,7 +757,7 @@ k_pad_flux(const float *__restrict__ flux, int32_t n_lambda, int32_t pitch, int6
 }
 
 // Cell order (spectral_cell.cu): composite sort key spaxel * cells + (i_age * n_z + i_z), so that the particles of a spaxel
-// come grouped by SSP cell.  The cell found here only ORDERS the particles (k_prepare_records finds the cell it uses with the
+// come grouped by SSP cell.  The cell found here only ORDERS the particles (prepare_records_body finds the cell it uses with the
 // same search); dropped particles keep the last key.
 struct CellKeyParams {
     AxisParams ax;
@@ -943,29 +983,10 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
     }
     const int32_t *key_sorted = kbuf[L.final_buf];
     const int32_t *perm = pbuf[L.final_buf];
-    {
-        const int32_t cells = n > 0 ? cell_order_cells(in, L) : 0;
-        int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
-        const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
-        const int compact = in.compact_units ? 1 : 0;
-        const SegSource compute{key_sorted, n, cells > 0 ? cells : 1}, read{nullptr, 0, 1};
-        // the segment offsets: inside the unit scan where that is one CTA and the searches are short, else a kernel of their own
-        // (one search per thread; measured: five searches per thread in the 88 CTAs of the medium detector cost 40 us more)
-        const bool fused_seg = tiles == 1 && n <= kFusedSegMaxN;
-        if (!fused_seg) {
-            k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, compute.mult, seg);
-            RUBIX_LAUNCH_CHECK();
-        }
-        if (tiles > 1) {                                   // a single tile has nothing before it: k_scan_units reads no tile sums
-            k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, read, n_s, compact, tile_tot);
-            RUBIX_LAUNCH_CHECK();
-        }
-        k_scan_units<<<tiles, kScanThreads, 0, st>>>(seg, fused_seg ? compute : read, n_s, compact, tile_tot, unit_off, part_off,
-                                                     multi, totals, (uint8_t *)(ws + L.off_occ[0]), units);
-        RUBIX_LAUNCH_CHECK();
-    }
-    if (n > 0) {
-        PrepParams P;
+    const int32_t cells = n > 0 ? cell_order_cells(in, L) : 0;
+    const int32_t mult = cells > 0 ? cells : 1;
+    PrepParams P;
+    if (n > 0) {                                           // what the records need, and the tables of the table / general-grid modes
         P.ax.n_age = in.ssp->n_age;
         P.ax.n_z = in.ssp->n_z;
         for (int i = 0; i < in.ssp->n_age; ++i) P.ax.age[i] = in.ssp->log_age_axis[i];
@@ -1009,8 +1030,32 @@ cudaError_t launch_particle_pass(const PassInputs &in, const Layout &L, char *ws
         P.dl_ssp = in.ssp->dlambda;
         P.l0_obs = in.tel->lambda0;
         P.dl_obs = in.tel->dlambda;
-        k_prepare_records<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
-            perm, seg, vlos, in.p->mass, in.p->log_age, in.p->log_z, P, rec, (AdjAux *)(ws + L.off_aux));
+    }
+    {
+        int32_t *tile_tot = (int32_t *)(ws + L.off_tiletot);
+        const unsigned tiles = (unsigned)(n_s / kScanTile + 1);
+        const int compact = in.compact_units ? 1 : 0;
+        const SegSource compute{key_sorted, n, mult}, read{nullptr, 0, 1};
+        // the segment offsets: inside the unit scan where that is one CTA and the searches are short, else a kernel of their own
+        // (one search per thread; measured: five searches per thread in the 88 CTAs of the medium detector cost 40 us more)
+        const bool fused_seg = tiles == 1 && n <= kFusedSegMaxN;
+        if (!fused_seg) {
+            k_segment_offsets<<<(unsigned)((n_s + 2 + 255) / 256), 256, 0, st>>>(key_sorted, n, n_s, mult, seg);
+            RUBIX_LAUNCH_CHECK();
+        }
+        if (tiles > 1) {                                   // a single tile has nothing before it: k_scan_units reads no tile sums
+            k_unit_tile_totals<<<tiles, kScanThreads, 0, st>>>(seg, read, n_s, compact, tile_tot);
+            RUBIX_LAUNCH_CHECK();
+        }
+        const ScanArgs S{seg, fused_seg ? compute : read, n_s, compact, (int32_t)tiles, tile_tot, unit_off, part_off, multi, totals,
+                         (uint8_t *)(ws + L.off_occ[0]), units};
+        if (n > 0) {                                       // the unit scan and the records share a launch
+            const PrepArgs A{perm, key_sorted, vlos, in.p->mass, in.p->log_age, in.p->log_z, rec, (AdjAux *)(ws + L.off_aux), n,
+                             n_s * mult};
+            k_scan_units_and_records<<<tiles + (unsigned)((n + 255) / 256), 256, 0, st>>>(S, A, P);
+        } else {
+            k_scan_units<<<tiles, kScanThreads, 0, st>>>(S);
+        }
         RUBIX_LAUNCH_CHECK();
     }
     return cudaSuccess;

@@ -107,7 +107,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
                 W.ka = max(k0, rc.x);
                 W.kb = min(k_end, rc.y);
                 j0 = 0; W.nw = 0;
-                if (W.ka <= W.kb) {                         // as k_prepare_records, for this tile's channels
+                if (W.ka <= W.kb) {                         // as prepare_records_body, for this tile's channels
                     const double x_top = (double)(P.n_lambda - 1);
                     const double xa = fmin(fmax(gen_coord_k<GEN - 1>(P.gen, P.gen.tab[W.ka], W.g) - 1e-6, 0.0), x_top);
                     const double xb = fmin(fmax(gen_coord_k<GEN - 1>(P.gen, P.gen.tab[W.kb + (FLUX ? 1 : 0)], W.g) + 1e-6, 0.0), x_top);
@@ -374,7 +374,7 @@ k_accumulate(const __grid_constant__ AccumParams P)
             // LOGX: x = (tile-relative table value of the channel) x c + (particle base), truncated to 2^-20
             const uint32_t x0 = LOGX ? (uint32_t)(W.base >> 8) : (uint32_t)((W.base + (int64_t)W.b * tid) >> 8);
             // LOGX: the sum of separately truncated terms can sit 1-2 units of 2^-20 BELOW the exact x_k that
-            // k_prepare_records used for k_lo.  Where the window starts at knot 0 (j0 = 0) a channel just above
+            // prepare_records_body used for k_lo.  Where the window starts at knot 0 (j0 = 0) a channel just above
             // the knot would wrap below zero: such windows take the guarded branch, which clamps at the knot.
             if (W.ka == k0 && W.kb == k_end && !(LOGX && W.j0 == 0)) {   // whole tile inside the SSP coverage
 #pragma unroll
